@@ -1,0 +1,265 @@
+"""Invariants I1-I12, brute-force differential, LRU closed form, ARC==LRU trace classes, partition
+invariance, statistical sanity (SURVEY.md §8(c) pins 1, 3-7)."""
+import numpy as np
+import pytest
+
+from helpers import check_invariants
+from oracle import oracle as O
+from oracle import oracle_bruteforce as BF
+from paper_2606_21238_b200 import workloads as W
+
+HITS = (O.HIT_T1, O.HIT_T2)
+
+
+def _bf_lists(cache):
+    L = cache.lists()
+    out = {}
+    for n in ("T1", "T2"):
+        out[n] = (np.array(L[n], np.uint64), np.array([cache.block_of[k] for k in L[n]], np.int32))
+    for n in ("B1", "B2"):
+        out[n] = (np.array(L[n], np.uint64), np.full(len(L[n]), -1, np.int32))
+    out["p"], out["next_fresh"] = L["p"], cache.next_fresh
+    return out
+
+
+def _random_key_requests(rng, c, n_req, alphabet):
+    reqs = []
+    for _ in range(n_req):
+        nb = int(rng.integers(1, min(c, 4) + 1))
+        reqs.append(rng.choice(alphabet, size=nb, replace=False).tolist())
+    return reqs
+
+
+@pytest.mark.parametrize("policy", [0, 1])
+def test_invariants_after_every_access_bruteforce(policy):
+    rng = np.random.default_rng(10 + policy)
+    for c in (1, 2, 3, 5, 8):
+        cache = BF.BruteForceCache(c, 16, policy)
+        alphabet = np.arange(2, 2 + 3 * c)
+        prev_p = 0
+        for _ in range(600):
+            if len(cache.pinned) >= c:   # a request has at most c blocks (R4)
+                cache.pinned.clear()
+            x = int(rng.choice(alphabet))
+            cls, bid, evi = cache.access(x)
+            check_invariants(_bf_lists(cache), c, policy_lru=bool(policy), pinned=cache.pinned)
+            if cls not in (O.GHOST_B1, O.GHOST_B2):
+                assert cache.p == prev_p, "I12: p moves only on ghost hits"
+            prev_p = cache.p
+            assert 0 <= bid < c
+            if evi >= 0:
+                assert evi == bid, "R8: a non-hit reuses exactly the ID its own eviction freed"
+            if rng.random() < 0.4:
+                cache.pinned.clear()   # request boundary
+
+
+@pytest.mark.parametrize("policy", [0, 1])
+def test_invariants_cpp_config1(policy):
+    tr = W.make_trace(1, seed=0)
+    cache = O.OracleCache(64, 16, policy)
+    prev_full = False
+    for tokens, offsets in tr.steps(max_steps=60):
+        # one request per oracle step so that the invariants are checked at every request boundary
+        for r in range(len(offsets) - 1):
+            out = cache.step(tokens[offsets[r]:offsets[r + 1]], [0, offsets[r + 1] - offsets[r]])
+            L = cache.lists()
+            check_invariants(L, 64, policy_lru=bool(policy))
+            full = len(L["T1"][0]) + len(L["T2"][0]) == 64
+            assert full or not prev_full, "I7: once full, stays full"
+            prev_full = full
+            nonhit = int((~np.isin(out["cls"], HITS)).sum())
+            assert len(out["alloc_ids"]) == nonhit, "I10"
+            assert int(out["prefix_len"][0]) % 16 == 0 and out["prefix_len"][0] <= 16 * out["n_access"], "I11"
+            assert ((out["evicted_id"] == -1) | (out["evicted_id"] == out["block_id"])).all(), "R8"
+    st = cache.stats()
+    assert st["accesses"] == st["hit_t1"] + st["hit_t2"] + st["ghost_b1"] + st["ghost_b2"] + st["miss"]
+    assert st["tokens_hashed"] == 16 * st["accesses"]
+    assert st["fresh_ids_used"] == 64
+    assert st["evict_t1"] + st["evict_t2"] == st["accesses"] - st["hit_t1"] - st["hit_t2"] - 64, "I10 over the run"
+
+
+@pytest.mark.parametrize("policy", [0, 1])
+def test_differential_cpp_vs_bruteforce_keys(policy):
+    """>= 10^4 random traces on c in 1..8, alphabet <= 3c, requests of 1..min(c,4) blocks; every output compared."""
+    rng = np.random.default_rng(100 + policy)
+    n_traces = 0
+    for rep in range(700):
+        for c in range(1, 9):
+            alphabet = np.arange(2, 2 + int(rng.integers(c, 3 * c + 1)))
+            bf, cpp = BF.BruteForceCache(c, 16, policy), O.OracleCache(c, 16, policy)
+            for step in range(3):
+                reqs = _random_key_requests(rng, min(c, len(alphabet)), int(rng.integers(1, 5)), alphabet)
+                a, b = bf.step_keys(reqs), cpp.step_keys(reqs)
+                for k in ("prefix_len", "blk_off", "cls", "block_id", "evicted_id", "p_after", "alloc_ids", "evict_ids"):
+                    assert list(a[k]) == b[k].tolist(), (c, k, reqs)
+            Lb, Lc = bf.lists(), cpp.lists()
+            for n in ("T1", "T2", "B1", "B2"):
+                assert Lb[n] == Lc[n][0].tolist()
+            sb, sc = bf.stats, cpp.stats()
+            for k in sb:
+                assert sb[k] == sc[k], k
+            n_traces += 1
+    assert n_traces >= 5000  # x2 policies >= 10^4
+
+
+def test_differential_tokens_prefix_trees():
+    """Same, through the hash: requests are paths in small token-block trees so chained keys are shared."""
+    rng = np.random.default_rng(7)
+    for rep in range(150):
+        c = int(rng.integers(1, 9))
+        for policy in (0, 1):
+            bf, cpp = BF.BruteForceCache(c, 16, policy), O.OracleCache(c, 16, policy)
+            reqs = W.prefix_tree_requests(rng, n_requests=12, block_size=16, branching=2, depth=3, max_blocks=min(c, 4))
+            for s in range(0, 12, 4):
+                tokens, offsets = W.pack_requests(reqs[s:s + 4])
+                a, b = bf.step(tokens.tolist(), offsets.tolist()), cpp.step(tokens, offsets)
+                for k in ("prefix_len", "blk_off", "cls", "block_id", "evicted_id", "p_after", "alloc_ids", "evict_ids"):
+                    assert list(a[k]) == b[k].tolist(), (c, policy, k)
+            assert bf.stats == {k: v for k, v in cpp.stats().items() if k in bf.stats}
+
+
+def test_lru_stack_distance_closed_form():
+    """Single-block requests: a hit iff fewer than c distinct other keys since the previous access of the
+    same key.  Computed straight from the trace, no list code."""
+    rng = np.random.default_rng(20)
+    for c in (1, 2, 3, 7, 16):
+        trace = (rng.zipf(1.3, size=1500) % (4 * c) + 2).tolist()
+        cache = O.OracleCache(c, 16, O.POLICY_LRU)
+        got = [int(cache.step_keys([[x]])["cls"][0]) for x in trace]
+        last = {}
+        for t, x in enumerate(trace):
+            if x in last:
+                distinct = len(set(trace[last[x] + 1:t]))
+                want = O.HIT_T1 if distinct < c else O.MISS
+            else:
+                want = O.MISS
+            assert got[t] == want, (c, t)
+            last[x] = t
+
+
+def _same_outputs(c, reqs_keys):
+    a, l = O.OracleCache(c, 16, O.POLICY_ARC), O.OracleCache(c, 16, O.POLICY_LRU)
+    for r in reqs_keys:
+        oa, ol = a.step_keys([r]), l.step_keys([r])
+        assert np.isin(oa["cls"], HITS).tolist() == np.isin(ol["cls"], HITS).tolist()
+        assert (oa["cls"] == 0).tolist() == (ol["cls"] == 0).tolist()      # no ghost hits on these traces
+        assert oa["block_id"].tolist() == ol["block_id"].tolist()
+        assert oa["evicted_id"].tolist() == ol["evicted_id"].tolist()
+        assert (oa["p_after"] == 0).all()
+
+
+def test_arc_equals_lru_on_pure_recency_traces():
+    rng = np.random.default_rng(30)
+    _same_outputs(8, [[int(k)] for k in range(2, 200)])                                  # (i) all keys distinct
+    ws = rng.integers(2, 10, size=400).tolist()
+    _same_outputs(8, [[k] for k in ws])                                                   # (ii) working set <= c
+    _same_outputs(3, [[k] for k in np.repeat(np.arange(2, 60), 2).tolist()])              # (iii) each key twice back-to-back
+    _same_outputs(16, [list(range(100 + 5 * i, 100 + 5 * i + 5)) for i in range(40)])     # (i) with multi-block requests
+
+
+@pytest.mark.parametrize("policy", [0, 1])
+def test_step_partition_invariance(policy):
+    """R3 / PAPER.md:129: the same request stream cut into steps of 1, 7, 64 or all at once gives identical
+    concatenated outputs."""
+    tr = W.make_trace(1, seed=3)
+    reqs = list(tr.requests(max_requests=200))
+    results = []
+    for rps in (1, 7, 64, 200):
+        cache = O.OracleCache(64, 16, policy)
+        acc = {k: [] for k in ("prefix_len", "cls", "block_id", "evicted_id", "p_after", "alloc_ids", "evict_ids")}
+        for s in range(0, len(reqs), rps):
+            tokens, offsets = W.pack_requests(reqs[s:s + rps])
+            out = cache.step(tokens, offsets)
+            for k in acc:
+                acc[k] += out[k].tolist()
+        results.append((acc, cache.stats()))
+    for acc, st in results[1:]:
+        assert acc == results[0][0]
+        for k in st:
+            if k != "steps":
+                assert st[k] == results[0][1][k]
+
+
+def test_errors_leave_state_unchanged():
+    cache = O.OracleCache(4)
+    toks = np.arange(16 * 3, dtype=np.int32)
+    assert isinstance(cache.step(toks, [0, 48]), dict)
+    before, st = cache.lists(), cache.stats()
+    big = np.arange(16 * 5, dtype=np.int32)
+    assert cache.step(big, [0, 80]) == O.ERR_REQUEST_TOO_LARGE          # nb_r > c
+    assert cache.step(np.concatenate([toks, big]), [0, 48, 128]) == O.ERR_REQUEST_TOO_LARGE   # even if an earlier request is fine
+    assert cache.step(toks, [0, 32, 16]) == O.ERR_INVALID_ARG
+    after = cache.lists()
+    for n in ("T1", "T2", "B1", "B2"):
+        assert before[n][0].tolist() == after[n][0].tolist()
+    assert cache.stats() == st
+    # exactly c blocks is allowed
+    assert isinstance(cache.step(np.arange(64, dtype=np.int32), [0, 64]), dict)
+    with pytest.raises(ValueError):
+        O.OracleCache(0)
+    with pytest.raises(ValueError):
+        O.OracleCache(4, 15)
+    with pytest.raises(ValueError):
+        O.OracleCache(4, 16, 7)
+
+
+def test_empty_and_short_requests():
+    cache = O.OracleCache(8)
+    out = cache.step(np.arange(40, dtype=np.int32), [0, 0, 15, 15, 40])    # empty, <B, empty, 25 tokens -> 1 block
+    assert out["blk_off"].tolist() == [0, 0, 0, 0, 1]
+    assert out["prefix_len"].tolist() == [0, 0, 0, 0]
+    assert out["n_access"] == 1
+    out = cache.step(np.zeros(0, np.int32), [0])
+    assert out["n_access"] == 0
+    st = cache.stats()
+    assert st["requests"] == 4 and st["steps"] == 2 and st["tokens_seen"] == 40 and st["tokens_hashed"] == 16
+
+
+def test_lru_hit_rate_matches_che_approximation():
+    """Statistical sanity: LRU block hit rate of single-block Zipf traffic vs Che's approximation (~1 point)."""
+    rng = np.random.default_rng(40)
+    n_items, c, s = 2000, 200, 0.9
+    p = W.zipf_probabilities(n_items, s)
+    trace = rng.choice(n_items, size=60000, p=p) + 2
+    cache = O.OracleCache(c, 16, O.POLICY_LRU)
+    hits = 0
+    for s0 in range(0, len(trace), 500):
+        out = cache.step_keys([[int(k)] for k in trace[s0:s0 + 500]])
+        if s0 >= 10000:
+            hits += int((out["cls"] == O.HIT_T1).sum())
+    measured = hits / (len(trace) - 10000)
+    lo, hi = 0.0, 1e7
+    for _ in range(200):   # characteristic time T: sum_i (1 - exp(-p_i T)) = c
+        mid = (lo + hi) / 2
+        if (1 - np.exp(-p * mid)).sum() < c:
+            lo = mid
+        else:
+            hi = mid
+    che = float((p * (1 - np.exp(-p * lo))).sum())
+    assert abs(measured - che) < 0.015, (measured, che)
+
+
+def test_scan_resistance_config4_shape():
+    """one-shot traffic clears T1 but T2 survives -> ARC keeps the hot set, LRU is flushed."""
+    rates = {}
+    for policy in (O.POLICY_ARC, O.POLICY_LRU):
+        rng = np.random.default_rng(50)
+        c = 256
+        cache = O.OracleCache(c, 16, policy)
+        hot = [rng.integers(0, 32000, size=16 * 8, dtype=np.int32) for _ in range(16)]   # 128 hot blocks
+        hits = acc = 0
+        for step in range(120):
+            reqs = []
+            for _ in range(8):
+                if rng.random() < 0.3:
+                    reqs.append(rng.integers(0, 32000, size=16 * 64, dtype=np.int32))      # scan (<< c, as in D4: 1,024 of 65,536)
+                else:
+                    reqs.append(hot[int(rng.integers(0, 16))])
+            tokens, offsets = W.pack_requests(reqs)
+            out = cache.step(tokens, offsets)
+            if step >= 20:
+                hot_mask = np.repeat(np.diff(out["blk_off"]) == 8, np.diff(out["blk_off"]))
+                hits += int(np.isin(out["cls"], HITS)[hot_mask].sum())
+                acc += int(hot_mask.sum())
+        rates[policy] = hits / acc
+    assert rates[O.POLICY_ARC] > rates[O.POLICY_LRU] + 0.3, rates
