@@ -1,0 +1,165 @@
+/* arc.h — C ABI of the B200-native prefix-KV-cache lookup + ARC block-replacement library.
+ *
+ * The method (PAPER.md = "Recency/Frequency Adaptive KV Caching for Large Language Model Serving",
+ * arxiv/paper_2606_21238): the KV cache is cut into fixed-size KV blocks (e.g. 16 tokens);
+ * prefixes shared between requests are reused at block level; the evictor keeps the
+ * Adaptive Replacement Cache lists T1/T2 (blocks in memory) and B1/B2 (metadata of evicted blocks,
+ * PAPER.md:47-48, :56-60), adapts the T1 target size p on ghost hits and is compared
+ * with vLLM's LRU eviction.  The exact rules (hash H1-H6, semantics R1-R12) are in
+ * DESIGN.md §3; they are restated from SURVEY.md §8(c).
+ *
+ * Everything behind this header runs in hand-written CUDA kernels for sm_100a; there is no CPU
+ * fallback.  Signatures use plain pointers and sizes only.  Every pointer argument says HOST or DEVICE.
+ *
+ * Conventions
+ *  - Every function returns ARC_OK (0) or a negative ARC_ERR_* code; nothing throws across the ABI.
+ *  - Validation happens before any work is enqueued and leaves the handle unchanged.
+ *  - A handle is not thread-safe; distinct handles are independent.  A handle is bound to the CUDA
+ *    device that was current when it was created.
+ *  - arc_step is asynchronous with respect to the host and ordered on `cuda_stream` (a cudaStream_t
+ *    passed as void*, NULL = the legacy default stream).  All steps of one handle must be enqueued on
+ *    streams that are ordered with respect to each other (normally: always the same stream).
+ */
+#ifndef ARC_B200_H
+#define ARC_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct arc_cache arc_cache; /* opaque, owned by the library */
+
+enum { ARC_POLICY_ARC = 0, ARC_POLICY_LRU = 1 };
+enum {
+  ARC_OK = 0,
+  ARC_ERR_INVALID_ARG = -1,       /* NULL pointer, capacity 0 or > 2^31-2, n_req > 2^20, offsets not monotone, bad policy */
+  ARC_ERR_UNSUPPORTED = -2,       /* block_size other than 16; capacity beyond what the node index width allows (2^28) */
+  ARC_ERR_REQUEST_TOO_LARGE = -3, /* some request has more full blocks than capacity_blocks (needed for the pin guarantee, R4) */
+  ARC_ERR_OOM = -4,               /* device or pinned-host allocation failed */
+  ARC_ERR_CUDA = -5               /* any other CUDA error; text in arc_last_error */
+};
+/* class of one block access, as decided against the live state at the moment of the access (R3, R5) */
+enum { ARC_MISS = 0, ARC_HIT_T1 = 1, ARC_HIT_T2 = 2, ARC_GHOST_B1 = 3, ARC_GHOST_B2 = 4 };
+
+/* Result of one arc_step.  The struct itself is HOST memory filled by the call; every pointer in it is
+ * DEVICE memory owned by the library.  The arrays are written by the step's kernels, i.e. they are valid
+ * in stream order after the call, and stay intact until the next arc_step / arc_reset / arc_destroy on
+ * the same handle is enqueued.  Index of logical block i of request r is blk_off[r] + i. */
+typedef struct {
+  uint64_t n_access;         /* N = total number of full blocks in the step (known on the host)            */
+  const int32_t *prefix_len; /* [n_req]    cached-prefix length in TOKENS (multiple of block_size), R9     */
+  const int64_t *blk_off;    /* [n_req+1]  exclusive scan of full blocks per request                       */
+  const uint8_t *cls;        /* [N]        ARC_MISS .. ARC_GHOST_B2                                        */
+  const int32_t *block_id;   /* [N]        physical block now holding the logical block, in [0, capacity)  */
+  const int32_t *evicted_id; /* [N]        block ID evicted by this access, or -1                          */
+  const int32_t *p_after;    /* [N]        p (target size of T1) after this access; 0 in LRU mode          */
+  const int32_t *alloc_ids;  /* [counts[0]] IDs handed to non-hit accesses, in ACCESS order (R2)           */
+  const int32_t *evict_ids;  /* [counts[1]] IDs evicted, in ACCESS order                                   */
+  const uint32_t *counts;    /* [2]        n_alloc, n_evict                                                */
+} arc_step_result;
+
+/* Result of arc_step_host: every pointer is pinned HOST memory owned by the library, filled when the
+ * call returns, valid until the next arc_step_host / arc_reset / arc_destroy on the handle. */
+typedef struct {
+  uint64_t n_access;
+  uint32_t n_alloc, n_evict;
+  const int32_t *prefix_len; /* [n_req] */
+  const int32_t *alloc_ids;  /* [n_alloc] */
+  const int32_t *evict_ids;  /* [n_evict] */
+} arc_host_result;
+
+/* Cumulative counters since create/reset plus the current list sizes (R12). */
+typedef struct {
+  uint64_t steps, requests, tokens_seen, tokens_hashed, accesses;
+  uint64_t hit_t1, hit_t2, ghost_b1, ghost_b2, miss;
+  uint64_t evict_t1, evict_t2, drop_b1, drop_b2, fresh_ids_used, prefix_hit_tokens;
+  uint64_t t1, t2, b1, b2, p, capacity_blocks;
+  uint32_t block_size;
+  int32_t policy;
+} arc_stats_t;
+
+/* Device time of the kernels of the last profiled step, in milliseconds (see arc_set_profiling). */
+typedef struct {
+  float hash_ms;     /* K1 chained block hashing                               */
+  float probe_ms;    /* K2 directory probe + reserve                            */
+  float machine_ms;  /* K3 ARC state machine (incl. its request bookkeeping)    */
+  float finalize_ms; /* K4 prefix lengths, directory cleanup                    */
+  float maint_ms;    /* directory rebuild / list compaction done before the step */
+  float total_ms;    /* first enqueue -> last kernel done                       */
+} arc_kernel_times;
+
+/* Create an empty cache of `capacity_blocks` KV blocks of `block_size` tokens (the cache
+ * size is the experiment knob).  *out receives the handle (HOST pointer to an
+ * opaque object).  Device memory for the directory is allocated here and grows when a larger step
+ * arrives (see arc_reserve). */
+int arc_create(uint64_t capacity_blocks, uint32_t block_size, int policy, arc_cache **out);
+
+/* Optional: pre-size all step-dependent device buffers for steps of up to max_req requests and
+ * max_blocks_per_step full blocks, so that no later arc_step reallocates. */
+int arc_reserve(arc_cache *h, uint32_t max_req, uint64_t max_blocks_per_step);
+
+/* One scheduler step (BASELINE.json north_star (a)-(d)): hashes every full block of every request
+ * (H1-H6), probes the device-resident directory, classifies every block access against the live
+ * state in the fixed order R2 (requests ascending; inside a request tail block first), applies the
+ * ARC (R5-R8) or LRU (R10) transitions with per-request pins (R4), and reports per-request cached
+ * prefix lengths and the allocated / evicted block IDs (R9).
+ *   d_tokens  DEVICE int32, CSR by h_offsets; any 4-byte alignment; borrowed until the step's work on
+ *             the stream is done.  Token IDs are reinterpreted as uint32, no range check (H1).
+ *   h_offsets HOST int64[n_req+1], monotone non-decreasing, h_offsets[0] >= 0; request r is
+ *             d_tokens[h_offsets[r] .. h_offsets[r+1]).  Copied before the call returns.
+ *   out       HOST struct, filled with DEVICE pointers (see arc_step_result).
+ * Errors: see the enum; on any error the handle is unchanged and nothing was enqueued. */
+int arc_step(arc_cache *h, const int32_t *d_tokens, const int64_t *h_offsets, uint32_t n_req,
+             void *cuda_stream, arc_step_result *out);
+
+/* Same step end to end from HOST memory: copies h_tokens (HOST int32, pinned or pageable) to a
+ * library-owned device buffer, runs the step, copies prefix_len, counts, alloc_ids and evict_ids back
+ * to pinned host memory and synchronises the stream before returning. */
+int arc_step_host(arc_cache *h, const int32_t *h_tokens, const int64_t *h_offsets, uint32_t n_req,
+                  void *cuda_stream, arc_host_result *out);
+
+/* Synchronises the stream of the handle's last step and copies the counters.  out: HOST. */
+int arc_stats(arc_cache *h, arc_stats_t *out);
+
+/* Back to the empty state (lists, ghosts, p, block IDs, counters); buffers are kept. */
+int arc_reset(arc_cache *h);
+
+/* Frees everything.  NULL is a no-op. */
+void arc_destroy(arc_cache *h);
+
+/* Text of the last error on this handle (HOST, handle-owned, never NULL); h == NULL returns the text
+ * of the last arc_create failure on this thread. */
+const char *arc_last_error(const arc_cache *h);
+
+/* Stateless K1: keys of every full block (H1-H6) in natural order, d_keys_out[blk_off[r] + i].
+ *   d_tokens DEVICE, h_offsets HOST (as in arc_step), d_keys_out DEVICE uint64[N] with
+ *   N = sum_r floor(len_r / block_size) (the caller computes it from the offsets). */
+int arc_hash_blocks(const int32_t *d_tokens, const int64_t *h_offsets, uint32_t n_req, uint32_t block_size,
+                    uint64_t *d_keys_out, void *cuda_stream);
+
+/* Diagnostics ------------------------------------------------------------------------------------ */
+
+/* When enabled, arc_step records CUDA events between its kernels (on the step's stream); the times of
+ * the last step are read with arc_last_kernel_times, which synchronises.  Off by default. */
+int arc_set_profiling(arc_cache *h, int enabled);
+int arc_last_kernel_times(arc_cache *h, arc_kernel_times *out);
+
+/* Number of kernels the library launched for this handle since create/reset (arc_hash_blocks launches
+ * are counted in a process-wide counter returned when h == NULL). */
+uint64_t arc_launch_count(const arc_cache *h);
+
+/* Selects the K3 implementation: 0 = batched warp-cooperative machine (default), 1 = single-thread
+ * serial walk (correctness reference on the device; same results, much slower). */
+int arc_set_machine(arc_cache *h, int which);
+
+/* Copies one list (1 = T1, 2 = T2, 3 = B1, 4 = B2) in LRU -> MRU order to HOST arrays keys_out /
+ * block_ids_out (either may be NULL), at most cap entries; *n_out receives the list length.
+ * Synchronises.  For tests. */
+int arc_debug_list(arc_cache *h, int which, uint64_t *keys_out, int32_t *block_ids_out, uint64_t cap, uint64_t *n_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ARC_B200_H */

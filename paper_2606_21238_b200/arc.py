@@ -1,0 +1,263 @@
+"""Thin Python binding of the C ABI in include/arc.h (same names, argument marshalling only).
+
+PyTorch is used for device memory and streams; every step of the path runs in the CUDA kernels of
+libarc_b200.so.  There is no CPU fallback: if the library is not built (or cannot be loaded) every entry
+point raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import build as _build
+
+POLICY_ARC, POLICY_LRU = 0, 1
+MISS, HIT_T1, HIT_T2, GHOST_B1, GHOST_B2 = 0, 1, 2, 3, 4
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_REQUEST_TOO_LARGE, ERR_OOM, ERR_CUDA = 0, -1, -2, -3, -4, -5
+
+STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", "hit_t1", "hit_t2", "ghost_b1",
+               "ghost_b2", "miss", "evict_t1", "evict_t2", "drop_b1", "drop_b2", "fresh_ids_used",
+               "prefix_hit_tokens", "t1", "t2", "b1", "b2", "p", "capacity_blocks"]
+
+# every symbol include/arc.h declares (checked by the CPU test-suite against the built library)
+EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats", "arc_reset", "arc_destroy",
+           "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
+           "arc_set_machine", "arc_debug_list"]
+
+
+class ArcError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"arc error {code}: {text}")
+        self.code = code
+
+
+class _StepResult(C.Structure):
+    _fields_ = [("n_access", C.c_uint64), ("prefix_len", C.c_void_p), ("blk_off", C.c_void_p), ("cls", C.c_void_p),
+                ("block_id", C.c_void_p), ("evicted_id", C.c_void_p), ("p_after", C.c_void_p), ("alloc_ids", C.c_void_p),
+                ("evict_ids", C.c_void_p), ("counts", C.c_void_p)]
+
+
+class _HostResult(C.Structure):
+    _fields_ = [("n_access", C.c_uint64), ("n_alloc", C.c_uint32), ("n_evict", C.c_uint32),
+                ("prefix_len", C.POINTER(C.c_int32)), ("alloc_ids", C.POINTER(C.c_int32)), ("evict_ids", C.POINTER(C.c_int32))]
+
+
+class _Stats(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in STAT_FIELDS] + [("block_size", C.c_uint32), ("policy", C.c_int32)]
+
+
+class _KernelTimes(C.Structure):
+    _fields_ = [(n, C.c_float) for n in ("hash_ms", "probe_ms", "machine_ms", "finalize_ms", "maint_ms", "total_ms")]
+
+
+_lib = None
+
+
+def load_library(path: Optional[Path] = None):
+    """dlopen libarc_b200.so (building it in-tree with nvcc if it is missing or stale)."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = Path(path) if path else _build.build()
+    if not p.exists():
+        raise RuntimeError(f"{p} is missing: the CUDA extension is not built (python -m paper_2606_21238_b200.build); "
+                           "there is no CPU fallback")
+    L = C.CDLL(str(p))
+    vp, u64, u32 = C.c_void_p, C.c_uint64, C.c_uint32
+    L.arc_create.argtypes = [u64, u32, C.c_int, C.POINTER(vp)]
+    L.arc_reserve.argtypes = [vp, u32, u64]
+    L.arc_step.argtypes = [vp, vp, vp, u32, vp, C.POINTER(_StepResult)]
+    L.arc_step_host.argtypes = [vp, vp, vp, u32, vp, C.POINTER(_HostResult)]
+    L.arc_stats.argtypes = [vp, C.POINTER(_Stats)]
+    L.arc_reset.argtypes = [vp]
+    L.arc_destroy.argtypes = [vp]
+    L.arc_destroy.restype = None
+    L.arc_last_error.argtypes = [vp]
+    L.arc_last_error.restype = C.c_char_p
+    L.arc_hash_blocks.argtypes = [vp, vp, u32, u32, vp, vp]
+    L.arc_set_profiling.argtypes = [vp, C.c_int]
+    L.arc_last_kernel_times.argtypes = [vp, C.POINTER(_KernelTimes)]
+    L.arc_launch_count.argtypes = [vp]
+    L.arc_launch_count.restype = u64
+    L.arc_set_machine.argtypes = [vp, C.c_int]
+    L.arc_debug_list.argtypes = [vp, C.c_int, vp, vp, u64, C.POINTER(u64)]
+    if path is None:
+        _lib = L
+    return L
+
+
+def _torch():
+    import torch
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2606_21238_b200.arc needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+class _DevView:
+    """Zero-copy view of library-owned device memory for torch.as_tensor."""
+
+    def __init__(self, ptr: int, n: int, typestr: str):
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr or 0, True), "version": 3, "strides": None}
+
+
+def _view(ptr, n, typestr, dtype):
+    torch = _torch()
+    if n == 0 or not ptr:
+        return torch.zeros(0, dtype=dtype, device="cuda")
+    return torch.as_tensor(_DevView(ptr, n, typestr), device="cuda")
+
+
+def _offsets(offsets) -> np.ndarray:
+    o = np.ascontiguousarray(offsets, dtype=np.int64)
+    if o.ndim != 1 or o.size < 1:
+        raise ValueError("offsets must have n_req + 1 entries")
+    return o
+
+
+def _stream_ptr(stream) -> int:
+    torch = _torch()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+class StepResult:
+    """Device-resident outputs of one arc_step (torch tensors viewing library-owned memory; valid until the
+    next step on the same cache)."""
+
+    def __init__(self, raw: _StepResult, n_req: int):
+        torch = _torch()
+        n = int(raw.n_access)
+        self.n_access = n
+        self.prefix_len = _view(raw.prefix_len, n_req, "<i4", torch.int32)
+        self.blk_off = _view(raw.blk_off, n_req + 1, "<i8", torch.int64)
+        self.cls = _view(raw.cls, n, "|u1", torch.uint8)
+        self.block_id = _view(raw.block_id, n, "<i4", torch.int32)
+        self.evicted_id = _view(raw.evicted_id, n, "<i4", torch.int32)
+        self.p_after = _view(raw.p_after, n, "<i4", torch.int32)
+        self.counts = _view(raw.counts, 2, "<i4", torch.int32)
+        self._alloc_ptr, self._evict_ptr = raw.alloc_ids, raw.evict_ids
+
+    def to_host(self) -> dict:
+        """Synchronising copy of everything to numpy (for tests)."""
+        torch = _torch()
+        counts = self.counts.cpu().numpy()
+        n_alloc, n_evict = int(counts[0]), int(counts[1])
+        return dict(n_access=self.n_access, prefix_len=self.prefix_len.cpu().numpy(), blk_off=self.blk_off.cpu().numpy(),
+                    cls=self.cls.cpu().numpy(), block_id=self.block_id.cpu().numpy(), evicted_id=self.evicted_id.cpu().numpy(),
+                    p_after=self.p_after.cpu().numpy(),
+                    alloc_ids=_view(self._alloc_ptr, n_alloc, "<i4", torch.int32).cpu().numpy(),
+                    evict_ids=_view(self._evict_ptr, n_evict, "<i4", torch.int32).cpu().numpy())
+
+
+class ArcCache:
+    """arc_create / arc_step / arc_stats / arc_destroy."""
+
+    def __init__(self, capacity_blocks: int, block_size: int = 16, policy: int = POLICY_ARC):
+        _torch().cuda.init()
+        self._L = load_library()
+        self._h = C.c_void_p()
+        rc = self._L.arc_create(capacity_blocks, block_size, policy, C.byref(self._h))
+        if rc != OK:
+            raise ArcError(rc, self._L.arc_last_error(None).decode())
+        self.capacity_blocks, self.block_size, self.policy = capacity_blocks, block_size, policy
+
+    def _check(self, rc):
+        if rc != OK:
+            raise ArcError(rc, self._L.arc_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.arc_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def reserve(self, max_req: int, max_blocks_per_step: int):
+        self._check(self._L.arc_reserve(self._h, max_req, max_blocks_per_step))
+
+    def step(self, tokens, offsets, stream=None) -> StepResult:
+        """tokens: CUDA int32 tensor (any 4-byte alignment); offsets: host int64[n_req+1]."""
+        torch = _torch()
+        if not (isinstance(tokens, torch.Tensor) and tokens.is_cuda and tokens.dtype == torch.int32 and tokens.is_contiguous()):
+            raise TypeError("tokens must be a contiguous CUDA int32 tensor")
+        o = _offsets(offsets)
+        if o[-1] > tokens.numel():
+            raise ValueError("offsets exceed the token tensor")
+        raw = _StepResult()
+        self._check(self._L.arc_step(self._h, tokens.data_ptr(), o.ctypes.data, len(o) - 1, _stream_ptr(stream), C.byref(raw)))
+        return StepResult(raw, len(o) - 1)
+
+    def step_raw(self, tokens_ptr: int, offsets: np.ndarray, stream_ptr: int) -> int:
+        """Marshalling-free variant for benchmarks: returns the error code only (results stay on the device)."""
+        raw = _StepResult()
+        return self._L.arc_step(self._h, tokens_ptr, offsets.ctypes.data, len(offsets) - 1, stream_ptr, C.byref(raw))
+
+    def step_host(self, tokens: np.ndarray, offsets, stream=None) -> dict:
+        """End to end from host memory (H2D of the tokens and D2H of the results inside the call)."""
+        t = np.ascontiguousarray(tokens, dtype=np.int32)
+        o = _offsets(offsets)
+        if o[-1] > t.size:
+            raise ValueError("offsets exceed the token array")
+        raw = _HostResult()
+        self._check(self._L.arc_step_host(self._h, t.ctypes.data, o.ctypes.data, len(o) - 1, _stream_ptr(stream), C.byref(raw)))
+        n_req = len(o) - 1
+        take = lambda p, n: np.ctypeslib.as_array(p, shape=(n,)).copy() if n else np.zeros(0, np.int32)
+        return dict(n_access=int(raw.n_access), prefix_len=take(raw.prefix_len, n_req), alloc_ids=take(raw.alloc_ids, raw.n_alloc),
+                    evict_ids=take(raw.evict_ids, raw.n_evict))
+
+    def stats(self) -> dict:
+        s = _Stats()
+        self._check(self._L.arc_stats(self._h, C.byref(s)))
+        return {n: int(getattr(s, n)) for n in STAT_FIELDS + ["block_size", "policy"]}
+
+    def reset(self):
+        self._check(self._L.arc_reset(self._h))
+
+    def set_profiling(self, enabled: bool):
+        self._check(self._L.arc_set_profiling(self._h, int(enabled)))
+
+    def last_kernel_times(self) -> dict:
+        t = _KernelTimes()
+        self._check(self._L.arc_last_kernel_times(self._h, C.byref(t)))
+        return {n: float(getattr(t, n)) for n, _ in _KernelTimes._fields_}
+
+    def launch_count(self) -> int:
+        return int(self._L.arc_launch_count(self._h))
+
+    def set_machine(self, which: int):
+        self._check(self._L.arc_set_machine(self._h, which))
+
+    def debug_lists(self) -> dict:
+        out = {}
+        for name, which in (("T1", 1), ("T2", 2), ("B1", 3), ("B2", 4)):
+            cap = 2 * self.capacity_blocks + 8
+            keys, blocks, n = np.zeros(cap, np.uint64), np.zeros(cap, np.int32), C.c_uint64()
+            self._check(self._L.arc_debug_list(self._h, which, keys.ctypes.data, blocks.ctypes.data, cap, C.byref(n)))
+            out[name] = (keys[:n.value].copy(), blocks[:n.value].copy())
+        return out
+
+
+def hash_blocks(tokens, offsets, block_size: int = 16, out=None, stream=None):
+    """arc_hash_blocks: keys of every full block in natural order, as a CUDA int64 tensor holding the uint64 bits."""
+    torch = _torch()
+    L = load_library()
+    o = _offsets(offsets)
+    n = int((np.diff(o) // block_size).sum())
+    if out is None:
+        out = torch.empty(n, dtype=torch.int64, device="cuda")
+    rc = L.arc_hash_blocks(tokens.data_ptr(), o.ctypes.data, len(o) - 1, block_size, out.data_ptr(), _stream_ptr(stream))
+    if rc != OK:
+        raise ArcError(rc, L.arc_last_error(None).decode())
+    return out
+
+
+def hash_launch_count() -> int:
+    return int(load_library().arc_launch_count(None))

@@ -1,0 +1,109 @@
+// Device-side types shared by the kernels of libarc_b200 (sm_100a).  Nothing here is shared with oracle/.
+//
+// Directory layout in HBM:
+//   Node[node_cap]      16 B records {list, pos, block, slot}; node ids are stable for the life of a key
+//   node_key[node_cap]  the 64-bit key of each node (only needed by rebuilds and debug dumps)
+//   Slot[table_slots]   open-addressing table, 16 B slots {key, node}, buckets of 8 slots = one 128 B line
+//   ring[L][ring_cap]   one lazy FIFO of node ids per list L in {T1, T2, B1, B2}: an entry at absolute
+//                       position q is *live* iff nodes[id].list == L && nodes[id].pos == q.  Every list
+//                       insertion is at the MRU end (tail++), every LRU-end removal scans from head and
+//                       skips stale entries; a hit leaves its old entry behind as stale.  Entries pushed
+//                       during the current request are exactly the pinned ones (R4), so the victim scan
+//                       simply stops at the tail position recorded when the request began.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace arc {
+
+constexpr uint32_t L_ABSENT = 0, L_T1 = 1, L_T2 = 2, L_B1 = 3, L_B2 = 4, L_FREE = 5;
+constexpr unsigned long long KEY_EMPTY = 0ull, KEY_TOMB = 1ull;  // H5 keeps real keys >= 2
+constexpr uint32_t NODE_PENDING = 0xFFFFFFFFu;   // slot claimed, node id not yet published
+constexpr uint32_t NODE_NONE = 0xFFFFFFFFu;
+constexpr uint32_t SLOT_FLAG = 0x80000000u;      // node_acc entry holds a slot index to resolve, not a node id
+constexpr uint32_t BUCKET_SLOTS = 8;             // 8 x 16 B = one 128 B line
+
+enum : int { CLS_MISS = 0, CLS_HIT_T1 = 1, CLS_HIT_T2 = 2, CLS_GHOST_B1 = 3, CLS_GHOST_B2 = 4 };
+enum : int { POLICY_ARC = 0, POLICY_LRU = 1 };
+
+struct __align__(16) Node {
+  uint32_t list;   // L_*
+  uint32_t pos;    // absolute ring position of the live entry (mod 2^32)
+  int32_t block;   // physical block id if resident, -1 otherwise
+  uint32_t slot;   // index of this key's table slot
+};
+
+struct __align__(16) Slot {
+  unsigned long long key;
+  uint32_t node;
+  uint32_t pad;
+};
+
+// indices into DevState::stat
+enum : int { ST_HIT_T1 = 0, ST_HIT_T2, ST_GHOST_B1, ST_GHOST_B2, ST_MISS, ST_EVICT_T1, ST_EVICT_T2, ST_DROP_B1,
+             ST_DROP_B2, ST_FRESH, ST_PREFIX_TOKENS, ST_ACCESSES, ST_COUNT };
+enum : uint32_t { DEV_ERR_NONE = 0, DEV_ERR_NODE_POOL = 1, DEV_ERR_NO_VICTIM = 2, DEV_ERR_RING_OVERFLOW = 3,
+                  DEV_ERR_BAD_NODE = 4 };
+
+struct DevState {
+  uint32_t head[5], tail[5];      // per list (index L_T1..L_B2); wrapping 32-bit absolute positions
+  int32_t t1, t2, b1, b2;         // live sizes
+  int32_t p;                      // target size of T1 (R6: integer)
+  int32_t next_fresh;             // R8
+  uint32_t free_top;              // number of ids on the free stack
+  uint32_t counts[2];             // n_alloc, n_evict of the current step
+  uint32_t error;                 // DEV_ERR_*
+  uint32_t tombs;                 // tombstones currently in the table
+  uint32_t pad0;
+  unsigned long long stat[ST_COUNT];
+  // scratch for ring compaction (old window of the list being compacted)
+  uint32_t cmp_head, cmp_tail;
+};
+
+// Everything a step's kernels need, passed by value.
+struct StepParams {
+  DevState* state;
+  Node* nodes;
+  unsigned long long* node_key;
+  uint32_t* free_stack;
+  Slot* table;
+  uint32_t bucket_mask;           // (table_slots / 8) - 1
+  uint32_t* ring[5];
+  uint32_t ring_mask;
+  // step inputs
+  const int32_t* tokens;
+  const int64_t* offsets;         // [n_req+1] token offsets
+  const int64_t* blk_off;         // [n_req+1]
+  uint32_t n_req;
+  uint32_t n_access;
+  // step scratch (access order: index blk_off[r] + (nb_r - 1 - i))
+  unsigned long long* keys_acc;
+  uint8_t* acc_start;             // 1 where a request's first access (its tail block) sits
+  uint32_t* node_acc;
+  uint32_t* dropped;              // node made ABSENT by access a, or NODE_NONE
+  // outputs (natural order: blk_off[r] + i)
+  int32_t* prefix_len;
+  uint8_t* cls;
+  int32_t* block_id;
+  int32_t* evicted_id;
+  int32_t* p_after;
+  int32_t* alloc_ids;
+  int32_t* evict_ids;
+  int32_t capacity;
+  int32_t policy;
+  uint32_t block_size;
+};
+
+__device__ __forceinline__ Node ld_node(const Node* p) {
+  // nodes are read-write shared between kernels of one stream only; within K3 they are re-read after
+  // other threads of the CTA wrote them, so go to L2 (ld.cg) rather than trusting L1.
+  uint4 v = __ldcg(reinterpret_cast<const uint4*>(p));
+  Node n;
+  n.list = v.x; n.pos = v.y; n.block = (int32_t)v.z; n.slot = v.w;
+  return n;
+}
+__device__ __forceinline__ void st_node(Node* p, uint32_t list, uint32_t pos, int32_t block, uint32_t slot) {
+  __stcg(reinterpret_cast<uint4*>(p), make_uint4(list, pos, (uint32_t)block, slot));
+}
+
+}  // namespace arc

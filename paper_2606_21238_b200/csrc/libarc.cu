@@ -1,0 +1,606 @@
+// libarc_b200 — host side of the C ABI declared in include/arc.h.
+// Validates, sizes buffers from the host offsets, enqueues the kernels on the caller's stream and owns
+// all device buffers.  No torch types, no CPU fallback: every step of the path runs in the kernels.
+#include <algorithm>
+#include <cstdarg>
+#include <cstddef>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/arc.h"
+#include "arc_device.cuh"
+#include "directory_kernels.cuh"
+#include "hash_kernels.cuh"
+#include "machine_batched.cuh"
+#include "machine_serial.cuh"
+
+using namespace arc;
+
+namespace {
+
+thread_local std::string g_create_error = "";
+uint64_t g_hash_launches = 0;
+
+constexpr int kStageSlots = 4;
+constexpr uint32_t kMaxReq = 1u << 20;
+constexpr uint64_t kMaxCapacity = 1ull << 28;   // node ids carry two flag bits
+
+uint32_t pow2_at_least(uint64_t x) {
+  uint64_t p = 64;
+  while (p < x) p <<= 1;
+  return (uint32_t)p;
+}
+
+template <typename T>
+cudaError_t dalloc(T** p, size_t n) {
+  *p = nullptr;
+  return cudaMalloc((void**)p, std::max<size_t>(n, 1) * sizeof(T));
+}
+template <typename T>
+void dfree(T*& p) {
+  if (p) cudaFree(p);
+  p = nullptr;
+}
+
+}  // namespace
+
+struct arc_cache {
+  int device = 0;
+  uint64_t c = 0;
+  uint32_t B = 16;
+  int policy = 0;
+  int machine = 0;            // 0 batched, 1 serial
+  // capacities
+  uint64_t n_cap = 0;         // max full blocks per step the buffers are sized for
+  uint32_t req_cap = 0;
+  uint32_t node_cap = 0, table_slots = 0, ring_cap = 0;
+  // directory
+  DevState* d_state = nullptr;
+  Node* d_nodes = nullptr;
+  unsigned long long* d_node_key = nullptr;
+  uint32_t* d_free_stack = nullptr;
+  Slot* d_table = nullptr;
+  uint32_t* d_ring[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  uint32_t* d_ring_alt[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  uint32_t* d_block_counts = nullptr;
+  // per-step buffers
+  int64_t* d_offsets = nullptr;   // [2 * (req_cap + 1)] : token offsets, then blk_off
+  unsigned long long* d_keys = nullptr;
+  uint8_t* d_acc_start = nullptr;
+  uint32_t* d_node_acc = nullptr;
+  uint32_t* d_dropped = nullptr;
+  int32_t* d_prefix_len = nullptr;
+  uint8_t* d_cls = nullptr;
+  int32_t *d_block_id = nullptr, *d_evicted_id = nullptr, *d_p_after = nullptr, *d_alloc_ids = nullptr, *d_evict_ids = nullptr;
+  void* d_machine_scratch = nullptr;
+  // host staging
+  int64_t* h_stage = nullptr;     // pinned, kStageSlots * 2 * (req_cap + 1)
+  cudaEvent_t stage_done[kStageSlots] = {};
+  int stage_next = 0;
+  // arc_step_host
+  int32_t* d_tokens_stage = nullptr;
+  uint64_t tokens_stage_cap = 0;
+  int32_t* h_result = nullptr;    // pinned: prefix_len[req_cap] | counts[2] | alloc[n_cap] | evict[n_cap]
+  // host-side conservative bounds (no device read-back on the hot path)
+  uint64_t slots_used_bound = 0;
+  uint64_t window_bound[5] = {0, 0, 0, 0, 0};
+  // host counters
+  uint64_t steps = 0, requests = 0, tokens_seen = 0, tokens_hashed = 0;
+  uint64_t launches = 0;
+  cudaStream_t last_stream = nullptr;
+  // profiling
+  bool profiling = false;
+  cudaEvent_t ev[7] = {};
+  bool ev_valid = false;
+  std::string err;
+};
+
+namespace {
+
+int fail(arc_cache* h, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  if (h) h->err = buf; else g_create_error = buf;
+  return code;
+}
+
+#define CUDA_TRY(h, expr)                                                                              \
+  do {                                                                                                 \
+    cudaError_t e_ = (expr);                                                                           \
+    if (e_ != cudaSuccess) {                                                                           \
+      int code_ = (e_ == cudaErrorMemoryAllocation) ? ARC_ERR_OOM : ARC_ERR_CUDA;                      \
+      return fail(h, code_, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    }                                                                                                  \
+  } while (0)
+
+StepParams make_params(arc_cache* h) {
+  StepParams P;
+  memset(&P, 0, sizeof(P));
+  P.state = h->d_state; P.nodes = h->d_nodes; P.node_key = h->d_node_key; P.free_stack = h->d_free_stack;
+  P.table = h->d_table; P.bucket_mask = h->table_slots / BUCKET_SLOTS - 1;
+  for (int L = 1; L <= 4; ++L) P.ring[L] = h->d_ring[L];
+  P.ring_mask = h->ring_cap - 1;
+  P.offsets = h->d_offsets; P.blk_off = h->d_offsets + (h->req_cap + 1);
+  P.keys_acc = h->d_keys; P.acc_start = h->d_acc_start; P.node_acc = h->d_node_acc; P.dropped = h->d_dropped;
+  P.prefix_len = h->d_prefix_len; P.cls = h->d_cls; P.block_id = h->d_block_id; P.evicted_id = h->d_evicted_id;
+  P.p_after = h->d_p_after; P.alloc_ids = h->d_alloc_ids; P.evict_ids = h->d_evict_ids;
+  P.capacity = (int32_t)h->c; P.policy = h->policy; P.block_size = h->B;
+  return P;
+}
+
+uint32_t grid_for(uint64_t work_items, uint32_t per_block, uint32_t max_blocks) {
+  uint64_t b = (work_items + per_block - 1) / per_block;
+  return (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(b, max_blocks));
+}
+
+int launch_rebuild(arc_cache* h, cudaStream_t s) {
+  CUDA_TRY(h, cudaMemsetAsync(h->d_table, 0, (size_t)h->table_slots * sizeof(Slot), s));   // key 0 = EMPTY
+  rebuild_table_kernel<<<grid_for(h->node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, h->d_nodes, h->d_node_key, h->node_cap,
+                                                                          h->d_table, h->table_slots / BUCKET_SLOTS - 1);
+  h->launches += 1;
+  CUDA_TRY(h, cudaGetLastError());
+  h->slots_used_bound = std::min<uint64_t>(h->slots_used_bound, 2 * h->c);
+  return ARC_OK;
+}
+
+// compacts list L from d_ring[L] (capacity src_cap) into d_ring_alt[L] (capacity dst_cap) and swaps
+int launch_compact(arc_cache* h, cudaStream_t s, int L, uint32_t src_cap, uint32_t dst_cap) {
+  const uint32_t blocks = std::max<uint32_t>(1, src_cap / CMP_THREADS);
+  ring_count_kernel<<<blocks, CMP_THREADS, 0, s>>>(h->d_state, h->d_nodes, h->d_ring[L], src_cap - 1, (uint32_t)L, h->d_block_counts);
+  ring_scatter_kernel<<<blocks, CMP_THREADS, 0, s>>>(h->d_state, h->d_nodes, h->d_ring[L], src_cap - 1, h->d_ring_alt[L],
+                                                    dst_cap - 1, (uint32_t)L, h->d_block_counts);
+  h->launches += 2;
+  CUDA_TRY(h, cudaGetLastError());
+  std::swap(h->d_ring[L], h->d_ring_alt[L]);
+  h->window_bound[L] = std::min<uint64_t>(h->window_bound[L], h->c);
+  return ARC_OK;
+}
+
+void free_step_buffers(arc_cache* h) {
+  dfree(h->d_offsets); dfree(h->d_keys); dfree(h->d_acc_start); dfree(h->d_node_acc); dfree(h->d_dropped);
+  dfree(h->d_prefix_len); dfree(h->d_cls); dfree(h->d_block_id); dfree(h->d_evicted_id); dfree(h->d_p_after);
+  dfree(h->d_alloc_ids); dfree(h->d_evict_ids);
+  if (h->h_stage) cudaFreeHost(h->h_stage);
+  h->h_stage = nullptr;
+  if (h->h_result) cudaFreeHost(h->h_result);
+  h->h_result = nullptr;
+}
+
+int alloc_step_buffers(arc_cache* h, uint32_t req_cap, uint64_t n_cap) {
+  free_step_buffers(h);
+  h->req_cap = req_cap; h->n_cap = n_cap;
+  CUDA_TRY(h, dalloc(&h->d_offsets, 2 * ((size_t)req_cap + 1)));
+  CUDA_TRY(h, dalloc(&h->d_keys, n_cap));
+  CUDA_TRY(h, dalloc(&h->d_acc_start, n_cap));
+  CUDA_TRY(h, dalloc(&h->d_node_acc, n_cap));
+  CUDA_TRY(h, dalloc(&h->d_dropped, n_cap));
+  CUDA_TRY(h, dalloc(&h->d_prefix_len, req_cap));
+  CUDA_TRY(h, dalloc(&h->d_cls, n_cap));
+  CUDA_TRY(h, dalloc(&h->d_block_id, n_cap));
+  CUDA_TRY(h, dalloc(&h->d_evicted_id, n_cap));
+  CUDA_TRY(h, dalloc(&h->d_p_after, n_cap));
+  CUDA_TRY(h, dalloc(&h->d_alloc_ids, n_cap));
+  CUDA_TRY(h, dalloc(&h->d_evict_ids, n_cap));
+  CUDA_TRY(h, cudaMallocHost((void**)&h->h_stage, (size_t)kStageSlots * 2 * ((size_t)req_cap + 1) * sizeof(int64_t)));
+  CUDA_TRY(h, cudaMallocHost((void**)&h->h_result, ((size_t)req_cap + 2 + 2 * n_cap + 1) * sizeof(int32_t)));
+  return ARC_OK;
+}
+
+// Makes every buffer large enough for steps of (n_req, N).  Directory content is preserved.
+int ensure_capacity(arc_cache* h, uint32_t n_req, uint64_t N, cudaStream_t s) {
+  if (n_req <= h->req_cap && N <= h->n_cap && h->d_state) return ARC_OK;
+  const bool first = (h->d_state == nullptr);
+  if (!first) CUDA_TRY(h, cudaDeviceSynchronize());   // results of earlier steps die here (documented)
+  const uint32_t req_cap = std::max<uint32_t>(first ? 64 : h->req_cap, pow2_at_least(n_req));
+  uint64_t n_cap = std::max<uint64_t>(first ? 4096 : h->n_cap, N);
+  if (!first && N > h->n_cap) n_cap = std::max<uint64_t>(n_cap, h->n_cap * 2);
+  int rc = alloc_step_buffers(h, req_cap, n_cap);
+  if (rc) return rc;
+
+  const uint64_t node_cap64 = 2 * h->c + n_cap + 64;
+  if (node_cap64 >= (1ull << 30)) return fail(h, ARC_ERR_UNSUPPORTED, "directory of %llu nodes exceeds the 30-bit node index", (unsigned long long)node_cap64);
+  const uint32_t node_cap = (uint32_t)node_cap64;
+  const uint32_t table_slots = pow2_at_least(2 * node_cap64);
+  const uint32_t ring_cap = pow2_at_least(2 * (h->c + n_cap));
+
+  if (first) {
+    CUDA_TRY(h, dalloc(&h->d_state, 1));
+    CUDA_TRY(h, dalloc(&h->d_nodes, node_cap));
+    CUDA_TRY(h, dalloc(&h->d_node_key, node_cap));
+    CUDA_TRY(h, dalloc(&h->d_free_stack, node_cap));
+    CUDA_TRY(h, dalloc(&h->d_table, table_slots));
+    for (int L = 1; L <= 4; ++L) {
+      CUDA_TRY(h, dalloc(&h->d_ring[L], ring_cap));
+      CUDA_TRY(h, dalloc(&h->d_ring_alt[L], ring_cap));
+    }
+    CUDA_TRY(h, dalloc(&h->d_block_counts, std::max<uint32_t>(1, ring_cap / CMP_THREADS)));
+    h->node_cap = node_cap; h->table_slots = table_slots; h->ring_cap = ring_cap;
+    CUDA_TRY(h, cudaMemsetAsync(h->d_table, 0, (size_t)table_slots * sizeof(Slot), s));
+    init_state_kernel<<<grid_for(node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, h->d_nodes, h->d_free_stack, node_cap);
+    h->launches += 1;
+    CUDA_TRY(h, cudaGetLastError());
+    h->slots_used_bound = 0;
+    for (int L = 1; L <= 4; ++L) h->window_bound[L] = 0;
+    return ARC_OK;
+  }
+
+  if (node_cap > h->node_cap) {       // grow the node pool; ids are stable
+    Node* nodes; unsigned long long* keys; uint32_t* stack;
+    CUDA_TRY(h, dalloc(&nodes, node_cap));
+    CUDA_TRY(h, dalloc(&keys, node_cap));
+    CUDA_TRY(h, dalloc(&stack, node_cap));
+    CUDA_TRY(h, cudaMemcpyAsync(nodes, h->d_nodes, (size_t)h->node_cap * sizeof(Node), cudaMemcpyDeviceToDevice, s));
+    CUDA_TRY(h, cudaMemcpyAsync(keys, h->d_node_key, (size_t)h->node_cap * sizeof(unsigned long long), cudaMemcpyDeviceToDevice, s));
+    extend_free_stack_kernel<<<grid_for(node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, nodes, h->d_free_stack, stack, h->node_cap, node_cap);
+    bump_free_top_kernel<<<1, 1, 0, s>>>(h->d_state, node_cap - h->node_cap);
+    h->launches += 2;
+    CUDA_TRY(h, cudaStreamSynchronize(s));
+    dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack);
+    h->d_nodes = nodes; h->d_node_key = keys; h->d_free_stack = stack; h->node_cap = node_cap;
+  }
+  if (table_slots > h->table_slots) {
+    dfree(h->d_table);
+    CUDA_TRY(h, dalloc(&h->d_table, table_slots));
+    h->table_slots = table_slots;
+    rc = launch_rebuild(h, s);
+    if (rc) return rc;
+  }
+  if (ring_cap > h->ring_cap) {
+    dfree(h->d_block_counts);
+    CUDA_TRY(h, dalloc(&h->d_block_counts, std::max<uint32_t>(1, ring_cap / CMP_THREADS)));
+    for (int L = 1; L <= 4; ++L) {
+      dfree(h->d_ring_alt[L]);
+      CUDA_TRY(h, dalloc(&h->d_ring_alt[L], ring_cap));
+      rc = launch_compact(h, s, L, h->ring_cap, ring_cap);   // swaps: d_ring[L] is now the big one
+      if (rc) return rc;
+      CUDA_TRY(h, cudaStreamSynchronize(s));
+      dfree(h->d_ring_alt[L]);
+      CUDA_TRY(h, dalloc(&h->d_ring_alt[L], ring_cap));
+    }
+    h->ring_cap = ring_cap;
+  }
+  return ARC_OK;
+}
+
+// Directory upkeep before a step of N accesses, decided from host-side upper bounds only.
+int maintain(arc_cache* h, uint64_t N, cudaStream_t s) {
+  if (h->slots_used_bound + N > (uint64_t)(0.70 * h->table_slots)) {
+    int rc = launch_rebuild(h, s);
+    if (rc) return rc;
+  }
+  for (int L = 1; L <= 4; ++L) {
+    if (h->window_bound[L] + N > h->ring_cap) {
+      int rc = launch_compact(h, s, L, h->ring_cap, h->ring_cap);
+      if (rc) return rc;
+    }
+  }
+  return ARC_OK;
+}
+
+int validate_offsets(arc_cache* h, const int64_t* off, uint32_t n_req, uint32_t B, uint64_t c, int64_t* blk_off_out, uint64_t* N_out) {
+  if (off[0] < 0) return fail(h, ARC_ERR_INVALID_ARG, "h_offsets[0] < 0");
+  uint64_t N = 0;
+  for (uint32_t r = 0; r < n_req; ++r) {
+    if (off[r + 1] < off[r]) return fail(h, ARC_ERR_INVALID_ARG, "h_offsets not monotone at request %u", r);
+    const uint64_t nb = (uint64_t)(off[r + 1] - off[r]) / B;
+    if (c && nb > c) return fail(h, ARC_ERR_REQUEST_TOO_LARGE, "request %u has %llu blocks > capacity %llu", r, (unsigned long long)nb, (unsigned long long)c);
+    if (blk_off_out) blk_off_out[r] = (int64_t)N;
+    N += nb;
+  }
+  if (blk_off_out) blk_off_out[n_req] = (int64_t)N;
+  if (N >= (1ull << 31)) return fail(h, ARC_ERR_INVALID_ARG, "step of %llu blocks is too large", (unsigned long long)N);
+  *N_out = N;
+  return ARC_OK;
+}
+
+void launch_hash(const int32_t* d_tokens, const int64_t* d_offsets, const int64_t* d_blk_off, uint32_t n_req, uint64_t N,
+                 unsigned long long* d_keys, uint8_t* d_acc_start, bool access_order, cudaStream_t s) {
+  (void)N;
+  const uint32_t blocks = grid_for(n_req, 8, 148 * 16);
+  if (access_order)
+    hash_warp_per_request_kernel<true><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_acc_start);
+  else
+    hash_warp_per_request_kernel<false><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, nullptr);
+}
+
+}  // namespace
+
+extern "C" {
+
+int arc_create(uint64_t capacity_blocks, uint32_t block_size, int policy, arc_cache** out) {
+  if (!out) return fail(nullptr, ARC_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  if (capacity_blocks == 0 || capacity_blocks > 0x7FFFFFFEull) return fail(nullptr, ARC_ERR_INVALID_ARG, "capacity_blocks out of range");
+  if (policy != ARC_POLICY_ARC && policy != ARC_POLICY_LRU) return fail(nullptr, ARC_ERR_INVALID_ARG, "unknown policy %d", policy);
+  if (block_size != 16) return fail(nullptr, ARC_ERR_UNSUPPORTED, "block_size %u: only 16 is built", block_size);
+  if (capacity_blocks > kMaxCapacity) return fail(nullptr, ARC_ERR_UNSUPPORTED, "capacity_blocks > 2^28");
+  arc_cache* h = new (std::nothrow) arc_cache();
+  if (!h) return fail(nullptr, ARC_ERR_OOM, "host allocation failed");
+  h->c = capacity_blocks; h->B = block_size; h->policy = policy;
+  cudaError_t e = cudaGetDevice(&h->device);
+  if (e != cudaSuccess) {
+    int rc = fail(nullptr, ARC_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    delete h;
+    return rc;
+  }
+  for (int i = 0; i < kStageSlots; ++i) cudaEventCreateWithFlags(&h->stage_done[i], cudaEventDisableTiming);
+  for (int i = 0; i < 7; ++i) cudaEventCreate(&h->ev[i]);
+  int rc = ensure_capacity(h, 64, std::max<uint64_t>(4096, std::min<uint64_t>(capacity_blocks, 1u << 20)), nullptr);
+  if (rc == ARC_OK) {
+    cudaError_t e2 = cudaStreamSynchronize(nullptr);
+    if (e2 != cudaSuccess) rc = fail(h, ARC_ERR_CUDA, "init: %s", cudaGetErrorString(e2));
+  }
+  if (rc != ARC_OK) {
+    g_create_error = h->err;
+    arc_destroy(h);
+    return rc;
+  }
+  *out = h;
+  return ARC_OK;
+}
+
+int arc_reserve(arc_cache* h, uint32_t max_req, uint64_t max_blocks_per_step) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  if (max_req > kMaxReq) return fail(h, ARC_ERR_INVALID_ARG, "max_req > 2^20");
+  return ensure_capacity(h, max_req, max_blocks_per_step, h->last_stream);
+}
+
+int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, uint32_t n_req, void* cuda_stream, arc_step_result* out) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  if (!h_offsets || !out) return fail(h, ARC_ERR_INVALID_ARG, "NULL argument");
+  if (n_req > kMaxReq) return fail(h, ARC_ERR_INVALID_ARG, "n_req > 2^20");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  // validation + block offsets on the host (a0), into a scratch vector first: no state change on error
+  static thread_local std::vector<int64_t> blk_off;
+  blk_off.resize((size_t)n_req + 1);
+  uint64_t N = 0;
+  int rc = validate_offsets(h, h_offsets, n_req, h->B, h->c, blk_off.data(), &N);
+  if (rc) return rc;
+  if (!d_tokens && h_offsets[n_req] > h_offsets[0]) return fail(h, ARC_ERR_INVALID_ARG, "d_tokens is NULL");
+
+  rc = ensure_capacity(h, n_req, N, s);
+  if (rc) return rc;
+  if (h->profiling) cudaEventRecord(h->ev[0], s);
+  rc = maintain(h, N, s);
+  if (rc) return rc;
+  if (h->profiling) cudaEventRecord(h->ev[1], s);
+
+  // host -> device boundary #1: offsets and block offsets (<= 16 MB at n_req = 2^20, usually a few KB)
+  const int slot = h->stage_next;
+  h->stage_next = (slot + 1) % kStageSlots;
+  CUDA_TRY(h, cudaEventSynchronize(h->stage_done[slot]));
+  int64_t* stage = h->h_stage + (size_t)slot * 2 * ((size_t)h->req_cap + 1);
+  memcpy(stage, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
+  memcpy(stage + (h->req_cap + 1), blk_off.data(), ((size_t)n_req + 1) * sizeof(int64_t));
+  CUDA_TRY(h, cudaMemcpyAsync(h->d_offsets, stage, 2 * ((size_t)h->req_cap + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, s));
+  CUDA_TRY(h, cudaEventRecord(h->stage_done[slot], s));
+
+  StepParams P = make_params(h);
+  P.tokens = d_tokens; P.n_req = n_req; P.n_access = (uint32_t)N;
+  if (N) {
+    launch_hash(d_tokens, P.offsets, P.blk_off, n_req, N, P.keys_acc, P.acc_start, true, s);               // K1
+    if (h->profiling) cudaEventRecord(h->ev[2], s);
+    probe_reserve_kernel<<<grid_for(N, 32, 148 * 8), 256, 0, s>>>(P);                                     // K2
+    resolve_nodes_kernel<<<grid_for(N, 256, 148 * 8), 256, 0, s>>>(P);
+    h->launches += 3;
+  } else if (h->profiling) {
+    cudaEventRecord(h->ev[2], s);
+  }
+  if (h->profiling) cudaEventRecord(h->ev[3], s);
+  if (h->machine == 1) {
+    arc_machine_serial_kernel<<<1, 32, 0, s>>>(P);                                                       // K3 (serial)
+  } else {
+    launch_machine_batched(P, s);                                                                        // K3 (batched)
+  }
+  if (h->profiling) cudaEventRecord(h->ev[4], s);
+  finalize_kernel<<<grid_for(std::max<uint64_t>(N, (uint64_t)n_req * 32), 256, 148 * 8), 256, 0, s>>>(P);  // K4
+  h->launches += 2;
+  if (h->profiling) { cudaEventRecord(h->ev[5], s); h->ev_valid = true; }
+  CUDA_TRY(h, cudaGetLastError());
+
+  h->slots_used_bound += N;
+  for (int L = 1; L <= 4; ++L) h->window_bound[L] += N;
+  h->steps += 1; h->requests += n_req;
+  h->tokens_seen += (uint64_t)(h_offsets[n_req] - h_offsets[0]);
+  h->tokens_hashed += N * h->B;
+  h->last_stream = s;
+
+  out->n_access = N;
+  out->prefix_len = h->d_prefix_len; out->blk_off = P.blk_off; out->cls = h->d_cls; out->block_id = h->d_block_id;
+  out->evicted_id = h->d_evicted_id; out->p_after = h->d_p_after; out->alloc_ids = h->d_alloc_ids;
+  out->evict_ids = h->d_evict_ids;
+  out->counts = reinterpret_cast<const uint32_t*>(reinterpret_cast<const char*>(h->d_state) + offsetof(DevState, counts));
+  return ARC_OK;
+}
+
+int arc_step_host(arc_cache* h, const int32_t* h_tokens, const int64_t* h_offsets, uint32_t n_req, void* cuda_stream, arc_host_result* out) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  if (!h_offsets || !out) return fail(h, ARC_ERR_INVALID_ARG, "NULL argument");
+  if (n_req > kMaxReq) return fail(h, ARC_ERR_INVALID_ARG, "n_req > 2^20");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  uint64_t N = 0;
+  int rc = validate_offsets(h, h_offsets, n_req, h->B, h->c, nullptr, &N);
+  if (rc) return rc;
+  const int64_t first = h_offsets[0], total = h_offsets[n_req] - first;
+  if (!h_tokens && total > 0) return fail(h, ARC_ERR_INVALID_ARG, "h_tokens is NULL");
+  if ((uint64_t)total > h->tokens_stage_cap) {
+    CUDA_TRY(h, cudaStreamSynchronize(s));
+    dfree(h->d_tokens_stage);
+    h->tokens_stage_cap = std::max<uint64_t>((uint64_t)total, h->tokens_stage_cap * 2);
+    CUDA_TRY(h, dalloc(&h->d_tokens_stage, h->tokens_stage_cap));
+  }
+  if (total) CUDA_TRY(h, cudaMemcpyAsync(h->d_tokens_stage, h_tokens + first, (size_t)total * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+  // offsets relative to the staged copy
+  static thread_local std::vector<int64_t> rel;
+  rel.resize((size_t)n_req + 1);
+  for (uint32_t r = 0; r <= n_req; ++r) rel[r] = h_offsets[r] - first;
+  arc_step_result res;
+  rc = arc_step(h, h->d_tokens_stage, rel.data(), n_req, cuda_stream, &res);
+  if (rc) return rc;
+  int32_t* hp = h->h_result;
+  int32_t* h_counts = hp + h->req_cap;
+  int32_t* h_alloc = h_counts + 2;
+  int32_t* h_evict = h_alloc + h->n_cap;
+  if (n_req) CUDA_TRY(h, cudaMemcpyAsync(hp, res.prefix_len, (size_t)n_req * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+  CUDA_TRY(h, cudaMemcpyAsync(h_counts, res.counts, 2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+  if (N) {
+    CUDA_TRY(h, cudaMemcpyAsync(h_alloc, res.alloc_ids, (size_t)N * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(h, cudaMemcpyAsync(h_evict, res.evict_ids, (size_t)N * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+  }
+  CUDA_TRY(h, cudaStreamSynchronize(s));
+  out->n_access = N;
+  out->n_alloc = (uint32_t)h_counts[0]; out->n_evict = (uint32_t)h_counts[1];
+  out->prefix_len = hp; out->alloc_ids = h_alloc; out->evict_ids = h_evict;
+  return ARC_OK;
+}
+
+int arc_stats(arc_cache* h, arc_stats_t* out) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  if (!out) return fail(h, ARC_ERR_INVALID_ARG, "out is NULL");
+  CUDA_TRY(h, cudaStreamSynchronize(h->last_stream));
+  DevState st;
+  CUDA_TRY(h, cudaMemcpy(&st, h->d_state, sizeof(st), cudaMemcpyDeviceToHost));
+  memset(out, 0, sizeof(*out));
+  out->steps = h->steps; out->requests = h->requests; out->tokens_seen = h->tokens_seen; out->tokens_hashed = h->tokens_hashed;
+  out->accesses = st.stat[ST_ACCESSES];
+  out->hit_t1 = st.stat[ST_HIT_T1]; out->hit_t2 = st.stat[ST_HIT_T2]; out->ghost_b1 = st.stat[ST_GHOST_B1];
+  out->ghost_b2 = st.stat[ST_GHOST_B2]; out->miss = st.stat[ST_MISS]; out->evict_t1 = st.stat[ST_EVICT_T1];
+  out->evict_t2 = st.stat[ST_EVICT_T2]; out->drop_b1 = st.stat[ST_DROP_B1]; out->drop_b2 = st.stat[ST_DROP_B2];
+  out->fresh_ids_used = st.stat[ST_FRESH]; out->prefix_hit_tokens = st.stat[ST_PREFIX_TOKENS];
+  out->t1 = (uint64_t)st.t1; out->t2 = (uint64_t)st.t2; out->b1 = (uint64_t)st.b1; out->b2 = (uint64_t)st.b2; out->p = (uint64_t)st.p;
+  out->capacity_blocks = h->c; out->block_size = h->B; out->policy = h->policy;
+  // we are synchronised: tighten the host-side bounds with the true values
+  h->slots_used_bound = (uint64_t)st.t1 + st.t2 + st.b1 + st.b2 + st.tombs;
+  for (int L = 1; L <= 4; ++L) h->window_bound[L] = (uint32_t)(st.tail[L] - st.head[L]);
+  if (st.error) return fail(h, ARC_ERR_CUDA, "device-side directory error %u (1 node pool, 2 no victim, 3 ring overflow, 4 bad node)", st.error);
+  return ARC_OK;
+}
+
+int arc_reset(arc_cache* h) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  cudaStream_t s = h->last_stream;
+  CUDA_TRY(h, cudaMemsetAsync(h->d_table, 0, (size_t)h->table_slots * sizeof(Slot), s));
+  init_state_kernel<<<grid_for(h->node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, h->d_nodes, h->d_free_stack, h->node_cap);
+  CUDA_TRY(h, cudaGetLastError());
+  CUDA_TRY(h, cudaStreamSynchronize(s));
+  h->slots_used_bound = 0;
+  for (int L = 1; L <= 4; ++L) h->window_bound[L] = 0;
+  h->steps = h->requests = h->tokens_seen = h->tokens_hashed = 0;
+  h->launches = 0;
+  h->ev_valid = false;
+  return ARC_OK;
+}
+
+void arc_destroy(arc_cache* h) {
+  if (!h) return;
+  cudaDeviceSynchronize();
+  free_step_buffers(h);
+  dfree(h->d_state); dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_table);
+  for (int L = 1; L <= 4; ++L) { dfree(h->d_ring[L]); dfree(h->d_ring_alt[L]); }
+  dfree(h->d_block_counts); dfree(h->d_tokens_stage); dfree(h->d_machine_scratch);
+  for (int i = 0; i < kStageSlots; ++i) if (h->stage_done[i]) cudaEventDestroy(h->stage_done[i]);
+  for (int i = 0; i < 7; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+  delete h;
+}
+
+const char* arc_last_error(const arc_cache* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int arc_hash_blocks(const int32_t* d_tokens, const int64_t* h_offsets, uint32_t n_req, uint32_t block_size, uint64_t* d_keys_out, void* cuda_stream) {
+  if (!h_offsets) return fail(nullptr, ARC_ERR_INVALID_ARG, "h_offsets is NULL");
+  if (n_req > kMaxReq) return fail(nullptr, ARC_ERR_INVALID_ARG, "n_req > 2^20");
+  if (block_size != 16) return fail(nullptr, ARC_ERR_UNSUPPORTED, "block_size %u: only 16 is built", block_size);
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  // process-wide scratch for the offsets (grow-only); calls are serialised by the mutex and each call
+  // waits for the previous one's copy before reusing the pinned staging area
+  static std::mutex mu;
+  static int64_t* d_off = nullptr;
+  static int64_t* h_off = nullptr;
+  static uint32_t cap = 0;
+  static cudaEvent_t copied = nullptr;
+  std::lock_guard<std::mutex> lock(mu);
+  if (n_req + 1 > cap) {
+    cudaDeviceSynchronize();
+    if (d_off) cudaFree(d_off);
+    if (h_off) cudaFreeHost(h_off);
+    cap = pow2_at_least((uint64_t)n_req + 1);
+    if (cudaMalloc((void**)&d_off, 2 * (size_t)cap * sizeof(int64_t)) != cudaSuccess ||
+        cudaMallocHost((void**)&h_off, 2 * (size_t)cap * sizeof(int64_t)) != cudaSuccess) {
+      cap = 0; d_off = nullptr; h_off = nullptr;
+      return fail(nullptr, ARC_ERR_OOM, "scratch allocation failed");
+    }
+  }
+  if (!copied) cudaEventCreateWithFlags(&copied, cudaEventDisableTiming);
+  cudaEventSynchronize(copied);
+  uint64_t N = 0;
+  int rc = validate_offsets(nullptr, h_offsets, n_req, block_size, 0, h_off + cap, &N);
+  if (rc) return rc;
+  if (N && (!d_tokens || !d_keys_out)) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
+  memcpy(h_off, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
+  cudaError_t e = cudaMemcpyAsync(d_off, h_off, 2 * (size_t)cap * sizeof(int64_t), cudaMemcpyHostToDevice, s);
+  if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "offset copy: %s", cudaGetErrorString(e));
+  cudaEventRecord(copied, s);
+  if (N) {
+    launch_hash(d_tokens, d_off, d_off + cap, n_req, N, (unsigned long long*)d_keys_out, nullptr, false, s);
+    g_hash_launches += 1;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "hash launch: %s", cudaGetErrorString(e));
+  }
+  return ARC_OK;
+}
+
+int arc_set_profiling(arc_cache* h, int enabled) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  h->profiling = enabled != 0;
+  h->ev_valid = false;
+  return ARC_OK;
+}
+
+int arc_last_kernel_times(arc_cache* h, arc_kernel_times* out) {
+  if (!h || !out) return ARC_ERR_INVALID_ARG;
+  if (!h->ev_valid) return fail(h, ARC_ERR_INVALID_ARG, "no profiled step");
+  CUDA_TRY(h, cudaEventSynchronize(h->ev[5]));
+  cudaEventElapsedTime(&out->maint_ms, h->ev[0], h->ev[1]);
+  cudaEventElapsedTime(&out->hash_ms, h->ev[1], h->ev[2]);
+  cudaEventElapsedTime(&out->probe_ms, h->ev[2], h->ev[3]);
+  cudaEventElapsedTime(&out->machine_ms, h->ev[3], h->ev[4]);
+  cudaEventElapsedTime(&out->finalize_ms, h->ev[4], h->ev[5]);
+  cudaEventElapsedTime(&out->total_ms, h->ev[0], h->ev[5]);
+  return ARC_OK;
+}
+
+uint64_t arc_launch_count(const arc_cache* h) { return h ? h->launches : g_hash_launches; }
+
+int arc_set_machine(arc_cache* h, int which) {
+  if (!h || (which != 0 && which != 1)) return ARC_ERR_INVALID_ARG;
+  h->machine = which;
+  return ARC_OK;
+}
+
+int arc_debug_list(arc_cache* h, int which, uint64_t* keys_out, int32_t* block_ids_out, uint64_t cap, uint64_t* n_out) {
+  if (!h || which < 1 || which > 4 || !n_out) return ARC_ERR_INVALID_ARG;
+  cudaStream_t s = h->last_stream;
+  unsigned long long* d_keys = nullptr; int32_t* d_blocks = nullptr; unsigned long long* d_n = nullptr;
+  CUDA_TRY(h, dalloc(&d_keys, cap));
+  CUDA_TRY(h, dalloc(&d_blocks, cap));
+  CUDA_TRY(h, dalloc(&d_n, 1));
+  dump_list_kernel<<<1, CMP_THREADS, 0, s>>>(h->d_state, h->d_nodes, h->d_node_key, h->d_ring[which], h->ring_cap - 1, (uint32_t)which,
+                                             d_keys, d_blocks, cap, d_n);
+  CUDA_TRY(h, cudaStreamSynchronize(s));
+  unsigned long long n = 0;
+  CUDA_TRY(h, cudaMemcpy(&n, d_n, sizeof(n), cudaMemcpyDeviceToHost));
+  const uint64_t m = std::min<uint64_t>(n, cap);
+  if (keys_out && m) CUDA_TRY(h, cudaMemcpy(keys_out, d_keys, m * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  if (block_ids_out && m) CUDA_TRY(h, cudaMemcpy(block_ids_out, d_blocks, m * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  cudaFree(d_keys); cudaFree(d_blocks); cudaFree(d_n);
+  *n_out = n;
+  return ARC_OK;
+}
+
+}  // extern "C"

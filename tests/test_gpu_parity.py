@@ -1,0 +1,225 @@
+"""Parity of the CUDA path against the CPU oracle, bit-exact, through the C ABI (-m gpu)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import oracle as O
+from paper_2606_21238_b200 import workloads as W
+
+OUT_KEYS = ("prefix_len", "blk_off", "cls", "block_id", "evicted_id", "p_after", "alloc_ids", "evict_ids")
+STAT_KEYS = ("steps", "requests", "tokens_seen", "tokens_hashed", "accesses", "hit_t1", "hit_t2", "ghost_b1", "ghost_b2",
+             "miss", "evict_t1", "evict_t2", "drop_b1", "drop_b2", "fresh_ids_used", "prefix_hit_tokens", "t1", "t2",
+             "b1", "b2", "p", "capacity_blocks", "block_size", "policy")
+
+
+@pytest.fixture(scope="module")
+def arc():
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device")
+    from paper_2606_21238_b200 import arc as A
+    A.load_library()   # fails loudly if the extension is missing
+    return A
+
+
+def dev(tokens):
+    return torch.from_numpy(np.ascontiguousarray(tokens, dtype=np.int32)).cuda()
+
+
+def assert_same_step(g, o, ctx=""):
+    assert g["n_access"] == o["n_access"], ctx
+    for k in OUT_KEYS:
+        assert np.array_equal(g[k], o[k]), f"{ctx}: {k} differs at {np.flatnonzero(np.asarray(g[k]) != np.asarray(o[k]))[:8] if len(g[k]) == len(o[k]) else (len(g[k]), len(o[k]))}"
+
+
+def assert_same_state(gc, oc, ctx=""):
+    gs, os_ = gc.stats(), oc.stats()
+    for k in STAT_KEYS:
+        assert gs[k] == os_[k], f"{ctx}: stat {k}: gpu {gs[k]} oracle {os_[k]}"
+    gl, ol = gc.debug_lists(), oc.lists()
+    for n in ("T1", "T2", "B1", "B2"):
+        assert np.array_equal(gl[n][0], ol[n][0]), f"{ctx}: list {n} keys differ"
+        assert np.array_equal(gl[n][1], ol[n][1]), f"{ctx}: list {n} block ids differ"
+
+
+def run_trace(arc, steps, c, policy, machine, check_every=1, ctx=""):
+    gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
+    gc.set_machine(machine)
+    for i, (tokens, offsets) in enumerate(steps):
+        g = gc.step(dev(tokens), offsets)
+        o = oc.step(tokens, offsets)
+        if i % check_every == 0:
+            assert_same_step(g.to_host(), o, f"{ctx} step {i}")
+    assert_same_state(gc, oc, ctx)
+    gc.close()
+    return oc.stats()
+
+
+# ------------------------------------------------------------------------------------------- K1
+
+def test_hash_parity_edge_requests(arc):
+    rng = np.random.default_rng(0)
+    lens = [0, 1, 15, 16, 17, 31, 32, 33, 47, 16 * 31, 16 * 32, 16 * 33 + 5, 16 * 2048, 16 * 2049 + 15, 0, 100]
+    reqs = [rng.integers(-3, 128000, size=n).astype(np.int32) for n in lens]
+    tokens, offsets = W.pack_requests(reqs)
+    want, _ = O.hash_blocks(tokens, offsets)
+    got = arc.hash_blocks(dev(tokens), offsets).cpu().numpy().view(np.uint64)
+    assert np.array_equal(got, want)
+
+
+@pytest.mark.parametrize("shift", [0, 1, 2, 3])
+def test_hash_parity_misaligned_base(arc, shift):
+    rng = np.random.default_rng(1)
+    reqs = [rng.integers(0, 32000, size=int(n)).astype(np.int32) for n in rng.integers(1, 700, size=50)]
+    tokens, offsets = W.pack_requests(reqs)
+    want, _ = O.hash_blocks(tokens, offsets)
+    buf = torch.zeros(len(tokens) + 8, dtype=torch.int32, device="cuda")
+    buf[shift:shift + len(tokens)] = dev(tokens)
+    got = arc.hash_blocks(buf[shift:], offsets).cpu().numpy().view(np.uint64)   # base pointer 4*shift bytes off 16-B alignment
+    assert np.array_equal(got, want)
+
+
+@pytest.mark.parametrize("config", [1, 2, 3])
+def test_hash_parity_configs(arc, config):
+    tr = W.make_trace(config, seed=0, scale=0.02 if config > 1 else 1.0)
+    for i, (tokens, offsets) in enumerate(tr.steps(max_steps=6)):
+        want, _ = O.hash_blocks(tokens, offsets)
+        got = arc.hash_blocks(dev(tokens), offsets).cpu().numpy().view(np.uint64)
+        assert np.array_equal(got, want), (config, i)
+
+
+# ------------------------------------------------------------------------------- whole arc_step
+
+@pytest.mark.parametrize("machine", [0, 1])
+@pytest.mark.parametrize("policy", [0, 1])
+def test_config1_full_trace(arc, policy, machine):
+    """BASELINE.json configs[0]: c = 64, 2,000 requests, 8 per step, ARC and LRU, every output of every step."""
+    tr = W.make_trace(1, seed=0)
+    st = run_trace(arc, tr.steps(), 64, policy, machine, ctx=f"config1 policy {policy} machine {machine}")
+    assert st["requests"] == 2000
+
+
+@pytest.mark.parametrize("machine", [0, 1])
+@pytest.mark.parametrize("config,scale,max_steps", [(2, 0.06, 40), (3, 0.03, 40), (4, 0.004, 8)])
+def test_larger_configs_scaled(arc, config, scale, max_steps, machine):
+    tr = W.make_trace(config, seed=0, scale=scale)
+    if machine == 1 and config == 4:
+        max_steps = 3
+    run_trace(arc, tr.steps(max_steps=max_steps), tr.info.capacity_blocks, 0, machine, ctx=f"config{config} m{machine}")
+
+
+@pytest.mark.parametrize("policy", [0, 1])
+def test_config2_lru_and_small_cache_pressure(arc, policy):
+    """Config-2 shaped requests against a cache of 600 blocks: constant eviction, ghost churn, pin fallbacks."""
+    tr = W.make_trace(2, seed=5, scale=0.01)
+    reqs = [r[:16 * 500 + 7] for r in tr.requests(max_requests=300)]
+    steps = [W.pack_requests(reqs[s:s + 16]) for s in range(0, len(reqs), 16)]
+    run_trace(arc, steps, 600, policy, 0, ctx=f"pressure policy {policy}")
+
+
+@pytest.mark.parametrize("machine", [0, 1])
+@pytest.mark.parametrize("c", [1, 2, 3, 5, 8])
+def test_tiny_caches_prefix_trees(arc, c, machine):
+    """Adversarial micro-traces: duplicate requests inside one step, keys dropped from a ghost list and
+    re-accessed in the same step, requests of exactly c blocks, empty and sub-block requests."""
+    rng = np.random.default_rng(100 + c)
+    for policy in (0, 1):
+        gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
+        gc.set_machine(machine)
+        for step in range(60):
+            reqs = W.prefix_tree_requests(rng, n_requests=int(rng.integers(1, 12)), block_size=16, branching=2, depth=3,
+                                          max_blocks=c)
+            if step % 7 == 3:
+                reqs += [reqs[0], reqs[0]]                                # duplicates inside the step
+            if step % 5 == 1:
+                reqs.insert(1, np.zeros(0, np.int32))                     # empty request
+                reqs.append(np.arange(9, dtype=np.int32))                 # shorter than one block
+            tokens, offsets = W.pack_requests(reqs)
+            assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), f"c={c} p={policy} step {step}")
+        assert_same_state(gc, oc, f"c={c} policy {policy}")
+        gc.close()
+
+
+def test_step_partition_invariance_on_gpu(arc):
+    tr = W.make_trace(1, seed=3)
+    reqs = list(tr.requests(max_requests=160))
+    outs = []
+    for rps in (1, 7, 160):
+        gc = arc.ArcCache(64)
+        acc = {k: [] for k in ("prefix_len", "cls", "block_id", "evicted_id", "p_after", "alloc_ids", "evict_ids")}
+        for s in range(0, len(reqs), rps):
+            tokens, offsets = W.pack_requests(reqs[s:s + rps])
+            h = gc.step(dev(tokens), offsets).to_host()
+            for k in acc:
+                acc[k] += h[k].tolist()
+        outs.append(acc)
+        gc.close()
+    assert outs[0] == outs[1] == outs[2]
+
+
+def test_errors_leave_state_unchanged(arc):
+    gc, oc = arc.ArcCache(4), O.OracleCache(4)
+    toks = np.arange(48, dtype=np.int32)
+    assert_same_step(gc.step(dev(toks), [0, 48]).to_host(), oc.step(toks, [0, 48]))
+    big = np.arange(16 * 5, dtype=np.int32)
+    with pytest.raises(arc.ArcError) as e:
+        gc.step(dev(big), [0, 80])
+    assert e.value.code == arc.ERR_REQUEST_TOO_LARGE == oc.step(big, [0, 80])
+    with pytest.raises(arc.ArcError) as e:
+        gc.step(dev(toks), np.array([0, 32, 16]))
+    assert e.value.code == arc.ERR_INVALID_ARG == oc.step(toks, [0, 32, 16])
+    assert_same_state(gc, oc, "after errors")
+    assert_same_step(gc.step(dev(toks[:40]), [0, 0, 15, 15, 40]).to_host(), oc.step(toks[:40], [0, 0, 15, 15, 40]))
+    assert_same_step(gc.step(dev(toks[:0]), [0]).to_host(), oc.step(toks[:0], [0]))
+    assert_same_state(gc, oc, "after empty steps")
+    for bad in ((0, 16, 0), (4, 15, 0), (4, 16, 9)):
+        with pytest.raises(arc.ArcError):
+            arc.ArcCache(*bad)
+    gc.close()
+    gc.close()   # double destroy is a no-op
+
+
+def test_growth_reset_and_host_entry(arc):
+    """Steps larger than the initial buffers (lazy growth with a live directory), arc_reset, arc_step_host."""
+    rng = np.random.default_rng(9)
+    c = 300
+    gc, oc = arc.ArcCache(c), O.OracleCache(c)
+    docs = [rng.integers(0, 32000, size=16 * 40, dtype=np.int32) for _ in range(30)]
+    for n_req in (10, 40, 200, 700, 90):      # 700 x 40 = 28,000 blocks > the initial 4,096
+        reqs = [docs[int(i)] for i in rng.integers(0, 30, size=n_req)]
+        tokens, offsets = W.pack_requests(reqs)
+        assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), f"growth n_req={n_req}")
+    assert_same_state(gc, oc, "growth")
+    gc.reset()
+    oc = O.OracleCache(c)
+    for n_req in (5, 50):
+        reqs = [docs[int(i)] for i in rng.integers(0, 30, size=n_req)]
+        tokens, offsets = W.pack_requests(reqs)
+        h = gc.step_host(tokens, offsets)
+        o = oc.step(tokens, offsets)
+        for k in ("prefix_len", "alloc_ids", "evict_ids"):
+            assert np.array_equal(h[k], o[k]), k
+    assert_same_state(gc, oc, "after reset + step_host")
+    assert gc.launch_count() > 0
+    gc.close()
+
+
+def test_maintenance_rebuild_and_compaction(arc):
+    """Many small steps on one handle: the table rebuild and the ring compaction both trigger many times."""
+    rng = np.random.default_rng(11)
+    c = 128
+    for policy in (0, 1):
+        gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
+        docs = [rng.integers(0, 32000, size=16 * int(n), dtype=np.int32) for n in rng.integers(1, 40, size=60)]
+        for step in range(400):
+            reqs = [np.concatenate([docs[int(i)], rng.integers(0, 32000, size=int(rng.integers(0, 50)), dtype=np.int32)])
+                    for i in rng.zipf(1.2, size=24) % 60]
+            tokens, offsets = W.pack_requests(reqs)
+            g = gc.step(dev(tokens), offsets)
+            o = oc.step(tokens, offsets)
+            if step % 20 == 0 or step > 390:
+                assert_same_step(g.to_host(), o, f"maint policy {policy} step {step}")
+        assert_same_state(gc, oc, f"maintenance policy {policy}")
+        gc.close()
