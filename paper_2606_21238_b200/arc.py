@@ -101,7 +101,7 @@ class _DevView:
     """Zero-copy view of library-owned device memory for torch.as_tensor."""
 
     def __init__(self, ptr: int, n: int, typestr: str):
-        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr or 0, True), "version": 3, "strides": None}
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr or 0, False), "version": 3, "strides": None}
 
 
 def _view(ptr, n, typestr, dtype):

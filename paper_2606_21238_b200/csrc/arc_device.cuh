@@ -18,7 +18,8 @@ namespace arc {
 
 constexpr uint32_t L_ABSENT = 0, L_T1 = 1, L_T2 = 2, L_B1 = 3, L_B2 = 4, L_FREE = 5;
 constexpr unsigned long long KEY_EMPTY = 0ull, KEY_TOMB = 1ull;  // H5 keeps real keys >= 2
-constexpr uint32_t NODE_PENDING = 0xFFFFFFFFu;   // slot claimed, node id not yet published
+constexpr uint32_t SLOT_NODE_PENDING = 0;        // Slot::node holds node id + 1; 0 (what the table memset leaves) =
+                                                 // slot claimed by a key whose node id is not yet published
 constexpr uint32_t NODE_NONE = 0xFFFFFFFFu;
 constexpr uint32_t SLOT_FLAG = 0x80000000u;      // node_acc entry holds a slot index to resolve, not a node id
 constexpr uint32_t BUCKET_SLOTS = 8;             // 8 x 16 B = one 128 B line

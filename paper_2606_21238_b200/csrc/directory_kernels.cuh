@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(256) probe_reserve_kernel(StepParams P) {
       if (match) {
         const int src = __ffs(match) - 1;
         const uint32_t node = tile.shfl(s.node, src);
-        result = (node == NODE_PENDING) ? (SLOT_FLAG | (bucket * BUCKET_SLOTS + src)) : node;
+        result = (node == SLOT_NODE_PENDING) ? (SLOT_FLAG | (bucket * BUCKET_SLOTS + src)) : node - 1;
         break;
       }
       const uint32_t empty = tile.ballot(s.key == KEY_EMPTY);
@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(256) probe_reserve_kernel(StepParams P) {
             st_node(P.nodes + got, L_ABSENT, 0, -1, idx);
             P.node_key[got] = key;
           }
-          __stcg(&P.table[idx].node, got);
+          __stcg(&P.table[idx].node, got + 1);
         }
       }
       got = tile.shfl(got, src);
@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(256) probe_reserve_kernel(StepParams P) {
 __global__ void __launch_bounds__(256) resolve_nodes_kernel(StepParams P) {
   for (uint32_t a = blockIdx.x * blockDim.x + threadIdx.x; a < P.n_access; a += gridDim.x * blockDim.x) {
     const uint32_t v = P.node_acc[a];
-    if (v != NODE_NONE && (v & SLOT_FLAG)) P.node_acc[a] = __ldcg(&P.table[v & ~SLOT_FLAG].node);
+    if (v != NODE_NONE && (v & SLOT_FLAG)) P.node_acc[a] = __ldcg(&P.table[v & ~SLOT_FLAG].node) - 1;
   }
 }
 
@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(StepParams P) {
     if (d == NODE_NONE) continue;
     if (atomicCAS(&P.nodes[d].list, L_ABSENT, L_FREE) == L_ABSENT) {   // still absent, and only once
       const uint32_t slot = P.nodes[d].slot;
-      P.table[slot].node = NODE_PENDING;
+      P.table[slot].node = SLOT_NODE_PENDING;
       P.table[slot].key = KEY_TOMB;
       const uint32_t top = atomicAdd(&P.state->free_top, 1u);
       P.free_stack[top] = d;
@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(256) rebuild_table_kernel(DevState* st, Node* 
       if (atomicCAS(&table[idx].key, KEY_EMPTY, key) == KEY_EMPTY) break;
       idx = (idx + 1) & slot_mask;
     }
-    table[idx].node = n;
+    table[idx].node = n + 1;
     nodes[n].slot = idx;
   }
 }

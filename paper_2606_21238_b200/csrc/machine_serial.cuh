@@ -90,7 +90,7 @@ __global__ void arc_machine_serial_kernel(StepParams P) {
     for (int64_t j = 0; j < nb; ++j) {          // access order: tail block first (R2)
       const int64_t a = o + j, out = o + (nb - 1 - j);
       uint32_t n = P.node_acc[a];
-      if (n & SLOT_FLAG) n = __ldcg(&P.table[n & ~SLOT_FLAG].node);
+      if (n & SLOT_FLAG) n = __ldcg(&P.table[n & ~SLOT_FLAG].node) - 1;
       const Node rec = ld_node(P.nodes + n);
       int cls;
       int32_t blk = rec.block, ev = -1;
