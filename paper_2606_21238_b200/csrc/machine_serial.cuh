@@ -7,26 +7,28 @@
 namespace arc {
 
 struct SerialCtx {
-  StepParams P;
-  uint32_t head[5], tail[5];
+  uint32_t head[5], tail[5];   // only ever indexed with compile-time constants, so they live in registers
   uint32_t bound[5];     // victim scans stop here: tail of T1/T2 when the request began (R4), current tail for B1/B2
   int32_t t1, t2, b1, b2, p, next_fresh;
-  unsigned long long stat[ST_COUNT];
+  uint32_t stat[ST_COUNT];   // per-step deltas (a step has < 2^31 accesses)
   uint32_t err;
+  uint32_t n_alloc, n_evict;
 };
 
-__device__ __forceinline__ void ring_push(SerialCtx& C, uint32_t L, uint32_t n, int32_t block, uint32_t slot) {
+template <uint32_t L>
+__device__ __forceinline__ void ring_push(SerialCtx& C, const StepParams& P, uint32_t n, int32_t block, uint32_t slot) {
   const uint32_t q = C.tail[L]++;
-  C.P.ring[L][q & C.P.ring_mask] = n;
-  st_node(C.P.nodes + n, L, q, block, slot);
+  P.ring[L][q & P.ring_mask] = n;
+  st_node(P.nodes + n, L, q, block, slot);
 }
 
 // first live entry of list L in [head, bound); advances head past everything it skipped.  NODE_NONE if none.
-__device__ __forceinline__ uint32_t ring_pop_lru(SerialCtx& C, uint32_t L, uint32_t bound, Node* rec_out) {
+template <uint32_t L>
+__device__ __forceinline__ uint32_t ring_pop_lru(SerialCtx& C, const StepParams& P, uint32_t bound, Node* rec_out) {
   uint32_t q = C.head[L];
   while (q != bound) {
-    const uint32_t n = C.P.ring[L][q & C.P.ring_mask];
-    const Node r = ld_node(C.P.nodes + n);
+    const uint32_t n = __ldcg(P.ring[L] + (q & P.ring_mask));
+    const Node r = ld_node(P.nodes + n);
     if (r.list == L && r.pos == q) { C.head[L] = q + 1; *rec_out = r; return n; }
     ++q;
   }
@@ -35,16 +37,22 @@ __device__ __forceinline__ uint32_t ring_pop_lru(SerialCtx& C, uint32_t L, uint3
 }
 
 // R7.  Returns the freed block id; the victim becomes a ghost at the MRU end of B1 / B2.
-__device__ __forceinline__ int32_t replace_serial(SerialCtx& C, bool in_b2) {
+__device__ __forceinline__ int32_t replace_serial(SerialCtx& C, const StepParams& P, bool in_b2) {
   const bool prefer_t1 = C.t1 >= 1 && (C.t1 > C.p || (in_b2 && C.t1 == C.p));
   for (int attempt = 0; attempt < 2; ++attempt) {
     const bool from_t1 = (attempt == 0) ? prefer_t1 : !prefer_t1;
-    const uint32_t L = from_t1 ? L_T1 : L_T2;
     Node r;
-    const uint32_t v = ring_pop_lru(C, L, C.bound[L], &r);
-    if (v == NODE_NONE) continue;
-    ring_push(C, from_t1 ? L_B1 : L_B2, v, -1, r.slot);
-    if (from_t1) { C.t1--; C.b1++; C.stat[ST_EVICT_T1]++; } else { C.t2--; C.b2++; C.stat[ST_EVICT_T2]++; }
+    if (from_t1) {
+      const uint32_t v = ring_pop_lru<L_T1>(C, P, C.bound[L_T1], &r);
+      if (v == NODE_NONE) continue;
+      ring_push<L_B1>(C, P, v, -1, r.slot);
+      C.t1--; C.b1++; C.stat[ST_EVICT_T1]++;
+    } else {
+      const uint32_t v = ring_pop_lru<L_T2>(C, P, C.bound[L_T2], &r);
+      if (v == NODE_NONE) continue;
+      ring_push<L_B2>(C, P, v, -1, r.slot);
+      C.t2--; C.b2++; C.stat[ST_EVICT_T2]++;
+    }
     return r.block;
   }
   C.err = DEV_ERR_NO_VICTIM;
@@ -52,109 +60,124 @@ __device__ __forceinline__ int32_t replace_serial(SerialCtx& C, bool in_b2) {
 }
 
 // evict the first unpinned entry of T1 without leaving a ghost (case 4A-else, LRU mode); node -> ABSENT
-__device__ __forceinline__ int32_t evict_t1_no_ghost_serial(SerialCtx& C, uint32_t* dropped) {
+__device__ __forceinline__ int32_t evict_t1_no_ghost_serial(SerialCtx& C, const StepParams& P, uint32_t* dropped) {
   Node r;
-  const uint32_t v = ring_pop_lru(C, L_T1, C.bound[L_T1], &r);
+  const uint32_t v = ring_pop_lru<L_T1>(C, P, C.bound[L_T1], &r);
   if (v == NODE_NONE) { C.err = DEV_ERR_NO_VICTIM; return -1; }
-  st_node(C.P.nodes + v, L_ABSENT, 0, -1, r.slot);
+  st_node(P.nodes + v, L_ABSENT, 0, -1, r.slot);
   *dropped = v;
   C.t1--; C.stat[ST_EVICT_T1]++;
   return r.block;
 }
 
-__device__ __forceinline__ void drop_ghost_serial(SerialCtx& C, uint32_t L, uint32_t* dropped) {
+template <uint32_t L>
+__device__ __forceinline__ void drop_ghost_serial(SerialCtx& C, const StepParams& P, uint32_t* dropped) {
   Node r;
-  const uint32_t d = ring_pop_lru(C, L, C.tail[L], &r);
+  const uint32_t d = ring_pop_lru<L>(C, P, C.tail[L], &r);
   if (d == NODE_NONE) { C.err = DEV_ERR_BAD_NODE; return; }
-  st_node(C.P.nodes + d, L_ABSENT, 0, -1, r.slot);
+  st_node(P.nodes + d, L_ABSENT, 0, -1, r.slot);
   *dropped = d;
   if (L == L_B1) { C.b1--; C.stat[ST_DROP_B1]++; } else { C.b2--; C.stat[ST_DROP_B2]++; }
+}
+
+// Loads / stores the scalar machine state kept in DevState.
+__device__ __forceinline__ void ctx_load(SerialCtx& C, const StepParams& P) {
+  const DevState* S = P.state;
+#pragma unroll
+  for (int L = 1; L <= 4; ++L) { C.head[L] = S->head[L]; C.tail[L] = S->tail[L]; C.bound[L] = S->tail[L]; }
+  C.t1 = S->t1; C.t2 = S->t2; C.b1 = S->b1; C.b2 = S->b2; C.p = S->p; C.next_fresh = S->next_fresh;
+#pragma unroll
+  for (int i = 0; i < ST_COUNT; ++i) C.stat[i] = 0;
+  C.err = 0;
+  C.n_alloc = 0; C.n_evict = 0;
+}
+__device__ __forceinline__ void ctx_store(const SerialCtx& C, const StepParams& P) {
+  DevState* S = P.state;
+#pragma unroll
+  for (int L = 1; L <= 4; ++L) { S->head[L] = C.head[L]; S->tail[L] = C.tail[L]; }
+  S->t1 = C.t1; S->t2 = C.t2; S->b1 = C.b1; S->b2 = C.b2; S->p = C.p; S->next_fresh = C.next_fresh;
+  S->counts[0] = C.n_alloc; S->counts[1] = C.n_evict;
+#pragma unroll
+  for (int i = 0; i < ST_COUNT; ++i) S->stat[i] += C.stat[i];
+  if (C.err) S->error = C.err;
+}
+
+// One access (R5 for ARC, R10 for LRU) against the live state: access index a (access order), output index out
+// (natural order).  C.bound[T1/T2] must hold the tails recorded when the access's request began (R4).
+__device__ __forceinline__ void serial_access(SerialCtx& C, const StepParams& P, int64_t a, int64_t out) {
+  const int32_t c = P.capacity;
+  uint32_t n = P.node_acc[a];
+  if (n & SLOT_FLAG) n = __ldcg(&P.table[n & ~SLOT_FLAG].node) - 1;
+  const Node rec = ld_node(P.nodes + n);
+  int cls;
+  int32_t blk = rec.block, ev = -1;
+  uint32_t dropped = NODE_NONE;
+  C.stat[ST_ACCESSES]++;
+  if (P.policy == POLICY_LRU) {             // R10
+    if (rec.list == L_T1) {
+      cls = CLS_HIT_T1; C.stat[ST_HIT_T1]++;
+      ring_push<L_T1>(C, P, n, blk, rec.slot);
+    } else {
+      cls = CLS_MISS; C.stat[ST_MISS]++;
+      if (C.t1 < c) { blk = C.next_fresh++; C.stat[ST_FRESH]++; }
+      else blk = ev = evict_t1_no_ghost_serial(C, P, &dropped);
+      ring_push<L_T1>(C, P, n, blk, rec.slot);
+      C.t1++;
+    }
+  } else if (rec.list == L_T1 || rec.list == L_T2) {      // R5 case 1
+    if (rec.list == L_T1) { cls = CLS_HIT_T1; C.stat[ST_HIT_T1]++; C.t1--; C.t2++; }
+    else { cls = CLS_HIT_T2; C.stat[ST_HIT_T2]++; }
+    ring_push<L_T2>(C, P, n, blk, rec.slot);
+  } else if (rec.list == L_B1) {                          // case 2
+    cls = CLS_GHOST_B1; C.stat[ST_GHOST_B1]++;
+    int32_t delta = C.b2 / C.b1; if (delta < 1) delta = 1;
+    C.p = min(c, C.p + delta);
+    blk = ev = replace_serial(C, P, false);
+    C.b1--; C.t2++;
+    ring_push<L_T2>(C, P, n, blk, rec.slot);
+  } else if (rec.list == L_B2) {                          // case 3
+    cls = CLS_GHOST_B2; C.stat[ST_GHOST_B2]++;
+    int32_t delta = C.b1 / C.b2; if (delta < 1) delta = 1;
+    C.p = max(0, C.p - delta);
+    blk = ev = replace_serial(C, P, true);
+    C.b2--; C.t2++;
+    ring_push<L_T2>(C, P, n, blk, rec.slot);
+  } else {                                                // case 4 (ABSENT)
+    cls = CLS_MISS; C.stat[ST_MISS]++;
+    if (rec.list != L_ABSENT) C.err = DEV_ERR_BAD_NODE;
+    if (C.t1 + C.b1 == c) {                               // (A)
+      if (C.t1 < c) { drop_ghost_serial<L_B1>(C, P, &dropped); blk = ev = replace_serial(C, P, false); }
+      else blk = ev = evict_t1_no_ghost_serial(C, P, &dropped);
+    } else {                                              // (B)
+      const int32_t tot = C.t1 + C.t2 + C.b1 + C.b2;
+      if (tot >= c) {
+        if (tot == 2 * c) drop_ghost_serial<L_B2>(C, P, &dropped);
+        blk = ev = replace_serial(C, P, false);
+      } else { blk = C.next_fresh++; C.stat[ST_FRESH]++; }
+    }
+    ring_push<L_T1>(C, P, n, blk, rec.slot);
+    C.t1++;
+  }
+  P.cls[out] = (uint8_t)cls;
+  P.block_id[out] = blk;
+  P.evicted_id[out] = ev;
+  P.p_after[out] = C.p;
+  P.dropped[a] = dropped;
+  if (cls != CLS_HIT_T1 && cls != CLS_HIT_T2) P.alloc_ids[C.n_alloc++] = blk;
+  if (ev >= 0) P.evict_ids[C.n_evict++] = ev;
 }
 
 __global__ void arc_machine_serial_kernel(StepParams P) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   SerialCtx C;
-  C.P = P;
-  DevState* S = P.state;
-  for (int L = 1; L <= 4; ++L) { C.head[L] = S->head[L]; C.tail[L] = S->tail[L]; }
-  C.t1 = S->t1; C.t2 = S->t2; C.b1 = S->b1; C.b2 = S->b2; C.p = S->p; C.next_fresh = S->next_fresh;
-  for (int i = 0; i < ST_COUNT; ++i) C.stat[i] = 0;
-  C.err = 0;
-  const int32_t c = P.capacity;
-  uint32_t n_alloc = 0, n_evict = 0;
-
+  ctx_load(C, P);
   for (uint32_t r = 0; r < P.n_req; ++r) {
     const int64_t o = P.blk_off[r], nb = P.blk_off[r + 1] - o;
     C.bound[L_T1] = C.tail[L_T1];   // entries pushed from here on belong to this request: pinned (R4)
     C.bound[L_T2] = C.tail[L_T2];
-    for (int64_t j = 0; j < nb; ++j) {          // access order: tail block first (R2)
-      const int64_t a = o + j, out = o + (nb - 1 - j);
-      uint32_t n = P.node_acc[a];
-      if (n & SLOT_FLAG) n = __ldcg(&P.table[n & ~SLOT_FLAG].node) - 1;
-      const Node rec = ld_node(P.nodes + n);
-      int cls;
-      int32_t blk = rec.block, ev = -1;
-      uint32_t dropped = NODE_NONE;
-      C.stat[ST_ACCESSES]++;
-      if (P.policy == POLICY_LRU) {             // R10
-        if (rec.list == L_T1) {
-          cls = CLS_HIT_T1; C.stat[ST_HIT_T1]++;
-          ring_push(C, L_T1, n, blk, rec.slot);
-        } else {
-          cls = CLS_MISS; C.stat[ST_MISS]++;
-          if (C.t1 < c) { blk = C.next_fresh++; C.stat[ST_FRESH]++; }
-          else blk = ev = evict_t1_no_ghost_serial(C, &dropped);
-          ring_push(C, L_T1, n, blk, rec.slot);
-          C.t1++;
-        }
-      } else if (rec.list == L_T1 || rec.list == L_T2) {      // R5 case 1
-        if (rec.list == L_T1) { cls = CLS_HIT_T1; C.stat[ST_HIT_T1]++; C.t1--; C.t2++; }
-        else { cls = CLS_HIT_T2; C.stat[ST_HIT_T2]++; }
-        ring_push(C, L_T2, n, blk, rec.slot);
-      } else if (rec.list == L_B1) {                          // case 2
-        cls = CLS_GHOST_B1; C.stat[ST_GHOST_B1]++;
-        int32_t delta = C.b2 / C.b1; if (delta < 1) delta = 1;
-        C.p = min(c, C.p + delta);
-        blk = ev = replace_serial(C, false);
-        C.b1--; C.t2++;
-        ring_push(C, L_T2, n, blk, rec.slot);
-      } else if (rec.list == L_B2) {                          // case 3
-        cls = CLS_GHOST_B2; C.stat[ST_GHOST_B2]++;
-        int32_t delta = C.b1 / C.b2; if (delta < 1) delta = 1;
-        C.p = max(0, C.p - delta);
-        blk = ev = replace_serial(C, true);
-        C.b2--; C.t2++;
-        ring_push(C, L_T2, n, blk, rec.slot);
-      } else {                                                // case 4 (ABSENT)
-        cls = CLS_MISS; C.stat[ST_MISS]++;
-        if (rec.list != L_ABSENT) C.err = DEV_ERR_BAD_NODE;
-        if (C.t1 + C.b1 == c) {                               // (A)
-          if (C.t1 < c) { drop_ghost_serial(C, L_B1, &dropped); blk = ev = replace_serial(C, false); }
-          else blk = ev = evict_t1_no_ghost_serial(C, &dropped);
-        } else {                                              // (B)
-          const int32_t tot = C.t1 + C.t2 + C.b1 + C.b2;
-          if (tot >= c) {
-            if (tot == 2 * c) drop_ghost_serial(C, L_B2, &dropped);
-            blk = ev = replace_serial(C, false);
-          } else { blk = C.next_fresh++; C.stat[ST_FRESH]++; }
-        }
-        ring_push(C, L_T1, n, blk, rec.slot);
-        C.t1++;
-      }
-      P.cls[out] = (uint8_t)cls;
-      P.block_id[out] = blk;
-      P.evicted_id[out] = ev;
-      P.p_after[out] = C.p;
-      P.dropped[a] = dropped;
-      if (cls != CLS_HIT_T1 && cls != CLS_HIT_T2) P.alloc_ids[n_alloc++] = blk;
-      if (ev >= 0) P.evict_ids[n_evict++] = ev;
-    }
+    for (int64_t j = 0; j < nb; ++j) serial_access(C, P, o + j, o + (nb - 1 - j));   // tail block first (R2)
   }
-  for (int L = 1; L <= 4; ++L) { S->head[L] = C.head[L]; S->tail[L] = C.tail[L]; }
-  S->t1 = C.t1; S->t2 = C.t2; S->b1 = C.b1; S->b2 = C.b2; S->p = C.p; S->next_fresh = C.next_fresh;
-  S->counts[0] = n_alloc; S->counts[1] = n_evict;
-  for (int i = 0; i < ST_COUNT; ++i) S->stat[i] += C.stat[i];
-  if (C.err) S->error = C.err;
+  ctx_store(C, P);
 }
 
 }  // namespace arc
