@@ -299,6 +299,7 @@ def run_ours(args):
         peak, peak_src = peaks()
         # per-kernel breakdown: a separate pass with CUDA events between the kernels (it syncs every step)
         c2, _, sums, _ = run_device_resident(torch, A, info, steps, dev, bases, W_, A.POLICY_ARC, stream, profile=True)
+        line["k3_debug"] = c2.debug_counters()
         c2.close()
         tot = max(sums.get("total_ms", 0.0), 1e-9)
         line["kernels"] = {k: {"ms_per_step": v / K, "share": v / tot} for k, v in sums.items() if k != "total_ms"}

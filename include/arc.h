@@ -154,6 +154,12 @@ uint64_t arc_launch_count(const arc_cache *h);
  * serial walk (correctness reference on the device; same results, much slower). */
 int arc_set_machine(arc_cache *h, int which);
 
+/* K3 diagnostics, cumulative since create/reset: out[0..n) (HOST) receives, in this order, the number of
+ * all-hit windows, general windows, by-the-book single accesses, windows cut at a repeated node, windows cut at a
+ * conflict, ring scan rounds, accesses applied in all-hit windows, accesses applied in general windows, then
+ * SM cycles spent in: fetch, roll-forward, victim scan, apply, single accesses, the whole kernel.  Synchronises. */
+int arc_debug_counters(arc_cache *h, uint64_t *out, uint32_t n);
+
 /* Copies one list (1 = T1, 2 = T2, 3 = B1, 4 = B2) in LRU -> MRU order to HOST arrays keys_out /
  * block_ids_out (either may be NULL), at most cap entries; *n_out receives the list length.
  * Synchronises.  For tests. */

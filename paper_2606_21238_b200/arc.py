@@ -25,7 +25,7 @@ STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", 
 # every symbol include/arc.h declares (checked by the CPU test-suite against the built library)
 EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats", "arc_reset", "arc_destroy",
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
-           "arc_set_machine", "arc_debug_list"]
+           "arc_set_machine", "arc_debug_list", "arc_debug_counters"]
 
 
 class ArcError(RuntimeError):
@@ -83,6 +83,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_launch_count.argtypes = [vp]
     L.arc_launch_count.restype = u64
     L.arc_set_machine.argtypes = [vp, C.c_int]
+    L.arc_debug_counters.argtypes = [vp, vp, u32]
     L.arc_debug_list.argtypes = [vp, C.c_int, vp, vp, u64, C.POINTER(u64)]
     if path is None:
         _lib = L
@@ -234,6 +235,14 @@ class ArcCache:
 
     def set_machine(self, which: int):
         self._check(self._L.arc_set_machine(self._h, which))
+
+    DEBUG_COUNTERS = ["win_hit", "win_general", "win_serial", "cut_twin", "cut_conflict", "scan_rounds", "acc_hit_win",
+                      "acc_general_win", "cyc_fetch", "cyc_roll", "cyc_scan", "cyc_apply", "cyc_serial", "cyc_total"]
+
+    def debug_counters(self) -> dict:
+        out = np.zeros(len(self.DEBUG_COUNTERS), np.uint64)
+        self._check(self._L.arc_debug_counters(self._h, out.ctypes.data, len(out)))
+        return {k: int(v) for k, v in zip(self.DEBUG_COUNTERS, out)}
 
     def debug_lists(self) -> dict:
         out = {}

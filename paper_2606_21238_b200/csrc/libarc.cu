@@ -583,6 +583,15 @@ int arc_set_machine(arc_cache* h, int which) {
   return ARC_OK;
 }
 
+int arc_debug_counters(arc_cache* h, uint64_t* out, uint32_t n) {
+  if (!h || !out) return ARC_ERR_INVALID_ARG;
+  CUDA_TRY(h, cudaStreamSynchronize(h->last_stream));
+  DevState st;
+  CUDA_TRY(h, cudaMemcpy(&st, h->d_state, sizeof(st), cudaMemcpyDeviceToHost));
+  for (uint32_t i = 0; i < n; ++i) out[i] = (i < (uint32_t)DBG_COUNT) ? st.dbg[i] : 0;
+  return ARC_OK;
+}
+
 int arc_debug_list(arc_cache* h, int which, uint64_t* keys_out, int32_t* block_ids_out, uint64_t cap, uint64_t* n_out) {
   if (!h || which < 1 || which > 4 || !n_out) return ARC_ERR_INVALID_ARG;
   cudaStream_t s = h->last_stream;

@@ -3,18 +3,23 @@
 //
 // Why a window can be applied at once:
 //  * K2 has already given every access its node id, so the 32 node records are fetched in parallel
-//    (one L2 round trip instead of 32 dependent ones).
+//    (one L2 round trip instead of 32 dependent ones); the node ids of the following window are
+//    prefetched, and the first 32 ring entries of every list head (the possible victims) travel in the
+//    same two round trips.
 //  * An access's class is decided by its node's list.  Inside a window the only ways an earlier access
 //    can change a later access's class are (1) both touch the same node (the window is cut before the
 //    second occurrence), (2) the earlier access evicts / drops the later one's node.  (2) needs the
 //    later node's ring position to lie inside the range of ring positions the window's victim scans
 //    consume; that is checked, and the window is cut before the first such access.
 //  * Given the classes, the counters t1,t2,b1,b2,p and with them every REPLACE decision (R5-R7) follow
-//    from a scalar recurrence that every lane rolls forward in registers (no memory access).
+//    from a scalar recurrence that every lane rolls forward in registers (no memory access).  The pin
+//    fallback of R7 is part of the recurrence: elig1 / elig2 count the entries of T1 / T2 that the
+//    current request may still evict.  Runs of equal classes whose decisions are provably identical
+//    (hits; misses at the fixed points of the recurrence) are rolled in O(1).
 //  * The j-th eviction from list L takes the j-th live entry from L's LRU end: a 32-wide scan of the
 //    lazy-FIFO ring with ballot/popc ranks; entries pushed by the current request sit at positions
 //    >= bound[L] and are therefore never reached (pins, R4).
-//  * If a list cannot supply the victims the recurrence assumed (the pin fallback of R7), the window is cut
+//  * If a ghost list cannot supply a drop from the entries it held before the window, the window is cut
 //    before that access and the access is done by the by-the-book single-access routine.
 // Windows never cross a request boundary (the pin scope changes there).
 #pragma once
@@ -23,54 +28,121 @@
 namespace arc {
 
 struct Roll {
-  int32_t t1, t2, b1, b2, p, nf;
-  uint32_t my_src;    // 0 none / fresh id, 1 T1 -> B1, 2 T2 -> B2, 3 T1 without a ghost
-  uint32_t my_drop;   // 0, L_B1, L_B2
-  int32_t my_p, my_fresh;
+  int32_t t1, t2, b1, b2, p, nf, e1, e2;
+  uint32_t s0, s1;     // eviction source of access i, bit-sliced: 0 none, 1 T1 -> B1, 2 T2 -> B2, 3 T1 without a ghost
+  uint32_t d1, d2;     // access i drops the LRU ghost of B1 / B2
+  uint32_t fm;         // access i takes a fresh block id
+  int32_t my_p;        // p after this lane's access
+  uint32_t err;
 };
 
-// The counter recurrence of R5-R7 / R10 over the first k accesses of the window whose node lists are given
-// bit-sliced in (m0, m1, m2).  Every lane runs it identically; lane i keeps the decisions of access i.
+__device__ __forceinline__ uint32_t bits_from(int i, int n) { return ((n >= 32) ? 0xFFFFFFFFu : ((1u << n) - 1u)) << i; }
+
+// R7 with pins: the preferred list if it still has an entry this request may evict, else the other one.
+__device__ __forceinline__ void roll_replace(Roll& R, bool inb2, int i) {
+  const bool prefer1 = R.t1 >= 1 && (R.t1 > R.p || (inb2 && R.t1 == R.p));
+  const bool from1 = prefer1 ? (R.e1 > 0) : !(R.e2 > 0);
+  if (from1) { R.s0 |= 1u << i; R.t1--; R.b1++; R.e1--; if (R.e1 < 0) R.err = DEV_ERR_NO_VICTIM; }
+  else { R.s1 |= 1u << i; R.t2--; R.b2++; R.e2--; }
+}
+
+// The counter recurrence of R5-R7 / R10 over the first k accesses of the window.  (m0, m1, m2) = the node lists,
+// bit-sliced; me = the access is a hit on an entry that was still evictable (below bound).  Uniform across lanes.
 __device__ __forceinline__ Roll roll_forward(const SerialCtx& C, int32_t c, bool lru, uint32_t m0, uint32_t m1, uint32_t m2,
-                                             int k, int lane) {
+                                             uint32_t me, int k, int lane) {
   Roll R;
-  R.t1 = C.t1; R.t2 = C.t2; R.b1 = C.b1; R.b2 = C.b2; R.p = C.p; R.nf = C.next_fresh;
-  R.my_src = 0; R.my_drop = 0; R.my_p = C.p; R.my_fresh = -1;
-  for (int i = 0; i < k; ++i) {
+  R.t1 = C.t1; R.t2 = C.t2; R.b1 = C.b1; R.b2 = C.b2; R.p = C.p; R.nf = C.next_fresh; R.e1 = C.elig1; R.e2 = C.elig2;
+  R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = C.p; R.err = 0;
+  const uint32_t km = bits_from(0, k);
+  int i = 0;
+  while (i < k) {
     const uint32_t li = ((m0 >> i) & 1u) | (((m1 >> i) & 1u) << 1) | (((m2 >> i) & 1u) << 2);
-    uint32_t src = 0, drop = 0;
-    int32_t fresh = -1;
+    // length of the run of accesses with this same list code
+    const uint32_t same = ((li & 1u) ? m0 : ~m0) & ((li & 2u) ? m1 : ~m1) & ((li & 4u) ? m2 : ~m2) & km;
+    const uint32_t brk = ~(same >> i);
+    const int m = brk ? (__ffs(brk) - 1) : 32;
+    int n = 1;
     if (lru) {
-      if (li != L_T1) {
-        if (R.t1 < c) { fresh = R.nf++; R.t1++; } else src = 3;
+      if (li == L_T1) {                       // hits: only the evictable count moves
+        n = m; R.e1 -= __popc(me & bits_from(i, n));
+      } else if (R.t1 < c) {                  // cold fill
+        n = min(m, c - R.t1); R.fm |= bits_from(i, n); R.t1 += n; R.nf += n;
+      } else {                                // full: every miss evicts T1's LRU entry, no ghost
+        n = max(1, min(m, R.e1));
+        R.s0 |= bits_from(i, n); R.s1 |= bits_from(i, n); R.e1 -= n;
+        if (R.e1 < 0) R.err = DEV_ERR_NO_VICTIM;
       }
     } else if (li == L_T1) {
-      R.t1--; R.t2++;
+      n = m; R.t1 -= n; R.t2 += n; R.e1 -= __popc(me & bits_from(i, n));
     } else if (li == L_T2) {
-    } else if (li == L_B1 || li == L_B2) {
-      const bool inb2 = (li == L_B2);
-      int32_t delta = inb2 ? (R.b1 / max(R.b2, 1)) : (R.b2 / max(R.b1, 1));
-      delta = max(delta, 1);
-      R.p = inb2 ? max(0, R.p - delta) : min(c, R.p + delta);
-      const bool from_t1 = R.t1 >= 1 && (R.t1 > R.p || (inb2 && R.t1 == R.p));
-      if (from_t1) { src = 1; R.t1--; R.b1++; } else { src = 2; R.t2--; R.b2++; }
-      if (inb2) R.b2--; else R.b1--;
-      R.t2++;
-    } else {
-      bool repl = false;
+      n = m; R.e2 -= __popc(me & bits_from(i, n));
+    } else if (li == L_B1) {
+      // ghost hit in B1 (R5 case 2).  With delta = 1 (b2 < 2 b1) the steps of a run are identical while the
+      // victim keeps coming from the same list, so the run is rolled in O(1); anything else is one by-the-book step.
+      const bool d_one = R.b2 < 2 * R.b1;
+      const int32_t J = max(0, (R.t1 - R.p) / 2);         // steps j with t1 - j > p + j + 1  (REPLACE prefers T1)
+      const int32_t p0 = R.p;
+      if (d_one && J > 0 && R.e1 > 0) {                   // victims from T1: t1--, t2++, p++ per step
+        n = min(min(m, R.e1), J);
+        R.s0 |= bits_from(i, n); R.t1 -= n; R.t2 += n; R.e1 -= n; R.p += n;
+      } else if (d_one && J == 0 && R.e2 > 0) {           // victims from T2: b1--, b2++, p++ per step, while delta stays 1
+        n = min(min(m, R.e2), (2 * R.b1 - R.b2 + 2) / 3);
+        R.s1 |= bits_from(i, n); R.b1 -= n; R.b2 += n; R.e2 -= n; R.p = min(c, R.p + n);
+      } else {
+        const int32_t d = (R.b2 >= 2 * R.b1 && R.b1 > 0) ? R.b2 / R.b1 : 1;
+        R.p = min(c, R.p + d);
+        roll_replace(R, false, i);
+        R.b1--; R.t2++;
+      }
+      if (lane >= i) R.my_p = (n > 1 || R.p - p0 == 1) ? min(c, p0 + min(lane - i + 1, n)) : R.p;
+    } else if (li == L_B2) {
+      // ghost hit in B2 (R5 case 3), same structure: p falls by delta = 1 while b1 < 2 b2
+      const bool d_one = R.b1 < 2 * R.b2;
+      const int32_t p0 = R.p;
+      if (d_one && R.t1 >= 1 && R.t1 >= R.p - 1 && R.e1 > 0) {   // REPLACE(true) takes T1 while t1 >= 1: t1--, t2++, b1++, b2--
+        n = min(min(m, R.e1), min((2 * R.b2 - R.b1 + 2) / 3, R.t1));
+        R.s0 |= bits_from(i, n); R.t1 -= n; R.t2 += n; R.b1 += n; R.b2 -= n; R.e1 -= n; R.p = max(0, R.p - n);
+      } else if (d_one && (R.t1 == 0 || R.t1 < R.p - 1) && R.e2 > 0) {   // victims from T2: only p and elig2 move
+        n = min(m, R.e2);
+        if (R.t1 >= 1) n = min(n, R.p - 1 - R.t1);
+        R.s1 |= bits_from(i, n); R.e2 -= n; R.p = max(0, R.p - n);
+      } else {
+        const int32_t d = (R.b1 >= 2 * R.b2 && R.b2 > 0) ? R.b1 / R.b2 : 1;
+        R.p = max(0, R.p - d);
+        roll_replace(R, true, i);
+        R.b2--; R.t2++;
+      }
+      if (lane >= i) R.my_p = (n > 1 || p0 - R.p <= 1) ? max(0, p0 - min(lane - i + 1, n)) : R.p;
+    } else if (R.t1 + R.t2 < c) {             // miss while the cache is filling: b1 = b2 = 0 (I7)
+      n = min(m, c - R.t1 - R.t2); R.fm |= bits_from(i, n); R.t1 += n; R.nf += n;
+    } else if (R.t1 < c && R.t1 > R.p && R.e1 > 0) {
+      // miss, REPLACE takes T1's LRU entry (t1 stays).  Case 4A (t1 + b1 = c): B1's LRU ghost is dropped, nothing moves.
+      // Case 4B: b1 grows by one per miss; B2's LRU ghost is dropped while b1 + b2 = c.
+      const int32_t gapA = c - R.t1 - R.b1, gapS = c - R.b1 - R.b2;
+      if (gapA == 0) { n = min(m, R.e1); R.d1 |= bits_from(i, n); }
+      else if (gapS == 0) { n = min(min(m, R.e1), gapA); R.d2 |= bits_from(i, n); R.b2 -= n; R.b1 += n; }
+      else { n = min(min(m, R.e1), min(gapA, gapS)); R.b1 += n; }
+      R.s0 |= bits_from(i, n); R.e1 -= n;
+    } else if (R.t1 < c && R.t1 <= R.p && R.e2 > 0) {
+      // miss while T1 is at or below its target: REPLACE takes T2's LRU entry, T1 grows by one per miss
+      const int32_t gapA = c - R.t1 - R.b1, gapS = c - R.b1 - R.b2;
+      n = min(min(m, R.e2), min(R.p - R.t1 + 1, c - R.t1));
+      if (gapA == 0) { R.d1 |= bits_from(i, n); R.b1 -= n; R.b2 += n; }
+      else if (gapS == 0) { n = min(n, gapA); R.d2 |= bits_from(i, n); }
+      else { n = min(n, min(gapA, gapS)); R.b2 += n; }
+      R.s1 |= bits_from(i, n); R.t1 += n; R.t2 -= n; R.e2 -= n;
+    } else {                                  // any other miss (pin fallback, T1 holding everything): one by-the-book step
       if (R.t1 + R.b1 == c) {
-        if (R.t1 < c) { drop = L_B1; R.b1--; repl = true; } else { src = 3; R.t1--; }
+        if (R.t1 < c) { R.d1 |= 1u << i; R.b1--; roll_replace(R, false, i); }
+        else { R.s0 |= 1u << i; R.s1 |= 1u << i; R.t1--; R.e1--; if (R.e1 < 0) R.err = DEV_ERR_NO_VICTIM; }
       } else {
         const int32_t tot = R.t1 + R.t2 + R.b1 + R.b2;
-        if (tot >= c) { if (tot == 2 * c) { drop = L_B2; R.b2--; } repl = true; }
-        else fresh = R.nf++;
-      }
-      if (repl) {
-        if (R.t1 >= 1 && R.t1 > R.p) { src = 1; R.t1--; R.b1++; } else { src = 2; R.t2--; R.b2++; }
+        if (tot == 2 * c) { R.d2 |= 1u << i; R.b2--; }
+        roll_replace(R, false, i);            // tot >= c here because the cache is full
       }
       R.t1++;
     }
-    if (i == lane) { R.my_src = src; R.my_drop = drop; R.my_p = R.p; R.my_fresh = fresh; }
+    i += n;
   }
   return R;
 }
@@ -81,8 +153,17 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
   const bool lru = (P.policy == POLICY_LRU);
   const int32_t c = P.capacity;
+  const int64_t N = (int64_t)P.n_access;
   SerialCtx C;            // identical in every lane
   ctx_load(C, P);
+  unsigned long long dbg[DBG_COUNT];
+#pragma unroll
+  for (int i = 0; i < DBG_COUNT; ++i) dbg[i] = 0;
+  const long long t_begin = clock64();
+
+  // node ids are prefetched one window ahead: pre_n = node_acc[pre_base + lane]
+  int64_t pre_base = 0;
+  uint32_t pre_n = (lane < N) ? P.node_acc[lane] : NODE_NONE;
 
   int64_t my_off = 0, my_off1 = 0;
   for (uint32_t r = 0; r < P.n_req; ++r) {
@@ -91,26 +172,45 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
       my_off = P.blk_off[rr]; my_off1 = P.blk_off[rr + 1];
     }
     const int64_t o = __shfl_sync(FULL, my_off, r & 31), nb = __shfl_sync(FULL, my_off1, r & 31) - o;
-    C.bound[L_T1] = C.tail[L_T1];
-    C.bound[L_T2] = C.tail[L_T2];
+    begin_request(C);
     int64_t j = 0;
     while (j < nb) {
-      int k = (int)min((int64_t)32, nb - j);
+      const int kmax = (int)min((int64_t)32, nb - j);
+      int k = kmax;
       const int64_t a0 = o + j;
       const bool act0 = lane < k;
-      const uint32_t n = act0 ? P.node_acc[a0 + lane] : NODE_NONE;
+      const long long tw0 = clock64();
+      uint32_t n = pre_n;
+      if (pre_base != a0) n = (a0 + lane < N) ? P.node_acc[a0 + lane] : NODE_NONE;   // the last window was cut short
       Node rec;
       rec.list = L_FREE; rec.pos = 0; rec.block = -1; rec.slot = 0;
       if (act0) rec = ld_node(P.nodes + n);
+      // the first 32 ring entries from every list head travel with the node records (used only by general windows)
+      uint32_t limit[5], ent[5];
+      bool valid[5];
+#pragma unroll
+      for (int L = 1; L <= 4; ++L) {
+        limit[L] = (L <= 2) ? C.bound[L] : C.tail[L];
+        const uint32_t q = C.head[L] + (uint32_t)lane;
+        valid[L] = (int32_t)(limit[L] - q) > 0;
+        ent[L] = valid[L] ? __ldcg(P.ring[L] + (q & P.ring_mask)) : 0u;
+      }
+      pre_base = a0 + kmax;
+      pre_n = (pre_base + lane < N) ? P.node_acc[pre_base + lane] : NODE_NONE;
       // (1) the same node twice: cut before the second occurrence (lane 0 never has an earlier twin)
       const uint32_t twins = __match_any_sync(FULL, act0 ? n : (0xF0000000u | (uint32_t)lane));
       const uint32_t dupm = __ballot_sync(FULL, act0 && (twins & lt));
-      if (dupm) k = __ffs(dupm) - 1;
-      uint32_t km = (k == 32) ? FULL : ((1u << k) - 1u);
+      if (dupm) { k = __ffs(dupm) - 1; dbg[DBG_CUT_TWIN]++; }
+      uint32_t km = bits_from(0, k);
       const uint32_t lst = rec.list;
       const uint32_t m0 = __ballot_sync(FULL, lst & 1u), m1 = __ballot_sync(FULL, lst & 2u), m2 = __ballot_sync(FULL, lst & 4u);
       if (m2 & m0 & km) C.err = DEV_ERR_BAD_NODE;                 // a FREE node reached K3
       const uint32_t hitm = lru ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);   // list T1 (LRU) / T1 or T2 (ARC)
+      // hits on entries that were still evictable by this request (below bound): they stop being so
+      const uint32_t me = __ballot_sync(FULL, (lst == L_T1 && (int32_t)(C.bound[L_T1] - rec.pos) > 0) ||
+                                                  (lst == L_T2 && (int32_t)(C.bound[L_T2] - rec.pos) > 0));
+      const long long tw1 = clock64();
+      dbg[DBG_CYC_FETCH] += (unsigned long long)(tw1 - tw0);
 
       if ((hitm & km) == km) {
         // ---- every access of the window is a hit: no counter other than t1/t2 moves, nothing is evicted
@@ -129,43 +229,47 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
         }
         if (lru) C.tail[L_T1] += (uint32_t)k; else C.tail[L_T2] += (uint32_t)k;
         C.t1 -= (int32_t)t1hits; C.t2 += (int32_t)t1hits;
+        C.elig1 -= __popc(me & m0 & km);
+        C.elig2 -= __popc(me & m1 & km);
         C.stat[ST_ACCESSES] += (uint32_t)k;
         C.stat[ST_HIT_T1] += lru ? (uint32_t)k : t1hits;
         C.stat[ST_HIT_T2] += lru ? 0u : (uint32_t)k - t1hits;
         j += k;
         __syncwarp();
+        dbg[DBG_WIN_HIT]++; dbg[DBG_ACC_HIT_WIN] += (unsigned)k;
+        dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw1);
         continue;
       }
 
       // ---- general window: roll the counters forward, fetch the victims, check, apply
-      Roll R = roll_forward(C, c, lru, m0, m1, m2, k, lane);
-      bool act = lane < k;
-      uint32_t srcT1m = __ballot_sync(FULL, act && (R.my_src == 1 || R.my_src == 3));
-      uint32_t srcT2m = __ballot_sync(FULL, act && R.my_src == 2);
-      uint32_t drop1m = __ballot_sync(FULL, act && R.my_drop == L_B1);
-      uint32_t drop2m = __ballot_sync(FULL, act && R.my_drop == L_B2);
-      uint32_t need[5], found[5], q0[5], limit[5], endpos[5];
-      need[0] = 0; need[L_T1] = __popc(srcT1m); need[L_T2] = __popc(srcT2m); need[L_B1] = __popc(drop1m); need[L_B2] = __popc(drop2m);
+      Roll R = roll_forward(C, c, lru, m0, m1, m2, me, k, lane);
+      const long long tw2 = clock64();
+      dbg[DBG_CYC_ROLL] += (unsigned long long)(tw2 - tw1);
+      uint32_t need[5], found[5], q0[5], endpos[5];
+      need[0] = 0; need[L_T1] = __popc(R.s0); need[L_T2] = __popc(R.s1 & ~R.s0); need[L_B1] = __popc(R.d1); need[L_B2] = __popc(R.d2);
 #pragma unroll
-      for (int L = 1; L <= 4; ++L) { found[L] = 0; q0[L] = C.head[L]; limit[L] = (L <= 2) ? C.bound[L] : C.tail[L]; }
+      for (int L = 1; L <= 4; ++L) { found[L] = 0; q0[L] = C.head[L]; }
+      bool first = true;
       for (;;) {
-        bool want[5], valid[5];
-        uint32_t ent[5];
+        bool want[5];
         Node vr[5];
         bool any = false;
 #pragma unroll
         for (int L = 1; L <= 4; ++L) {
           want[L] = found[L] < need[L] && q0[L] != limit[L];
           any |= want[L];
-          const uint32_t q = q0[L] + (uint32_t)lane;
-          valid[L] = want[L] && (int32_t)(limit[L] - q) > 0;
-          ent[L] = valid[L] ? __ldcg(P.ring[L] + (q & P.ring_mask)) : 0u;
+          if (!first) {                       // later rounds: the next 32 ring entries
+            const uint32_t q = q0[L] + (uint32_t)lane;
+            valid[L] = want[L] && (int32_t)(limit[L] - q) > 0;
+            ent[L] = valid[L] ? __ldcg(P.ring[L] + (q & P.ring_mask)) : 0u;
+          }
         }
         if (!any) break;
+        dbg[DBG_SCAN_ROUNDS]++;
 #pragma unroll
         for (int L = 1; L <= 4; ++L) {
           vr[L].list = L_FREE; vr[L].pos = 0; vr[L].block = -1; vr[L].slot = 0;
-          if (valid[L]) vr[L] = ld_node(P.nodes + ent[L]);
+          if (want[L] && valid[L]) vr[L] = ld_node(P.nodes + ent[L]);
         }
 #pragma unroll
         for (int L = 1; L <= 4; ++L) {
@@ -178,6 +282,7 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
           found[L] += (uint32_t)__popc(bal);
           q0[L] = ((int32_t)(limit[L] - (q0[L] + 32u)) > 0) ? q0[L] + 32u : limit[L];
         }
+        first = false;
       }
       __syncwarp();
 #pragma unroll
@@ -186,65 +291,73 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
         if (need[L]) endpos[L] = (found[L] >= need[L]) ? s_vic[L][need[L] - 1].w + 1u : limit[L];
       }
       // (2) an accessed node whose ring entry lies inside a consumed range, or a victim that does not exist
+      bool act = lane < k;
+      uint32_t my_src = ((R.s0 >> lane) & 1u) | (((R.s1 >> lane) & 1u) << 1);
+      uint32_t srcT1m = R.s0, srcT2m = R.s1 & ~R.s0;
       bool bad = false;
       if (act) {
 #pragma unroll
         for (int L = 1; L <= 4; ++L)
           if (lst == (uint32_t)L && need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
-        if ((R.my_src == 1 || R.my_src == 3) && (uint32_t)__popc(srcT1m & lt) >= found[L_T1]) bad = true;
-        if (R.my_src == 2 && (uint32_t)__popc(srcT2m & lt) >= found[L_T2]) bad = true;
-        if (R.my_drop == L_B1 && (uint32_t)__popc(drop1m & lt) >= found[L_B1]) bad = true;
-        if (R.my_drop == L_B2 && (uint32_t)__popc(drop2m & lt) >= found[L_B2]) bad = true;
+        if ((my_src & 1u) && (uint32_t)__popc(srcT1m & lt) >= found[L_T1]) bad = true;
+        if (my_src == 2 && (uint32_t)__popc(srcT2m & lt) >= found[L_T2]) bad = true;
+        if (((R.d1 >> lane) & 1u) && (uint32_t)__popc(R.d1 & lt) >= found[L_B1]) bad = true;
+        if (((R.d2 >> lane) & 1u) && (uint32_t)__popc(R.d2 & lt) >= found[L_B2]) bad = true;
       }
       const uint32_t badm = __ballot_sync(FULL, bad);
+      const long long tw3 = clock64();
+      dbg[DBG_CYC_SCAN] += (unsigned long long)(tw3 - tw2);
       if (badm) {
         k = __ffs(badm) - 1;
+        dbg[DBG_CUT_CONFLICT]++;
         if (k == 0) {                       // the by-the-book routine, run identically by every lane
           serial_access(C, P, a0, o + (nb - 1 - j));
           j += 1;
           __syncwarp();
+          dbg[DBG_WIN_SERIAL]++;
+          dbg[DBG_CYC_SERIAL] += (unsigned long long)(clock64() - tw3);
           continue;
         }
-        km = (1u << k) - 1u;
-        R = roll_forward(C, c, lru, m0, m1, m2, k, lane);
+        km = bits_from(0, k);
+        R = roll_forward(C, c, lru, m0, m1, m2, me, k, lane);
         act = lane < k;
-        srcT1m = __ballot_sync(FULL, act && (R.my_src == 1 || R.my_src == 3));
-        srcT2m = __ballot_sync(FULL, act && R.my_src == 2);
-        drop1m = __ballot_sync(FULL, act && R.my_drop == L_B1);
-        drop2m = __ballot_sync(FULL, act && R.my_drop == L_B2);
-        need[L_T1] = __popc(srcT1m); need[L_T2] = __popc(srcT2m); need[L_B1] = __popc(drop1m); need[L_B2] = __popc(drop2m);
+        my_src = ((R.s0 >> lane) & 1u) | (((R.s1 >> lane) & 1u) << 1);
+        srcT1m = R.s0; srcT2m = R.s1 & ~R.s0;
+        need[L_T1] = __popc(R.s0); need[L_T2] = __popc(srcT2m); need[L_B1] = __popc(R.d1); need[L_B2] = __popc(R.d2);
 #pragma unroll
         for (int L = 1; L <= 4; ++L) endpos[L] = need[L] ? s_vic[L][need[L] - 1].w + 1u : C.head[L];
       }
+      if (R.err) C.err = R.err;
 
-      // ---- apply (lanes < k); ranks come from the ballots
-      const uint32_t ghost1m = __ballot_sync(FULL, act && R.my_src == 1);            // pushes to B1, in access order
+      // ---- apply (lanes < k); ranks come from the decision masks
+      const uint32_t ghost1m = R.s0 & ~R.s1;                                          // pushes to B1, in access order
+      const uint32_t src3m = R.s0 & R.s1;
       const uint32_t pushT1m = lru ? km : (~(m0 | m1 | m2) & km);                     // ABSENT nodes enter T1 (LRU: everything)
       const uint32_t pushT2m = km & ~pushT1m;
       const uint32_t nonhitm = km & ~hitm;
       const uint32_t evictm = srcT1m | srcT2m;
       if (act) {
         const bool is_hit = (hitm >> lane) & 1u;
+        const bool my_d1 = (R.d1 >> lane) & 1u, my_d2 = (R.d2 >> lane) & 1u;
         int32_t blk = rec.block, ev = -1;
         uint32_t dropped = NODE_NONE;
-        if (R.my_src) {
-          const uint32_t Ls = (R.my_src == 2) ? L_T2 : L_T1;
-          const uint4 v = s_vic[Ls][__popc(((R.my_src == 2) ? srcT2m : srcT1m) & lt)];
+        if (my_src) {
+          const uint4 v = (my_src == 2) ? s_vic[L_T2][__popc(srcT2m & lt)] : s_vic[L_T1][__popc(srcT1m & lt)];
           blk = ev = (int32_t)v.y;
-          if (R.my_src == 3) {                      // leaves no ghost: the key leaves the directory in K4
+          if (my_src == 3) {                        // leaves no ghost: the key leaves the directory in K4
             st_node(P.nodes + v.x, L_ABSENT, 0, -1, v.z);
             dropped = v.x;
           } else {
-            const uint32_t G = (R.my_src == 1) ? L_B1 : L_B2;
-            const uint32_t q = ((R.my_src == 1) ? C.tail[L_B1] : C.tail[L_B2]) + (uint32_t)__popc(((R.my_src == 1) ? ghost1m : srcT2m) & lt);
-            ((R.my_src == 1) ? P.ring[L_B1] : P.ring[L_B2])[q & P.ring_mask] = v.x;
+            const uint32_t G = (my_src == 1) ? L_B1 : L_B2;
+            const uint32_t q = (my_src == 1) ? C.tail[L_B1] + (uint32_t)__popc(ghost1m & lt) : C.tail[L_B2] + (uint32_t)__popc(srcT2m & lt);
+            ((my_src == 1) ? P.ring[L_B1] : P.ring[L_B2])[q & P.ring_mask] = v.x;
             st_node(P.nodes + v.x, G, q, -1, v.z);
           }
-        } else if (!is_hit) {
-          blk = R.my_fresh;
+        } else if ((R.fm >> lane) & 1u) {
+          blk = C.next_fresh + __popc(R.fm & lt);
         }
-        if (R.my_drop) {
-          const uint4 d = s_vic[R.my_drop][__popc(((R.my_drop == L_B1) ? drop1m : drop2m) & lt)];
+        if (my_d1 || my_d2) {
+          const uint4 d = my_d1 ? s_vic[L_B1][__popc(R.d1 & lt)] : s_vic[L_B2][__popc(R.d2 & lt)];
           st_node(P.nodes + d.x, L_ABSENT, 0, -1, d.z);
           dropped = d.x;
         }
@@ -263,7 +376,6 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
         if (ev >= 0) P.evict_ids[C.n_evict + (uint32_t)__popc(evictm & lt)] = ev;
       }
       // uniform state
-      const uint32_t n3 = __popc(__ballot_sync(FULL, act && R.my_src == 3));
       C.stat[ST_ACCESSES] += (uint32_t)k;
       C.stat[ST_HIT_T1] += __popc(hitm & km & m0);
       C.stat[ST_HIT_T2] += lru ? 0u : (uint32_t)__popc(hitm & km & m1);
@@ -281,14 +393,23 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
       for (int L = 1; L <= 4; ++L) C.head[L] = endpos[L];
       C.tail[L_T1] += __popc(pushT1m);
       C.tail[L_T2] += __popc(pushT2m);
-      C.tail[L_B1] += need[L_T1] - n3;
+      C.tail[L_B1] += __popc(ghost1m);
       C.tail[L_B2] += need[L_T2];
+      (void)src3m;
       C.t1 = R.t1; C.t2 = R.t2; C.b1 = R.b1; C.b2 = R.b2; C.p = R.p; C.next_fresh = R.nf;
+      C.elig1 = R.e1; C.elig2 = R.e2;
       j += k;
       __syncwarp();
+      dbg[DBG_WIN_GENERAL]++; dbg[DBG_ACC_GENERAL_WIN] += (unsigned)k;
+      dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw3);
     }
   }
-  if (lane == 0) ctx_store(C, P);
+  dbg[DBG_CYC_TOTAL] = (unsigned long long)(clock64() - t_begin);
+  if (lane == 0) {
+    ctx_store(C, P);
+#pragma unroll
+    for (int i = 0; i < DBG_COUNT; ++i) P.state->dbg[i] += dbg[i];
+  }
 }
 
 inline void launch_machine_batched(const StepParams& P, cudaStream_t s) { arc_machine_batched_kernel<<<1, 32, 0, s>>>(P); }

@@ -10,6 +10,7 @@ struct SerialCtx {
   uint32_t head[5], tail[5];   // only ever indexed with compile-time constants, so they live in registers
   uint32_t bound[5];     // victim scans stop here: tail of T1/T2 when the request began (R4), current tail for B1/B2
   int32_t t1, t2, b1, b2, p, next_fresh;
+  int32_t elig1, elig2;  // live entries of T1 / T2 below bound[] = victims still available to the current request (R4, R7)
   uint32_t stat[ST_COUNT];   // per-step deltas (a step has < 2^31 accesses)
   uint32_t err;
   uint32_t n_alloc, n_evict;
@@ -46,12 +47,12 @@ __device__ __forceinline__ int32_t replace_serial(SerialCtx& C, const StepParams
       const uint32_t v = ring_pop_lru<L_T1>(C, P, C.bound[L_T1], &r);
       if (v == NODE_NONE) continue;
       ring_push<L_B1>(C, P, v, -1, r.slot);
-      C.t1--; C.b1++; C.stat[ST_EVICT_T1]++;
+      C.t1--; C.b1++; C.elig1--; C.stat[ST_EVICT_T1]++;
     } else {
       const uint32_t v = ring_pop_lru<L_T2>(C, P, C.bound[L_T2], &r);
       if (v == NODE_NONE) continue;
       ring_push<L_B2>(C, P, v, -1, r.slot);
-      C.t2--; C.b2++; C.stat[ST_EVICT_T2]++;
+      C.t2--; C.b2++; C.elig2--; C.stat[ST_EVICT_T2]++;
     }
     return r.block;
   }
@@ -66,7 +67,7 @@ __device__ __forceinline__ int32_t evict_t1_no_ghost_serial(SerialCtx& C, const 
   if (v == NODE_NONE) { C.err = DEV_ERR_NO_VICTIM; return -1; }
   st_node(P.nodes + v, L_ABSENT, 0, -1, r.slot);
   *dropped = v;
-  C.t1--; C.stat[ST_EVICT_T1]++;
+  C.t1--; C.elig1--; C.stat[ST_EVICT_T1]++;
   return r.block;
 }
 
@@ -86,6 +87,7 @@ __device__ __forceinline__ void ctx_load(SerialCtx& C, const StepParams& P) {
 #pragma unroll
   for (int L = 1; L <= 4; ++L) { C.head[L] = S->head[L]; C.tail[L] = S->tail[L]; C.bound[L] = S->tail[L]; }
   C.t1 = S->t1; C.t2 = S->t2; C.b1 = S->b1; C.b2 = S->b2; C.p = S->p; C.next_fresh = S->next_fresh;
+  C.elig1 = C.t1; C.elig2 = C.t2;
 #pragma unroll
   for (int i = 0; i < ST_COUNT; ++i) C.stat[i] = 0;
   C.err = 0;
@@ -102,6 +104,13 @@ __device__ __forceinline__ void ctx_store(const SerialCtx& C, const StepParams& 
   if (C.err) S->error = C.err;
 }
 
+// Entries pushed from here on belong to the new request: pinned (R4); everything already in T1 / T2 is a possible victim.
+__device__ __forceinline__ void begin_request(SerialCtx& C) {
+  C.bound[L_T1] = C.tail[L_T1];
+  C.bound[L_T2] = C.tail[L_T2];
+  C.elig1 = C.t1; C.elig2 = C.t2;
+}
+
 // One access (R5 for ARC, R10 for LRU) against the live state: access index a (access order), output index out
 // (natural order).  C.bound[T1/T2] must hold the tails recorded when the access's request began (R4).
 __device__ __forceinline__ void serial_access(SerialCtx& C, const StepParams& P, int64_t a, int64_t out) {
@@ -116,6 +125,7 @@ __device__ __forceinline__ void serial_access(SerialCtx& C, const StepParams& P,
   if (P.policy == POLICY_LRU) {             // R10
     if (rec.list == L_T1) {
       cls = CLS_HIT_T1; C.stat[ST_HIT_T1]++;
+      if ((int32_t)(C.bound[L_T1] - rec.pos) > 0) C.elig1--;
       ring_push<L_T1>(C, P, n, blk, rec.slot);
     } else {
       cls = CLS_MISS; C.stat[ST_MISS]++;
@@ -125,8 +135,13 @@ __device__ __forceinline__ void serial_access(SerialCtx& C, const StepParams& P,
       C.t1++;
     }
   } else if (rec.list == L_T1 || rec.list == L_T2) {      // R5 case 1
-    if (rec.list == L_T1) { cls = CLS_HIT_T1; C.stat[ST_HIT_T1]++; C.t1--; C.t2++; }
-    else { cls = CLS_HIT_T2; C.stat[ST_HIT_T2]++; }
+    if (rec.list == L_T1) {
+      cls = CLS_HIT_T1; C.stat[ST_HIT_T1]++; C.t1--; C.t2++;
+      if ((int32_t)(C.bound[L_T1] - rec.pos) > 0) C.elig1--;
+    } else {
+      cls = CLS_HIT_T2; C.stat[ST_HIT_T2]++;
+      if ((int32_t)(C.bound[L_T2] - rec.pos) > 0) C.elig2--;
+    }
     ring_push<L_T2>(C, P, n, blk, rec.slot);
   } else if (rec.list == L_B1) {                          // case 2
     cls = CLS_GHOST_B1; C.stat[ST_GHOST_B1]++;
@@ -173,8 +188,7 @@ __global__ void arc_machine_serial_kernel(StepParams P) {
   ctx_load(C, P);
   for (uint32_t r = 0; r < P.n_req; ++r) {
     const int64_t o = P.blk_off[r], nb = P.blk_off[r + 1] - o;
-    C.bound[L_T1] = C.tail[L_T1];   // entries pushed from here on belong to this request: pinned (R4)
-    C.bound[L_T2] = C.tail[L_T2];
+    begin_request(C);
     for (int64_t j = 0; j < nb; ++j) serial_access(C, P, o + j, o + (nb - 1 - j));   // tail block first (R2)
   }
   ctx_store(C, P);
