@@ -50,6 +50,7 @@ def parse_args():
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--bulk-gib", type=float, default=1.0, help="size of the K1 roofline run in GiB of tokens")
     ap.add_argument("--no-extras", action="store_true", help="skip the breakdown / roofline / hit-rate / cpu legs")
+    ap.add_argument("--only-k1", action="store_true", help="run only the K1 bulk roofline leg (for ncu captures of the hashing kernel)")
     return ap.parse_args()
 
 
@@ -254,6 +255,13 @@ def run_ours(args):
     from paper_2606_21238_b200 import parallel as P
 
     A.load_library()
+    if args.only_k1:
+        peak, peak_src = peaks()
+        nb, nreq_b, mean_ms, best_ms = k1_bulk_roofline(torch, A, args.bulk_gib, torch.cuda.current_stream(), args.seed)
+        achieved = ALGO_BYTES_PER_BLOCK * nb / (mean_ms * 1e-3) / 1e9
+        print(json.dumps({"kernel": "K1 chained block hashing (arc_hash_blocks)", "blocks": nb, "requests": nreq_b, "ms_per_launch": mean_ms,
+                          "best_ms": best_ms, "achieved_GBps": achieved, "peak": peak, "frac": achieved / peak, "peak_source": peak_src}))
+        return
     W_, K = args.warmup, args.steps
     info, steps = build_steps(args.config, W_ + K, P.replica_seed(args.seed, rank))
     acc, tok, req = step_counts(steps)

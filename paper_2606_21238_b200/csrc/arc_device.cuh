@@ -55,7 +55,7 @@ struct DevState {
   uint32_t counts[2];             // n_alloc, n_evict of the current step
   uint32_t error;                 // DEV_ERR_*
   uint32_t tombs;                 // tombstones currently in the table
-  uint32_t pad0;
+  uint32_t k1_ticket;             // K1 work ticket: 0 between steps (K4 resets it)
   unsigned long long stat[ST_COUNT];
   // scratch for ring compaction (old window of the list being compacted)
   uint32_t cmp_head, cmp_tail;
@@ -83,7 +83,6 @@ struct StepParams {
   uint32_t n_access;
   // step scratch (access order: index blk_off[r] + (nb_r - 1 - i))
   unsigned long long* keys_acc;
-  uint8_t* acc_start;             // 1 where a request's first access (its tail block) sits
   uint32_t* node_acc;
   uint32_t* dropped;              // node made ABSENT by access a, or NODE_NONE
   // outputs (natural order: blk_off[r] + i)

@@ -3,6 +3,19 @@
 //   s_i   = s_{i-1} K + g_i,  s_{-1} = S0      (affine => a segmented scan over the blocks of a request)
 //   key_i = mix(s_i), values 0 and 1 bumped by 2
 // The constants below are typed in from the definition; the oracle has its own copy (no shared header).
+//
+// Kernel shape.  HBM-bound: 64 B read + 8 B written per block.  One warp owns one request
+// at a time (requests are handed out through an atomic ticket, so long and short requests balance) and
+// walks it in rounds of 32 blocks = 2 KB of tokens:
+//   * loads: the round's tokens are fetched as 128-bit vectors from the 16-byte-ALIGNED cover of the
+//     round, lane l taking vector 32*it + l (it = 0..3): every load instruction is one fully coalesced
+//     512-byte access whatever the request's alignment; the next round's vectors are issued before the
+//     current round is hashed (register double buffer), streaming through L1/L2 (ld.global.cs);
+//   * a request that starts s tokens past a 16-byte boundary is realigned in registers with s shuffles;
+//   * lane l then holds 4 tokens = words 2q, 2q+1 (q = l % 4) of block 8*it + l/4; the four partial sums
+//     of a block are combined with a transpose-reduce (6 shuffles for the four iterations together),
+//     one more shuffle puts block i in lane i, and a 5-step warp scan with the constants K^(2^d)
+//     evaluates the affine chain; the carry into the next round is lane 31's state.
 #pragma once
 #include "arc_device.cuh"
 
@@ -20,9 +33,10 @@ __host__ __device__ constexpr unsigned long long kpow(unsigned n) {
   return r;
 }
 
-__device__ __forceinline__ unsigned long long hash_word(uint32_t lo, uint32_t hi, unsigned k) {
-  unsigned long long w = (unsigned long long)lo | ((unsigned long long)hi << 32);
-  unsigned long long e = (w + (unsigned long long)(k + 1) * H_M) * H_C1;
+// fold((w + salt) C1) with w = lo | hi << 32; salt = (k+1) M is passed in
+__device__ __forceinline__ unsigned long long hash_word(uint32_t lo, uint32_t hi, unsigned long long salt) {
+  const unsigned long long w = (unsigned long long)lo | ((unsigned long long)hi << 32);
+  const unsigned long long e = (w + salt) * H_C1;
   return e ^ (e >> 32);
 }
 
@@ -33,9 +47,9 @@ __device__ __forceinline__ unsigned long long finalize_key(unsigned long long z)
   return z < 2 ? z + 2 : z;
 }
 
-__device__ __forceinline__ unsigned long long shfl_up64(unsigned long long v, int d) {
-  return __shfl_up_sync(0xFFFFFFFFu, v, d);
-}
+__device__ __forceinline__ unsigned long long shfl64(unsigned long long v, int src) { return __shfl_sync(0xFFFFFFFFu, v, src); }
+__device__ __forceinline__ unsigned long long shfl_xor64(unsigned long long v, int m) { return __shfl_xor_sync(0xFFFFFFFFu, v, m); }
+__device__ __forceinline__ unsigned long long shfl_up64(unsigned long long v, int d) { return __shfl_up_sync(0xFFFFFFFFu, v, d); }
 
 // Inclusive warp scan of the affine chain: on return lane l holds sum_{j<=l} K^(l-j) g_j.
 __device__ __forceinline__ unsigned long long warp_chain_scan(unsigned long long g, int lane) {
@@ -48,8 +62,8 @@ __device__ __forceinline__ unsigned long long warp_chain_scan(unsigned long long
   return s;
 }
 
-// K^(lane+1) without a table: square-and-multiply over the 6 bits of lane+1.
-__device__ __forceinline__ unsigned long long kpow_lane(int e) {
+// K^e for e in 1..32, without a table: square-and-multiply over the 6 bits of e.
+__device__ __forceinline__ unsigned long long kpow_small(int e) {
   unsigned long long r = 1;
   if (e & 1) r *= kpow(1);
   if (e & 2) r *= kpow(2);
@@ -60,49 +74,110 @@ __device__ __forceinline__ unsigned long long kpow_lane(int e) {
   return r;
 }
 
-// v1 kernel: one warp per request, 32 blocks per round, lane l hashes block base+l.
-// ACCESS_ORDER = true writes keys at blk_off[r] + (nb-1-i) (the order K3 consumes, R2) plus the
-// request-start flags; false writes natural order (arc_hash_blocks).
+// The tokens of one round as this lane sees them: vector 32*it + lane of the round's aligned cover (it = 0..3),
+// and vector 128 (x) in lane 0 only (needed when the request is misaligned and the round is full).
+struct RoundVecs {
+  uint4 v[4];
+  uint4 x;
+};
+
+// 128-bit streaming load of tokens [g0, g0 + 4) (absolute token indices, tok + g0 is 16-byte aligned); words outside
+// the valid range [lo, hi) of the caller's buffer are not touched and read as 0.
+__device__ __forceinline__ uint4 ld_tokens4(const uint32_t* __restrict__ tok, int64_t g0, int64_t lo, int64_t hi) {
+  if (g0 >= lo && g0 + 4 <= hi) return __ldcs(reinterpret_cast<const uint4*>(tok + g0));
+  uint4 r = make_uint4(0, 0, 0, 0);
+  if (g0 + 0 >= lo && g0 + 0 < hi) r.x = __ldcs(tok + g0 + 0);
+  if (g0 + 1 >= lo && g0 + 1 < hi) r.y = __ldcs(tok + g0 + 1);
+  if (g0 + 2 >= lo && g0 + 2 < hi) r.z = __ldcs(tok + g0 + 2);
+  if (g0 + 3 >= lo && g0 + 3 < hi) r.w = __ldcs(tok + g0 + 3);
+  return r;
+}
+
+// va = absolute token index of the aligned cover's first word for this round; n_vec = vectors the round needs.
+__device__ __forceinline__ RoundVecs load_round(const uint32_t* __restrict__ tok, int64_t va, int n_vec, int lane, int64_t lo, int64_t hi) {
+  RoundVecs R;
+#pragma unroll
+  for (int it = 0; it < 4; ++it) {
+    const int e = it * 32 + lane;
+    R.v[it] = (e < n_vec) ? ld_tokens4(tok, va + 4 * (int64_t)e, lo, hi) : make_uint4(0, 0, 0, 0);
+  }
+  R.x = (lane == 0 && n_vec > 128) ? ld_tokens4(tok, va + 512, lo, hi) : make_uint4(0, 0, 0, 0);
+  return R;
+}
+
+// word c (0..2) of the vector that FOLLOWS this lane's vector `cur` in the round: lane l+1's cur, and for lane 31
+// lane 0's `nxt` (the same lane-0 register of the next iteration / the 129th vector).
+__device__ __forceinline__ uint32_t next_word(uint32_t cur, uint32_t nxt, int lane) {
+  return __shfl_sync(0xFFFFFFFFu, lane == 0 ? nxt : cur, (lane + 1) & 31);
+}
+
+// ACCESS_ORDER = true writes keys at blk_off[r] + (nb-1-i) (the order K3 consumes, R2); false writes natural
+// order (arc_hash_blocks).  ticket: device counter, 0 at launch, reset by the caller's stream work.
 template <bool ACCESS_ORDER>
-__global__ void __launch_bounds__(256) hash_warp_per_request_kernel(const int32_t* __restrict__ tokens,
-                                                                   const int64_t* __restrict__ offsets,
-                                                                   const int64_t* __restrict__ blk_off, uint32_t n_req,
-                                                                   unsigned long long* __restrict__ keys,
-                                                                   uint8_t* __restrict__ acc_start) {
+__global__ void __launch_bounds__(256) hash_blocks_kernel(const int32_t* __restrict__ tokens, const int64_t* __restrict__ offsets,
+                                                         const int64_t* __restrict__ blk_off, uint32_t n_req,
+                                                         unsigned long long* __restrict__ keys, uint32_t* __restrict__ ticket) {
   const int lane = threadIdx.x & 31;
-  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
-  for (uint32_t r = warp; r < n_req; r += n_warps) {
-    const int64_t o = blk_off[r];
-    const int64_t nb = blk_off[r + 1] - o;
-    const uint32_t* t0 = reinterpret_cast<const uint32_t*>(tokens) + offsets[r];
-    const bool aligned = (reinterpret_cast<uintptr_t>(t0) & 15) == 0;
+  const uint32_t* tok = reinterpret_cast<const uint32_t*>(tokens);
+  const int64_t lo = offsets[0], hi = offsets[n_req];
+  // per-lane constants: this lane hashes words 2q and 2q+1 (q = lane % 4) of its blocks; K^(lane+1) carries the chain in
+  const int q = lane & 3;
+  const unsigned long long salt0 = (unsigned long long)(2 * q + 1) * H_M, salt1 = (unsigned long long)(2 * q + 2) * H_M;
+  const unsigned long long kp = kpow_small(lane + 1);
+  const int owner = 4 * (lane & 7) + (lane >> 3);     // after the transpose-reduce, block i of the round sits in this lane
+  // misalignment of the token buffer itself, in tokens past a 16-byte boundary
+  const int base_mis = (int)((reinterpret_cast<uintptr_t>(tok) >> 2) & 3);
+
+  for (;;) {
+    uint32_t r = 0;
+    if (lane == 0) r = atomicAdd(ticket, 1u);
+    r = __shfl_sync(0xFFFFFFFFu, r, 0);
+    if (r >= n_req) break;
+    const int64_t o = blk_off[r], nb = blk_off[r + 1] - o;
+    if (nb == 0) continue;
+    const int64_t ts = offsets[r];
+    const int s = (int)((base_mis + ts) & 3);          // tokens of the request's start past a 16-byte boundary (same for every round)
     unsigned long long carry = H_S0;
-    for (int64_t base = 0; base < nb; base += 32) {
-      const int64_t i = base + lane;
-      unsigned long long g = 0;
-      if (i < nb) {
-        const uint32_t* t = t0 + i * 16;
-        if (aligned) {
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            uint4 v = __ldg(reinterpret_cast<const uint4*>(t) + q);
-            g += hash_word(v.x, v.y, 2 * q) + hash_word(v.z, v.w, 2 * q + 1);
-          }
-        } else {
-#pragma unroll
-          for (int k = 0; k < 8; ++k) g += hash_word(__ldg(t + 2 * k), __ldg(t + 2 * k + 1), k);
-        }
+    int cnt = (int)min((int64_t)32, nb);
+    RoundVecs nxt = load_round(tok, ts - s, (16 * cnt + s + 3) >> 2, lane, lo, hi);
+    for (int64_t rb = 0; rb < nb; rb += 32) {
+      const RoundVecs cur = nxt;
+      const int cnt_cur = cnt;
+      if (rb + 32 < nb) {
+        cnt = (int)min((int64_t)32, nb - rb - 32);
+        nxt = load_round(tok, ts - s + 16 * (rb + 32), (16 * cnt + s + 3) >> 2, lane, lo, hi);
       }
-      const unsigned long long s = warp_chain_scan(g, lane) + kpow_lane(lane + 1) * carry;
-      if (i < nb) {
-        const int64_t dst = ACCESS_ORDER ? (o + (nb - 1 - i)) : (o + i);
-        keys[dst] = finalize_key(s);
-        if (ACCESS_ORDER) acc_start[dst] = (i == nb - 1) ? 1 : 0;
+      // realign and hash this lane's two words of blocks 8*it + lane/4
+      unsigned long long part[4];
+#pragma unroll
+      for (int it = 0; it < 4; ++it) {
+        const uint4 v = cur.v[it];
+        const uint4 w = (it < 3) ? cur.v[it + 1] : cur.x;     // lane 0's copy is what lane 31 needs
+        uint32_t a, b, c2, d;
+        if (s == 0) { a = v.x; b = v.y; c2 = v.z; d = v.w; }
+        else if (s == 1) { a = v.y; b = v.z; c2 = v.w; d = next_word(v.x, w.x, lane); }
+        else if (s == 2) { a = v.z; b = v.w; c2 = next_word(v.x, w.x, lane); d = next_word(v.y, w.y, lane); }
+        else { a = v.w; b = next_word(v.x, w.x, lane); c2 = next_word(v.y, w.y, lane); d = next_word(v.z, w.z, lane); }
+        part[it] = hash_word(a, b, salt0) + hash_word(c2, d, salt1);
       }
-      carry = __shfl_sync(0xFFFFFFFFu, s, 31);
+      // transpose-reduce over the 4 lanes of a block: afterwards lane l holds g of block (l/4) + 8*(l%4)
+      const bool b0 = lane & 1, b1 = lane & 2;
+      const unsigned long long r0 = shfl_xor64(b0 ? part[0] : part[1], 1), r1 = shfl_xor64(b0 ? part[2] : part[3], 1);
+      const unsigned long long pa = (b0 ? part[1] : part[0]) + r0, pb = (b0 ? part[3] : part[2]) + r1;
+      const unsigned long long g_own = (b1 ? pb : pa) + shfl_xor64(b1 ? pa : pb, 2);
+      unsigned long long g = shfl64(g_own, owner);      // lane i <- block i
+      if (lane >= cnt_cur) g = 0;
+      const unsigned long long st = warp_chain_scan(g, lane) + kp * carry;
+      if (lane < cnt_cur) {
+        const int64_t i = rb + lane;
+        keys[ACCESS_ORDER ? (o + (nb - 1 - i)) : (o + i)] = finalize_key(st);
+      }
+      carry = shfl64(st, 31);
     }
   }
 }
+
+// the last thing on the stream after a hashing launch: the ticket returns to 0 for the next launch
+__global__ void reset_ticket_kernel(uint32_t* ticket) { *ticket = 0; }
 
 }  // namespace arc

@@ -70,7 +70,6 @@ struct arc_cache {
   // per-step buffers
   int64_t* d_offsets = nullptr;   // [2 * (req_cap + 1)] : token offsets, then blk_off
   unsigned long long* d_keys = nullptr;
-  uint8_t* d_acc_start = nullptr;
   uint32_t* d_node_acc = nullptr;
   uint32_t* d_dropped = nullptr;
   int32_t* d_prefix_len = nullptr;
@@ -128,7 +127,7 @@ StepParams make_params(arc_cache* h) {
   for (int L = 1; L <= 4; ++L) P.ring[L] = h->d_ring[L];
   P.ring_mask = h->ring_cap - 1;
   P.offsets = h->d_offsets; P.blk_off = h->d_offsets + (h->req_cap + 1);
-  P.keys_acc = h->d_keys; P.acc_start = h->d_acc_start; P.node_acc = h->d_node_acc; P.dropped = h->d_dropped;
+  P.keys_acc = h->d_keys; P.node_acc = h->d_node_acc; P.dropped = h->d_dropped;
   P.prefix_len = h->d_prefix_len; P.cls = h->d_cls; P.block_id = h->d_block_id; P.evicted_id = h->d_evicted_id;
   P.p_after = h->d_p_after; P.alloc_ids = h->d_alloc_ids; P.evict_ids = h->d_evict_ids;
   P.capacity = (int32_t)h->c; P.policy = h->policy; P.block_size = h->B;
@@ -164,7 +163,7 @@ int launch_compact(arc_cache* h, cudaStream_t s, int L, uint32_t src_cap, uint32
 }
 
 void free_step_buffers(arc_cache* h) {
-  dfree(h->d_offsets); dfree(h->d_keys); dfree(h->d_acc_start); dfree(h->d_node_acc); dfree(h->d_dropped);
+  dfree(h->d_offsets); dfree(h->d_keys); dfree(h->d_node_acc); dfree(h->d_dropped);
   dfree(h->d_prefix_len); dfree(h->d_cls); dfree(h->d_block_id); dfree(h->d_evicted_id); dfree(h->d_p_after);
   dfree(h->d_alloc_ids); dfree(h->d_evict_ids);
   if (h->h_stage) cudaFreeHost(h->h_stage);
@@ -178,7 +177,6 @@ int alloc_step_buffers(arc_cache* h, uint32_t req_cap, uint64_t n_cap) {
   h->req_cap = req_cap; h->n_cap = n_cap;
   CUDA_TRY(h, dalloc(&h->d_offsets, 2 * ((size_t)req_cap + 1)));
   CUDA_TRY(h, dalloc(&h->d_keys, n_cap));
-  CUDA_TRY(h, dalloc(&h->d_acc_start, n_cap));
   CUDA_TRY(h, dalloc(&h->d_node_acc, n_cap));
   CUDA_TRY(h, dalloc(&h->d_dropped, n_cap));
   CUDA_TRY(h, dalloc(&h->d_prefix_len, req_cap));
@@ -300,14 +298,15 @@ int validate_offsets(arc_cache* h, const int64_t* off, uint32_t n_req, uint32_t 
   return ARC_OK;
 }
 
-void launch_hash(const int32_t* d_tokens, const int64_t* d_offsets, const int64_t* d_blk_off, uint32_t n_req, uint64_t N,
-                 unsigned long long* d_keys, uint8_t* d_acc_start, bool access_order, cudaStream_t s) {
-  (void)N;
-  const uint32_t blocks = grid_for(n_req, 8, 148 * 16);
+// K1 grid: persistent warps that take requests through the ticket; enough CTAs to fill the 148 SMs, never more
+// warps than requests.
+void launch_hash(const int32_t* d_tokens, const int64_t* d_offsets, const int64_t* d_blk_off, uint32_t n_req,
+                 unsigned long long* d_keys, uint32_t* d_ticket, bool access_order, cudaStream_t s) {
+  const uint32_t blocks = grid_for(n_req, 8, 148 * 6);
   if (access_order)
-    hash_warp_per_request_kernel<true><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_acc_start);
+    hash_blocks_kernel<true><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket);
   else
-    hash_warp_per_request_kernel<false><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, nullptr);
+    hash_blocks_kernel<false><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket);
 }
 
 }  // namespace
@@ -385,7 +384,7 @@ int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, ui
   StepParams P = make_params(h);
   P.tokens = d_tokens; P.n_req = n_req; P.n_access = (uint32_t)N;
   if (N) {
-    launch_hash(d_tokens, P.offsets, P.blk_off, n_req, N, P.keys_acc, P.acc_start, true, s);               // K1
+    launch_hash(d_tokens, P.offsets, P.blk_off, n_req, P.keys_acc, &h->d_state->k1_ticket, true, s);               // K1
     if (h->profiling) cudaEventRecord(h->ev[2], s);
     probe_reserve_kernel<<<grid_for(N, 32, 148 * 8), 256, 0, s>>>(P);                                     // K2
     resolve_nodes_kernel<<<grid_for(N, 256, 148 * 8), 256, 0, s>>>(P);
@@ -523,6 +522,7 @@ int arc_hash_blocks(const int32_t* d_tokens, const int64_t* h_offsets, uint32_t 
   static int64_t* d_off = nullptr;
   static int64_t* h_off = nullptr;
   static uint32_t cap = 0;
+  static uint32_t* d_ticket = nullptr;
   static cudaEvent_t copied = nullptr;
   std::lock_guard<std::mutex> lock(mu);
   if (n_req + 1 > cap) {
@@ -537,6 +537,10 @@ int arc_hash_blocks(const int32_t* d_tokens, const int64_t* h_offsets, uint32_t 
     }
   }
   if (!copied) cudaEventCreateWithFlags(&copied, cudaEventDisableTiming);
+  if (!d_ticket) {
+    if (cudaMalloc((void**)&d_ticket, sizeof(uint32_t)) != cudaSuccess) { d_ticket = nullptr; return fail(nullptr, ARC_ERR_OOM, "scratch allocation failed"); }
+    cudaMemset(d_ticket, 0, sizeof(uint32_t));
+  }
   cudaEventSynchronize(copied);
   uint64_t N = 0;
   int rc = validate_offsets(nullptr, h_offsets, n_req, block_size, 0, h_off + cap, &N);
@@ -547,8 +551,9 @@ int arc_hash_blocks(const int32_t* d_tokens, const int64_t* h_offsets, uint32_t 
   if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "offset copy: %s", cudaGetErrorString(e));
   cudaEventRecord(copied, s);
   if (N) {
-    launch_hash(d_tokens, d_off, d_off + cap, n_req, N, (unsigned long long*)d_keys_out, nullptr, false, s);
-    g_hash_launches += 1;
+    launch_hash(d_tokens, d_off, d_off + cap, n_req, (unsigned long long*)d_keys_out, d_ticket, false, s);
+    reset_ticket_kernel<<<1, 1, 0, s>>>(d_ticket);
+    g_hash_launches += 2;
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "hash launch: %s", cudaGetErrorString(e));
   }
