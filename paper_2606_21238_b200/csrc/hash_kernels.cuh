@@ -5,8 +5,8 @@
 // The constants below are typed in from the definition; the oracle has its own copy (no shared header).
 //
 // Kernel shape.  HBM-bound: 64 B read + 8 B written per block.  One warp owns one request
-// at a time (requests are handed out through an atomic ticket, so long and short requests balance) and
-// walks it in rounds of 32 blocks = 2 KB of tokens:
+// at a time; requests are handed out through an atomic ticket, longest length class first, so long and
+// short requests balance.  A warp walks its request in rounds of 32 blocks = 2 KB of tokens:
 //   * loads: the round's tokens are fetched as 128-bit vectors from the 16-byte-ALIGNED cover of the
 //     round, lane l taking vector 32*it + l (it = 0..3): every load instruction is one fully coalesced
 //     512-byte access whatever the request's alignment; the next round's vectors are issued before the
@@ -82,9 +82,9 @@ struct RoundVecs {
 };
 
 // 128-bit streaming load of tokens [g0, g0 + 4) (absolute token indices, tok + g0 is 16-byte aligned); words outside
-// the valid range [lo, hi) of the caller's buffer are not touched and read as 0.
-__device__ __forceinline__ uint4 ld_tokens4(const uint32_t* __restrict__ tok, int64_t g0, int64_t lo, int64_t hi) {
-  if (g0 >= lo && g0 + 4 <= hi) return __ldcs(reinterpret_cast<const uint4*>(tok + g0));
+// the valid range [lo, hi) of the caller's buffer are not touched and read as 0.  Only rounds at the very edge of the
+// caller's buffer come here.
+__device__ __noinline__ uint4 ld_tokens4_guarded(const uint32_t* __restrict__ tok, int64_t g0, int64_t lo, int64_t hi) {
   uint4 r = make_uint4(0, 0, 0, 0);
   if (g0 + 0 >= lo && g0 + 0 < hi) r.x = __ldcs(tok + g0 + 0);
   if (g0 + 1 >= lo && g0 + 1 < hi) r.y = __ldcs(tok + g0 + 1);
@@ -93,15 +93,22 @@ __device__ __forceinline__ uint4 ld_tokens4(const uint32_t* __restrict__ tok, in
   return r;
 }
 
-// va = absolute token index of the aligned cover's first word for this round; n_vec = vectors the round needs.
+// va = absolute token index of the aligned cover's first word for this round; n_vec = vectors the round needs (0..129).
 __device__ __forceinline__ RoundVecs load_round(const uint32_t* __restrict__ tok, int64_t va, int n_vec, int lane, int64_t lo, int64_t hi) {
   RoundVecs R;
+  if (va >= lo && va + 4 * (int64_t)n_vec <= hi) {            // the whole cover is inside the caller's buffer (warp-uniform)
+    const uint4* p = reinterpret_cast<const uint4*>(tok + va) + lane;
 #pragma unroll
-  for (int it = 0; it < 4; ++it) {
-    const int e = it * 32 + lane;
-    R.v[it] = (e < n_vec) ? ld_tokens4(tok, va + 4 * (int64_t)e, lo, hi) : make_uint4(0, 0, 0, 0);
+    for (int it = 0; it < 4; ++it) R.v[it] = (it * 32 + lane < n_vec) ? __ldcs(p + it * 32) : make_uint4(0, 0, 0, 0);
+    R.x = (lane == 0 && n_vec > 128) ? __ldcs(p + 128) : make_uint4(0, 0, 0, 0);
+  } else {
+#pragma unroll
+    for (int it = 0; it < 4; ++it) {
+      const int e = it * 32 + lane;
+      R.v[it] = (e < n_vec) ? ld_tokens4_guarded(tok, va + 4 * (int64_t)e, lo, hi) : make_uint4(0, 0, 0, 0);
+    }
+    R.x = (lane == 0 && n_vec > 128) ? ld_tokens4_guarded(tok, va + 512, lo, hi) : make_uint4(0, 0, 0, 0);
   }
-  R.x = (lane == 0 && n_vec > 128) ? ld_tokens4(tok, va + 512, lo, hi) : make_uint4(0, 0, 0, 0);
   return R;
 }
 
@@ -111,68 +118,103 @@ __device__ __forceinline__ uint32_t next_word(uint32_t cur, uint32_t nxt, int la
   return __shfl_sync(0xFFFFFFFFu, lane == 0 ? nxt : cur, (lane + 1) & 31);
 }
 
+struct LaneConsts {
+  unsigned long long salt0, salt1;   // (k+1) M C1 for this lane's two words k = 2q, 2q+1 (the salt is folded into the multiply-add)
+  unsigned long long kp;             // K^(lane+1)
+  int owner;                         // after the transpose-reduce, block i of the round sits in lane `owner` of lane i
+};
+
+// Local chain states of one round: lane i returns sum_{j<=i} K^(i-j) g_j over the round's blocks (no carry-in);
+// lanes >= cnt contribute g = 0.  s = request misalignment in tokens.
+__device__ __forceinline__ unsigned long long round_local_scan(const RoundVecs& cur, int s, int cnt, int lane, const LaneConsts& LC) {
+  unsigned long long part[4];
+#pragma unroll
+  for (int it = 0; it < 4; ++it) {
+    const uint4 v = cur.v[it];
+    const uint4 w = (it < 3) ? cur.v[it + 1] : cur.x;     // lane 0's copy is what lane 31 needs
+    uint32_t a, b, c2, d;
+    if (s == 0) { a = v.x; b = v.y; c2 = v.z; d = v.w; }
+    else if (s == 1) { a = v.y; b = v.z; c2 = v.w; d = next_word(v.x, w.x, lane); }
+    else if (s == 2) { a = v.z; b = v.w; c2 = next_word(v.x, w.x, lane); d = next_word(v.y, w.y, lane); }
+    else { a = v.w; b = next_word(v.x, w.x, lane); c2 = next_word(v.y, w.y, lane); d = next_word(v.z, w.z, lane); }
+    // fold((w + (k+1) M) C1) = fold(w C1 + (k+1) M C1)
+    const unsigned long long e0 = ((unsigned long long)a | ((unsigned long long)b << 32)) * H_C1 + LC.salt0;
+    const unsigned long long e1 = ((unsigned long long)c2 | ((unsigned long long)d << 32)) * H_C1 + LC.salt1;
+    part[it] = (e0 ^ (e0 >> 32)) + (e1 ^ (e1 >> 32));
+  }
+  // transpose-reduce over the 4 lanes of a block: afterwards lane l holds g of block (l/4) + 8*(l%4)
+  const bool b0 = lane & 1, b1 = lane & 2;
+  const unsigned long long r0 = shfl_xor64(b0 ? part[0] : part[1], 1), r1 = shfl_xor64(b0 ? part[2] : part[3], 1);
+  const unsigned long long pa = (b0 ? part[1] : part[0]) + r0, pb = (b0 ? part[3] : part[2]) + r1;
+  const unsigned long long g_own = (b1 ? pb : pa) + shfl_xor64(b1 ? pa : pb, 2);
+  unsigned long long g = shfl64(g_own, LC.owner);      // lane i <- block i
+  if (lane >= cnt) g = 0;
+  return warp_chain_scan(g, lane);
+}
+
+// Length classes for the ticket passes: requests of at least K1_CLASS_MIN[c] blocks are started in pass c, so the
+// longest chains start first and the short requests fill the tail of the launch (longest-processing-time-first).
+constexpr int K1_PASSES = 4;
+__device__ __forceinline__ int k1_class(int64_t nb) { return nb >= 1024 ? 0 : nb >= 384 ? 1 : nb >= 128 ? 2 : 3; }
+
 // ACCESS_ORDER = true writes keys at blk_off[r] + (nb-1-i) (the order K3 consumes, R2); false writes natural
-// order (arc_hash_blocks).  ticket: device counter, 0 at launch, reset by the caller's stream work.
+// order (arc_hash_blocks).  ticket: device counter, 0 at launch, reset by the caller's stream work; it runs over
+// K1_PASSES * n_req values: ticket t is request t % n_req in pass t / n_req.
 template <bool ACCESS_ORDER>
 __global__ void __launch_bounds__(256) hash_blocks_kernel(const int32_t* __restrict__ tokens, const int64_t* __restrict__ offsets,
                                                          const int64_t* __restrict__ blk_off, uint32_t n_req,
-                                                         unsigned long long* __restrict__ keys, uint32_t* __restrict__ ticket) {
+                                                         unsigned long long* __restrict__ keys, uint32_t* __restrict__ ticket, uint32_t batch) {
   const int lane = threadIdx.x & 31;
   const uint32_t* tok = reinterpret_cast<const uint32_t*>(tokens);
   const int64_t lo = offsets[0], hi = offsets[n_req];
-  // per-lane constants: this lane hashes words 2q and 2q+1 (q = lane % 4) of its blocks; K^(lane+1) carries the chain in
+  LaneConsts LC;
   const int q = lane & 3;
-  const unsigned long long salt0 = (unsigned long long)(2 * q + 1) * H_M, salt1 = (unsigned long long)(2 * q + 2) * H_M;
-  const unsigned long long kp = kpow_small(lane + 1);
-  const int owner = 4 * (lane & 7) + (lane >> 3);     // after the transpose-reduce, block i of the round sits in this lane
-  // misalignment of the token buffer itself, in tokens past a 16-byte boundary
-  const int base_mis = (int)((reinterpret_cast<uintptr_t>(tok) >> 2) & 3);
+  LC.salt0 = (unsigned long long)(2 * q + 1) * H_M * H_C1;
+  LC.salt1 = (unsigned long long)(2 * q + 2) * H_M * H_C1;
+  LC.kp = kpow_small(lane + 1);
+  LC.owner = 4 * (lane & 7) + (lane >> 3);
+  const int base_mis = (int)((reinterpret_cast<uintptr_t>(tok) >> 2) & 3);   // tokens of the buffer start past a 16-byte boundary
+  const unsigned long long total = (unsigned long long)K1_PASSES * n_req;
 
   for (;;) {
-    uint32_t r = 0;
-    if (lane == 0) r = atomicAdd(ticket, 1u);
-    r = __shfl_sync(0xFFFFFFFFu, r, 0);
-    if (r >= n_req) break;
-    const int64_t o = blk_off[r], nb = blk_off[r + 1] - o;
-    if (nb == 0) continue;
-    const int64_t ts = offsets[r];
-    const int s = (int)((base_mis + ts) & 3);          // tokens of the request's start past a 16-byte boundary (same for every round)
-    unsigned long long carry = H_S0;
-    int cnt = (int)min((int64_t)32, nb);
-    RoundVecs nxt = load_round(tok, ts - s, (16 * cnt + s + 3) >> 2, lane, lo, hi);
-    for (int64_t rb = 0; rb < nb; rb += 32) {
-      const RoundVecs cur = nxt;
-      const int cnt_cur = cnt;
-      if (rb + 32 < nb) {
-        cnt = (int)min((int64_t)32, nb - rb - 32);
-        nxt = load_round(tok, ts - s + 16 * (rb + 32), (16 * cnt + s + 3) >> 2, lane, lo, hi);
+    // `batch` (<= 32) tickets per atomic: lane l < batch examines ticket t0 + l, the warp then hashes the ones that belong to the pass
+    uint32_t t0 = 0;
+    if (lane == 0) t0 = atomicAdd(ticket, batch);
+    t0 = __shfl_sync(0xFFFFFFFFu, t0, 0);
+    if (t0 >= total) break;
+    const unsigned long long t = (unsigned long long)t0 + lane;
+    bool mine = false;
+    uint32_t my_r = 0;
+    if (t < total && (uint32_t)lane < batch) {
+      my_r = (uint32_t)(t % n_req);
+      const int64_t nb = blk_off[my_r + 1] - blk_off[my_r];
+      mine = nb > 0 && k1_class(nb) == (int)(t / n_req);
+    }
+    uint32_t todo = __ballot_sync(0xFFFFFFFFu, mine);
+    while (todo) {
+      const int src = __ffs(todo) - 1;
+      todo &= todo - 1;
+      const uint32_t r = __shfl_sync(0xFFFFFFFFu, my_r, src);
+      const int64_t o = blk_off[r], nb = blk_off[r + 1] - o;
+      const int64_t ts = offsets[r];
+      const int s = (int)((base_mis + ts) & 3);          // tokens of the request's start past a 16-byte boundary (same for every round)
+      unsigned long long carry = H_S0;
+      int cnt = (int)min((int64_t)32, nb);
+      RoundVecs nxt = load_round(tok, ts - s, (16 * cnt + s + 3) >> 2, lane, lo, hi);
+      for (int64_t rb = 0; rb < nb; rb += 32) {
+        const RoundVecs cur = nxt;
+        const int cnt_cur = cnt;
+        if (rb + 32 < nb) {
+          cnt = (int)min((int64_t)32, nb - rb - 32);
+          nxt = load_round(tok, ts - s + 16 * (rb + 32), (16 * cnt + s + 3) >> 2, lane, lo, hi);
+        }
+        const unsigned long long st = round_local_scan(cur, s, cnt_cur, lane, LC) + LC.kp * carry;
+        if (lane < cnt_cur) {
+          const int64_t i = rb + lane;
+          keys[ACCESS_ORDER ? (o + (nb - 1 - i)) : (o + i)] = finalize_key(st);
+        }
+        carry = shfl64(st, 31);
       }
-      // realign and hash this lane's two words of blocks 8*it + lane/4
-      unsigned long long part[4];
-#pragma unroll
-      for (int it = 0; it < 4; ++it) {
-        const uint4 v = cur.v[it];
-        const uint4 w = (it < 3) ? cur.v[it + 1] : cur.x;     // lane 0's copy is what lane 31 needs
-        uint32_t a, b, c2, d;
-        if (s == 0) { a = v.x; b = v.y; c2 = v.z; d = v.w; }
-        else if (s == 1) { a = v.y; b = v.z; c2 = v.w; d = next_word(v.x, w.x, lane); }
-        else if (s == 2) { a = v.z; b = v.w; c2 = next_word(v.x, w.x, lane); d = next_word(v.y, w.y, lane); }
-        else { a = v.w; b = next_word(v.x, w.x, lane); c2 = next_word(v.y, w.y, lane); d = next_word(v.z, w.z, lane); }
-        part[it] = hash_word(a, b, salt0) + hash_word(c2, d, salt1);
-      }
-      // transpose-reduce over the 4 lanes of a block: afterwards lane l holds g of block (l/4) + 8*(l%4)
-      const bool b0 = lane & 1, b1 = lane & 2;
-      const unsigned long long r0 = shfl_xor64(b0 ? part[0] : part[1], 1), r1 = shfl_xor64(b0 ? part[2] : part[3], 1);
-      const unsigned long long pa = (b0 ? part[1] : part[0]) + r0, pb = (b0 ? part[3] : part[2]) + r1;
-      const unsigned long long g_own = (b1 ? pb : pa) + shfl_xor64(b1 ? pa : pb, 2);
-      unsigned long long g = shfl64(g_own, owner);      // lane i <- block i
-      if (lane >= cnt_cur) g = 0;
-      const unsigned long long st = warp_chain_scan(g, lane) + kp * carry;
-      if (lane < cnt_cur) {
-        const int64_t i = rb + lane;
-        keys[ACCESS_ORDER ? (o + (nb - 1 - i)) : (o + i)] = finalize_key(st);
-      }
-      carry = shfl64(st, 31);
     }
   }
 }

@@ -5,6 +5,7 @@
 #include <cstdarg>
 #include <cstddef>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -303,10 +304,11 @@ int validate_offsets(arc_cache* h, const int64_t* off, uint32_t n_req, uint32_t 
 void launch_hash(const int32_t* d_tokens, const int64_t* d_offsets, const int64_t* d_blk_off, uint32_t n_req,
                  unsigned long long* d_keys, uint32_t* d_ticket, bool access_order, cudaStream_t s) {
   const uint32_t blocks = grid_for(n_req, 8, 148 * 6);
+  static uint32_t batch = getenv("ARC_K1_BATCH") ? (uint32_t)atoi(getenv("ARC_K1_BATCH")) : 2u;
   if (access_order)
-    hash_blocks_kernel<true><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket);
+    hash_blocks_kernel<true><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, batch);
   else
-    hash_blocks_kernel<false><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket);
+    hash_blocks_kernel<false><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, batch);
 }
 
 }  // namespace
