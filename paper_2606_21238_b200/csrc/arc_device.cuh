@@ -4,7 +4,7 @@
 //   Node[node_cap]      16 B records {list, pos, block, slot}; node ids are stable for the life of a key
 //   node_key[node_cap]  the 64-bit key of each node (only needed by rebuilds and debug dumps)
 //   Slot[table_slots]   open-addressing table, 16 B slots {key, node}, buckets of 8 slots = one 128 B line
-//   ring[L][ring_cap]   one lazy FIFO of node ids per list L in {T1, T2, B1, B2}: an entry at absolute
+//   ring[L][ring_cap]   one lazy FIFO of 8 B entries {node id, block id} per list L in {T1, T2, B1, B2}: an entry at absolute
 //                       position q is *live* iff nodes[id].list == L && nodes[id].pos == q.  Every list
 //                       insertion is at the MRU end (tail++), every LRU-end removal scans from head and
 //                       skips stale entries; a hit leaves its old entry behind as stale.  Entries pushed
@@ -26,6 +26,15 @@ constexpr uint32_t BUCKET_SLOTS = 8;             // 8 x 16 B = one 128 B line
 
 enum : int { CLS_MISS = 0, CLS_HIT_T1 = 1, CLS_HIT_T2 = 2, CLS_GHOST_B1 = 3, CLS_GHOST_B2 = 4 };
 enum : int { POLICY_ARC = 0, POLICY_LRU = 1 };
+
+// Ring entry: low word = node id (RING_TOMB once the node has left that position by a hit / ghost hit), high word = the
+// block id the node held when it was pushed.  Inside [head, tail) an entry is live iff it is not a tombstone; the node
+// record (list, pos) stays the authoritative copy, used by the maintenance kernels and the by-the-book routine.
+typedef unsigned long long RingEnt;
+constexpr uint32_t RING_TOMB = 0xFFFFFFFFu;
+__host__ __device__ __forceinline__ RingEnt ring_ent(uint32_t node, int32_t block) { return (RingEnt)node | ((RingEnt)(uint32_t)block << 32); }
+__host__ __device__ __forceinline__ uint32_t ent_node(RingEnt e) { return (uint32_t)e; }
+__host__ __device__ __forceinline__ int32_t ent_block(RingEnt e) { return (int32_t)(uint32_t)(e >> 32); }
 
 struct __align__(16) Node {
   uint32_t list;   // L_*
@@ -73,7 +82,7 @@ struct StepParams {
   uint32_t* free_stack;
   Slot* table;
   uint32_t bucket_mask;           // (table_slots / 8) - 1
-  uint32_t* ring[5];
+  RingEnt* ring[5];
   uint32_t ring_mask;
   // step inputs
   const int32_t* tokens;
@@ -108,6 +117,11 @@ __device__ __forceinline__ Node ld_node(const Node* p) {
 }
 __device__ __forceinline__ void st_node(Node* p, uint32_t list, uint32_t pos, int32_t block, uint32_t slot) {
   __stcg(reinterpret_cast<uint4*>(p), make_uint4(list, pos, (uint32_t)block, slot));
+}
+// same, leaving the slot field as it is (for nodes whose record was never read: victims taken from a ring entry)
+__device__ __forceinline__ void st_node_keep_slot(Node* p, uint32_t list, uint32_t pos, int32_t block) {
+  __stcg(reinterpret_cast<uint2*>(p), make_uint2(list, pos));
+  __stcg(reinterpret_cast<int*>(p) + 2, block);
 }
 
 }  // namespace arc

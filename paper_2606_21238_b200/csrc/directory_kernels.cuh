@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(256) rebuild_table_kernel(DevState* st, Node* 
 // [old_tail, old_tail + live) of the *other* buffer: new positions never overlap old ones, so a stale
 // entry can never be mistaken for a live one while CTAs run concurrently.
 constexpr int CMP_THREADS = 1024;
-__global__ void __launch_bounds__(CMP_THREADS) ring_count_kernel(DevState* st, const Node* nodes, const uint32_t* ring,
+__global__ void __launch_bounds__(CMP_THREADS) ring_count_kernel(DevState* st, const Node* nodes, const RingEnt* ring,
                                                                 uint32_t ring_mask, uint32_t L, uint32_t* block_counts) {
   const uint32_t head = st->head[L], tail = st->tail[L];
   const uint32_t window = tail - head;
@@ -178,9 +178,11 @@ __global__ void __launch_bounds__(CMP_THREADS) ring_count_kernel(DevState* st, c
   bool live = false;
   if (off < window) {
     const uint32_t q = head + off;
-    const uint32_t n = ring[q & ring_mask];
-    const Node r = ld_node(nodes + n);
-    live = (r.list == L && r.pos == q);
+    const uint32_t n = ent_node(ring[q & ring_mask]);
+    if (n != RING_TOMB) {
+      const Node r = ld_node(nodes + n);
+      live = (r.list == L && r.pos == q);
+    }
   }
   const int cnt = __syncthreads_count(live);
   if (threadIdx.x == 0) {
@@ -188,8 +190,8 @@ __global__ void __launch_bounds__(CMP_THREADS) ring_count_kernel(DevState* st, c
     if (blockIdx.x == 0) { st->cmp_head = head; st->cmp_tail = tail; }
   }
 }
-__global__ void __launch_bounds__(CMP_THREADS) ring_scatter_kernel(DevState* st, Node* nodes, const uint32_t* ring,
-                                                                  uint32_t ring_mask, uint32_t* ring_dst, uint32_t dst_mask,
+__global__ void __launch_bounds__(CMP_THREADS) ring_scatter_kernel(DevState* st, Node* nodes, const RingEnt* ring,
+                                                                  uint32_t ring_mask, RingEnt* ring_dst, uint32_t dst_mask,
                                                                   uint32_t L, const uint32_t* block_counts) {
   __shared__ uint32_t s_warp[32];
   __shared__ uint32_t s_base, s_total;
@@ -223,11 +225,15 @@ __global__ void __launch_bounds__(CMP_THREADS) ring_scatter_kernel(DevState* st,
   const uint32_t off = blockIdx.x * CMP_THREADS + threadIdx.x;
   bool live = false;
   uint32_t n = 0;
+  int32_t blk = -1;
   if (off < window) {
     const uint32_t q = head + off;
-    n = ring[q & ring_mask];
-    const Node r = ld_node(nodes + n);
-    live = (r.list == L && r.pos == q);
+    n = ent_node(ring[q & ring_mask]);
+    if (n != RING_TOMB) {
+      const Node r = ld_node(nodes + n);
+      live = (r.list == L && r.pos == q);
+      blk = r.block;
+    }
   }
   const uint32_t bal = __ballot_sync(0xFFFFFFFFu, live);
   __syncthreads();
@@ -237,7 +243,7 @@ __global__ void __launch_bounds__(CMP_THREADS) ring_scatter_kernel(DevState* st,
   for (uint32_t w = 0; w < warp; ++w) before += s_warp[w];
   if (live) {
     const uint32_t q_new = tail + s_base + before + __popc(bal & ((1u << lane) - 1));
-    ring_dst[q_new & dst_mask] = n;
+    ring_dst[q_new & dst_mask] = ring_ent(n, blk);
     nodes[n].pos = q_new;
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) { st->head[L] = tail; st->tail[L] = tail + s_total; }
@@ -245,7 +251,7 @@ __global__ void __launch_bounds__(CMP_THREADS) ring_scatter_kernel(DevState* st,
 
 // Debug: write list L (LRU -> MRU) as keys and block ids.  Single CTA, sequential chunks.
 __global__ void __launch_bounds__(CMP_THREADS) dump_list_kernel(const DevState* st, const Node* nodes,
-                                                               const unsigned long long* node_key, const uint32_t* ring,
+                                                               const unsigned long long* node_key, const RingEnt* ring,
                                                                uint32_t ring_mask, uint32_t L, unsigned long long* keys_out,
                                                                int32_t* blocks_out, unsigned long long cap,
                                                                unsigned long long* n_out) {
@@ -262,9 +268,11 @@ __global__ void __launch_bounds__(CMP_THREADS) dump_list_kernel(const DevState* 
     Node r;
     r.block = -1;
     if (off < window) {
-      n = ring[(head + off) & ring_mask];
-      r = ld_node(nodes + n);
-      live = (r.list == L && r.pos == head + off);
+      n = ent_node(ring[(head + off) & ring_mask]);
+      if (n != RING_TOMB) {
+        r = ld_node(nodes + n);
+        live = (r.list == L && r.pos == head + off);
+      }
     }
     const uint32_t bal = __ballot_sync(0xFFFFFFFFu, live);
     if (lane == 0) s_warp[warp] = __popc(bal);

@@ -65,8 +65,8 @@ struct arc_cache {
   unsigned long long* d_node_key = nullptr;
   uint32_t* d_free_stack = nullptr;
   Slot* d_table = nullptr;
-  uint32_t* d_ring[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-  uint32_t* d_ring_alt[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  RingEnt* d_ring[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  RingEnt* d_ring_alt[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   uint32_t* d_block_counts = nullptr;
   // per-step buffers
   int64_t* d_offsets = nullptr;   // [2 * (req_cap + 1)] : token offsets, then blk_off

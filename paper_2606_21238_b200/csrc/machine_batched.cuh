@@ -185,15 +185,15 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
       Node rec;
       rec.list = L_FREE; rec.pos = 0; rec.block = -1; rec.slot = 0;
       if (act0) rec = ld_node(P.nodes + n);
-      // the first 32 ring entries from every list head travel with the node records (used only by general windows)
-      uint32_t limit[5], ent[5];
-      bool valid[5];
+      // the first 64 ring entries from every list head travel with the node records (used only by general windows):
+      // lane l holds positions qa + 2l and qa + 2l + 1 of each list, qa = head rounded down to even (16-byte aligned load)
+      uint32_t limit[5];
+      uint4 ent[5];
 #pragma unroll
       for (int L = 1; L <= 4; ++L) {
         limit[L] = (L <= 2) ? C.bound[L] : C.tail[L];
-        const uint32_t q = C.head[L] + (uint32_t)lane;
-        valid[L] = (int32_t)(limit[L] - q) > 0;
-        ent[L] = valid[L] ? __ldcg(P.ring[L] + (q & P.ring_mask)) : 0u;
+        const uint32_t qA = (C.head[L] & ~1u) + 2u * (uint32_t)lane;
+        ent[L] = __ldcg(reinterpret_cast<const uint4*>(P.ring[L] + (qA & P.ring_mask)));
       }
       pre_base = a0 + kmax;
       pre_n = (pre_base + lane < N) ? P.node_acc[pre_base + lane] : NODE_NONE;
@@ -218,7 +218,8 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
         const uint32_t Lp = lru ? L_T1 : L_T2;
         if (lane < k) {
           const uint32_t q = (lru ? C.tail[L_T1] : C.tail[L_T2]) + (uint32_t)lane;
-          (lru ? P.ring[L_T1] : P.ring[L_T2])[q & P.ring_mask] = n;
+          ring_tomb(P, lst, rec.pos);
+          __stcg((lru ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, rec.block));
           st_node(P.nodes + n, Lp, q, rec.block, rec.slot);
           const int64_t out = o + (nb - 1 - (j + lane));
           P.cls[out] = (uint8_t)lst;                               // L_T1 == CLS_HIT_T1, L_T2 == CLS_HIT_T2
@@ -248,39 +249,34 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
       uint32_t need[5], found[5], q0[5], endpos[5];
       need[0] = 0; need[L_T1] = __popc(R.s0); need[L_T2] = __popc(R.s1 & ~R.s0); need[L_B1] = __popc(R.d1); need[L_B2] = __popc(R.d2);
 #pragma unroll
-      for (int L = 1; L <= 4; ++L) { found[L] = 0; q0[L] = C.head[L]; }
+      for (int L = 1; L <= 4; ++L) { found[L] = 0; q0[L] = C.head[L] & ~1u; }
       bool first = true;
       for (;;) {
         bool want[5];
-        Node vr[5];
         bool any = false;
 #pragma unroll
         for (int L = 1; L <= 4; ++L) {
-          want[L] = found[L] < need[L] && q0[L] != limit[L];
+          want[L] = found[L] < need[L] && (int32_t)(limit[L] - q0[L]) > 0;
           any |= want[L];
-          if (!first) {                       // later rounds: the next 32 ring entries
-            const uint32_t q = q0[L] + (uint32_t)lane;
-            valid[L] = want[L] && (int32_t)(limit[L] - q) > 0;
-            ent[L] = valid[L] ? __ldcg(P.ring[L] + (q & P.ring_mask)) : 0u;
-          }
+          if (!first && want[L])               // later rounds: the next 64 ring entries
+            ent[L] = __ldcg(reinterpret_cast<const uint4*>(P.ring[L] + ((q0[L] + 2u * (uint32_t)lane) & P.ring_mask)));
         }
         if (!any) break;
         dbg[DBG_SCAN_ROUNDS]++;
 #pragma unroll
         for (int L = 1; L <= 4; ++L) {
-          vr[L].list = L_FREE; vr[L].pos = 0; vr[L].block = -1; vr[L].slot = 0;
-          if (want[L] && valid[L]) vr[L] = ld_node(P.nodes + ent[L]);
-        }
-#pragma unroll
-        for (int L = 1; L <= 4; ++L) {
           if (!want[L]) continue;                                   // warp-uniform
-          const uint32_t q = q0[L] + (uint32_t)lane;
-          const bool live = valid[L] && vr[L].list == (uint32_t)L && vr[L].pos == q;
-          const uint32_t bal = __ballot_sync(FULL, live);
-          const uint32_t rank = found[L] + (uint32_t)__popc(bal & lt);
-          if (live && rank < 32u) s_vic[L][rank] = make_uint4(ent[L], (uint32_t)vr[L].block, vr[L].slot, q);
-          found[L] += (uint32_t)__popc(bal);
-          q0[L] = ((int32_t)(limit[L] - (q0[L] + 32u)) > 0) ? q0[L] + 32u : limit[L];
+          const uint32_t qA = q0[L] + 2u * (uint32_t)lane, qB = qA + 1u;
+          // live = inside [head, limit) and not a tombstone (entries leave a ring only by head consumption or a tombstone)
+          const bool liveA = (int32_t)(qA - C.head[L]) >= 0 && (int32_t)(limit[L] - qA) > 0 && ent[L].x != RING_TOMB;
+          const bool liveB = (int32_t)(qB - C.head[L]) >= 0 && (int32_t)(limit[L] - qB) > 0 && ent[L].z != RING_TOMB;
+          const uint32_t balA = __ballot_sync(FULL, liveA), balB = __ballot_sync(FULL, liveB);
+          const uint32_t rankA = found[L] + (uint32_t)__popc(balA & lt) + (uint32_t)__popc(balB & lt);
+          const uint32_t rankB = rankA + (liveA ? 1u : 0u);
+          if (liveA && rankA < 32u) s_vic[L][rankA] = make_uint4(ent[L].x, ent[L].y, 0u, qA);
+          if (liveB && rankB < 32u) s_vic[L][rankB] = make_uint4(ent[L].z, ent[L].w, 0u, qB);
+          found[L] += (uint32_t)__popc(balA) + (uint32_t)__popc(balB);
+          q0[L] += 64u;
         }
         first = false;
       }
@@ -345,26 +341,27 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
           const uint4 v = (my_src == 2) ? s_vic[L_T2][__popc(srcT2m & lt)] : s_vic[L_T1][__popc(srcT1m & lt)];
           blk = ev = (int32_t)v.y;
           if (my_src == 3) {                        // leaves no ghost: the key leaves the directory in K4
-            st_node(P.nodes + v.x, L_ABSENT, 0, -1, v.z);
+            st_node_keep_slot(P.nodes + v.x, L_ABSENT, 0, -1);
             dropped = v.x;
           } else {
             const uint32_t G = (my_src == 1) ? L_B1 : L_B2;
             const uint32_t q = (my_src == 1) ? C.tail[L_B1] + (uint32_t)__popc(ghost1m & lt) : C.tail[L_B2] + (uint32_t)__popc(srcT2m & lt);
-            ((my_src == 1) ? P.ring[L_B1] : P.ring[L_B2])[q & P.ring_mask] = v.x;
-            st_node(P.nodes + v.x, G, q, -1, v.z);
+            __stcg(((my_src == 1) ? P.ring[L_B1] : P.ring[L_B2]) + (q & P.ring_mask), ring_ent(v.x, -1));
+            st_node_keep_slot(P.nodes + v.x, G, q, -1);
           }
         } else if ((R.fm >> lane) & 1u) {
           blk = C.next_fresh + __popc(R.fm & lt);
         }
         if (my_d1 || my_d2) {
           const uint4 d = my_d1 ? s_vic[L_B1][__popc(R.d1 & lt)] : s_vic[L_B2][__popc(R.d2 & lt)];
-          st_node(P.nodes + d.x, L_ABSENT, 0, -1, d.z);
+          st_node_keep_slot(P.nodes + d.x, L_ABSENT, 0, -1);
           dropped = d.x;
         }
         const bool toT1 = (pushT1m >> lane) & 1u;
         const uint32_t Lp = toT1 ? L_T1 : L_T2;
         const uint32_t q = (toT1 ? C.tail[L_T1] : C.tail[L_T2]) + (uint32_t)__popc((toT1 ? pushT1m : pushT2m) & lt);
-        (toT1 ? P.ring[L_T1] : P.ring[L_T2])[q & P.ring_mask] = n;
+        if (lst >= L_T1 && lst <= L_B2) ring_tomb(P, lst, rec.pos);     // the node leaves its old position
+        __stcg((toT1 ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, blk));
         st_node(P.nodes + n, Lp, q, blk, rec.slot);
         const int64_t out = o + (nb - 1 - (j + lane));
         P.cls[out] = (uint8_t)lst;                    // ABSENT -> MISS(0), T1 -> 1, T2 -> 2, B1 -> 3, B2 -> 4

@@ -19,7 +19,7 @@ struct SerialCtx {
 template <uint32_t L>
 __device__ __forceinline__ void ring_push(SerialCtx& C, const StepParams& P, uint32_t n, int32_t block, uint32_t slot) {
   const uint32_t q = C.tail[L]++;
-  P.ring[L][q & P.ring_mask] = n;
+  __stcg(P.ring[L] + (q & P.ring_mask), ring_ent(n, block));
   st_node(P.nodes + n, L, q, block, slot);
 }
 
@@ -28,9 +28,11 @@ template <uint32_t L>
 __device__ __forceinline__ uint32_t ring_pop_lru(SerialCtx& C, const StepParams& P, uint32_t bound, Node* rec_out) {
   uint32_t q = C.head[L];
   while (q != bound) {
-    const uint32_t n = __ldcg(P.ring[L] + (q & P.ring_mask));
-    const Node r = ld_node(P.nodes + n);
-    if (r.list == L && r.pos == q) { C.head[L] = q + 1; *rec_out = r; return n; }
+    const uint32_t n = ent_node(__ldcg(P.ring[L] + (q & P.ring_mask)));
+    if (n != RING_TOMB) {
+      const Node r = ld_node(P.nodes + n);
+      if (r.list == L && r.pos == q) { C.head[L] = q + 1; *rec_out = r; return n; }
+    }
     ++q;
   }
   C.head[L] = bound;
@@ -111,6 +113,12 @@ __device__ __forceinline__ void begin_request(SerialCtx& C) {
   C.elig1 = C.t1; C.elig2 = C.t2;
 }
 
+// The node leaves ring position (list, pos) by a hit or a ghost hit: its old entry becomes a tombstone.
+__device__ __forceinline__ void ring_tomb(const StepParams& P, uint32_t list, uint32_t pos) {
+  RingEnt* r = (list == L_T1) ? P.ring[L_T1] : (list == L_T2) ? P.ring[L_T2] : (list == L_B1) ? P.ring[L_B1] : P.ring[L_B2];
+  __stcg(r + (pos & P.ring_mask), ring_ent(RING_TOMB, -1));
+}
+
 // One access (R5 for ARC, R10 for LRU) against the live state: access index a (access order), output index out
 // (natural order).  C.bound[T1/T2] must hold the tails recorded when the access's request began (R4).
 __device__ __forceinline__ void serial_access(SerialCtx& C, const StepParams& P, int64_t a, int64_t out) {
@@ -122,6 +130,7 @@ __device__ __forceinline__ void serial_access(SerialCtx& C, const StepParams& P,
   int32_t blk = rec.block, ev = -1;
   uint32_t dropped = NODE_NONE;
   C.stat[ST_ACCESSES]++;
+  if (rec.list >= L_T1 && rec.list <= L_B2) ring_tomb(P, rec.list, rec.pos);   // every class but MISS moves the node
   if (P.policy == POLICY_LRU) {             // R10
     if (rec.list == L_T1) {
       cls = CLS_HIT_T1; C.stat[ST_HIT_T1]++;
