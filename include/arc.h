@@ -150,8 +150,9 @@ int arc_last_kernel_times(arc_cache *h, arc_kernel_times *out);
  * are counted in a process-wide counter returned when h == NULL). */
 uint64_t arc_launch_count(const arc_cache *h);
 
-/* Selects the K3 implementation: 0 = batched warp-cooperative machine (default), 1 = single-thread
- * serial walk (correctness reference on the device; same results, much slower). */
+/* Selects the K3 implementation: 0 = four-warp machine with 128-access windows (default), 1 = single-thread
+ * serial walk (correctness reference on the device; same results, much slower), 2 = one-warp machine with
+ * 32-access windows. */
 int arc_set_machine(arc_cache *h, int which);
 
 /* K3 diagnostics, cumulative since create/reset: out[0..n) (HOST) receives, in this order, the number of

@@ -18,6 +18,7 @@
 #include "hash_kernels.cuh"
 #include "machine_batched.cuh"
 #include "machine_serial.cuh"
+#include "machine_wide.cuh"
 
 using namespace arc;
 
@@ -54,7 +55,7 @@ struct arc_cache {
   uint64_t c = 0;
   uint32_t B = 16;
   int policy = 0;
-  int machine = 0;            // 0 batched, 1 serial
+  int machine = 0;            // 0 wide (4 warps), 1 serial, 2 one-warp batched
   // capacities
   uint64_t n_cap = 0;         // max full blocks per step the buffers are sized for
   uint32_t req_cap = 0;
@@ -397,8 +398,10 @@ int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, ui
   if (h->profiling) cudaEventRecord(h->ev[3], s);
   if (h->machine == 1) {
     arc_machine_serial_kernel<<<1, 32, 0, s>>>(P);                                                       // K3 (serial)
+  } else if (h->machine == 2) {
+    launch_machine_batched(P, s);                                                                        // K3 (one warp, 32-wide windows)
   } else {
-    launch_machine_batched(P, s);                                                                        // K3 (batched)
+    launch_machine_wide(P, s);                                                                           // K3 (four warps, 128-wide windows)
   }
   if (h->profiling) cudaEventRecord(h->ev[4], s);
   finalize_kernel<<<grid_for(std::max<uint64_t>(N, (uint64_t)n_req * 32), 256, 148 * 8), 256, 0, s>>>(P);  // K4
@@ -585,7 +588,7 @@ int arc_last_kernel_times(arc_cache* h, arc_kernel_times* out) {
 uint64_t arc_launch_count(const arc_cache* h) { return h ? h->launches : g_hash_launches; }
 
 int arc_set_machine(arc_cache* h, int which) {
-  if (!h || (which != 0 && which != 1)) return ARC_ERR_INVALID_ARG;
+  if (!h || which < 0 || which > 2) return ARC_ERR_INVALID_ARG;
   h->machine = which;
   return ARC_OK;
 }

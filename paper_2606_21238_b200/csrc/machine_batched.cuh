@@ -48,11 +48,18 @@ __device__ __forceinline__ void roll_replace(Roll& R, bool inb2, int i) {
 
 // The counter recurrence of R5-R7 / R10 over the first k accesses of the window.  (m0, m1, m2) = the node lists,
 // bit-sliced; me = the access is a hit on an entry that was still evictable (below bound).  Uniform across lanes.
-__device__ __forceinline__ Roll roll_forward(const SerialCtx& C, int32_t c, bool lru, uint32_t m0, uint32_t m1, uint32_t m2,
-                                             uint32_t me, int k, int lane) {
+__device__ __forceinline__ Roll roll_init(const SerialCtx& C) {
   Roll R;
   R.t1 = C.t1; R.t2 = C.t2; R.b1 = C.b1; R.b2 = C.b2; R.p = C.p; R.nf = C.next_fresh; R.e1 = C.elig1; R.e2 = C.elig2;
   R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = C.p; R.err = 0;
+  return R;
+}
+
+// Rolls k (<= 32) accesses from the state in R; the decision masks of these accesses replace those in R.  lane = this
+// thread's index among the k accesses (my_p is captured for it), or >= 32 when the thread owns none of them.
+__device__ __forceinline__ void roll_chunk(Roll& R, int32_t c, bool lru, uint32_t m0, uint32_t m1, uint32_t m2,
+                                           uint32_t me, int k, int lane) {
+  R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = R.p;
   const uint32_t km = bits_from(0, k);
   int i = 0;
   while (i < k) {
@@ -144,6 +151,12 @@ __device__ __forceinline__ Roll roll_forward(const SerialCtx& C, int32_t c, bool
     }
     i += n;
   }
+}
+
+__device__ __forceinline__ Roll roll_forward(const SerialCtx& C, int32_t c, bool lru, uint32_t m0, uint32_t m1, uint32_t m2,
+                                             uint32_t me, int k, int lane) {
+  Roll R = roll_init(C);
+  roll_chunk(R, c, lru, m0, m1, m2, me, k, lane);
   return R;
 }
 

@@ -1,0 +1,406 @@
+// K3, wide form: one CTA of 4 warps consumes the step's accesses in the fixed order R2, a window of up to 128
+// accesses at a time.  Same equivalence argument as machine_batched.cuh; what changes is who does what:
+//   * thread g = 32 w + lane owns access g of the window: it fetches the node record, checks the window's cut
+//     conditions for its access, and applies its access;
+//   * the counter recurrence (roll_chunk, 32 accesses at a time) is run redundantly and identically by all four
+//     warps on the class masks exchanged through shared memory, so no decision is ever broadcast;
+//   * warp w scans the LRU end of list w + 1 (T1, T2, B1, B2): 128 self-validating ring entries per round;
+//   * latencies (node fetch, ring fetch, barriers) are paid once per 128 accesses instead of once per 32.
+// The same node twice in a window (possible inside one request only through a 64-bit key collision) is found
+// exactly with a 512-slot shared-memory hash set and cuts the window, as in the 32-wide machine.
+#pragma once
+#include "machine_batched.cuh"
+
+namespace arc {
+
+constexpr int WIDE_WARPS = 4;
+constexpr int WIDE_W = 32 * WIDE_WARPS;      // accesses per window
+constexpr int WIDE_SET = 512;                // slots of the twin-detection hash set
+
+struct WideShared {
+  uint32_t m[4][WIDE_WARPS];                 // m0, m1, m2, me per chunk
+  uint32_t bad[WIDE_WARPS];
+  uint32_t twin[WIDE_WARPS];
+  uint32_t found[5], endpos[5];
+  uint32_t set_id[WIDE_SET], set_min[WIDE_SET];
+  uint4 vic[5][WIDE_W];                      // per list: entries found from the LRU end {node, block, -, position}
+  SerialCtx ctx;                             // the machine state after a by-the-book access done by warp 0
+};
+
+// sum of popcounts of the chunk masks below chunk w, plus the bits below `lane` in chunk w
+__device__ __forceinline__ uint32_t wide_rank(const uint32_t (&mask)[WIDE_WARPS], int w, uint32_t lt) {
+  uint32_t r = 0;
+#pragma unroll
+  for (int u = 0; u < WIDE_WARPS; ++u) r += (u < w) ? (uint32_t)__popc(mask[u]) : (u == w ? (uint32_t)__popc(mask[u] & lt) : 0u);
+  return r;
+}
+__device__ __forceinline__ uint32_t wide_count(const uint32_t (&mask)[WIDE_WARPS]) {
+  uint32_t r = 0;
+#pragma unroll
+  for (int u = 0; u < WIDE_WARPS; ++u) r += (uint32_t)__popc(mask[u]);
+  return r;
+}
+
+__device__ __forceinline__ uint32_t wide_pick(const uint32_t (&mask)[WIDE_WARPS], int w) {
+  uint32_t r = mask[0];
+#pragma unroll
+  for (int u = 1; u < WIDE_WARPS; ++u) r = (u == w) ? mask[u] : r;
+  return r;
+}
+
+struct WideDecisions {
+  uint32_t s0[WIDE_WARPS], s1[WIDE_WARPS], d1[WIDE_WARPS], d2[WIDE_WARPS], fm[WIDE_WARPS];
+  int32_t my_p;
+  Roll R;                                    // state after the window
+};
+
+// The recurrence over the first k accesses of the window, chunk by chunk (every warp computes the same thing).
+__device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, int32_t c, bool lru, const WideShared& S, int k,
+                                          int warp, int lane) {
+  D.R = roll_init(C);
+  D.my_p = C.p;
+#pragma unroll
+  for (int u = 0; u < WIDE_WARPS; ++u) {
+    const int ku = min(32, max(0, k - 32 * u));
+    D.s0[u] = D.s1[u] = D.d1[u] = D.d2[u] = D.fm[u] = 0;
+    if (ku > 0) {
+      roll_chunk(D.R, c, lru, S.m[0][u], S.m[1][u], S.m[2][u], S.m[3][u], ku, (u == warp) ? lane : 64);
+      D.s0[u] = D.R.s0; D.s1[u] = D.R.s1; D.d1[u] = D.R.d1; D.d2[u] = D.R.d2; D.fm[u] = D.R.fm;
+      if (u == warp) D.my_p = D.R.my_p;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(StepParams P) {
+  __shared__ WideShared S;
+  __shared__ uint32_t s_any_twin;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
+  const bool lru = (P.policy == POLICY_LRU);
+  const int32_t c = P.capacity;
+  const int64_t N = (int64_t)P.n_access;
+  SerialCtx C;            // identical in every thread
+  ctx_load(C, P);
+  for (int i = tid; i < WIDE_SET; i += WIDE_W) { S.set_id[i] = 0xFFFFFFFFu; S.set_min[i] = 0xFFFFFFFFu; }
+  if (tid == 0) s_any_twin = 0;
+  __syncthreads();
+  unsigned long long dbg[DBG_COUNT];
+#pragma unroll
+  for (int i = 0; i < DBG_COUNT; ++i) dbg[i] = 0;
+  const long long t_begin = clock64();
+  const uint32_t myL = (uint32_t)warp + 1u;                 // the list this warp scans
+  RingEnt* const my_ring = P.ring[warp + 1];
+
+  // node ids are prefetched one window ahead: pre_n = node_acc[pre_base + tid]
+  int64_t pre_base = 0;
+  uint32_t pre_n = (tid < N) ? P.node_acc[tid] : NODE_NONE;
+
+  int64_t my_off = 0, my_off1 = 0;
+  for (uint32_t r = 0; r < P.n_req; ++r) {
+    if ((r & 31u) == 0) {      // block offsets of the next 32 requests, one per lane (every warp keeps its own copy)
+      const uint32_t rr = min(r + (uint32_t)lane, P.n_req - 1);
+      my_off = P.blk_off[rr]; my_off1 = P.blk_off[rr + 1];
+    }
+    const int64_t o = __shfl_sync(FULL, my_off, r & 31), nb = __shfl_sync(FULL, my_off1, r & 31) - o;
+    begin_request(C);
+    int64_t j = 0;
+    while (j < nb) {
+      const int kmax = (int)min((int64_t)WIDE_W, nb - j);
+      int k = kmax;
+      const int64_t a0 = o + j;
+      const bool act0 = tid < k;
+      const long long tw0 = clock64();
+      uint32_t n = pre_n;
+      if (pre_base != a0) n = (a0 + tid < N) ? P.node_acc[a0 + tid] : NODE_NONE;     // the last window was cut short
+      Node rec;
+      rec.list = L_FREE; rec.pos = 0; rec.block = -1; rec.slot = 0;
+      if (act0) rec = ld_node(P.nodes + n);
+      // this warp's list: the first 128 ring entries from the head travel with the node records; lane l holds
+      // positions qa + 4l .. qa + 4l + 3, qa = head rounded down to a multiple of 4 (two 16-byte loads)
+      const uint32_t head_my = (myL == L_T1) ? C.head[L_T1] : (myL == L_T2) ? C.head[L_T2] : (myL == L_B1) ? C.head[L_B1] : C.head[L_B2];
+      const uint32_t limit_my = (myL == L_T1) ? C.bound[L_T1] : (myL == L_T2) ? C.bound[L_T2] : (myL == L_B1) ? C.tail[L_B1] : C.tail[L_B2];
+      uint32_t q0 = head_my & ~3u;
+      uint4 e0 = __ldcg(reinterpret_cast<const uint4*>(my_ring + ((q0 + 4u * (uint32_t)lane) & P.ring_mask)));
+      uint4 e1 = __ldcg(reinterpret_cast<const uint4*>(my_ring + ((q0 + 4u * (uint32_t)lane + 2u) & P.ring_mask)));
+      pre_base = a0 + kmax;
+      pre_n = (pre_base + tid < N) ? P.node_acc[pre_base + tid] : NODE_NONE;
+
+      // (1) the same node twice in the window: exact detection with a shared-memory hash set
+      uint32_t slot = 0xFFFFFFFFu;
+      if (act0) {
+        uint32_t h = (n * 2654435761u) >> 23;                        // 9 bits
+        for (;;) {
+          const uint32_t old = atomicCAS(&S.set_id[h], 0xFFFFFFFFu, n);
+          if (old == 0xFFFFFFFFu) break;
+          if (old == n) { s_any_twin = 1; break; }
+          h = (h + 1) & (WIDE_SET - 1);
+        }
+        slot = h;
+        atomicMin(&S.set_min[slot], (uint32_t)tid);
+      }
+      const uint32_t lst = rec.list;
+      {
+        const uint32_t b0 = __ballot_sync(FULL, lst & 1u), b1 = __ballot_sync(FULL, lst & 2u), b2 = __ballot_sync(FULL, lst & 4u);
+        // hits on entries that were still evictable by this request (below bound): they stop being so
+        const uint32_t be = __ballot_sync(FULL, (lst == L_T1 && (int32_t)(C.bound[L_T1] - rec.pos) > 0) ||
+                                                    (lst == L_T2 && (int32_t)(C.bound[L_T2] - rec.pos) > 0));
+        if (lane == 0) { S.m[0][warp] = b0; S.m[1][warp] = b1; S.m[2][warp] = b2; S.m[3][warp] = be; }
+      }
+      __syncthreads();                                               // (B1) class masks and the hash set are complete
+      if (s_any_twin) {                                              // CTA-uniform, next to never taken
+        const bool later = act0 && S.set_min[slot] < (uint32_t)tid;
+        const uint32_t tb = __ballot_sync(FULL, later);
+        if (lane == 0) S.twin[warp] = tb;
+        __syncthreads();
+        int first = k;
+#pragma unroll
+        for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.twin[u]) first = 32 * u + __ffs(S.twin[u]) - 1;
+        if (first < k) { k = first; dbg[DBG_CUT_TWIN]++; }
+        __syncthreads();
+        if (tid == 0) s_any_twin = 0;
+      }
+      uint32_t M0[WIDE_WARPS], M1[WIDE_WARPS], M2[WIDE_WARPS], ME[WIDE_WARPS], KM[WIDE_WARPS], HIT[WIDE_WARPS];
+      bool all_hit = true;
+      uint32_t badnode = 0;
+#pragma unroll
+      for (int u = 0; u < WIDE_WARPS; ++u) {
+        M0[u] = S.m[0][u]; M1[u] = S.m[1][u]; M2[u] = S.m[2][u]; ME[u] = S.m[3][u];
+        KM[u] = bits_from(0, min(32, max(0, k - 32 * u)));
+        HIT[u] = (lru ? (M0[u] & ~M1[u] & ~M2[u]) : ((M0[u] ^ M1[u]) & ~M2[u])) & KM[u];
+        all_hit = all_hit && (HIT[u] == KM[u]);
+        badnode |= M2[u] & M0[u] & KM[u];
+      }
+      if (badnode) C.err = DEV_ERR_BAD_NODE;                         // a FREE node reached K3
+      const long long tw1 = clock64();
+      dbg[DBG_CYC_FETCH] += (unsigned long long)(tw1 - tw0);
+
+      if (all_hit) {
+        // ---- every access of the window is a hit: no counter other than t1/t2 moves, nothing is evicted
+        if (tid < k) {
+          const uint32_t q = (lru ? C.tail[L_T1] : C.tail[L_T2]) + (uint32_t)tid;
+          ring_tomb(P, lst, rec.pos);
+          __stcg((lru ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, rec.block));
+          st_node(P.nodes + n, lru ? L_T1 : L_T2, q, rec.block, rec.slot);
+          const int64_t out = o + (nb - 1 - (j + tid));
+          P.cls[out] = (uint8_t)lst;                               // L_T1 == CLS_HIT_T1, L_T2 == CLS_HIT_T2
+          P.block_id[out] = rec.block;
+          P.evicted_id[out] = -1;
+          P.p_after[out] = C.p;
+          P.dropped[a0 + tid] = NODE_NONE;
+        }
+        uint32_t t1hits = 0, e1d = 0, e2d = 0;
+#pragma unroll
+        for (int u = 0; u < WIDE_WARPS; ++u) {
+          t1hits += (uint32_t)__popc(M0[u] & KM[u]);
+          e1d += (uint32_t)__popc(ME[u] & M0[u] & KM[u]);
+          e2d += (uint32_t)__popc(ME[u] & M1[u] & KM[u]);
+        }
+        if (lru) { C.tail[L_T1] += (uint32_t)k; C.stat[ST_HIT_T1] += (uint32_t)k; }
+        else { C.tail[L_T2] += (uint32_t)k; C.t1 -= (int32_t)t1hits; C.t2 += (int32_t)t1hits; C.stat[ST_HIT_T1] += t1hits; C.stat[ST_HIT_T2] += (uint32_t)k - t1hits; }
+        C.elig1 -= (int32_t)e1d; C.elig2 -= (int32_t)e2d;
+        C.stat[ST_ACCESSES] += (uint32_t)k;
+        if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
+        j += k;
+        dbg[DBG_WIN_HIT]++; dbg[DBG_ACC_HIT_WIN] += (unsigned)k;
+        __syncthreads();
+        dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw1);
+        continue;
+      }
+
+      // ---- general window: roll the counters forward (every warp, identically), scan the lists (one warp each)
+      WideDecisions D;
+      wide_roll(D, C, c, lru, S, k, warp, lane);
+      const long long tw2 = clock64();
+      dbg[DBG_CYC_ROLL] += (unsigned long long)(tw2 - tw1);
+      uint32_t S2[WIDE_WARPS];                                     // evictions from T2
+#pragma unroll
+      for (int u = 0; u < WIDE_WARPS; ++u) S2[u] = D.s1[u] & ~D.s0[u];
+      uint32_t need[5];
+      need[0] = 0; need[L_T1] = wide_count(D.s0); need[L_T2] = wide_count(S2); need[L_B1] = wide_count(D.d1); need[L_B2] = wide_count(D.d2);
+      {
+        const uint32_t my_need = (myL == L_T1) ? need[L_T1] : (myL == L_T2) ? need[L_T2] : (myL == L_B1) ? need[L_B1] : need[L_B2];
+        uint32_t found = 0;
+        bool first = true;
+        while (found < my_need && (int32_t)(limit_my - q0) > 0) {
+          if (!first) {
+            e0 = __ldcg(reinterpret_cast<const uint4*>(my_ring + ((q0 + 4u * (uint32_t)lane) & P.ring_mask)));
+            e1 = __ldcg(reinterpret_cast<const uint4*>(my_ring + ((q0 + 4u * (uint32_t)lane + 2u) & P.ring_mask)));
+          }
+          if (warp == 0) dbg[DBG_SCAN_ROUNDS]++;
+          const uint32_t qA = q0 + 4u * (uint32_t)lane;
+          // live = inside [head, limit) and not a tombstone
+          const bool l0 = (int32_t)(qA - head_my) >= 0 && (int32_t)(limit_my - qA) > 0 && e0.x != RING_TOMB;
+          const bool l1 = (int32_t)(qA + 1u - head_my) >= 0 && (int32_t)(limit_my - qA - 1u) > 0 && e0.z != RING_TOMB;
+          const bool l2 = (int32_t)(qA + 2u - head_my) >= 0 && (int32_t)(limit_my - qA - 2u) > 0 && e1.x != RING_TOMB;
+          const bool l3 = (int32_t)(qA + 3u - head_my) >= 0 && (int32_t)(limit_my - qA - 3u) > 0 && e1.z != RING_TOMB;
+          const uint32_t c0 = __ballot_sync(FULL, l0), c1 = __ballot_sync(FULL, l1), c2 = __ballot_sync(FULL, l2), c3 = __ballot_sync(FULL, l3);
+          uint32_t rk = found + (uint32_t)(__popc(c0 & lt) + __popc(c1 & lt) + __popc(c2 & lt) + __popc(c3 & lt));
+          if (l0) { if (rk < (uint32_t)WIDE_W) S.vic[myL][rk] = make_uint4(e0.x, e0.y, 0u, qA); ++rk; }
+          if (l1) { if (rk < (uint32_t)WIDE_W) S.vic[myL][rk] = make_uint4(e0.z, e0.w, 0u, qA + 1u); ++rk; }
+          if (l2) { if (rk < (uint32_t)WIDE_W) S.vic[myL][rk] = make_uint4(e1.x, e1.y, 0u, qA + 2u); ++rk; }
+          if (l3) { if (rk < (uint32_t)WIDE_W) S.vic[myL][rk] = make_uint4(e1.z, e1.w, 0u, qA + 3u); ++rk; }
+          found += (uint32_t)(__popc(c0) + __popc(c1) + __popc(c2) + __popc(c3));
+          q0 += (uint32_t)WIDE_W;
+          first = false;
+        }
+        __syncwarp();
+        if (lane == 0) {
+          S.found[myL] = found;
+          S.endpos[myL] = my_need ? ((found >= my_need) ? S.vic[myL][my_need - 1].w + 1u : limit_my) : head_my;
+        }
+      }
+      __syncthreads();                                               // (B2) victims of all four lists are in shared memory
+      uint32_t found[5], endpos[5];
+#pragma unroll
+      for (int L = 1; L <= 4; ++L) { found[L] = S.found[L]; endpos[L] = S.endpos[L]; }
+      // (2) an accessed node whose ring entry lies inside a consumed range, or a victim / drop that does not exist
+      bool act = tid < k;
+      uint32_t my_src = ((wide_pick(D.s0, warp) >> lane) & 1u) | (((wide_pick(D.s1, warp) >> lane) & 1u) << 1);
+      bool my_d1 = (wide_pick(D.d1, warp) >> lane) & 1u, my_d2 = (wide_pick(D.d2, warp) >> lane) & 1u;
+      {
+        bool bad = false;
+        if (act) {
+#pragma unroll
+          for (int L = 1; L <= 4; ++L)
+            if (lst == (uint32_t)L && need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
+          if ((my_src & 1u) && wide_rank(D.s0, warp, lt) >= found[L_T1]) bad = true;
+          if (my_src == 2 && wide_rank(S2, warp, lt) >= found[L_T2]) bad = true;
+          if (my_d1 && wide_rank(D.d1, warp, lt) >= found[L_B1]) bad = true;
+          if (my_d2 && wide_rank(D.d2, warp, lt) >= found[L_B2]) bad = true;
+        }
+        const uint32_t bb = __ballot_sync(FULL, bad);
+        if (lane == 0) S.bad[warp] = bb;
+      }
+      __syncthreads();                                               // (B3)
+      int first_bad = -1;
+#pragma unroll
+      for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.bad[u]) first_bad = 32 * u + __ffs(S.bad[u]) - 1;
+      const long long tw3 = clock64();
+      dbg[DBG_CYC_SCAN] += (unsigned long long)(tw3 - tw2);
+      if (first_bad >= 0) {
+        k = first_bad;
+        dbg[DBG_CUT_CONFLICT]++;
+        if (k == 0) {
+          // the by-the-book routine, by warp 0 alone; the new machine state reaches the other warps through shared memory
+          if (warp == 0) {
+            serial_access(C, P, a0, o + (nb - 1 - j));
+            __syncwarp();
+            if (lane == 0) S.ctx = C;
+          }
+          if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
+          __syncthreads();
+          if (warp != 0) C = S.ctx;
+          j += 1;
+          dbg[DBG_WIN_SERIAL]++;
+          __syncthreads();
+          dbg[DBG_CYC_SERIAL] += (unsigned long long)(clock64() - tw3);
+          continue;
+        }
+#pragma unroll
+        for (int u = 0; u < WIDE_WARPS; ++u) {
+          KM[u] = bits_from(0, min(32, max(0, k - 32 * u)));
+          HIT[u] &= KM[u];
+        }
+        wide_roll(D, C, c, lru, S, k, warp, lane);
+#pragma unroll
+        for (int u = 0; u < WIDE_WARPS; ++u) S2[u] = D.s1[u] & ~D.s0[u];
+        need[L_T1] = wide_count(D.s0); need[L_T2] = wide_count(S2); need[L_B1] = wide_count(D.d1); need[L_B2] = wide_count(D.d2);
+#pragma unroll
+        for (int L = 1; L <= 4; ++L) endpos[L] = need[L] ? S.vic[L][need[L] - 1].w + 1u : C.head[L];
+        act = tid < k;
+        my_src = ((wide_pick(D.s0, warp) >> lane) & 1u) | (((wide_pick(D.s1, warp) >> lane) & 1u) << 1);
+        my_d1 = (wide_pick(D.d1, warp) >> lane) & 1u; my_d2 = (wide_pick(D.d2, warp) >> lane) & 1u;
+      }
+      if (D.R.err) C.err = D.R.err;
+
+
+      // ---- apply (threads < k); ranks come from the decision masks of all chunks
+      uint32_t G1[WIDE_WARPS], PT1[WIDE_WARPS], PT2[WIDE_WARPS], NH[WIDE_WARPS], EV[WIDE_WARPS];
+#pragma unroll
+      for (int u = 0; u < WIDE_WARPS; ++u) {
+        G1[u] = D.s0[u] & ~D.s1[u];                                         // pushes to B1, in access order
+        PT1[u] = lru ? KM[u] : (~(M0[u] | M1[u] | M2[u]) & KM[u]);          // ABSENT nodes enter T1 (LRU: everything)
+        PT2[u] = KM[u] & ~PT1[u];
+        NH[u] = KM[u] & ~HIT[u];
+        EV[u] = D.s0[u] | D.s1[u];
+      }
+      if (act) {
+        const bool is_hit = (wide_pick(HIT, warp) >> lane) & 1u;
+        int32_t blk = rec.block, ev = -1;
+        uint32_t dropped = NODE_NONE;
+        if (my_src) {
+          const uint4 v = (my_src == 2) ? S.vic[L_T2][wide_rank(S2, warp, lt)] : S.vic[L_T1][wide_rank(D.s0, warp, lt)];
+          blk = ev = (int32_t)v.y;
+          if (my_src == 3) {                        // leaves no ghost: the key leaves the directory in K4
+            st_node_keep_slot(P.nodes + v.x, L_ABSENT, 0, -1);
+            dropped = v.x;
+          } else {
+            const uint32_t q = (my_src == 1) ? C.tail[L_B1] + wide_rank(G1, warp, lt) : C.tail[L_B2] + wide_rank(S2, warp, lt);
+            __stcg(((my_src == 1) ? P.ring[L_B1] : P.ring[L_B2]) + (q & P.ring_mask), ring_ent(v.x, -1));
+            st_node_keep_slot(P.nodes + v.x, (my_src == 1) ? L_B1 : L_B2, q, -1);
+          }
+        } else if ((wide_pick(D.fm, warp) >> lane) & 1u) {
+          blk = C.next_fresh + (int32_t)wide_rank(D.fm, warp, lt);
+        }
+        if (my_d1 || my_d2) {
+          const uint4 d = my_d1 ? S.vic[L_B1][wide_rank(D.d1, warp, lt)] : S.vic[L_B2][wide_rank(D.d2, warp, lt)];
+          st_node_keep_slot(P.nodes + d.x, L_ABSENT, 0, -1);
+          dropped = d.x;
+        }
+        const bool toT1 = (wide_pick(PT1, warp) >> lane) & 1u;
+        const uint32_t q = toT1 ? C.tail[L_T1] + wide_rank(PT1, warp, lt) : C.tail[L_T2] + wide_rank(PT2, warp, lt);
+        if (lst >= L_T1 && lst <= L_B2) ring_tomb(P, lst, rec.pos);     // the node leaves its old position
+        __stcg((toT1 ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, blk));
+        st_node(P.nodes + n, toT1 ? L_T1 : L_T2, q, blk, rec.slot);
+        const int64_t out = o + (nb - 1 - (j + tid));
+        P.cls[out] = (uint8_t)lst;                    // ABSENT -> MISS(0), T1 -> 1, T2 -> 2, B1 -> 3, B2 -> 4
+        P.block_id[out] = blk;
+        P.evicted_id[out] = ev;
+        P.p_after[out] = D.my_p;
+        P.dropped[a0 + tid] = dropped;
+        if (!is_hit) P.alloc_ids[C.n_alloc + wide_rank(NH, warp, lt)] = blk;
+        if (ev >= 0) P.evict_ids[C.n_evict + wide_rank(EV, warp, lt)] = ev;
+      }
+      // uniform state (every thread computes the same)
+#pragma unroll
+      for (int u = 0; u < WIDE_WARPS; ++u) {
+        C.stat[ST_HIT_T1] += __popc(HIT[u] & M0[u]);
+        C.stat[ST_HIT_T2] += lru ? 0u : (uint32_t)__popc(HIT[u] & M1[u]);
+        C.stat[ST_GHOST_B1] += __popc(M0[u] & M1[u] & ~M2[u] & KM[u]);
+        C.stat[ST_GHOST_B2] += __popc(M2[u] & ~M0[u] & ~M1[u] & KM[u]);
+        C.stat[ST_MISS] += __popc(~(M0[u] | M1[u] | M2[u]) & KM[u]);
+      }
+      C.stat[ST_ACCESSES] += (uint32_t)k;
+      C.stat[ST_EVICT_T1] += need[L_T1];
+      C.stat[ST_EVICT_T2] += need[L_T2];
+      C.stat[ST_DROP_B1] += need[L_B1];
+      C.stat[ST_DROP_B2] += need[L_B2];
+      C.stat[ST_FRESH] += (uint32_t)(D.R.nf - C.next_fresh);
+      C.n_alloc += wide_count(NH);
+      C.n_evict += wide_count(EV);
+#pragma unroll
+      for (int L = 1; L <= 4; ++L) C.head[L] = endpos[L];
+      C.tail[L_T1] += wide_count(PT1);
+      C.tail[L_T2] += wide_count(PT2);
+      C.tail[L_B1] += wide_count(G1);
+      C.tail[L_B2] += need[L_T2];
+      C.t1 = D.R.t1; C.t2 = D.R.t2; C.b1 = D.R.b1; C.b2 = D.R.b2; C.p = D.R.p; C.next_fresh = D.R.nf;
+      C.elig1 = D.R.e1; C.elig2 = D.R.e2;
+      if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
+      j += k;
+      dbg[DBG_WIN_GENERAL]++; dbg[DBG_ACC_GENERAL_WIN] += (unsigned)k;
+      __syncthreads();                                               // (B4) this window's writes are visible to the next fetch
+      dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw3);
+    }
+  }
+  dbg[DBG_CYC_TOTAL] = (unsigned long long)(clock64() - t_begin);
+  if (tid == 0) {
+    ctx_store(C, P);
+#pragma unroll
+    for (int i = 0; i < DBG_COUNT; ++i) P.state->dbg[i] += dbg[i];
+  }
+}
+
+inline void launch_machine_wide(const StepParams& P, cudaStream_t s) { arc_machine_wide_kernel<<<1, WIDE_W, 0, s>>>(P); }
+
+}  // namespace arc
