@@ -72,7 +72,7 @@ struct DevState {
   unsigned long long dbg[32];
 };
 enum : int { DBG_WIN_HIT = 0, DBG_WIN_GENERAL, DBG_WIN_SERIAL, DBG_CUT_TWIN, DBG_CUT_CONFLICT, DBG_SCAN_ROUNDS, DBG_ACC_HIT_WIN,
-             DBG_ACC_GENERAL_WIN, DBG_CYC_FETCH, DBG_CYC_ROLL, DBG_CYC_SCAN, DBG_CYC_APPLY, DBG_CYC_SERIAL, DBG_CYC_TOTAL, DBG_COUNT };
+             DBG_ACC_GENERAL_WIN, DBG_CYC_FETCH, DBG_CYC_ROLL, DBG_CYC_SCAN, DBG_CYC_APPLY, DBG_CYC_SERIAL, DBG_CYC_TOTAL, DBG_ROLL_CALLS, DBG_ROLL_PHASES, DBG_COUNT };
 
 // Everything a step's kernels need, passed by value.
 struct StepParams {

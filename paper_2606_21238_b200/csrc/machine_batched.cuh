@@ -34,6 +34,7 @@ struct Roll {
   uint32_t fm;         // access i takes a fresh block id
   int32_t my_p;        // p after this lane's access
   uint32_t err;
+  uint32_t calls, phases;   // diagnostics
 };
 
 __device__ __forceinline__ uint32_t bits_from(int i, int n) { return ((n >= 32) ? 0xFFFFFFFFu : ((1u << n) - 1u)) << i; }
@@ -51,21 +52,27 @@ __device__ __forceinline__ void roll_replace(Roll& R, bool inb2, int i) {
 __device__ __forceinline__ Roll roll_init(const SerialCtx& C) {
   Roll R;
   R.t1 = C.t1; R.t2 = C.t2; R.b1 = C.b1; R.b2 = C.b2; R.p = C.p; R.nf = C.next_fresh; R.e1 = C.elig1; R.e2 = C.elig2;
-  R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = C.p; R.err = 0;
+  R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = C.p; R.err = 0; R.calls = 0; R.phases = 0;
   return R;
 }
 
 // Rolls k (<= 32) accesses from the state in R; the decision masks of these accesses replace those in R.  lane = this
 // thread's index among the k accesses (my_p is captured for it), or >= 32 when the thread owns none of them.
-__device__ __forceinline__ void roll_chunk(Roll& R, int32_t c, bool lru, uint32_t m0, uint32_t m1, uint32_t m2,
-                                           uint32_t me, int k, int lane) {
+// Deliberately NOT inlined: K3 runs one CTA, so instruction fetch is never hidden by other warps and the kernel has to
+// stay inside the instruction cache; this is the one large routine and it is called up to eight times per window.
+__device__ __noinline__ void roll_chunk(Roll& Rio, int32_t c, bool lru, uint32_t m0, uint32_t m1, uint32_t m2,
+                                        uint32_t me, int k, int lane) {
+  Roll R = Rio;
   R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = R.p;
+  R.calls++;
   const uint32_t km = bits_from(0, k);
   int i = 0;
   while (i < k) {
+    R.phases++;
     const uint32_t li = ((m0 >> i) & 1u) | (((m1 >> i) & 1u) << 1) | (((m2 >> i) & 1u) << 2);
-    // length of the run of accesses with this same list code
-    const uint32_t same = ((li & 1u) ? m0 : ~m0) & ((li & 2u) ? m1 : ~m1) & ((li & 4u) ? m2 : ~m2) & km;
+    // length of the run of accesses with this same list code (ARC: hits in T1 and in T2 form one run)
+    const bool arc_hit = !lru && (li == L_T1 || li == L_T2);
+    const uint32_t same = (arc_hit ? ((m0 ^ m1) & ~m2) : (((li & 1u) ? m0 : ~m0) & ((li & 2u) ? m1 : ~m1) & ((li & 4u) ? m2 : ~m2))) & km;
     const uint32_t brk = ~(same >> i);
     const int m = brk ? (__ffs(brk) - 1) : 32;
     int n = 1;
@@ -79,10 +86,11 @@ __device__ __forceinline__ void roll_chunk(Roll& R, int32_t c, bool lru, uint32_
         R.s0 |= bits_from(i, n); R.s1 |= bits_from(i, n); R.e1 -= n;
         if (R.e1 < 0) R.err = DEV_ERR_NO_VICTIM;
       }
-    } else if (li == L_T1) {
-      n = m; R.t1 -= n; R.t2 += n; R.e1 -= __popc(me & bits_from(i, n));
-    } else if (li == L_T2) {
-      n = m; R.e2 -= __popc(me & bits_from(i, n));
+    } else if (arc_hit) {                     // hits: T1 entries move to T2; evictable entries stop being so
+      n = m;
+      const uint32_t run = bits_from(i, n);
+      const int32_t h1 = __popc(m0 & run);
+      R.t1 -= h1; R.t2 += h1; R.e1 -= __popc(me & m0 & run); R.e2 -= __popc(me & m1 & run);
     } else if (li == L_B1) {
       // ghost hit in B1 (R5 case 2).  With delta = 1 (b2 < 2 b1) the steps of a run are identical while the
       // victim keeps coming from the same list, so the run is rolled in O(1); anything else is one by-the-book step.
@@ -151,16 +159,18 @@ __device__ __forceinline__ void roll_chunk(Roll& R, int32_t c, bool lru, uint32_
     }
     i += n;
   }
+  Rio = R;
 }
 
 __device__ __forceinline__ Roll roll_forward(const SerialCtx& C, int32_t c, bool lru, uint32_t m0, uint32_t m1, uint32_t m2,
                                              uint32_t me, int k, int lane) {
-  Roll R = roll_init(C);
-  roll_chunk(R, c, lru, m0, m1, m2, me, k, lane);
+  Roll T = roll_init(C);
+  roll_chunk(T, c, lru, m0, m1, m2, me, k, lane);
+  Roll R = T;
   return R;
 }
 
-__global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
+__global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_constant__ StepParams P) {
   __shared__ uint4 s_vic[5][32];    // per list: the first entries found from the LRU end {node, block, slot, position}
   const int lane = threadIdx.x;
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
@@ -320,7 +330,9 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
         k = __ffs(badm) - 1;
         dbg[DBG_CUT_CONFLICT]++;
         if (k == 0) {                       // the by-the-book routine, run identically by every lane
-          serial_access(C, P, a0, o + (nb - 1 - j));
+          SerialCtx T = C;                           // the callee is not inlined: keep C itself in registers
+          serial_access(T, P, a0, o + (nb - 1 - j));
+          C = T;
           j += 1;
           __syncwarp();
           dbg[DBG_WIN_SERIAL]++;
@@ -337,6 +349,7 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(StepParams P) {
         for (int L = 1; L <= 4; ++L) endpos[L] = need[L] ? s_vic[L][need[L] - 1].w + 1u : C.head[L];
       }
       if (R.err) C.err = R.err;
+      dbg[DBG_ROLL_CALLS] += R.calls; dbg[DBG_ROLL_PHASES] += R.phases;
 
       // ---- apply (lanes < k); ranks come from the decision masks
       const uint32_t ghost1m = R.s0 & ~R.s1;                                          // pushes to B1, in access order

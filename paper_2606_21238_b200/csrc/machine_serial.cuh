@@ -121,7 +121,7 @@ __device__ __forceinline__ void ring_tomb(const StepParams& P, uint32_t list, ui
 
 // One access (R5 for ARC, R10 for LRU) against the live state: access index a (access order), output index out
 // (natural order).  C.bound[T1/T2] must hold the tails recorded when the access's request began (R4).
-__device__ __forceinline__ void serial_access(SerialCtx& C, const StepParams& P, int64_t a, int64_t out) {
+__device__ __noinline__ void serial_access(SerialCtx& C, const StepParams& P, int64_t a, int64_t out) {
   const int32_t c = P.capacity;
   uint32_t n = P.node_acc[a];
   if (n & SLOT_FLAG) n = __ldcg(&P.table[n & ~SLOT_FLAG].node) - 1;
@@ -191,7 +191,7 @@ __device__ __forceinline__ void serial_access(SerialCtx& C, const StepParams& P,
   if (ev >= 0) P.evict_ids[C.n_evict++] = ev;
 }
 
-__global__ void arc_machine_serial_kernel(StepParams P) {
+__global__ void arc_machine_serial_kernel(const __grid_constant__ StepParams P) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   SerialCtx C;
   ctx_load(C, P);

@@ -64,14 +64,31 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
     const int ku = min(32, max(0, k - 32 * u));
     D.s0[u] = D.s1[u] = D.d1[u] = D.d2[u] = D.fm[u] = 0;
     if (ku > 0) {
-      roll_chunk(D.R, c, lru, S.m[0][u], S.m[1][u], S.m[2][u], S.m[3][u], ku, (u == warp) ? lane : 64);
+      const uint32_t km = bits_from(0, ku);
+      const uint32_t m0 = S.m[0][u] & km, m1 = S.m[1][u] & km, m2 = S.m[2][u] & km, me = S.m[3][u] & km;
+      Roll& R = D.R;
+      const uint32_t hits = lru ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);
+      if (hits == km) {
+        // the chunk is all hits: T1 entries move to T2 (ARC); evictable entries stop being so
+        if (!lru) { const int32_t h1 = __popc(m0); R.t1 -= h1; R.t2 += h1; R.e2 -= __popc(me & m1); }
+        R.e1 -= __popc(me & m0);
+        R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = R.p;
+      } else if (!lru && (m0 | m1 | m2) == 0 && R.t1 + R.b1 == c && R.t1 < c && R.t1 > R.p && R.e1 >= ku && R.t1 + R.t2 == c) {
+        // the chunk is all misses at the fixed point of case 4A: drop B1's LRU ghost, evict T1's LRU entry, no counter moves
+        R.e1 -= ku;
+        R.s0 = km; R.d1 = km; R.s1 = R.d2 = R.fm = 0; R.my_p = R.p;
+      } else {
+        Roll T = D.R;                                // the callee is not inlined: keep D.R itself in registers
+        roll_chunk(T, c, lru, S.m[0][u], S.m[1][u], S.m[2][u], S.m[3][u], ku, (u == warp) ? lane : 64);
+        D.R = T;
+      }
       D.s0[u] = D.R.s0; D.s1[u] = D.R.s1; D.d1[u] = D.R.d1; D.d2[u] = D.R.d2; D.fm[u] = D.R.fm;
       if (u == warp) D.my_p = D.R.my_p;
     }
   }
 }
 
-__global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(StepParams P) {
+__global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(const __grid_constant__ StepParams P) {
   __shared__ WideShared S;
   __shared__ uint32_t s_any_twin;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -283,13 +300,14 @@ __global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(StepParams P) 
         if (k == 0) {
           // the by-the-book routine, by warp 0 alone; the new machine state reaches the other warps through shared memory
           if (warp == 0) {
-            serial_access(C, P, a0, o + (nb - 1 - j));
+            SerialCtx T = C;                           // the callee is not inlined: keep C itself in registers
+            serial_access(T, P, a0, o + (nb - 1 - j));
             __syncwarp();
-            if (lane == 0) S.ctx = C;
+            if (lane == 0) S.ctx = T;
           }
           if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
           __syncthreads();
-          if (warp != 0) C = S.ctx;
+          C = S.ctx;
           j += 1;
           dbg[DBG_WIN_SERIAL]++;
           __syncthreads();
@@ -312,6 +330,7 @@ __global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(StepParams P) 
         my_d1 = (wide_pick(D.d1, warp) >> lane) & 1u; my_d2 = (wide_pick(D.d2, warp) >> lane) & 1u;
       }
       if (D.R.err) C.err = D.R.err;
+      dbg[DBG_ROLL_CALLS] += D.R.calls; dbg[DBG_ROLL_PHASES] += D.R.phases;
 
 
       // ---- apply (threads < k); ranks come from the decision masks of all chunks
