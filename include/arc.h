@@ -155,10 +155,17 @@ uint64_t arc_launch_count(const arc_cache *h);
  * 32-access windows. */
 int arc_set_machine(arc_cache *h, int which);
 
+/* Test hook: from the next step on every block key is ANDed with `mask` (results below 2 are bumped by 2) before the
+ * directory probe, so that a test can force equal keys inside one request, which the 64-bit hash makes unobservable
+ * otherwise (the "same node twice in a window" paths of K3).  ~0 restores normal operation.  Not for production use:
+ * with a mask, different blocks share cache entries. */
+int arc_debug_set_key_mask(arc_cache *h, uint64_t mask);
+
 /* K3 diagnostics, cumulative since create/reset: out[0..n) (HOST) receives, in this order, the number of
  * all-hit windows, general windows, by-the-book single accesses, windows cut at a repeated node, windows cut at a
  * conflict, ring scan rounds, accesses applied in all-hit windows, accesses applied in general windows, then
- * SM cycles spent in: fetch, roll-forward, victim scan, apply, single accesses, the whole kernel.  Synchronises. */
+ * SM cycles spent in: fetch, roll-forward, victim scan, apply, single accesses, the whole kernel; then the number of
+ * calls of the roll-forward routine and of its phases.  Synchronises. */
 int arc_debug_counters(arc_cache *h, uint64_t *out, uint32_t n);
 
 /* Copies one list (1 = T1, 2 = T2, 3 = B1, 4 = B2) in LRU -> MRU order to HOST arrays keys_out /

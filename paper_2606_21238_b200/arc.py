@@ -25,7 +25,7 @@ STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", 
 # every symbol include/arc.h declares (checked by the CPU test-suite against the built library)
 EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats", "arc_reset", "arc_destroy",
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
-           "arc_set_machine", "arc_debug_list", "arc_debug_counters"]
+           "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask"]
 
 
 class ArcError(RuntimeError):
@@ -84,6 +84,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_launch_count.restype = u64
     L.arc_set_machine.argtypes = [vp, C.c_int]
     L.arc_debug_counters.argtypes = [vp, vp, u32]
+    L.arc_debug_set_key_mask.argtypes = [vp, u64]
     L.arc_debug_list.argtypes = [vp, C.c_int, vp, vp, u64, C.POINTER(u64)]
     if path is None:
         _lib = L
@@ -243,6 +244,9 @@ class ArcCache:
         out = np.zeros(len(self.DEBUG_COUNTERS), np.uint64)
         self._check(self._L.arc_debug_counters(self._h, out.ctypes.data, len(out)))
         return {k: int(v) for k, v in zip(self.DEBUG_COUNTERS, out)}
+
+    def debug_set_key_mask(self, mask: int):
+        self._check(self._L.arc_debug_set_key_mask(self._h, mask & 0xFFFFFFFFFFFFFFFF))
 
     def debug_lists(self) -> dict:
         out = {}

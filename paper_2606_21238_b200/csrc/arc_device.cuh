@@ -105,6 +105,7 @@ struct StepParams {
   int32_t capacity;
   int32_t policy;
   uint32_t block_size;
+  unsigned long long key_and;     // test hook (arc_debug_set_key_mask): keys are ANDed with this before the probe; all ones normally
 };
 
 __device__ __forceinline__ Node ld_node(const Node* p) {

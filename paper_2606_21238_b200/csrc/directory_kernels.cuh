@@ -30,7 +30,8 @@ __global__ void __launch_bounds__(256) probe_reserve_kernel(StepParams P) {
   const uint32_t sub = tile.thread_rank();
   const uint32_t tiles = (gridDim.x * blockDim.x) >> 3;
   for (uint32_t a = (blockIdx.x * blockDim.x + threadIdx.x) >> 3; a < P.n_access; a += tiles) {
-    const unsigned long long key = P.keys_acc[a];
+    unsigned long long key = P.keys_acc[a] & P.key_and;
+    if (key < 2) key += 2;                       // 0 and 1 stay reserved under the test mask too
     uint32_t bucket = (uint32_t)key & P.bucket_mask;
     uint32_t result = NODE_NONE;
     for (;;) {

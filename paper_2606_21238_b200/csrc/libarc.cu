@@ -55,6 +55,7 @@ struct arc_cache {
   uint64_t c = 0;
   uint32_t B = 16;
   int policy = 0;
+  unsigned long long key_and = ~0ull;   // test hook
   int machine = 0;            // 0 wide (4 warps), 1 serial, 2 one-warp batched
   // capacities
   uint64_t n_cap = 0;         // max full blocks per step the buffers are sized for
@@ -132,7 +133,7 @@ StepParams make_params(arc_cache* h) {
   P.keys_acc = h->d_keys; P.node_acc = h->d_node_acc; P.dropped = h->d_dropped;
   P.prefix_len = h->d_prefix_len; P.cls = h->d_cls; P.block_id = h->d_block_id; P.evicted_id = h->d_evicted_id;
   P.p_after = h->d_p_after; P.alloc_ids = h->d_alloc_ids; P.evict_ids = h->d_evict_ids;
-  P.capacity = (int32_t)h->c; P.policy = h->policy; P.block_size = h->B;
+  P.capacity = (int32_t)h->c; P.policy = h->policy; P.block_size = h->B; P.key_and = h->key_and;
   return P;
 }
 
@@ -590,6 +591,12 @@ uint64_t arc_launch_count(const arc_cache* h) { return h ? h->launches : g_hash_
 int arc_set_machine(arc_cache* h, int which) {
   if (!h || which < 0 || which > 2) return ARC_ERR_INVALID_ARG;
   h->machine = which;
+  return ARC_OK;
+}
+
+int arc_debug_set_key_mask(arc_cache* h, uint64_t mask) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  h->key_and = mask;
   return ARC_OK;
 }
 

@@ -223,3 +223,32 @@ def test_maintenance_rebuild_and_compaction(arc):
                 assert_same_step(g.to_host(), o, f"maint policy {policy} step {step}")
         assert_same_state(gc, oc, f"maintenance policy {policy}")
         gc.close()
+
+
+@pytest.mark.parametrize("machine", [0, 1, 2])
+@pytest.mark.parametrize("bits", [3, 6])
+def test_equal_keys_inside_a_request(arc, machine, bits):
+    """The same key several times inside one request (forced with the key-mask test hook; the 64-bit hash never does
+    it): the second access is a hit on a block its own request has pinned.  Exercises the window cuts at repeated nodes."""
+    rng = np.random.default_rng(40 + bits)
+    mask = (1 << bits) - 1
+    for policy in (0, 1):
+        c = 40
+        gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
+        gc.set_machine(machine)
+        gc.debug_set_key_mask(mask)
+        for step in range(25):
+            reqs = [rng.integers(0, 50, size=16 * int(rng.integers(1, c + 1)) + int(rng.integers(0, 16)), dtype=np.int32)
+                    for _ in range(int(rng.integers(1, 6)))]
+            tokens, offsets = W.pack_requests(reqs)
+            keys, blk_off = O.hash_blocks(tokens, offsets)
+            keys = keys & np.uint64(mask)
+            keys[keys < 2] += np.uint64(2)
+            o = oc.step_keys([keys[blk_off[r]:blk_off[r + 1]] for r in range(len(reqs))])
+            g = gc.step(dev(tokens), offsets).to_host()
+            for k in OUT_KEYS:
+                assert np.array_equal(g[k], o[k]), f"bits {bits} policy {policy} machine {machine} step {step}: {k}"
+        gl, ol = gc.debug_lists(), oc.lists()
+        for n in ("T1", "T2", "B1", "B2"):
+            assert np.array_equal(gl[n][0], ol[n][0]) and np.array_equal(gl[n][1], ol[n][1]), n
+        gc.close()
