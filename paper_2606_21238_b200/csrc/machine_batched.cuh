@@ -91,71 +91,78 @@ __device__ __noinline__ void roll_chunk(Roll& Rio, int32_t c, bool lru, uint32_t
       const uint32_t run = bits_from(i, n);
       const int32_t h1 = __popc(m0 & run);
       R.t1 -= h1; R.t2 += h1; R.e1 -= __popc(me & m0 & run); R.e2 -= __popc(me & m1 & run);
-    } else if (li == L_B1) {
-      // ghost hit in B1 (R5 case 2).  With delta = 1 (b2 < 2 b1) the steps of a run are identical while the
-      // victim keeps coming from the same list, so the run is rolled in O(1); anything else is one by-the-book step.
-      const bool d_one = R.b2 < 2 * R.b1;
-      const int32_t J = max(0, (R.t1 - R.p) / 2);         // steps j with t1 - j > p + j + 1  (REPLACE prefers T1)
+    } else if (li == L_B1 || li == L_B2) {
+      // Ghost hit (R5 cases 2, 3).  While delta = 1 the steps of a run are identical as long as the victim keeps coming
+      // from the same list, so the run is rolled in O(1): the regime and its length are computed with selects (no
+      // branches: one warp has no other warp to hide a branch behind); anything else is one by-the-book step.
+      const bool inb2 = (li == L_B2);
+      const int32_t bx = inb2 ? R.b2 : R.b1, by = inb2 ? R.b1 : R.b2;      // bx: the list that was hit
+      const bool d_one = by < 2 * bx;
       const int32_t p0 = R.p;
-      if (d_one && J > 0 && R.e1 > 0) {                   // victims from T1: t1--, t2++, p++ per step
-        n = min(min(m, R.e1), J);
-        R.s0 |= bits_from(i, n); R.t1 -= n; R.t2 += n; R.e1 -= n; R.p += n;
-      } else if (d_one && J == 0 && R.e2 > 0) {           // victims from T2: b1--, b2++, p++ per step, while delta stays 1
-        n = min(min(m, R.e2), (2 * R.b1 - R.b2 + 2) / 3);
-        R.s1 |= bits_from(i, n); R.b1 -= n; R.b2 += n; R.e2 -= n; R.p = min(c, R.p + n);
+      // B1: REPLACE prefers T1 for the steps j with t1 - j > p + j + 1, i.e. J = (t1 - p) / 2 of them
+      // B2: REPLACE(true) prefers T1 while t1 - j >= 1 and t1 >= p - 1
+      const int32_t J1 = max(0, (R.t1 - R.p) / 2);
+      const bool pref1 = inb2 ? (R.t1 >= 1 && R.t1 >= R.p - 1) : (J1 > 0);
+      const int32_t n_delta = (2 * bx - by + 2) / 3;                         // steps while delta stays 1 when bx shrinks and by grows
+      // regime a: victims from T1;  regime b: victims from T2
+      const bool ra = d_one && pref1 && R.e1 > 0, rb = d_one && !pref1 && R.e2 > 0;
+      int32_t na = min(m, R.e1), nbb = min(m, R.e2);
+      na = inb2 ? min(na, min(n_delta, R.t1)) : min(na, J1);                 // B2+T1 moves b1 up / b2 down; B1+T1 leaves b1, b2
+      nbb = inb2 ? ((R.t1 >= 1) ? min(nbb, R.p - 1 - R.t1) : nbb) : min(nbb, n_delta);
+      if (ra || rb) {
+        n = ra ? na : nbb;
+        const uint32_t run = bits_from(i, n);
+        R.s0 |= ra ? run : 0u; R.s1 |= ra ? 0u : run;
+        R.e1 -= ra ? n : 0; R.e2 -= ra ? 0 : n;
+        R.t1 -= ra ? n : 0; R.t2 += ra ? n : 0;
+        // ghost list sizes: B1+T1 none; B1+T2: b1 -= n, b2 += n; B2+T1: b1 += n, b2 -= n; B2+T2: none
+        const int32_t db1 = (!inb2 && !ra) ? -n : ((inb2 && ra) ? n : 0);
+        R.b1 += db1; R.b2 -= db1;
+        R.p = inb2 ? max(0, R.p - n) : min(c, R.p + n);
+        if (lane >= i) R.my_p = inb2 ? max(0, p0 - min(lane - i + 1, n)) : min(c, p0 + min(lane - i + 1, n));
       } else {
-        const int32_t d = (R.b2 >= 2 * R.b1 && R.b1 > 0) ? R.b2 / R.b1 : 1;
-        R.p = min(c, R.p + d);
-        roll_replace(R, false, i);
-        R.b1--; R.t2++;
+        const int32_t d = (by >= 2 * bx && bx > 0) ? by / bx : 1;
+        R.p = inb2 ? max(0, R.p - d) : min(c, R.p + d);
+        roll_replace(R, inb2, i);
+        if (inb2) R.b2--; else R.b1--;
+        R.t2++;
+        if (lane >= i) R.my_p = R.p;
       }
-      if (lane >= i) R.my_p = (n > 1 || R.p - p0 == 1) ? min(c, p0 + min(lane - i + 1, n)) : R.p;
-    } else if (li == L_B2) {
-      // ghost hit in B2 (R5 case 3), same structure: p falls by delta = 1 while b1 < 2 b2
-      const bool d_one = R.b1 < 2 * R.b2;
-      const int32_t p0 = R.p;
-      if (d_one && R.t1 >= 1 && R.t1 >= R.p - 1 && R.e1 > 0) {   // REPLACE(true) takes T1 while t1 >= 1: t1--, t2++, b1++, b2--
-        n = min(min(m, R.e1), min((2 * R.b2 - R.b1 + 2) / 3, R.t1));
-        R.s0 |= bits_from(i, n); R.t1 -= n; R.t2 += n; R.b1 += n; R.b2 -= n; R.e1 -= n; R.p = max(0, R.p - n);
-      } else if (d_one && (R.t1 == 0 || R.t1 < R.p - 1) && R.e2 > 0) {   // victims from T2: only p and elig2 move
-        n = min(m, R.e2);
-        if (R.t1 >= 1) n = min(n, R.p - 1 - R.t1);
-        R.s1 |= bits_from(i, n); R.e2 -= n; R.p = max(0, R.p - n);
-      } else {
-        const int32_t d = (R.b1 >= 2 * R.b2 && R.b2 > 0) ? R.b1 / R.b2 : 1;
-        R.p = max(0, R.p - d);
-        roll_replace(R, true, i);
-        R.b2--; R.t2++;
-      }
-      if (lane >= i) R.my_p = (n > 1 || p0 - R.p <= 1) ? max(0, p0 - min(lane - i + 1, n)) : R.p;
-    } else if (R.t1 + R.t2 < c) {             // miss while the cache is filling: b1 = b2 = 0 (I7)
-      n = min(m, c - R.t1 - R.t2); R.fm |= bits_from(i, n); R.t1 += n; R.nf += n;
-    } else if (R.t1 < c && R.t1 > R.p && R.e1 > 0) {
-      // miss, REPLACE takes T1's LRU entry (t1 stays).  Case 4A (t1 + b1 = c): B1's LRU ghost is dropped, nothing moves.
-      // Case 4B: b1 grows by one per miss; B2's LRU ghost is dropped while b1 + b2 = c.
+    } else {
+      // Miss (R5 case 4), same idea.  fill: the cache is not full yet (b1 = b2 = 0, I7).  r1: REPLACE takes T1's LRU
+      // entry (t1 stays); r2: T1 is at or below its target, REPLACE takes T2's LRU entry and T1 grows by one per miss.
+      // In case 4A (t1 + b1 = c) B1's LRU ghost is dropped; in case 4B B2's LRU ghost is dropped while b1 + b2 = c.
+      const bool fill = R.t1 + R.t2 < c;
       const int32_t gapA = c - R.t1 - R.b1, gapS = c - R.b1 - R.b2;
-      if (gapA == 0) { n = min(m, R.e1); R.d1 |= bits_from(i, n); }
-      else if (gapS == 0) { n = min(min(m, R.e1), gapA); R.d2 |= bits_from(i, n); R.b2 -= n; R.b1 += n; }
-      else { n = min(min(m, R.e1), min(gapA, gapS)); R.b1 += n; }
-      R.s0 |= bits_from(i, n); R.e1 -= n;
-    } else if (R.t1 < c && R.t1 <= R.p && R.e2 > 0) {
-      // miss while T1 is at or below its target: REPLACE takes T2's LRU entry, T1 grows by one per miss
-      const int32_t gapA = c - R.t1 - R.b1, gapS = c - R.b1 - R.b2;
-      n = min(min(m, R.e2), min(R.p - R.t1 + 1, c - R.t1));
-      if (gapA == 0) { R.d1 |= bits_from(i, n); R.b1 -= n; R.b2 += n; }
-      else if (gapS == 0) { n = min(n, gapA); R.d2 |= bits_from(i, n); }
-      else { n = min(n, min(gapA, gapS)); R.b2 += n; }
-      R.s1 |= bits_from(i, n); R.t1 += n; R.t2 -= n; R.e2 -= n;
-    } else {                                  // any other miss (pin fallback, T1 holding everything): one by-the-book step
-      if (R.t1 + R.b1 == c) {
-        if (R.t1 < c) { R.d1 |= 1u << i; R.b1--; roll_replace(R, false, i); }
-        else { R.s0 |= 1u << i; R.s1 |= 1u << i; R.t1--; R.e1--; if (R.e1 < 0) R.err = DEV_ERR_NO_VICTIM; }
-      } else {
-        const int32_t tot = R.t1 + R.t2 + R.b1 + R.b2;
-        if (tot == 2 * c) { R.d2 |= 1u << i; R.b2--; }
-        roll_replace(R, false, i);            // tot >= c here because the cache is full
+      const bool isA = gapA == 0, isS = gapS == 0;
+      const bool pref1 = R.t1 > R.p;
+      const bool r1 = !fill && R.t1 < c && pref1 && R.e1 > 0, r2 = !fill && R.t1 < c && !pref1 && R.e2 > 0;
+      const int32_t lim_gap = isA ? m : (isS ? gapA : min(gapA, gapS));     // steps until the case changes
+      const int32_t nf = min(m, c - R.t1 - R.t2);
+      const int32_t n1 = min(min(m, R.e1), lim_gap);
+      const int32_t n2 = min(min(min(m, R.e2), lim_gap), min(R.p - R.t1 + 1, c - R.t1));
+      if (fill || r1 || r2) {
+        n = fill ? nf : (r1 ? n1 : n2);
+        const uint32_t run = bits_from(i, n);
+        R.fm |= fill ? run : 0u;
+        R.s0 |= r1 ? run : 0u; R.s1 |= r2 ? run : 0u;
+        R.d1 |= (!fill && isA) ? run : 0u; R.d2 |= (!fill && !isA && isS) ? run : 0u;
+        R.nf += fill ? n : 0;
+        R.e1 -= r1 ? n : 0; R.e2 -= r2 ? n : 0;
+        R.t1 += (fill || r2) ? n : 0; R.t2 -= r2 ? n : 0;
+        // r1: 4A nothing, 4B b1 += n and (b1 + b2 = c) b2 -= n.   r2: 4A b1 -= n, b2 += n; 4B (b1 + b2 < c) b2 += n
+        R.b1 += (r1 && !isA) ? n : ((r2 && isA) ? -n : 0);
+        R.b2 += (r1 && !isA && isS) ? -n : ((r2 && (isA || !isS)) ? n : 0);
+      } else {                                // pin fallback, or T1 holding everything: one by-the-book step
+        if (isA) {
+          if (R.t1 < c) { R.d1 |= 1u << i; R.b1--; roll_replace(R, false, i); }
+          else { R.s0 |= 1u << i; R.s1 |= 1u << i; R.t1--; R.e1--; if (R.e1 < 0) R.err = DEV_ERR_NO_VICTIM; }
+        } else {
+          if (isS) { R.d2 |= 1u << i; R.b2--; }
+          roll_replace(R, false, i);          // t1 + t2 + b1 + b2 >= c here because the cache is full
+        }
+        R.t1++;
       }
-      R.t1++;
     }
     i += n;
   }
