@@ -21,7 +21,8 @@ struct WideShared {
   uint32_t m[4][WIDE_WARPS];                 // m0, m1, m2, me per chunk
   uint32_t bad[WIDE_WARPS];
   uint32_t twin[WIDE_WARPS];
-  uint32_t found[5], endpos[5];
+  uint32_t found[5], endpos[5], need[5];
+  uint32_t ctl_done, ctl_head[5], ctl_limit[5]; // published by thread 0 before a window's first barrier, read by the scanner warps
   uint32_t set_id[WIDE_SET], set_min[WIDE_SET];
   uint4 vic[5][WIDE_W];                      // per list: entries found from the LRU end {node, block, -, position}
   SerialCtx ctx;                             // the machine state after a by-the-book access done by warp 0
@@ -88,7 +89,64 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
   }
 }
 
-__global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(const __grid_constant__ StepParams P) {
+// One scan round of a scanner warp: 128 ring entries from q0 (a multiple of 4), 4 per lane; live entries are appended
+// to vic[] in LRU order.  Returns the number of live entries found in the round.
+__device__ __forceinline__ uint32_t wide_scan_round(const RingEnt* ring, uint32_t ring_mask, uint32_t q0, uint32_t head, uint32_t limit,
+                                                    uint32_t found, uint4* vic, int lane, uint32_t lt) {
+  const uint32_t FULL = 0xFFFFFFFFu;
+  const uint32_t qA = q0 + 4u * (uint32_t)lane;
+  const uint4 e0 = __ldcg(reinterpret_cast<const uint4*>(ring + (qA & ring_mask)));
+  const uint4 e1 = __ldcg(reinterpret_cast<const uint4*>(ring + ((qA + 2u) & ring_mask)));
+  // live = inside [head, limit) and not a tombstone
+  const bool l0 = (int32_t)(qA - head) >= 0 && (int32_t)(limit - qA) > 0 && e0.x != RING_TOMB;
+  const bool l1 = (int32_t)(qA + 1u - head) >= 0 && (int32_t)(limit - qA - 1u) > 0 && e0.z != RING_TOMB;
+  const bool l2 = (int32_t)(qA + 2u - head) >= 0 && (int32_t)(limit - qA - 2u) > 0 && e1.x != RING_TOMB;
+  const bool l3 = (int32_t)(qA + 3u - head) >= 0 && (int32_t)(limit - qA - 3u) > 0 && e1.z != RING_TOMB;
+  const uint32_t c0 = __ballot_sync(FULL, l0), c1 = __ballot_sync(FULL, l1), c2 = __ballot_sync(FULL, l2), c3 = __ballot_sync(FULL, l3);
+  uint32_t rk = found + (uint32_t)(__popc(c0 & lt) + __popc(c1 & lt) + __popc(c2 & lt) + __popc(c3 & lt));
+  if (l0) { if (rk < (uint32_t)WIDE_W) vic[rk] = make_uint4(e0.x, e0.y, 0u, qA); ++rk; }
+  if (l1) { if (rk < (uint32_t)WIDE_W) vic[rk] = make_uint4(e0.z, e0.w, 0u, qA + 1u); ++rk; }
+  if (l2) { if (rk < (uint32_t)WIDE_W) vic[rk] = make_uint4(e1.x, e1.y, 0u, qA + 2u); ++rk; }
+  if (l3) { if (rk < (uint32_t)WIDE_W) vic[rk] = make_uint4(e1.z, e1.w, 0u, qA + 3u); ++rk; }
+  return (uint32_t)(__popc(c0) + __popc(c1) + __popc(c2) + __popc(c3));
+}
+
+// Scanner warp for list L (warps 4..7 of the CTA): follows the owners' barrier sequence window by window.  The first
+// 128 entries from the list head are scanned while the owners fetch node records and roll the counters forward; more
+// rounds follow only if the window turns out to need more victims than that.
+__device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S, volatile uint32_t* any_twin, uint32_t L, int lane) {
+  const uint32_t lt = (1u << lane) - 1u;
+  const RingEnt* ring = P.ring[L];
+  unsigned long long rounds = 0;
+  for (;;) {
+    __syncthreads();                                   // (S0) the window's control block is published
+    if (S.ctl_done) break;
+    const uint32_t head = S.ctl_head[L], limit = S.ctl_limit[L];
+    uint32_t q0 = head & ~3u, found = 0;
+    if ((int32_t)(limit - q0) > 0) { found += wide_scan_round(ring, P.ring_mask, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds; }
+    __syncthreads();                                   // (B1)
+    if (*any_twin) { __syncthreads(); __syncthreads(); }
+    __syncthreads();                                   // (B2) the owners have published what the window needs
+    const uint32_t need = S.need[L];
+    while (found < need && (int32_t)(limit - q0) > 0) {
+      found += wide_scan_round(ring, P.ring_mask, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
+    }
+    __syncwarp();
+    if (lane == 0) {
+      S.found[L] = found;
+      S.endpos[L] = need ? ((found >= need) ? S.vic[L][need - 1].w + 1u : limit) : head;
+    }
+    __syncthreads();                                   // (B2') victims of all four lists are in shared memory
+    __syncthreads();                                   // (B3)
+    bool serial = false;
+#pragma unroll
+    for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.bad[u]) serial = (32 * u + __ffs(S.bad[u]) - 1) == 0;
+    if (serial) __syncthreads();                       // the by-the-book access of warp 0
+  }
+  if (lane == 0 && rounds) atomicAdd(&P.state->dbg[DBG_SCAN_ROUNDS], rounds);
+}
+
+__global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __grid_constant__ StepParams P) {
   __shared__ WideShared S;
   __shared__ uint32_t s_any_twin;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -98,15 +156,17 @@ __global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(const __grid_c
   const int64_t N = (int64_t)P.n_access;
   SerialCtx C;            // identical in every thread
   ctx_load(C, P);
-  for (int i = tid; i < WIDE_SET; i += WIDE_W) { S.set_id[i] = 0xFFFFFFFFu; S.set_min[i] = 0xFFFFFFFFu; }
+  for (int i = tid; i < WIDE_SET; i += 2 * WIDE_W) { S.set_id[i] = 0xFFFFFFFFu; S.set_min[i] = 0xFFFFFFFFu; }
   if (tid == 0) s_any_twin = 0;
   __syncthreads();
   unsigned long long dbg[DBG_COUNT];
 #pragma unroll
   for (int i = 0; i < DBG_COUNT; ++i) dbg[i] = 0;
   const long long t_begin = clock64();
-  const uint32_t myL = (uint32_t)warp + 1u;                 // the list this warp scans
-  RingEnt* const my_ring = P.ring[warp + 1];
+  if (warp >= WIDE_WARPS) {                                 // warps 4..7 scan the LRU ends of T1, T2, B1, B2
+    wide_scanner(P, S, &s_any_twin, (uint32_t)(warp - WIDE_WARPS) + 1u, lane);
+    return;
+  }
 
   // node ids are prefetched one window ahead: pre_n = node_acc[pre_base + tid]
   int64_t pre_base = 0;
@@ -126,19 +186,18 @@ __global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(const __grid_c
       int k = kmax;
       const int64_t a0 = o + j;
       const bool act0 = tid < k;
+      if (tid == 0) {
+        S.ctl_done = 0;
+#pragma unroll
+        for (int L = 1; L <= 4; ++L) { S.ctl_head[L] = C.head[L]; S.ctl_limit[L] = (L <= 2) ? C.bound[L] : C.tail[L]; }
+      }
+      __syncthreads();                                               // (S0) the previous window's writes are visible; the scanners start
       const long long tw0 = clock64();
       uint32_t n = pre_n;
       if (pre_base != a0) n = (a0 + tid < N) ? P.node_acc[a0 + tid] : NODE_NONE;     // the last window was cut short
       Node rec;
       rec.list = L_FREE; rec.pos = 0; rec.block = -1; rec.slot = 0;
       if (act0) rec = ld_node(P.nodes + n);
-      // this warp's list: the first 128 ring entries from the head travel with the node records; lane l holds
-      // positions qa + 4l .. qa + 4l + 3, qa = head rounded down to a multiple of 4 (two 16-byte loads)
-      const uint32_t head_my = (myL == L_T1) ? C.head[L_T1] : (myL == L_T2) ? C.head[L_T2] : (myL == L_B1) ? C.head[L_B1] : C.head[L_B2];
-      const uint32_t limit_my = (myL == L_T1) ? C.bound[L_T1] : (myL == L_T2) ? C.bound[L_T2] : (myL == L_B1) ? C.tail[L_B1] : C.tail[L_B2];
-      uint32_t q0 = head_my & ~3u;
-      uint4 e0 = __ldcg(reinterpret_cast<const uint4*>(my_ring + ((q0 + 4u * (uint32_t)lane) & P.ring_mask)));
-      uint4 e1 = __ldcg(reinterpret_cast<const uint4*>(my_ring + ((q0 + 4u * (uint32_t)lane + 2u) & P.ring_mask)));
       pre_base = a0 + kmax;
       pre_n = (pre_base + tid < N) ? P.node_acc[pre_base + tid] : NODE_NONE;
 
@@ -217,8 +276,12 @@ __global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(const __grid_c
         C.elig1 -= (int32_t)e1d; C.elig2 -= (int32_t)e2d;
         C.stat[ST_ACCESSES] += (uint32_t)k;
         if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
+        if (tid < 5) S.need[tid] = 0;
+        if (lane == 0) S.bad[warp] = 0;
         j += k;
         dbg[DBG_WIN_HIT]++; dbg[DBG_ACC_HIT_WIN] += (unsigned)k;
+        __syncthreads();                                             // (B2), (B2'), (B3): the scanners' sequence
+        __syncthreads();
         __syncthreads();
         dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw1);
         continue;
@@ -234,39 +297,9 @@ __global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(const __grid_c
       for (int u = 0; u < WIDE_WARPS; ++u) S2[u] = D.s1[u] & ~D.s0[u];
       uint32_t need[5];
       need[0] = 0; need[L_T1] = wide_count(D.s0); need[L_T2] = wide_count(S2); need[L_B1] = wide_count(D.d1); need[L_B2] = wide_count(D.d2);
-      {
-        const uint32_t my_need = (myL == L_T1) ? need[L_T1] : (myL == L_T2) ? need[L_T2] : (myL == L_B1) ? need[L_B1] : need[L_B2];
-        uint32_t found = 0;
-        bool first = true;
-        while (found < my_need && (int32_t)(limit_my - q0) > 0) {
-          if (!first) {
-            e0 = __ldcg(reinterpret_cast<const uint4*>(my_ring + ((q0 + 4u * (uint32_t)lane) & P.ring_mask)));
-            e1 = __ldcg(reinterpret_cast<const uint4*>(my_ring + ((q0 + 4u * (uint32_t)lane + 2u) & P.ring_mask)));
-          }
-          if (warp == 0) dbg[DBG_SCAN_ROUNDS]++;
-          const uint32_t qA = q0 + 4u * (uint32_t)lane;
-          // live = inside [head, limit) and not a tombstone
-          const bool l0 = (int32_t)(qA - head_my) >= 0 && (int32_t)(limit_my - qA) > 0 && e0.x != RING_TOMB;
-          const bool l1 = (int32_t)(qA + 1u - head_my) >= 0 && (int32_t)(limit_my - qA - 1u) > 0 && e0.z != RING_TOMB;
-          const bool l2 = (int32_t)(qA + 2u - head_my) >= 0 && (int32_t)(limit_my - qA - 2u) > 0 && e1.x != RING_TOMB;
-          const bool l3 = (int32_t)(qA + 3u - head_my) >= 0 && (int32_t)(limit_my - qA - 3u) > 0 && e1.z != RING_TOMB;
-          const uint32_t c0 = __ballot_sync(FULL, l0), c1 = __ballot_sync(FULL, l1), c2 = __ballot_sync(FULL, l2), c3 = __ballot_sync(FULL, l3);
-          uint32_t rk = found + (uint32_t)(__popc(c0 & lt) + __popc(c1 & lt) + __popc(c2 & lt) + __popc(c3 & lt));
-          if (l0) { if (rk < (uint32_t)WIDE_W) S.vic[myL][rk] = make_uint4(e0.x, e0.y, 0u, qA); ++rk; }
-          if (l1) { if (rk < (uint32_t)WIDE_W) S.vic[myL][rk] = make_uint4(e0.z, e0.w, 0u, qA + 1u); ++rk; }
-          if (l2) { if (rk < (uint32_t)WIDE_W) S.vic[myL][rk] = make_uint4(e1.x, e1.y, 0u, qA + 2u); ++rk; }
-          if (l3) { if (rk < (uint32_t)WIDE_W) S.vic[myL][rk] = make_uint4(e1.z, e1.w, 0u, qA + 3u); ++rk; }
-          found += (uint32_t)(__popc(c0) + __popc(c1) + __popc(c2) + __popc(c3));
-          q0 += (uint32_t)WIDE_W;
-          first = false;
-        }
-        __syncwarp();
-        if (lane == 0) {
-          S.found[myL] = found;
-          S.endpos[myL] = my_need ? ((found >= my_need) ? S.vic[myL][my_need - 1].w + 1u : limit_my) : head_my;
-        }
-      }
-      __syncthreads();                                               // (B2) victims of all four lists are in shared memory
+      if (tid == 0) { S.need[L_T1] = need[L_T1]; S.need[L_T2] = need[L_T2]; S.need[L_B1] = need[L_B1]; S.need[L_B2] = need[L_B2]; }
+      __syncthreads();                                               // (B2) the scanners learn what the window needs
+      __syncthreads();                                               // (B2') victims of all four lists are in shared memory
       uint32_t found[5], endpos[5];
 #pragma unroll
       for (int L = 1; L <= 4; ++L) { found[L] = S.found[L]; endpos[L] = S.endpos[L]; }
@@ -310,7 +343,6 @@ __global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(const __grid_c
           C = S.ctx;
           j += 1;
           dbg[DBG_WIN_SERIAL]++;
-          __syncthreads();
           dbg[DBG_CYC_SERIAL] += (unsigned long long)(clock64() - tw3);
           continue;
         }
@@ -408,10 +440,11 @@ __global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(const __grid_c
       if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
       j += k;
       dbg[DBG_WIN_GENERAL]++; dbg[DBG_ACC_GENERAL_WIN] += (unsigned)k;
-      __syncthreads();                                               // (B4) this window's writes are visible to the next fetch
       dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw3);
     }
   }
+  if (tid == 0) S.ctl_done = 1;
+  __syncthreads();                                                   // the scanners leave; the last window's writes are done
   dbg[DBG_CYC_TOTAL] = (unsigned long long)(clock64() - t_begin);
   if (tid == 0) {
     ctx_store(C, P);
@@ -420,6 +453,6 @@ __global__ void __launch_bounds__(WIDE_W) arc_machine_wide_kernel(const __grid_c
   }
 }
 
-inline void launch_machine_wide(const StepParams& P, cudaStream_t s) { arc_machine_wide_kernel<<<1, WIDE_W, 0, s>>>(P); }
+inline void launch_machine_wide(const StepParams& P, cudaStream_t s) { arc_machine_wide_kernel<<<1, 2 * WIDE_W, 0, s>>>(P); }
 
 }  // namespace arc
