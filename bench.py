@@ -218,6 +218,35 @@ def k1_bulk_roofline(torch, A, gib, stream, seed):
     return n_blocks, len(offs) - 1, float(np.mean(ms)), ms[0]
 
 
+def k2_probe_bench(torch, A, stream, seed, n_keys=1 << 24):
+    """K2 alone on a directory far larger than L2: capacity 16 M blocks (2 GiB table), 16 M distinct random keys inserted,
+    then looked up again in a different random order (every probe is one random 128-B bucket read from HBM)."""
+    cache = A.ArcCache(n_keys, 16, A.POLICY_ARC)
+    g = torch.Generator(device="cuda")
+    g.manual_seed(seed + 91)
+    keys = torch.randint(2, 2 ** 62, (n_keys,), dtype=torch.int64, device="cuda", generator=g)
+    nodes = torch.empty(n_keys, dtype=torch.int32, device="cuda")
+    cache.reserve(1, n_keys)
+    cache.debug_probe(keys, nodes, stream)                      # inserts
+    stream.synchronize()
+    first = nodes.clone()
+    perm = torch.randperm(n_keys, device="cuda", generator=g)
+    keys2 = keys[perm].contiguous()
+    for _ in range(2):
+        cache.debug_probe(keys2, nodes, stream)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+    stream.synchronize()
+    for a, b in evs:
+        a.record(stream)
+        cache.debug_probe(keys2, nodes, stream)
+        b.record(stream)
+    stream.synchronize()
+    ok = bool(torch.equal(nodes, first[perm]))                  # every key found again, at the node it was given
+    ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+    cache.close()
+    return n_keys, ms, ok
+
+
 def cpu_oracle_leg(info, steps, policy=0):
     """The oracle as it stands (g++ -O2, std::list + unordered_map, one thread) over the same steps."""
     from oracle import oracle as O
@@ -323,6 +352,14 @@ def run_ours(args):
                             "best_ms": best_ms, "tokens_per_s": 16 * nb / (mean_ms * 1e-3),
                             "workload": f"{nreq_b} D5-shaped requests, {nb} blocks, {64 * nb / 2**30:.2f} GiB of tokens (>> 126 MB L2)",
                             "in_situ_GBps": k1_insitu}
+        # K2 alone, table >> L2
+        nk, k2_ms, k2_ok = k2_probe_bench(torch, A, stream, args.seed)
+        line["probe"] = {"kernel": "K2 probe_reserve + resolve (arc_debug_probe)", "keys": nk, "ms_per_launch": k2_ms, "keys_per_s": nk / (k2_ms * 1e-3),
+                         "found_all": k2_ok, "table": "capacity 16 M blocks: 2 GiB table of 16-B slots in 128-B buckets, load 0.125",
+                         "algorithmic_GBps": 28 * nk / (k2_ms * 1e-3) / 1e9, "sector_level_GBps": 140 * nk / (k2_ms * 1e-3) / 1e9,
+                         "frac_of_measured_hbm_sector_level": 140 * nk / (k2_ms * 1e-3) / 1e9 / peak,
+                         "bytes_model": "algorithmic 28 B/key (8 B key + 16 B slot + 4 B node id); sector level 140 B/key (8 + one 128-B bucket + 4)",
+                         "in_situ_us_per_step": 1e3 * sums.get("probe_ms", 0.0) / K}
         # ARC vs LRU on the same steps
         c3, _, _, _ = run_device_resident(torch, A, info, steps, dev, bases, W_, A.POLICY_LRU, stream)
         st_lru = c3.stats()

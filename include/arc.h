@@ -155,6 +155,12 @@ uint64_t arc_launch_count(const arc_cache *h);
  * 32-access windows. */
 int arc_set_machine(arc_cache *h, int which);
 
+/* K2 alone, for the probe microbenchmark and its tests: looks every key of d_keys (DEVICE uint64[n], values >= 2) up in
+ * the handle's directory, inserting unknown keys as placeholder nodes exactly as arc_step's probe does, and writes the
+ * node index of key i to d_nodes_out[i] (DEVICE uint32[n]).  Asynchronous on cuda_stream.  The placeholders are never
+ * cleaned up (no K4 runs), so use a handle that is destroyed afterwards. */
+int arc_debug_probe(arc_cache *h, const uint64_t *d_keys, uint64_t n, uint32_t *d_nodes_out, void *cuda_stream);
+
 /* Test hook: from the next step on every block key is ANDed with `mask` (results below 2 are bumped by 2) before the
  * directory probe, so that a test can force equal keys inside one request, which the 64-bit hash makes unobservable
  * otherwise (the "same node twice in a window" paths of K3).  ~0 restores normal operation.  Not for production use:

@@ -25,7 +25,7 @@ STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", 
 # every symbol include/arc.h declares (checked by the CPU test-suite against the built library)
 EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats", "arc_reset", "arc_destroy",
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
-           "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask"]
+           "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe"]
 
 
 class ArcError(RuntimeError):
@@ -85,6 +85,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_set_machine.argtypes = [vp, C.c_int]
     L.arc_debug_counters.argtypes = [vp, vp, u32]
     L.arc_debug_set_key_mask.argtypes = [vp, u64]
+    L.arc_debug_probe.argtypes = [vp, vp, u64, vp, vp]
     L.arc_debug_list.argtypes = [vp, C.c_int, vp, vp, u64, C.POINTER(u64)]
     if path is None:
         _lib = L
@@ -244,6 +245,14 @@ class ArcCache:
         out = np.zeros(len(self.DEBUG_COUNTERS), np.uint64)
         self._check(self._L.arc_debug_counters(self._h, out.ctypes.data, len(out)))
         return {k: int(v) for k, v in zip(self.DEBUG_COUNTERS, out)}
+
+    def debug_probe(self, keys, nodes_out=None, stream=None):
+        """K2 alone: keys = CUDA int64 tensor holding uint64 bits (>= 2); returns the CUDA int32 tensor of node indices."""
+        torch = _torch()
+        if nodes_out is None:
+            nodes_out = torch.empty(keys.numel(), dtype=torch.int32, device="cuda")
+        self._check(self._L.arc_debug_probe(self._h, keys.data_ptr(), keys.numel(), nodes_out.data_ptr(), _stream_ptr(stream)))
+        return nodes_out
 
     def debug_set_key_mask(self, mask: int):
         self._check(self._L.arc_debug_set_key_mask(self._h, mask & 0xFFFFFFFFFFFFFFFF))

@@ -594,6 +594,31 @@ int arc_set_machine(arc_cache* h, int which) {
   return ARC_OK;
 }
 
+int arc_debug_probe(arc_cache* h, const uint64_t* d_keys, uint64_t n, uint32_t* d_nodes_out, void* cuda_stream) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  if (n && (!d_keys || !d_nodes_out)) return fail(h, ARC_ERR_INVALID_ARG, "NULL device pointer");
+  if (n >= (1ull << 31)) return fail(h, ARC_ERR_INVALID_ARG, "too many keys");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int rc = ensure_capacity(h, 1, n, s);
+  if (rc) return rc;
+  rc = maintain(h, n, s);
+  if (rc) return rc;
+  StepParams P = make_params(h);
+  P.keys_acc = const_cast<unsigned long long*>(reinterpret_cast<const unsigned long long*>(d_keys));
+  P.node_acc = d_nodes_out;
+  P.n_access = (uint32_t)n; P.n_req = 0;
+  if (n) {
+    probe_reserve_kernel<<<grid_for(n, 32, 148 * 8), 256, 0, s>>>(P);
+    resolve_nodes_kernel<<<grid_for(n, 256, 148 * 8), 256, 0, s>>>(P);
+    h->launches += 2;
+  }
+  CUDA_TRY(h, cudaGetLastError());
+  // every used slot belongs to a node and this entry creates no tombstones
+  h->slots_used_bound = std::min<uint64_t>(h->slots_used_bound + n, h->node_cap);
+  h->last_stream = s;
+  return ARC_OK;
+}
+
 int arc_debug_set_key_mask(arc_cache* h, uint64_t mask) {
   if (!h) return ARC_ERR_INVALID_ARG;
   h->key_and = mask;

@@ -252,3 +252,23 @@ def test_equal_keys_inside_a_request(arc, machine, bits):
         for n in ("T1", "T2", "B1", "B2"):
             assert np.array_equal(gl[n][0], ol[n][0]) and np.array_equal(gl[n][1], ol[n][1]), n
         gc.close()
+
+
+def test_probe_alone_is_a_consistent_map(arc):
+    """K2 through arc_debug_probe: equal keys get equal nodes, different keys different nodes, lookups repeat."""
+    g = torch.Generator(device="cuda")
+    g.manual_seed(5)
+    n = 300_000
+    keys = torch.randint(2, 2 ** 62, (n,), dtype=torch.int64, device="cuda", generator=g)
+    keys[1000:2000] = keys[0:1000]                      # duplicates inside one launch race for the same slot
+    gc = arc.ArcCache(50_000)
+    nodes = gc.debug_probe(keys).clone()
+    torch.cuda.synchronize()
+    assert torch.equal(nodes[1000:2000], nodes[0:1000])
+    uniq_keys = torch.unique(keys).numel()
+    assert torch.unique(nodes).numel() == uniq_keys
+    again = gc.debug_probe(keys.flip(0))
+    torch.cuda.synchronize()
+    assert torch.equal(again.flip(0), nodes)
+    gc.stats()                                          # no device-side error
+    gc.close()
