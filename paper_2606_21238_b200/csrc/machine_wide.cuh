@@ -22,7 +22,7 @@ struct WideShared {
   uint32_t bad[WIDE_WARPS];
   uint32_t twin[WIDE_WARPS];
   uint32_t found[5], endpos[5], need[5];
-  uint32_t ctl_done, ctl_head[5], ctl_limit[5]; // published by thread 0 before a window's first barrier, read by the scanner warps
+  uint32_t ctl_done, ctl_k, ctl_head[5], ctl_limit[5]; // published by thread 0 before a window's first barrier, read by the scanner warps
   uint32_t set_id[WIDE_SET], set_min[WIDE_SET];
   uint4 vic[5][WIDE_W];                      // per list: entries found from the LRU end {node, block, -, position}
   SerialCtx ctx;                             // the machine state after a by-the-book access done by warp 0
@@ -123,9 +123,23 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
     if (S.ctl_done) break;
     const uint32_t head = S.ctl_head[L], limit = S.ctl_limit[L];
     uint32_t q0 = head & ~3u, found = 0;
+    const int want = (int)S.ctl_k;
     if ((int32_t)(limit - q0) > 0) { found += wide_scan_round(ring, P.ring_mask, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds; }
     __syncthreads();                                   // (B1)
     if (*any_twin) { __syncthreads(); __syncthreads(); }
+    // while the owners roll (not in an all-hit window): up to 2 more rounds, until as many live entries are known as the
+    // window has accesses, so that the owners rarely wait for a scan after the roll
+    bool all_hit = true;
+#pragma unroll
+    for (int u = 0; u < WIDE_WARPS; ++u) {
+      const uint32_t km = bits_from(0, min(32, max(0, want - 32 * u)));
+      const uint32_t m0 = S.m[0][u], m1 = S.m[1][u], m2 = S.m[2][u];
+      const uint32_t hit = (P.policy == POLICY_LRU) ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);
+      all_hit = all_hit && ((hit & km) == km);
+    }
+    for (int it = 0; !all_hit && it < 2 && (int)found < want && (int32_t)(limit - q0) > 0; ++it) {
+      found += wide_scan_round(ring, P.ring_mask, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
+    }
     __syncthreads();                                   // (B2) the owners have published what the window needs
     const uint32_t need = S.need[L];
     while (found < need && (int32_t)(limit - q0) > 0) {
@@ -187,7 +201,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       const int64_t a0 = o + j;
       const bool act0 = tid < k;
       if (tid == 0) {
-        S.ctl_done = 0;
+        S.ctl_done = 0; S.ctl_k = (uint32_t)kmax;
 #pragma unroll
         for (int L = 1; L <= 4; ++L) { S.ctl_head[L] = C.head[L]; S.ctl_limit[L] = (L <= 2) ? C.bound[L] : C.tail[L]; }
       }
