@@ -161,7 +161,7 @@ __device__ __forceinline__ int k1_class(int64_t nb) { return nb >= 1024 ? 0 : nb
 // order (arc_hash_blocks).  ticket: device counter, 0 at launch, reset by the caller's stream work; it runs over
 // K1_PASSES * n_req values: ticket t is request t % n_req in pass t / n_req.
 template <bool ACCESS_ORDER>
-__global__ void __launch_bounds__(256) hash_blocks_kernel(const int32_t* __restrict__ tokens, const int64_t* __restrict__ offsets,
+__global__ void __launch_bounds__(256, 4) hash_blocks_kernel(const int32_t* __restrict__ tokens, const int64_t* __restrict__ offsets,
                                                          const int64_t* __restrict__ blk_off, uint32_t n_req,
                                                          unsigned long long* __restrict__ keys, uint32_t* __restrict__ ticket, uint32_t batch) {
   const int lane = threadIdx.x & 31;
@@ -199,21 +199,28 @@ __global__ void __launch_bounds__(256) hash_blocks_kernel(const int32_t* __restr
       const int64_t ts = offsets[r];
       const int s = (int)((base_mis + ts) & 3);          // tokens of the request's start past a 16-byte boundary (same for every round)
       unsigned long long carry = H_S0;
-      int cnt = (int)min((int64_t)32, nb);
-      RoundVecs nxt = load_round(tok, ts - s, (16 * cnt + s + 3) >> 2, lane, lo, hi);
-      for (int64_t rb = 0; rb < nb; rb += 32) {
-        const RoundVecs cur = nxt;
-        const int cnt_cur = cnt;
-        if (rb + 32 < nb) {
-          cnt = (int)min((int64_t)32, nb - rb - 32);
-          nxt = load_round(tok, ts - s + 16 * (rb + 32), (16 * cnt + s + 3) >> 2, lane, lo, hi);
-        }
-        const unsigned long long st = round_local_scan(cur, s, cnt_cur, lane, LC) + LC.kp * carry;
-        if (lane < cnt_cur) {
+      const int64_t va = ts - s;                         // absolute token index of the aligned cover of round 0
+      // two register buffers ping-pong (no copies): the loads of round i+1 are in flight while round i is hashed
+      auto n_vec = [&](int64_t rb) { return (int)((16 * min((int64_t)32, nb - rb) + s + 3) >> 2); };
+      auto finish = [&](const RoundVecs& cur, int64_t rb) {
+        const int cnt = (int)min((int64_t)32, nb - rb);
+        const unsigned long long st = round_local_scan(cur, s, cnt, lane, LC) + LC.kp * carry;
+        if (lane < cnt) {
           const int64_t i = rb + lane;
           keys[ACCESS_ORDER ? (o + (nb - 1 - i)) : (o + i)] = finalize_key(st);
         }
         carry = shfl64(st, 31);
+      };
+      RoundVecs A = load_round(tok, va, n_vec(0), lane, lo, hi), B;
+      for (int64_t rb = 0;;) {
+        if (rb + 32 < nb) B = load_round(tok, va + 16 * (rb + 32), n_vec(rb + 32), lane, lo, hi);
+        finish(A, rb);
+        rb += 32;
+        if (rb >= nb) break;
+        if (rb + 32 < nb) A = load_round(tok, va + 16 * (rb + 32), n_vec(rb + 32), lane, lo, hi);
+        finish(B, rb);
+        rb += 32;
+        if (rb >= nb) break;
       }
     }
   }
