@@ -56,6 +56,108 @@ __device__ __forceinline__ Roll roll_init(const SerialCtx& C) {
   return R;
 }
 
+// One phase of a run of m ghost hits starting at window position i (ARC).  Returns the number of accesses it covers.
+__device__ __forceinline__ int phase_ghost(Roll& R, int32_t c, uint32_t li, int i, int m, int lane) {
+  int n = 1;
+  // Ghost hit (R5 cases 2, 3).  While delta = 1 the steps of a run are identical as long as the victim keeps coming
+  // from the same list, so the run is rolled in O(1): the regime and its length are computed with selects (no
+  // branches: one warp has no other warp to hide a branch behind); anything else is one by-the-book step.
+  const bool inb2 = (li == L_B2);
+  const int32_t bx = inb2 ? R.b2 : R.b1, by = inb2 ? R.b1 : R.b2;      // bx: the list that was hit
+  const bool d_one = by < 2 * bx;
+  const int32_t p0 = R.p;
+  // B1: REPLACE prefers T1 for the steps j with t1 - j > p + j + 1, i.e. J = (t1 - p) / 2 of them
+  // B2: REPLACE(true) prefers T1 while t1 - j >= 1 and t1 >= p - 1
+  const int32_t J1 = max(0, (R.t1 - R.p) / 2);
+  const bool pref1 = inb2 ? (R.t1 >= 1 && R.t1 >= R.p - 1) : (J1 > 0);
+  const int32_t n_delta = (2 * bx - by + 2) / 3;                         // steps while delta stays 1 when bx shrinks and by grows
+  // regime a: victims from T1;  regime b: victims from T2
+  const bool ra = d_one && pref1 && R.e1 > 0, rb = d_one && !pref1 && R.e2 > 0;
+  int32_t na = min(m, R.e1), nbb = min(m, R.e2);
+  na = inb2 ? min(na, min(n_delta, R.t1)) : min(na, J1);                 // B2+T1 moves b1 up / b2 down; B1+T1 leaves b1, b2
+  nbb = inb2 ? ((R.t1 >= 1) ? min(nbb, R.p - 1 - R.t1) : nbb) : min(nbb, n_delta);
+  if (ra || rb) {
+    n = ra ? na : nbb;
+    const uint32_t run = bits_from(i, n);
+    R.s0 |= ra ? run : 0u; R.s1 |= ra ? 0u : run;
+    R.e1 -= ra ? n : 0; R.e2 -= ra ? 0 : n;
+    R.t1 -= ra ? n : 0; R.t2 += ra ? n : 0;
+    // ghost list sizes: B1+T1 none; B1+T2: b1 -= n, b2 += n; B2+T1: b1 += n, b2 -= n; B2+T2: none
+    const int32_t db1 = (!inb2 && !ra) ? -n : ((inb2 && ra) ? n : 0);
+    R.b1 += db1; R.b2 -= db1;
+    R.p = inb2 ? max(0, R.p - n) : min(c, R.p + n);
+    if (lane >= i) R.my_p = inb2 ? max(0, p0 - min(lane - i + 1, n)) : min(c, p0 + min(lane - i + 1, n));
+  } else {
+    const int32_t d = (by >= 2 * bx && bx > 0) ? by / bx : 1;
+    R.p = inb2 ? max(0, R.p - d) : min(c, R.p + d);
+    roll_replace(R, inb2, i);
+    if (inb2) R.b2--; else R.b1--;
+    R.t2++;
+    if (lane >= i) R.my_p = R.p;
+  }
+  return n;
+}
+
+// One phase of a run of m misses starting at window position i (ARC).  Returns the number of accesses it covers.
+__device__ __forceinline__ int phase_miss(Roll& R, int32_t c, int i, int m) {
+  // the steady state first, on its own short path: full cache, case 4A, T1 above its target, enough evictable entries
+  // for the whole run: drop B1's LRU ghost, evict T1's LRU entry, no counter moves
+  if (R.t1 + R.t2 == c && R.t1 + R.b1 == c && R.t1 < c && R.t1 > R.p && R.e1 >= m) {
+    const uint32_t run = bits_from(i, m);
+    R.s0 |= run; R.d1 |= run; R.e1 -= m;
+    return m;
+  }
+  int n = 1;
+  // Miss (R5 case 4), same idea.  fill: the cache is not full yet (b1 = b2 = 0, I7).  r1: REPLACE takes T1's LRU
+  // entry (t1 stays); r2: T1 is at or below its target, REPLACE takes T2's LRU entry and T1 grows by one per miss.
+  // In case 4A (t1 + b1 = c) B1's LRU ghost is dropped; in case 4B B2's LRU ghost is dropped while b1 + b2 = c.
+  const bool fill = R.t1 + R.t2 < c;
+  const int32_t gapA = c - R.t1 - R.b1, gapS = c - R.b1 - R.b2;
+  const bool isA = gapA == 0, isS = gapS == 0;
+  const bool pref1 = R.t1 > R.p;
+  const bool r1 = !fill && R.t1 < c && pref1 && R.e1 > 0, r2 = !fill && R.t1 < c && !pref1 && R.e2 > 0;
+  const int32_t lim_gap = isA ? m : (isS ? gapA : min(gapA, gapS));     // steps until the case changes
+  const int32_t nf = min(m, c - R.t1 - R.t2);
+  const int32_t n1 = min(min(m, R.e1), lim_gap);
+  const int32_t n2 = min(min(min(m, R.e2), lim_gap), min(R.p - R.t1 + 1, c - R.t1));
+  if (fill || r1 || r2) {
+    n = fill ? nf : (r1 ? n1 : n2);
+    const uint32_t run = bits_from(i, n);
+    R.fm |= fill ? run : 0u;
+    R.s0 |= r1 ? run : 0u; R.s1 |= r2 ? run : 0u;
+    R.d1 |= (!fill && isA) ? run : 0u; R.d2 |= (!fill && !isA && isS) ? run : 0u;
+    R.nf += fill ? n : 0;
+    R.e1 -= r1 ? n : 0; R.e2 -= r2 ? n : 0;
+    R.t1 += (fill || r2) ? n : 0; R.t2 -= r2 ? n : 0;
+    // r1: 4A nothing, 4B b1 += n and (b1 + b2 = c) b2 -= n.   r2: 4A b1 -= n, b2 += n; 4B (b1 + b2 < c) b2 += n
+    R.b1 += (r1 && !isA) ? n : ((r2 && isA) ? -n : 0);
+    R.b2 += (r1 && !isA && isS) ? -n : ((r2 && (isA || !isS)) ? n : 0);
+  } else {                                // pin fallback, or T1 holding everything: one by-the-book step
+    if (isA) {
+      if (R.t1 < c) { R.d1 |= 1u << i; R.b1--; roll_replace(R, false, i); }
+      else { R.s0 |= 1u << i; R.s1 |= 1u << i; R.t1--; R.e1--; if (R.e1 < 0) R.err = DEV_ERR_NO_VICTIM; }
+    } else {
+      if (isS) { R.d2 |= 1u << i; R.b2--; }
+      roll_replace(R, false, i);          // t1 + t2 + b1 + b2 >= c here because the cache is full
+    }
+    R.t1++;
+  }
+  return n;
+}
+
+// One phase of a run of m misses in LRU mode (R10).
+__device__ __forceinline__ int phase_lru_miss(Roll& R, int32_t c, int i, int m) {
+  int n;
+  if (R.t1 < c) {                           // cold fill
+    n = min(m, c - R.t1); R.fm |= bits_from(i, n); R.t1 += n; R.nf += n;
+  } else {                                  // full: every miss evicts T1's LRU entry, no ghost
+    n = max(1, min(m, R.e1));
+    R.s0 |= bits_from(i, n); R.s1 |= bits_from(i, n); R.e1 -= n;
+    if (R.e1 < 0) R.err = DEV_ERR_NO_VICTIM;
+  }
+  return n;
+}
+
 // Rolls k (<= 32) accesses from the state in R; the decision masks of these accesses replace those in R.  lane = this
 // thread's index among the k accesses (my_p is captured for it), or >= 32 when the thread owns none of them.
 // Deliberately NOT inlined: K3 runs one CTA, so instruction fetch is never hidden by other warps and the kernel has to
@@ -75,94 +177,19 @@ __device__ __noinline__ void roll_chunk(Roll& Rio, int32_t c, bool lru, uint32_t
     const uint32_t same = (arc_hit ? ((m0 ^ m1) & ~m2) : (((li & 1u) ? m0 : ~m0) & ((li & 2u) ? m1 : ~m1) & ((li & 4u) ? m2 : ~m2))) & km;
     const uint32_t brk = ~(same >> i);
     const int m = brk ? (__ffs(brk) - 1) : 32;
-    int n = 1;
+    int n;
     if (lru) {
-      if (li == L_T1) {                       // hits: only the evictable count moves
-        n = m; R.e1 -= __popc(me & bits_from(i, n));
-      } else if (R.t1 < c) {                  // cold fill
-        n = min(m, c - R.t1); R.fm |= bits_from(i, n); R.t1 += n; R.nf += n;
-      } else {                                // full: every miss evicts T1's LRU entry, no ghost
-        n = max(1, min(m, R.e1));
-        R.s0 |= bits_from(i, n); R.s1 |= bits_from(i, n); R.e1 -= n;
-        if (R.e1 < 0) R.err = DEV_ERR_NO_VICTIM;
-      }
+      if (li == L_T1) { n = m; R.e1 -= __popc(me & bits_from(i, n)); }      // hits: only the evictable count moves
+      else n = phase_lru_miss(R, c, i, m);
     } else if (arc_hit) {                     // hits: T1 entries move to T2; evictable entries stop being so
       n = m;
       const uint32_t run = bits_from(i, n);
       const int32_t h1 = __popc(m0 & run);
       R.t1 -= h1; R.t2 += h1; R.e1 -= __popc(me & m0 & run); R.e2 -= __popc(me & m1 & run);
     } else if (li == L_B1 || li == L_B2) {
-      // Ghost hit (R5 cases 2, 3).  While delta = 1 the steps of a run are identical as long as the victim keeps coming
-      // from the same list, so the run is rolled in O(1): the regime and its length are computed with selects (no
-      // branches: one warp has no other warp to hide a branch behind); anything else is one by-the-book step.
-      const bool inb2 = (li == L_B2);
-      const int32_t bx = inb2 ? R.b2 : R.b1, by = inb2 ? R.b1 : R.b2;      // bx: the list that was hit
-      const bool d_one = by < 2 * bx;
-      const int32_t p0 = R.p;
-      // B1: REPLACE prefers T1 for the steps j with t1 - j > p + j + 1, i.e. J = (t1 - p) / 2 of them
-      // B2: REPLACE(true) prefers T1 while t1 - j >= 1 and t1 >= p - 1
-      const int32_t J1 = max(0, (R.t1 - R.p) / 2);
-      const bool pref1 = inb2 ? (R.t1 >= 1 && R.t1 >= R.p - 1) : (J1 > 0);
-      const int32_t n_delta = (2 * bx - by + 2) / 3;                         // steps while delta stays 1 when bx shrinks and by grows
-      // regime a: victims from T1;  regime b: victims from T2
-      const bool ra = d_one && pref1 && R.e1 > 0, rb = d_one && !pref1 && R.e2 > 0;
-      int32_t na = min(m, R.e1), nbb = min(m, R.e2);
-      na = inb2 ? min(na, min(n_delta, R.t1)) : min(na, J1);                 // B2+T1 moves b1 up / b2 down; B1+T1 leaves b1, b2
-      nbb = inb2 ? ((R.t1 >= 1) ? min(nbb, R.p - 1 - R.t1) : nbb) : min(nbb, n_delta);
-      if (ra || rb) {
-        n = ra ? na : nbb;
-        const uint32_t run = bits_from(i, n);
-        R.s0 |= ra ? run : 0u; R.s1 |= ra ? 0u : run;
-        R.e1 -= ra ? n : 0; R.e2 -= ra ? 0 : n;
-        R.t1 -= ra ? n : 0; R.t2 += ra ? n : 0;
-        // ghost list sizes: B1+T1 none; B1+T2: b1 -= n, b2 += n; B2+T1: b1 += n, b2 -= n; B2+T2: none
-        const int32_t db1 = (!inb2 && !ra) ? -n : ((inb2 && ra) ? n : 0);
-        R.b1 += db1; R.b2 -= db1;
-        R.p = inb2 ? max(0, R.p - n) : min(c, R.p + n);
-        if (lane >= i) R.my_p = inb2 ? max(0, p0 - min(lane - i + 1, n)) : min(c, p0 + min(lane - i + 1, n));
-      } else {
-        const int32_t d = (by >= 2 * bx && bx > 0) ? by / bx : 1;
-        R.p = inb2 ? max(0, R.p - d) : min(c, R.p + d);
-        roll_replace(R, inb2, i);
-        if (inb2) R.b2--; else R.b1--;
-        R.t2++;
-        if (lane >= i) R.my_p = R.p;
-      }
+      n = phase_ghost(R, c, li, i, m, lane);
     } else {
-      // Miss (R5 case 4), same idea.  fill: the cache is not full yet (b1 = b2 = 0, I7).  r1: REPLACE takes T1's LRU
-      // entry (t1 stays); r2: T1 is at or below its target, REPLACE takes T2's LRU entry and T1 grows by one per miss.
-      // In case 4A (t1 + b1 = c) B1's LRU ghost is dropped; in case 4B B2's LRU ghost is dropped while b1 + b2 = c.
-      const bool fill = R.t1 + R.t2 < c;
-      const int32_t gapA = c - R.t1 - R.b1, gapS = c - R.b1 - R.b2;
-      const bool isA = gapA == 0, isS = gapS == 0;
-      const bool pref1 = R.t1 > R.p;
-      const bool r1 = !fill && R.t1 < c && pref1 && R.e1 > 0, r2 = !fill && R.t1 < c && !pref1 && R.e2 > 0;
-      const int32_t lim_gap = isA ? m : (isS ? gapA : min(gapA, gapS));     // steps until the case changes
-      const int32_t nf = min(m, c - R.t1 - R.t2);
-      const int32_t n1 = min(min(m, R.e1), lim_gap);
-      const int32_t n2 = min(min(min(m, R.e2), lim_gap), min(R.p - R.t1 + 1, c - R.t1));
-      if (fill || r1 || r2) {
-        n = fill ? nf : (r1 ? n1 : n2);
-        const uint32_t run = bits_from(i, n);
-        R.fm |= fill ? run : 0u;
-        R.s0 |= r1 ? run : 0u; R.s1 |= r2 ? run : 0u;
-        R.d1 |= (!fill && isA) ? run : 0u; R.d2 |= (!fill && !isA && isS) ? run : 0u;
-        R.nf += fill ? n : 0;
-        R.e1 -= r1 ? n : 0; R.e2 -= r2 ? n : 0;
-        R.t1 += (fill || r2) ? n : 0; R.t2 -= r2 ? n : 0;
-        // r1: 4A nothing, 4B b1 += n and (b1 + b2 = c) b2 -= n.   r2: 4A b1 -= n, b2 += n; 4B (b1 + b2 < c) b2 += n
-        R.b1 += (r1 && !isA) ? n : ((r2 && isA) ? -n : 0);
-        R.b2 += (r1 && !isA && isS) ? -n : ((r2 && (isA || !isS)) ? n : 0);
-      } else {                                // pin fallback, or T1 holding everything: one by-the-book step
-        if (isA) {
-          if (R.t1 < c) { R.d1 |= 1u << i; R.b1--; roll_replace(R, false, i); }
-          else { R.s0 |= 1u << i; R.s1 |= 1u << i; R.t1--; R.e1--; if (R.e1 < 0) R.err = DEV_ERR_NO_VICTIM; }
-        } else {
-          if (isS) { R.d2 |= 1u << i; R.b2--; }
-          roll_replace(R, false, i);          // t1 + t2 + b1 + b2 >= c here because the cache is full
-        }
-        R.t1++;
-      }
+      n = phase_miss(R, c, i, m);
     }
     i += n;
   }

@@ -69,15 +69,21 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
       const uint32_t m0 = S.m[0][u] & km, m1 = S.m[1][u] & km, m2 = S.m[2][u] & km, me = S.m[3][u] & km;
       Roll& R = D.R;
       const uint32_t hits = lru ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);
+      const uint32_t absent = ~(m0 | m1 | m2) & km, gb1 = m0 & m1 & ~m2, gb2 = m2 & ~m0 & ~m1;
       if (hits == km) {
         // the chunk is all hits: T1 entries move to T2 (ARC); evictable entries stop being so
         if (!lru) { const int32_t h1 = __popc(m0); R.t1 -= h1; R.t2 += h1; R.e2 -= __popc(me & m1); }
         R.e1 -= __popc(me & m0);
         R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = R.p;
-      } else if (!lru && (m0 | m1 | m2) == 0 && R.t1 + R.b1 == c && R.t1 < c && R.t1 > R.p && R.e1 >= ku && R.t1 + R.t2 == c) {
-        // the chunk is all misses at the fixed point of case 4A: drop B1's LRU ghost, evict T1's LRU entry, no counter moves
-        R.e1 -= ku;
-        R.s0 = km; R.d1 = km; R.s1 = R.d2 = R.fm = 0; R.my_p = R.p;
+      } else if (absent == km || (!lru && (gb1 == km || gb2 == km))) {
+        // the chunk is one run of misses or of ghost hits: its phases are rolled here, without the call
+        R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = R.p;
+        const uint32_t li = (absent == km) ? L_ABSENT : ((gb1 == km) ? L_B1 : L_B2);
+        const int my = (u == warp) ? lane : 64;
+        for (int i = 0; i < ku;) {
+          R.phases++;
+          i += (li == L_ABSENT) ? (lru ? phase_lru_miss(R, c, i, ku - i) : phase_miss(R, c, i, ku - i)) : phase_ghost(R, c, li, i, ku - i, my);
+        }
       } else {
         Roll T = D.R;                                // the callee is not inlined: keep D.R itself in registers
         roll_chunk(T, c, lru, S.m[0][u], S.m[1][u], S.m[2][u], S.m[3][u], ku, (u == warp) ? lane : 64);
