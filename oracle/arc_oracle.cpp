@@ -72,7 +72,7 @@ void request_keys(const int32_t* t, int64_t len, uint32_t B, uint64_t* out) {
 
 enum { MISS = 0, HIT_T1 = 1, HIT_T2 = 2, GHOST_B1 = 3, GHOST_B2 = 4 };
 enum { IN_T1 = 1, IN_T2 = 2, IN_B1 = 3, IN_B2 = 4 };
-enum { POLICY_ARC = 0, POLICY_LRU = 1 };
+enum { POLICY_ARC = 0, POLICY_LRU = 1, POLICY_DBL = 2 };   // DBL = ARC's lists with p frozen at c/2
 enum { OK = 0, ERR_INVALID_ARG = -1, ERR_UNSUPPORTED = -2, ERR_REQUEST_TOO_LARGE = -3, ERR_OOM = -4 };
 
 typedef std::list<uint64_t> KeyList;  // front = LRU end, back = MRU end
@@ -230,13 +230,13 @@ void access(oracle_cache* h, uint64_t x, uint8_t* cls_out, int32_t* block_out, i
   } else if (f != h->dir.end() && f->second.where == IN_B1) {  // case 2
     cls = GHOST_B1; h->st.ghost_b1++;
     uint64_t delta = b2 / b1; if (delta < 1) delta = 1;          // R6: floor, at least 1
-    h->p = (h->p + delta > c) ? c : h->p + delta;
+    if (h->policy != POLICY_DBL) h->p = (h->p + delta > c) ? c : h->p + delta;   // DBL: no adaptation
     int32_t v = evicted = replace(h, false);
     remove_key(h, x); put_mru(h, x, IN_T2, v);
   } else if (f != h->dir.end() && f->second.where == IN_B2) {  // case 3
     cls = GHOST_B2; h->st.ghost_b2++;
     uint64_t delta = b1 / b2; if (delta < 1) delta = 1;
-    h->p = (h->p < delta) ? 0 : h->p - delta;
+    if (h->policy != POLICY_DBL) h->p = (h->p < delta) ? 0 : h->p - delta;
     int32_t v = evicted = replace(h, true);
     remove_key(h, x); put_mru(h, x, IN_T2, v);
   } else {  // case 4
@@ -314,10 +314,11 @@ int oracle_create(uint64_t capacity_blocks, uint32_t block_size, int policy, ora
   if (!out) return ERR_INVALID_ARG;
   *out = 0;
   if (capacity_blocks == 0 || capacity_blocks > 0x7FFFFFFEull) return ERR_INVALID_ARG;
-  if (policy != POLICY_ARC && policy != POLICY_LRU) return ERR_INVALID_ARG;
+  if (policy != POLICY_ARC && policy != POLICY_LRU && policy != POLICY_DBL) return ERR_INVALID_ARG;
   if (block_size == 0 || (block_size & 1)) return ERR_UNSUPPORTED;   // the hash is defined for even B
   oracle_cache* h = new oracle_cache();
-  h->c = capacity_blocks; h->B = block_size; h->policy = policy; h->p = 0; h->next_fresh = 0;
+  h->c = capacity_blocks; h->B = block_size; h->policy = policy; h->next_fresh = 0;
+  h->p = (policy == POLICY_DBL) ? capacity_blocks / 2 : 0;   // DBL: the fixed 1:1 split
   std::memset(&h->st, 0, sizeof(h->st));
   h->hash_seconds = h->arc_seconds = 0.0;
   *out = h;

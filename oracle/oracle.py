@@ -17,7 +17,7 @@ _SRC = _HERE / "arc_oracle.cpp"
 _LIB = _HERE / "liboracle.so"
 
 MISS, HIT_T1, HIT_T2, GHOST_B1, GHOST_B2 = 0, 1, 2, 3, 4
-POLICY_ARC, POLICY_LRU = 0, 1
+POLICY_ARC, POLICY_LRU, POLICY_DBL = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_REQUEST_TOO_LARGE = 0, -1, -2, -3
 
 STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", "hit_t1", "hit_t2", "ghost_b1",

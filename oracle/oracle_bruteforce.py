@@ -83,7 +83,7 @@ def block_keys(tokens, block_size=16):
 
 # ---- classes / codes (numbers fixed by the C ABI contract) ----------------
 MISS, HIT_T1, HIT_T2, GHOST_B1, GHOST_B2 = 0, 1, 2, 3, 4
-POLICY_ARC, POLICY_LRU = 0, 1
+POLICY_ARC, POLICY_LRU, POLICY_DBL = 0, 1, 2   # DBL: ARC's lists with p frozen at c // 2
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_REQUEST_TOO_LARGE = 0, -1, -2, -3
 
 
@@ -94,7 +94,7 @@ class BruteForceCache:
         assert capacity_blocks >= 1 and block_size % 2 == 0
         self.c, self.B, self.policy = capacity_blocks, block_size, policy
         self.T1, self.T2, self.B1, self.B2 = [], [], [], []
-        self.p = 0
+        self.p = capacity_blocks // 2 if policy == POLICY_DBL else 0
         self.block_of = {}  # resident key -> block ID (ghosts hold no ID, I8)
         self.next_fresh = 0
         self.pinned = set()
@@ -169,7 +169,8 @@ class BruteForceCache:
             cls = GHOST_B1
             st["ghost_b1"] += 1
             delta = max(1, b2 // b1)
-            self.p = min(c, self.p + delta)
+            if self.policy != POLICY_DBL:  # DBL: no adaptation
+                self.p = min(c, self.p + delta)
             v = evicted = self._replace(False)
             self.B1.remove(x)
             self.T2.append(x)
@@ -178,7 +179,8 @@ class BruteForceCache:
             cls = GHOST_B2
             st["ghost_b2"] += 1
             delta = max(1, b1 // b2)
-            self.p = max(0, self.p - delta)
+            if self.policy != POLICY_DBL:
+                self.p = max(0, self.p - delta)
             v = evicted = self._replace(True)
             self.B2.remove(x)
             self.T2.append(x)

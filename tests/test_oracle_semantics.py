@@ -30,19 +30,19 @@ def _random_key_requests(rng, c, n_req, alphabet):
     return reqs
 
 
-@pytest.mark.parametrize("policy", [0, 1])
+@pytest.mark.parametrize("policy", [0, 1, 2])
 def test_invariants_after_every_access_bruteforce(policy):
     rng = np.random.default_rng(10 + policy)
     for c in (1, 2, 3, 5, 8):
         cache = BF.BruteForceCache(c, 16, policy)
         alphabet = np.arange(2, 2 + 3 * c)
-        prev_p = 0
+        prev_p = cache.p
         for _ in range(600):
             if len(cache.pinned) >= c:   # a request has at most c blocks (R4)
                 cache.pinned.clear()
             x = int(rng.choice(alphabet))
             cls, bid, evi = cache.access(x)
-            check_invariants(_bf_lists(cache), c, policy_lru=bool(policy), pinned=cache.pinned)
+            check_invariants(_bf_lists(cache), c, policy_lru=(policy == 1), pinned=cache.pinned)
             if cls not in (O.GHOST_B1, O.GHOST_B2):
                 assert cache.p == prev_p, "I12: p moves only on ghost hits"
             prev_p = cache.p
@@ -53,7 +53,7 @@ def test_invariants_after_every_access_bruteforce(policy):
                 cache.pinned.clear()   # request boundary
 
 
-@pytest.mark.parametrize("policy", [0, 1])
+@pytest.mark.parametrize("policy", [0, 1, 2])
 def test_invariants_cpp_config1(policy):
     tr = W.make_trace(1, seed=0)
     cache = O.OracleCache(64, 16, policy)
@@ -63,7 +63,7 @@ def test_invariants_cpp_config1(policy):
         for r in range(len(offsets) - 1):
             out = cache.step(tokens[offsets[r]:offsets[r + 1]], [0, offsets[r + 1] - offsets[r]])
             L = cache.lists()
-            check_invariants(L, 64, policy_lru=bool(policy))
+            check_invariants(L, 64, policy_lru=(policy == 1))
             full = len(L["T1"][0]) + len(L["T2"][0]) == 64
             assert full or not prev_full, "I7: once full, stays full"
             prev_full = full
@@ -78,7 +78,7 @@ def test_invariants_cpp_config1(policy):
     assert st["evict_t1"] + st["evict_t2"] == st["accesses"] - st["hit_t1"] - st["hit_t2"] - 64, "I10 over the run"
 
 
-@pytest.mark.parametrize("policy", [0, 1])
+@pytest.mark.parametrize("policy", [0, 1, 2])
 def test_differential_cpp_vs_bruteforce_keys(policy):
     """>= 10^4 random traces on c in 1..8, alphabet <= 3c, requests of 1..min(c,4) blocks; every output compared."""
     rng = np.random.default_rng(100 + policy)
@@ -107,7 +107,7 @@ def test_differential_tokens_prefix_trees():
     rng = np.random.default_rng(7)
     for rep in range(150):
         c = int(rng.integers(1, 9))
-        for policy in (0, 1):
+        for policy in (0, 1, 2):
             bf, cpp = BF.BruteForceCache(c, 16, policy), O.OracleCache(c, 16, policy)
             reqs = W.prefix_tree_requests(rng, n_requests=12, block_size=16, branching=2, depth=3, max_blocks=min(c, 4))
             for s in range(0, 12, 4):
@@ -157,7 +157,7 @@ def test_arc_equals_lru_on_pure_recency_traces():
     _same_outputs(16, [list(range(100 + 5 * i, 100 + 5 * i + 5)) for i in range(40)])     # (i) with multi-block requests
 
 
-@pytest.mark.parametrize("policy", [0, 1])
+@pytest.mark.parametrize("policy", [0, 1, 2])
 def test_step_partition_invariance(policy):
     """R3 / PAPER.md:129: the same request stream cut into steps of 1, 7, 64 or all at once gives identical
     concatenated outputs."""
@@ -263,3 +263,21 @@ def test_scan_resistance_config4_shape():
                 acc += int(hot_mask.sum())
         rates[policy] = hits / acc
     assert rates[O.POLICY_ARC] > rates[O.POLICY_LRU] + 0.3, rates
+
+
+def test_dbl_never_moves_p_and_equals_arc_without_resident_pressure():
+    """DBL (PAPER.md:101, :109): p stays at c // 2 whatever is accessed; on a working set that fits the cache
+    (no eviction ever) DBL, ARC and LRU agree on classes and block IDs."""
+    rng = np.random.default_rng(77)
+    c = 16
+    dbl = O.OracleCache(c, 16, O.POLICY_DBL)
+    for _ in range(300):
+        out = dbl.step_keys([[int(k) for k in rng.integers(2, 60, size=int(rng.integers(1, 5)))]])
+        assert set(out["p_after"].tolist()) <= {c // 2}
+    assert dbl.stats()["p"] == c // 2
+    a, d = O.OracleCache(c, 16, O.POLICY_ARC), O.OracleCache(c, 16, O.POLICY_DBL)
+    for _ in range(200):
+        req = [[int(k) for k in rng.integers(2, 2 + c, size=int(rng.integers(1, 4)))]]
+        oa, od = a.step_keys(req), d.step_keys(req)
+        for k in ("cls", "block_id", "evicted_id", "prefix_len"):
+            assert np.array_equal(oa[k], od[k]), k

@@ -24,12 +24,12 @@ def _replay(trace_file, c, policy, impl, compare_lists=True, lru_classes=False):
             assert int(out["cls"][i]) == want_cls, (trace_file, acc)
             assert int(out["block_id"][i]) == acc["id"], (trace_file, acc)
             assert int(out["evicted_id"][i]) == acc["evicted"], (trace_file, acc)
-            if policy == 0:
+            if policy in (0, 2):
                 assert int(out["p_after"][i]) == acc["p"], (trace_file, acc)
         if r["prefix_len"] is not None:
             assert int(out["prefix_len"][0]) == r["prefix_len"]
         # the fixture gives the lists after every access; after the request's LAST access they must match
-        if compare_lists and policy == 0:
+        if compare_lists and policy in (0, 2):
             L = cache.lists()
             got = [names.names(L[n] if impl == "bf" else L[n][0]) for n in ("T1", "T2", "B1", "B2")]
             assert got == r["accesses"][-1]["lists"], (trace_file, r["accesses"][-1])
@@ -62,6 +62,25 @@ def test_trace_C(impl):
 def test_trace_D_and_E(impl):
     _replay("trace_DE.txt", 2, 0, impl)
     _replay("trace_DE.txt", 2, 1, impl, lru_classes=True)
+
+
+@pytest.mark.parametrize("impl", ["bf", "cpp"])
+def test_trace_F_dbl(impl):
+    """DBL = ARC's lists and REPLACE with p frozen at c // 2 (PAPER.md:101, :109)."""
+    _replay("trace_F.txt", 4, 2, impl)
+
+
+def test_trace_F_intermediate_lists():
+    reqs = parse_trace("trace_F.txt")
+    names = KeyNames()
+    for impl in ("bf", "cpp"):
+        cache = BF.BruteForceCache(4, 16, 2) if impl == "bf" else O.OracleCache(4, 16, 2)
+        for r in reqs:
+            cache.step_keys([[names.key(r["keys"][0])]])
+            L = cache.lists()
+            got = [names.names(L[n] if impl == "bf" else L[n][0]) for n in ("T1", "T2", "B1", "B2")]
+            assert got == r["accesses"][0]["lists"], r
+            assert L["p"] == 2
 
 
 def test_trace_A_intermediate_lists_bruteforce():
