@@ -31,7 +31,8 @@ extern "C" {
 
 typedef struct arc_cache arc_cache; /* opaque, owned by the library */
 
-enum { ARC_POLICY_ARC = 0, ARC_POLICY_LRU = 1 };
+enum { ARC_POLICY_ARC = 0, ARC_POLICY_LRU = 1,
+       ARC_POLICY_DBL = 2 /* ARC's lists and REPLACE with p frozen at capacity_blocks / 2: the paper's DBL ablation */ };
 enum {
   ARC_OK = 0,
   ARC_ERR_INVALID_ARG = -1,       /* NULL pointer, capacity 0 or > 2^31-2, n_req > 2^20, offsets not monotone, bad policy */
@@ -54,7 +55,7 @@ typedef struct {
   const uint8_t *cls;        /* [N]        ARC_MISS .. ARC_GHOST_B2                                        */
   const int32_t *block_id;   /* [N]        physical block now holding the logical block, in [0, capacity)  */
   const int32_t *evicted_id; /* [N]        block ID evicted by this access, or -1                          */
-  const int32_t *p_after;    /* [N]        p (target size of T1) after this access; 0 in LRU mode          */
+  const int32_t *p_after;    /* [N]        p (target size of T1) after this access; 0 in LRU, c/2 in DBL mode */
   const int32_t *alloc_ids;  /* [counts[0]] IDs handed to non-hit accesses, in ACCESS order (R2)           */
   const int32_t *evict_ids;  /* [counts[1]] IDs evicted, in ACCESS order                                   */
   const uint32_t *counts;    /* [2]        n_alloc, n_evict                                                */

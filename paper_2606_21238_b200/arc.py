@@ -14,7 +14,7 @@ import numpy as np
 
 from . import build as _build
 
-POLICY_ARC, POLICY_LRU = 0, 1
+POLICY_ARC, POLICY_LRU, POLICY_DBL = 0, 1, 2
 MISS, HIT_T1, HIT_T2, GHOST_B1, GHOST_B2 = 0, 1, 2, 3, 4
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_REQUEST_TOO_LARGE, ERR_OOM, ERR_CUDA = 0, -1, -2, -3, -4, -5
 

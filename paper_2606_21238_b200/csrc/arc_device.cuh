@@ -25,7 +25,7 @@ constexpr uint32_t SLOT_FLAG = 0x80000000u;      // node_acc entry holds a slot 
 constexpr uint32_t BUCKET_SLOTS = 8;             // 8 x 16 B = one 128 B line
 
 enum : int { CLS_MISS = 0, CLS_HIT_T1 = 1, CLS_HIT_T2 = 2, CLS_GHOST_B1 = 3, CLS_GHOST_B2 = 4 };
-enum : int { POLICY_ARC = 0, POLICY_LRU = 1 };
+enum : int { POLICY_ARC = 0, POLICY_LRU = 1, POLICY_DBL = 2 };
 
 // Ring entry: low word = node id (RING_TOMB once the node has left that position by a hit / ghost hit), high word = the
 // block id the node held when it was pushed.  Inside [head, tail) an entry is live iff it is not a tombstone; the node

@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(StepParams P) {
 // ---------------------------------------------------------------------------------------------------
 // Maintenance
 
-__global__ void init_state_kernel(DevState* st, Node* nodes, uint32_t* free_stack, uint32_t node_cap) {
+__global__ void init_state_kernel(DevState* st, Node* nodes, uint32_t* free_stack, uint32_t node_cap, int32_t p0) {
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
   for (uint32_t i = tid; i < node_cap; i += gridDim.x * blockDim.x) {
     st_node(nodes + i, L_FREE, 0, -1, 0);
@@ -129,6 +129,7 @@ __global__ void init_state_kernel(DevState* st, Node* nodes, uint32_t* free_stac
     DevState z;
     memset(&z, 0, sizeof(z));
     z.free_top = node_cap;
+    z.p = p0;                           // 0, or capacity / 2 for the DBL policy
     *st = z;
   }
 }

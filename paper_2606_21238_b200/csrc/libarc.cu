@@ -224,7 +224,7 @@ int ensure_capacity(arc_cache* h, uint32_t n_req, uint64_t N, cudaStream_t s) {
     CUDA_TRY(h, dalloc(&h->d_block_counts, std::max<uint32_t>(1, ring_cap / CMP_THREADS)));
     h->node_cap = node_cap; h->table_slots = table_slots; h->ring_cap = ring_cap;
     CUDA_TRY(h, cudaMemsetAsync(h->d_table, 0, (size_t)table_slots * sizeof(Slot), s));
-    init_state_kernel<<<grid_for(node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, h->d_nodes, h->d_free_stack, node_cap);
+    init_state_kernel<<<grid_for(node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, h->d_nodes, h->d_free_stack, node_cap, (h->policy == ARC_POLICY_DBL) ? (int32_t)(h->c / 2) : 0);
     h->launches += 1;
     CUDA_TRY(h, cudaGetLastError());
     h->slots_used_bound = 0;
@@ -321,7 +321,7 @@ int arc_create(uint64_t capacity_blocks, uint32_t block_size, int policy, arc_ca
   if (!out) return fail(nullptr, ARC_ERR_INVALID_ARG, "out is NULL");
   *out = nullptr;
   if (capacity_blocks == 0 || capacity_blocks > 0x7FFFFFFEull) return fail(nullptr, ARC_ERR_INVALID_ARG, "capacity_blocks out of range");
-  if (policy != ARC_POLICY_ARC && policy != ARC_POLICY_LRU) return fail(nullptr, ARC_ERR_INVALID_ARG, "unknown policy %d", policy);
+  if (policy != ARC_POLICY_ARC && policy != ARC_POLICY_LRU && policy != ARC_POLICY_DBL) return fail(nullptr, ARC_ERR_INVALID_ARG, "unknown policy %d", policy);
   if (block_size != 16) return fail(nullptr, ARC_ERR_UNSUPPORTED, "block_size %u: only 16 is built", block_size);
   if (capacity_blocks > kMaxCapacity) return fail(nullptr, ARC_ERR_UNSUPPORTED, "capacity_blocks > 2^28");
   arc_cache* h = new (std::nothrow) arc_cache();
@@ -492,7 +492,7 @@ int arc_reset(arc_cache* h) {
   if (!h) return ARC_ERR_INVALID_ARG;
   cudaStream_t s = h->last_stream;
   CUDA_TRY(h, cudaMemsetAsync(h->d_table, 0, (size_t)h->table_slots * sizeof(Slot), s));
-  init_state_kernel<<<grid_for(h->node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, h->d_nodes, h->d_free_stack, h->node_cap);
+  init_state_kernel<<<grid_for(h->node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, h->d_nodes, h->d_free_stack, h->node_cap, (h->policy == ARC_POLICY_DBL) ? (int32_t)(h->c / 2) : 0);
   CUDA_TRY(h, cudaGetLastError());
   CUDA_TRY(h, cudaStreamSynchronize(s));
   h->slots_used_bound = 0;

@@ -35,6 +35,7 @@ struct Roll {
   int32_t my_p;        // p after this lane's access
   uint32_t err;
   uint32_t calls, phases;   // diagnostics
+  bool dbl;                 // DBL policy: p never moves
 };
 
 __device__ __forceinline__ uint32_t bits_from(int i, int n) { return ((n >= 32) ? 0xFFFFFFFFu : ((1u << n) - 1u)) << i; }
@@ -52,13 +53,34 @@ __device__ __forceinline__ void roll_replace(Roll& R, bool inb2, int i) {
 __device__ __forceinline__ Roll roll_init(const SerialCtx& C) {
   Roll R;
   R.t1 = C.t1; R.t2 = C.t2; R.b1 = C.b1; R.b2 = C.b2; R.p = C.p; R.nf = C.next_fresh; R.e1 = C.elig1; R.e2 = C.elig2;
-  R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = C.p; R.err = 0; R.calls = 0; R.phases = 0;
+  R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = C.p; R.err = 0; R.calls = 0; R.phases = 0; R.dbl = C.dbl;
   return R;
 }
 
 // One phase of a run of m ghost hits starting at window position i (ARC).  Returns the number of accesses it covers.
 __device__ __forceinline__ int phase_ghost(Roll& R, int32_t c, uint32_t li, int i, int m, int lane) {
   int n = 1;
+  if (R.dbl) {
+    // DBL: p is frozen.  B1: REPLACE prefers T1 while t1 > p; B2: while t1 >= max(p, 1).  Victims from T1 shrink t1 by one
+    // per step (regime a), victims from T2 change nothing that REPLACE looks at (regime b).
+    const bool inb2 = (li == L_B2);
+    const bool pref1 = inb2 ? (R.t1 >= 1 && R.t1 >= R.p) : (R.t1 > R.p);
+    const bool ra = pref1 && R.e1 > 0, rb = !pref1 && R.e2 > 0;
+    if (ra || rb) {
+      n = ra ? min(min(m, R.e1), inb2 ? (R.t1 - max(R.p, 1) + 1) : (R.t1 - R.p)) : min(m, R.e2);
+      const uint32_t run = bits_from(i, n);
+      R.s0 |= ra ? run : 0u; R.s1 |= ra ? 0u : run;
+      R.e1 -= ra ? n : 0; R.e2 -= ra ? 0 : n;
+      R.t1 -= ra ? n : 0; R.t2 += ra ? n : 0;
+      const int32_t db1 = (!inb2 && !ra) ? -n : ((inb2 && ra) ? n : 0);   // B1+T2: b1 -= n, b2 += n; B2+T1: b1 += n, b2 -= n
+      R.b1 += db1; R.b2 -= db1;
+    } else {
+      roll_replace(R, inb2, i);
+      if (inb2) R.b2--; else R.b1--;
+      R.t2++;
+    }
+    return n;
+  }
   // Ghost hit (R5 cases 2, 3).  While delta = 1 the steps of a run are identical as long as the victim keeps coming
   // from the same list, so the run is rolled in O(1): the regime and its length are computed with selects (no
   // branches: one warp has no other warp to hide a branch behind); anything else is one by-the-book step.

@@ -14,6 +14,7 @@ struct SerialCtx {
   uint32_t stat[ST_COUNT];   // per-step deltas (a step has < 2^31 accesses)
   uint32_t err;
   uint32_t n_alloc, n_evict;
+  bool dbl;              // DBL policy: p is frozen at capacity / 2
 };
 
 template <uint32_t L>
@@ -90,6 +91,7 @@ __device__ __forceinline__ void ctx_load(SerialCtx& C, const StepParams& P) {
   for (int L = 1; L <= 4; ++L) { C.head[L] = S->head[L]; C.tail[L] = S->tail[L]; C.bound[L] = S->tail[L]; }
   C.t1 = S->t1; C.t2 = S->t2; C.b1 = S->b1; C.b2 = S->b2; C.p = S->p; C.next_fresh = S->next_fresh;
   C.elig1 = C.t1; C.elig2 = C.t2;
+  C.dbl = (P.policy == POLICY_DBL);
 #pragma unroll
   for (int i = 0; i < ST_COUNT; ++i) C.stat[i] = 0;
   C.err = 0;
@@ -155,14 +157,14 @@ __device__ __noinline__ void serial_access(SerialCtx& C, const StepParams& P, in
   } else if (rec.list == L_B1) {                          // case 2
     cls = CLS_GHOST_B1; C.stat[ST_GHOST_B1]++;
     int32_t delta = C.b2 / C.b1; if (delta < 1) delta = 1;
-    C.p = min(c, C.p + delta);
+    if (P.policy != POLICY_DBL) C.p = min(c, C.p + delta);      // DBL: no adaptation
     blk = ev = replace_serial(C, P, false);
     C.b1--; C.t2++;
     ring_push<L_T2>(C, P, n, blk, rec.slot);
   } else if (rec.list == L_B2) {                          // case 3
     cls = CLS_GHOST_B2; C.stat[ST_GHOST_B2]++;
     int32_t delta = C.b1 / C.b2; if (delta < 1) delta = 1;
-    C.p = max(0, C.p - delta);
+    if (P.policy != POLICY_DBL) C.p = max(0, C.p - delta);
     blk = ev = replace_serial(C, P, true);
     C.b2--; C.t2++;
     ring_push<L_T2>(C, P, n, blk, rec.slot);

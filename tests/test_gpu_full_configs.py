@@ -18,7 +18,7 @@ STAT_KEYS = ("steps", "requests", "tokens_seen", "tokens_hashed", "accesses", "h
              "b1", "b2", "p")
 
 
-@pytest.mark.parametrize("config,max_steps,policy", [(2, None, 0), (2, 300, 1), (3, None, 0), (4, 500, 0), (4, 60, 1), (5, 120, 0)])
+@pytest.mark.parametrize("config,max_steps,policy", [(2, None, 0), (2, 300, 1), (2, None, 2), (3, None, 0), (3, 400, 2), (4, 500, 0), (4, 60, 1), (5, 120, 0)])
 def test_full_size_config(config, max_steps, policy):
     if not torch.cuda.is_available():
         pytest.fail("-m gpu tests need a CUDA device")

@@ -93,7 +93,7 @@ def test_hash_parity_configs(arc, config):
 # ------------------------------------------------------------------------------- whole arc_step
 
 @pytest.mark.parametrize("machine", [0, 1, 2])
-@pytest.mark.parametrize("policy", [0, 1])
+@pytest.mark.parametrize("policy", [0, 1, 2])
 def test_config1_full_trace(arc, policy, machine):
     """BASELINE.json configs[0]: c = 64, 2,000 requests, 8 per step, ARC and LRU, every output of every step."""
     tr = W.make_trace(1, seed=0)
@@ -110,7 +110,7 @@ def test_larger_configs_scaled(arc, config, scale, max_steps, machine):
     run_trace(arc, tr.steps(max_steps=max_steps), tr.info.capacity_blocks, 0, machine, ctx=f"config{config} m{machine}")
 
 
-@pytest.mark.parametrize("policy", [0, 1])
+@pytest.mark.parametrize("policy", [0, 1, 2])
 def test_config2_lru_and_small_cache_pressure(arc, policy):
     """Config-2 shaped requests against a cache of 600 blocks: constant eviction, ghost churn, pin fallbacks."""
     tr = W.make_trace(2, seed=5, scale=0.01)
@@ -125,7 +125,7 @@ def test_tiny_caches_prefix_trees(arc, c, machine):
     """Adversarial micro-traces: duplicate requests inside one step, keys dropped from a ghost list and
     re-accessed in the same step, requests of exactly c blocks, empty and sub-block requests."""
     rng = np.random.default_rng(100 + c)
-    for policy in (0, 1):
+    for policy in (0, 1, 2):
         gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
         gc.set_machine(machine)
         for step in range(60):
@@ -174,7 +174,7 @@ def test_errors_leave_state_unchanged(arc):
     assert_same_step(gc.step(dev(toks[:40]), [0, 0, 15, 15, 40]).to_host(), oc.step(toks[:40], [0, 0, 15, 15, 40]))
     assert_same_step(gc.step(dev(toks[:0]), [0]).to_host(), oc.step(toks[:0], [0]))
     assert_same_state(gc, oc, "after empty steps")
-    for bad in ((0, 16, 0), (4, 15, 0), (4, 16, 9)):
+    for bad in ((0, 16, 0), (4, 15, 0), (4, 16, 3), (4, 16, 9)):
         with pytest.raises(arc.ArcError):
             arc.ArcCache(*bad)
     gc.close()
@@ -232,7 +232,7 @@ def test_equal_keys_inside_a_request(arc, machine, bits):
     it): the second access is a hit on a block its own request has pinned.  Exercises the window cuts at repeated nodes."""
     rng = np.random.default_rng(40 + bits)
     mask = (1 << bits) - 1
-    for policy in (0, 1):
+    for policy in (0, 1, 2):
         c = 40
         gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
         gc.set_machine(machine)
