@@ -364,8 +364,11 @@ def run_ours(args):
         c3, _, _, _ = run_device_resident(torch, A, info, steps, dev, bases, W_, A.POLICY_LRU, stream)
         st_lru = c3.stats()
         c3.close()
+        c4, _, _, _ = run_device_resident(torch, A, info, steps, dev, bases, W_, A.POLICY_DBL, stream)
+        st_dbl = c4.stats()
+        c4.close()
         ha, hl = hit_rates(st_arc), hit_rates(st_lru)
-        line["hit_rate"] = {"arc": ha, "lru": hl,
+        line["hit_rate"] = {"arc": ha, "lru": hl, "dbl": hit_rates(st_dbl),
                             "arc_minus_lru_points": {k: 100 * (ha[k] - hl[k]) for k in ha},
                             "scope": f"all {W_ + K} steps from an empty cache",
                             "paper_context": "+10.8% hit rate / -12.6% TTFT (doc QA), +2.1% / -2.0% (conversation): Qwen3-14B, vLLM, 1x H100 PCIe 80 GB (PAPER.md:7, :86, :111, :117)"}
