@@ -151,9 +151,10 @@ int arc_last_kernel_times(arc_cache *h, arc_kernel_times *out);
  * are counted in a process-wide counter returned when h == NULL). */
 uint64_t arc_launch_count(const arc_cache *h);
 
-/* Selects the K3 implementation: 0 = four-warp machine with 128-access windows (default), 1 = single-thread
- * serial walk (correctness reference on the device; same results, much slower), 2 = one-warp machine with
- * 32-access windows. */
+/* Selects the K3 implementation (all give identical results): 0 = automatic (default): the wide machine, or the
+ * one-warp machine for steps whose requests average fewer than 48 blocks; 1 = single-thread serial walk (the by-the-book
+ * routine on the device, much slower); 2 = one-warp machine with 32-access windows; 3 = wide machine: one CTA of 8 warps,
+ * 128-access windows. */
 int arc_set_machine(arc_cache *h, int which);
 
 /* K2 alone, for the probe microbenchmark and its tests: looks every key of d_keys (DEVICE uint64[n], values >= 2) up in

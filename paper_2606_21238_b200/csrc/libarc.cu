@@ -56,7 +56,7 @@ struct arc_cache {
   uint32_t B = 16;
   int policy = 0;
   unsigned long long key_and = ~0ull;   // test hook
-  int machine = 0;            // 0 wide (4 warps), 1 serial, 2 one-warp batched
+  int machine = 0;            // 0 auto (wide, or one-warp when requests are short), 1 serial, 2 one-warp, 3 wide
   // capacities
   uint64_t n_cap = 0;         // max full blocks per step the buffers are sized for
   uint32_t req_cap = 0;
@@ -399,8 +399,10 @@ int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, ui
   if (h->profiling) cudaEventRecord(h->ev[3], s);
   if (h->machine == 1) {
     arc_machine_serial_kernel<<<1, 32, 0, s>>>(P);                                                       // K3 (serial)
-  } else if (h->machine == 2) {
-    launch_machine_batched(P, s);                                                                        // K3 (one warp, 32-wide windows)
+  } else if (h->machine == 2 || (h->machine == 0 && N < 48ull * n_req)) {
+    // one warp, 32-wide windows: a window of the wide machine costs about twice as much, which only pays when requests
+    // are long enough to fill it (windows never cross a request boundary)
+    launch_machine_batched(P, s);
   } else {
     launch_machine_wide(P, s);                                                                           // K3 (four warps, 128-wide windows)
   }
@@ -589,7 +591,7 @@ int arc_last_kernel_times(arc_cache* h, arc_kernel_times* out) {
 uint64_t arc_launch_count(const arc_cache* h) { return h ? h->launches : g_hash_launches; }
 
 int arc_set_machine(arc_cache* h, int which) {
-  if (!h || which < 0 || which > 2) return ARC_ERR_INVALID_ARG;
+  if (!h || which < 0 || which > 3) return ARC_ERR_INVALID_ARG;
   h->machine = which;
   return ARC_OK;
 }

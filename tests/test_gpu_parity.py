@@ -92,7 +92,7 @@ def test_hash_parity_configs(arc, config):
 
 # ------------------------------------------------------------------------------- whole arc_step
 
-@pytest.mark.parametrize("machine", [0, 1, 2])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3])
 @pytest.mark.parametrize("policy", [0, 1, 2])
 def test_config1_full_trace(arc, policy, machine):
     """BASELINE.json configs[0]: c = 64, 2,000 requests, 8 per step, ARC and LRU, every output of every step."""
@@ -101,7 +101,7 @@ def test_config1_full_trace(arc, policy, machine):
     assert st["requests"] == 2000
 
 
-@pytest.mark.parametrize("machine", [0, 1, 2])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3])
 @pytest.mark.parametrize("config,scale,max_steps", [(2, 0.06, 40), (3, 0.03, 40), (4, 0.004, 8)])
 def test_larger_configs_scaled(arc, config, scale, max_steps, machine):
     tr = W.make_trace(config, seed=0, scale=scale)
@@ -119,7 +119,7 @@ def test_config2_lru_and_small_cache_pressure(arc, policy):
     run_trace(arc, steps, 600, policy, 0, ctx=f"pressure policy {policy}")
 
 
-@pytest.mark.parametrize("machine", [0, 1, 2])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3])
 @pytest.mark.parametrize("c", [1, 2, 3, 5, 8])
 def test_tiny_caches_prefix_trees(arc, c, machine):
     """Adversarial micro-traces: duplicate requests inside one step, keys dropped from a ghost list and
@@ -225,7 +225,7 @@ def test_maintenance_rebuild_and_compaction(arc):
         gc.close()
 
 
-@pytest.mark.parametrize("machine", [0, 1, 2])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3])
 @pytest.mark.parametrize("bits", [3, 6])
 def test_equal_keys_inside_a_request(arc, machine, bits):
     """The same key several times inside one request (forced with the key-mask test hook; the 64-bit hash never does
