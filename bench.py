@@ -43,7 +43,7 @@ ALGO_BYTES_PER_BLOCK = 72          # K1: 64 B of tokens read + 8 B key written (
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--steps", type=int, default=600)
     ap.add_argument("--warmup", type=int, default=30)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index + 1 (default 2 = doc-QA)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -100,7 +100,7 @@ class ClockSampler:
                     self.rows.append([x.strip() for x in out.splitlines()[0].split(",")])
             except Exception:
                 pass
-            self._stop.wait(0.2)
+            self._stop.wait(0.05)
 
     def __enter__(self):
         self._t = threading.Thread(target=self._run, daemon=True)

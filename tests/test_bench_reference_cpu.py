@@ -1,0 +1,33 @@
+"""bench.py's reference arm (the CPU oracle on the bench workload) runs without a GPU and prints the contract's JSON line."""
+import json
+import subprocess
+import sys
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+def test_reference_arm_prints_one_json_line():
+    out = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--impl", "reference", "--steps", "3", "--warmup", "1"],
+                         capture_output=True, text=True, timeout=300, cwd=str(ROOT))
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == "arc_block_accesses_per_s" and d["unit"] == "accesses/s"
+    assert d["steps"] == 3 and d["warmup"] == 1 and d["value"] > 0 and d["higher_is_better"] is True
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] == 1
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0
+    assert "configs[1]" in d["config"]["workload"]
+
+
+def test_our_arm_refuses_to_run_without_a_gpu():
+    """No CPU fallback: without CUDA the product arm must fail loudly, not fall back to the oracle."""
+    import torch
+
+    if torch.cuda.is_available():
+        return
+    out = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--steps", "2", "--warmup", "1"],
+                         capture_output=True, text=True, timeout=300, cwd=str(ROOT))
+    assert out.returncode != 0
+    assert "no CPU fallback" in (out.stderr + out.stdout)
