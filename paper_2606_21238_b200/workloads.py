@@ -227,6 +227,49 @@ class InterleaveTrace(Trace):
             yield next(sa) if t else next(sb)
 
 
+class WindowedZipfTrace(Trace):
+    """The paper's own workload shape: `n_windows` windows of `window` requests; inside a window documents
+    are drawn Zipf(s); the rank -> document assignment is reshuffled for every window (popularity shifts).  Whole document
+    ++ fresh question, one request per step by default (the paper runs batch size 1).  Documents are
+    synthetic (lognormal lengths, uniform tokens); the QuALITY / WikiQA texts are not available and not imitated."""
+
+    def __init__(self, info: TraceInfo, *, n_docs: int, vocab: int, zipf_s: float, doc_len, q_len: Tuple[int, int],
+                 window: int, n_windows: int, seed: int):
+        info.n_requests = window * n_windows
+        self.info = info
+        ss_corpus, ss_pop, ss_suffix, ss_perm = _children(seed, 4)
+        rng_corpus, rng_pop, rng_perm = _gen(ss_corpus), _gen(ss_pop), _gen(ss_perm)
+        lengths = doc_len(rng_corpus, n_docs)
+        self.docs = [rng_corpus.integers(0, vocab, size=int(n), dtype=np.int32) for n in lengths]
+        p = zipf_probabilities(n_docs, zipf_s)
+        choice = []
+        self.window_perms = []
+        for _ in range(n_windows):
+            perm = rng_perm.permutation(n_docs)            # rank k -> document perm[k], redrawn per window
+            self.window_perms.append(perm)
+            choice.append(perm[rng_pop.choice(n_docs, size=window, p=p)])
+        self.choice = np.concatenate(choice)
+        self.window = window
+        self.ss_suffix, self.vocab, self.q_len = ss_suffix, vocab, q_len
+
+    def _request_stream(self):
+        rng = _gen(self.ss_suffix)
+        lo, hi = self.q_len
+        for d in self.choice:
+            q = rng.integers(0, self.vocab, size=int(rng.integers(lo, hi + 1)), dtype=np.int32)
+            yield np.concatenate([self.docs[int(d)], q])
+
+
+def make_windowed_zipf(capacity_blocks: int, seed: int = 0, *, n_docs: int = 381, mean_doc_tokens: float = 5000.0,
+                       window: int = 512, n_windows: int = 6, zipf_s: float = 1.0, requests_per_step: int = 1) -> WindowedZipfTrace:
+    """3,072 requests = 6 windows x 512, Zipf exponent 1.0, items reshuffled per window
+    (PAPER.md:99); 381 documents of about 5k tokens (the counts PAPER.md:97 quotes for its document set)."""
+    info = TraceInfo("windowed-zipf", capacity_blocks, 16, requests_per_step, 0)
+    return WindowedZipfTrace(info, n_docs=n_docs, vocab=128000, zipf_s=zipf_s,
+                             doc_len=_lognormal_len(mean_doc_tokens, 0.5, 1000, 16000), q_len=(16, 64),
+                             window=window, n_windows=n_windows, seed=seed)
+
+
 # ---------------------------------------------------------------------------- configs
 
 CONFIG_NAMES = {1: "tiny-docqa", 2: "docqa", 3: "conversation", 4: "scan-hotset", 5: "scale-stress"}

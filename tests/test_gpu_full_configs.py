@@ -47,3 +47,42 @@ def test_full_size_config(config, max_steps, policy):
     if config in (2, 3) and max_steps is None:
         assert n_steps == tr.info.n_steps
     gc.close()
+
+
+@pytest.mark.parametrize("policy", [0, 1, 2])
+def test_windowed_zipf_batch1(policy):
+    """The paper-shaped workload at batch size 1: 3,072 one-request steps, every output and
+    the T1 ratio trajectory against the oracle."""
+    from paper_2606_21238_b200 import arc as A
+
+    c = 30000 // 16                                  # the paper's smallest cache size, 30K tokens
+    tr = W.make_windowed_zipf(c, seed=0)
+    gc, oc = A.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
+    n = 0
+    for i, (tokens, offsets) in enumerate(tr.steps()):
+        if int((np.diff(offsets) // 16).max()) > c:
+            continue
+        g = gc.step(torch.from_numpy(tokens).cuda(), offsets).to_host()
+        o = oc.step(tokens, offsets)
+        for k in OUT_KEYS:
+            assert np.array_equal(g[k], o[k]), f"policy {policy} request {i}: {k}"
+        if i % 64 == 0:
+            gs, os_ = gc.stats(), oc.stats()
+            assert (gs["t1"], gs["t2"], gs["b1"], gs["b2"], gs["p"]) == (os_["t1"], os_["t2"], os_["b1"], os_["b2"], os_["p"])
+        n += 1
+    assert n > 2500
+    gs, os_ = gc.stats(), oc.stats()
+    for k in STAT_KEYS:
+        assert gs[k] == os_[k], k
+    gc.close()
+
+
+def test_report_tool_runs():
+    from paper_2606_21238_b200 import report
+
+    rep = report.run([30000], seed=0, policies=(0, 1), sample_every=256)
+    assert len(rep["runs"]) == 2
+    arc, lru = rep["runs"]
+    assert arc["policy"] == "ARC" and lru["policy"] == "LRU"
+    assert 0.0 < lru["block_hit_rate"] <= arc["block_hit_rate"] + 0.02 < 1.0
+    assert all(0.0 <= x <= 1.0 for x in arc["t1_ratio_every_256_requests"])

@@ -281,3 +281,27 @@ def test_dbl_never_moves_p_and_equals_arc_without_resident_pressure():
         oa, od = a.step_keys(req), d.step_keys(req)
         for k in ("cls", "block_id", "evicted_id", "prefix_len"):
             assert np.array_equal(oa[k], od[k]), k
+
+
+def test_windowed_zipf_generator_shape_and_shift():
+    """NEXT-2 workload: 6 windows x 512 requests, deterministic, popularity reshuffled per window."""
+    from paper_2606_21238_b200 import workloads as W
+
+    tr = W.make_windowed_zipf(2048, seed=3, n_docs=50, mean_doc_tokens=1200.0)
+    assert tr.info.n_requests == 3072 and len(tr.choice) == 3072
+    tr2 = W.make_windowed_zipf(2048, seed=3, n_docs=50, mean_doc_tokens=1200.0)
+    assert np.array_equal(tr.choice, tr2.choice) and W.trace_digest(tr, max_steps=40) == W.trace_digest(tr2, max_steps=40)
+    tops = [int(np.bincount(tr.choice[w * 512:(w + 1) * 512], minlength=50).argmax()) for w in range(6)]
+    assert len(set(tops)) >= 3                                   # the hot document changes between windows
+    for w in range(6):                                           # inside a window the head of the Zipf law dominates
+        cnt = np.sort(np.bincount(tr.choice[w * 512:(w + 1) * 512], minlength=50))[::-1]
+        assert cnt[0] > 3 * cnt[9]
+    # ARC tracks the shifts at least as well as LRU on this workload (oracle, small cache)
+    rates = {}
+    for pol in (O.POLICY_ARC, O.POLICY_LRU):
+        oc = O.OracleCache(1024, 16, pol)
+        for tok, off in W.make_windowed_zipf(1024, seed=3, n_docs=50, mean_doc_tokens=1200.0).steps():
+            oc.step(tok, off, unpack=False)
+        st = oc.stats()
+        rates[pol] = (st["hit_t1"] + st["hit_t2"]) / st["accesses"]
+    assert rates[O.POLICY_ARC] >= rates[O.POLICY_LRU] - 0.01, rates
