@@ -39,3 +39,102 @@ def route_requests(first_block_keys, world: int):
 
     k = np.asarray(first_block_keys, dtype=np.uint64)
     return ((k >> np.uint64(33)) % np.uint64(max(1, world))).astype(np.int64)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# NEXT-4: prefix-affinity sharding.  The paper's deployment context is a router in front of per-GPU
+# cache managers (collaborative caching is future work).  N shards = N independent caches;
+# a request goes to the shard chosen by the key of its FIRST block, so that all requests sharing a document or a
+# conversation prefix meet in the same cache.  This is a different system from one cache of N x the capacity and is not
+# bit-comparable to it; each shard is bit-comparable to an oracle fed the same sub-stream.  No data-path collective.
+
+def first_block_offsets(offsets, block_size: int = 16):
+    """offsets of the sub-batch holding only the first full block of every request (empty for shorter requests)."""
+    import numpy as np
+
+    o = np.asarray(offsets, dtype=np.int64)
+    has = (o[1:] - o[:-1]) >= block_size
+    return o[:-1], has
+
+
+def split_batch(offsets, dst, shard: int):
+    """-> (indices of the requests routed to `shard`, their offsets rebased to a packed sub-batch, the token slices)."""
+    import numpy as np
+
+    o = np.asarray(offsets, dtype=np.int64)
+    idx = np.flatnonzero(np.asarray(dst) == shard)
+    lens = o[idx + 1] - o[idx]
+    sub = np.zeros(len(idx) + 1, dtype=np.int64)
+    sub[1:] = np.cumsum(lens)
+    return idx, sub, [(int(o[i]), int(o[i + 1])) for i in idx]
+
+
+class ShardedArc:
+    """`world` caches with prefix-affinity routing.  With `rank` given (one process per GPU) only the local shard lives
+    here and `step` serves the local share of the batch; with rank=None all shards live in this process (single-GPU
+    simulation, used by the tests)."""
+
+    def __init__(self, capacity_blocks_per_shard: int, world: int, rank=None, block_size: int = 16, policy: int = 0):
+        from . import arc as A
+
+        self._A = A
+        self.world, self.rank, self.B = int(world), rank, block_size
+        shards = range(self.world) if rank is None else [int(rank)]
+        self.caches = {s: A.ArcCache(capacity_blocks_per_shard, block_size, policy) for s in shards}
+
+    def route(self, tokens, offsets):
+        """Destination shard of every request: by its first block's key (K1 on the first 16 tokens of each request);
+        requests without a full block go to shard 0 (they make no access anywhere)."""
+        import numpy as np
+        import torch
+
+        o = np.asarray(offsets, dtype=np.int64)
+        starts, has = first_block_offsets(o, self.B)
+        dst = np.zeros(len(starts), dtype=np.int64)
+        if has.any():
+            # one-block requests: [start, start + B) for every request that has a full block
+            sel = starts[has]
+            first = torch.stack([tokens[int(s):int(s) + self.B] for s in sel]).reshape(-1) if len(sel) < 64 else \
+                tokens[(torch.from_numpy(sel).to(tokens.device)[:, None] + torch.arange(self.B, device=tokens.device)[None, :]).reshape(-1)]
+            fo = np.arange(len(sel) + 1, dtype=np.int64) * self.B
+            keys = self._A.hash_blocks(first.contiguous(), fo, self.B).cpu().numpy().view(np.uint64)
+            dst[has] = route_requests(keys, self.world)
+        return dst
+
+    def step(self, tokens, offsets):
+        """-> {shard: (request indices, StepResult)} for the shards that live in this process."""
+        import torch
+
+        dst = self.route(tokens, offsets)
+        out = {}
+        for s, cache in self.caches.items():
+            idx, sub, slices = split_batch(offsets, dst, s)
+            sub_tokens = torch.cat([tokens[a:b] for a, b in slices]) if slices else tokens[:0]
+            out[s] = (idx, cache.step(sub_tokens.contiguous(), sub))
+        return out
+
+    def stats(self, dist=None, torch=None):
+        """Counters summed over the local shards and, with an initialised process group, over all ranks."""
+        keys = [k for k in self._A.STAT_FIELDS if k not in ("p", "capacity_blocks")]
+        tot = {k: 0 for k in keys}
+        for c in self.caches.values():
+            st = c.stats()
+            for k in keys:
+                tot[k] += st[k]
+        return aggregate_counters(dist, torch, tot)
+
+    def close(self):
+        for c in self.caches.values():
+            c.close()
+
+
+def aggregate_counters(dist, torch, counters: dict, device=None) -> dict:
+    """One all-reduce (SUM) of a dict of integer counters over the ranks; a pass-through without a process group."""
+    if dist is None or not dist.is_initialized():
+        return dict(counters)
+    if device is None:
+        device = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend() == "nccl" else torch.device("cpu")
+    keys = sorted(counters)
+    t = torch.tensor([int(counters[k]) for k in keys], dtype=torch.int64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return {k: int(v) for k, v in zip(keys, t.tolist())}

@@ -86,3 +86,35 @@ def test_report_tool_runs():
     assert arc["policy"] == "ARC" and lru["policy"] == "LRU"
     assert 0.0 < lru["block_hit_rate"] <= arc["block_hit_rate"] + 0.02 < 1.0
     assert all(0.0 <= x <= 1.0 for x in arc["t1_ratio_every_256_requests"])
+
+
+def test_prefix_affinity_shards_match_per_shard_oracles():
+    """NEXT-4: four shards in one process; routing by the first block's key computed on the GPU must equal the routing
+    computed from the oracle's keys, and every shard must match an oracle fed the same sub-stream."""
+    from paper_2606_21238_b200 import parallel as P
+
+    world, c = 4, 48
+    sh = P.ShardedArc(c, world, rank=None)
+    oracles = [O.OracleCache(c, 16, 0) for _ in range(world)]
+    tr = W.make_trace(1, seed=2)
+    for step, (tokens, offsets) in enumerate(tr.steps(max_steps=60)):
+        keys, blk_off = O.hash_blocks(tokens, offsets)
+        nb = np.diff(blk_off)
+        want_dst = np.zeros(len(nb), dtype=np.int64)
+        want_dst[nb > 0] = P.route_requests(keys[blk_off[:-1][nb > 0]], world)
+        dev_tokens = torch.from_numpy(tokens).cuda()
+        assert np.array_equal(sh.route(dev_tokens, offsets), want_dst)
+        res = sh.step(dev_tokens, offsets)
+        for s in range(world):
+            idx, sub, slices = P.split_batch(offsets, want_dst, s)
+            sub_tokens = np.concatenate([tokens[a:b] for a, b in slices]) if slices else np.zeros(0, np.int32)
+            o = oracles[s].step(sub_tokens, sub)
+            gi, g = res[s]
+            assert np.array_equal(gi, idx)
+            g = g.to_host()
+            for k in OUT_KEYS:
+                assert np.array_equal(g[k], o[k]), f"step {step} shard {s}: {k}"
+    tot = sh.stats()
+    assert tot["accesses"] == sum(o.stats()["accesses"] for o in oracles)
+    assert tot["hit_t1"] + tot["hit_t2"] == sum(o.stats()["hit_t1"] + o.stats()["hit_t2"] for o in oracles)
+    sh.close()

@@ -32,6 +32,8 @@ def _worker(rank, world, port, q):
         n_req += len(offsets) - 1
     P.barrier(dist)
     out = P.reduce_timing(dist, torch, 10.0 * (rank + 1), n_acc, n_tok, n_req)
+    agg = P.aggregate_counters(dist, torch, {"accesses": n_acc, "requests": n_req})
+    assert agg["accesses"] == out[1] and agg["requests"] == out[3]
     q.put((rank, (n_acc, n_tok, n_req), out))
     dist.destroy_process_group()
 
@@ -62,3 +64,19 @@ def test_single_process_passthrough_and_routing():
     assert dst.min() >= 0 and dst.max() < 8
     assert np.array_equal(dst, P.route_requests(keys, 8))      # deterministic: same prefix -> same replica
     assert np.bincount(dst, minlength=8).min() > 1000          # and roughly balanced
+
+
+def test_split_batch_partitions_the_requests():
+    rng = np.random.default_rng(1)
+    lens = rng.integers(0, 90, size=40)
+    offsets = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    dst = rng.integers(0, 3, size=40)
+    seen = []
+    for s in range(3):
+        idx, sub, slices = P.split_batch(offsets, dst, s)
+        assert np.array_equal(np.diff(sub), lens[idx]) and len(slices) == len(idx)
+        assert all(b - a == lens[i] for (a, b), i in zip(slices, idx))
+        seen += idx.tolist()
+    assert sorted(seen) == list(range(40))
+    starts, has = P.first_block_offsets(offsets)
+    assert np.array_equal(has, lens >= 16) and np.array_equal(starts, offsets[:-1])
