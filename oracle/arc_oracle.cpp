@@ -114,6 +114,7 @@ struct oracle_cache {
   uint64_t c;
   uint32_t B;
   int policy;
+  int pin_scope;          // 0: pins end with their request (R4); 1: with the step (NEXT-3)
   KeyList T1, T2, B1, B2;
   std::unordered_map<uint64_t, Entry> dir;
   uint64_t p;
@@ -273,6 +274,7 @@ int step_keys(oracle_cache* h, const uint64_t* keys, const int64_t* blk_off, uin
   for (uint32_t r = 0; r < n_req; ++r)
     if ((uint64_t)(blk_off[r + 1] - blk_off[r]) > h->c) return ERR_REQUEST_TOO_LARGE;  // R11: before any change
   const int64_t N = blk_off[n_req];
+  if (h->pin_scope == 1 && (uint64_t)N > h->c) return ERR_REQUEST_TOO_LARGE;   // step-wide pins: a step may pin at most c blocks
   h->prefix_len.assign(n_req, 0);
   h->blk_off.assign(blk_off, blk_off + n_req + 1);
   h->cls.assign(N, 0); h->block_id.assign(N, -1); h->evicted_id.assign(N, -1); h->p_after.assign(N, 0);
@@ -285,16 +287,23 @@ int step_keys(oracle_cache* h, const uint64_t* keys, const int64_t* blk_off, uin
       if (h->cls[o + i] != HIT_T1 && h->cls[o + i] != HIT_T2) h->alloc_ids.push_back(h->block_id[o + i]);
       if (h->evicted_id[o + i] >= 0) h->evict_ids.push_back(h->evicted_id[o + i]);
     }
-    for (size_t k = 0; k < h->pinned_keys.size(); ++k) {   // R4: pins drop when the request completes
-      std::unordered_map<uint64_t, Entry>::iterator f = h->dir.find(h->pinned_keys[k]);
-      if (f != h->dir.end()) f->second.pinned = false;
+    if (h->pin_scope == 0) {
+      for (size_t k = 0; k < h->pinned_keys.size(); ++k) {   // R4: pins drop when the request completes
+        std::unordered_map<uint64_t, Entry>::iterator f = h->dir.find(h->pinned_keys[k]);
+        if (f != h->dir.end()) f->second.pinned = false;
+      }
+      h->pinned_keys.clear();
     }
-    h->pinned_keys.clear();
     int64_t lead = 0;                               // R9
     while (lead < nb && (h->cls[o + lead] == HIT_T1 || h->cls[o + lead] == HIT_T2)) ++lead;
     h->prefix_len[r] = (int32_t)(lead * h->B);
     h->st.prefix_hit_tokens += lead * h->B;
   }
+  for (size_t k = 0; k < h->pinned_keys.size(); ++k) {     // step-wide scope: pins drop when the step completes
+    std::unordered_map<uint64_t, Entry>::iterator f = h->dir.find(h->pinned_keys[k]);
+    if (f != h->dir.end()) f->second.pinned = false;
+  }
+  h->pinned_keys.clear();
   h->st.steps++; h->st.requests += n_req;
   if (out) {
     out->n_access = (uint64_t)N;
@@ -317,7 +326,7 @@ int oracle_create(uint64_t capacity_blocks, uint32_t block_size, int policy, ora
   if (policy != POLICY_ARC && policy != POLICY_LRU && policy != POLICY_DBL) return ERR_INVALID_ARG;
   if (block_size == 0 || (block_size & 1)) return ERR_UNSUPPORTED;   // the hash is defined for even B
   oracle_cache* h = new oracle_cache();
-  h->c = capacity_blocks; h->B = block_size; h->policy = policy; h->next_fresh = 0;
+  h->c = capacity_blocks; h->B = block_size; h->policy = policy; h->next_fresh = 0; h->pin_scope = 0;
   h->p = (policy == POLICY_DBL) ? capacity_blocks / 2 : 0;   // DBL: the fixed 1:1 split
   std::memset(&h->st, 0, sizeof(h->st));
   h->hash_seconds = h->arc_seconds = 0.0;
@@ -326,6 +335,14 @@ int oracle_create(uint64_t capacity_blocks, uint32_t block_size, int policy, ora
 }
 
 void oracle_destroy(oracle_cache* h) { delete h; }
+
+// 0 = pins end with their request (R4, default); 1 = with the step (every block a step touches stays resident until the
+// step's last access; a step of more than capacity blocks is refused).
+int oracle_set_pin_scope(oracle_cache* h, int scope) {
+  if (!h || (scope != 0 && scope != 1)) return ERR_INVALID_ARG;
+  h->pin_scope = scope;
+  return OK;
+}
 
 // Stateless: keys of every full block, natural order (index blk_off[r]+i).  keys_out may be NULL to
 // only fill blk_off_out ([n_req+1]).
@@ -364,6 +381,7 @@ int oracle_step(oracle_cache* h, const int32_t* tokens, const int64_t* offsets, 
   oracle_hash_blocks(tokens, offsets, n_req, h->B, 0, blk_off.data());
   for (uint32_t r = 0; r < n_req; ++r)
     if ((uint64_t)(blk_off[r + 1] - blk_off[r]) > h->c) return ERR_REQUEST_TOO_LARGE;   // before hashing: no state change
+  if (h->pin_scope == 1 && (uint64_t)blk_off[n_req] > h->c) return ERR_REQUEST_TOO_LARGE;
   h->keys.resize(blk_off[n_req]);
   oracle_hash_blocks(tokens, offsets, n_req, h->B, h->keys.data(), 0);
   double t1 = now_s();

@@ -56,6 +56,7 @@ def lib():
         L.oracle_hash_blocks.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p]
         L.oracle_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(_Result)]
         L.oracle_step_keys.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(_Result)]
+        L.oracle_set_pin_scope.argtypes = [C.c_void_p, C.c_int]
         L.oracle_stats.argtypes = [C.c_void_p, C.POINTER(_Stats)]
         L.oracle_timing.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.oracle_timing.restype = None
@@ -111,6 +112,11 @@ class OracleCache:
         if rc != OK:
             raise ValueError(f"oracle_create: {rc}")
         self.block_size = block_size
+
+    def set_pin_scope(self, scope):
+        rc = lib().oracle_set_pin_scope(self._h, scope)
+        if rc != OK:
+            raise ValueError(f"oracle_set_pin_scope: {rc}")
 
     def close(self):
         if self._h:

@@ -98,6 +98,7 @@ class BruteForceCache:
         self.block_of = {}  # resident key -> block ID (ghosts hold no ID, I8)
         self.next_fresh = 0
         self.pinned = set()
+        self.pin_scope = 0  # 0: pins end with their request (R4); 1: with the step (NEXT-3)
         self.stats = dict(steps=0, requests=0, tokens_seen=0, tokens_hashed=0, accesses=0, hit_t1=0, hit_t2=0,
                           ghost_b1=0, ghost_b2=0, miss=0, evict_t1=0, evict_t2=0, drop_b1=0, drop_b2=0,
                           fresh_ids_used=0, prefix_hit_tokens=0)
@@ -221,6 +222,8 @@ class BruteForceCache:
         for keys in requests_keys:
             if len(keys) > self.c:
                 return ERR_REQUEST_TOO_LARGE  # R11: no state change
+        if self.pin_scope == 1 and sum(len(k) for k in requests_keys) > self.c:
+            return ERR_REQUEST_TOO_LARGE  # step-wide pins: the step may pin at most c blocks (admission rule)
         out = dict(prefix_len=[], blk_off=[0], cls=[], block_id=[], evicted_id=[], p_after=[], alloc_ids=[], evict_ids=[])
         for keys in requests_keys:  # R2: requests in ascending index
             nb = len(keys)
@@ -235,7 +238,8 @@ class BruteForceCache:
                     out["alloc_ids"].append(bid[i])
                 if evi[i] >= 0:
                     out["evict_ids"].append(evi[i])
-            self.pinned.clear()  # R4: all pins of the request drop together
+            if self.pin_scope == 0:
+                self.pinned.clear()  # R4: all pins of the request drop together
             lead = 0
             while lead < nb and cls[lead] in (HIT_T1, HIT_T2):  # R9
                 lead += 1
@@ -246,6 +250,7 @@ class BruteForceCache:
             out["block_id"] += bid
             out["evicted_id"] += evi
             out["p_after"] += paf
+        self.pinned.clear()  # step-wide scope: all pins of the step drop together
         self.stats["steps"] += 1
         self.stats["requests"] += len(requests_keys)
         return out

@@ -305,3 +305,74 @@ def test_windowed_zipf_generator_shape_and_shift():
         st = oc.stats()
         rates[pol] = (st["hit_t1"] + st["hit_t2"]) / st["accesses"]
     assert rates[O.POLICY_ARC] >= rates[O.POLICY_LRU] - 0.01, rates
+
+
+def _keys(names, n):
+    return [n.key(x) for x in names]
+
+
+@pytest.mark.parametrize("impl", ["bf", "cpp"])
+def test_step_wide_pins_hand_trace_G(impl):
+    """NEXT-3, step-wide pin scope: c = 4, ARC.  Steps [X0..X3], [X0..X3], [Y0][Z0].  In the third step
+    Z0's REPLACE prefers T1 (t1 = 1 > p = 0) whose only entry Y0 was brought in by an earlier request of the SAME step:
+    under step-wide pins it is still pinned and the victim comes from T2 (X2); under the default request scope Y0 itself
+    is evicted.  Derived by hand from R5/R7."""
+    from helpers import KeyNames
+
+    def make(scope):
+        cch = BF.BruteForceCache(4) if impl == "bf" else O.OracleCache(4)
+        if impl == "bf":
+            cch.pin_scope = scope
+        else:
+            cch.set_pin_scope(scope)
+        return cch
+
+    for scope in (0, 1):
+        n = KeyNames()
+        cch = make(scope)
+        X = _keys(["X0", "X1", "X2", "X3"], n)
+        o1 = cch.step_keys([X])
+        assert list(o1["block_id"]) == [3, 2, 1, 0] and list(o1["cls"]) == [0, 0, 0, 0]      # tail first: X3 gets ID 0
+        o2 = cch.step_keys([X])
+        assert list(o2["cls"]) == [1, 1, 1, 1] and list(o2["prefix_len"]) == [64]
+        o3 = cch.step_keys([_keys(["Y0"], n), _keys(["Z0"], n)])
+        assert list(o3["cls"]) == [0, 0]
+        L = cch.lists()
+        name = lambda lst: n.names(lst if impl == "bf" else lst[0])
+        if scope == 1:
+            assert list(o3["block_id"]) == [0, 1] and list(o3["evicted_id"]) == [0, 1]      # X3 then X2 leave T2
+            assert name(L["T1"]) == ["Y0", "Z0"] and name(L["T2"]) == ["X1", "X0"] and name(L["B2"]) == ["X3", "X2"] and name(L["B1"]) == []
+        else:
+            assert list(o3["block_id"]) == [0, 0] and list(o3["evicted_id"]) == [0, 0]      # X3, then Y0 itself
+            assert name(L["T1"]) == ["Z0"] and name(L["T2"]) == ["X2", "X1", "X0"] and name(L["B2"]) == ["X3"] and name(L["B1"]) == ["Y0"]
+        # admission rule of the step scope: a step may pin at most c blocks; refused without a state change
+        big = [_keys(["P0", "P1", "P2"], n), _keys(["Q0", "Q1"], n)]
+        before = cch.lists()
+        r = cch.step_keys(big)
+        if scope == 1:
+            assert r == O.ERR_REQUEST_TOO_LARGE
+            after = cch.lists()
+            assert all(list(np.asarray(before[k] if impl == "bf" else before[k][0])) == list(np.asarray(after[k] if impl == "bf" else after[k][0])) for k in ("T1", "T2", "B1", "B2"))
+        else:
+            assert isinstance(r, dict)
+
+
+@pytest.mark.parametrize("policy", [0, 1, 2])
+def test_step_wide_pins_differential_and_invariants(policy):
+    rng = np.random.default_rng(300 + policy)
+    for c in (2, 3, 5, 8):
+        bf, cpp = BF.BruteForceCache(c, 16, policy), O.OracleCache(c, 16, policy)
+        bf.pin_scope = 1
+        cpp.set_pin_scope(1)
+        for _ in range(300):
+            reqs, left = [], c
+            while left > 0 and rng.random() < 0.8:
+                nb = int(rng.integers(1, min(left, 3) + 1))
+                base = int(rng.integers(0, 4))
+                reqs.append([1000 + 10 * base + i for i in range(nb)])       # shared prefixes
+                left -= nb
+            a, b = bf.step_keys(reqs), cpp.step_keys(reqs)
+            for k in ("cls", "block_id", "evicted_id", "p_after", "prefix_len", "alloc_ids", "evict_ids"):
+                assert list(a[k]) == b[k].tolist(), (c, policy, k)
+            L = cpp.lists()
+            check_invariants(L, c, policy_lru=(policy == 1))
