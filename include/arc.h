@@ -41,6 +41,9 @@ enum {
   ARC_ERR_OOM = -4,               /* device or pinned-host allocation failed */
   ARC_ERR_CUDA = -5               /* any other CUDA error; text in arc_last_error */
 };
+/* Scope of the pins (R4): a block accessed by a request is never a victim until ... */
+enum { ARC_PIN_REQUEST = 0,   /* ... its request's last access (default)                                                  */
+       ARC_PIN_STEP = 1 };    /* ... the step's last access: everything a step touches stays resident for the whole step */
 /* class of one block access, as decided against the live state at the moment of the access (R3, R5) */
 enum { ARC_MISS = 0, ARC_HIT_T1 = 1, ARC_HIT_T2 = 2, ARC_GHOST_B1 = 3, ARC_GHOST_B2 = 4 };
 
@@ -120,6 +123,11 @@ int arc_step(arc_cache *h, const int32_t *d_tokens, const int64_t *h_offsets, ui
  * to pinned host memory and synchronises the stream before returning. */
 int arc_step_host(arc_cache *h, const int32_t *h_tokens, const int64_t *h_offsets, uint32_t n_req,
                   void *cuda_stream, arc_host_result *out);
+
+/* Sets the pin scope for the following steps.  With ARC_PIN_STEP a step whose
+ * requests hold more than capacity_blocks full blocks in total is refused with ARC_ERR_REQUEST_TOO_LARGE (nothing is
+ * enqueued, the handle is unchanged): the admission rule that guarantees a victim always exists. */
+int arc_set_pin_scope(arc_cache *h, int scope);
 
 /* Synchronises the stream of the handle's last step and copies the counters.  out: HOST. */
 int arc_stats(arc_cache *h, arc_stats_t *out);

@@ -15,6 +15,7 @@ import numpy as np
 from . import build as _build
 
 POLICY_ARC, POLICY_LRU, POLICY_DBL = 0, 1, 2
+PIN_REQUEST, PIN_STEP = 0, 1
 MISS, HIT_T1, HIT_T2, GHOST_B1, GHOST_B2 = 0, 1, 2, 3, 4
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_REQUEST_TOO_LARGE, ERR_OOM, ERR_CUDA = 0, -1, -2, -3, -4, -5
 
@@ -25,7 +26,7 @@ STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", 
 # every symbol include/arc.h declares (checked by the CPU test-suite against the built library)
 EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats", "arc_reset", "arc_destroy",
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
-           "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe"]
+           "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe", "arc_set_pin_scope"]
 
 
 class ArcError(RuntimeError):
@@ -86,6 +87,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_debug_counters.argtypes = [vp, vp, u32]
     L.arc_debug_set_key_mask.argtypes = [vp, u64]
     L.arc_debug_probe.argtypes = [vp, vp, u64, vp, vp]
+    L.arc_set_pin_scope.argtypes = [vp, C.c_int]
     L.arc_debug_list.argtypes = [vp, C.c_int, vp, vp, u64, C.POINTER(u64)]
     if path is None:
         _lib = L
@@ -234,6 +236,9 @@ class ArcCache:
 
     def launch_count(self) -> int:
         return int(self._L.arc_launch_count(self._h))
+
+    def set_pin_scope(self, scope: int):
+        self._check(self._L.arc_set_pin_scope(self._h, scope))
 
     def set_machine(self, which: int):
         self._check(self._L.arc_set_machine(self._h, which))

@@ -105,6 +105,7 @@ struct StepParams {
   int32_t capacity;
   int32_t policy;
   uint32_t block_size;
+  int32_t pin_scope;              // 0: pins end with their request, 1: with the step
   unsigned long long key_and;     // test hook (arc_debug_set_key_mask): keys are ANDed with this before the probe; all ones normally
 };
 

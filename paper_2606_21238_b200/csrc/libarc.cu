@@ -56,6 +56,7 @@ struct arc_cache {
   uint32_t B = 16;
   int policy = 0;
   unsigned long long key_and = ~0ull;   // test hook
+  int pin_scope = ARC_PIN_REQUEST;
   int machine = 0;            // 0 auto (wide, or one-warp when requests are short), 1 serial, 2 one-warp, 3 wide
   // capacities
   uint64_t n_cap = 0;         // max full blocks per step the buffers are sized for
@@ -133,7 +134,7 @@ StepParams make_params(arc_cache* h) {
   P.keys_acc = h->d_keys; P.node_acc = h->d_node_acc; P.dropped = h->d_dropped;
   P.prefix_len = h->d_prefix_len; P.cls = h->d_cls; P.block_id = h->d_block_id; P.evicted_id = h->d_evicted_id;
   P.p_after = h->d_p_after; P.alloc_ids = h->d_alloc_ids; P.evict_ids = h->d_evict_ids;
-  P.capacity = (int32_t)h->c; P.policy = h->policy; P.block_size = h->B; P.key_and = h->key_and;
+  P.capacity = (int32_t)h->c; P.policy = h->policy; P.block_size = h->B; P.key_and = h->key_and; P.pin_scope = h->pin_scope;
   return P;
 }
 
@@ -366,6 +367,8 @@ int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, ui
   uint64_t N = 0;
   int rc = validate_offsets(h, h_offsets, n_req, h->B, h->c, blk_off.data(), &N);
   if (rc) return rc;
+  if (h->pin_scope == ARC_PIN_STEP && N > h->c)
+    return fail(h, ARC_ERR_REQUEST_TOO_LARGE, "step-wide pins: the step holds %llu blocks > capacity %llu", (unsigned long long)N, (unsigned long long)h->c);
   if (!d_tokens && h_offsets[n_req] > h_offsets[0]) return fail(h, ARC_ERR_INVALID_ARG, "d_tokens is NULL");
 
   rc = ensure_capacity(h, n_req, N, s);
@@ -593,6 +596,13 @@ uint64_t arc_launch_count(const arc_cache* h) { return h ? h->launches : g_hash_
 int arc_set_machine(arc_cache* h, int which) {
   if (!h || which < 0 || which > 3) return ARC_ERR_INVALID_ARG;
   h->machine = which;
+  return ARC_OK;
+}
+
+int arc_set_pin_scope(arc_cache* h, int scope) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  if (scope != ARC_PIN_REQUEST && scope != ARC_PIN_STEP) return fail(h, ARC_ERR_INVALID_ARG, "unknown pin scope %d", scope);
+  h->pin_scope = scope;
   return ARC_OK;
 }
 

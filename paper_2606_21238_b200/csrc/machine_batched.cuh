@@ -251,7 +251,7 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
       my_off = P.blk_off[rr]; my_off1 = P.blk_off[rr + 1];
     }
     const int64_t o = __shfl_sync(FULL, my_off, r & 31), nb = __shfl_sync(FULL, my_off1, r & 31) - o;
-    begin_request(C);
+    if (r == 0 || P.pin_scope == 0) begin_request(C);   // step-wide scope: the pins of earlier requests of the step stay
     int64_t j = 0;
     while (j < nb) {
       const int kmax = (int)min((int64_t)32, nb - j);

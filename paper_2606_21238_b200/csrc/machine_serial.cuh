@@ -199,7 +199,7 @@ __global__ void arc_machine_serial_kernel(const __grid_constant__ StepParams P) 
   ctx_load(C, P);
   for (uint32_t r = 0; r < P.n_req; ++r) {
     const int64_t o = P.blk_off[r], nb = P.blk_off[r + 1] - o;
-    begin_request(C);
+    if (r == 0 || P.pin_scope == 0) begin_request(C);   // step-wide scope: the pins of earlier requests of the step stay
     for (int64_t j = 0; j < nb; ++j) serial_access(C, P, o + j, o + (nb - 1 - j));   // tail block first (R2)
   }
   ctx_store(C, P);

@@ -272,3 +272,46 @@ def test_probe_alone_is_a_consistent_map(arc):
     assert torch.equal(again.flip(0), nodes)
     gc.stats()                                          # no device-side error
     gc.close()
+
+
+@pytest.mark.parametrize("machine", [0, 1, 2, 3])
+def test_step_wide_pin_scope(arc, machine):
+    """NEXT-3 (part): ARC_PIN_STEP.  Hand trace G's situation (an earlier request's block is still pinned when a later
+    request of the same step needs a victim), the admission rule, and random steps on small caches, against the oracle."""
+    X = np.arange(100, 164, dtype=np.int32)
+    Y, Z = np.arange(500, 516, dtype=np.int32), np.arange(700, 716, dtype=np.int32)
+    for scope in (arc.PIN_REQUEST, arc.PIN_STEP):
+        gc, oc = arc.ArcCache(4), O.OracleCache(4)
+        gc.set_machine(machine)
+        gc.set_pin_scope(scope)
+        oc.set_pin_scope(scope)
+        for reqs in ([X], [X], [Y, Z]):
+            tokens, offsets = W.pack_requests(reqs)
+            assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), f"scope {scope}")
+        assert_same_state(gc, oc, f"scope {scope}")
+        t1 = gc.debug_lists()["T1"][0]
+        assert len(t1) == (2 if scope == arc.PIN_STEP else 1)          # Y0 survives only under step-wide pins
+        big, boff = W.pack_requests([np.arange(48, dtype=np.int32), np.arange(900, 932, dtype=np.int32)])   # 3 + 2 blocks > c
+        if scope == arc.PIN_STEP:
+            with pytest.raises(arc.ArcError) as e:
+                gc.step(dev(big), boff)
+            assert e.value.code == arc.ERR_REQUEST_TOO_LARGE == oc.step(big, boff)
+            assert_same_state(gc, oc, "after the refused step")
+        gc.close()
+    rng = np.random.default_rng(17)
+    for policy in (0, 1, 2):
+        for c in (3, 6, 40):
+            gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
+            gc.set_machine(machine)
+            gc.set_pin_scope(arc.PIN_STEP)
+            oc.set_pin_scope(arc.PIN_STEP)
+            for step in range(50):
+                reqs, left = [], c
+                while left > 0 and rng.random() < 0.85:
+                    r = W.prefix_tree_requests(rng, n_requests=1, block_size=16, branching=2, depth=4, max_blocks=min(left, 6))[0]
+                    reqs.append(r)
+                    left -= len(r) // 16
+                tokens, offsets = W.pack_requests(reqs)
+                assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), f"step scope p{policy} c{c} step {step}")
+            assert_same_state(gc, oc, f"step scope p{policy} c{c}")
+            gc.close()
