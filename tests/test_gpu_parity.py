@@ -315,3 +315,26 @@ def test_step_wide_pin_scope(arc, machine):
                 assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), f"step scope p{policy} c{c} step {step}")
             assert_same_state(gc, oc, f"step scope p{policy} c{c}")
             gc.close()
+
+
+@pytest.mark.parametrize("policy", [0, 1, 2])
+def test_many_tiny_requests_and_cache_sized_requests(arc, policy):
+    """Edge shapes: 20,000 requests of 0-2 blocks in one step (most of K3's windows are one or two accesses), then requests
+    of exactly c blocks (everything resident is replaced by one request), then a hit on all of it."""
+    rng = np.random.default_rng(61 + policy)
+    c = 3000
+    gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
+    base = rng.integers(0, 5000, size=(300, 32), dtype=np.int32)          # 300 two-block prefixes
+    reqs = []
+    for _ in range(20000):
+        b = base[int(rng.integers(0, 300))]
+        reqs.append(b[:int(rng.integers(0, 40))])                          # 0 .. 39 tokens: 0, 1 or 2 full blocks
+    tokens, offsets = W.pack_requests(reqs)
+    assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), "tiny requests")
+    big1 = rng.integers(0, 5000, size=16 * c, dtype=np.int32)
+    big2 = rng.integers(0, 5000, size=16 * c + 9, dtype=np.int32)
+    for name, r in (("cache-sized", [big1]), ("another", [big2]), ("again", [big2]), ("first again", [big1])):
+        tokens, offsets = W.pack_requests(r)
+        assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), name)
+    assert_same_state(gc, oc, "edge shapes")
+    gc.close()
