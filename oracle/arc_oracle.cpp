@@ -82,6 +82,7 @@ struct Entry {
   KeyList::iterator it;   // position in that list
   int32_t block;          // block ID if resident, -1 for ghosts (I8)
   bool pinned;            // R4
+  uint32_t holds;         // pin scope 2: accesses not yet released; > 0 = not evictable
 };
 
 }  // namespace
@@ -114,7 +115,10 @@ struct oracle_cache {
   uint64_t c;
   uint32_t B;
   int policy;
-  int pin_scope;          // 0: pins end with their request (R4); 1: with the step (NEXT-3)
+  int pin_scope;          // 0: pins end with their request (R4); 1: with the step (NEXT-3);
+                          // 2: held until oracle_release (NEXT-3)
+  uint64_t hold_units;    // scope 2: accesses made minus block IDs released = the sum of all hold counts
+  std::vector<uint64_t> owner;   // scope 2: owner[block ID] = key of the resident entry that has it
   KeyList T1, T2, B1, B2;
   std::unordered_map<uint64_t, Entry> dir;
   uint64_t p;
@@ -150,7 +154,9 @@ void put_mru(oracle_cache* h, uint64_t x, int where, int32_t block) {
   e.it = --l.end();
   e.block = block;
   e.pinned = false;
+  e.holds = 0;
   h->dir[x] = e;
+  if (block >= 0) { if (h->owner.size() <= (size_t)block) h->owner.resize((size_t)block + 1, 0); h->owner[block] = x; }
 }
 
 void remove_key(oracle_cache* h, uint64_t x) {
@@ -162,7 +168,7 @@ void remove_key(oracle_cache* h, uint64_t x) {
 // first unpinned entry from the LRU end; returns false if none (R7)
 bool first_unpinned(oracle_cache* h, KeyList& l, uint64_t* out) {
   for (KeyList::iterator it = l.begin(); it != l.end(); ++it)
-    if (!h->dir.at(*it).pinned) { *out = *it; return true; }
+    if (!h->dir.at(*it).pinned && h->dir.at(*it).holds == 0) { *out = *it; return true; }
   return false;
 }
 
@@ -195,6 +201,7 @@ int32_t evict_t1_no_ghost(oracle_cache* h) {
 
 void pin(oracle_cache* h, uint64_t x) {
   Entry& e = h->dir.at(x);
+  if (h->pin_scope == 2) { e.holds++; return; }     // held until released: one hold per access
   if (!e.pinned) { e.pinned = true; h->pinned_keys.push_back(x); }
 }
 
@@ -209,8 +216,8 @@ void access(oracle_cache* h, uint64_t x, uint8_t* cls_out, int32_t* block_out, i
   if (h->policy == POLICY_LRU) {
     if (f != h->dir.end()) {  // hit: move to MRU
       cls = HIT_T1; h->st.hit_t1++;
-      int32_t block = f->second.block; bool was_pinned = f->second.pinned;
-      remove_key(h, x); put_mru(h, x, IN_T1, block); h->dir.at(x).pinned = was_pinned;
+      int32_t block = f->second.block; bool was_pinned = f->second.pinned; uint32_t holds = f->second.holds;
+      remove_key(h, x); put_mru(h, x, IN_T1, block); h->dir.at(x).pinned = was_pinned; h->dir.at(x).holds = holds;
     } else {
       cls = MISS; h->st.miss++;
       int32_t v;
@@ -226,8 +233,8 @@ void access(oracle_cache* h, uint64_t x, uint8_t* cls_out, int32_t* block_out, i
   const uint64_t t1 = h->T1.size(), t2 = h->T2.size(), b1 = h->B1.size(), b2 = h->B2.size();
   if (f != h->dir.end() && (f->second.where == IN_T1 || f->second.where == IN_T2)) {  // case 1
     if (f->second.where == IN_T1) { cls = HIT_T1; h->st.hit_t1++; } else { cls = HIT_T2; h->st.hit_t2++; }
-    int32_t block = f->second.block; bool was_pinned = f->second.pinned;
-    remove_key(h, x); put_mru(h, x, IN_T2, block); h->dir.at(x).pinned = was_pinned;
+    int32_t block = f->second.block; bool was_pinned = f->second.pinned; uint32_t holds = f->second.holds;
+    remove_key(h, x); put_mru(h, x, IN_T2, block); h->dir.at(x).pinned = was_pinned; h->dir.at(x).holds = holds;
   } else if (f != h->dir.end() && f->second.where == IN_B1) {  // case 2
     cls = GHOST_B1; h->st.ghost_b1++;
     uint64_t delta = b2 / b1; if (delta < 1) delta = 1;          // R6: floor, at least 1
@@ -275,6 +282,8 @@ int step_keys(oracle_cache* h, const uint64_t* keys, const int64_t* blk_off, uin
     if ((uint64_t)(blk_off[r + 1] - blk_off[r]) > h->c) return ERR_REQUEST_TOO_LARGE;  // R11: before any change
   const int64_t N = blk_off[n_req];
   if (h->pin_scope == 1 && (uint64_t)N > h->c) return ERR_REQUEST_TOO_LARGE;   // step-wide pins: a step may pin at most c blocks
+  if (h->pin_scope == 2 && h->hold_units + (uint64_t)N > h->c) return ERR_REQUEST_TOO_LARGE;   // holds outstanding + new <= c
+  if (h->pin_scope == 2) h->hold_units += (uint64_t)N;
   h->prefix_len.assign(n_req, 0);
   h->blk_off.assign(blk_off, blk_off + n_req + 1);
   h->cls.assign(N, 0); h->block_id.assign(N, -1); h->evicted_id.assign(N, -1); h->p_after.assign(N, 0);
@@ -326,7 +335,7 @@ int oracle_create(uint64_t capacity_blocks, uint32_t block_size, int policy, ora
   if (policy != POLICY_ARC && policy != POLICY_LRU && policy != POLICY_DBL) return ERR_INVALID_ARG;
   if (block_size == 0 || (block_size & 1)) return ERR_UNSUPPORTED;   // the hash is defined for even B
   oracle_cache* h = new oracle_cache();
-  h->c = capacity_blocks; h->B = block_size; h->policy = policy; h->next_fresh = 0; h->pin_scope = 0;
+  h->c = capacity_blocks; h->B = block_size; h->policy = policy; h->next_fresh = 0; h->pin_scope = 0; h->hold_units = 0;
   h->p = (policy == POLICY_DBL) ? capacity_blocks / 2 : 0;   // DBL: the fixed 1:1 split
   std::memset(&h->st, 0, sizeof(h->st));
   h->hash_seconds = h->arc_seconds = 0.0;
@@ -338,11 +347,40 @@ void oracle_destroy(oracle_cache* h) { delete h; }
 
 // 0 = pins end with their request (R4, default); 1 = with the step (every block a step touches stays resident until the
 // step's last access; a step of more than capacity blocks is refused).
+// 2 = held: every access adds one hold to its block; a block with holds is never a victim; holds
+// end only through oracle_release.  Scope 2 can be entered or left only while nothing is held.
 int oracle_set_pin_scope(oracle_cache* h, int scope) {
-  if (!h || (scope != 0 && scope != 1)) return ERR_INVALID_ARG;
+  if (!h || (scope != 0 && scope != 1 && scope != 2)) return ERR_INVALID_ARG;
+  if (h->hold_units != 0) return ERR_INVALID_ARG;
   h->pin_scope = scope;
   return OK;
 }
+
+// Scope 2: gives back one hold for every block ID listed (a request's block_id output, in any order; an ID may appear
+// several times).  IDs are processed in the order given; a block whose hold count reaches zero moves to the MRU end of
+// the list it is in (T1 or T2) at that moment - the position it had while held never matters, because held blocks are
+// skipped by every victim choice.  All IDs are checked first: an ID that is not a resident block, or that is listed more
+// often than it is held, makes the call fail with no change.
+int oracle_release(oracle_cache* h, const int32_t* ids, uint64_t n) {
+  if (!h || (!ids && n) || h->pin_scope != 2) return ERR_INVALID_ARG;
+  std::unordered_map<int32_t, uint32_t> mult;
+  for (uint64_t i = 0; i < n; ++i) {
+    int32_t id = ids[i];
+    if (id < 0 || (size_t)id >= h->owner.size()) return ERR_INVALID_ARG;
+    std::unordered_map<uint64_t, Entry>::iterator f = h->dir.find(h->owner[id]);
+    if (f == h->dir.end() || f->second.block != id) return ERR_INVALID_ARG;
+    if (++mult[id] > f->second.holds) return ERR_INVALID_ARG;
+  }
+  for (uint64_t i = 0; i < n; ++i) {
+    uint64_t x = h->owner[ids[i]];
+    Entry& e = h->dir.at(x);
+    if (--e.holds == 0) { int where = e.where; int32_t block = e.block; remove_key(h, x); put_mru(h, x, where, block); }
+  }
+  h->hold_units -= n;
+  return OK;
+}
+
+uint64_t oracle_hold_units(oracle_cache* h) { return h->hold_units; }
 
 // Stateless: keys of every full block, natural order (index blk_off[r]+i).  keys_out may be NULL to
 // only fill blk_off_out ([n_req+1]).
@@ -382,6 +420,7 @@ int oracle_step(oracle_cache* h, const int32_t* tokens, const int64_t* offsets, 
   for (uint32_t r = 0; r < n_req; ++r)
     if ((uint64_t)(blk_off[r + 1] - blk_off[r]) > h->c) return ERR_REQUEST_TOO_LARGE;   // before hashing: no state change
   if (h->pin_scope == 1 && (uint64_t)blk_off[n_req] > h->c) return ERR_REQUEST_TOO_LARGE;
+  if (h->pin_scope == 2 && h->hold_units + (uint64_t)blk_off[n_req] > h->c) return ERR_REQUEST_TOO_LARGE;
   h->keys.resize(blk_off[n_req]);
   oracle_hash_blocks(tokens, offsets, n_req, h->B, h->keys.data(), 0);
   double t1 = now_s();
@@ -408,15 +447,18 @@ void oracle_timing(oracle_cache* h, double* hash_seconds, double* arc_seconds) {
 }
 
 // Introspection for the invariant tests: copies list `which` (1=T1, 2=T2, 3=B1, 4=B2) LRU -> MRU into
-// keys_out / blocks_out (either may be NULL), at most cap entries; returns the list length.
+// keys_out / blocks_out (either may be NULL), at most cap entries; returns the list length.  Held entries (scope 2) are
+// left out: their position means nothing until they are released.
 uint64_t oracle_dump_list(oracle_cache* h, int which, uint64_t* keys_out, int32_t* blocks_out, uint64_t cap) {
   KeyList& l = list_of(h, which);
   uint64_t n = 0;
-  for (KeyList::iterator it = l.begin(); it != l.end(); ++it, ++n) {
+  for (KeyList::iterator it = l.begin(); it != l.end(); ++it) {
+    if (h->dir.at(*it).holds > 0) continue;
     if (n < cap) {
       if (keys_out) keys_out[n] = *it;
       if (blocks_out) blocks_out[n] = h->dir.at(*it).block;
     }
+    ++n;
   }
   return n;
 }

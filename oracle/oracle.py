@@ -57,6 +57,9 @@ def lib():
         L.oracle_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(_Result)]
         L.oracle_step_keys.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(_Result)]
         L.oracle_set_pin_scope.argtypes = [C.c_void_p, C.c_int]
+        L.oracle_release.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
+        L.oracle_hold_units.argtypes = [C.c_void_p]
+        L.oracle_hold_units.restype = C.c_uint64
         L.oracle_stats.argtypes = [C.c_void_p, C.POINTER(_Stats)]
         L.oracle_timing.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.oracle_timing.restype = None
@@ -117,6 +120,14 @@ class OracleCache:
         rc = lib().oracle_set_pin_scope(self._h, scope)
         if rc != OK:
             raise ValueError(f"oracle_set_pin_scope: {rc}")
+
+    def release(self, block_ids):
+        """Pin scope 2: one hold back per listed block ID, in order.  Returns 0 or a negative error code (no change)."""
+        ids = np.ascontiguousarray(block_ids, dtype=np.int32)
+        return int(lib().oracle_release(self._h, _ptr(ids), len(ids)))
+
+    def hold_units(self):
+        return int(lib().oracle_hold_units(self._h))
 
     def close(self):
         if self._h:

@@ -98,7 +98,8 @@ class BruteForceCache:
         self.block_of = {}  # resident key -> block ID (ghosts hold no ID, I8)
         self.next_fresh = 0
         self.pinned = set()
-        self.pin_scope = 0  # 0: pins end with their request (R4); 1: with the step (NEXT-3)
+        self.pin_scope = 0  # 0: pins end with their request (R4); 1: with the step (NEXT-3); 2: held (§3.4)
+        self.holds = {}  # scope 2: resident key -> accesses not yet released (absent = 0)
         self.stats = dict(steps=0, requests=0, tokens_seen=0, tokens_hashed=0, accesses=0, hit_t1=0, hit_t2=0,
                           ghost_b1=0, ghost_b2=0, miss=0, evict_t1=0, evict_t2=0, drop_b1=0, drop_b2=0,
                           fresh_ids_used=0, prefix_hit_tokens=0)
@@ -106,7 +107,7 @@ class BruteForceCache:
     # -- R7 -------------------------------------------------------------------------------
     def _first_unpinned(self, lst):
         for x in lst:  # from the LRU end
-            if x not in self.pinned:
+            if x not in self.pinned and self.holds.get(x, 0) == 0:
                 return x
         return None
 
@@ -152,7 +153,7 @@ class BruteForceCache:
                     st["evict_t1"] += 1
                 self.T1.append(x)
                 self.block_of[x] = v
-            self.pinned.add(x)
+            self._pin(x)
             return cls, self.block_of[x], evicted
 
         t1, t2, b1, b2 = len(self.T1), len(self.T2), len(self.B1), len(self.B2)  # read before any change
@@ -213,8 +214,36 @@ class BruteForceCache:
                     st["fresh_ids_used"] += 1
             self.T1.append(x)
             self.block_of[x] = v
-        self.pinned.add(x)  # R4
+        self._pin(x)  # R4
         return cls, self.block_of[x], evicted
+
+    def _pin(self, x):
+        if self.pin_scope == 2:
+            self.holds[x] = self.holds.get(x, 0) + 1  # held until released: one hold per access
+        else:
+            self.pinned.add(x)
+
+    # -- scope 2: one hold back per listed block ID, in order; at zero the block goes to the MRU end
+    def release(self, block_ids):
+        key_of = {b: x for x, b in self.block_of.items()}
+        left = dict(self.holds)
+        for b in block_ids:  # check everything first: a bad ID fails the call with no change
+            x = key_of.get(int(b))
+            if x is None or left.get(x, 0) == 0:
+                return ERR_INVALID_ARG
+            left[x] -= 1
+        for b in block_ids:
+            x = key_of[int(b)]
+            self.holds[x] -= 1
+            if self.holds[x] == 0:
+                del self.holds[x]
+                lst = self.T1 if x in self.T1 else self.T2
+                lst.remove(x)
+                lst.append(x)
+        return 0
+
+    def hold_units(self):
+        return sum(self.holds.values())
 
     # -- R2, R3, R4, R9: one step over lists of keys (block 0 first inside each request) ----------
     def step_keys(self, requests_keys):
@@ -224,6 +253,8 @@ class BruteForceCache:
                 return ERR_REQUEST_TOO_LARGE  # R11: no state change
         if self.pin_scope == 1 and sum(len(k) for k in requests_keys) > self.c:
             return ERR_REQUEST_TOO_LARGE  # step-wide pins: the step may pin at most c blocks (admission rule)
+        if self.pin_scope == 2 and self.hold_units() + sum(len(k) for k in requests_keys) > self.c:
+            return ERR_REQUEST_TOO_LARGE  # held: holds outstanding plus the step's accesses may not exceed c
         out = dict(prefix_len=[], blk_off=[0], cls=[], block_id=[], evicted_id=[], p_after=[], alloc_ids=[], evict_ids=[])
         for keys in requests_keys:  # R2: requests in ascending index
             nb = len(keys)

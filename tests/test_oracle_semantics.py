@@ -376,3 +376,143 @@ def test_step_wide_pins_differential_and_invariants(policy):
                 assert list(a[k]) == b[k].tolist(), (c, policy, k)
             L = cpp.lists()
             check_invariants(L, c, policy_lru=(policy == 1))
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# NEXT-3, held pins with explicit release
+
+def _make_held(impl, c, policy=0):
+    cch = BF.BruteForceCache(c, 16, policy) if impl == "bf" else O.OracleCache(c, 16, policy)
+    if impl == "bf":
+        cch.pin_scope = 2
+    else:
+        cch.set_pin_scope(2)
+    return cch
+
+
+def _unheld(cch, impl, n):
+    """names of the unheld entries of every list, LRU -> MRU"""
+    L = cch.lists()
+    if impl == "bf":
+        return {k: n.names([x for x in L[k] if cch.holds.get(x, 0) == 0]) for k in ("T1", "T2", "B1", "B2")}
+    return {k: n.names(L[k][0]) for k in ("T1", "T2", "B1", "B2")}
+
+
+@pytest.mark.parametrize("impl", ["bf", "cpp"])
+def test_held_pins_hand_trace_H(impl):
+    """c = 4, ARC, pin scope 2.  Worked by hand from R5/R7 and the release rule of DESIGN.md §3.4: a block with holds is
+    never a victim; a block re-enters at the MRU end of its list when its last hold is released, in the order of the
+    release call; a step is refused when holds outstanding + its accesses exceed c."""
+    from helpers import KeyNames
+
+    n = KeyNames()
+    cch = _make_held(impl, 4)
+    A, B, Cq = _keys(["A0", "A1"], n), _keys(["B0", "B1"], n), _keys(["C0", "C1"], n)
+    o = cch.step_keys([A])
+    assert list(o["block_id"]) == [1, 0] and list(o["cls"]) == [0, 0]
+    o = cch.step_keys([B])
+    assert list(o["block_id"]) == [3, 2] and cch.hold_units() == 4
+    assert cch.step_keys([_keys(["C0"], n)]) == O.ERR_REQUEST_TOO_LARGE          # 4 holds outstanding + 1 > c
+    assert _unheld(cch, impl, n) == dict(T1=[], T2=[], B1=[], B2=[])
+    assert cch.release([1, 0]) == 0 and cch.hold_units() == 2                    # A0 first, then A1
+    assert _unheld(cch, impl, n)["T1"] == ["A0", "A1"]
+    # T1 holds everything (t1 = c, no ghosts): case 4A-else evicts T1's first unheld entry without a ghost: A0, then A1
+    o = cch.step_keys([Cq])
+    assert list(o["cls"]) == [0, 0] and list(o["block_id"]) == [0, 1] and list(o["evicted_id"]) == [0, 1]
+    assert cch.release([3, 2]) == 0 and cch.release([0, 1]) == 0 and cch.hold_units() == 0
+    assert _unheld(cch, impl, n) == dict(T1=["B0", "B1", "C0", "C1"], T2=[], B1=[], B2=[])
+    o = cch.step_keys([B])
+    assert list(o["cls"]) == [1, 1] and list(o["prefix_len"]) == [32]
+    assert _unheld(cch, impl, n) == dict(T1=["C0", "C1"], T2=[], B1=[], B2=[])   # B0, B1 are in T2 but held
+    assert cch.release([3, 2]) == 0
+    assert _unheld(cch, impl, n)["T2"] == ["B0", "B1"]
+    o = cch.step_keys([_keys(["D0"], n)])                                        # REPLACE: t1 = 2 > p = 0 -> T1's LRU entry C0
+    assert list(o["cls"]) == [0] and list(o["block_id"]) == [0] and list(o["evicted_id"]) == [0]
+    assert _unheld(cch, impl, n) == dict(T1=["C1"], T2=["B0", "B1"], B1=["C0"], B2=[])
+    assert cch.release([0]) == 0
+    o = cch.step_keys([_keys(["B0"], n), _keys(["B0"], n)])                      # two requests hold the same block
+    assert list(o["cls"]) == [2, 2] and list(o["prefix_len"]) == [16, 16] and cch.hold_units() == 2
+    assert cch.release([3]) == 0 and cch.hold_units() == 1                       # one hold left: B0 stays out of reach
+    assert _unheld(cch, impl, n)["T2"] == ["B1"]
+    o = cch.step_keys([_keys(["E0", "E1"], n)])
+    # E1: n = 5 >= c -> REPLACE takes C1 (ID 1) from T1;  E0: t1 + b1 = c -> drop B1's LRU ghost C0, REPLACE takes D0 (ID 0)
+    assert list(o["cls"]) == [0, 0] and list(o["block_id"]) == [0, 1] and list(o["evicted_id"]) == [0, 1]
+    assert _unheld(cch, impl, n) == dict(T1=[], T2=["B1"], B1=["C1", "D0"], B2=[])
+    assert cch.release([3]) == 0
+    assert _unheld(cch, impl, n)["T2"] == ["B1", "B0"]
+    assert cch.release([3]) == O.ERR_INVALID_ARG                                 # nothing left to release: refused, no change
+    assert cch.release([0, 1]) == 0 and cch.hold_units() == 0
+    assert _unheld(cch, impl, n) == dict(T1=["E0", "E1"], T2=["B1", "B0"], B1=["C1", "D0"], B2=[])
+    st = cch.stats if impl == "bf" else cch.stats()
+    assert st["evict_t1"] == 5 and st["drop_b1"] == 1 and st["hit_t1"] == 2 and st["hit_t2"] == 2
+
+
+@pytest.mark.parametrize("policy", [0, 1, 2])
+def test_held_pins_released_in_access_order_equal_request_scope(policy):
+    """If every request is released right after its own batch-1 step, tail block first (the access order R2), the held
+    scope is the default scope: same outputs, same lists.  Pins the release rule to the already pinned R4 semantics."""
+    rng = np.random.default_rng(410 + policy)
+    for c in (3, 6, 16):
+        ref, held = O.OracleCache(c, 16, policy), O.OracleCache(c, 16, policy)
+        held.set_pin_scope(2)
+        for _ in range(400):
+            nb = int(rng.integers(1, min(c, 5) + 1))
+            base = int(rng.integers(0, 6))
+            req = [[5000 + 100 * base + i for i in range(nb)]]
+            a, b = ref.step_keys(req), held.step_keys(req)
+            for k in ("cls", "block_id", "evicted_id", "p_after", "prefix_len", "alloc_ids", "evict_ids"):
+                assert a[k].tolist() == b[k].tolist(), (c, policy, k)
+            assert held.release(b["block_id"][::-1]) == 0
+            La, Lb = ref.lists(), held.lists()
+            for k in ("T1", "T2", "B1", "B2"):
+                assert La[k][0].tolist() == Lb[k][0].tolist() and La[k][1].tolist() == Lb[k][1].tolist(), (c, policy, k)
+
+
+@pytest.mark.parametrize("policy", [0, 1, 2])
+def test_held_pins_differential_and_invariants(policy):
+    """Brute force against the C++ oracle under random steps and random releases (whole requests, in random order, some
+    sharing blocks so that hold counts exceed one); held blocks are resident and never evicted."""
+    rng = np.random.default_rng(500 + policy)
+    for c in (3, 5, 9):
+        bf, cpp = BF.BruteForceCache(c, 16, policy), O.OracleCache(c, 16, policy)
+        bf.pin_scope = 2
+        cpp.set_pin_scope(2)
+        live = []                     # block-ID arrays of the requests not yet released
+        for it in range(400):
+            if live and (rng.random() < 0.5 or cpp.hold_units() > c - 2):
+                k = int(rng.integers(0, len(live)))
+                ids = live.pop(k)
+                ids = ids[rng.permutation(len(ids))]
+                if len(live) and rng.random() < 0.3:      # two requests in one call
+                    ids = np.concatenate([ids, live.pop(int(rng.integers(0, len(live))))])
+                assert bf.release(ids.tolist()) == 0 and cpp.release(ids) == 0
+            else:
+                reqs, left = [], c - cpp.hold_units()
+                while left > 0 and rng.random() < 0.7:
+                    nb = int(rng.integers(1, min(left, 3) + 1))
+                    base = int(rng.integers(0, 4))
+                    reqs.append([1000 + 10 * base + i for i in range(nb)])
+                    left -= nb
+                held_before = {x: h for x, h in bf.holds.items()}
+                a, b = bf.step_keys(reqs), cpp.step_keys(reqs)
+                for k in ("cls", "block_id", "evicted_id", "p_after", "prefix_len", "alloc_ids", "evict_ids"):
+                    assert list(a[k]) == b[k].tolist(), (c, policy, k)
+                off = b["blk_off"]
+                for r in range(len(reqs)):
+                    live.append(b["block_id"][off[r]:off[r + 1]].copy())
+                resident = set(bf.T1) | set(bf.T2)
+                assert set(held_before) <= resident, "a held block was evicted"
+            assert bf.hold_units() == cpp.hold_units() == sum(len(x) for x in live)
+            Lb, Lc = bf.lists(), cpp.lists()
+            for k in ("T1", "T2", "B1", "B2"):
+                assert [x for x in Lb[k] if bf.holds.get(x, 0) == 0] == Lc[k][0].tolist(), (c, policy, k, it)
+            sc = cpp.stats()
+            assert (len(bf.T1), len(bf.T2), len(bf.B1), len(bf.B2), bf.p) == (sc["t1"], sc["t2"], sc["b1"], sc["b2"], sc["p"])
+        # over-releasing and unknown IDs are refused without a change
+        before = cpp.lists()
+        assert cpp.release(np.array([c + 5], np.int32)) == O.ERR_INVALID_ARG
+        if live:
+            twice = np.concatenate([live[0], live[0], live[0], live[0]])
+            if cpp.release(twice) == O.ERR_INVALID_ARG:
+                after = cpp.lists()
+                assert all(before[k][0].tolist() == after[k][0].tolist() for k in ("T1", "T2", "B1", "B2"))
