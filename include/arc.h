@@ -43,7 +43,8 @@ enum {
 };
 /* Scope of the pins (R4): a block accessed by a request is never a victim until ... */
 enum { ARC_PIN_REQUEST = 0,   /* ... its request's last access (default)                                                  */
-       ARC_PIN_STEP = 1 };    /* ... the step's last access: everything a step touches stays resident for the whole step */
+       ARC_PIN_STEP = 1,      /* ... the step's last access: everything a step touches stays resident for the whole step */
+       ARC_PIN_HELD = 2 };    /* ... arc_release gives the access's hold back (one hold per access, across steps)           */
 /* class of one block access, as decided against the live state at the moment of the access (R3, R5) */
 enum { ARC_MISS = 0, ARC_HIT_T1 = 1, ARC_HIT_T2 = 2, ARC_GHOST_B1 = 3, ARC_GHOST_B2 = 4 };
 
@@ -127,7 +128,23 @@ int arc_step_host(arc_cache *h, const int32_t *h_tokens, const int64_t *h_offset
 /* Sets the pin scope for the following steps.  With ARC_PIN_STEP a step whose
  * requests hold more than capacity_blocks full blocks in total is refused with ARC_ERR_REQUEST_TOO_LARGE (nothing is
  * enqueued, the handle is unchanged): the admission rule that guarantees a victim always exists. */
+/* With ARC_PIN_HELD every access adds one hold to its block; a block with holds is never a victim, in
+ * this step or any later one, until arc_release has given all its holds back.  A step is refused with
+ * ARC_ERR_REQUEST_TOO_LARGE when the holds outstanding plus its full blocks exceed capacity_blocks.  The scope can be
+ * changed only while no hold is outstanding (else ARC_ERR_INVALID_ARG).  Steps under ARC_PIN_HELD run the one-warp K3
+ * machine (or the serial one if arc_set_machine asked for it). */
 int arc_set_pin_scope(arc_cache *h, int scope);
+
+/* ARC_PIN_HELD only: gives back one hold for every block ID listed - normally a finished request's block_id output, in
+ * any order; an ID may appear several times.  d_block_ids: DEVICE int32[n], read in stream order.  The IDs are processed
+ * in the order given; a block whose last hold goes re-enters the list it belongs to (T1 or T2) at the MRU end at that
+ * moment.  Asynchronous.  n greater than the holds outstanding -> ARC_ERR_INVALID_ARG, nothing enqueued.  An ID that is
+ * not a resident held block, or is listed more often than it is held, is found on the device: the call then changes
+ * nothing and the handle carries a sticky device error that the next arc_stats reports as ARC_ERR_CUDA. */
+int arc_release(arc_cache *h, const int32_t *d_block_ids, uint64_t n, void *cuda_stream);
+
+/* Holds outstanding (accesses made under ARC_PIN_HELD minus IDs released); host-side, exact, no synchronisation. */
+uint64_t arc_hold_units(const arc_cache *h);
 
 /* Synchronises the stream of the handle's last step and copies the counters.  out: HOST. */
 int arc_stats(arc_cache *h, arc_stats_t *out);

@@ -15,7 +15,7 @@ import numpy as np
 from . import build as _build
 
 POLICY_ARC, POLICY_LRU, POLICY_DBL = 0, 1, 2
-PIN_REQUEST, PIN_STEP = 0, 1
+PIN_REQUEST, PIN_STEP, PIN_HELD = 0, 1, 2
 MISS, HIT_T1, HIT_T2, GHOST_B1, GHOST_B2 = 0, 1, 2, 3, 4
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_REQUEST_TOO_LARGE, ERR_OOM, ERR_CUDA = 0, -1, -2, -3, -4, -5
 
@@ -26,7 +26,8 @@ STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", 
 # every symbol include/arc.h declares (checked by the CPU test-suite against the built library)
 EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats", "arc_reset", "arc_destroy",
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
-           "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe", "arc_set_pin_scope"]
+           "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe", "arc_set_pin_scope",
+           "arc_release", "arc_hold_units"]
 
 
 class ArcError(RuntimeError):
@@ -88,6 +89,9 @@ def load_library(path: Optional[Path] = None):
     L.arc_debug_set_key_mask.argtypes = [vp, u64]
     L.arc_debug_probe.argtypes = [vp, vp, u64, vp, vp]
     L.arc_set_pin_scope.argtypes = [vp, C.c_int]
+    L.arc_release.argtypes = [vp, vp, u64, vp]
+    L.arc_hold_units.argtypes = [vp]
+    L.arc_hold_units.restype = u64
     L.arc_debug_list.argtypes = [vp, C.c_int, vp, vp, u64, C.POINTER(u64)]
     if path is None:
         _lib = L
@@ -239,6 +243,20 @@ class ArcCache:
 
     def set_pin_scope(self, scope: int):
         self._check(self._L.arc_set_pin_scope(self._h, scope))
+
+    def release(self, block_ids, stream=None):
+        """PIN_HELD: one hold back per listed block ID (a CUDA int32 tensor, or anything numpy can read: copied to the
+        device first).  Asynchronous on the current stream."""
+        torch = _torch()
+        if not (hasattr(block_ids, "is_cuda") and block_ids.is_cuda):
+            block_ids = torch.from_numpy(np.ascontiguousarray(block_ids, dtype=np.int32)).cuda()
+        if block_ids.dtype != torch.int32 or not block_ids.is_contiguous():
+            block_ids = block_ids.to(torch.int32).contiguous()
+        self._keep_release = block_ids          # stays alive until the kernel has read it (next call replaces it)
+        self._check(self._L.arc_release(self._h, block_ids.data_ptr(), block_ids.numel(), _stream_ptr(stream)))
+
+    def hold_units(self) -> int:
+        return int(self._L.arc_hold_units(self._h))
 
     def set_machine(self, which: int):
         self._check(self._L.arc_set_machine(self._h, which))

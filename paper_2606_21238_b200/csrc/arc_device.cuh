@@ -21,6 +21,9 @@ constexpr unsigned long long KEY_EMPTY = 0ull, KEY_TOMB = 1ull;  // H5 keeps rea
 constexpr uint32_t SLOT_NODE_PENDING = 0;        // Slot::node holds node id + 1; 0 (what the table memset leaves) =
                                                  // slot claimed by a key whose node id is not yet published
 constexpr uint32_t NODE_NONE = 0xFFFFFFFFu;
+constexpr uint32_t NODE_HELD = 0x100u;           // Node::list flag (pin scope 2): the node is resident, has holds and is in NO ring;
+                                                 // Node::pos then carries the hold count instead of a ring position
+constexpr uint32_t NODE_LIST_MASK = 0xFFu;
 constexpr uint32_t SLOT_FLAG = 0x80000000u;      // node_acc entry holds a slot index to resolve, not a node id
 constexpr uint32_t BUCKET_SLOTS = 8;             // 8 x 16 B = one 128 B line
 
@@ -53,7 +56,7 @@ struct __align__(16) Slot {
 enum : int { ST_HIT_T1 = 0, ST_HIT_T2, ST_GHOST_B1, ST_GHOST_B2, ST_MISS, ST_EVICT_T1, ST_EVICT_T2, ST_DROP_B1,
              ST_DROP_B2, ST_FRESH, ST_PREFIX_TOKENS, ST_ACCESSES, ST_COUNT };
 enum : uint32_t { DEV_ERR_NONE = 0, DEV_ERR_NODE_POOL = 1, DEV_ERR_NO_VICTIM = 2, DEV_ERR_RING_OVERFLOW = 3,
-                  DEV_ERR_BAD_NODE = 4 };
+                  DEV_ERR_BAD_NODE = 4, DEV_ERR_BAD_RELEASE = 5 };
 
 struct DevState {
   uint32_t head[5], tail[5];      // per list (index L_T1..L_B2); wrapping 32-bit absolute positions
@@ -70,6 +73,9 @@ struct DevState {
   uint32_t cmp_head, cmp_tail;
   // K3 diagnostics, cumulative (arc_debug_counters): see DBG_* below
   unsigned long long dbg[32];
+  // pin scope 2: entries of T1 / T2 without holds (= the entries in the rings = the possible victims), kept across steps
+  int32_t u1, u2;
+  uint32_t release_bad;           // scratch of release_kernel
 };
 enum : int { DBG_WIN_HIT = 0, DBG_WIN_GENERAL, DBG_WIN_SERIAL, DBG_CUT_TWIN, DBG_CUT_CONFLICT, DBG_SCAN_ROUNDS, DBG_ACC_HIT_WIN,
              DBG_ACC_GENERAL_WIN, DBG_CYC_FETCH, DBG_CYC_ROLL, DBG_CYC_SCAN, DBG_CYC_APPLY, DBG_CYC_SERIAL, DBG_CYC_TOTAL, DBG_ROLL_CALLS, DBG_ROLL_PHASES, DBG_COUNT };
@@ -105,7 +111,8 @@ struct StepParams {
   int32_t capacity;
   int32_t policy;
   uint32_t block_size;
-  int32_t pin_scope;              // 0: pins end with their request, 1: with the step
+  int32_t pin_scope;              // 0: pins end with their request, 1: with the step, 2: held until arc_release
+  uint32_t* node_of_block;        // pin scope 2: node id of the resident entry that owns each block id
   unsigned long long key_and;     // test hook (arc_debug_set_key_mask): keys are ANDed with this before the probe; all ones normally
 };
 

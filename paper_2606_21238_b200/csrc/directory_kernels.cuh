@@ -295,4 +295,77 @@ __global__ void __launch_bounds__(CMP_THREADS) dump_list_kernel(const DevState* 
   if (threadIdx.x == 0) *n_out = s_done;
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// arc_release (pin scope 2): one hold back per listed block id, in the order given; a block whose last
+// hold goes re-enters its list (T1 or T2) at the MRU end.  One CTA: all 256 threads check the whole call first (every id a
+// resident held block, none listed more often than it is held - else nothing changes and the handle gets the sticky
+// error DEV_ERR_BAD_RELEASE), then warp 0 applies it 32 ids at a time: equal ids inside a chunk are grouped with
+// match_any and the group's LAST lane acts for it, which is the position the by-the-book walk zeroes the count at.
+// rel_cnt[capacity] is all zero between calls.
+__global__ void __launch_bounds__(256) release_kernel(const __grid_constant__ StepParams P, const int32_t* ids, uint32_t n,
+                                                      uint32_t* rel_cnt) {
+  __shared__ uint32_t s_bad;
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
+  DevState* S = P.state;
+  if (tid == 0) s_bad = 0;
+  __syncthreads();
+  for (uint32_t i = tid; i < n; i += 256) {
+    const int32_t id = ids[i];
+    bool ok = id >= 0 && id < P.capacity;
+    if (ok) {
+      const uint32_t nd = P.node_of_block[id];
+      ok = nd != NODE_NONE;
+      if (ok) { const Node r = ld_node(P.nodes + nd); ok = (r.list & NODE_HELD) && r.block == id; }
+    }
+    if (ok) atomicAdd(&rel_cnt[id], 1u); else s_bad = 1;
+  }
+  __syncthreads();
+  if (!s_bad) {
+    for (uint32_t i = tid; i < n; i += 256) {
+      const int32_t id = ids[i];
+      if (__ldcg(&rel_cnt[id]) > ld_node(P.nodes + P.node_of_block[id]).pos) s_bad = 1;
+    }
+  }
+  __syncthreads();
+  const bool bad = s_bad != 0;
+  if (!bad && tid < 32) {
+    uint32_t tail1 = S->tail[L_T1], tail2 = S->tail[L_T2];
+    int32_t u1 = S->u1, u2 = S->u2;
+    for (uint32_t base = 0; base < n; base += 32) {
+      const bool valid = base + lane < n;
+      const int32_t id = valid ? ids[base + lane] : -1;
+      const uint32_t nd = valid ? P.node_of_block[id] : (0xF0000000u | lane);
+      Node r;
+      r.list = 0; r.pos = 0; r.block = -1; r.slot = 0;
+      if (valid) r = ld_node(P.nodes + nd);
+      const uint32_t grp = __match_any_sync(FULL, nd);
+      const bool rep = valid && (31u - (uint32_t)__clz(grp)) == lane;
+      const uint32_t left = r.pos - (uint32_t)__popc(grp);
+      const bool zero = rep && left == 0;
+      const uint32_t L = r.list & NODE_LIST_MASK;
+      const uint32_t z1 = __ballot_sync(FULL, zero && L == L_T1), z2 = __ballot_sync(FULL, zero && L == L_T2);
+      if (zero) {
+        const uint32_t q = (L == L_T1) ? tail1 + (uint32_t)__popc(z1 & lt) : tail2 + (uint32_t)__popc(z2 & lt);
+        __stcg(((L == L_T1) ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(nd, r.block));
+        st_node(P.nodes + nd, L, q, r.block, r.slot);
+      } else if (rep) {
+        st_node(P.nodes + nd, r.list, left, r.block, r.slot);
+      }
+      tail1 += (uint32_t)__popc(z1); tail2 += (uint32_t)__popc(z2);
+      u1 += __popc(z1); u2 += __popc(z2);
+      __syncwarp();
+    }
+    if (lane == 0) { S->tail[L_T1] = tail1; S->tail[L_T2] = tail2; S->u1 = u1; S->u2 = u2; }
+  }
+  __syncthreads();
+  for (uint32_t i = tid; i < n; i += 256) {
+    const int32_t id = ids[i];
+    if (id >= 0 && id < P.capacity) rel_cnt[id] = 0;
+  }
+  if (bad && tid == 0) S->error = DEV_ERR_BAD_RELEASE;
+}
+
+// entering pin scope 2 with nothing held: every resident entry is in a ring
+__global__ void set_unheld_kernel(DevState* st) { st->u1 = st->t1; st->u2 = st->t2; }
+
 }  // namespace arc

@@ -80,6 +80,10 @@ struct arc_cache {
   uint8_t* d_cls = nullptr;
   int32_t *d_block_id = nullptr, *d_evicted_id = nullptr, *d_p_after = nullptr, *d_alloc_ids = nullptr, *d_evict_ids = nullptr;
   void* d_machine_scratch = nullptr;
+  // pin scope 2 (held): block id -> node id, per-block scratch of arc_release, holds outstanding (host-side, exact)
+  uint32_t* d_node_of_block = nullptr;
+  uint32_t* d_rel_cnt = nullptr;
+  uint64_t hold_units = 0;
   // host staging
   int64_t* h_stage = nullptr;     // pinned, kStageSlots * 2 * (req_cap + 1)
   cudaEvent_t stage_done[kStageSlots] = {};
@@ -135,6 +139,7 @@ StepParams make_params(arc_cache* h) {
   P.prefix_len = h->d_prefix_len; P.cls = h->d_cls; P.block_id = h->d_block_id; P.evicted_id = h->d_evicted_id;
   P.p_after = h->d_p_after; P.alloc_ids = h->d_alloc_ids; P.evict_ids = h->d_evict_ids;
   P.capacity = (int32_t)h->c; P.policy = h->policy; P.block_size = h->B; P.key_and = h->key_and; P.pin_scope = h->pin_scope;
+  P.node_of_block = h->d_node_of_block;
   return P;
 }
 
@@ -369,6 +374,9 @@ int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, ui
   if (rc) return rc;
   if (h->pin_scope == ARC_PIN_STEP && N > h->c)
     return fail(h, ARC_ERR_REQUEST_TOO_LARGE, "step-wide pins: the step holds %llu blocks > capacity %llu", (unsigned long long)N, (unsigned long long)h->c);
+  if (h->pin_scope == ARC_PIN_HELD && h->hold_units + N > h->c)
+    return fail(h, ARC_ERR_REQUEST_TOO_LARGE, "held pins: %llu holds outstanding + %llu blocks in the step > capacity %llu",
+                (unsigned long long)h->hold_units, (unsigned long long)N, (unsigned long long)h->c);
   if (!d_tokens && h_offsets[n_req] > h_offsets[0]) return fail(h, ARC_ERR_INVALID_ARG, "d_tokens is NULL");
 
   rc = ensure_capacity(h, n_req, N, s);
@@ -402,7 +410,7 @@ int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, ui
   if (h->profiling) cudaEventRecord(h->ev[3], s);
   if (h->machine == 1) {
     arc_machine_serial_kernel<<<1, 32, 0, s>>>(P);                                                       // K3 (serial)
-  } else if (h->machine == 2 || (h->machine == 0 && N < 48ull * n_req)) {
+  } else if (h->machine == 2 || h->pin_scope == ARC_PIN_HELD || (h->machine == 0 && N < 48ull * n_req)) {
     // one warp, 32-wide windows: a window of the wide machine costs about twice as much, which only pays when requests
     // are long enough to fill it (windows never cross a request boundary)
     launch_machine_batched(P, s);
@@ -417,6 +425,7 @@ int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, ui
 
   h->slots_used_bound += N;
   for (int L = 1; L <= 4; ++L) h->window_bound[L] += N;
+  if (h->pin_scope == ARC_PIN_HELD) h->hold_units += N;
   h->steps += 1; h->requests += n_req;
   h->tokens_seen += (uint64_t)(h_offsets[n_req] - h_offsets[0]);
   h->tokens_hashed += N * h->B;
@@ -489,7 +498,7 @@ int arc_stats(arc_cache* h, arc_stats_t* out) {
   // we are synchronised: tighten the host-side bounds with the true values
   h->slots_used_bound = (uint64_t)st.t1 + st.t2 + st.b1 + st.b2 + st.tombs;
   for (int L = 1; L <= 4; ++L) h->window_bound[L] = (uint32_t)(st.tail[L] - st.head[L]);
-  if (st.error) return fail(h, ARC_ERR_CUDA, "device-side directory error %u (1 node pool, 2 no victim, 3 ring overflow, 4 bad node)", st.error);
+  if (st.error) return fail(h, ARC_ERR_CUDA, "device-side directory error %u (1 node pool, 2 no victim, 3 ring overflow, 4 bad node, 5 bad release)", st.error);
   return ARC_OK;
 }
 
@@ -502,6 +511,8 @@ int arc_reset(arc_cache* h) {
   CUDA_TRY(h, cudaStreamSynchronize(s));
   h->slots_used_bound = 0;
   for (int L = 1; L <= 4; ++L) h->window_bound[L] = 0;
+  if (h->d_node_of_block) CUDA_TRY(h, cudaMemset(h->d_node_of_block, 0xFF, (size_t)h->c * sizeof(uint32_t)));
+  h->hold_units = 0;
   h->steps = h->requests = h->tokens_seen = h->tokens_hashed = 0;
   h->launches = 0;
   h->ev_valid = false;
@@ -515,6 +526,7 @@ void arc_destroy(arc_cache* h) {
   dfree(h->d_state); dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_table);
   for (int L = 1; L <= 4; ++L) { dfree(h->d_ring[L]); dfree(h->d_ring_alt[L]); }
   dfree(h->d_block_counts); dfree(h->d_tokens_stage); dfree(h->d_machine_scratch);
+  dfree(h->d_node_of_block); dfree(h->d_rel_cnt);
   for (int i = 0; i < kStageSlots; ++i) if (h->stage_done[i]) cudaEventDestroy(h->stage_done[i]);
   for (int i = 0; i < 7; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
   delete h;
@@ -601,10 +613,43 @@ int arc_set_machine(arc_cache* h, int which) {
 
 int arc_set_pin_scope(arc_cache* h, int scope) {
   if (!h) return ARC_ERR_INVALID_ARG;
-  if (scope != ARC_PIN_REQUEST && scope != ARC_PIN_STEP) return fail(h, ARC_ERR_INVALID_ARG, "unknown pin scope %d", scope);
+  if (scope != ARC_PIN_REQUEST && scope != ARC_PIN_STEP && scope != ARC_PIN_HELD) return fail(h, ARC_ERR_INVALID_ARG, "unknown pin scope %d", scope);
+  if (h->hold_units) return fail(h, ARC_ERR_INVALID_ARG, "%llu holds outstanding: release them before changing the pin scope", (unsigned long long)h->hold_units);
+  if (scope == ARC_PIN_HELD && h->pin_scope != ARC_PIN_HELD) {
+    if (!h->d_node_of_block) {
+      CUDA_TRY(h, dalloc(&h->d_node_of_block, h->c));
+      CUDA_TRY(h, dalloc(&h->d_rel_cnt, h->c));
+      CUDA_TRY(h, cudaMemset(h->d_node_of_block, 0xFF, (size_t)h->c * sizeof(uint32_t)));
+      CUDA_TRY(h, cudaMemset(h->d_rel_cnt, 0, (size_t)h->c * sizeof(uint32_t)));
+    }
+    set_unheld_kernel<<<1, 1, 0, h->last_stream>>>(h->d_state);      // nothing is held: every resident entry is in a ring
+    h->launches += 1;
+    CUDA_TRY(h, cudaGetLastError());
+  }
   h->pin_scope = scope;
   return ARC_OK;
 }
+
+int arc_release(arc_cache* h, const int32_t* d_block_ids, uint64_t n, void* cuda_stream) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  if (h->pin_scope != ARC_PIN_HELD) return fail(h, ARC_ERR_INVALID_ARG, "arc_release needs pin scope ARC_PIN_HELD");
+  if (n && !d_block_ids) return fail(h, ARC_ERR_INVALID_ARG, "d_block_ids is NULL");
+  if (n > h->hold_units) return fail(h, ARC_ERR_INVALID_ARG, "%llu ids released but only %llu holds are outstanding", (unsigned long long)n, (unsigned long long)h->hold_units);
+  if (!n) return ARC_OK;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int rc = maintain(h, n, s);            // room for up to n pushes at the MRU ends of T1 / T2
+  if (rc) return rc;
+  StepParams P = make_params(h);
+  release_kernel<<<1, 256, 0, s>>>(P, d_block_ids, (uint32_t)n, h->d_rel_cnt);
+  h->launches += 1;
+  CUDA_TRY(h, cudaGetLastError());
+  h->window_bound[L_T1] += n; h->window_bound[L_T2] += n;
+  h->hold_units -= n;
+  h->last_stream = s;
+  return ARC_OK;
+}
+
+uint64_t arc_hold_units(const arc_cache* h) { return h ? h->hold_units : 0; }
 
 int arc_debug_probe(arc_cache* h, const uint64_t* d_keys, uint64_t n, uint32_t* d_nodes_out, void* cuda_stream) {
   if (!h) return ARC_ERR_INVALID_ARG;

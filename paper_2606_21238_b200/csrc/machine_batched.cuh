@@ -231,6 +231,7 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
   const int lane = threadIdx.x;
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
   const bool lru = (P.policy == POLICY_LRU);
+  const bool hold = (P.pin_scope == 2);
   const int32_t c = P.capacity;
   const int64_t N = (int64_t)P.n_access;
   SerialCtx C;            // identical in every lane
@@ -251,7 +252,10 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
       my_off = P.blk_off[rr]; my_off1 = P.blk_off[rr + 1];
     }
     const int64_t o = __shfl_sync(FULL, my_off, r & 31), nb = __shfl_sync(FULL, my_off1, r & 31) - o;
-    if (r == 0 || P.pin_scope == 0) begin_request(C);   // step-wide scope: the pins of earlier requests of the step stay
+    // step-wide scope: the pins of earlier requests of the step stay.  Held scope (2): accessed nodes leave the rings and
+    // come back through arc_release, so every ring entry is a possible victim (bound = tail), no tail of T1 / T2 moves
+    // during a step, and elig1 / elig2 (the unheld entries) carry over from step to step in DevState.
+    if (!hold && (r == 0 || P.pin_scope == 0)) begin_request(C);
     int64_t j = 0;
     while (j < nb) {
       const int kmax = (int)min((int64_t)32, nb - j);
@@ -281,13 +285,14 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
       const uint32_t dupm = __ballot_sync(FULL, act0 && (twins & lt));
       if (dupm) { k = __ffs(dupm) - 1; dbg[DBG_CUT_TWIN]++; }
       uint32_t km = bits_from(0, k);
-      const uint32_t lst = rec.list;
+      const uint32_t lst = rec.list & NODE_LIST_MASK;
+      const bool held = (rec.list & NODE_HELD) != 0;            // held scope: in no ring, rec.pos = its holds
       const uint32_t m0 = __ballot_sync(FULL, lst & 1u), m1 = __ballot_sync(FULL, lst & 2u), m2 = __ballot_sync(FULL, lst & 4u);
       if (m2 & m0 & km) C.err = DEV_ERR_BAD_NODE;                 // a FREE node reached K3
       const uint32_t hitm = lru ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);   // list T1 (LRU) / T1 or T2 (ARC)
       // hits on entries that were still evictable by this request (below bound): they stop being so
-      const uint32_t me = __ballot_sync(FULL, (lst == L_T1 && (int32_t)(C.bound[L_T1] - rec.pos) > 0) ||
-                                                  (lst == L_T2 && (int32_t)(C.bound[L_T2] - rec.pos) > 0));
+      const uint32_t me = __ballot_sync(FULL, !held && ((lst == L_T1 && (int32_t)(C.bound[L_T1] - rec.pos) > 0) ||
+                                                            (lst == L_T2 && (int32_t)(C.bound[L_T2] - rec.pos) > 0)));
       const long long tw1 = clock64();
       dbg[DBG_CYC_FETCH] += (unsigned long long)(tw1 - tw0);
 
@@ -297,9 +302,14 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
         const uint32_t Lp = lru ? L_T1 : L_T2;
         if (lane < k) {
           const uint32_t q = (lru ? C.tail[L_T1] : C.tail[L_T2]) + (uint32_t)lane;
-          ring_tomb(P, lst, rec.pos);
-          __stcg((lru ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, rec.block));
-          st_node(P.nodes + n, Lp, q, rec.block, rec.slot);
+          if (!held) ring_tomb(P, lst, rec.pos);
+          if (hold) {
+            st_node(P.nodes + n, Lp | NODE_HELD, held ? rec.pos + 1u : 1u, rec.block, rec.slot);
+            P.node_of_block[rec.block] = n;
+          } else {
+            __stcg((lru ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, rec.block));
+            st_node(P.nodes + n, Lp, q, rec.block, rec.slot);
+          }
           const int64_t out = o + (nb - 1 - (j + lane));
           P.cls[out] = (uint8_t)lst;                               // L_T1 == CLS_HIT_T1, L_T2 == CLS_HIT_T2
           P.block_id[out] = rec.block;
@@ -307,7 +317,7 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
           P.p_after[out] = C.p;
           P.dropped[a0 + lane] = NODE_NONE;
         }
-        if (lru) C.tail[L_T1] += (uint32_t)k; else C.tail[L_T2] += (uint32_t)k;
+        if (!hold) { if (lru) C.tail[L_T1] += (uint32_t)k; else C.tail[L_T2] += (uint32_t)k; }
         C.t1 -= (int32_t)t1hits; C.t2 += (int32_t)t1hits;
         C.elig1 -= __popc(me & m0 & km);
         C.elig2 -= __popc(me & m1 & km);
@@ -373,7 +383,7 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
       if (act) {
 #pragma unroll
         for (int L = 1; L <= 4; ++L)
-          if (lst == (uint32_t)L && need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
+          if (lst == (uint32_t)L && !held && need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
         if ((my_src & 1u) && (uint32_t)__popc(srcT1m & lt) >= found[L_T1]) bad = true;
         if (my_src == 2 && (uint32_t)__popc(srcT2m & lt) >= found[L_T2]) bad = true;
         if (((R.d1 >> lane) & 1u) && (uint32_t)__popc(R.d1 & lt) >= found[L_B1]) bad = true;
@@ -442,9 +452,14 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
         const bool toT1 = (pushT1m >> lane) & 1u;
         const uint32_t Lp = toT1 ? L_T1 : L_T2;
         const uint32_t q = (toT1 ? C.tail[L_T1] : C.tail[L_T2]) + (uint32_t)__popc((toT1 ? pushT1m : pushT2m) & lt);
-        if (lst >= L_T1 && lst <= L_B2) ring_tomb(P, lst, rec.pos);     // the node leaves its old position
-        __stcg((toT1 ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, blk));
-        st_node(P.nodes + n, Lp, q, blk, rec.slot);
+        if (lst >= L_T1 && lst <= L_B2 && !held) ring_tomb(P, lst, rec.pos);     // the node leaves its old position
+        if (hold) {
+          st_node(P.nodes + n, Lp | NODE_HELD, held ? rec.pos + 1u : 1u, blk, rec.slot);
+          P.node_of_block[blk] = n;
+        } else {
+          __stcg((toT1 ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, blk));
+          st_node(P.nodes + n, Lp, q, blk, rec.slot);
+        }
         const int64_t out = o + (nb - 1 - (j + lane));
         P.cls[out] = (uint8_t)lst;                    // ABSENT -> MISS(0), T1 -> 1, T2 -> 2, B1 -> 3, B2 -> 4
         P.block_id[out] = blk;
@@ -470,8 +485,7 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
       C.n_evict += __popc(evictm);
 #pragma unroll
       for (int L = 1; L <= 4; ++L) C.head[L] = endpos[L];
-      C.tail[L_T1] += __popc(pushT1m);
-      C.tail[L_T2] += __popc(pushT2m);
+      if (!hold) { C.tail[L_T1] += __popc(pushT1m); C.tail[L_T2] += __popc(pushT2m); }
       C.tail[L_B1] += __popc(ghost1m);
       C.tail[L_B2] += need[L_T2];
       (void)src3m;

@@ -24,6 +24,18 @@ __device__ __forceinline__ void ring_push(SerialCtx& C, const StepParams& P, uin
   st_node(P.nodes + n, L, q, block, slot);
 }
 
+// The accessed node takes its place in list L: at the MRU end of the ring, or (pin scope 2) outside every ring with one
+// more hold; holds_before = the holds it had (0 if it was not held).
+template <uint32_t L>
+__device__ __forceinline__ void place_accessed(SerialCtx& C, const StepParams& P, uint32_t n, int32_t block, uint32_t slot, uint32_t holds_before) {
+  if (P.pin_scope == 2) {
+    st_node(P.nodes + n, L | NODE_HELD, holds_before + 1u, block, slot);
+    P.node_of_block[block] = n;
+  } else {
+    ring_push<L>(C, P, n, block, slot);
+  }
+}
+
 // first live entry of list L in [head, bound); advances head past everything it skipped.  NODE_NONE if none.
 template <uint32_t L>
 __device__ __forceinline__ uint32_t ring_pop_lru(SerialCtx& C, const StepParams& P, uint32_t bound, Node* rec_out) {
@@ -91,6 +103,7 @@ __device__ __forceinline__ void ctx_load(SerialCtx& C, const StepParams& P) {
   for (int L = 1; L <= 4; ++L) { C.head[L] = S->head[L]; C.tail[L] = S->tail[L]; C.bound[L] = S->tail[L]; }
   C.t1 = S->t1; C.t2 = S->t2; C.b1 = S->b1; C.b2 = S->b2; C.p = S->p; C.next_fresh = S->next_fresh;
   C.elig1 = C.t1; C.elig2 = C.t2;
+  if (P.pin_scope == 2) { C.elig1 = S->u1; C.elig2 = S->u2; }   // held scope: the unheld entries, whatever step held the others
   C.dbl = (P.policy == POLICY_DBL);
 #pragma unroll
   for (int i = 0; i < ST_COUNT; ++i) C.stat[i] = 0;
@@ -103,6 +116,7 @@ __device__ __forceinline__ void ctx_store(const SerialCtx& C, const StepParams& 
   for (int L = 1; L <= 4; ++L) { S->head[L] = C.head[L]; S->tail[L] = C.tail[L]; }
   S->t1 = C.t1; S->t2 = C.t2; S->b1 = C.b1; S->b2 = C.b2; S->p = C.p; S->next_fresh = C.next_fresh;
   S->counts[0] = C.n_alloc; S->counts[1] = C.n_evict;
+  S->u1 = C.elig1; S->u2 = C.elig2;
 #pragma unroll
   for (int i = 0; i < ST_COUNT; ++i) S->stat[i] += C.stat[i];
   if (C.err) S->error = C.err;
@@ -127,47 +141,50 @@ __device__ __noinline__ void serial_access(SerialCtx& C, const StepParams& P, in
   const int32_t c = P.capacity;
   uint32_t n = P.node_acc[a];
   if (n & SLOT_FLAG) n = __ldcg(&P.table[n & ~SLOT_FLAG].node) - 1;
-  const Node rec = ld_node(P.nodes + n);
+  Node rec = ld_node(P.nodes + n);
+  const bool held = (rec.list & NODE_HELD) != 0;             // pin scope 2 only: resident, in no ring, rec.pos = holds
+  const uint32_t holds = held ? rec.pos : 0u;
+  rec.list &= NODE_LIST_MASK;
   int cls;
   int32_t blk = rec.block, ev = -1;
   uint32_t dropped = NODE_NONE;
   C.stat[ST_ACCESSES]++;
-  if (rec.list >= L_T1 && rec.list <= L_B2) ring_tomb(P, rec.list, rec.pos);   // every class but MISS moves the node
+  if (rec.list >= L_T1 && rec.list <= L_B2 && !held) ring_tomb(P, rec.list, rec.pos);   // every class but MISS moves the node
   if (P.policy == POLICY_LRU) {             // R10
     if (rec.list == L_T1) {
       cls = CLS_HIT_T1; C.stat[ST_HIT_T1]++;
-      if ((int32_t)(C.bound[L_T1] - rec.pos) > 0) C.elig1--;
-      ring_push<L_T1>(C, P, n, blk, rec.slot);
+      if (!held && (int32_t)(C.bound[L_T1] - rec.pos) > 0) C.elig1--;
+      place_accessed<L_T1>(C, P, n, blk, rec.slot, holds);
     } else {
       cls = CLS_MISS; C.stat[ST_MISS]++;
       if (C.t1 < c) { blk = C.next_fresh++; C.stat[ST_FRESH]++; }
       else blk = ev = evict_t1_no_ghost_serial(C, P, &dropped);
-      ring_push<L_T1>(C, P, n, blk, rec.slot);
+      place_accessed<L_T1>(C, P, n, blk, rec.slot, 0);
       C.t1++;
     }
   } else if (rec.list == L_T1 || rec.list == L_T2) {      // R5 case 1
     if (rec.list == L_T1) {
       cls = CLS_HIT_T1; C.stat[ST_HIT_T1]++; C.t1--; C.t2++;
-      if ((int32_t)(C.bound[L_T1] - rec.pos) > 0) C.elig1--;
+      if (!held && (int32_t)(C.bound[L_T1] - rec.pos) > 0) C.elig1--;
     } else {
       cls = CLS_HIT_T2; C.stat[ST_HIT_T2]++;
-      if ((int32_t)(C.bound[L_T2] - rec.pos) > 0) C.elig2--;
+      if (!held && (int32_t)(C.bound[L_T2] - rec.pos) > 0) C.elig2--;
     }
-    ring_push<L_T2>(C, P, n, blk, rec.slot);
+    place_accessed<L_T2>(C, P, n, blk, rec.slot, holds);
   } else if (rec.list == L_B1) {                          // case 2
     cls = CLS_GHOST_B1; C.stat[ST_GHOST_B1]++;
     int32_t delta = C.b2 / C.b1; if (delta < 1) delta = 1;
     if (P.policy != POLICY_DBL) C.p = min(c, C.p + delta);      // DBL: no adaptation
     blk = ev = replace_serial(C, P, false);
     C.b1--; C.t2++;
-    ring_push<L_T2>(C, P, n, blk, rec.slot);
+    place_accessed<L_T2>(C, P, n, blk, rec.slot, 0);
   } else if (rec.list == L_B2) {                          // case 3
     cls = CLS_GHOST_B2; C.stat[ST_GHOST_B2]++;
     int32_t delta = C.b1 / C.b2; if (delta < 1) delta = 1;
     if (P.policy != POLICY_DBL) C.p = max(0, C.p - delta);
     blk = ev = replace_serial(C, P, true);
     C.b2--; C.t2++;
-    ring_push<L_T2>(C, P, n, blk, rec.slot);
+    place_accessed<L_T2>(C, P, n, blk, rec.slot, 0);
   } else {                                                // case 4 (ABSENT)
     cls = CLS_MISS; C.stat[ST_MISS]++;
     if (rec.list != L_ABSENT) C.err = DEV_ERR_BAD_NODE;
@@ -181,7 +198,7 @@ __device__ __noinline__ void serial_access(SerialCtx& C, const StepParams& P, in
         blk = ev = replace_serial(C, P, false);
       } else { blk = C.next_fresh++; C.stat[ST_FRESH]++; }
     }
-    ring_push<L_T1>(C, P, n, blk, rec.slot);
+    place_accessed<L_T1>(C, P, n, blk, rec.slot, 0);
     C.t1++;
   }
   P.cls[out] = (uint8_t)cls;
@@ -199,7 +216,9 @@ __global__ void arc_machine_serial_kernel(const __grid_constant__ StepParams P) 
   ctx_load(C, P);
   for (uint32_t r = 0; r < P.n_req; ++r) {
     const int64_t o = P.blk_off[r], nb = P.blk_off[r + 1] - o;
-    if (r == 0 || P.pin_scope == 0) begin_request(C);   // step-wide scope: the pins of earlier requests of the step stay
+    // step-wide scope: the pins of earlier requests of the step stay; held scope: nothing enters T1 / T2's rings during a
+    // step, every ring entry is a possible victim (bound = tail, set by ctx_load) and elig1/2 carry over from DevState
+    if (P.pin_scope != 2 && (r == 0 || P.pin_scope == 0)) begin_request(C);
     for (int64_t j = 0; j < nb; ++j) serial_access(C, P, o + j, o + (nb - 1 - j));   // tail block first (R2)
   }
   ctx_store(C, P);

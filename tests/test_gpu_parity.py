@@ -338,3 +338,117 @@ def test_many_tiny_requests_and_cache_sized_requests(arc, policy):
         assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), name)
     assert_same_state(gc, oc, "edge shapes")
     gc.close()
+
+
+def _serving_loop(arc, gc, oc, rng, c, steps, ctx, max_req_blocks=6, depth=4):
+    """Random steps and random releases under ARC_PIN_HELD, GPU against the oracle; returns the requests still held."""
+    live = []
+    refused = 0
+    for step in range(steps):
+        assert gc.hold_units() == oc.hold_units() == sum(len(x) for x in live), ctx
+        if live and (rng.random() < 0.45 or oc.hold_units() > c - 2):
+            ids = live.pop(int(rng.integers(0, len(live))))
+            ids = ids[rng.permutation(len(ids))]
+            while live and rng.random() < 0.4:          # several requests in one call: shared blocks appear several times
+                ids = np.concatenate([ids, live.pop(int(rng.integers(0, len(live))))])
+            gc.release(ids)
+            assert oc.release(ids) == 0, ctx
+        else:
+            reqs, left = [], c - oc.hold_units() + (2 if rng.random() < 0.1 else 0)   # now and then one step too many
+            while left > 0 and rng.random() < 0.85:
+                r = W.prefix_tree_requests(rng, n_requests=1, block_size=16, branching=2, depth=depth, max_blocks=min(left, max_req_blocks))[0]
+                reqs.append(r)
+                left -= len(r) // 16
+            tokens, offsets = W.pack_requests(reqs)
+            o = oc.step(tokens, offsets)
+            if isinstance(o, int):
+                assert o == arc.ERR_REQUEST_TOO_LARGE
+                with pytest.raises(arc.ArcError) as e:
+                    gc.step(dev(tokens), offsets)
+                assert e.value.code == arc.ERR_REQUEST_TOO_LARGE
+                refused += 1
+                continue
+            g = gc.step(dev(tokens), offsets).to_host()
+            assert_same_step(g, o, f"{ctx} step {step}")
+            off = o["blk_off"]
+            live += [o["block_id"][off[r]:off[r + 1]].copy() for r in range(len(reqs)) if off[r + 1] > off[r]]
+        if step % 16 == 0:
+            assert_same_state(gc, oc, f"{ctx} step {step}")
+    assert_same_state(gc, oc, ctx)
+    return live, refused
+
+
+@pytest.mark.parametrize("machine", [0, 1, 2])
+@pytest.mark.parametrize("policy", [0, 1, 2])
+def test_held_pins_and_release(arc, policy, machine):
+    """NEXT-3: ARC_PIN_HELD and arc_release.  A serving loop - steps add holds, finished requests give
+    them back in arbitrary order, several requests per call - on small and medium caches; the scope is entered on a cache
+    that already has content and left again; everything bit-exact against the oracle, lists included."""
+    rng = np.random.default_rng(900 + 10 * policy + machine)
+    for c, steps, mrb, depth in ((5, 150, 3, 3), (24, 250, 6, 4), (300, 200, 40, 7)):
+        gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
+        gc.set_machine(machine)
+        ctx = f"held p{policy} m{machine} c{c}"
+        for i in range(10):                               # default scope first: the cache has content when the scope changes
+            reqs = W.prefix_tree_requests(rng, n_requests=3, block_size=16, branching=2, depth=depth, max_blocks=min(c, mrb))
+            tokens, offsets = W.pack_requests(reqs)
+            assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), f"{ctx} warm {i}")
+        gc.set_pin_scope(arc.PIN_HELD)
+        oc.set_pin_scope(2)
+        live, refused = _serving_loop(arc, gc, oc, rng, c, steps, ctx, mrb, depth)
+        if live:                                          # the scope cannot change while holds are outstanding
+            with pytest.raises(arc.ArcError):
+                gc.set_pin_scope(arc.PIN_REQUEST)
+            ids = np.concatenate(live)
+            gc.release(ids)
+            assert oc.release(ids) == 0
+        assert gc.hold_units() == oc.hold_units() == 0
+        assert_same_state(gc, oc, ctx + " all released")
+        gs = gc.stats()
+        assert gs["t1"] + gs["t2"] == len(gc.debug_lists()["T1"][0]) + len(gc.debug_lists()["T2"][0])   # everything is back in a ring
+        gc.set_pin_scope(arc.PIN_REQUEST)
+        oc.set_pin_scope(0)
+        for i in range(10):
+            reqs = W.prefix_tree_requests(rng, n_requests=3, block_size=16, branching=2, depth=depth, max_blocks=min(c, mrb))
+            tokens, offsets = W.pack_requests(reqs)
+            assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), f"{ctx} after {i}")
+        assert_same_state(gc, oc, ctx + " back in the request scope")
+        gc.close()
+
+
+def test_held_pins_protect_blocks_and_bad_release_is_flagged(arc):
+    """A held request survives any amount of traffic; releasing what is not held changes nothing and raises the sticky
+    device error."""
+    c = 64
+    gc, oc = arc.ArcCache(c), O.OracleCache(c)
+    gc.set_pin_scope(arc.PIN_HELD)
+    oc.set_pin_scope(2)
+    doc = np.arange(5000, 5000 + 16 * 20, dtype=np.int32)             # 20 blocks, held for the whole test
+    off = np.array([0, len(doc)], np.int64)
+    g0 = gc.step(dev(doc), off).to_host()
+    assert_same_step(g0, oc.step(doc, off), "held doc")
+    rng = np.random.default_rng(5)
+    for i in range(60):                                               # 60 x 40 fresh blocks through the other 44 slots
+        t = rng.integers(10 ** 6, 2 * 10 ** 6, size=16 * 40).astype(np.int32)
+        o2 = np.array([0, len(t)], np.int64)
+        g, o = gc.step(dev(t), o2).to_host(), oc.step(t, o2)
+        assert_same_step(g, o, f"traffic {i}")
+        assert not np.isin(g["evicted_id"], g0["block_id"]).any()     # never a held block
+        gc.release(g["block_id"])
+        assert oc.release(o["block_id"]) == 0
+    g1 = gc.step(dev(doc), off).to_host()
+    assert_same_step(g1, oc.step(doc, off), "held doc again")
+    assert (g1["cls"] != 0).all() and np.array_equal(g1["block_id"], g0["block_id"]) and g1["prefix_len"][0] == len(doc)
+    assert gc.hold_units() == 40
+    with pytest.raises(arc.ArcError):
+        gc.release(np.arange(41, dtype=np.int32))                     # more IDs than holds: refused on the host
+    assert_same_state(gc, oc, "before the bad release")
+    bad = np.concatenate([g0["block_id"][:3], g0["block_id"][:1], g0["block_id"][:1]])   # the first block three times: held twice
+    assert oc.release(bad) == O.ERR_INVALID_ARG
+    gc.release(bad)
+    with pytest.raises(arc.ArcError):
+        gc.stats()
+    gl, ol = gc.debug_lists(), oc.lists()
+    for n in ("T1", "T2", "B1", "B2"):
+        assert np.array_equal(gl[n][0], ol[n][0]), n                   # nothing changed
+    gc.close()
