@@ -131,8 +131,7 @@ int arc_step_host(arc_cache *h, const int32_t *h_tokens, const int64_t *h_offset
 /* With ARC_PIN_HELD every access adds one hold to its block; a block with holds is never a victim, in
  * this step or any later one, until arc_release has given all its holds back.  A step is refused with
  * ARC_ERR_REQUEST_TOO_LARGE when the holds outstanding plus its full blocks exceed capacity_blocks.  The scope can be
- * changed only while no hold is outstanding (else ARC_ERR_INVALID_ARG).  Steps under ARC_PIN_HELD run the one-warp K3
- * machine (or the serial one if arc_set_machine asked for it). */
+ * changed only while no hold is outstanding (else ARC_ERR_INVALID_ARG). */
 int arc_set_pin_scope(arc_cache *h, int scope);
 
 /* ARC_PIN_HELD only: gives back one hold for every block ID listed - normally a finished request's block_id output, in

@@ -130,8 +130,8 @@ class OracleCache:
         return int(lib().oracle_hold_units(self._h))
 
     def close(self):
-        if self._h:
-            lib().oracle_destroy(self._h)
+        if self._h and _lib is not None:      # at interpreter exit the module globals may already be gone
+            _lib.oracle_destroy(self._h)
             self._h = C.c_void_p()
 
     __del__ = close

@@ -297,19 +297,25 @@ __global__ void __launch_bounds__(CMP_THREADS) dump_list_kernel(const DevState* 
 
 // ---------------------------------------------------------------------------------------------------------------------
 // arc_release (pin scope 2): one hold back per listed block id, in the order given; a block whose last
-// hold goes re-enters its list (T1 or T2) at the MRU end.  One CTA: all 256 threads check the whole call first (every id a
-// resident held block, none listed more often than it is held - else nothing changes and the handle gets the sticky
-// error DEV_ERR_BAD_RELEASE), then warp 0 applies it 32 ids at a time: equal ids inside a chunk are grouped with
-// match_any and the group's LAST lane acts for it, which is the position the by-the-book walk zeroes the count at.
-// rel_cnt[capacity] is all zero between calls.
-__global__ void __launch_bounds__(256) release_kernel(const __grid_constant__ StepParams P, const int32_t* ids, uint32_t n,
-                                                      uint32_t* rel_cnt) {
+// hold goes re-enters its list (T1 or T2) at the MRU end.  One CTA of 1024 threads, everything data-parallel:
+//   pass 1  every id must name a resident held block; rel_cnt[id] counts how often it is listed, rel_last[id] keeps the
+//           index (+1) of its last occurrence;
+//   pass 2  no id is listed more often than it is held.  If either check fails nothing changes and the handle gets the
+//           sticky error DEV_ERR_BAD_RELEASE;
+//   pass 3  walking the ids in order, a block's count reaches zero exactly at its LAST occurrence and only if
+//           rel_cnt == holds, so the occurrences that re-enter a ring are known up front; their ring positions are the
+//           tail plus a CTA-wide exclusive scan of those flags, 1024 ids per round, per list;
+//   pass 4  the scratch is zeroed again (rel_cnt / rel_last are all zero between calls).
+constexpr int REL_THREADS = 1024;
+__global__ void __launch_bounds__(REL_THREADS) release_kernel(const __grid_constant__ StepParams P, const int32_t* ids, uint32_t n,
+                                                              uint32_t* rel_cnt, uint32_t* rel_last) {
   __shared__ uint32_t s_bad;
-  const uint32_t tid = threadIdx.x, lane = tid & 31u, FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
+  __shared__ uint32_t s_w1[32], s_w2[32];
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
   DevState* S = P.state;
   if (tid == 0) s_bad = 0;
   __syncthreads();
-  for (uint32_t i = tid; i < n; i += 256) {
+  for (uint32_t i = tid; i < n; i += REL_THREADS) {
     const int32_t id = ids[i];
     bool ok = id >= 0 && id < P.capacity;
     if (ok) {
@@ -317,50 +323,70 @@ __global__ void __launch_bounds__(256) release_kernel(const __grid_constant__ St
       ok = nd != NODE_NONE;
       if (ok) { const Node r = ld_node(P.nodes + nd); ok = (r.list & NODE_HELD) && r.block == id; }
     }
-    if (ok) atomicAdd(&rel_cnt[id], 1u); else s_bad = 1;
+    if (ok) { atomicAdd(&rel_cnt[id], 1u); atomicMax(&rel_last[id], i + 1u); } else s_bad = 1;
   }
   __syncthreads();
   if (!s_bad) {
-    for (uint32_t i = tid; i < n; i += 256) {
+    for (uint32_t i = tid; i < n; i += REL_THREADS) {
       const int32_t id = ids[i];
       if (__ldcg(&rel_cnt[id]) > ld_node(P.nodes + P.node_of_block[id]).pos) s_bad = 1;
     }
   }
   __syncthreads();
   const bool bad = s_bad != 0;
-  if (!bad && tid < 32) {
-    uint32_t tail1 = S->tail[L_T1], tail2 = S->tail[L_T2];
-    int32_t u1 = S->u1, u2 = S->u2;
-    for (uint32_t base = 0; base < n; base += 32) {
-      const bool valid = base + lane < n;
-      const int32_t id = valid ? ids[base + lane] : -1;
-      const uint32_t nd = valid ? P.node_of_block[id] : (0xF0000000u | lane);
+  if (!bad) {
+    uint32_t tail1 = S->tail[L_T1], tail2 = S->tail[L_T2];      // every thread carries the same running tails
+    for (uint32_t base = 0; base < n; base += REL_THREADS) {
+      const uint32_t i = base + tid;
+      bool last = false, zero = false;
+      uint32_t nd = 0, L = 0, left = 0;
       Node r;
       r.list = 0; r.pos = 0; r.block = -1; r.slot = 0;
-      if (valid) r = ld_node(P.nodes + nd);
-      const uint32_t grp = __match_any_sync(FULL, nd);
-      const bool rep = valid && (31u - (uint32_t)__clz(grp)) == lane;
-      const uint32_t left = r.pos - (uint32_t)__popc(grp);
-      const bool zero = rep && left == 0;
-      const uint32_t L = r.list & NODE_LIST_MASK;
+      if (i < n) {
+        const int32_t id = ids[i];
+        last = __ldcg(&rel_last[id]) == i + 1u;
+        if (last) {
+          nd = P.node_of_block[id];
+          r = ld_node(P.nodes + nd);
+          left = r.pos - __ldcg(&rel_cnt[id]);
+          zero = left == 0;
+          L = r.list & NODE_LIST_MASK;
+        }
+      }
       const uint32_t z1 = __ballot_sync(FULL, zero && L == L_T1), z2 = __ballot_sync(FULL, zero && L == L_T2);
+      if (lane == 0) { s_w1[warp] = (uint32_t)__popc(z1); s_w2[warp] = (uint32_t)__popc(z2); }
+      __syncthreads();
+      uint32_t before1 = 0, before2 = 0, tot1 = 0, tot2 = 0;
+      {
+        const uint32_t a1 = s_w1[lane], a2 = s_w2[lane];              // REL_THREADS / 32 = 32 warps: one per lane
+        uint32_t p1 = a1, p2 = a2;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const uint32_t x1 = __shfl_up_sync(FULL, p1, d), x2 = __shfl_up_sync(FULL, p2, d);
+          if ((int)lane >= d) { p1 += x1; p2 += x2; }
+        }
+        before1 = __shfl_sync(FULL, p1 - a1, warp); before2 = __shfl_sync(FULL, p2 - a2, warp);
+        tot1 = __shfl_sync(FULL, p1, 31); tot2 = __shfl_sync(FULL, p2, 31);
+      }
       if (zero) {
-        const uint32_t q = (L == L_T1) ? tail1 + (uint32_t)__popc(z1 & lt) : tail2 + (uint32_t)__popc(z2 & lt);
+        const uint32_t q = (L == L_T1) ? tail1 + before1 + (uint32_t)__popc(z1 & lt) : tail2 + before2 + (uint32_t)__popc(z2 & lt);
         __stcg(((L == L_T1) ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(nd, r.block));
         st_node(P.nodes + nd, L, q, r.block, r.slot);
-      } else if (rep) {
+      } else if (last) {
         st_node(P.nodes + nd, r.list, left, r.block, r.slot);
       }
-      tail1 += (uint32_t)__popc(z1); tail2 += (uint32_t)__popc(z2);
-      u1 += __popc(z1); u2 += __popc(z2);
-      __syncwarp();
+      tail1 += tot1; tail2 += tot2;
+      __syncthreads();
     }
-    if (lane == 0) { S->tail[L_T1] = tail1; S->tail[L_T2] = tail2; S->u1 = u1; S->u2 = u2; }
+    if (tid == 0) {
+      S->u1 += (int32_t)(tail1 - S->tail[L_T1]); S->u2 += (int32_t)(tail2 - S->tail[L_T2]);
+      S->tail[L_T1] = tail1; S->tail[L_T2] = tail2;
+    }
   }
   __syncthreads();
-  for (uint32_t i = tid; i < n; i += 256) {
+  for (uint32_t i = tid; i < n; i += REL_THREADS) {
     const int32_t id = ids[i];
-    if (id >= 0 && id < P.capacity) rel_cnt[id] = 0;
+    if (id >= 0 && id < P.capacity) { rel_cnt[id] = 0; rel_last[id] = 0; }
   }
   if (bad && tid == 0) S->error = DEV_ERR_BAD_RELEASE;
 }

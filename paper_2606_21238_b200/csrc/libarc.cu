@@ -410,7 +410,7 @@ int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, ui
   if (h->profiling) cudaEventRecord(h->ev[3], s);
   if (h->machine == 1) {
     arc_machine_serial_kernel<<<1, 32, 0, s>>>(P);                                                       // K3 (serial)
-  } else if (h->machine == 2 || h->pin_scope == ARC_PIN_HELD || (h->machine == 0 && N < 48ull * n_req)) {
+  } else if (h->machine == 2 || (h->machine == 0 && N < 48ull * n_req)) {
     // one warp, 32-wide windows: a window of the wide machine costs about twice as much, which only pays when requests
     // are long enough to fill it (windows never cross a request boundary)
     launch_machine_batched(P, s);
@@ -618,9 +618,9 @@ int arc_set_pin_scope(arc_cache* h, int scope) {
   if (scope == ARC_PIN_HELD && h->pin_scope != ARC_PIN_HELD) {
     if (!h->d_node_of_block) {
       CUDA_TRY(h, dalloc(&h->d_node_of_block, h->c));
-      CUDA_TRY(h, dalloc(&h->d_rel_cnt, h->c));
+      CUDA_TRY(h, dalloc(&h->d_rel_cnt, 2 * h->c));          // multiplicities, then last-occurrence indices
       CUDA_TRY(h, cudaMemset(h->d_node_of_block, 0xFF, (size_t)h->c * sizeof(uint32_t)));
-      CUDA_TRY(h, cudaMemset(h->d_rel_cnt, 0, (size_t)h->c * sizeof(uint32_t)));
+      CUDA_TRY(h, cudaMemset(h->d_rel_cnt, 0, 2 * (size_t)h->c * sizeof(uint32_t)));
     }
     set_unheld_kernel<<<1, 1, 0, h->last_stream>>>(h->d_state);      // nothing is held: every resident entry is in a ring
     h->launches += 1;
@@ -640,7 +640,7 @@ int arc_release(arc_cache* h, const int32_t* d_block_ids, uint64_t n, void* cuda
   int rc = maintain(h, n, s);            // room for up to n pushes at the MRU ends of T1 / T2
   if (rc) return rc;
   StepParams P = make_params(h);
-  release_kernel<<<1, 256, 0, s>>>(P, d_block_ids, (uint32_t)n, h->d_rel_cnt);
+  release_kernel<<<1, REL_THREADS, 0, s>>>(P, d_block_ids, (uint32_t)n, h->d_rel_cnt, h->d_rel_cnt + h->c);
   h->launches += 1;
   CUDA_TRY(h, cudaGetLastError());
   h->window_bound[L_T1] += n; h->window_bound[L_T2] += n;

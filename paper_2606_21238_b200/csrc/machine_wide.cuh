@@ -172,6 +172,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
   const bool lru = (P.policy == POLICY_LRU);
+  const bool hold = (P.pin_scope == 2);      // held scope: see machine_batched.cuh
   const int32_t c = P.capacity;
   const int64_t N = (int64_t)P.n_access;
   SerialCtx C;            // identical in every thread
@@ -199,7 +200,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       my_off = P.blk_off[rr]; my_off1 = P.blk_off[rr + 1];
     }
     const int64_t o = __shfl_sync(FULL, my_off, r & 31), nb = __shfl_sync(FULL, my_off1, r & 31) - o;
-    if (r == 0 || P.pin_scope == 0) begin_request(C);   // step-wide scope: the pins of earlier requests of the step stay
+    if (!hold && (r == 0 || P.pin_scope == 0)) begin_request(C);   // step-wide scope: the pins of earlier requests of the step stay
     int64_t j = 0;
     while (j < nb) {
       const int kmax = (int)min((int64_t)WIDE_W, nb - j);
@@ -234,12 +235,13 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         slot = h;
         atomicMin(&S.set_min[slot], (uint32_t)tid);
       }
-      const uint32_t lst = rec.list;
+      const uint32_t lst = rec.list & NODE_LIST_MASK;
+      const bool held = (rec.list & NODE_HELD) != 0;                 // held scope: in no ring, rec.pos = its holds
       {
         const uint32_t b0 = __ballot_sync(FULL, lst & 1u), b1 = __ballot_sync(FULL, lst & 2u), b2 = __ballot_sync(FULL, lst & 4u);
         // hits on entries that were still evictable by this request (below bound): they stop being so
-        const uint32_t be = __ballot_sync(FULL, (lst == L_T1 && (int32_t)(C.bound[L_T1] - rec.pos) > 0) ||
-                                                    (lst == L_T2 && (int32_t)(C.bound[L_T2] - rec.pos) > 0));
+        const uint32_t be = __ballot_sync(FULL, !held && ((lst == L_T1 && (int32_t)(C.bound[L_T1] - rec.pos) > 0) ||
+                                                              (lst == L_T2 && (int32_t)(C.bound[L_T2] - rec.pos) > 0)));
         if (lane == 0) { S.m[0][warp] = b0; S.m[1][warp] = b1; S.m[2][warp] = b2; S.m[3][warp] = be; }
       }
       __syncthreads();                                               // (B1) class masks and the hash set are complete
@@ -274,9 +276,14 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         // ---- every access of the window is a hit: no counter other than t1/t2 moves, nothing is evicted
         if (tid < k) {
           const uint32_t q = (lru ? C.tail[L_T1] : C.tail[L_T2]) + (uint32_t)tid;
-          ring_tomb(P, lst, rec.pos);
-          __stcg((lru ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, rec.block));
-          st_node(P.nodes + n, lru ? L_T1 : L_T2, q, rec.block, rec.slot);
+          if (!held) ring_tomb(P, lst, rec.pos);
+          if (hold) {
+            st_node(P.nodes + n, (lru ? L_T1 : L_T2) | NODE_HELD, held ? rec.pos + 1u : 1u, rec.block, rec.slot);
+            P.node_of_block[rec.block] = n;
+          } else {
+            __stcg((lru ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, rec.block));
+            st_node(P.nodes + n, lru ? L_T1 : L_T2, q, rec.block, rec.slot);
+          }
           const int64_t out = o + (nb - 1 - (j + tid));
           P.cls[out] = (uint8_t)lst;                               // L_T1 == CLS_HIT_T1, L_T2 == CLS_HIT_T2
           P.block_id[out] = rec.block;
@@ -291,8 +298,8 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
           e1d += (uint32_t)__popc(ME[u] & M0[u] & KM[u]);
           e2d += (uint32_t)__popc(ME[u] & M1[u] & KM[u]);
         }
-        if (lru) { C.tail[L_T1] += (uint32_t)k; C.stat[ST_HIT_T1] += (uint32_t)k; }
-        else { C.tail[L_T2] += (uint32_t)k; C.t1 -= (int32_t)t1hits; C.t2 += (int32_t)t1hits; C.stat[ST_HIT_T1] += t1hits; C.stat[ST_HIT_T2] += (uint32_t)k - t1hits; }
+        if (lru) { C.tail[L_T1] += hold ? 0u : (uint32_t)k; C.stat[ST_HIT_T1] += (uint32_t)k; }
+        else { C.tail[L_T2] += hold ? 0u : (uint32_t)k; C.t1 -= (int32_t)t1hits; C.t2 += (int32_t)t1hits; C.stat[ST_HIT_T1] += t1hits; C.stat[ST_HIT_T2] += (uint32_t)k - t1hits; }
         C.elig1 -= (int32_t)e1d; C.elig2 -= (int32_t)e2d;
         C.stat[ST_ACCESSES] += (uint32_t)k;
         if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
@@ -332,7 +339,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         if (act) {
 #pragma unroll
           for (int L = 1; L <= 4; ++L)
-            if (lst == (uint32_t)L && need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
+            if (lst == (uint32_t)L && !held && need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
           if ((my_src & 1u) && wide_rank(D.s0, warp, lt) >= found[L_T1]) bad = true;
           if (my_src == 2 && wide_rank(S2, warp, lt) >= found[L_T2]) bad = true;
           if (my_d1 && wide_rank(D.d1, warp, lt) >= found[L_B1]) bad = true;
@@ -420,9 +427,14 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         }
         const bool toT1 = (wide_pick(PT1, warp) >> lane) & 1u;
         const uint32_t q = toT1 ? C.tail[L_T1] + wide_rank(PT1, warp, lt) : C.tail[L_T2] + wide_rank(PT2, warp, lt);
-        if (lst >= L_T1 && lst <= L_B2) ring_tomb(P, lst, rec.pos);     // the node leaves its old position
-        __stcg((toT1 ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, blk));
-        st_node(P.nodes + n, toT1 ? L_T1 : L_T2, q, blk, rec.slot);
+        if (lst >= L_T1 && lst <= L_B2 && !held) ring_tomb(P, lst, rec.pos);     // the node leaves its old position
+        if (hold) {
+          st_node(P.nodes + n, (toT1 ? L_T1 : L_T2) | NODE_HELD, held ? rec.pos + 1u : 1u, blk, rec.slot);
+          P.node_of_block[blk] = n;
+        } else {
+          __stcg((toT1 ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, blk));
+          st_node(P.nodes + n, toT1 ? L_T1 : L_T2, q, blk, rec.slot);
+        }
         const int64_t out = o + (nb - 1 - (j + tid));
         P.cls[out] = (uint8_t)lst;                    // ABSENT -> MISS(0), T1 -> 1, T2 -> 2, B1 -> 3, B2 -> 4
         P.block_id[out] = blk;
@@ -451,8 +463,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       C.n_evict += wide_count(EV);
 #pragma unroll
       for (int L = 1; L <= 4; ++L) C.head[L] = endpos[L];
-      C.tail[L_T1] += wide_count(PT1);
-      C.tail[L_T2] += wide_count(PT2);
+      if (!hold) { C.tail[L_T1] += wide_count(PT1); C.tail[L_T2] += wide_count(PT2); }
       C.tail[L_B1] += wide_count(G1);
       C.tail[L_B2] += need[L_T2];
       C.t1 = D.R.t1; C.t2 = D.R.t2; C.b1 = D.R.b1; C.b2 = D.R.b2; C.p = D.R.p; C.next_fresh = D.R.nf;

@@ -128,9 +128,11 @@ def test_tiny_caches_prefix_trees(arc, c, machine):
     for policy in (0, 1, 2):
         gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
         gc.set_machine(machine)
+        table = rng.integers(0, 1000, size=(3, 2, 16), dtype=np.int32)    # a tree that lasts: prefixes shared ACROSS steps too
         for step in range(60):
             reqs = W.prefix_tree_requests(rng, n_requests=int(rng.integers(1, 12)), block_size=16, branching=2, depth=3,
                                           max_blocks=c)
+            reqs += [_tree_request(rng, table, c) for _ in range(int(rng.integers(0, 5)))]
             if step % 7 == 3:
                 reqs += [reqs[0], reqs[0]]                                # duplicates inside the step
             if step % 5 == 1:
@@ -305,10 +307,11 @@ def test_step_wide_pin_scope(arc, machine):
             gc.set_machine(machine)
             gc.set_pin_scope(arc.PIN_STEP)
             oc.set_pin_scope(arc.PIN_STEP)
+            table = rng.integers(0, 1000, size=(4, 2, 16), dtype=np.int32)
             for step in range(50):
                 reqs, left = [], c
                 while left > 0 and rng.random() < 0.85:
-                    r = W.prefix_tree_requests(rng, n_requests=1, block_size=16, branching=2, depth=4, max_blocks=min(left, 6))[0]
+                    r = _tree_request(rng, table, min(left, 6))
                     reqs.append(r)
                     left -= len(r) // 16
                 tokens, offsets = W.pack_requests(reqs)
@@ -340,7 +343,20 @@ def test_many_tiny_requests_and_cache_sized_requests(arc, policy):
     gc.close()
 
 
-def _serving_loop(arc, gc, oc, rng, c, steps, ctx, max_req_blocks=6, depth=4):
+def _tree_request(rng, table, max_blocks):
+    """A root-to-node path in a FIXED token-block tree (table[level, branch] = one block): requests drawn from the same
+    table share prefixes, so hits, ghost hits and hold counts above one all occur."""
+    depth, branching, B = table.shape
+    nb = int(rng.integers(1, max_blocks + 1))
+    path = rng.integers(0, branching, size=nb)
+    if rng.random() < 0.5:
+        path[: min(nb, 3)] = 0                         # a popular trunk
+    toks = [table[min(l, depth - 1), int(b)] for l, b in enumerate(path)]
+    toks.append(rng.integers(0, 1000, size=int(rng.integers(0, B)), dtype=np.int32))
+    return np.concatenate(toks).astype(np.int32)
+
+
+def _serving_loop(arc, gc, oc, rng, c, steps, ctx, table, max_req_blocks=6):
     """Random steps and random releases under ARC_PIN_HELD, GPU against the oracle; returns the requests still held."""
     live = []
     refused = 0
@@ -356,7 +372,7 @@ def _serving_loop(arc, gc, oc, rng, c, steps, ctx, max_req_blocks=6, depth=4):
         else:
             reqs, left = [], c - oc.hold_units() + (2 if rng.random() < 0.1 else 0)   # now and then one step too many
             while left > 0 and rng.random() < 0.85:
-                r = W.prefix_tree_requests(rng, n_requests=1, block_size=16, branching=2, depth=depth, max_blocks=min(left, max_req_blocks))[0]
+                r = _tree_request(rng, table, min(left, max_req_blocks))
                 reqs.append(r)
                 left -= len(r) // 16
             tokens, offsets = W.pack_requests(reqs)
@@ -378,24 +394,26 @@ def _serving_loop(arc, gc, oc, rng, c, steps, ctx, max_req_blocks=6, depth=4):
     return live, refused
 
 
-@pytest.mark.parametrize("machine", [0, 1, 2])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3])
 @pytest.mark.parametrize("policy", [0, 1, 2])
 def test_held_pins_and_release(arc, policy, machine):
     """NEXT-3: ARC_PIN_HELD and arc_release.  A serving loop - steps add holds, finished requests give
     them back in arbitrary order, several requests per call - on small and medium caches; the scope is entered on a cache
     that already has content and left again; everything bit-exact against the oracle, lists included."""
     rng = np.random.default_rng(900 + 10 * policy + machine)
-    for c, steps, mrb, depth in ((5, 150, 3, 3), (24, 250, 6, 4), (300, 200, 40, 7)):
+    seen = dict(hit=0, ghost=0, refused=0)
+    for c, steps, mrb, depth in ((5, 150, 3, 3), (24, 250, 6, 4), (300, 200, 40, 7), (3000, 60, 700, 12)):
+        table = rng.integers(0, 1000, size=(depth, 2, 16), dtype=np.int32)
         gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
         gc.set_machine(machine)
         ctx = f"held p{policy} m{machine} c{c}"
         for i in range(10):                               # default scope first: the cache has content when the scope changes
-            reqs = W.prefix_tree_requests(rng, n_requests=3, block_size=16, branching=2, depth=depth, max_blocks=min(c, mrb))
-            tokens, offsets = W.pack_requests(reqs)
+            tokens, offsets = W.pack_requests([_tree_request(rng, table, min(c, mrb)) for _ in range(3)])
             assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), f"{ctx} warm {i}")
         gc.set_pin_scope(arc.PIN_HELD)
         oc.set_pin_scope(2)
-        live, refused = _serving_loop(arc, gc, oc, rng, c, steps, ctx, mrb, depth)
+        live, refused = _serving_loop(arc, gc, oc, rng, c, steps, ctx, table, mrb)
+        seen["refused"] += refused
         if live:                                          # the scope cannot change while holds are outstanding
             with pytest.raises(arc.ArcError):
                 gc.set_pin_scope(arc.PIN_REQUEST)
@@ -406,14 +424,18 @@ def test_held_pins_and_release(arc, policy, machine):
         assert_same_state(gc, oc, ctx + " all released")
         gs = gc.stats()
         assert gs["t1"] + gs["t2"] == len(gc.debug_lists()["T1"][0]) + len(gc.debug_lists()["T2"][0])   # everything is back in a ring
+        seen["hit"] += gs["hit_t1"] + gs["hit_t2"]
+        seen["ghost"] += gs["ghost_b1"] + gs["ghost_b2"]
         gc.set_pin_scope(arc.PIN_REQUEST)
         oc.set_pin_scope(0)
         for i in range(10):
-            reqs = W.prefix_tree_requests(rng, n_requests=3, block_size=16, branching=2, depth=depth, max_blocks=min(c, mrb))
-            tokens, offsets = W.pack_requests(reqs)
+            tokens, offsets = W.pack_requests([_tree_request(rng, table, min(c, mrb)) for _ in range(3)])
             assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), f"{ctx} after {i}")
         assert_same_state(gc, oc, ctx + " back in the request scope")
         gc.close()
+    assert seen["hit"] > 100 and seen["refused"] > 0, seen     # the loop really shares prefixes and really hits the admission rule
+    if policy != 1:
+        assert seen["ghost"] > 0, seen
 
 
 def test_held_pins_protect_blocks_and_bad_release_is_flagged(arc):
