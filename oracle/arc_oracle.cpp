@@ -61,13 +61,15 @@ uint64_t key_from_state(uint64_t s) {  // H5: 0 and 1 are reserved for table sen
   return key;
 }
 
-// keys of the full blocks of one request, block 0 first (H4, H5, H6)
-void request_keys(const int32_t* t, int64_t len, uint32_t B, uint64_t* out) {
-  uint64_t s = HS0;
+// keys of the full blocks of one request, block 0 first (H4, H5, H6).  s = the chain state before block 0: S0 for a
+// prompt, or the state a previous call returned for the same sequence (a request that continues at a
+// block boundary).  Returns the state after the last full block.
+uint64_t request_keys(const int32_t* t, int64_t len, uint32_t B, uint64_t* out, uint64_t s = HS0) {
   for (int64_t i = 0; i < len / B; ++i) {
     s = s * HK + content_hash(t + i * B, B);
-    out[i] = key_from_state(s);
+    if (out) out[i] = key_from_state(s);
   }
+  return s;
 }
 
 enum { MISS = 0, HIT_T1 = 1, HIT_T2 = 2, GHOST_B1 = 3, GHOST_B2 = 4 };
@@ -109,6 +111,7 @@ struct oracle_step_result {  // HOST pointers, owned by the handle, valid until 
   const int32_t* alloc_ids;    // [n_alloc]  access order
   const int32_t* evict_ids;    // [n_evict]  access order
   uint32_t n_alloc, n_evict;
+  const uint64_t* chain_state; // [n_req]    H4 state after each request's last full block (oracle_step / oracle_step_resume)
 };
 
 struct oracle_cache {
@@ -130,7 +133,7 @@ struct oracle_cache {
   std::vector<int32_t> prefix_len, block_id, evicted_id, p_after, alloc_ids, evict_ids;
   std::vector<int64_t> blk_off;
   std::vector<uint8_t> cls;
-  std::vector<uint64_t> keys;
+  std::vector<uint64_t> keys, chain_state;
 };
 
 }  // extern "C"
@@ -320,6 +323,7 @@ int step_keys(oracle_cache* h, const uint64_t* keys, const int64_t* blk_off, uin
     out->block_id = h->block_id.data(); out->evicted_id = h->evicted_id.data(); out->p_after = h->p_after.data();
     out->alloc_ids = h->alloc_ids.data(); out->evict_ids = h->evict_ids.data();
     out->n_alloc = (uint32_t)h->alloc_ids.size(); out->n_evict = (uint32_t)h->evict_ids.size();
+    out->chain_state = h->chain_state.data();
   }
   return OK;
 }
@@ -409,7 +413,10 @@ int oracle_step_keys(oracle_cache* h, const uint64_t* keys, const int64_t* blk_o
   return rc;
 }
 
-int oracle_step(oracle_cache* h, const int32_t* tokens, const int64_t* offsets, uint32_t n_req, oracle_step_result* out) {
+// One step whose request r continues a sequence at a block boundary: chain_in[r] is the H4 state before its first block
+// (S0 for a new prompt; chain_in == NULL means S0 for all).  Everything else is oracle_step.
+int oracle_step_resume(oracle_cache* h, const int32_t* tokens, const int64_t* offsets, const uint64_t* chain_in, uint32_t n_req,
+                       oracle_step_result* out) {
   if (!h || !offsets || n_req > (1u << 20)) return ERR_INVALID_ARG;
   if (offsets[0] < 0) return ERR_INVALID_ARG;
   for (uint32_t r = 0; r < n_req; ++r) if (offsets[r + 1] < offsets[r]) return ERR_INVALID_ARG;
@@ -422,7 +429,10 @@ int oracle_step(oracle_cache* h, const int32_t* tokens, const int64_t* offsets, 
   if (h->pin_scope == 1 && (uint64_t)blk_off[n_req] > h->c) return ERR_REQUEST_TOO_LARGE;
   if (h->pin_scope == 2 && h->hold_units + (uint64_t)blk_off[n_req] > h->c) return ERR_REQUEST_TOO_LARGE;
   h->keys.resize(blk_off[n_req]);
-  oracle_hash_blocks(tokens, offsets, n_req, h->B, h->keys.data(), 0);
+  h->chain_state.resize(n_req);
+  for (uint32_t r = 0; r < n_req; ++r)
+    h->chain_state[r] = request_keys(tokens + offsets[r], offsets[r + 1] - offsets[r], h->B, h->keys.data() + blk_off[r],
+                                     chain_in ? chain_in[r] : HS0);
   double t1 = now_s();
   int rc = step_keys(h, h->keys.data(), blk_off.data(), n_req, out);
   double t2 = now_s();
@@ -432,6 +442,10 @@ int oracle_step(oracle_cache* h, const int32_t* tokens, const int64_t* offsets, 
     h->st.tokens_hashed += (uint64_t)blk_off[n_req] * h->B;
   }
   return rc;
+}
+
+int oracle_step(oracle_cache* h, const int32_t* tokens, const int64_t* offsets, uint32_t n_req, oracle_step_result* out) {
+  return oracle_step_resume(h, tokens, offsets, 0, n_req, out);
 }
 
 int oracle_stats(oracle_cache* h, oracle_stats_t* out) {

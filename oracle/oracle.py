@@ -33,7 +33,8 @@ class _Result(C.Structure):
     _fields_ = [("n_access", C.c_uint64), ("prefix_len", C.POINTER(C.c_int32)), ("blk_off", C.POINTER(C.c_int64)),
                 ("cls", C.POINTER(C.c_uint8)), ("block_id", C.POINTER(C.c_int32)), ("evicted_id", C.POINTER(C.c_int32)),
                 ("p_after", C.POINTER(C.c_int32)), ("alloc_ids", C.POINTER(C.c_int32)),
-                ("evict_ids", C.POINTER(C.c_int32)), ("n_alloc", C.c_uint32), ("n_evict", C.c_uint32)]
+                ("evict_ids", C.POINTER(C.c_int32)), ("n_alloc", C.c_uint32), ("n_evict", C.c_uint32),
+                ("chain_state", C.POINTER(C.c_uint64))]
 
 
 def build(force: bool = False) -> Path:
@@ -55,6 +56,7 @@ def lib():
         L.oracle_destroy.restype = None
         L.oracle_hash_blocks.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p]
         L.oracle_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(_Result)]
+        L.oracle_step_resume.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(_Result)]
         L.oracle_step_keys.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(_Result)]
         L.oracle_set_pin_scope.argtypes = [C.c_void_p, C.c_int]
         L.oracle_release.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
@@ -143,16 +145,22 @@ class OracleCache:
                     evicted_id=_arr(res.evicted_id, n, np.int32), p_after=_arr(res.p_after, n, np.int32),
                     alloc_ids=_arr(res.alloc_ids, res.n_alloc, np.int32), evict_ids=_arr(res.evict_ids, res.n_evict, np.int32))
 
-    def step(self, tokens, offsets, unpack=True):
-        """Returns the outputs dict, or a negative error code (state unchanged)."""
+    def step(self, tokens, offsets, unpack=True, chain_in=None):
+        """Returns the outputs dict, or a negative error code (state unchanged).  chain_in: uint64[n_req] H4 states the
+        requests continue from (None = every request is a new prompt); the dict then also has chain_state[n_req]."""
         tokens = np.ascontiguousarray(tokens, dtype=np.int32)
         offsets = np.ascontiguousarray(offsets, dtype=np.int64)
         n_req = len(offsets) - 1
         res = _Result()
-        rc = lib().oracle_step(self._h, _ptr(tokens), _ptr(offsets), n_req, C.byref(res))
+        ci = None if chain_in is None else np.ascontiguousarray(chain_in, dtype=np.uint64)
+        rc = lib().oracle_step_resume(self._h, _ptr(tokens), _ptr(offsets), _ptr(ci), n_req, C.byref(res))
         if rc != OK:
             return rc
-        return self._unpack(res, n_req) if unpack else int(res.n_access)
+        if not unpack:
+            return int(res.n_access)
+        out = self._unpack(res, n_req)
+        out["chain_state"] = _arr(res.chain_state, n_req, np.uint64)
+        return out
 
     def step_keys(self, requests_keys):
         """requests_keys: list of sequences of uint64 keys (block 0 first)."""

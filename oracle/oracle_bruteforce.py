@@ -67,10 +67,10 @@ def content_hash(block_tokens):
     return g
 
 
-def block_keys(tokens, block_size=16):
-    """H4-H6: keys of the full blocks of one request, block 0 first."""
+def block_keys(tokens, block_size=16, s=S0, return_state=False):
+    """H4-H6: keys of the full blocks of one request, block 0 first.  s: the chain state before block 0 (S0 for a prompt,
+    or the state returned for the sequence's earlier blocks: a request that continues at a block boundary)."""
     keys = []
-    s = S0
     for i in range(len(tokens) // block_size):  # H6: only full blocks
         g = content_hash(tokens[i * block_size:(i + 1) * block_size])
         s = (s * K + g) & MASK  # H4
@@ -78,7 +78,7 @@ def block_keys(tokens, block_size=16):
         if key < 2:  # H5: 0 and 1 are reserved
             key += 2
         keys.append(key)
-    return keys
+    return (keys, s) if return_state else keys
 
 
 # ---- classes / codes (numbers fixed by the C ABI contract) ----------------
@@ -286,15 +286,19 @@ class BruteForceCache:
         self.stats["requests"] += len(requests_keys)
         return out
 
-    def step(self, tokens, offsets):
-        """Same on token IDs: tokens is a flat sequence, offsets has n_req+1 entries."""
+    def step(self, tokens, offsets, chain_in=None):
+        """Same on token IDs: tokens is a flat sequence, offsets has n_req+1 entries; chain_in[r] = the chain state request
+        r continues from (None: new prompts).  The outputs then carry chain_state[r], the state after r's last full block."""
         n_req = len(offsets) - 1
         for r in range(n_req):
             if offsets[r + 1] < offsets[r] or offsets[0] < 0:
                 return ERR_INVALID_ARG
-        reqs = [block_keys(tokens[offsets[r]:offsets[r + 1]], self.B) for r in range(n_req)]
+        pairs = [block_keys(tokens[offsets[r]:offsets[r + 1]], self.B, S0 if chain_in is None else int(chain_in[r]), True)
+                 for r in range(n_req)]
+        reqs = [k for k, _ in pairs]
         out = self.step_keys(reqs)
         if isinstance(out, dict):
+            out["chain_state"] = [st for _, st in pairs]
             self.stats["tokens_seen"] += int(offsets[n_req] - offsets[0])
             self.stats["tokens_hashed"] += self.B * sum(len(k) for k in reqs)
         return out

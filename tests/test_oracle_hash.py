@@ -137,3 +137,74 @@ def test_hash_errors():
     assert O.lib().oracle_hash_blocks(O._ptr(t), O._ptr(offs), 2, 16, None, None) == O.ERR_INVALID_ARG
     offs = np.array([0, 32], np.int64)
     assert O.lib().oracle_hash_blocks(O._ptr(t), O._ptr(offs), 1, 15, None, None) == O.ERR_UNSUPPORTED
+
+
+def test_resumed_chain_split_invariance_and_closed_form():
+    """a request may continue a sequence at a block boundary from the H4 state returned for its earlier
+    blocks.  (1) Splitting a prompt at ANY block boundary and resuming gives the keys of the unsplit prompt, and the
+    same final state; tokens after the last full block never enter the state.  (2) The returned state is the closed form
+    s K^n + sum_j K^(n-1-j) g_j in Python big integers.  Both oracle implementations."""
+    rng = np.random.default_rng(77)
+    for _ in range(60):
+        nb = int(rng.integers(1, 40))
+        tail = int(rng.integers(0, 16))
+        tok = rng.integers(-2 ** 31, 2 ** 31, size=16 * nb + tail).astype(np.int32)
+        off = np.array([0, len(tok)], np.int64)
+        whole_keys, _ = O.hash_blocks(tok, off)
+        oc = O.OracleCache(64)
+        whole = oc.step(tok, off)
+        g = [BF.content_hash(tok[16 * i:16 * i + 16].tolist()) for i in range(nb)]
+        s = BF.S0
+        for gi in g:
+            s = (s * BF.K + gi) & MASK
+        assert int(whole["chain_state"][0]) == s == (BF.S0 * pow(BF.K, nb, 1 << 64) + sum(pow(BF.K, nb - 1 - j, 1 << 64) * g[j] for j in range(nb))) & MASK
+        cut = int(rng.integers(0, nb + 1))
+        part_tail = int(rng.integers(0, 16)) if cut < nb else 0
+        a = tok[:16 * cut + part_tail]                       # may end inside block `cut`: those tokens are not hashed yet
+        b = tok[16 * cut:]                                   # the continuation starts again at the block boundary
+        oa, ob = O.OracleCache(64), O.OracleCache(64)
+        ra = oa.step(a, np.array([0, len(a)], np.int64))
+        rb = ob.step(b, np.array([0, len(b)], np.int64), chain_in=ra["chain_state"])
+        assert int(rb["chain_state"][0]) == s
+        ka, _ = O.hash_blocks(a, np.array([0, len(a)], np.int64))
+        kb_bf, sb_bf = BF.block_keys(b.tolist(), 16, int(ra["chain_state"][0]), True)
+        assert sb_bf == s and BF.block_keys(a.tolist(), 16, BF.S0, True)[1] == int(ra["chain_state"][0])
+        assert np.array_equal(np.concatenate([ka, np.array(kb_bf, np.uint64)]), whole_keys)
+        # the C++ oracle's resumed keys, seen through the cache: after the whole prompt was served by `oc`, the
+        # continuation's blocks are all hits there iff the keys are the same
+        rc = oc.step(b, np.array([0, len(b)], np.int64), chain_in=ra["chain_state"])
+        assert (rc["cls"] != 0).all() and rc["prefix_len"][0] == 16 * (nb - cut)
+
+
+@pytest.mark.parametrize("policy", [0, 1, 2])
+def test_resumed_requests_differential(policy):
+    """Brute force against the C++ oracle on decode-shaped traffic: sequences grow by one or two blocks per step from
+    their stored chain state while new prompts arrive; outputs and states agree."""
+    rng = np.random.default_rng(80 + policy)
+    for c in (4, 9):
+        bf, cpp = BF.BruteForceCache(c, 16, policy), O.OracleCache(c, 16, policy)
+        seqs = []                                            # (chain state, blocks so far)
+        for _ in range(120):
+            reqs, chain = [], []
+            for i in range(len(seqs)):
+                if rng.random() < 0.6:
+                    reqs.append(rng.integers(0, 3, size=16 * int(rng.integers(1, 3)) + int(rng.integers(0, 16))).astype(np.int32))
+                    chain.append(seqs[i])
+                else:
+                    reqs.append(np.zeros(0, np.int32))       # not scheduled this step
+                    chain.append(seqs[i])
+            n_old = len(reqs)
+            if len(seqs) < 3 and rng.random() < 0.5:
+                reqs.append(rng.integers(0, 3, size=16 * int(rng.integers(1, min(c, 3) + 1))).astype(np.int32))
+                chain.append(BF.S0)
+            off = np.zeros(len(reqs) + 1, np.int64)
+            off[1:] = np.cumsum([len(r) for r in reqs])
+            tok = np.concatenate(reqs) if reqs else np.zeros(0, np.int32)
+            a = bf.step(tok.tolist(), off.tolist(), chain_in=chain)
+            b = cpp.step(tok, off, chain_in=np.array(chain, np.uint64))
+            for k in ("cls", "block_id", "evicted_id", "p_after", "prefix_len"):
+                assert list(a[k]) == b[k].tolist(), (c, policy, k)
+            assert [int(x) for x in a["chain_state"]] == [int(x) for x in b["chain_state"]]
+            seqs = [int(x) for x in b["chain_state"]]
+            if len(seqs) == 3 and rng.random() < 0.3:
+                seqs.pop(int(rng.integers(0, 3)))            # a sequence finishes
