@@ -63,6 +63,8 @@ typedef struct {
   const int32_t *alloc_ids;  /* [counts[0]] IDs handed to non-hit accesses, in ACCESS order (R2)           */
   const int32_t *evict_ids;  /* [counts[1]] IDs evicted, in ACCESS order                                   */
   const uint32_t *counts;    /* [2]        n_alloc, n_evict                                                */
+  const uint64_t *chain_state; /* [n_req]  H4 state after each request's last full block: what arc_step_resume takes
+                                *          to continue the sequence (the state the request came with if it had no full block) */
 } arc_step_result;
 
 /* Result of arc_step_host: every pointer is pinned HOST memory owned by the library, filled when the
@@ -118,6 +120,16 @@ int arc_reserve(arc_cache *h, uint32_t max_req, uint64_t max_blocks_per_step);
  * Errors: see the enum; on any error the handle is unchanged and nothing was enqueued. */
 int arc_step(arc_cache *h, const int32_t *d_tokens, const int64_t *h_offsets, uint32_t n_req,
              void *cuda_stream, arc_step_result *out);
+
+/* arc_step for requests that CONTINUE a sequence at a block boundary (a running request whose generated
+ * tokens fill new blocks, or a prompt sent in chunks).  d_chain_in: DEVICE uint64[n_req], read in stream order; entry r
+ * is the H4 state before request r's first block - the chain_state a previous step returned for the same sequence, or
+ * the constant S0 = 0x243F6A8885A308D3 for a new prompt.  NULL = S0 for every request (= arc_step).  Request r's tokens
+ * then start at that block boundary: the caller re-sends the tokens of a block that was not full last time.  The keys,
+ * and with them every result, are those of the unsplit sequence.  May alias a previous result's chain_state only if that
+ * result is from another handle (a step overwrites its handle's chain_state). */
+int arc_step_resume(arc_cache *h, const int32_t *d_tokens, const int64_t *h_offsets, const uint64_t *d_chain_in,
+                    uint32_t n_req, void *cuda_stream, arc_step_result *out);
 
 /* Same step end to end from HOST memory: copies h_tokens (HOST int32, pinned or pageable) to a
  * library-owned device buffer, runs the step, copies prefix_len, counts, alloc_ids and evict_ids back

@@ -27,7 +27,7 @@ STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", 
 EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats", "arc_reset", "arc_destroy",
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
            "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe", "arc_set_pin_scope",
-           "arc_release", "arc_hold_units"]
+           "arc_release", "arc_hold_units", "arc_step_resume"]
 
 
 class ArcError(RuntimeError):
@@ -39,7 +39,7 @@ class ArcError(RuntimeError):
 class _StepResult(C.Structure):
     _fields_ = [("n_access", C.c_uint64), ("prefix_len", C.c_void_p), ("blk_off", C.c_void_p), ("cls", C.c_void_p),
                 ("block_id", C.c_void_p), ("evicted_id", C.c_void_p), ("p_after", C.c_void_p), ("alloc_ids", C.c_void_p),
-                ("evict_ids", C.c_void_p), ("counts", C.c_void_p)]
+                ("evict_ids", C.c_void_p), ("counts", C.c_void_p), ("chain_state", C.c_void_p)]
 
 
 class _HostResult(C.Structure):
@@ -72,6 +72,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_create.argtypes = [u64, u32, C.c_int, C.POINTER(vp)]
     L.arc_reserve.argtypes = [vp, u32, u64]
     L.arc_step.argtypes = [vp, vp, vp, u32, vp, C.POINTER(_StepResult)]
+    L.arc_step_resume.argtypes = [vp, vp, vp, vp, u32, vp, C.POINTER(_StepResult)]
     L.arc_step_host.argtypes = [vp, vp, vp, u32, vp, C.POINTER(_HostResult)]
     L.arc_stats.argtypes = [vp, C.POINTER(_Stats)]
     L.arc_reset.argtypes = [vp]
@@ -148,6 +149,7 @@ class StepResult:
         self.evicted_id = _view(raw.evicted_id, n, "<i4", torch.int32)
         self.p_after = _view(raw.p_after, n, "<i4", torch.int32)
         self.counts = _view(raw.counts, 2, "<i4", torch.int32)
+        self.chain_state = _view(raw.chain_state, n_req, "<i8", torch.int64)   # uint64 bit patterns
         self._alloc_ptr, self._evict_ptr = raw.alloc_ids, raw.evict_ids
 
     def to_host(self) -> dict:
@@ -157,7 +159,7 @@ class StepResult:
         n_alloc, n_evict = int(counts[0]), int(counts[1])
         return dict(n_access=self.n_access, prefix_len=self.prefix_len.cpu().numpy(), blk_off=self.blk_off.cpu().numpy(),
                     cls=self.cls.cpu().numpy(), block_id=self.block_id.cpu().numpy(), evicted_id=self.evicted_id.cpu().numpy(),
-                    p_after=self.p_after.cpu().numpy(),
+                    p_after=self.p_after.cpu().numpy(), chain_state=self.chain_state.cpu().numpy().view(np.uint64),
                     alloc_ids=_view(self._alloc_ptr, n_alloc, "<i4", torch.int32).cpu().numpy(),
                     evict_ids=_view(self._evict_ptr, n_evict, "<i4", torch.int32).cpu().numpy())
 
@@ -192,8 +194,10 @@ class ArcCache:
     def reserve(self, max_req: int, max_blocks_per_step: int):
         self._check(self._L.arc_reserve(self._h, max_req, max_blocks_per_step))
 
-    def step(self, tokens, offsets, stream=None) -> StepResult:
-        """tokens: CUDA int32 tensor (any 4-byte alignment); offsets: host int64[n_req+1]."""
+    def step(self, tokens, offsets, stream=None, chain_in=None) -> StepResult:
+        """tokens: CUDA int32 tensor (any 4-byte alignment); offsets: host int64[n_req+1].  chain_in (arc_step_resume):
+        per request the chain state it continues from - a CUDA int64 tensor of uint64 bit patterns (e.g. gathered from
+        an earlier result's chain_state) or a numpy uint64 array; None = new prompts."""
         torch = _torch()
         if not (isinstance(tokens, torch.Tensor) and tokens.is_cuda and tokens.dtype == torch.int32 and tokens.is_contiguous()):
             raise TypeError("tokens must be a contiguous CUDA int32 tensor")
@@ -201,7 +205,17 @@ class ArcCache:
         if o[-1] > tokens.numel():
             raise ValueError("offsets exceed the token tensor")
         raw = _StepResult()
-        self._check(self._L.arc_step(self._h, tokens.data_ptr(), o.ctypes.data, len(o) - 1, _stream_ptr(stream), C.byref(raw)))
+        if chain_in is None:
+            self._check(self._L.arc_step(self._h, tokens.data_ptr(), o.ctypes.data, len(o) - 1, _stream_ptr(stream), C.byref(raw)))
+            return StepResult(raw, len(o) - 1)
+        if not (hasattr(chain_in, "is_cuda") and chain_in.is_cuda):
+            chain_in = torch.from_numpy(np.ascontiguousarray(chain_in, dtype=np.uint64).view(np.int64)).cuda()
+        chain_in = chain_in.to(torch.int64).contiguous().clone()     # never the handle's own chain_state buffer
+        if chain_in.numel() != len(o) - 1:
+            raise ValueError("chain_in needs one state per request")
+        self._keep_chain = chain_in
+        self._check(self._L.arc_step_resume(self._h, tokens.data_ptr(), o.ctypes.data, chain_in.data_ptr(), len(o) - 1,
+                                            _stream_ptr(stream), C.byref(raw)))
         return StepResult(raw, len(o) - 1)
 
     def step_raw(self, tokens_ptr: int, offsets: np.ndarray, stream_ptr: int) -> int:

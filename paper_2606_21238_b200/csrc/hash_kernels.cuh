@@ -160,10 +160,14 @@ __device__ __forceinline__ int k1_class(int64_t nb) { return nb >= 1024 ? 0 : nb
 // ACCESS_ORDER = true writes keys at blk_off[r] + (nb-1-i) (the order K3 consumes, R2); false writes natural
 // order (arc_hash_blocks).  ticket: device counter, 0 at launch, reset by the caller's stream work; it runs over
 // K1_PASSES * n_req values: ticket t is request t % n_req in pass t / n_req.
-template <bool ACCESS_ORDER>
+// CHAIN = true reads each request's initial H4 state from chain_in (NULL = S0) and writes its final state to chain_out
+// (arc_step / arc_step_resume); false is the stateless arc_hash_blocks, which pays nothing for it.
+template <bool ACCESS_ORDER, bool CHAIN>
 __global__ void __launch_bounds__(256, 4) hash_blocks_kernel(const int32_t* __restrict__ tokens, const int64_t* __restrict__ offsets,
                                                          const int64_t* __restrict__ blk_off, uint32_t n_req,
-                                                         unsigned long long* __restrict__ keys, uint32_t* __restrict__ ticket, uint32_t batch) {
+                                                         unsigned long long* __restrict__ keys, uint32_t* __restrict__ ticket, uint32_t batch,
+                                                         const unsigned long long* __restrict__ chain_in,
+                                                         unsigned long long* __restrict__ chain_out) {
   const int lane = threadIdx.x & 31;
   const uint32_t* tok = reinterpret_cast<const uint32_t*>(tokens);
   const int64_t lo = offsets[0], hi = offsets[n_req];
@@ -189,6 +193,8 @@ __global__ void __launch_bounds__(256, 4) hash_blocks_kernel(const int32_t* __re
       my_r = (uint32_t)(t % n_req);
       const int64_t nb = blk_off[my_r + 1] - blk_off[my_r];
       mine = nb > 0 && k1_class(nb) == (int)(t / n_req);
+      // a request without a full block keeps the state it came with (written once, in the last pass)
+      if (CHAIN && nb == 0 && t / n_req == K1_PASSES - 1) chain_out[my_r] = chain_in ? chain_in[my_r] : H_S0;
     }
     uint32_t todo = __ballot_sync(0xFFFFFFFFu, mine);
     while (todo) {
@@ -198,7 +204,7 @@ __global__ void __launch_bounds__(256, 4) hash_blocks_kernel(const int32_t* __re
       const int64_t o = blk_off[r], nb = blk_off[r + 1] - o;
       const int64_t ts = offsets[r];
       const int s = (int)((base_mis + ts) & 3);          // tokens of the request's start past a 16-byte boundary (same for every round)
-      unsigned long long carry = H_S0;
+      unsigned long long carry = (CHAIN && chain_in) ? chain_in[r] : H_S0;     // the H4 state before block 0 (a prompt: S0)
       const int64_t va = ts - s;                         // absolute token index of the aligned cover of round 0
       // two register buffers ping-pong (no copies): the loads of round i+1 are in flight while round i is hashed
       auto n_vec = [&](int64_t rb) { return (int)((16 * min((int64_t)32, nb - rb) + s + 3) >> 2); };
@@ -208,6 +214,7 @@ __global__ void __launch_bounds__(256, 4) hash_blocks_kernel(const int32_t* __re
         if (lane < cnt) {
           const int64_t i = rb + lane;
           keys[ACCESS_ORDER ? (o + (nb - 1 - i)) : (o + i)] = finalize_key(st);
+          if (CHAIN && i == nb - 1) chain_out[r] = st;           // the state a continuation of this sequence starts from
         }
         carry = shfl64(st, 31);
       };
@@ -228,5 +235,9 @@ __global__ void __launch_bounds__(256, 4) hash_blocks_kernel(const int32_t* __re
 
 // the last thing on the stream after a hashing launch: the ticket returns to 0 for the next launch
 __global__ void reset_ticket_kernel(uint32_t* ticket) { *ticket = 0; }
+
+__global__ void fill_u64_kernel(unsigned long long* p, uint32_t n, unsigned long long v) {
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) p[i] = v;
+}
 
 }  // namespace arc

@@ -77,6 +77,7 @@ struct arc_cache {
   uint32_t* d_node_acc = nullptr;
   uint32_t* d_dropped = nullptr;
   int32_t* d_prefix_len = nullptr;
+  unsigned long long* d_chain_state = nullptr;   // [req_cap] H4 state after each request's last full block
   uint8_t* d_cls = nullptr;
   int32_t *d_block_id = nullptr, *d_evicted_id = nullptr, *d_p_after = nullptr, *d_alloc_ids = nullptr, *d_evict_ids = nullptr;
   void* d_machine_scratch = nullptr;
@@ -173,7 +174,7 @@ int launch_compact(arc_cache* h, cudaStream_t s, int L, uint32_t src_cap, uint32
 
 void free_step_buffers(arc_cache* h) {
   dfree(h->d_offsets); dfree(h->d_keys); dfree(h->d_node_acc); dfree(h->d_dropped);
-  dfree(h->d_prefix_len); dfree(h->d_cls); dfree(h->d_block_id); dfree(h->d_evicted_id); dfree(h->d_p_after);
+  dfree(h->d_prefix_len); dfree(h->d_chain_state); dfree(h->d_cls); dfree(h->d_block_id); dfree(h->d_evicted_id); dfree(h->d_p_after);
   dfree(h->d_alloc_ids); dfree(h->d_evict_ids);
   if (h->h_stage) cudaFreeHost(h->h_stage);
   h->h_stage = nullptr;
@@ -189,6 +190,7 @@ int alloc_step_buffers(arc_cache* h, uint32_t req_cap, uint64_t n_cap) {
   CUDA_TRY(h, dalloc(&h->d_node_acc, n_cap));
   CUDA_TRY(h, dalloc(&h->d_dropped, n_cap));
   CUDA_TRY(h, dalloc(&h->d_prefix_len, req_cap));
+  CUDA_TRY(h, dalloc(&h->d_chain_state, req_cap));
   CUDA_TRY(h, dalloc(&h->d_cls, n_cap));
   CUDA_TRY(h, dalloc(&h->d_block_id, n_cap));
   CUDA_TRY(h, dalloc(&h->d_evicted_id, n_cap));
@@ -310,13 +312,14 @@ int validate_offsets(arc_cache* h, const int64_t* off, uint32_t n_req, uint32_t 
 // K1 grid: persistent warps that take requests through the ticket; enough CTAs to fill the 148 SMs, never more
 // warps than requests.
 void launch_hash(const int32_t* d_tokens, const int64_t* d_offsets, const int64_t* d_blk_off, uint32_t n_req,
-                 unsigned long long* d_keys, uint32_t* d_ticket, bool access_order, cudaStream_t s) {
+                 unsigned long long* d_keys, uint32_t* d_ticket, bool access_order, cudaStream_t s,
+                 const unsigned long long* d_chain_in = nullptr, unsigned long long* d_chain_out = nullptr) {
   const uint32_t blocks = grid_for(n_req, 8, 148 * 6);
   static uint32_t batch = getenv("ARC_K1_BATCH") ? (uint32_t)atoi(getenv("ARC_K1_BATCH")) : 2u;
   if (access_order)
-    hash_blocks_kernel<true><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, batch);
+    hash_blocks_kernel<true, true><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, batch, d_chain_in, d_chain_out);
   else
-    hash_blocks_kernel<false><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, batch);
+    hash_blocks_kernel<false, false><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, batch, d_chain_in, d_chain_out);
 }
 
 }  // namespace
@@ -362,6 +365,11 @@ int arc_reserve(arc_cache* h, uint32_t max_req, uint64_t max_blocks_per_step) {
 }
 
 int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, uint32_t n_req, void* cuda_stream, arc_step_result* out) {
+  return arc_step_resume(h, d_tokens, h_offsets, nullptr, n_req, cuda_stream, out);
+}
+
+int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, const uint64_t* d_chain_in, uint32_t n_req,
+                    void* cuda_stream, arc_step_result* out) {
   if (!h) return ARC_ERR_INVALID_ARG;
   if (!h_offsets || !out) return fail(h, ARC_ERR_INVALID_ARG, "NULL argument");
   if (n_req > kMaxReq) return fail(h, ARC_ERR_INVALID_ARG, "n_req > 2^20");
@@ -399,13 +407,19 @@ int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, ui
   StepParams P = make_params(h);
   P.tokens = d_tokens; P.n_req = n_req; P.n_access = (uint32_t)N;
   if (N) {
-    launch_hash(d_tokens, P.offsets, P.blk_off, n_req, P.keys_acc, &h->d_state->k1_ticket, true, s);               // K1
+    launch_hash(d_tokens, P.offsets, P.blk_off, n_req, P.keys_acc, &h->d_state->k1_ticket, true, s,                 // K1
+                reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state);
     if (h->profiling) cudaEventRecord(h->ev[2], s);
     probe_reserve_kernel<<<grid_for(N, 32, 148 * 8), 256, 0, s>>>(P);                                     // K2
     resolve_nodes_kernel<<<grid_for(N, 256, 148 * 8), 256, 0, s>>>(P);
     h->launches += 3;
-  } else if (h->profiling) {
-    cudaEventRecord(h->ev[2], s);
+  } else {
+    // no full block anywhere: every request keeps the state it came with
+    if (n_req) {
+      if (d_chain_in) CUDA_TRY(h, cudaMemcpyAsync(h->d_chain_state, d_chain_in, (size_t)n_req * sizeof(uint64_t), cudaMemcpyDeviceToDevice, s));
+      else { fill_u64_kernel<<<grid_for(n_req, 256, 148), 256, 0, s>>>(h->d_chain_state, n_req, H_S0); h->launches += 1; }
+    }
+    if (h->profiling) cudaEventRecord(h->ev[2], s);
   }
   if (h->profiling) cudaEventRecord(h->ev[3], s);
   if (h->machine == 1) {
@@ -435,6 +449,7 @@ int arc_step(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offsets, ui
   out->prefix_len = h->d_prefix_len; out->blk_off = P.blk_off; out->cls = h->d_cls; out->block_id = h->d_block_id;
   out->evicted_id = h->d_evicted_id; out->p_after = h->d_p_after; out->alloc_ids = h->d_alloc_ids;
   out->evict_ids = h->d_evict_ids;
+  out->chain_state = reinterpret_cast<const uint64_t*>(h->d_chain_state);
   out->counts = reinterpret_cast<const uint32_t*>(reinterpret_cast<const char*>(h->d_state) + offsetof(DevState, counts));
   return ARC_OK;
 }

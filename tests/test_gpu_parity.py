@@ -474,3 +474,104 @@ def test_held_pins_protect_blocks_and_bad_release_is_flagged(arc):
     for n in ("T1", "T2", "B1", "B2"):
         assert np.array_equal(gl[n][0], ol[n][0]), n                   # nothing changed
     gc.close()
+
+
+def test_resumed_requests_chain_state_and_split_invariance(arc):
+    """arc_step_resume: chain_state equals the oracle's for requests of every shape (empty, shorter
+    than a block, many rounds, misaligned starts); a prompt sent in chunks that continue from the returned state gets
+    the keys of the unsplit prompt (seen as hits on a cache that served the whole prompt), mixed in one step with new
+    prompts; everything bit-exact against the oracle."""
+    rng = np.random.default_rng(4242)
+    c = 4096
+    gc, oc = arc.ArcCache(c), O.OracleCache(c)
+    lens = [0, 5, 16, 17, 31, 32, 16 * 33 + 3, 16 * 64, 16 * 100 + 15, 16 * 257 + 9]
+    prompts = [rng.integers(0, 128000, size=n).astype(np.int32) for n in lens]
+    tokens, offsets = W.pack_requests(prompts)
+    g, o = gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets)
+    assert_same_step(g, o, "whole prompts")
+    assert np.array_equal(g["chain_state"], o["chain_state"])
+    assert g["chain_state"][0] == g["chain_state"][1] == np.uint64(0x243F6A8885A308D3)      # no full block: S0
+    whole_state = g["chain_state"].copy()
+    # the same prompts in two chunks; chunk 1 may end inside a block, chunk 2 starts again at the block boundary
+    cuts = [int(rng.integers(0, n // 16 + 1)) for n in lens]
+    part1 = [p[:16 * k + (int(rng.integers(0, 16)) if 16 * k + 16 <= len(p) else 0)] for p, k in zip(prompts, cuts)]
+    part2 = [p[16 * k:] for p, k in zip(prompts, cuts)]
+    g2c, o2c = arc.ArcCache(c), O.OracleCache(c)
+    t1, o1 = W.pack_requests(part1)
+    ga, oa = g2c.step(dev(t1), o1).to_host(), o2c.step(t1, o1)
+    assert_same_step(ga, oa, "chunk 1")
+    assert np.array_equal(ga["chain_state"], oa["chain_state"])
+    fresh = [rng.integers(0, 128000, size=16 * 7 + 3).astype(np.int32)]                       # a new prompt in the same step
+    t2, o2 = W.pack_requests(part2 + fresh)
+    chain = np.concatenate([ga["chain_state"], np.array([0x243F6A8885A308D3], np.uint64)])
+    gb = g2c.step(dev(t2), o2, chain_in=chain).to_host()
+    ob = o2c.step(t2, o2, chain_in=chain)
+    assert_same_step(gb, ob, "chunk 2")
+    assert np.array_equal(gb["chain_state"], ob["chain_state"])
+    assert np.array_equal(gb["chain_state"][:-1], whole_state)
+    # on the cache that served the unsplit prompts the chunks are hits from block 0 of each chunk on
+    gh = gc.step(dev(t2), o2, chain_in=torch.from_numpy(chain.view(np.int64)).cuda()).to_host()
+    oh = oc.step(t2, o2, chain_in=chain)
+    assert_same_step(gh, oh, "chunks against the whole")
+    nb2 = np.array([len(p) // 16 for p in part2])
+    assert np.array_equal(gh["prefix_len"][:-1], 16 * nb2)
+    assert_same_state(gc, oc, "resume")
+    assert_same_state(g2c, o2c, "resume, chunked")
+    gc.close(); g2c.close()
+
+
+@pytest.mark.parametrize("policy", [0, 1, 2])
+def test_decode_loop_with_held_pins(arc, policy):
+    """The serving loop NEXT-3 describes: held pins, running sequences that grow by the tokens generated since the last
+    step (one block when 16 have accumulated, nothing otherwise) from their stored chain state, new prompts arriving,
+    finished sequences releasing every block they hold.  GPU against the oracle, outputs, chain states, lists."""
+    rng = np.random.default_rng(600 + policy)
+    c = 160
+    table = rng.integers(0, 1000, size=(6, 2, 16), dtype=np.int32)
+    gc, oc = arc.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
+    gc.set_pin_scope(arc.PIN_HELD)
+    oc.set_pin_scope(2)
+    S0 = np.uint64(0x243F6A8885A308D3)
+    running = []                      # dicts: state (uint64), pending (tokens of the block being filled), ids (block IDs held)
+    grown = 0
+    for step in range(300):
+        reqs, chain, owner = [], [], []
+        for q in running:
+            q["pending"] = np.concatenate([q["pending"], rng.integers(0, 50, size=int(rng.integers(3, 12))).astype(np.int32)])
+            reqs.append(q["pending"]); chain.append(q["state"]); owner.append(q)
+        budget = c - oc.hold_units() - sum(len(r) // 16 for r in reqs)
+        while len(running) + (len(reqs) - len(running)) < 6 and budget > 12 and rng.random() < 0.5:
+            r = _tree_request(rng, table, min(budget - 6, 24))
+            q = dict(state=S0, pending=np.zeros(0, np.int32), ids=[], new=True)
+            reqs.append(r); chain.append(S0); owner.append(q)
+            budget -= len(r) // 16
+        if not reqs:
+            continue
+        tokens, offsets = W.pack_requests(reqs)
+        chain = np.array(chain, np.uint64)
+        g = gc.step(dev(tokens), offsets, chain_in=chain).to_host()
+        o = oc.step(tokens, offsets, chain_in=chain)
+        assert_same_step(g, o, f"decode p{policy} step {step}")
+        assert np.array_equal(g["chain_state"], o["chain_state"]), step
+        off = g["blk_off"]
+        for r, q in enumerate(owner):
+            nb = int(off[r + 1] - off[r])
+            q["state"] = g["chain_state"][r]
+            q["ids"] += g["block_id"][off[r]:off[r + 1]].tolist()
+            q["pending"] = reqs[r][16 * nb:]                  # the tokens of the block still being filled
+            if q.pop("new", False):
+                running.append(q)
+            elif nb:
+                grown += nb
+        for q in list(running):                               # some sequences finish: all their holds go back in one call
+            if rng.random() < 0.08 or oc.hold_units() > c - 30:
+                running.remove(q)
+                ids = np.array(q["ids"], np.int32)
+                gc.release(ids)
+                assert oc.release(ids) == 0
+        assert gc.hold_units() == oc.hold_units()
+        if step % 25 == 0:
+            assert_same_state(gc, oc, f"decode p{policy} step {step}")
+    assert grown > 50                                         # sequences really grew block by block
+    assert_same_state(gc, oc, f"decode p{policy}")
+    gc.close()
