@@ -247,6 +247,105 @@ def k2_probe_bench(torch, A, stream, seed, n_keys=1 << 24):
     return n_keys, ms, ok
 
 
+def serving_loop_leg(torch, A, info, steps, stream, seed, n_steps=240, new_per_step=8, decode_steps=2):
+    """NEXT-3 measured: continuous batching under held pins.  Every step admits `new_per_step` prompts of
+    the configured trace, every sequence admitted in the last `decode_steps` steps grows by one block of generated tokens
+    from its stored chain state (arc_step_resume), and the sequences admitted `decode_steps` steps ago finish: all their
+    holds go back in one arc_release.  Timed on the device; the same loop is then replayed on the CPU oracle and the
+    counters compared."""
+    from oracle import oracle as O
+
+    S0 = 0x243F6A8885A308D3
+    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence(seed + 99)))
+    prompts = []
+    for tok, off in steps:
+        prompts += [tok[off[r]:off[r + 1]] for r in range(len(off) - 1)]
+    need = n_steps * new_per_step
+    prompts = [p[:len(p) // 16 * 16] for p in prompts[:need]]           # whole blocks: decode continues at a block boundary
+    n_steps = len(prompts) // new_per_step
+    gen = rng.integers(0, 128000, size=(n_steps, decode_steps * new_per_step, 16)).astype(np.int32)
+    plan = []                                                            # per step: (tokens, offsets, n_new, n_dec)
+    held = []                                                            # holds of the cohorts still running, oldest first
+    for i in range(n_steps):
+        new = prompts[i * new_per_step:(i + 1) * new_per_step]
+        n_dec = new_per_step * min(i, decode_steps)
+        # admission (the scheduler's job): holds outstanding + this step's blocks <= c; the longest prompts are cut until it fits
+        budget = info.capacity_blocks - sum(held) - n_dec
+        while sum(len(p) for p in new) // 16 > budget:
+            k = max(range(len(new)), key=lambda j: len(new[j]))
+            new[k] = new[k][:len(new[k]) // 32 * 16]
+        held = [h + new_per_step for h in held] + [sum(len(p) for p in new) // 16]
+        if len(held) > decode_steps:
+            held.pop(0)
+        reqs = new + [gen[i, d] for d in range(n_dec)]
+        off = np.zeros(len(reqs) + 1, np.int64)
+        off[1:] = np.cumsum([len(r) for r in reqs])
+        plan.append((np.concatenate(reqs), off, len(new), n_dec))
+    dev_tok = [torch.from_numpy(t).cuda() for t, _, _, _ in plan]
+    s0_new = torch.full((new_per_step,), S0, dtype=torch.int64, device="cuda")                 # S0 < 2^63: same bit pattern
+
+    def run(cache, on_gpu):
+        """One pass of the loop; returns (accesses, ids released)."""
+        hist = []                # per step: (block ids of each of its sequences so far, their chain states)
+        n_acc = n_rel = 0
+        for i, (tok, off, n_new, n_dec) in enumerate(plan):
+            # decode requests are ordered oldest cohort first: cohort i-decode_steps .. i-1, new_per_step sequences each
+            cohorts = hist[-min(i, decode_steps):] if i else []
+            if on_gpu:
+                chain = torch.cat([s0_new] + [c["state"] for c in cohorts])
+                r = cache.step(dev_tok[i], off, stream, chain_in=chain)
+                ids, st, bo = r.block_id.clone(), r.chain_state.clone(), off // 16
+            else:
+                chain = np.concatenate([np.full(n_new, S0, np.uint64)] + [c["state"] for c in cohorts])
+                r = cache.step(tok, off, chain_in=chain)
+                ids, st, bo = r["block_id"], r["chain_state"], off // 16
+            n_acc += int(bo[-1])
+            for k, c in enumerate(cohorts):                               # each running sequence took one more block
+                a = int(bo[n_new + k * new_per_step])
+                c["ids"].append(ids[a:a + new_per_step])
+                c["state"] = st[n_new + k * new_per_step:n_new + (k + 1) * new_per_step]
+            hist.append(dict(ids=[ids[:int(bo[n_new])]], state=st[:n_new]))
+            if len(hist) > decode_steps:                                  # the oldest cohort finishes
+                done = hist.pop(0)
+                rel = (torch.cat if on_gpu else np.concatenate)(done["ids"])
+                cache.release(rel)
+                n_rel += int(rel.shape[0])
+        for done in hist:                                                 # the pass ends with nothing held
+            rel = (torch.cat if on_gpu else np.concatenate)(done["ids"])
+            cache.release(rel)
+            n_rel += int(rel.shape[0])
+        return n_acc, n_rel
+
+    cache = A.ArcCache(info.capacity_blocks, info.block_size, A.POLICY_ARC)
+    cache.set_pin_scope(A.PIN_HELD)
+    cache.reserve(new_per_step * (decode_steps + 1), max(int(o[-1]) // 16 for _, o, _, _ in plan))
+    run(cache, True)                                                      # warm-up pass: buffers sized, cache in steady state
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream.synchronize()
+    ev0.record(stream)
+    n_acc, n_rel = run(cache, True)
+    ev1.record(stream)
+    stream.synchronize()
+    ms = ev0.elapsed_time(ev1)
+    st = cache.stats()
+    cache.close()
+    oc = O.OracleCache(info.capacity_blocks, info.block_size, 0)
+    oc.set_pin_scope(2)
+    run(oc, False)
+    t0 = time.perf_counter()
+    run(oc, False)
+    cpu_s = time.perf_counter() - t0
+    so = oc.stats()
+    same = all(st[k] == so[k] for k in ("accesses", "hit_t1", "hit_t2", "ghost_b1", "ghost_b2", "miss", "evict_t1", "evict_t2", "p", "t1", "t2", "b1", "b2"))
+    return {"what": f"held pins + arc_step_resume + arc_release: {new_per_step} prompts admitted per step, each sequence decodes {decode_steps} blocks "
+                    f"(one per step) and then releases everything it holds; c={info.capacity_blocks}",
+            "steps": n_steps, "accesses_per_step": n_acc / n_steps, "released_ids_per_step": n_rel / n_steps,
+            "ms_per_step": ms / n_steps, "accesses_per_s": n_acc / (ms * 1e-3),
+            "includes": "binding work per step (chain-state gather, clone of block_id for the later release) and one release launch",
+            "hit_rate_blocks": (st["hit_t1"] + st["hit_t2"]) / max(1, st["accesses"]),
+            "cpu_oracle_accesses_per_s": n_acc / cpu_s, "parity_spot_check": same}
+
+
 def cpu_oracle_leg(info, steps, policy=0):
     """The oracle as it stands (g++ -O2, std::list + unordered_map, one thread) over the same steps."""
     from oracle import oracle as O
@@ -379,6 +478,9 @@ def run_ours(args):
                             "scope": f"all {W_ + K} steps from an empty cache",
                             "paper_context": "+10.8% hit rate / -12.6% TTFT (doc QA), +2.1% / -2.0% (conversation): Qwen3-14B, vLLM, 1x H100 PCIe 80 GB (PAPER.md:7, :86, :111, :117)"}
         line["state"] = {k: st_arc[k] for k in ("t1", "t2", "b1", "b2", "p")}
+        # NEXT-3 measured: a continuous-batching loop under held pins (only where a batch fits the cache)
+        if args.config == 2:
+            line["serving_loop"] = serving_loop_leg(torch, A, info, steps, stream, args.seed)
         # the CPU oracle on the same steps, on this box's host cores
         n_o, dt, tm, st_o = cpu_oracle_leg(info, steps)
         line["cpu_baseline"] = {"value": n_o / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
