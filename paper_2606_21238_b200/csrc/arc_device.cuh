@@ -68,6 +68,8 @@ struct DevState {
   uint32_t error;                 // DEV_ERR_*
   uint32_t tombs;                 // tombstones currently in the table
   uint32_t k1_ticket;             // K1 work ticket: 0 between steps (K4 resets it)
+  uint32_t step_twins;            // set by K2 when some request of the step reaches the same node twice (a 64-bit key
+                                  // collision inside one request, or the test hook); 0 between steps (K4 resets it)
   unsigned long long stat[ST_COUNT];
   // scratch for ring compaction (old window of the list being compacted)
   uint32_t cmp_head, cmp_tail;
@@ -113,6 +115,8 @@ struct StepParams {
   uint32_t block_size;
   int32_t pin_scope;              // 0: pins end with their request, 1: with the step, 2: held until arc_release
   uint32_t* node_of_block;        // pin scope 2: node id of the resident entry that owns each block id
+  uint32_t* node_stamp;           // [node_cap] (step, request) tag of the last access that resolved to the node (K2's twin check)
+  uint32_t step_tag;              // 0x80000000 | (step & 0x7FF) << 20: ORed with the request index
   unsigned long long key_and;     // test hook (arc_debug_set_key_mask): keys are ANDed with this before the probe; all ones normally
 };
 

@@ -73,10 +73,21 @@ __global__ void __launch_bounds__(256) probe_reserve_kernel(StepParams P) {
 
 // After K2: entries that raced with the winner of their key carry a slot index; the winner's node id is
 // visible now (kernel boundary).
+// Also K2's twin check: every access stamps its node with (step, request); finding one's own stamp already there means
+// the request reaches that node twice - possible only through a 64-bit key collision inside one request (or the test
+// hook that forces equal keys).  K3's wide machine pays for exact twin detection only in steps that carry the flag.
 __global__ void __launch_bounds__(256) resolve_nodes_kernel(StepParams P) {
   for (uint32_t a = blockIdx.x * blockDim.x + threadIdx.x; a < P.n_access; a += gridDim.x * blockDim.x) {
-    const uint32_t v = P.node_acc[a];
-    if (v != NODE_NONE && (v & SLOT_FLAG)) P.node_acc[a] = __ldcg(&P.table[v & ~SLOT_FLAG].node) - 1;
+    uint32_t v = P.node_acc[a];
+    if (v != NODE_NONE && (v & SLOT_FLAG)) { v = __ldcg(&P.table[v & ~SLOT_FLAG].node) - 1; P.node_acc[a] = v; }
+    if (P.n_req == 0 || v == NODE_NONE) continue;          // arc_debug_probe: no requests
+    uint32_t lo = 0, hi = P.n_req;                          // request r with blk_off[r] <= a < blk_off[r+1]
+    while (hi - lo > 1) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (P.blk_off[mid] <= (int64_t)a) lo = mid; else hi = mid;
+    }
+    const uint32_t tag = P.step_tag | lo;
+    if (atomicExch(&P.node_stamp[v], tag) == tag) P.state->step_twins = 1;
   }
 }
 
@@ -113,7 +124,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(StepParams P) {
     if (lane == 0) { P.prefix_len[r] = (int32_t)(lead * P.block_size); tokens_hit += (unsigned long long)lead * P.block_size; }
   }
   if (lane == 0 && tokens_hit) atomicAdd(&P.state->stat[ST_PREFIX_TOKENS], tokens_hit);
-  if (tid == 0) P.state->k1_ticket = 0;     // K1 of the next step starts from request 0
+  if (tid == 0) { P.state->k1_ticket = 0; P.state->step_twins = 0; }   // K1 of the next step starts from request 0
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -67,6 +67,7 @@ struct arc_cache {
   Node* d_nodes = nullptr;
   unsigned long long* d_node_key = nullptr;
   uint32_t* d_free_stack = nullptr;
+  uint32_t* d_node_stamp = nullptr;   // [node_cap] K2's twin check
   Slot* d_table = nullptr;
   RingEnt* d_ring[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   RingEnt* d_ring_alt[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -141,6 +142,8 @@ StepParams make_params(arc_cache* h) {
   P.p_after = h->d_p_after; P.alloc_ids = h->d_alloc_ids; P.evict_ids = h->d_evict_ids;
   P.capacity = (int32_t)h->c; P.policy = h->policy; P.block_size = h->B; P.key_and = h->key_and; P.pin_scope = h->pin_scope;
   P.node_of_block = h->d_node_of_block;
+  P.node_stamp = h->d_node_stamp;
+  P.step_tag = 0x80000000u | (uint32_t)((h->steps & 0x7FFull) << 20);
   return P;
 }
 
@@ -224,6 +227,8 @@ int ensure_capacity(arc_cache* h, uint32_t n_req, uint64_t N, cudaStream_t s) {
     CUDA_TRY(h, dalloc(&h->d_nodes, node_cap));
     CUDA_TRY(h, dalloc(&h->d_node_key, node_cap));
     CUDA_TRY(h, dalloc(&h->d_free_stack, node_cap));
+    CUDA_TRY(h, dalloc(&h->d_node_stamp, node_cap));
+    CUDA_TRY(h, cudaMemsetAsync(h->d_node_stamp, 0, (size_t)node_cap * sizeof(uint32_t), s));
     CUDA_TRY(h, dalloc(&h->d_table, table_slots));
     for (int L = 1; L <= 4; ++L) {
       CUDA_TRY(h, dalloc(&h->d_ring[L], ring_cap));
@@ -251,7 +256,9 @@ int ensure_capacity(arc_cache* h, uint32_t n_req, uint64_t N, cudaStream_t s) {
     bump_free_top_kernel<<<1, 1, 0, s>>>(h->d_state, node_cap - h->node_cap);
     h->launches += 2;
     CUDA_TRY(h, cudaStreamSynchronize(s));
-    dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack);
+    dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_node_stamp);
+    CUDA_TRY(h, dalloc(&h->d_node_stamp, node_cap));       // stamps only matter inside a step: start again from zero
+    CUDA_TRY(h, cudaMemsetAsync(h->d_node_stamp, 0, (size_t)node_cap * sizeof(uint32_t), s));
     h->d_nodes = nodes; h->d_node_key = keys; h->d_free_stack = stack; h->node_cap = node_cap;
   }
   if (table_slots > h->table_slots) {
@@ -527,6 +534,7 @@ int arc_reset(arc_cache* h) {
   h->slots_used_bound = 0;
   for (int L = 1; L <= 4; ++L) h->window_bound[L] = 0;
   if (h->d_node_of_block) CUDA_TRY(h, cudaMemset(h->d_node_of_block, 0xFF, (size_t)h->c * sizeof(uint32_t)));
+  CUDA_TRY(h, cudaMemset(h->d_node_stamp, 0, (size_t)h->node_cap * sizeof(uint32_t)));
   h->hold_units = 0;
   h->steps = h->requests = h->tokens_seen = h->tokens_hashed = 0;
   h->launches = 0;
@@ -538,7 +546,7 @@ void arc_destroy(arc_cache* h) {
   if (!h) return;
   cudaDeviceSynchronize();
   free_step_buffers(h);
-  dfree(h->d_state); dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_table);
+  dfree(h->d_state); dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_table); dfree(h->d_node_stamp);
   for (int L = 1; L <= 4; ++L) { dfree(h->d_ring[L]); dfree(h->d_ring_alt[L]); }
   dfree(h->d_block_counts); dfree(h->d_tokens_stage); dfree(h->d_machine_scratch);
   dfree(h->d_node_of_block); dfree(h->d_rel_cnt);

@@ -6,8 +6,10 @@
 //     warps on the class masks exchanged through shared memory, so no decision is ever broadcast;
 //   * warp w scans the LRU end of list w + 1 (T1, T2, B1, B2): 128 self-validating ring entries per round;
 //   * latencies (node fetch, ring fetch, barriers) are paid once per 128 accesses instead of once per 32.
-// The same node twice in a window (possible inside one request only through a 64-bit key collision) is found
-// exactly with a 512-slot shared-memory hash set and cuts the window, as in the 32-wide machine.
+// The same node twice in a window is possible only through a 64-bit key collision inside one request (windows never
+// cross a request boundary).  K2 flags the steps in which some request reaches a node twice (DevState::step_twins); only
+// in those steps are twins looked for, exactly, with a 512-slot shared-memory hash set, and the window cut before the
+// second occurrence as in the 32-wide machine.  In all other steps the set is never touched.
 #pragma once
 #include "machine_batched.cuh"
 
@@ -16,6 +18,13 @@ namespace arc {
 constexpr int WIDE_WARPS = 4;
 constexpr int WIDE_W = 32 * WIDE_WARPS;      // accesses per window
 constexpr int WIDE_SET = 512;                // slots of the twin-detection hash set
+constexpr int WIDE_IDS = 512;                // node-id staging ring: the current window, the next one and what is in flight
+
+__device__ __forceinline__ void cp_async_u32(uint32_t* smem_dst, const uint32_t* gmem_src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 struct WideShared {
   uint32_t m[4][WIDE_WARPS];                 // m0, m1, m2, me per chunk
@@ -24,6 +33,7 @@ struct WideShared {
   uint32_t found[5], endpos[5], need[5];
   uint32_t ctl_done, ctl_k, ctl_head[5], ctl_limit[5]; // published by thread 0 before a window's first barrier, read by the scanner warps
   uint32_t set_id[WIDE_SET], set_min[WIDE_SET];
+  uint32_t ids[WIDE_IDS];                    // node ids of the upcoming accesses: access a sits in ids[a % WIDE_IDS] (filled by cp.async)
   uint4 vic[5][WIDE_W];                      // per list: entries found from the LRU end {node, block, -, position}
   SerialCtx ctx;                             // the machine state after a by-the-book access done by warp 0
 };
@@ -130,11 +140,10 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
     const uint32_t head = S.ctl_head[L], limit = S.ctl_limit[L];
     uint32_t q0 = head & ~3u, found = 0;
     const int want = (int)S.ctl_k;
-    if ((int32_t)(limit - q0) > 0) { found += wide_scan_round(ring, P.ring_mask, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds; }
-    __syncthreads();                                   // (B1)
+    __syncthreads();                                   // (B1) the scanners never hold this barrier up
     if (*any_twin) { __syncthreads(); __syncthreads(); }
-    // while the owners roll (not in an all-hit window): up to 2 more rounds, until as many live entries are known as the
-    // window has accesses, so that the owners rarely wait for a scan after the roll
+    // while the owners roll (not in an all-hit window, which needs no victim): up to 3 rounds, until as many live entries
+    // are known as the window has accesses, so that the owners rarely wait for a scan after the roll
     bool all_hit = true;
 #pragma unroll
     for (int u = 0; u < WIDE_WARPS; ++u) {
@@ -143,7 +152,7 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
       const uint32_t hit = (P.policy == POLICY_LRU) ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);
       all_hit = all_hit && ((hit & km) == km);
     }
-    for (int it = 0; !all_hit && it < 2 && (int)found < want && (int32_t)(limit - q0) > 0; ++it) {
+    for (int it = 0; !all_hit && it < 3 && (int)found < want && (int32_t)(limit - q0) > 0; ++it) {
       found += wide_scan_round(ring, P.ring_mask, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
     }
     __syncthreads();                                   // (B2) the owners have published what the window needs
@@ -173,6 +182,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
   const bool lru = (P.policy == POLICY_LRU);
   const bool hold = (P.pin_scope == 2);      // held scope: see machine_batched.cuh
+  const bool twins = P.state->step_twins != 0;   // K2 saw a request reach some node twice: look for twins in every window
   const int32_t c = P.capacity;
   const int64_t N = (int64_t)P.n_access;
   SerialCtx C;            // identical in every thread
@@ -189,9 +199,30 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
     return;
   }
 
-  // node ids are prefetched one window ahead: pre_n = node_acc[pre_base + tid]
-  int64_t pre_base = 0;
-  uint32_t pre_n = (tid < N) ? P.node_acc[tid] : NODE_NONE;
+  // Node ids travel ahead of the windows through a shared-memory ring filled with cp.async: at the start of a window the
+  // ids of that window AND of the one after it are already there (they were requested at least one window earlier),
+  // wherever a cut made the window start.
+  uint32_t ids_loaded = 0;                               // ids [0, ids_loaded) have been requested; a multiple of WIDE_W
+  auto ids_request = [&](int64_t upto) {
+    while ((int64_t)ids_loaded < upto && (int64_t)ids_loaded < N) {
+      const uint32_t a = ids_loaded + (uint32_t)tid;
+      if ((int64_t)a < N) cp_async_u32(&S.ids[a & (WIDE_IDS - 1)], P.node_acc + a);
+      ids_loaded += (uint32_t)WIDE_W;
+    }
+    cp_async_commit();
+  };
+  ids_request(2 * WIDE_W);
+  int64_t spec_base = -1;                                // the access index the speculative record below belongs to, minus tid
+  // ... and so is the node RECORD, speculatively: it is loaded while the current window rolls (after B1, when everything
+  // the previous window wrote is visible) and is exact unless the current window itself changes that node, which happens
+  // in two ways only: the window also accesses the node (found by probing the window's twin-detection set), or it takes
+  // the node as a victim / dropped ghost (the node's ring position lies in a range the window consumes).  Either way the
+  // record is then loaded again at the start of the next window, as it is after a cut window.  Without the step's twin
+  // flag no set exists and a window can share a node only with a window of ANOTHER request, so the speculation then stops
+  // at request boundaries; with the flag (next to never) there is no speculation at all.
+  Node spec;
+  spec.list = L_FREE; spec.pos = 0; spec.block = -1; spec.slot = 0;
+  bool spec_ok = false;
 
   int64_t my_off = 0, my_off1 = 0;
   for (uint32_t r = 0; r < P.n_req; ++r) {
@@ -212,19 +243,22 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
 #pragma unroll
         for (int L = 1; L <= 4; ++L) { S.ctl_head[L] = C.head[L]; S.ctl_limit[L] = (L <= 2) ? C.bound[L] : C.tail[L]; }
       }
+      cp_async_wait_all();                                           // ids requested in earlier windows have landed
       __syncthreads();                                               // (S0) the previous window's writes are visible; the scanners start
       const long long tw0 = clock64();
-      uint32_t n = pre_n;
-      if (pre_base != a0) n = (a0 + tid < N) ? P.node_acc[a0 + tid] : NODE_NONE;     // the last window was cut short
+      const uint32_t n = act0 ? S.ids[(uint32_t)(a0 + tid) & (WIDE_IDS - 1)] : NODE_NONE;
       Node rec;
       rec.list = L_FREE; rec.pos = 0; rec.block = -1; rec.slot = 0;
-      if (act0) rec = ld_node(P.nodes + n);
-      pre_base = a0 + kmax;
-      pre_n = (pre_base + tid < N) ? P.node_acc[pre_base + tid] : NODE_NONE;
+      if (act0) {
+        if (spec_base == a0 && spec_ok) rec = spec; else rec = ld_node(P.nodes + n);
+      }
+      // the id this thread will own if the next window starts where this one is due to end
+      const uint32_t pre_n = (a0 + kmax + tid < N) ? S.ids[(uint32_t)(a0 + kmax + tid) & (WIDE_IDS - 1)] : NODE_NONE;
+      ids_request(a0 + kmax + 2 * WIDE_W);
 
       // (1) the same node twice in the window: exact detection with a shared-memory hash set
       uint32_t slot = 0xFFFFFFFFu;
-      if (act0) {
+      if (twins && act0) {
         uint32_t h = (n * 2654435761u) >> 23;                        // 9 bits
         for (;;) {
           const uint32_t old = atomicCAS(&S.set_id[h], 0xFFFFFFFFu, n);
@@ -245,7 +279,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         if (lane == 0) { S.m[0][warp] = b0; S.m[1][warp] = b1; S.m[2][warp] = b2; S.m[3][warp] = be; }
       }
       __syncthreads();                                               // (B1) class masks and the hash set are complete
-      if (s_any_twin) {                                              // CTA-uniform, next to never taken
+      if (twins && s_any_twin) {                                     // CTA-uniform, next to never taken
         const bool later = act0 && S.set_min[slot] < (uint32_t)tid;
         const uint32_t tb = __ballot_sync(FULL, later);
         if (lane == 0) S.twin[warp] = tb;
@@ -256,6 +290,13 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         if (first < k) { k = first; dbg[DBG_CUT_TWIN]++; }
         __syncthreads();
         if (tid == 0) s_any_twin = 0;
+      }
+      // the next window's record, speculatively (see above); a node this window accesses too is not trusted
+      spec_ok = false;
+      spec_base = a0 + kmax;
+      if (!twins && j + kmax < nb && pre_n != NODE_NONE) {           // the next window belongs to the same request
+        spec = ld_node(P.nodes + pre_n);
+        spec_ok = true;
       }
       uint32_t M0[WIDE_WARPS], M1[WIDE_WARPS], M2[WIDE_WARPS], ME[WIDE_WARPS], KM[WIDE_WARPS], HIT[WIDE_WARPS];
       bool all_hit = true;
@@ -302,11 +343,11 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         else { C.tail[L_T2] += hold ? 0u : (uint32_t)k; C.t1 -= (int32_t)t1hits; C.t2 += (int32_t)t1hits; C.stat[ST_HIT_T1] += t1hits; C.stat[ST_HIT_T2] += (uint32_t)k - t1hits; }
         C.elig1 -= (int32_t)e1d; C.elig2 -= (int32_t)e2d;
         C.stat[ST_ACCESSES] += (uint32_t)k;
-        if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
         if (tid < 5) S.need[tid] = 0;
         if (lane == 0) S.bad[warp] = 0;
         j += k;
         dbg[DBG_WIN_HIT]++; dbg[DBG_ACC_HIT_WIN] += (unsigned)k;
+        if (twins && act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
         __syncthreads();                                             // (B2), (B2'), (B3): the scanners' sequence
         __syncthreads();
         __syncthreads();
@@ -365,10 +406,11 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
             __syncwarp();
             if (lane == 0) S.ctx = T;
           }
-          if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
+          if (twins && act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
           __syncthreads();
           C = S.ctx;
           j += 1;
+          spec_ok = false;                             // the by-the-book access may have changed any node
           dbg[DBG_WIN_SERIAL]++;
           dbg[DBG_CYC_SERIAL] += (unsigned long long)(clock64() - tw3);
           continue;
@@ -461,6 +503,11 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       C.stat[ST_FRESH] += (uint32_t)(D.R.nf - C.next_fresh);
       C.n_alloc += wide_count(NH);
       C.n_evict += wide_count(EV);
+      if (spec_ok) {                                 // did this window take the speculated node as a victim or drop it?
+#pragma unroll
+        for (int L = 1; L <= 4; ++L)
+          if (spec.list == (uint32_t)L && need[L] && (spec.pos - C.head[L]) < (endpos[L] - C.head[L])) spec_ok = false;
+      }
 #pragma unroll
       for (int L = 1; L <= 4; ++L) C.head[L] = endpos[L];
       if (!hold) { C.tail[L_T1] += wide_count(PT1); C.tail[L_T2] += wide_count(PT2); }
@@ -468,7 +515,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       C.tail[L_B2] += need[L_T2];
       C.t1 = D.R.t1; C.t2 = D.R.t2; C.b1 = D.R.b1; C.b2 = D.R.b2; C.p = D.R.p; C.next_fresh = D.R.nf;
       C.elig1 = D.R.e1; C.elig2 = D.R.e2;
-      if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
+      if (twins && act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
       j += k;
       dbg[DBG_WIN_GENERAL]++; dbg[DBG_ACC_GENERAL_WIN] += (unsigned)k;
       dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw3);
