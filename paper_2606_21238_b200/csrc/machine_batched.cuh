@@ -81,36 +81,58 @@ __device__ __forceinline__ int phase_ghost(Roll& R, int32_t c, uint32_t li, int 
     }
     return n;
   }
-  // Ghost hit (R5 cases 2, 3).  While delta = 1 the steps of a run are identical as long as the victim keeps coming
-  // from the same list, so the run is rolled in O(1): the regime and its length are computed with selects (no
-  // branches: one warp has no other warp to hide a branch behind); anything else is one by-the-book step.
+  // Ghost hit (R5 cases 2, 3).  A run of ghost hits in the same list is rolled in O(1) for as long as (1) delta, the step
+  // of p, keeps its value d and (2) the victim keeps coming from the same list.  The regime and its length are computed
+  // with selects (one warp has no other warp to hide a branch behind); anything else is one by-the-book step.
+  //   bx = the list that was hit, by = the other ghost list.  d = max(1, by / bx) (R6).
+  //   victims from T1 while hitting B2, or from T2 while hitting B1, move one entry from bx's side to by's side per step:
+  //   bx -= 1, by += 1, and d stays the same for the steps j with (by + j) < (d + 1)(bx - j); the other two combinations
+  //   leave b1, b2 and with them d alone.
+  //   R7's fallback is part of the regimes: a list with nothing left to evict (e = 0) stays that way, so once the
+  //   preferred list is exhausted the victims come from the other one whatever the preference does.
   const bool inb2 = (li == L_B2);
-  const int32_t bx = inb2 ? R.b2 : R.b1, by = inb2 ? R.b1 : R.b2;      // bx: the list that was hit
-  const bool d_one = by < 2 * bx;
+  const int32_t bx = inb2 ? R.b2 : R.b1, by = inb2 ? R.b1 : R.b2;
   const int32_t p0 = R.p;
-  // B1: REPLACE prefers T1 for the steps j with t1 - j > p + j + 1, i.e. J = (t1 - p) / 2 of them
-  // B2: REPLACE(true) prefers T1 while t1 - j >= 1 and t1 >= p - 1
-  const int32_t J1 = max(0, (R.t1 - R.p) / 2);
-  const bool pref1 = inb2 ? (R.t1 >= 1 && R.t1 >= R.p - 1) : (J1 > 0);
-  const int32_t n_delta = (2 * bx - by + 2) / 3;                         // steps while delta stays 1 when bx shrinks and by grows
-  // regime a: victims from T1;  regime b: victims from T2
-  const bool ra = d_one && pref1 && R.e1 > 0, rb = d_one && !pref1 && R.e2 > 0;
-  int32_t na = min(m, R.e1), nbb = min(m, R.e2);
-  na = inb2 ? min(na, min(n_delta, R.t1)) : min(na, J1);                 // B2+T1 moves b1 up / b2 down; B1+T1 leaves b1, b2
-  nbb = inb2 ? ((R.t1 >= 1) ? min(nbb, R.p - 1 - R.t1) : nbb) : min(nbb, n_delta);
-  if (ra || rb) {
-    n = ra ? na : nbb;
-    const uint32_t run = bits_from(i, n);
-    R.s0 |= ra ? run : 0u; R.s1 |= ra ? 0u : run;
-    R.e1 -= ra ? n : 0; R.e2 -= ra ? 0 : n;
-    R.t1 -= ra ? n : 0; R.t2 += ra ? n : 0;
-    // ghost list sizes: B1+T1 none; B1+T2: b1 -= n, b2 += n; B2+T1: b1 += n, b2 -= n; B2+T2: none
-    const int32_t db1 = (!inb2 && !ra) ? -n : ((inb2 && ra) ? n : 0);
-    R.b1 += db1; R.b2 -= db1;
-    R.p = inb2 ? max(0, R.p - n) : min(c, R.p + n);
-    if (lane >= i) R.my_p = inb2 ? max(0, p0 - min(lane - i + 1, n)) : min(c, p0 + min(lane - i + 1, n));
+  int32_t d = 1, n_delta;
+  if (by < 2 * bx) {
+    n_delta = (2 * bx - by + 2) / 3;
   } else {
-    const int32_t d = (by >= 2 * bx && bx > 0) ? by / bx : 1;
+    d = by / max(bx, 1);
+    n_delta = (bx - (by - d * bx) + d + 1) / (d + 2);             // ((d + 1) bx - by + d + 1) / (d + 2), without the overflow
+  }
+  // the preference of REPLACE at the run's first step, and for how many steps it keeps it
+  //   B1: p rises by d, T1 is preferred at step j iff t1_j > p + (j + 1) d
+  //   B2: p falls by d, T1 is preferred at step j iff t1_j >= 1 and t1_j >= p - (j + 1) d
+  const bool pref1 = inb2 ? (R.t1 >= 1 && R.t1 >= R.p - d) : (R.t1 > R.p + d);
+  const bool from1 = pref1 ? (R.e1 > 0) : !(R.e2 > 0);              // R7 with its fallback, first step
+  const bool ok = from1 ? (R.e1 > 0) : (R.e2 > 0);
+  int32_t keep;                                                     // steps for which the victim's list cannot change
+  if (from1) {
+    // victims from T1: t1 falls by one per step.  Forced (T2 exhausted): no limit from the preference.
+    // B1: preferred while t1 - j > p + (j + 1) d, i.e. (t1 - p) / (d + 1) steps; B2: the preference only gets stronger.
+    keep = (R.e2 > 0 && !inb2) ? ((d == 1) ? (R.t1 - R.p) / 2 : (R.t1 - R.p) / (d + 1)) : R.e1;
+    keep = min(keep, R.e1);
+    if (inb2) keep = min(keep, n_delta);                            // B2 + T1: b2 -= 1, b1 += 1
+  } else {
+    // victims from T2: t1 stays.  Forced (T1 exhausted): no limit.  B1: p only rises, T1 stays unpreferred.
+    // B2: unpreferred while t1 < p - (j + 1) d, i.e. (p - t1 - 1) / d steps (t1 = 0: for ever).
+    keep = (R.e1 > 0 && inb2 && R.t1 >= 1) ? ((d == 1) ? (R.p - R.t1 - 1) : (R.p - R.t1 - 1) / d) : R.e2;
+    keep = min(keep, R.e2);
+    if (!inb2) keep = min(keep, n_delta);                           // B1 + T2: b1 -= 1, b2 += 1
+  }
+  if (ok && keep >= 1) {
+    n = min(m, keep);
+    const uint32_t run = bits_from(i, n);
+    R.s0 |= from1 ? run : 0u; R.s1 |= from1 ? 0u : run;
+    R.e1 -= from1 ? n : 0; R.e2 -= from1 ? 0 : n;
+    R.t1 -= from1 ? n : 0; R.t2 += from1 ? n : 0;
+    // ghost list sizes: B1+T1 none; B1+T2: b1 -= n, b2 += n; B2+T1: b1 += n, b2 -= n; B2+T2: none
+    const int32_t db1 = (!inb2 && !from1) ? -n : ((inb2 && from1) ? n : 0);
+    R.b1 += db1; R.b2 -= db1;
+    const long long dd = d;                                         // n d can exceed 32 bits when one ghost list is tiny
+    R.p = inb2 ? (int32_t)max(0ll, p0 - n * dd) : (int32_t)min((long long)c, p0 + n * dd);
+    if (lane >= i) { const int32_t t = min(lane - i + 1, n); R.my_p = inb2 ? (int32_t)max(0ll, p0 - t * dd) : (int32_t)min((long long)c, p0 + t * dd); }
+  } else {
     R.p = inb2 ? max(0, R.p - d) : min(c, R.p + d);
     roll_replace(R, inb2, i);
     if (inb2) R.b2--; else R.b1--;
@@ -131,17 +153,21 @@ __device__ __forceinline__ int phase_miss(Roll& R, int32_t c, int i, int m) {
   }
   int n = 1;
   // Miss (R5 case 4), same idea.  fill: the cache is not full yet (b1 = b2 = 0, I7).  r1: REPLACE takes T1's LRU
-  // entry (t1 stays); r2: T1 is at or below its target, REPLACE takes T2's LRU entry and T1 grows by one per miss.
+  // entry (t1 stays); r2: REPLACE takes T2's LRU entry and T1 grows by one per miss.  REPLACE prefers T1 while t1 > p;
+  // R7's fallback is part of the regimes: a list with nothing left to evict stays that way, so with T2 exhausted the
+  // victims come from T1 whatever the preference (r1), with T1 exhausted from T2 (r2).
   // In case 4A (t1 + b1 = c) B1's LRU ghost is dropped; in case 4B B2's LRU ghost is dropped while b1 + b2 = c.
   const bool fill = R.t1 + R.t2 < c;
   const int32_t gapA = c - R.t1 - R.b1, gapS = c - R.b1 - R.b2;
   const bool isA = gapA == 0, isS = gapS == 0;
   const bool pref1 = R.t1 > R.p;
-  const bool r1 = !fill && R.t1 < c && pref1 && R.e1 > 0, r2 = !fill && R.t1 < c && !pref1 && R.e2 > 0;
+  const bool r1 = !fill && R.t1 < c && R.e1 > 0 && (pref1 || R.e2 <= 0);
+  const bool r2 = !fill && R.t1 < c && R.e2 > 0 && (!pref1 || R.e1 <= 0);
   const int32_t lim_gap = isA ? m : (isS ? gapA : min(gapA, gapS));     // steps until the case changes
   const int32_t nf = min(m, c - R.t1 - R.t2);
   const int32_t n1 = min(min(m, R.e1), lim_gap);
-  const int32_t n2 = min(min(min(m, R.e2), lim_gap), min(R.p - R.t1 + 1, c - R.t1));
+  // r2 by preference lasts until t1 passes p; r2 because T1 is exhausted has no such end
+  const int32_t n2 = min(min(min(m, R.e2), lim_gap), min((!pref1 && R.e1 > 0) ? (R.p - R.t1 + 1) : m, c - R.t1));
   if (fill || r1 || r2) {
     n = fill ? nf : (r1 ? n1 : n2);
     const uint32_t run = bits_from(i, n);
