@@ -30,32 +30,35 @@ struct WideShared {
   uint32_t m[4][WIDE_WARPS];                 // m0, m1, m2, me per chunk
   uint32_t bad[WIDE_WARPS];
   uint32_t twin[WIDE_WARPS];
-  uint32_t found[5], endpos[5], need[5];
+  uint32_t found[5], more[5], need[5];       // scanners: live entries found so far, whether the list has more to scan; owners: victims needed
   uint32_t ctl_done, ctl_k, ctl_head[5], ctl_limit[5]; // published by thread 0 before a window's first barrier, read by the scanner warps
+  uint32_t ctl_twins;                        // the step carries K2's twin flag: no barrier of the sequence is ever skipped
+  uint32_t red[WIDE_WARPS][5];               // per-warp class counts, summed by thread 0 at the end
   uint32_t set_id[WIDE_SET], set_min[WIDE_SET];
   uint32_t ids[WIDE_IDS];                    // node ids of the upcoming accesses: access a sits in ids[a % WIDE_IDS] (filled by cp.async)
   uint4 vic[5][WIDE_W];                      // per list: entries found from the LRU end {node, block, -, position}
   SerialCtx ctx;                             // the machine state after a by-the-book access done by warp 0
 };
 
-// sum of popcounts of the chunk masks below chunk w, plus the bits below `lane` in chunk w
-__device__ __forceinline__ uint32_t wide_rank(const uint32_t (&mask)[WIDE_WARPS], int w, uint32_t lt) {
+// Rank of a thread's access inside a window-wide mask (four 32-bit chunks): the set bits below it.  lm[] is per thread
+// and fixed for the kernel: all ones for the chunks below its own, the bits below its lane for its own chunk, zero above;
+// me[] has the thread's own bit in its own chunk.  No selects on the (run-time) warp index.
+__device__ __forceinline__ uint32_t wide_rank(const uint32_t (&mask)[WIDE_WARPS], const uint32_t (&lm)[WIDE_WARPS]) {
   uint32_t r = 0;
 #pragma unroll
-  for (int u = 0; u < WIDE_WARPS; ++u) r += (u < w) ? (uint32_t)__popc(mask[u]) : (u == w ? (uint32_t)__popc(mask[u] & lt) : 0u);
+  for (int u = 0; u < WIDE_WARPS; ++u) r += (uint32_t)__popc(mask[u] & lm[u]);
   return r;
+}
+__device__ __forceinline__ bool wide_has(const uint32_t (&mask)[WIDE_WARPS], const uint32_t (&me)[WIDE_WARPS]) {
+  uint32_t r = 0;
+#pragma unroll
+  for (int u = 0; u < WIDE_WARPS; ++u) r |= mask[u] & me[u];
+  return r != 0;
 }
 __device__ __forceinline__ uint32_t wide_count(const uint32_t (&mask)[WIDE_WARPS]) {
   uint32_t r = 0;
 #pragma unroll
   for (int u = 0; u < WIDE_WARPS; ++u) r += (uint32_t)__popc(mask[u]);
-  return r;
-}
-
-__device__ __forceinline__ uint32_t wide_pick(const uint32_t (&mask)[WIDE_WARPS], int w) {
-  uint32_t r = mask[0];
-#pragma unroll
-  for (int u = 1; u < WIDE_WARPS; ++u) r = (u == w) ? mask[u] : r;
   return r;
 }
 
@@ -107,12 +110,21 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
 
 // One scan round of a scanner warp: 128 ring entries from q0 (a multiple of 4), 4 per lane; live entries are appended
 // to vic[] in LRU order.  Returns the number of live entries found in the round.
-__device__ __forceinline__ uint32_t wide_scan_round(const RingEnt* ring, uint32_t ring_mask, uint32_t q0, uint32_t head, uint32_t limit,
+struct ScanRegs { uint4 e0, e1; };
+// the loads of one round (positions q0 + 4 lane .. + 3); issued a round ahead so that their latency overlaps the previous
+// round's bookkeeping.  Positions past the limit are loaded too (the ring is a power-of-two buffer) and ignored.
+__device__ __forceinline__ ScanRegs wide_scan_load(const RingEnt* ring, uint32_t ring_mask, uint32_t q0, int lane) {
+  const uint32_t qA = q0 + 4u * (uint32_t)lane;
+  ScanRegs r;
+  r.e0 = __ldcg(reinterpret_cast<const uint4*>(ring + (qA & ring_mask)));
+  r.e1 = __ldcg(reinterpret_cast<const uint4*>(ring + ((qA + 2u) & ring_mask)));
+  return r;
+}
+__device__ __forceinline__ uint32_t wide_scan_round(const ScanRegs& regs, uint32_t q0, uint32_t head, uint32_t limit,
                                                     uint32_t found, uint4* vic, int lane, uint32_t lt) {
   const uint32_t FULL = 0xFFFFFFFFu;
   const uint32_t qA = q0 + 4u * (uint32_t)lane;
-  const uint4 e0 = __ldcg(reinterpret_cast<const uint4*>(ring + (qA & ring_mask)));
-  const uint4 e1 = __ldcg(reinterpret_cast<const uint4*>(ring + ((qA + 2u) & ring_mask)));
+  const uint4 e0 = regs.e0, e1 = regs.e1;
   // live = inside [head, limit) and not a tombstone
   const bool l0 = (int32_t)(qA - head) >= 0 && (int32_t)(limit - qA) > 0 && e0.x != RING_TOMB;
   const bool l1 = (int32_t)(qA + 1u - head) >= 0 && (int32_t)(limit - qA - 1u) > 0 && e0.z != RING_TOMB;
@@ -140,6 +152,7 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
     const uint32_t head = S.ctl_head[L], limit = S.ctl_limit[L];
     uint32_t q0 = head & ~3u, found = 0;
     const int want = (int)S.ctl_k;
+    ScanRegs cur = wide_scan_load(ring, P.ring_mask, q0, lane);   // in flight while the owners fetch; used after B1
     __syncthreads();                                   // (B1) the scanners never hold this barrier up
     if (*any_twin) { __syncthreads(); __syncthreads(); }
     // while the owners roll (not in an all-hit window, which needs no victim): up to 3 rounds, until as many live entries
@@ -152,20 +165,29 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
       const uint32_t hit = (P.policy == POLICY_LRU) ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);
       all_hit = all_hit && ((hit & km) == km);
     }
-    for (int it = 0; !all_hit && it < 3 && (int)found < want && (int32_t)(limit - q0) > 0; ++it) {
-      found += wide_scan_round(ring, P.ring_mask, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
-    }
-    __syncthreads();                                   // (B2) the owners have published what the window needs
-    const uint32_t need = S.need[L];
-    while (found < need && (int32_t)(limit - q0) > 0) {
-      found += wide_scan_round(ring, P.ring_mask, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
+    if (all_hit && !S.ctl_twins) continue;             // the owners apply an all-hit window without any further barrier
+    for (int it = 0; !all_hit && it < 4 && (int)found < want && (int32_t)(limit - q0) > 0; ++it) {
+      const ScanRegs nxt = wide_scan_load(ring, P.ring_mask, q0 + (uint32_t)WIDE_W, lane);
+      found += wide_scan_round(cur, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
+      cur = nxt;
     }
     __syncwarp();
-    if (lane == 0) {
-      S.found[L] = found;
-      S.endpos[L] = need ? ((found >= need) ? S.vic[L][need - 1].w + 1u : limit) : head;
+    if (lane == 0) { S.found[L] = found; S.more[L] = (int32_t)(limit - q0) > 0; }
+    __syncthreads();                                   // (B2) the owners have published what the window needs, the scanners what they have
+    bool extra = false;                                // some list must be scanned further: CTA-uniform, computed by everybody
+#pragma unroll
+    for (int X = 1; X <= 4; ++X) extra = extra || (S.found[X] < S.need[X] && S.more[X]);
+    if (extra) {
+      const uint32_t need = S.need[L];
+      while (found < need && (int32_t)(limit - q0) > 0) {
+        cur = wide_scan_load(ring, P.ring_mask, q0, lane);
+        found += wide_scan_round(cur, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
+      }
+      __syncthreads();                                 // (B2x) everybody has read the first report
+      __syncwarp();
+      if (lane == 0) S.found[L] = found;
+      __syncthreads();                                 // (B2') victims of all four lists are in shared memory
     }
-    __syncthreads();                                   // (B2') victims of all four lists are in shared memory
     __syncthreads();                                   // (B3)
     bool serial = false;
 #pragma unroll
@@ -180,6 +202,9 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
   __shared__ uint32_t s_any_twin;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
+  uint32_t lm[WIDE_WARPS], me[WIDE_WARPS];   // see wide_rank / wide_has
+#pragma unroll
+  for (int u = 0; u < WIDE_WARPS; ++u) { lm[u] = (u < warp) ? FULL : ((u == warp) ? lt : 0u); me[u] = (u == warp) ? (1u << lane) : 0u; }
   const bool lru = (P.policy == POLICY_LRU);
   const bool hold = (P.pin_scope == 2);      // held scope: see machine_batched.cuh
   const bool twins = P.state->step_twins != 0;   // K2 saw a request reach some node twice: look for twins in every window
@@ -188,7 +213,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
   SerialCtx C;            // identical in every thread
   ctx_load(C, P);
   for (int i = tid; i < WIDE_SET; i += 2 * WIDE_W) { S.set_id[i] = 0xFFFFFFFFu; S.set_min[i] = 0xFFFFFFFFu; }
-  if (tid == 0) s_any_twin = 0;
+  if (tid == 0) { s_any_twin = 0; S.ctl_twins = twins ? 1u : 0u; }
   __syncthreads();
   unsigned long long dbg[DBG_COUNT];
 #pragma unroll
@@ -223,6 +248,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
   Node spec;
   spec.list = L_FREE; spec.pos = 0; spec.block = -1; spec.slot = 0;
   bool spec_ok = false;
+  uint32_t my_cls[5] = {0, 0, 0, 0, 0};                  // accesses of general windows this thread applied, by class
 
   int64_t my_off = 0, my_off1 = 0;
   for (uint32_t r = 0; r < P.n_req; ++r) {
@@ -347,10 +373,11 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         if (lane == 0) S.bad[warp] = 0;
         j += k;
         dbg[DBG_WIN_HIT]++; dbg[DBG_ACC_HIT_WIN] += (unsigned)k;
-        if (twins && act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
-        __syncthreads();                                             // (B2), (B2'), (B3): the scanners' sequence
-        __syncthreads();
-        __syncthreads();
+        if (twins) {                                                 // the full barrier sequence (need = 0: no B2'), else none at all
+          if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
+          __syncthreads();                                           // (B2)
+          __syncthreads();                                           // (B3)
+        }
         dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw1);
         continue;
       }
@@ -366,25 +393,36 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       uint32_t need[5];
       need[0] = 0; need[L_T1] = wide_count(D.s0); need[L_T2] = wide_count(S2); need[L_B1] = wide_count(D.d1); need[L_B2] = wide_count(D.d2);
       if (tid == 0) { S.need[L_T1] = need[L_T1]; S.need[L_T2] = need[L_T2]; S.need[L_B1] = need[L_B1]; S.need[L_B2] = need[L_B2]; }
-      __syncthreads();                                               // (B2) the scanners learn what the window needs
-      __syncthreads();                                               // (B2') victims of all four lists are in shared memory
+      __syncthreads();                                               // (B2) the scanners learn what the window needs, the owners what they have
       uint32_t found[5], endpos[5];
+      bool extra = false;                                            // CTA-uniform: some list must be scanned further
 #pragma unroll
-      for (int L = 1; L <= 4; ++L) { found[L] = S.found[L]; endpos[L] = S.endpos[L]; }
+      for (int L = 1; L <= 4; ++L) { found[L] = S.found[L]; extra = extra || (found[L] < need[L] && S.more[L]); }
+      if (extra) {
+        __syncthreads();                                             // (B2x) everybody has read the first report
+        __syncthreads();                                             // (B2') victims of all four lists are in shared memory
+#pragma unroll
+        for (int L = 1; L <= 4; ++L) found[L] = S.found[L];
+      }
+#pragma unroll
+      for (int L = 1; L <= 4; ++L) {
+        const uint32_t limit = (L <= 2) ? C.bound[L] : C.tail[L];
+        endpos[L] = need[L] ? ((found[L] >= need[L]) ? S.vic[L][need[L] - 1].w + 1u : limit) : C.head[L];
+      }
       // (2) an accessed node whose ring entry lies inside a consumed range, or a victim / drop that does not exist
       bool act = tid < k;
-      uint32_t my_src = ((wide_pick(D.s0, warp) >> lane) & 1u) | (((wide_pick(D.s1, warp) >> lane) & 1u) << 1);
-      bool my_d1 = (wide_pick(D.d1, warp) >> lane) & 1u, my_d2 = (wide_pick(D.d2, warp) >> lane) & 1u;
+      uint32_t my_src = (wide_has(D.s0, me)) | ((wide_has(D.s1, me)) << 1);
+      bool my_d1 = wide_has(D.d1, me), my_d2 = wide_has(D.d2, me);
       {
         bool bad = false;
         if (act) {
 #pragma unroll
           for (int L = 1; L <= 4; ++L)
             if (lst == (uint32_t)L && !held && need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
-          if ((my_src & 1u) && wide_rank(D.s0, warp, lt) >= found[L_T1]) bad = true;
-          if (my_src == 2 && wide_rank(S2, warp, lt) >= found[L_T2]) bad = true;
-          if (my_d1 && wide_rank(D.d1, warp, lt) >= found[L_B1]) bad = true;
-          if (my_d2 && wide_rank(D.d2, warp, lt) >= found[L_B2]) bad = true;
+          if ((my_src & 1u) && wide_rank(D.s0, lm) >= found[L_T1]) bad = true;
+          if (my_src == 2 && wide_rank(S2, lm) >= found[L_T2]) bad = true;
+          if (my_d1 && wide_rank(D.d1, lm) >= found[L_B1]) bad = true;
+          if (my_d2 && wide_rank(D.d2, lm) >= found[L_B2]) bad = true;
         }
         const uint32_t bb = __ballot_sync(FULL, bad);
         if (lane == 0) S.bad[warp] = bb;
@@ -427,8 +465,8 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
 #pragma unroll
         for (int L = 1; L <= 4; ++L) endpos[L] = need[L] ? S.vic[L][need[L] - 1].w + 1u : C.head[L];
         act = tid < k;
-        my_src = ((wide_pick(D.s0, warp) >> lane) & 1u) | (((wide_pick(D.s1, warp) >> lane) & 1u) << 1);
-        my_d1 = (wide_pick(D.d1, warp) >> lane) & 1u; my_d2 = (wide_pick(D.d2, warp) >> lane) & 1u;
+        my_src = (wide_has(D.s0, me)) | ((wide_has(D.s1, me)) << 1);
+        my_d1 = wide_has(D.d1, me); my_d2 = wide_has(D.d2, me);
       }
       if (D.R.err) C.err = D.R.err;
       dbg[DBG_ROLL_CALLS] += D.R.calls; dbg[DBG_ROLL_PHASES] += D.R.phases;
@@ -445,30 +483,30 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         EV[u] = D.s0[u] | D.s1[u];
       }
       if (act) {
-        const bool is_hit = (wide_pick(HIT, warp) >> lane) & 1u;
+        const bool is_hit = wide_has(HIT, me);
         int32_t blk = rec.block, ev = -1;
         uint32_t dropped = NODE_NONE;
         if (my_src) {
-          const uint4 v = (my_src == 2) ? S.vic[L_T2][wide_rank(S2, warp, lt)] : S.vic[L_T1][wide_rank(D.s0, warp, lt)];
+          const uint4 v = (my_src == 2) ? S.vic[L_T2][wide_rank(S2, lm)] : S.vic[L_T1][wide_rank(D.s0, lm)];
           blk = ev = (int32_t)v.y;
           if (my_src == 3) {                        // leaves no ghost: the key leaves the directory in K4
             st_node_keep_slot(P.nodes + v.x, L_ABSENT, 0, -1);
             dropped = v.x;
           } else {
-            const uint32_t q = (my_src == 1) ? C.tail[L_B1] + wide_rank(G1, warp, lt) : C.tail[L_B2] + wide_rank(S2, warp, lt);
+            const uint32_t q = (my_src == 1) ? C.tail[L_B1] + wide_rank(G1, lm) : C.tail[L_B2] + wide_rank(S2, lm);
             __stcg(((my_src == 1) ? P.ring[L_B1] : P.ring[L_B2]) + (q & P.ring_mask), ring_ent(v.x, -1));
             st_node_keep_slot(P.nodes + v.x, (my_src == 1) ? L_B1 : L_B2, q, -1);
           }
-        } else if ((wide_pick(D.fm, warp) >> lane) & 1u) {
-          blk = C.next_fresh + (int32_t)wide_rank(D.fm, warp, lt);
+        } else if (wide_has(D.fm, me)) {
+          blk = C.next_fresh + (int32_t)wide_rank(D.fm, lm);
         }
         if (my_d1 || my_d2) {
-          const uint4 d = my_d1 ? S.vic[L_B1][wide_rank(D.d1, warp, lt)] : S.vic[L_B2][wide_rank(D.d2, warp, lt)];
+          const uint4 d = my_d1 ? S.vic[L_B1][wide_rank(D.d1, lm)] : S.vic[L_B2][wide_rank(D.d2, lm)];
           st_node_keep_slot(P.nodes + d.x, L_ABSENT, 0, -1);
           dropped = d.x;
         }
-        const bool toT1 = (wide_pick(PT1, warp) >> lane) & 1u;
-        const uint32_t q = toT1 ? C.tail[L_T1] + wide_rank(PT1, warp, lt) : C.tail[L_T2] + wide_rank(PT2, warp, lt);
+        const bool toT1 = wide_has(PT1, me);
+        const uint32_t q = toT1 ? C.tail[L_T1] + wide_rank(PT1, lm) : C.tail[L_T2] + wide_rank(PT2, lm);
         if (lst >= L_T1 && lst <= L_B2 && !held) ring_tomb(P, lst, rec.pos);     // the node leaves its old position
         if (hold) {
           st_node(P.nodes + n, (toT1 ? L_T1 : L_T2) | NODE_HELD, held ? rec.pos + 1u : 1u, blk, rec.slot);
@@ -483,18 +521,15 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         P.evicted_id[out] = ev;
         P.p_after[out] = D.my_p;
         P.dropped[a0 + tid] = dropped;
-        if (!is_hit) P.alloc_ids[C.n_alloc + wide_rank(NH, warp, lt)] = blk;
-        if (ev >= 0) P.evict_ids[C.n_evict + wide_rank(EV, warp, lt)] = ev;
+        if (!is_hit) P.alloc_ids[C.n_alloc + wide_rank(NH, lm)] = blk;
+        if (ev >= 0) P.evict_ids[C.n_evict + wide_rank(EV, lm)] = ev;
+      }
+      // class counts: every thread counts its own access, the warps add them up at the end of the kernel
+      if (act) {
+        my_cls[0] += (lst == L_ABSENT); my_cls[1] += (lst == L_T1); my_cls[2] += (lst == L_T2) && !lru;
+        my_cls[3] += (lst == L_B1); my_cls[4] += (lst == L_B2);
       }
       // uniform state (every thread computes the same)
-#pragma unroll
-      for (int u = 0; u < WIDE_WARPS; ++u) {
-        C.stat[ST_HIT_T1] += __popc(HIT[u] & M0[u]);
-        C.stat[ST_HIT_T2] += lru ? 0u : (uint32_t)__popc(HIT[u] & M1[u]);
-        C.stat[ST_GHOST_B1] += __popc(M0[u] & M1[u] & ~M2[u] & KM[u]);
-        C.stat[ST_GHOST_B2] += __popc(M2[u] & ~M0[u] & ~M1[u] & KM[u]);
-        C.stat[ST_MISS] += __popc(~(M0[u] | M1[u] | M2[u]) & KM[u]);
-      }
       C.stat[ST_ACCESSES] += (uint32_t)k;
       C.stat[ST_EVICT_T1] += need[L_T1];
       C.stat[ST_EVICT_T2] += need[L_T2];
@@ -521,8 +556,20 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw3);
     }
   }
+#pragma unroll
+  for (int i = 0; i < 5; ++i) {
+    const uint32_t t = __reduce_add_sync(FULL, my_cls[i]);
+    if (lane == 0) S.red[warp][i] = t;
+  }
   if (tid == 0) S.ctl_done = 1;
   __syncthreads();                                                   // the scanners leave; the last window's writes are done
+  if (tid == 0) {
+#pragma unroll
+    for (int w = 0; w < WIDE_WARPS; ++w) {
+      C.stat[ST_MISS] += S.red[w][0]; C.stat[ST_HIT_T1] += S.red[w][1]; C.stat[ST_HIT_T2] += S.red[w][2];
+      C.stat[ST_GHOST_B1] += S.red[w][3]; C.stat[ST_GHOST_B2] += S.red[w][4];
+    }
+  }
   dbg[DBG_CYC_TOTAL] = (unsigned long long)(clock64() - t_begin);
   if (tid == 0) {
     ctx_store(C, P);
