@@ -188,11 +188,13 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
       if (lane == 0) S.found[L] = found;
       __syncthreads();                                 // (B2') victims of all four lists are in shared memory
     }
-    __syncthreads();                                   // (B3)
-    bool serial = false;
+    if (__syncthreads_or(0)) {                         // (B3) some access cannot be applied with the window
+      __syncthreads();                                 // (B3x) the owners' reports are in shared memory
+      bool serial = false;
 #pragma unroll
-    for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.bad[u]) serial = (32 * u + __ffs(S.bad[u]) - 1) == 0;
-    if (serial) __syncthreads();                       // the by-the-book access of warp 0
+      for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.bad[u]) serial = (32 * u + __ffs(S.bad[u]) - 1) == 0;
+      if (serial) __syncthreads();                     // the by-the-book access of warp 0
+    }
   }
   if (lane == 0 && rounds) atomicAdd(&P.state->dbg[DBG_SCAN_ROUNDS], rounds);
 }
@@ -376,7 +378,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         if (twins) {                                                 // the full barrier sequence (need = 0: no B2'), else none at all
           if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
           __syncthreads();                                           // (B2)
-          __syncthreads();                                           // (B3)
+          __syncthreads_or(0);                                       // (B3)
         }
         dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw1);
         continue;
@@ -413,24 +415,27 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       bool act = tid < k;
       uint32_t my_src = (wide_has(D.s0, me)) | ((wide_has(D.s1, me)) << 1);
       bool my_d1 = wide_has(D.d1, me), my_d2 = wide_has(D.d2, me);
-      {
-        bool bad = false;
-        if (act) {
+      bool bad = false;
+      if (act) {
 #pragma unroll
-          for (int L = 1; L <= 4; ++L)
-            if (lst == (uint32_t)L && !held && need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
+        for (int L = 1; L <= 4; ++L)
+          if (lst == (uint32_t)L && !held && need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
+        // a victim / drop can be missing only from a list that has fewer live entries than the window wants (uniform)
+        if (found[L_T1] < need[L_T1] || found[L_T2] < need[L_T2] || found[L_B1] < need[L_B1] || found[L_B2] < need[L_B2]) {
           if ((my_src & 1u) && wide_rank(D.s0, lm) >= found[L_T1]) bad = true;
           if (my_src == 2 && wide_rank(S2, lm) >= found[L_T2]) bad = true;
           if (my_d1 && wide_rank(D.d1, lm) >= found[L_B1]) bad = true;
           if (my_d2 && wide_rank(D.d2, lm) >= found[L_B2]) bad = true;
         }
+      }
+      int first_bad = -1;
+      if (__syncthreads_or(bad)) {                                   // (B3) next to always: nobody is bad, nothing to exchange
         const uint32_t bb = __ballot_sync(FULL, bad);
         if (lane == 0) S.bad[warp] = bb;
-      }
-      __syncthreads();                                               // (B3)
-      int first_bad = -1;
+        __syncthreads();                                             // (B3x)
 #pragma unroll
-      for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.bad[u]) first_bad = 32 * u + __ffs(S.bad[u]) - 1;
+        for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.bad[u]) first_bad = 32 * u + __ffs(S.bad[u]) - 1;
+      }
       const long long tw3 = clock64();
       dbg[DBG_CYC_SCAN] += (unsigned long long)(tw3 - tw2);
       if (first_bad >= 0) {
