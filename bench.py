@@ -444,7 +444,7 @@ def run_ours(args):
         line["dominant_kernel"] = {"kernel": "K3 ARC machine (arc_machine_wide_kernel, one CTA)", "share_of_step": sums.get("machine_ms", 0.0) / tot,
                                    "bound": "latency: dependent instructions of one serial state machine (DESIGN.md 7.3); neither HBM nor tensor nor ALU throughput",
                                    "ns_per_access": 1e6 * sums.get("machine_ms", 0.0) / max(1, n_acc),
-                                   "ncu": "profiles/r01d_scanner_warps.md: 48 warp instructions per access over 8 warps, 17 % issue-active per scheduler"}
+                                   "ncu": "profiles/r01e_held_resume_roll.md: 41 warp instructions per access over 8 warps, 19 % issue-active per scheduler"}
         k1_insitu = ALGO_BYTES_PER_BLOCK * n_acc / max(sums.get("hash_ms", 0.0) * 1e-3, 1e-12) / 1e9
         # K1 roofline: bulk run through arc_hash_blocks
         nb, nreq_b, mean_ms, best_ms = k1_bulk_roofline(torch, A, args.bulk_gib, stream, args.seed)
@@ -452,7 +452,7 @@ def run_ours(args):
         line["roofline"] = {"kernel": "K1 chained block hashing (arc_hash_blocks)", "bound": "hbm", "achieved": achieved, "peak": peak,
                             "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8000": achieved / 8000.0, "peak_source": peak_src,
                             "traffic": 1.168e9 if abs(args.bulk_gib - 1.0) < 1e-9 else None,
-                            "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this launch (profiles/r01d_scanner_warps.md: 1.086 GB + 82.2 MB)",
+                            "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this launch (profiles/r01e_held_resume_roll.md: 1.0855 GB + 82.3 MB)",
                             "algorithmic_bytes_per_launch": ALGO_BYTES_PER_BLOCK * nb, "ms_per_launch": mean_ms,
                             "best_ms": best_ms, "tokens_per_s": 16 * nb / (mean_ms * 1e-3),
                             "workload": f"{nreq_b} D5-shaped requests, {nb} blocks, {64 * nb / 2**30:.2f} GiB of tokens (>> 126 MB L2)",
