@@ -233,6 +233,134 @@ __global__ void __launch_bounds__(256, 4) hash_blocks_kernel(const int32_t* __re
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// In-step hashing of steps with FEW requests: one warp per request leaves the step waiting for its longest request (a
+// 1,000-block document is 32 dependent rounds).  H4 is affine, so a request is cut into segments of K1_SEG blocks that are
+// scanned independently from a zero carry (hash_segments_kernel: one warp per segment, the same loads and scans as
+// above) and put together afterwards (hash_fixup_kernel): with c_s the true state before segment s and E_s the local end
+// state of the segment, c_{s+1} = E_s + K^len_s c_s, and block i of the segment has state local_i + K^(i+1) c_s.
+constexpr int K1_SEG = 128;
+
+// states[] gets the LOCAL states, in access order (index blk_off[r] + nb - 1 - i); seg_end[r * max_seg + s] = E_s.
+__global__ void __launch_bounds__(256, 4) hash_segments_kernel(const int32_t* __restrict__ tokens, const int64_t* __restrict__ offsets,
+                                                               const int64_t* __restrict__ blk_off, uint32_t n_req, uint32_t max_seg,
+                                                               unsigned long long* __restrict__ states,
+                                                               unsigned long long* __restrict__ seg_end, uint32_t* __restrict__ ticket) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t* tok = reinterpret_cast<const uint32_t*>(tokens);
+  const int64_t lo = offsets[0], hi = offsets[n_req];
+  LaneConsts LC;
+  const int q = lane & 3;
+  LC.salt0 = (unsigned long long)(2 * q + 1) * H_M * H_C1;
+  LC.salt1 = (unsigned long long)(2 * q + 2) * H_M * H_C1;
+  LC.kp = kpow_small(lane + 1);
+  LC.owner = 4 * (lane & 7) + (lane >> 3);
+  const int base_mis = (int)((reinterpret_cast<uintptr_t>(tok) >> 2) & 3);
+  const unsigned long long total = (unsigned long long)max_seg * n_req;
+  for (;;) {
+    uint32_t t0 = 0;
+    if (lane == 0) t0 = atomicAdd(ticket, 1u);                      // one segment per ticket: segments are equal pieces of work
+    t0 = __shfl_sync(0xFFFFFFFFu, t0, 0);
+    if (t0 >= total) break;
+    const uint32_t r = t0 % n_req, sg = t0 / n_req;                 // ticket t = segment t / n_req of request t % n_req
+    if ((int64_t)sg * K1_SEG >= blk_off[r + 1] - blk_off[r]) continue;
+    {
+      const int64_t o = blk_off[r], nb = blk_off[r + 1] - o;
+      const int64_t b0 = (int64_t)sg * K1_SEG, nbs = min((int64_t)K1_SEG, nb - b0);
+      const int64_t ts = offsets[r] + 16 * b0;
+      const int s = (int)((base_mis + ts) & 3);
+      const int64_t va = ts - s;
+      unsigned long long carry = 0;
+      auto n_vec = [&](int64_t rb) { return (int)((16 * min((int64_t)32, nbs - rb) + s + 3) >> 2); };
+      auto finish = [&](const RoundVecs& cur, int64_t rb) {
+        const int cnt = (int)min((int64_t)32, nbs - rb);
+        const unsigned long long st = round_local_scan(cur, s, cnt, lane, LC) + LC.kp * carry;
+        if (lane < cnt) {
+          const int64_t i = b0 + rb + lane;
+          states[o + (nb - 1 - i)] = st;
+          if (rb + lane == nbs - 1) seg_end[(size_t)r * max_seg + sg] = st;
+        }
+        carry = shfl64(st, 31);
+      };
+      RoundVecs A = load_round(tok, va, n_vec(0), lane, lo, hi), B;
+      for (int64_t rb = 0;;) {
+        if (rb + 32 < nbs) B = load_round(tok, va + 16 * (rb + 32), n_vec(rb + 32), lane, lo, hi);
+        finish(A, rb);
+        rb += 32;
+        if (rb >= nbs) break;
+        if (rb + 32 < nbs) A = load_round(tok, va + 16 * (rb + 32), n_vec(rb + 32), lane, lo, hi);
+        finish(B, rb);
+        rb += 32;
+        if (rb >= nbs) break;
+      }
+    }
+  }
+}
+
+// K^(128 m): square-and-multiply over the bits of m (m < 2^11)
+__device__ __forceinline__ unsigned long long kpow_seg(uint32_t m) {
+  unsigned long long r = 1;
+#pragma unroll
+  for (int b = 0; b < 11; ++b) {
+    unsigned long long f = 1;                       // K^(128 2^b) as a compile-time constant
+    switch (b) {
+      case 0: f = kpow(128u); break;       case 1: f = kpow(256u); break;      case 2: f = kpow(512u); break;
+      case 3: f = kpow(1024u); break;      case 4: f = kpow(2048u); break;     case 5: f = kpow(4096u); break;
+      case 6: f = kpow(8192u); break;      case 7: f = kpow(16384u); break;    case 8: f = kpow(32768u); break;
+      case 9: f = kpow(65536u); break;     default: f = kpow(131072u); break;
+    }
+    if (m & (1u << b)) r *= f;
+  }
+  return r;
+}
+
+// One warp per segment (warp w: segment w / n_req of request w % n_req).  All segments before the warp's own are full,
+// so the true state before segment s is c_s = K^(128 s) c_0 + sum_{j<s} K^(128 (s-1-j)) E_j: one term per lane and a
+// warp sum; then the segment's local states become keys.  The warp of a request's last segment also writes chain_out.
+__global__ void __launch_bounds__(256) hash_fixup_kernel(const int64_t* __restrict__ blk_off, uint32_t n_req, uint32_t max_seg,
+                                                         unsigned long long* __restrict__ keys, const unsigned long long* __restrict__ seg_end,
+                                                         const unsigned long long* __restrict__ chain_in, unsigned long long* __restrict__ chain_out) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+  const unsigned long long kp = kpow_small(lane + 1);                 // K^(lane+1)
+  const uint32_t total = n_req * max_seg;
+  for (uint32_t w = warp0; w < total; w += n_warps) {
+    const uint32_t r = w % n_req, sg = w / n_req;
+    const int64_t o = blk_off[r], nb = blk_off[r + 1] - o;
+    const int64_t b0 = (int64_t)sg * K1_SEG;
+    const unsigned long long c0 = chain_in ? chain_in[r] : H_S0;
+    if (nb == 0) { if (sg == 0 && lane == 0 && chain_out) chain_out[r] = c0; continue; }
+    if (b0 >= nb) continue;
+    unsigned long long part = 0;
+    for (uint32_t jb = 0; jb < sg; jb += 32) {
+      const uint32_t jj = jb + (uint32_t)lane;
+      if (jj < sg) part += kpow_seg(sg - 1 - jj) * seg_end[(size_t)r * max_seg + jj];
+    }
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) part += shfl_xor64(part, d);
+    const unsigned long long carry = kpow_seg(sg) * c0 + part;        // the state before this segment's first block
+    const int len = (int)min((int64_t)K1_SEG, nb - b0);
+    unsigned long long kr = kp;                                        // K^(32 it + lane + 1)
+    unsigned long long last = 0;
+#pragma unroll
+    for (int it = 0; it < K1_SEG / 32; ++it) {
+      const int i = 32 * it + lane;
+      if (i < len) {
+        const int64_t at = o + (nb - 1 - (b0 + i));
+        const unsigned long long st = keys[at] + kr * carry;
+        keys[at] = finalize_key(st);
+        if (i == len - 1) last = st;
+      }
+      kr *= kpow(32);
+    }
+    if (b0 + len == nb && chain_out) {                                 // the request's last segment: its end state goes out
+      const int src = (len - 1) & 31;
+      last = shfl64(last, src);
+      if (lane == 0) chain_out[r] = last;
+    }
+  }
+}
+
 // the last thing on the stream after a hashing launch: the ticket returns to 0 for the next launch
 __global__ void reset_ticket_kernel(uint32_t* ticket) { *ticket = 0; }
 

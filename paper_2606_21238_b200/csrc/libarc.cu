@@ -30,6 +30,8 @@ uint64_t g_hash_launches = 0;
 constexpr int kStageSlots = 4;
 constexpr uint32_t kMaxReq = 1u << 20;
 constexpr uint64_t kMaxCapacity = 1ull << 28;   // node ids carry two flag bits
+constexpr uint32_t kSegEndCap = 1u << 16;       // n_req * segments-per-request the segmented K1 is used up to
+constexpr uint32_t kSegMaxReq = 512;            // with more requests than this one warp per request already fills the GPU
 
 uint32_t pow2_at_least(uint64_t x) {
   uint64_t p = 64;
@@ -68,6 +70,7 @@ struct arc_cache {
   unsigned long long* d_node_key = nullptr;
   uint32_t* d_free_stack = nullptr;
   uint32_t* d_node_stamp = nullptr;   // [node_cap] K2's twin check
+  unsigned long long* d_seg_end = nullptr;   // [kSegEndCap] end states of K1's segments (steps with few, long requests)
   Slot* d_table = nullptr;
   RingEnt* d_ring[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   RingEnt* d_ring_alt[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -414,8 +417,21 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
   StepParams P = make_params(h);
   P.tokens = d_tokens; P.n_req = n_req; P.n_access = (uint32_t)N;
   if (N) {
-    launch_hash(d_tokens, P.offsets, P.blk_off, n_req, P.keys_acc, &h->d_state->k1_ticket, true, s,                 // K1
-                reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state);
+    uint64_t max_nb = 0;
+    for (uint32_t r = 0; r < n_req; ++r) max_nb = std::max<uint64_t>(max_nb, (uint64_t)(blk_off[r + 1] - blk_off[r]));
+    const uint32_t max_seg = (uint32_t)((max_nb + K1_SEG - 1) / K1_SEG);
+    if (n_req <= kSegMaxReq && max_seg >= 2 && max_seg <= 1024 && (uint64_t)n_req * max_seg <= kSegEndCap) {
+      // K1, few long requests: segments hashed independently, then put together (hash_kernels.cuh)
+      if (!h->d_seg_end) CUDA_TRY(h, dalloc(&h->d_seg_end, kSegEndCap));
+      hash_segments_kernel<<<grid_for((uint64_t)n_req * max_seg, 8, 148 * 4), 256, 0, s>>>(d_tokens, P.offsets, P.blk_off, n_req, max_seg, P.keys_acc,
+                                                                                           h->d_seg_end, &h->d_state->k1_ticket);
+      hash_fixup_kernel<<<grid_for((uint64_t)n_req * max_seg, 8, 148 * 4), 256, 0, s>>>(P.blk_off, n_req, max_seg, P.keys_acc, h->d_seg_end,
+                                                                    reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state);
+      h->launches += 1;
+    } else {
+      launch_hash(d_tokens, P.offsets, P.blk_off, n_req, P.keys_acc, &h->d_state->k1_ticket, true, s,               // K1
+                  reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state);
+    }
     if (h->profiling) cudaEventRecord(h->ev[2], s);
     probe_reserve_kernel<<<grid_for(N, 32, 148 * 8), 256, 0, s>>>(P);                                     // K2
     resolve_nodes_kernel<<<grid_for(N, 256, 148 * 8), 256, 0, s>>>(P);
@@ -549,7 +565,7 @@ void arc_destroy(arc_cache* h) {
   dfree(h->d_state); dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_table); dfree(h->d_node_stamp);
   for (int L = 1; L <= 4; ++L) { dfree(h->d_ring[L]); dfree(h->d_ring_alt[L]); }
   dfree(h->d_block_counts); dfree(h->d_tokens_stage); dfree(h->d_machine_scratch);
-  dfree(h->d_node_of_block); dfree(h->d_rel_cnt);
+  dfree(h->d_node_of_block); dfree(h->d_rel_cnt); dfree(h->d_seg_end);
   for (int i = 0; i < kStageSlots; ++i) if (h->stage_done[i]) cudaEventDestroy(h->stage_done[i]);
   for (int i = 0; i < 7; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
   delete h;

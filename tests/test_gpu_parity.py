@@ -575,3 +575,27 @@ def test_decode_loop_with_held_pins(arc, policy):
     assert grown > 50                                         # sequences really grew block by block
     assert_same_state(gc, oc, f"decode p{policy}")
     gc.close()
+
+
+@pytest.mark.parametrize("shift", [0, 1, 2, 3])
+def test_segmented_in_step_hashing(arc, shift):
+    """Steps with few, long requests hash every request in 128-block segments (hash_segments_kernel + hash_fixup_kernel).
+    Request lengths around the segment and round boundaries, a misaligned token buffer, continuation states: the keys
+    (seen through the lists), the classes and the chain states equal the oracle's."""
+    rng = np.random.default_rng(31 + shift)
+    blocks = [128, 129, 127, 1, 0, 255, 256, 257, 33, 1023, 1024, 640]
+    reqs = [rng.integers(0, 128000, size=16 * nb + int(rng.integers(0, 16))).astype(np.int32) for nb in blocks]
+    tokens, offsets = W.pack_requests(reqs)
+    buf = torch.zeros(len(tokens) + 8, dtype=torch.int32, device="cuda")
+    buf[shift:shift + len(tokens)] = torch.from_numpy(tokens).cuda()
+    view = buf[shift:shift + len(tokens)]                               # 4-byte aligned only for shift != 0
+    c = 8192
+    gc, oc = arc.ArcCache(c), O.OracleCache(c)
+    chain = rng.integers(0, 2 ** 63, size=len(reqs)).astype(np.uint64)
+    for rep, ci in enumerate((None, None, chain)):
+        g = gc.step(view, offsets, chain_in=ci).to_host()
+        o = oc.step(tokens, offsets, chain_in=ci)
+        assert_same_step(g, o, f"segmented rep {rep}")
+        assert np.array_equal(g["chain_state"], o["chain_state"]), rep
+        assert_same_state(gc, oc, f"segmented rep {rep}")
+    gc.close()
