@@ -73,6 +73,25 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
                                           int warp, int lane) {
   D.R = roll_init(C);
   D.my_p = C.p;
+  {
+    // The commonest whole window of a cache in steady state: every access a miss, case 4A (t1 + b1 = c) with T1 above its
+    // target and enough evictable entries for all of them: each miss drops B1's LRU ghost and evicts T1's LRU entry, no
+    // counter moves (phase_miss's first case, for the window instead of chunk by chunk).
+    uint32_t any = 0;
+#pragma unroll
+    for (int u = 0; u < WIDE_WARPS; ++u) any |= (S.m[0][u] | S.m[1][u] | S.m[2][u]) & bits_from(0, min(32, max(0, k - 32 * u)));
+    Roll& R = D.R;
+    if (!lru && any == 0 && R.t1 + R.t2 == c && R.t1 + R.b1 == c && R.t1 < c && R.t1 > R.p && R.e1 >= k) {
+#pragma unroll
+      for (int u = 0; u < WIDE_WARPS; ++u) {
+        const uint32_t km = bits_from(0, min(32, max(0, k - 32 * u)));
+        D.s0[u] = km; D.d1[u] = km; D.s1[u] = D.d2[u] = D.fm[u] = 0;
+      }
+      R.e1 -= k;
+      R.phases++;
+      return;
+    }
+  }
 #pragma unroll
   for (int u = 0; u < WIDE_WARPS; ++u) {
     const int ku = min(32, max(0, k - 32 * u));
