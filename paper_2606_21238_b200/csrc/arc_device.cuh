@@ -78,6 +78,7 @@ struct DevState {
   // pin scope 2: entries of T1 / T2 without holds (= the entries in the rings = the possible victims), kept across steps
   int32_t u1, u2;
   uint32_t release_bad;           // scratch of release_kernel
+  uint32_t win_seq;               // K3 wide machine: number of the last window (31 bits, never 0), see node_stamp
 };
 enum : int { DBG_WIN_HIT = 0, DBG_WIN_GENERAL, DBG_WIN_SERIAL, DBG_CUT_TWIN, DBG_CUT_CONFLICT, DBG_SCAN_ROUNDS, DBG_ACC_HIT_WIN,
              DBG_ACC_GENERAL_WIN, DBG_CYC_FETCH, DBG_CYC_ROLL, DBG_CYC_SCAN, DBG_CYC_APPLY, DBG_CYC_SERIAL, DBG_CYC_TOTAL, DBG_ROLL_CALLS, DBG_ROLL_PHASES, DBG_COUNT };
@@ -115,7 +116,8 @@ struct StepParams {
   uint32_t block_size;
   int32_t pin_scope;              // 0: pins end with their request, 1: with the step, 2: held until arc_release
   uint32_t* node_of_block;        // pin scope 2: node id of the resident entry that owns each block id
-  uint32_t* node_stamp;           // [node_cap] (step, request) tag of the last access that resolved to the node (K2's twin check)
+  uint32_t* node_stamp;           // [node_cap] K2: (step, request) tag of the last access that resolved to the node (twin check,
+                                  // bit 31 set); K3 wide machine: number of the last window that accessed the node (bit 31 clear)
   uint32_t step_tag;              // 0x80000000 | (step & 0x7FF) << 20: ORed with the request index
   unsigned long long key_and;     // test hook (arc_debug_set_key_mask): keys are ANDed with this before the probe; all ones normally
 };

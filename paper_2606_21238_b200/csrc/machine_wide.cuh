@@ -264,11 +264,15 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
   // in two ways only: the window also accesses the node (found by probing the window's twin-detection set), or it takes
   // the node as a victim / dropped ghost (the node's ring position lies in a range the window consumes).  Either way the
   // record is then loaded again at the start of the next window, as it is after a cut window.  Without the step's twin
-  // flag no set exists and a window can share a node only with a window of ANOTHER request, so the speculation then stops
-  // at request boundaries; with the flag (next to never) there is no speculation at all.
+  // flag no set exists; instead every owner writes its window's number into node_stamp[n] BEFORE the window's first
+  // barrier and the speculative load, issued AFTER it, reads the stamp along with the record: equal to the current
+  // window's number = this window accesses the node too (only a window of another request can).  With the flag (next to
+  // never) there is no speculation at all.
   Node spec;
   spec.list = L_FREE; spec.pos = 0; spec.block = -1; spec.slot = 0;
   bool spec_ok = false;
+  uint32_t win_seq = P.state->win_seq;                     // numbers the windows across steps; 31 bits, never 0
+  uint32_t spec_mark = 0;                                  // node_stamp of the speculated node, read with its record
   uint32_t my_cls[5] = {0, 0, 0, 0, 0};                  // accesses of general windows this thread applied, by class
 
   int64_t my_off = 0, my_off1 = 0;
@@ -296,7 +300,11 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       const uint32_t n = act0 ? S.ids[(uint32_t)(a0 + tid) & (WIDE_IDS - 1)] : NODE_NONE;
       Node rec;
       rec.list = L_FREE; rec.pos = 0; rec.block = -1; rec.slot = 0;
+      if (spec_mark == win_seq) spec_ok = false;                     // the previous window accessed the speculated node too
+      win_seq = (win_seq + 1u) & 0x7FFFFFFFu;
+      if (win_seq == 0) win_seq = 1;
       if (act0) {
+        if (!twins) __stcg(P.node_stamp + n, win_seq);               // seen by the speculative loads after B1
         if (spec_base == a0 && spec_ok) rec = spec; else rec = ld_node(P.nodes + n);
       }
       // the id this thread will own if the next window starts where this one is due to end
@@ -341,8 +349,9 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       // the next window's record, speculatively (see above); a node this window accesses too is not trusted
       spec_ok = false;
       spec_base = a0 + kmax;
-      if (!twins && j + kmax < nb && pre_n != NODE_NONE) {           // the next window belongs to the same request
+      if (!twins && pre_n != NODE_NONE) {
         spec = ld_node(P.nodes + pre_n);
+        spec_mark = __ldcg(P.node_stamp + pre_n);                    // looked at when the next window starts, not now
         spec_ok = true;
       }
       uint32_t M0[WIDE_WARPS], M1[WIDE_WARPS], M2[WIDE_WARPS], ME[WIDE_WARPS], KM[WIDE_WARPS], HIT[WIDE_WARPS];
@@ -596,6 +605,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
   }
   dbg[DBG_CYC_TOTAL] = (unsigned long long)(clock64() - t_begin);
   if (tid == 0) {
+    P.state->win_seq = win_seq;
     ctx_store(C, P);
 #pragma unroll
     for (int i = 0; i < DBG_COUNT; ++i) P.state->dbg[i] += dbg[i];
