@@ -174,7 +174,7 @@ def run_e2e(torch, A, info, steps, host, bases, warmup, stream):
     cache.reserve(max(req), max(acc))
     hv = host.numpy()
     views = [hv[bases[i]:bases[i] + len(steps[i][0])] for i in range(len(steps))]
-    d2h = 0
+    d2h = h2d = 0
     for i in range(warmup):
         cache.step_host(views[i], steps[i][1], stream)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -183,12 +183,13 @@ def run_e2e(torch, A, info, steps, host, bases, warmup, stream):
     ev0.record(stream)
     for i in range(warmup, len(steps)):
         r = cache.step_host(views[i], steps[i][1], stream)
-        d2h += 4 * (len(r["prefix_len"]) + 2 + 2 * r["n_access"])   # prefix_len, counts, alloc_ids[N], evict_ids[N]
+        d2h += r["d2h_bytes"]   # one packed copy: prefix_len | counts | alloc_ids | evict_ids, as the library counts it
+        h2d += r["h2d_bytes"]   # tokens + offsets and block offsets
     ev1.record(stream)
     stream.synchronize()
     wall_ms = (time.perf_counter() - t0) * 1e3
     cache.close()
-    return max(wall_ms, ev0.elapsed_time(ev1)), d2h
+    return max(wall_ms, ev0.elapsed_time(ev1)), d2h, h2d
 
 
 def k1_bulk_roofline(torch, A, gib, stream, seed):
@@ -409,9 +410,9 @@ def run_ours(args):
     ms_max, tot_acc, tot_tok, tot_req = P.reduce_timing(dist if world > 1 else None, torch, ms, n_acc, n_tok, n_req)
 
     # ---- e2e: the same steps through arc_step_host (H2D + D2H inside) ----------------------------------
-    e2e_ms, d2h = run_e2e(torch, A, info, steps, host, bases, W_, stream)
+    e2e_ms, d2h, h2d_total = run_e2e(torch, A, info, steps, host, bases, W_, stream)
     e2e_ms_max, _, _, _ = P.reduce_timing(dist if world > 1 else None, torch, e2e_ms, n_acc, n_tok, n_req)
-    h2d = (4 * n_tok + 8 * 2 * (n_req + K)) / K
+    h2d = h2d_total / K
 
     line = {
         "metric": METRIC, "value": tot_acc / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,

@@ -75,6 +75,7 @@ typedef struct {
   const int32_t *prefix_len; /* [n_req] */
   const int32_t *alloc_ids;  /* [n_alloc] */
   const int32_t *evict_ids;  /* [n_evict] */
+  uint64_t h2d_bytes, d2h_bytes; /* what the call moved over the bus: tokens + offsets in; one packed copy out */
 } arc_host_result;
 
 /* Cumulative counters since create/reset plus the current list sizes (R12). */
@@ -133,7 +134,8 @@ int arc_step_resume(arc_cache *h, const int32_t *d_tokens, const int64_t *h_offs
 
 /* Same step end to end from HOST memory: copies h_tokens (HOST int32, pinned or pageable) to a
  * library-owned device buffer, runs the step, copies prefix_len, counts, alloc_ids and evict_ids back
- * to pinned host memory and synchronises the stream before returning. */
+ * to pinned host memory (ONE device-to-host copy: the device keeps them in one buffer laid out like the
+ * host's) and synchronises the stream before returning. */
 int arc_step_host(arc_cache *h, const int32_t *h_tokens, const int64_t *h_offsets, uint32_t n_req,
                   void *cuda_stream, arc_host_result *out);
 

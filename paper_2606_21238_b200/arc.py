@@ -44,7 +44,8 @@ class _StepResult(C.Structure):
 
 class _HostResult(C.Structure):
     _fields_ = [("n_access", C.c_uint64), ("n_alloc", C.c_uint32), ("n_evict", C.c_uint32),
-                ("prefix_len", C.POINTER(C.c_int32)), ("alloc_ids", C.POINTER(C.c_int32)), ("evict_ids", C.POINTER(C.c_int32))]
+                ("prefix_len", C.POINTER(C.c_int32)), ("alloc_ids", C.POINTER(C.c_int32)), ("evict_ids", C.POINTER(C.c_int32)),
+                ("h2d_bytes", C.c_uint64), ("d2h_bytes", C.c_uint64)]
 
 
 class _Stats(C.Structure):
@@ -234,7 +235,7 @@ class ArcCache:
         n_req = len(o) - 1
         take = lambda p, n: np.ctypeslib.as_array(p, shape=(n,)).copy() if n else np.zeros(0, np.int32)
         return dict(n_access=int(raw.n_access), prefix_len=take(raw.prefix_len, n_req), alloc_ids=take(raw.alloc_ids, raw.n_alloc),
-                    evict_ids=take(raw.evict_ids, raw.n_evict))
+                    evict_ids=take(raw.evict_ids, raw.n_evict), h2d_bytes=int(raw.h2d_bytes), d2h_bytes=int(raw.d2h_bytes))
 
     def stats(self) -> dict:
         s = _Stats()

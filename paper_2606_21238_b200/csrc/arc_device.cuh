@@ -119,6 +119,7 @@ struct StepParams {
   uint32_t* node_stamp;           // [node_cap] K2: (step, request) tag of the last access that resolved to the node (twin check,
                                   // bit 31 set); K3 wide machine: number of the last window that accessed the node (bit 31 clear)
   uint32_t step_tag;              // 0x80000000 | (step & 0x7FF) << 20: ORed with the request index
+  uint32_t* counts_out;           // [2] copy of DevState::counts next to prefix_len / alloc_ids / evict_ids (one D2H copy in arc_step_host)
   unsigned long long key_and;     // test hook (arc_debug_set_key_mask): keys are ANDed with this before the probe; all ones normally
 };
 

@@ -124,7 +124,10 @@ __global__ void __launch_bounds__(256) finalize_kernel(StepParams P) {
     if (lane == 0) { P.prefix_len[r] = (int32_t)(lead * P.block_size); tokens_hit += (unsigned long long)lead * P.block_size; }
   }
   if (lane == 0 && tokens_hit) atomicAdd(&P.state->stat[ST_PREFIX_TOKENS], tokens_hit);
-  if (tid == 0) { P.state->k1_ticket = 0; P.state->step_twins = 0; }   // K1 of the next step starts from request 0
+  if (tid == 0) {
+    P.state->k1_ticket = 0; P.state->step_twins = 0;                   // K1 of the next step starts from request 0
+    P.counts_out[0] = P.state->counts[0]; P.counts_out[1] = P.state->counts[1];
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -80,7 +80,8 @@ struct arc_cache {
   unsigned long long* d_keys = nullptr;
   uint32_t* d_node_acc = nullptr;
   uint32_t* d_dropped = nullptr;
-  int32_t* d_prefix_len = nullptr;
+  int32_t* d_result_pack = nullptr;   // prefix_len[req_cap] | counts[2] | alloc_ids[n_cap] | evict_ids[n_cap]: same layout as h_result
+  int32_t* d_prefix_len = nullptr;    // = d_result_pack
   unsigned long long* d_chain_state = nullptr;   // [req_cap] H4 state after each request's last full block
   uint8_t* d_cls = nullptr;
   int32_t *d_block_id = nullptr, *d_evicted_id = nullptr, *d_p_after = nullptr, *d_alloc_ids = nullptr, *d_evict_ids = nullptr;
@@ -146,6 +147,7 @@ StepParams make_params(arc_cache* h) {
   P.capacity = (int32_t)h->c; P.policy = h->policy; P.block_size = h->B; P.key_and = h->key_and; P.pin_scope = h->pin_scope;
   P.node_of_block = h->d_node_of_block;
   P.node_stamp = h->d_node_stamp;
+  P.counts_out = reinterpret_cast<uint32_t*>(h->d_result_pack + h->req_cap);
   P.step_tag = 0x80000000u | (uint32_t)((h->steps & 0x7FFull) << 20);
   return P;
 }
@@ -180,8 +182,8 @@ int launch_compact(arc_cache* h, cudaStream_t s, int L, uint32_t src_cap, uint32
 
 void free_step_buffers(arc_cache* h) {
   dfree(h->d_offsets); dfree(h->d_keys); dfree(h->d_node_acc); dfree(h->d_dropped);
-  dfree(h->d_prefix_len); dfree(h->d_chain_state); dfree(h->d_cls); dfree(h->d_block_id); dfree(h->d_evicted_id); dfree(h->d_p_after);
-  dfree(h->d_alloc_ids); dfree(h->d_evict_ids);
+  dfree(h->d_result_pack); h->d_prefix_len = h->d_alloc_ids = h->d_evict_ids = nullptr;
+  dfree(h->d_chain_state); dfree(h->d_cls); dfree(h->d_block_id); dfree(h->d_evicted_id); dfree(h->d_p_after);
   if (h->h_stage) cudaFreeHost(h->h_stage);
   h->h_stage = nullptr;
   if (h->h_result) cudaFreeHost(h->h_result);
@@ -195,14 +197,15 @@ int alloc_step_buffers(arc_cache* h, uint32_t req_cap, uint64_t n_cap) {
   CUDA_TRY(h, dalloc(&h->d_keys, n_cap));
   CUDA_TRY(h, dalloc(&h->d_node_acc, n_cap));
   CUDA_TRY(h, dalloc(&h->d_dropped, n_cap));
-  CUDA_TRY(h, dalloc(&h->d_prefix_len, req_cap));
+  CUDA_TRY(h, dalloc(&h->d_result_pack, (size_t)req_cap + 2 + 2 * n_cap));
+  h->d_prefix_len = h->d_result_pack;
+  h->d_alloc_ids = h->d_result_pack + req_cap + 2;
+  h->d_evict_ids = h->d_alloc_ids + n_cap;
   CUDA_TRY(h, dalloc(&h->d_chain_state, req_cap));
   CUDA_TRY(h, dalloc(&h->d_cls, n_cap));
   CUDA_TRY(h, dalloc(&h->d_block_id, n_cap));
   CUDA_TRY(h, dalloc(&h->d_evicted_id, n_cap));
   CUDA_TRY(h, dalloc(&h->d_p_after, n_cap));
-  CUDA_TRY(h, dalloc(&h->d_alloc_ids, n_cap));
-  CUDA_TRY(h, dalloc(&h->d_evict_ids, n_cap));
   CUDA_TRY(h, cudaMallocHost((void**)&h->h_stage, (size_t)kStageSlots * 2 * ((size_t)req_cap + 1) * sizeof(int64_t)));
   CUDA_TRY(h, cudaMallocHost((void**)&h->h_result, ((size_t)req_cap + 2 + 2 * n_cap + 1) * sizeof(int32_t)));
   return ARC_OK;
@@ -505,16 +508,14 @@ int arc_step_host(arc_cache* h, const int32_t* h_tokens, const int64_t* h_offset
   int32_t* h_counts = hp + h->req_cap;
   int32_t* h_alloc = h_counts + 2;
   int32_t* h_evict = h_alloc + h->n_cap;
-  if (n_req) CUDA_TRY(h, cudaMemcpyAsync(hp, res.prefix_len, (size_t)n_req * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-  CUDA_TRY(h, cudaMemcpyAsync(h_counts, res.counts, 2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-  if (N) {
-    CUDA_TRY(h, cudaMemcpyAsync(h_alloc, res.alloc_ids, (size_t)N * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-    CUDA_TRY(h, cudaMemcpyAsync(h_evict, res.evict_ids, (size_t)N * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-  }
+  // one copy: the device side keeps prefix_len | counts | alloc_ids | evict_ids in one buffer laid out like h_result
+  CUDA_TRY(h, cudaMemcpyAsync(hp, h->d_result_pack, ((size_t)h->req_cap + 2 + (N ? h->n_cap + N : 0)) * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
   CUDA_TRY(h, cudaStreamSynchronize(s));
   out->n_access = N;
   out->n_alloc = (uint32_t)h_counts[0]; out->n_evict = (uint32_t)h_counts[1];
   out->prefix_len = hp; out->alloc_ids = h_alloc; out->evict_ids = h_evict;
+  out->h2d_bytes = (uint64_t)total * sizeof(int32_t) + 2 * ((uint64_t)h->req_cap + 1) * sizeof(int64_t);
+  out->d2h_bytes = ((uint64_t)h->req_cap + 2 + (N ? h->n_cap + N : 0)) * sizeof(int32_t);
   return ARC_OK;
 }
 
