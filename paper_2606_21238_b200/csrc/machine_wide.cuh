@@ -65,7 +65,6 @@ __device__ __forceinline__ uint32_t wide_count(const uint32_t (&mask)[WIDE_WARPS
 struct WideDecisions {
   uint32_t s0[WIDE_WARPS], s1[WIDE_WARPS], d1[WIDE_WARPS], d2[WIDE_WARPS], fm[WIDE_WARPS];
   int32_t my_p;
-  bool fast;                                 // the whole window took the all-miss steady-state path: every rank is the thread index
   Roll R;                                    // state after the window
 };
 
@@ -74,7 +73,6 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
                                           int warp, int lane) {
   D.R = roll_init(C);
   D.my_p = C.p;
-  D.fast = false;
   {
     // The commonest whole window of a cache in steady state: every access a miss, case 4A (t1 + b1 = c) with T1 above its
     // target and enough evictable entries for all of them: each miss drops B1's LRU ghost and evicts T1's LRU entry, no
@@ -91,7 +89,6 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
       }
       R.e1 -= k;
       R.phases++;
-      D.fast = true;
       return;
     }
   }
@@ -508,38 +505,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       dbg[DBG_ROLL_CALLS] += D.R.calls; dbg[DBG_ROLL_PHASES] += D.R.phases;
 
 
-      // ---- apply (threads < k)
-      uint32_t cntNH, cntEV, cntPT1, cntPT2, cntG1;
-      if (D.fast) {
-        // all-miss window in the steady state: access g takes T1's g-th live entry as its victim (it becomes a ghost at B1's
-        // MRU end), drops B1's g-th live ghost, and enters T1; every rank is the thread index
-        if (act) {
-          const uint4 v = S.vic[L_T1][tid], d = S.vic[L_B1][tid];
-          const int32_t blk = (int32_t)v.y;
-          const uint32_t qg = C.tail[L_B1] + (uint32_t)tid;
-          __stcg(P.ring[L_B1] + (qg & P.ring_mask), ring_ent(v.x, -1));
-          st_node_keep_slot(P.nodes + v.x, L_B1, qg, -1);
-          st_node_keep_slot(P.nodes + d.x, L_ABSENT, 0, -1);
-          if (hold) {
-            st_node(P.nodes + n, L_T1 | NODE_HELD, 1u, blk, rec.slot);
-            P.node_of_block[blk] = n;
-          } else {
-            const uint32_t q = C.tail[L_T1] + (uint32_t)tid;
-            __stcg(P.ring[L_T1] + (q & P.ring_mask), ring_ent(n, blk));
-            st_node(P.nodes + n, L_T1, q, blk, rec.slot);
-          }
-          const int64_t out = o + (nb - 1 - (j + tid));
-          P.cls[out] = (uint8_t)CLS_MISS;
-          P.block_id[out] = blk;
-          P.evicted_id[out] = blk;
-          P.p_after[out] = D.my_p;
-          P.dropped[a0 + tid] = d.x;
-          P.alloc_ids[C.n_alloc + (uint32_t)tid] = blk;
-          P.evict_ids[C.n_evict + (uint32_t)tid] = blk;
-        }
-        cntNH = cntEV = cntPT1 = cntG1 = (uint32_t)k; cntPT2 = 0;
-      } else {
-      // ranks come from the decision masks of all chunks
+      // ---- apply (threads < k); ranks come from the decision masks of all chunks
       uint32_t G1[WIDE_WARPS], PT1[WIDE_WARPS], PT2[WIDE_WARPS], NH[WIDE_WARPS], EV[WIDE_WARPS];
 #pragma unroll
       for (int u = 0; u < WIDE_WARPS; ++u) {
@@ -591,8 +557,6 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         if (!is_hit) P.alloc_ids[C.n_alloc + wide_rank(NH, lm)] = blk;
         if (ev >= 0) P.evict_ids[C.n_evict + wide_rank(EV, lm)] = ev;
       }
-      cntNH = wide_count(NH); cntEV = wide_count(EV); cntPT1 = wide_count(PT1); cntPT2 = wide_count(PT2); cntG1 = wide_count(G1);
-      }
       // class counts: every thread counts its own access, the warps add them up at the end of the kernel
       if (act) {
         my_cls[0] += (lst == L_ABSENT); my_cls[1] += (lst == L_T1); my_cls[2] += (lst == L_T2) && !lru;
@@ -605,8 +569,8 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       C.stat[ST_DROP_B1] += need[L_B1];
       C.stat[ST_DROP_B2] += need[L_B2];
       C.stat[ST_FRESH] += (uint32_t)(D.R.nf - C.next_fresh);
-      C.n_alloc += cntNH;
-      C.n_evict += cntEV;
+      C.n_alloc += wide_count(NH);
+      C.n_evict += wide_count(EV);
       if (spec_ok) {                                 // did this window take the speculated node as a victim or drop it?
 #pragma unroll
         for (int L = 1; L <= 4; ++L)
@@ -614,8 +578,8 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       }
 #pragma unroll
       for (int L = 1; L <= 4; ++L) C.head[L] = endpos[L];
-      if (!hold) { C.tail[L_T1] += cntPT1; C.tail[L_T2] += cntPT2; }
-      C.tail[L_B1] += cntG1;
+      if (!hold) { C.tail[L_T1] += wide_count(PT1); C.tail[L_T2] += wide_count(PT2); }
+      C.tail[L_B1] += wide_count(G1);
       C.tail[L_B2] += need[L_T2];
       C.t1 = D.R.t1; C.t2 = D.R.t2; C.b1 = D.R.b1; C.b2 = D.R.b2; C.p = D.R.p; C.next_fresh = D.R.nf;
       C.elig1 = D.R.e1; C.elig2 = D.R.e2;
