@@ -107,19 +107,38 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
         if (!lru) { const int32_t h1 = __popc(m0); R.t1 -= h1; R.t2 += h1; R.e2 -= __popc(me & m1); }
         R.e1 -= __popc(me & m0);
         R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = R.p;
-      } else if (absent == km || (!lru && (gb1 == km || gb2 == km))) {
-        // the chunk is one run of misses or of ghost hits: its phases are rolled here, without the call
+      } else {
+        // anything else: run after run, the phases inlined here (no call, no copy of the roll state); a chunk that is one
+        // run of misses or of ghost hits skips the run detection
         R.s0 = R.s1 = R.d1 = R.d2 = R.fm = 0; R.my_p = R.p;
-        const uint32_t li = (absent == km) ? L_ABSENT : ((gb1 == km) ? L_B1 : L_B2);
+        const bool pure = absent == km || (!lru && (gb1 == km || gb2 == km));
+        const uint32_t li_pure = (absent == km) ? L_ABSENT : ((gb1 == km) ? L_B1 : L_B2);
         const int my = (u == warp) ? lane : 64;
         for (int i = 0; i < ku;) {
           R.phases++;
-          i += (li == L_ABSENT) ? (lru ? phase_lru_miss(R, c, i, ku - i) : phase_miss(R, c, i, ku - i)) : phase_ghost(R, c, li, i, ku - i, my);
+          uint32_t li = li_pure;
+          int m = ku - i;
+          if (!pure) {
+            li = ((m0 >> i) & 1u) | (((m1 >> i) & 1u) << 1) | (((m2 >> i) & 1u) << 2);
+            // the run of accesses with this same list code (ARC: hits in T1 and in T2 form one run)
+            const bool hit_run = !lru && (li == L_T1 || li == L_T2);
+            const uint32_t same = (hit_run ? hits : (((li & 1u) ? m0 : ~m0) & ((li & 2u) ? m1 : ~m1) & ((li & 4u) ? m2 : ~m2))) & km;
+            const uint32_t brk = ~(same >> i);
+            m = brk ? (__ffs(brk) - 1) : 32;
+          }
+          int n;
+          if (li == L_T1 || (!lru && li == L_T2)) {             // hits: T1 entries move to T2 (ARC); evictable entries stop being so
+            n = m;
+            const uint32_t run = bits_from(i, n);
+            if (!lru) { const int32_t h1 = __popc(m0 & run); R.t1 -= h1; R.t2 += h1; R.e2 -= __popc(me & m1 & run); }
+            R.e1 -= __popc(me & m0 & run);
+          } else if (li == L_ABSENT || lru) {
+            n = lru ? phase_lru_miss(R, c, i, m) : phase_miss(R, c, i, m);
+          } else {
+            n = phase_ghost(R, c, li, i, m, my);
+          }
+          i += n;
         }
-      } else {
-        Roll T = D.R;                                // the callee is not inlined: keep D.R itself in registers
-        roll_chunk(T, c, lru, S.m[0][u], S.m[1][u], S.m[2][u], S.m[3][u], ku, (u == warp) ? lane : 64);
-        D.R = T;
       }
       D.s0[u] = D.R.s0; D.s1[u] = D.R.s1; D.d1[u] = D.R.d1; D.d2[u] = D.R.d2; D.fm[u] = D.R.fm;
       if (u == warp) D.my_p = D.R.my_p;
