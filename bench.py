@@ -445,11 +445,11 @@ def run_ours(args):
         line["dominant_kernel"] = {"kernel": "K3 ARC machine (arc_machine_wide_kernel, one CTA)", "share_of_step": sums.get("machine_ms", 0.0) / tot,
                                    "bound": "latency: dependent instructions of one serial state machine (DESIGN.md 7.3); neither HBM nor tensor nor ALU throughput",
                                    "ns_per_access": 1e6 * sums.get("machine_ms", 0.0) / max(1, n_acc),
-                                   "ncu": "profiles/r01e_held_resume_roll.md: about 44 warp instructions per access over 8 warps (39-53 on steps 15-17), 19 % issue-active per scheduler",
+                                   "ncu": "profiles/r01e_held_resume_roll.md: about 43 warp instructions per access over 8 warps (38-52 on steps 15-17), 19 % issue-active per scheduler",
                                    "issue_roofline": {"bound": "alu", "what": "warp-instruction issue of the ONE SM the machine runs on (4 schedulers x 1 instruction per clock)",
-                                                      "achieved": 44.0 * n_acc / max(sums.get("machine_ms", 0.0) * 1e-3, 1e-12), "unit": "warp instructions/s",
-                                                      "peak": 4 * 1.965e9, "frac": 44.0 * n_acc / max(sums.get("machine_ms", 0.0) * 1e-3, 1e-12) / (4 * 1.965e9),
-                                                      "instructions_per_access": "44, from the ncu capture named above (smsp__inst_executed.sum / accesses of that step)"}}
+                                                      "achieved": 43.0 * n_acc / max(sums.get("machine_ms", 0.0) * 1e-3, 1e-12), "unit": "warp instructions/s",
+                                                      "peak": 4 * 1.965e9, "frac": 43.0 * n_acc / max(sums.get("machine_ms", 0.0) * 1e-3, 1e-12) / (4 * 1.965e9),
+                                                      "instructions_per_access": "43, from the ncu capture named above (smsp__inst_executed.sum / accesses of that step)"}}
         k1_insitu = ALGO_BYTES_PER_BLOCK * n_acc / max(sums.get("hash_ms", 0.0) * 1e-3, 1e-12) / 1e9
         # K1 roofline: bulk run through arc_hash_blocks
         nb, nreq_b, mean_ms, best_ms = k1_bulk_roofline(torch, A, args.bulk_gib, stream, args.seed)
