@@ -2,7 +2,7 @@
 // accesses at a time.  Same equivalence argument as machine_batched.cuh; what changes is who does what:
 //   * thread g = 32 w + lane owns access g of the window: it fetches the node record, checks the window's cut
 //     conditions for its access, and applies its access;
-//   * the counter recurrence (roll_chunk, 32 accesses at a time) is run redundantly and identically by all four
+//   * the counter recurrence (wide_roll: 32 accesses at a time, phases inlined) is run redundantly and identically by all four
 //     warps on the class masks exchanged through shared memory, so no decision is ever broadcast;
 //   * warp w scans the LRU end of list w + 1 (T1, T2, B1, B2): 128 self-validating ring entries per round;
 //   * latencies (node fetch, ring fetch, barriers) are paid once per 128 accesses instead of once per 32.
