@@ -72,7 +72,7 @@ struct DevState {
                                   // collision inside one request, or the test hook); 0 between steps (K4 resets it)
   unsigned long long stat[ST_COUNT];
   // scratch for ring compaction (old window of the list being compacted)
-  uint32_t cmp_head, cmp_tail;
+  uint32_t cmp_head[5], cmp_tail[5];
   // K3 diagnostics, cumulative (arc_debug_counters): see DBG_* below
   unsigned long long dbg[32];
   // pin scope 2: entries of T1 / T2 without holds (= the entries in the rings = the possible victims), kept across steps

@@ -185,9 +185,15 @@ __global__ void __launch_bounds__(256) rebuild_table_kernel(DevState* st, Node* 
 // Ring compaction, two kernels.  The live entries of list L move, in order, to fresh positions
 // [old_tail, old_tail + live) of the *other* buffer: new positions never overlap old ones, so a stale
 // entry can never be mistaken for a live one while CTAs run concurrently.
+// blockIdx.y selects the list (L0 + blockIdx.y): all four lists are compacted by ONE pair of launches when the step-time
+// upkeep asks for it (their host-side bounds grow together, so they are due together).
 constexpr int CMP_THREADS = 1024;
-__global__ void __launch_bounds__(CMP_THREADS) ring_count_kernel(DevState* st, const Node* nodes, const RingEnt* ring,
-                                                                uint32_t ring_mask, uint32_t L, uint32_t* block_counts) {
+struct RingPtrs { const RingEnt* src[5]; RingEnt* dst[5]; };
+__global__ void __launch_bounds__(CMP_THREADS) ring_count_kernel(DevState* st, const Node* nodes, const RingPtrs rp,
+                                                                uint32_t ring_mask, uint32_t L0, uint32_t* block_counts_all) {
+  const uint32_t L = L0 + blockIdx.y;
+  const RingEnt* ring = rp.src[L];
+  uint32_t* block_counts = block_counts_all + (size_t)blockIdx.y * gridDim.x;
   const uint32_t head = st->head[L], tail = st->tail[L];
   const uint32_t window = tail - head;
   const uint32_t off = blockIdx.x * CMP_THREADS + threadIdx.x;
@@ -203,15 +209,19 @@ __global__ void __launch_bounds__(CMP_THREADS) ring_count_kernel(DevState* st, c
   const int cnt = __syncthreads_count(live);
   if (threadIdx.x == 0) {
     block_counts[blockIdx.x] = cnt;
-    if (blockIdx.x == 0) { st->cmp_head = head; st->cmp_tail = tail; }
+    if (blockIdx.x == 0) { st->cmp_head[L] = head; st->cmp_tail[L] = tail; }
   }
 }
-__global__ void __launch_bounds__(CMP_THREADS) ring_scatter_kernel(DevState* st, Node* nodes, const RingEnt* ring,
-                                                                  uint32_t ring_mask, RingEnt* ring_dst, uint32_t dst_mask,
-                                                                  uint32_t L, const uint32_t* block_counts) {
+__global__ void __launch_bounds__(CMP_THREADS) ring_scatter_kernel(DevState* st, Node* nodes, const RingPtrs rp,
+                                                                  uint32_t ring_mask, uint32_t dst_mask,
+                                                                  uint32_t L0, const uint32_t* block_counts_all) {
   __shared__ uint32_t s_warp[32];
   __shared__ uint32_t s_base, s_total;
-  const uint32_t head = st->cmp_head, tail = st->cmp_tail;
+  const uint32_t L = L0 + blockIdx.y;
+  const RingEnt* ring = rp.src[L];
+  RingEnt* ring_dst = rp.dst[L];
+  const uint32_t* block_counts = block_counts_all + (size_t)blockIdx.y * gridDim.x;
+  const uint32_t head = st->cmp_head[L], tail = st->cmp_tail[L];
   const uint32_t window = tail - head;
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   // exclusive prefix of block_counts up to this block (and the grand total in block 0)

@@ -167,16 +167,21 @@ int launch_rebuild(arc_cache* h, cudaStream_t s) {
   return ARC_OK;
 }
 
-// compacts list L from d_ring[L] (capacity src_cap) into d_ring_alt[L] (capacity dst_cap) and swaps
-int launch_compact(arc_cache* h, cudaStream_t s, int L, uint32_t src_cap, uint32_t dst_cap) {
+// compacts lists L .. L + n_lists - 1 from d_ring[] (capacity src_cap) into d_ring_alt[] (capacity dst_cap) and swaps them:
+// one pair of launches whatever n_lists is
+int launch_compact(arc_cache* h, cudaStream_t s, int L, uint32_t src_cap, uint32_t dst_cap, int n_lists = 1) {
   const uint32_t blocks = std::max<uint32_t>(1, src_cap / CMP_THREADS);
-  ring_count_kernel<<<blocks, CMP_THREADS, 0, s>>>(h->d_state, h->d_nodes, h->d_ring[L], src_cap - 1, (uint32_t)L, h->d_block_counts);
-  ring_scatter_kernel<<<blocks, CMP_THREADS, 0, s>>>(h->d_state, h->d_nodes, h->d_ring[L], src_cap - 1, h->d_ring_alt[L],
-                                                    dst_cap - 1, (uint32_t)L, h->d_block_counts);
+  RingPtrs rp;
+  for (int X = 0; X <= 4; ++X) { rp.src[X] = h->d_ring[X]; rp.dst[X] = h->d_ring_alt[X]; }
+  const dim3 grid(blocks, (unsigned)n_lists);
+  ring_count_kernel<<<grid, CMP_THREADS, 0, s>>>(h->d_state, h->d_nodes, rp, src_cap - 1, (uint32_t)L, h->d_block_counts);
+  ring_scatter_kernel<<<grid, CMP_THREADS, 0, s>>>(h->d_state, h->d_nodes, rp, src_cap - 1, dst_cap - 1, (uint32_t)L, h->d_block_counts);
   h->launches += 2;
   CUDA_TRY(h, cudaGetLastError());
-  std::swap(h->d_ring[L], h->d_ring_alt[L]);
-  h->window_bound[L] = std::min<uint64_t>(h->window_bound[L], h->c);
+  for (int X = L; X < L + n_lists; ++X) {
+    std::swap(h->d_ring[X], h->d_ring_alt[X]);
+    h->window_bound[X] = std::min<uint64_t>(h->window_bound[X], h->c);
+  }
   return ARC_OK;
 }
 
@@ -240,7 +245,7 @@ int ensure_capacity(arc_cache* h, uint32_t n_req, uint64_t N, cudaStream_t s) {
       CUDA_TRY(h, dalloc(&h->d_ring[L], ring_cap));
       CUDA_TRY(h, dalloc(&h->d_ring_alt[L], ring_cap));
     }
-    CUDA_TRY(h, dalloc(&h->d_block_counts, std::max<uint32_t>(1, ring_cap / CMP_THREADS)));
+    CUDA_TRY(h, dalloc(&h->d_block_counts, 4 * (size_t)std::max<uint32_t>(1, ring_cap / CMP_THREADS)));
     h->node_cap = node_cap; h->table_slots = table_slots; h->ring_cap = ring_cap;
     CUDA_TRY(h, cudaMemsetAsync(h->d_table, 0, (size_t)table_slots * sizeof(Slot), s));
     init_state_kernel<<<grid_for(node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, h->d_nodes, h->d_free_stack, node_cap, (h->policy == ARC_POLICY_DBL) ? (int32_t)(h->c / 2) : 0);
@@ -276,7 +281,7 @@ int ensure_capacity(arc_cache* h, uint32_t n_req, uint64_t N, cudaStream_t s) {
   }
   if (ring_cap > h->ring_cap) {
     dfree(h->d_block_counts);
-    CUDA_TRY(h, dalloc(&h->d_block_counts, std::max<uint32_t>(1, ring_cap / CMP_THREADS)));
+    CUDA_TRY(h, dalloc(&h->d_block_counts, 4 * (size_t)std::max<uint32_t>(1, ring_cap / CMP_THREADS)));
     for (int L = 1; L <= 4; ++L) {
       dfree(h->d_ring_alt[L]);
       CUDA_TRY(h, dalloc(&h->d_ring_alt[L], ring_cap));
@@ -297,11 +302,11 @@ int maintain(arc_cache* h, uint64_t N, cudaStream_t s) {
     int rc = launch_rebuild(h, s);
     if (rc) return rc;
   }
-  for (int L = 1; L <= 4; ++L) {
-    if (h->window_bound[L] + N > h->ring_cap) {
-      int rc = launch_compact(h, s, L, h->ring_cap, h->ring_cap);
-      if (rc) return rc;
-    }
+  bool due = false;
+  for (int L = 1; L <= 4; ++L) due = due || (h->window_bound[L] + N > h->ring_cap);
+  if (due) {                             // the bounds grow together: all four lists in one pair of launches
+    int rc = launch_compact(h, s, 1, h->ring_cap, h->ring_cap, 4);
+    if (rc) return rc;
   }
   return ARC_OK;
 }
