@@ -361,6 +361,14 @@ __global__ void __launch_bounds__(256) hash_fixup_kernel(const int64_t* __restri
   }
 }
 
+// Steps with up to K1_INLINE_REQ requests hand their offsets and block offsets to the device as a kernel argument: a launch
+// costs a few microseconds less than the copy engine's round trip, and the step's first kernel waits for them.
+constexpr uint32_t K1_INLINE_REQ = 253;
+struct OffsetsArg { long long v[2 * (K1_INLINE_REQ + 1)]; };       // offsets[n_req + 1] then blk_off[n_req + 1]: 4,064 bytes
+__global__ void __launch_bounds__(256) store_offsets_kernel(const __grid_constant__ OffsetsArg a, uint32_t n_req, int64_t* offsets, int64_t* blk_off) {
+  for (uint32_t i = threadIdx.x; i <= n_req; i += blockDim.x) { offsets[i] = a.v[i]; blk_off[i] = a.v[n_req + 1 + i]; }
+}
+
 // the last thing on the stream after a hashing launch: the ticket returns to 0 for the next launch
 __global__ void reset_ticket_kernel(uint32_t* ticket) { *ticket = 0; }
 

@@ -413,6 +413,13 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
   if (h->profiling) cudaEventRecord(h->ev[1], s);
 
   // host -> device boundary #1: offsets and block offsets (<= 16 MB at n_req = 2^20, usually a few KB)
+  if (n_req <= K1_INLINE_REQ) {          // small enough for a kernel argument: no copy-engine round trip, no staging
+    OffsetsArg a;
+    memcpy(a.v, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
+    memcpy(a.v + n_req + 1, blk_off.data(), ((size_t)n_req + 1) * sizeof(int64_t));
+    store_offsets_kernel<<<1, 256, 0, s>>>(a, n_req, h->d_offsets, h->d_offsets + (h->req_cap + 1));
+    h->launches += 1;
+  } else {
   const int slot = h->stage_next;
   h->stage_next = (slot + 1) % kStageSlots;
   CUDA_TRY(h, cudaEventSynchronize(h->stage_done[slot]));
@@ -421,6 +428,7 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
   memcpy(stage + (h->req_cap + 1), blk_off.data(), ((size_t)n_req + 1) * sizeof(int64_t));
   CUDA_TRY(h, cudaMemcpyAsync(h->d_offsets, stage, 2 * ((size_t)h->req_cap + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, s));
   CUDA_TRY(h, cudaEventRecord(h->stage_done[slot], s));
+  }
 
   StepParams P = make_params(h);
   P.tokens = d_tokens; P.n_req = n_req; P.n_access = (uint32_t)N;
@@ -519,7 +527,8 @@ int arc_step_host(arc_cache* h, const int32_t* h_tokens, const int64_t* h_offset
   out->n_access = N;
   out->n_alloc = (uint32_t)h_counts[0]; out->n_evict = (uint32_t)h_counts[1];
   out->prefix_len = hp; out->alloc_ids = h_alloc; out->evict_ids = h_evict;
-  out->h2d_bytes = (uint64_t)total * sizeof(int32_t) + 2 * ((uint64_t)h->req_cap + 1) * sizeof(int64_t);
+  out->h2d_bytes = (uint64_t)total * sizeof(int32_t) +
+                   2 * ((uint64_t)(n_req <= K1_INLINE_REQ ? n_req : h->req_cap) + 1) * sizeof(int64_t);   // offsets: kernel argument or staged copy
   out->d2h_bytes = ((uint64_t)h->req_cap + 2 + (N ? h->n_cap + N : 0)) * sizeof(int32_t);
   return ARC_OK;
 }
