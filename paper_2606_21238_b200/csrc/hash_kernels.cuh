@@ -239,14 +239,30 @@ __global__ void __launch_bounds__(256, 4) hash_blocks_kernel(const int32_t* __re
 // scanned independently from a zero carry (hash_segments_kernel: one warp per segment, the same loads and scans as
 // above) and put together afterwards (hash_fixup_kernel): with c_s the true state before segment s and E_s the local end
 // state of the segment, c_{s+1} = E_s + K^len_s c_s, and block i of the segment has state local_i + K^(i+1) c_s.
+// Steps with up to K1_INLINE_REQ requests hand their offsets and block offsets to the device as a kernel argument: a launch
+// costs a few microseconds less than the copy engine's round trip, and the step's first kernel waits for them.
+constexpr uint32_t K1_INLINE_REQ = 253;
+struct OffsetsArg { long long v[2 * (K1_INLINE_REQ + 1)]; };       // offsets[n_req + 1] then blk_off[n_req + 1]: 4,064 bytes
+__global__ void __launch_bounds__(256) store_offsets_kernel(const __grid_constant__ OffsetsArg a, uint32_t n_req, int64_t* offsets, int64_t* blk_off) {
+  for (uint32_t i = threadIdx.x; i <= n_req; i += blockDim.x) { offsets[i] = a.v[i]; blk_off[i] = a.v[n_req + 1 + i]; }
+}
+
 constexpr int K1_SEG = 128;
 
 // states[] gets the LOCAL states, in access order (index blk_off[r] + nb - 1 - i); seg_end[r * max_seg + s] = E_s.
-__global__ void __launch_bounds__(256, 4) hash_segments_kernel(const int32_t* __restrict__ tokens, const int64_t* __restrict__ offsets,
-                                                               const int64_t* __restrict__ blk_off, uint32_t n_req, uint32_t max_seg,
+// ARG = true: the offsets come as the kernel argument `arg` (steps of up to K1_INLINE_REQ requests) and CTA 0 also stores
+// them to offsets_g / blk_off_g for the kernels that follow; false: they are read from those arrays.
+template <bool ARG>
+__global__ void __launch_bounds__(256, 4) hash_segments_kernel(const int32_t* __restrict__ tokens, int64_t* __restrict__ offsets_g,
+                                                               int64_t* __restrict__ blk_off_g, uint32_t n_req, uint32_t max_seg,
                                                                unsigned long long* __restrict__ states,
-                                                               unsigned long long* __restrict__ seg_end, uint32_t* __restrict__ ticket) {
+                                                               unsigned long long* __restrict__ seg_end, uint32_t* __restrict__ ticket,
+                                                               const __grid_constant__ OffsetsArg arg) {
   const int lane = threadIdx.x & 31;
+  const long long* offsets = ARG ? arg.v : reinterpret_cast<const long long*>(offsets_g);
+  const long long* blk_off = ARG ? arg.v + (n_req + 1) : reinterpret_cast<const long long*>(blk_off_g);
+  if (ARG && blockIdx.x == 0)
+    for (uint32_t i = threadIdx.x; i <= n_req; i += blockDim.x) { offsets_g[i] = arg.v[i]; blk_off_g[i] = arg.v[n_req + 1 + i]; }
   const uint32_t* tok = reinterpret_cast<const uint32_t*>(tokens);
   const int64_t lo = offsets[0], hi = offsets[n_req];
   LaneConsts LC;
@@ -359,14 +375,6 @@ __global__ void __launch_bounds__(256) hash_fixup_kernel(const int64_t* __restri
       if (lane == 0) chain_out[r] = last;
     }
   }
-}
-
-// Steps with up to K1_INLINE_REQ requests hand their offsets and block offsets to the device as a kernel argument: a launch
-// costs a few microseconds less than the copy engine's round trip, and the step's first kernel waits for them.
-constexpr uint32_t K1_INLINE_REQ = 253;
-struct OffsetsArg { long long v[2 * (K1_INLINE_REQ + 1)]; };       // offsets[n_req + 1] then blk_off[n_req + 1]: 4,064 bytes
-__global__ void __launch_bounds__(256) store_offsets_kernel(const __grid_constant__ OffsetsArg a, uint32_t n_req, int64_t* offsets, int64_t* blk_off) {
-  for (uint32_t i = threadIdx.x; i <= n_req; i += blockDim.x) { offsets[i] = a.v[i]; blk_off[i] = a.v[n_req + 1 + i]; }
 }
 
 // the last thing on the stream after a hashing launch: the ticket returns to 0 for the next launch

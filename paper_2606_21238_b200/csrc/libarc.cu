@@ -413,12 +413,19 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
   if (h->profiling) cudaEventRecord(h->ev[1], s);
 
   // host -> device boundary #1: offsets and block offsets (<= 16 MB at n_req = 2^20, usually a few KB)
-  if (n_req <= K1_INLINE_REQ) {          // small enough for a kernel argument: no copy-engine round trip, no staging
-    OffsetsArg a;
-    memcpy(a.v, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
-    memcpy(a.v + n_req + 1, blk_off.data(), ((size_t)n_req + 1) * sizeof(int64_t));
-    store_offsets_kernel<<<1, 256, 0, s>>>(a, n_req, h->d_offsets, h->d_offsets + (h->req_cap + 1));
-    h->launches += 1;
+  uint64_t max_nb = 0;
+  for (uint32_t r = 0; r < n_req; ++r) max_nb = std::max<uint64_t>(max_nb, (uint64_t)(blk_off[r + 1] - blk_off[r]));
+  const uint32_t max_seg = (uint32_t)((max_nb + K1_SEG - 1) / K1_SEG);
+  const bool segmented = N && n_req <= kSegMaxReq && max_seg >= 2 && max_seg <= 1024 && (uint64_t)n_req * max_seg <= kSegEndCap;
+  static thread_local OffsetsArg off_arg;
+  const bool inline_off = n_req <= K1_INLINE_REQ;      // small enough for a kernel argument: no copy-engine round trip, no staging
+  if (inline_off) {
+    memcpy(off_arg.v, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
+    memcpy(off_arg.v + n_req + 1, blk_off.data(), ((size_t)n_req + 1) * sizeof(int64_t));
+    if (!segmented) {                                  // the segmented K1 takes the argument itself and stores the arrays
+      store_offsets_kernel<<<1, 256, 0, s>>>(off_arg, n_req, h->d_offsets, h->d_offsets + (h->req_cap + 1));
+      h->launches += 1;
+    }
   } else {
   const int slot = h->stage_next;
   h->stage_next = (slot + 1) % kStageSlots;
@@ -433,14 +440,13 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
   StepParams P = make_params(h);
   P.tokens = d_tokens; P.n_req = n_req; P.n_access = (uint32_t)N;
   if (N) {
-    uint64_t max_nb = 0;
-    for (uint32_t r = 0; r < n_req; ++r) max_nb = std::max<uint64_t>(max_nb, (uint64_t)(blk_off[r + 1] - blk_off[r]));
-    const uint32_t max_seg = (uint32_t)((max_nb + K1_SEG - 1) / K1_SEG);
-    if (n_req <= kSegMaxReq && max_seg >= 2 && max_seg <= 1024 && (uint64_t)n_req * max_seg <= kSegEndCap) {
+    if (segmented) {
       // K1, few long requests: segments hashed independently, then put together (hash_kernels.cuh)
       if (!h->d_seg_end) CUDA_TRY(h, dalloc(&h->d_seg_end, kSegEndCap));
-      hash_segments_kernel<<<grid_for((uint64_t)n_req * max_seg, 8, 148 * 4), 256, 0, s>>>(d_tokens, P.offsets, P.blk_off, n_req, max_seg, P.keys_acc,
-                                                                                           h->d_seg_end, &h->d_state->k1_ticket);
+      int64_t* d_off = h->d_offsets; int64_t* d_boff = h->d_offsets + (h->req_cap + 1);
+      const uint32_t g = grid_for((uint64_t)n_req * max_seg, 8, 148 * 4);
+      if (inline_off) hash_segments_kernel<true><<<g, 256, 0, s>>>(d_tokens, d_off, d_boff, n_req, max_seg, P.keys_acc, h->d_seg_end, &h->d_state->k1_ticket, off_arg);
+      else hash_segments_kernel<false><<<g, 256, 0, s>>>(d_tokens, d_off, d_boff, n_req, max_seg, P.keys_acc, h->d_seg_end, &h->d_state->k1_ticket, off_arg);
       hash_fixup_kernel<<<grid_for((uint64_t)n_req * max_seg, 8, 148 * 4), 256, 0, s>>>(P.blk_off, n_req, max_seg, P.keys_acc, h->d_seg_end,
                                                                     reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state);
       h->launches += 1;
