@@ -114,11 +114,15 @@ __global__ void __launch_bounds__(256) finalize_kernel(StepParams P) {
   for (uint32_t r = warp; r < P.n_req; r += n_warps) {
     const int64_t o = P.blk_off[r], nb = P.blk_off[r + 1] - o;
     int64_t lead = nb;
-    for (int64_t base = 0; base < nb; base += 32) {
-      const int64_t i = base + lane;
-      const int c = (i < nb) ? P.cls[o + i] : CLS_MISS;
-      const uint32_t nonhit = __ballot_sync(0xFFFFFFFFu, !(c == CLS_HIT_T1 || c == CLS_HIT_T2));
-      if (nonhit) { lead = base + (__ffs(nonhit) - 1); break; }
+    for (int64_t base = 0; base < nb && lead == nb; base += 128) {      // 128 classes per round trip: four independent loads per lane
+      int c[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) { const int64_t i = base + 32 * q + lane; c[q] = (i < nb) ? P.cls[o + i] : CLS_MISS; }
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const uint32_t nonhit = __ballot_sync(0xFFFFFFFFu, !(c[q] == CLS_HIT_T1 || c[q] == CLS_HIT_T2));
+        if (nonhit && lead == nb) lead = base + 32 * q + (__ffs(nonhit) - 1);
+      }
     }
     if (lead > nb) lead = nb;
     if (lane == 0) { P.prefix_len[r] = (int32_t)(lead * P.block_size); tokens_hit += (unsigned long long)lead * P.block_size; }
