@@ -198,8 +198,16 @@ int arc_set_machine(arc_cache *h, int which);
 /* K2 alone, for the probe microbenchmark and its tests: looks every key of d_keys (DEVICE uint64[n], values >= 2) up in
  * the handle's directory, inserting unknown keys as placeholder nodes exactly as arc_step's probe does, and writes the
  * node index of key i to d_nodes_out[i] (DEVICE uint32[n]).  Asynchronous on cuda_stream.  The placeholders are never
- * cleaned up (no K4 runs), so use a handle that is destroyed afterwards. */
+ * cleaned up (no K4 runs), so use a handle that is destroyed afterwards.  Since round 2 the probe is one thread per key
+ * reading one 32-byte bucket (two 16-byte slots) per probe, inserts publish key and node id with one 128-bit CAS. */
 int arc_debug_probe(arc_cache *h, const uint64_t *d_keys, uint64_t n, uint32_t *d_nodes_out, void *cuda_stream);
+
+/* Measurement aid: the random-sector ceiling K2 is compared with ("a measured random-sector ceiling").
+ * For every d_keys[i] (DEVICE uint64[n]) reads the 32-byte sector number (low 32 bits of the key) & (n_sectors - 1) of
+ * d_buf (DEVICE, 32-byte aligned, n_sectors * 32 bytes, n_sectors a power of two <= 2^32) with the load K2 uses and
+ * writes the XOR of its eight words to d_out[i] (DEVICE uint32[n]).  Same grid and loads as K2, no compare, no insert.
+ * Stateless; asynchronous on cuda_stream. */
+int arc_debug_gather_sectors(const uint64_t *d_keys, uint64_t n, const void *d_buf, uint64_t n_sectors, uint32_t *d_out, void *cuda_stream);
 
 /* Test hook: from the next step on every block key is ANDed with `mask` (results below 2 are bumped by 2) before the
  * directory probe, so that a test can force equal keys inside one request, which the 64-bit hash makes unobservable

@@ -27,7 +27,7 @@ STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", 
 EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats", "arc_reset", "arc_destroy",
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
            "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe", "arc_set_pin_scope",
-           "arc_release", "arc_hold_units", "arc_step_resume"]
+           "arc_release", "arc_hold_units", "arc_step_resume", "arc_debug_gather_sectors"]
 
 
 class ArcError(RuntimeError):
@@ -95,6 +95,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_hold_units.argtypes = [vp]
     L.arc_hold_units.restype = u64
     L.arc_debug_list.argtypes = [vp, C.c_int, vp, vp, u64, C.POINTER(u64)]
+    L.arc_debug_gather_sectors.argtypes = [vp, u64, vp, u64, vp, vp]
     if path is None:
         _lib = L
     return L
@@ -314,6 +315,20 @@ def hash_blocks(tokens, offsets, block_size: int = 16, out=None, stream=None):
     if out is None:
         out = torch.empty(n, dtype=torch.int64, device="cuda")
     rc = L.arc_hash_blocks(tokens.data_ptr(), o.ctypes.data, len(o) - 1, block_size, out.data_ptr(), _stream_ptr(stream))
+    if rc != OK:
+        raise ArcError(rc, L.arc_last_error(None).decode())
+    return out
+
+
+def debug_gather_sectors(keys, buf, out=None, stream=None):
+    """arc_debug_gather_sectors: the random-32-byte-sector read ceiling K2 is compared with.  keys: CUDA int64 tensor; buf: CUDA
+    tensor whose byte size is a power of two (>= 32); returns the CUDA int32 tensor of XORs."""
+    torch = _torch()
+    L = load_library()
+    n_sectors = buf.numel() * buf.element_size() // 32
+    if out is None:
+        out = torch.empty(keys.numel(), dtype=torch.int32, device="cuda")
+    rc = L.arc_debug_gather_sectors(keys.data_ptr(), keys.numel(), buf.data_ptr(), n_sectors, out.data_ptr(), _stream_ptr(stream))
     if rc != OK:
         raise ArcError(rc, L.arc_last_error(None).decode())
     return out

@@ -3,7 +3,7 @@
 // Directory layout in HBM:
 //   Node[node_cap]      16 B records {list, pos, block, slot}; node ids are stable for the life of a key
 //   node_key[node_cap]  the 64-bit key of each node (only needed by rebuilds and debug dumps)
-//   Slot[table_slots]   open-addressing table, 16 B slots {key, node}, buckets of 8 slots = one 128 B line
+//   Slot[table_slots]   open-addressing table, 16 B slots {key, node + 1}, buckets of 2 slots = one 32 B sector
 //   ring[L][ring_cap]   one lazy FIFO of 8 B entries {node id, block id} per list L in {T1, T2, B1, B2}: an entry at absolute
 //                       position q is *live* iff nodes[id].list == L && nodes[id].pos == q.  Every list
 //                       insertion is at the MRU end (tail++), every LRU-end removal scans from head and
@@ -18,14 +18,14 @@ namespace arc {
 
 constexpr uint32_t L_ABSENT = 0, L_T1 = 1, L_T2 = 2, L_B1 = 3, L_B2 = 4, L_FREE = 5;
 constexpr unsigned long long KEY_EMPTY = 0ull, KEY_TOMB = 1ull;  // H5 keeps real keys >= 2
-constexpr uint32_t SLOT_NODE_PENDING = 0;        // Slot::node holds node id + 1; 0 (what the table memset leaves) =
-                                                 // slot claimed by a key whose node id is not yet published
+constexpr uint32_t SLOT_NODE_PENDING = 0;        // Slot::node holds node id + 1; 0 = no node (EMPTY slot or tombstone).  Key and node
+                                                 // id are published together by one 128-bit CAS, so a live key always has its node
 constexpr uint32_t NODE_NONE = 0xFFFFFFFFu;
 constexpr uint32_t NODE_HELD = 0x100u;           // Node::list flag (pin scope 2): the node is resident, has holds and is in NO ring;
                                                  // Node::pos then carries the hold count instead of a ring position
 constexpr uint32_t NODE_LIST_MASK = 0xFFu;
-constexpr uint32_t SLOT_FLAG = 0x80000000u;      // node_acc entry holds a slot index to resolve, not a node id
-constexpr uint32_t BUCKET_SLOTS = 8;             // 8 x 16 B = one 128 B line
+constexpr uint32_t BUCKET_SLOTS = 2;             // 2 x 16 B = one 32 B sector: what one probe reads
+constexpr uint32_t K2_MAX_THREADS = 148 * 8 * 256;   // largest K2 grid: at most one unused node id per thread comes back (StepParams::spare)
 
 enum : int { CLS_MISS = 0, CLS_HIT_T1 = 1, CLS_HIT_T2 = 2, CLS_GHOST_B1 = 3, CLS_GHOST_B2 = 4 };
 enum : int { POLICY_ARC = 0, POLICY_LRU = 1, POLICY_DBL = 2 };
@@ -68,8 +68,7 @@ struct DevState {
   uint32_t error;                 // DEV_ERR_*
   uint32_t tombs;                 // tombstones currently in the table
   uint32_t k1_ticket;             // K1 work ticket: 0 between steps (K4 resets it)
-  uint32_t step_twins;            // set by K2 when some request of the step reaches the same node twice (a 64-bit key
-                                  // collision inside one request, or the test hook); 0 between steps (K4 resets it)
+  uint32_t n_spare;               // node ids K2 popped and did not use (lost slot races), listed in StepParams::spare; K4 pushes them back
   unsigned long long stat[ST_COUNT];
   // scratch for ring compaction (old window of the list being compacted)
   uint32_t cmp_head[5], cmp_tail[5];
@@ -116,9 +115,8 @@ struct StepParams {
   uint32_t block_size;
   int32_t pin_scope;              // 0: pins end with their request, 1: with the step, 2: held until arc_release
   uint32_t* node_of_block;        // pin scope 2: node id of the resident entry that owns each block id
-  uint32_t* node_stamp;           // [node_cap] K2: (step, request) tag of the last access that resolved to the node (twin check,
-                                  // bit 31 set); K3 wide machine: number of the last window that accessed the node (bit 31 clear)
-  uint32_t step_tag;              // 0x80000000 | (step & 0x7FF) << 20: ORed with the request index
+  uint32_t* node_stamp;           // [node_cap] K3 wide machine: number of the last window that accessed the node (twin check, speculation)
+  uint32_t* spare;                // [K2_MAX_THREADS] see DevState::n_spare
   uint32_t* counts_out;           // [2] copy of DevState::counts next to prefix_len / alloc_ids / evict_ids (one D2H copy in arc_step_host)
   unsigned long long key_and;     // test hook (arc_debug_set_key_mask): keys are ANDed with this before the probe; all ones normally
 };

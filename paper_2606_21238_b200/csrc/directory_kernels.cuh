@@ -8,93 +8,141 @@
 namespace arc {
 namespace cg = cooperative_groups;
 
-__device__ __forceinline__ Slot ld_slot(const Slot* p) {
-  uint4 v = __ldcg(reinterpret_cast<const uint4*>(p));   // L2: other CTAs CAS into this line during K2
-  Slot s;
-  s.key = (unsigned long long)v.x | ((unsigned long long)v.y << 32);
-  s.node = v.z; s.pad = v.w;
-  return s;
-}
-
 // ---------------------------------------------------------------------------------------------------
 // K2: for every key of the step find its node; if the key is not in the table, insert it and reserve a
 // node in state ABSENT, so that every access carries a node index into K3 and duplicates inside the
-// step share one node.  Warp-cooperative: a tile of 8 lanes probes one 128 B bucket
-// (8 slots x 16 B) per iteration with one coalesced load; the probe sequence is linear over buckets and
-// ends at the first bucket that still has a never-used (EMPTY) slot.  Inserts claim the lowest EMPTY
-// slot of that bucket with a 64-bit CAS on the key; a failed CAS re-reads the bucket, so two tiles
-// inserting the same key can never both succeed.  Tombstones are not reused;
-// rebuild_table clears them.
-__global__ void __launch_bounds__(256) probe_reserve_kernel(StepParams P) {
-  cg::thread_block_tile<8> tile = cg::tiled_partition<8>(cg::this_thread_block());
-  const uint32_t sub = tile.thread_rank();
-  const uint32_t tiles = (gridDim.x * blockDim.x) >> 3;
-  for (uint32_t a = (blockIdx.x * blockDim.x + threadIdx.x) >> 3; a < P.n_access; a += tiles) {
-    unsigned long long key = P.keys_acc[a] & P.key_and;
-    if (key < 2) key += 2;                       // 0 and 1 stay reserved under the test mask too
-    uint32_t bucket = (uint32_t)key & P.bucket_mask;
-    uint32_t result = NODE_NONE;
-    for (;;) {
-      const uint32_t idx = bucket * BUCKET_SLOTS + sub;
-      const Slot s = ld_slot(P.table + idx);
-      const uint32_t match = tile.ballot(s.key == key);
-      if (match) {
-        const int src = __ffs(match) - 1;
-        const uint32_t node = tile.shfl(s.node, src);
-        result = (node == SLOT_NODE_PENDING) ? (SLOT_FLAG | (bucket * BUCKET_SLOTS + src)) : node - 1;
-        break;
+// step share one node.
+//
+// Layout: buckets of BUCKET_SLOTS = 2 slots x 16 B = ONE 32-byte sector, the unit HBM and L2 move.  One thread owns one
+// key: it fetches the key's bucket with a single 256-bit load (LDG.256), compares both slots, and moves to the next
+// bucket only when this one is full of other keys (linear over buckets; the probe ends at the first bucket that still
+// has a never-used slot).  A probe therefore costs one sector = 32 B next to the 8 B of the key and the 4 B of the
+// node id: 44 B per key against 28 B algorithmic.  Each thread keeps PROBE_ILP keys in flight.
+//
+// Insert-if-absent: the lowest EMPTY slot of that bucket is claimed with ONE 128-bit compare-and-swap
+// (atom.cas.b128, sm_90+) that writes key and node id together, so a slot is never seen half-published: there is no
+// "claimed, node pending" state, no second pass and no spinning.  The node id is popped from the free stack before the
+// CAS; a thread that loses the race (another thread took the slot - possibly for the same key, which the re-read of
+// the bucket then finds) keeps the id for its next insert and hands a leftover to DevState::spare[], which K4 pushes
+// back (pushes never run concurrently with pops).  Tombstones are not reused; rebuild_table clears them.
+constexpr int PROBE_ILP = 4;
+
+struct Bucket { Slot s[BUCKET_SLOTS]; };
+__device__ __forceinline__ Bucket ld_bucket(const Slot* p) {          // p is 32-byte aligned
+  uint32_t r[8];
+  asm volatile("ld.global.cg.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "l"(p) : "memory");
+  Bucket b;
+  b.s[0].key = (unsigned long long)r[0] | ((unsigned long long)r[1] << 32); b.s[0].node = r[2]; b.s[0].pad = r[3];
+  b.s[1].key = (unsigned long long)r[4] | ((unsigned long long)r[5] << 32); b.s[1].node = r[6]; b.s[1].pad = r[7];
+  return b;
+}
+// {EMPTY, 0, 0} -> {key, node + 1, 0} in one atomic; true if this thread now owns the slot
+__device__ __forceinline__ bool slot_claim(Slot* p, unsigned long long key, uint32_t node_plus_1) {
+  unsigned long long ok, ov;
+  asm volatile("{\n\t.reg .b128 c, n, o;\n\tmov.b128 c, {%2, %3};\n\tmov.b128 n, {%4, %5};\n\t"
+               "atom.relaxed.gpu.global.cas.b128 o, [%6], c, n;\n\tmov.b128 {%0, %1}, o;\n\t}"
+               : "=l"(ok), "=l"(ov) : "l"(0ull), "l"(0ull), "l"(key), "l"((unsigned long long)node_plus_1), "l"(p) : "memory");
+  return ok == KEY_EMPTY && ov == 0ull;
+}
+
+// Finds or inserts `key`, starting with bucket content `b` already loaded for bucket index `bucket`.  `spare` is a node
+// id this thread popped earlier and did not use (NODE_NONE if none).  Returns the node id, or NODE_NONE when the node
+// pool is exhausted (sticky DEV_ERR_NODE_POOL: the step's results are void, K3 does not run).
+__device__ __forceinline__ uint32_t probe_one(const StepParams& P, unsigned long long key, uint32_t bucket, Bucket b, uint32_t& spare) {
+  for (;;) {
+    if (b.s[0].key == key) return b.s[0].node - 1;
+    if (b.s[1].key == key) return b.s[1].node - 1;
+    const int e = (b.s[0].key == KEY_EMPTY) ? 0 : ((b.s[1].key == KEY_EMPTY) ? 1 : -1);
+    if (e < 0) { bucket = (bucket + 1) & P.bucket_mask; b = ld_bucket(P.table + (size_t)bucket * BUCKET_SLOTS); continue; }
+    if (spare == NODE_NONE) {
+      const uint32_t top = atomicSub(&P.state->free_top, 1u);
+      if (top == 0 || top > 0x7FFFFFFFu) {
+        atomicAdd(&P.state->free_top, 1u);
+        atomicExch(&P.state->error, DEV_ERR_NODE_POOL);
+        return NODE_NONE;
       }
-      const uint32_t empty = tile.ballot(s.key == KEY_EMPTY);
-      if (!empty) { bucket = (bucket + 1) & P.bucket_mask; continue; }
-      const int src = __ffs(empty) - 1;
-      uint32_t got = NODE_NONE;
-      if ((int)sub == src) {
-        const unsigned long long old = atomicCAS(&P.table[idx].key, KEY_EMPTY, key);
-        if (old == KEY_EMPTY) {            // we own the slot: take a node and publish it
-          const uint32_t top = atomicSub(&P.state->free_top, 1u);
-          if (top == 0 || top > 0x7FFFFFFFu) {
-            atomicExch(&P.state->error, DEV_ERR_NODE_POOL);
-            got = 0;
-          } else {
-            got = P.free_stack[top - 1];
-            st_node(P.nodes + got, L_ABSENT, 0, -1, idx);
-            P.node_key[got] = key;
-          }
-          __stcg(&P.table[idx].node, got + 1);
-        }
-      }
-      got = tile.shfl(got, src);
-      if (got != NODE_NONE) { result = got; break; }
-      // lost the race for that slot: look at the bucket again (the winner may hold our key)
+      spare = P.free_stack[top - 1];
     }
-    if (sub == 0) P.node_acc[a] = result;
+    const uint32_t idx = bucket * BUCKET_SLOTS + (uint32_t)e;
+    st_node(P.nodes + spare, L_ABSENT, 0, -1, idx);        // read by K3 only, after the kernel boundary
+    P.node_key[spare] = key;
+    if (slot_claim(P.table + idx, key, spare + 1)) { const uint32_t got = spare; spare = NODE_NONE; return got; }
+    b = ld_bucket(P.table + (size_t)bucket * BUCKET_SLOTS);   // lost the race for that slot: the winner may hold our key
   }
 }
 
-// After K2: entries that raced with the winner of their key carry a slot index; the winner's node id is
-// visible now (kernel boundary).
-// Also K2's twin check: every access stamps its node with (step, request); finding one's own stamp already there means
-// the request reaches that node twice - possible only through a 64-bit key collision inside one request (or the test
-// hook that forces equal keys).  K3's wide machine pays for exact twin detection only in steps that carry the flag.
-__global__ void __launch_bounds__(256) resolve_nodes_kernel(StepParams P) {
-  for (uint32_t a = blockIdx.x * blockDim.x + threadIdx.x; a < P.n_access; a += gridDim.x * blockDim.x) {
-    uint32_t v = P.node_acc[a];
-    if (v != NODE_NONE && (v & SLOT_FLAG)) { v = __ldcg(&P.table[v & ~SLOT_FLAG].node) - 1; P.node_acc[a] = v; }
-    if (P.n_req == 0 || v == NODE_NONE) continue;          // arc_debug_probe: no requests
-    uint32_t lo = 0, hi = P.n_req;                          // request r with blk_off[r] <= a < blk_off[r+1]
-    while (hi - lo > 1) {
-      const uint32_t mid = (lo + hi) >> 1;
-      if (P.blk_off[mid] <= (int64_t)a) lo = mid; else hi = mid;
+__device__ __forceinline__ void probe_range(const StepParams& P, uint32_t first, uint32_t stride) {
+  uint32_t spare = NODE_NONE;
+  for (uint32_t a0 = first; a0 < P.n_access; a0 += stride * PROBE_ILP) {
+    unsigned long long key[PROBE_ILP];
+    uint32_t bucket[PROBE_ILP];
+    Bucket b[PROBE_ILP];
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) {
+      const uint32_t a = a0 + u * stride;
+      key[u] = (a < P.n_access) ? (__ldcg(P.keys_acc + a) & P.key_and) : 2ull;
+      if (key[u] < 2) key[u] += 2;                   // 0 and 1 stay reserved under the test mask too
+      bucket[u] = (uint32_t)key[u] & P.bucket_mask;
     }
-    const uint32_t tag = P.step_tag | lo;
-    if (atomicExch(&P.node_stamp[v], tag) == tag) P.state->step_twins = 1;
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) b[u] = ld_bucket(P.table + (size_t)bucket[u] * BUCKET_SLOTS);
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) {
+      const uint32_t a = a0 + u * stride;
+      if (a < P.n_access) P.node_acc[a] = probe_one(P, key[u], bucket[u], b[u], spare);
+    }
   }
+  if (spare != NODE_NONE) P.spare[atomicAdd(&P.state->n_spare, 1u)] = spare;     // at most one per thread: P.spare has K2_MAX_THREADS entries
+}
+
+__global__ void __launch_bounds__(256) probe_reserve_kernel(const __grid_constant__ StepParams P) {
+  probe_range(P, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+
+// The ceiling K2 is measured against (arc_debug_gather_sectors): the same grid, the same loads - an 8-byte key, the 32-byte
+// sector it selects, a 4-byte result - and nothing else (no compare, no insert).  What this kernel reaches is what random
+// 32-byte sector reads can reach on the machine.
+__global__ void __launch_bounds__(256) gather32_kernel(const unsigned long long* __restrict__ keys, uint32_t n, const Slot* __restrict__ buf,
+                                                       uint32_t sector_mask, uint32_t* __restrict__ out) {
+  const uint32_t first = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x;
+  for (uint32_t a0 = first; a0 < n; a0 += stride * PROBE_ILP) {
+    Bucket b[PROBE_ILP];
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) {
+      const uint32_t a = a0 + u * stride;
+      const unsigned long long key = (a < n) ? __ldcg(keys + a) : 0ull;
+      b[u] = ld_bucket(buf + (size_t)((uint32_t)key & sector_mask) * BUCKET_SLOTS);
+    }
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) {
+      const uint32_t a = a0 + u * stride;
+      if (a < n) out[a] = (uint32_t)b[u].s[0].key ^ (uint32_t)(b[u].s[0].key >> 32) ^ b[u].s[0].node ^ b[u].s[0].pad ^
+                          (uint32_t)b[u].s[1].key ^ (uint32_t)(b[u].s[1].key >> 32) ^ b[u].s[1].node ^ b[u].s[1].pad;
+    }
+  }
+}
+
+// Node ids that K2's threads popped and did not use go back on the free stack (no pop runs concurrently: K4, or the
+// tail of arc_debug_probe).
+__device__ __forceinline__ void return_spares(const StepParams& P, uint32_t tid, uint32_t nthr) {
+  const uint32_t n = P.state->n_spare;
+  for (uint32_t i = tid; i < n; i += nthr) {
+    const uint32_t d = P.spare[i];
+    st_node(P.nodes + d, L_FREE, 0, -1, 0);
+    P.free_stack[atomicAdd(&P.state->free_top, 1u)] = d;
+  }
+}
+__global__ void __launch_bounds__(256) return_spares_kernel(const __grid_constant__ StepParams P) {
+  return_spares(P, threadIdx.x, blockDim.x);
+  __syncthreads();
+  if (threadIdx.x == 0) P.state->n_spare = 0;
 }
 
 // ---------------------------------------------------------------------------------------------------
 // K4: (1) keys whose node ended the step ABSENT (dropped ghosts, evictions that leave no ghost) leave
 // the table and their nodes return to the free stack; (2) prefix_len[r] = B x leading hit blocks (R9).
-__global__ void __launch_bounds__(256) finalize_kernel(StepParams P) {
+__device__ __forceinline__ void finalize_body(const StepParams& P) {
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
   for (uint32_t a = tid; a < P.n_access; a += nthr) {
     const uint32_t d = P.dropped[a];
@@ -129,10 +177,17 @@ __global__ void __launch_bounds__(256) finalize_kernel(StepParams P) {
   }
   if (lane == 0 && tokens_hit) atomicAdd(&P.state->stat[ST_PREFIX_TOKENS], tokens_hit);
   if (tid == 0) {
-    P.state->k1_ticket = 0; P.state->step_twins = 0;                   // K1 of the next step starts from request 0
+    P.state->k1_ticket = 0;                                            // K1 of the next step starts from request 0
     P.counts_out[0] = P.state->counts[0]; P.counts_out[1] = P.state->counts[1];
   }
+  if (blockIdx.x == 0 && P.state->n_spare) {                           // CTA-uniform (nobody writes n_spare during K4 but this CTA)
+    return_spares(P, threadIdx.x, blockDim.x);
+    __syncthreads();
+    if (threadIdx.x == 0) P.state->n_spare = 0;
+  }
 }
+
+__global__ void __launch_bounds__(256) finalize_kernel(const __grid_constant__ StepParams P) { finalize_body(P); }
 
 // ---------------------------------------------------------------------------------------------------
 // Maintenance

@@ -69,7 +69,8 @@ struct arc_cache {
   Node* d_nodes = nullptr;
   unsigned long long* d_node_key = nullptr;
   uint32_t* d_free_stack = nullptr;
-  uint32_t* d_node_stamp = nullptr;   // [node_cap] K2's twin check
+  uint32_t* d_node_stamp = nullptr;   // [node_cap] K3 wide machine: window numbers (twin check, speculation)
+  uint32_t* d_spare = nullptr;        // [K2_MAX_THREADS] node ids K2 popped and did not use
   unsigned long long* d_seg_end = nullptr;   // [kSegEndCap] end states of K1's segments (steps with few, long requests)
   Slot* d_table = nullptr;
   RingEnt* d_ring[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -109,6 +110,7 @@ struct arc_cache {
   bool profiling = false;
   cudaEvent_t ev[7] = {};
   bool ev_valid = false;
+  bool poisoned = false;      // a growth step failed half way (see ensure_capacity): every later call fails
   std::string err;
 };
 
@@ -148,7 +150,7 @@ StepParams make_params(arc_cache* h) {
   P.node_of_block = h->d_node_of_block;
   P.node_stamp = h->d_node_stamp;
   P.counts_out = reinterpret_cast<uint32_t*>(h->d_result_pack + h->req_cap);
-  P.step_tag = 0x80000000u | (uint32_t)((h->steps & 0x7FFull) << 20);
+  P.spare = h->d_spare;
   return P;
 }
 
@@ -185,55 +187,87 @@ int launch_compact(arc_cache* h, cudaStream_t s, int L, uint32_t src_cap, uint32
   return ARC_OK;
 }
 
-void free_step_buffers(arc_cache* h) {
-  dfree(h->d_offsets); dfree(h->d_keys); dfree(h->d_node_acc); dfree(h->d_dropped);
-  dfree(h->d_result_pack); h->d_prefix_len = h->d_alloc_ids = h->d_evict_ids = nullptr;
-  dfree(h->d_chain_state); dfree(h->d_cls); dfree(h->d_block_id); dfree(h->d_evicted_id); dfree(h->d_p_after);
-  if (h->h_stage) cudaFreeHost(h->h_stage);
-  h->h_stage = nullptr;
-  if (h->h_result) cudaFreeHost(h->h_result);
-  h->h_result = nullptr;
+// The buffers whose size follows the largest step seen (req_cap requests, n_cap full blocks).
+struct StepBuffers {
+  int64_t* d_offsets = nullptr;
+  unsigned long long* d_keys = nullptr;
+  uint32_t* d_node_acc = nullptr;
+  uint32_t* d_dropped = nullptr;
+  int32_t* d_result_pack = nullptr;
+  unsigned long long* d_chain_state = nullptr;
+  uint8_t* d_cls = nullptr;
+  int32_t *d_block_id = nullptr, *d_evicted_id = nullptr, *d_p_after = nullptr;
+  int64_t* h_stage = nullptr;
+  int32_t* h_result = nullptr;
+};
+
+void free_step_buffers(StepBuffers& b) {
+  dfree(b.d_offsets); dfree(b.d_keys); dfree(b.d_node_acc); dfree(b.d_dropped); dfree(b.d_result_pack);
+  dfree(b.d_chain_state); dfree(b.d_cls); dfree(b.d_block_id); dfree(b.d_evicted_id); dfree(b.d_p_after);
+  if (b.h_stage) cudaFreeHost(b.h_stage);
+  b.h_stage = nullptr;
+  if (b.h_result) cudaFreeHost(b.h_result);
+  b.h_result = nullptr;
 }
 
-int alloc_step_buffers(arc_cache* h, uint32_t req_cap, uint64_t n_cap) {
-  free_step_buffers(h);
-  h->req_cap = req_cap; h->n_cap = n_cap;
-  CUDA_TRY(h, dalloc(&h->d_offsets, 2 * ((size_t)req_cap + 1)));
-  CUDA_TRY(h, dalloc(&h->d_keys, n_cap));
-  CUDA_TRY(h, dalloc(&h->d_node_acc, n_cap));
-  CUDA_TRY(h, dalloc(&h->d_dropped, n_cap));
-  CUDA_TRY(h, dalloc(&h->d_result_pack, (size_t)req_cap + 2 + 2 * n_cap));
-  h->d_prefix_len = h->d_result_pack;
-  h->d_alloc_ids = h->d_result_pack + req_cap + 2;
-  h->d_evict_ids = h->d_alloc_ids + n_cap;
-  CUDA_TRY(h, dalloc(&h->d_chain_state, req_cap));
-  CUDA_TRY(h, dalloc(&h->d_cls, n_cap));
-  CUDA_TRY(h, dalloc(&h->d_block_id, n_cap));
-  CUDA_TRY(h, dalloc(&h->d_evicted_id, n_cap));
-  CUDA_TRY(h, dalloc(&h->d_p_after, n_cap));
-  CUDA_TRY(h, cudaMallocHost((void**)&h->h_stage, (size_t)kStageSlots * 2 * ((size_t)req_cap + 1) * sizeof(int64_t)));
-  CUDA_TRY(h, cudaMallocHost((void**)&h->h_result, ((size_t)req_cap + 2 + 2 * n_cap + 1) * sizeof(int32_t)));
+int alloc_step_buffers(arc_cache* h, StepBuffers& b, uint32_t req_cap, uint64_t n_cap) {
+  CUDA_TRY(h, dalloc(&b.d_offsets, 2 * ((size_t)req_cap + 1)));
+  CUDA_TRY(h, dalloc(&b.d_keys, n_cap));
+  CUDA_TRY(h, dalloc(&b.d_node_acc, n_cap));
+  CUDA_TRY(h, dalloc(&b.d_dropped, n_cap));
+  CUDA_TRY(h, dalloc(&b.d_result_pack, (size_t)req_cap + 2 + 2 * n_cap));
+  CUDA_TRY(h, dalloc(&b.d_chain_state, req_cap));
+  CUDA_TRY(h, dalloc(&b.d_cls, n_cap));
+  CUDA_TRY(h, dalloc(&b.d_block_id, n_cap));
+  CUDA_TRY(h, dalloc(&b.d_evicted_id, n_cap));
+  CUDA_TRY(h, dalloc(&b.d_p_after, n_cap));
+  CUDA_TRY(h, cudaMallocHost((void**)&b.h_stage, (size_t)kStageSlots * 2 * ((size_t)req_cap + 1) * sizeof(int64_t)));
+  CUDA_TRY(h, cudaMallocHost((void**)&b.h_result, ((size_t)req_cap + 2 + 2 * n_cap + 1) * sizeof(int32_t)));
   return ARC_OK;
 }
 
-// Makes every buffer large enough for steps of (n_req, N).  Directory content is preserved.
+StepBuffers take_step_buffers(arc_cache* h) {
+  StepBuffers b;
+  b.d_offsets = h->d_offsets; b.d_keys = h->d_keys; b.d_node_acc = h->d_node_acc; b.d_dropped = h->d_dropped;
+  b.d_result_pack = h->d_result_pack; b.d_chain_state = h->d_chain_state; b.d_cls = h->d_cls; b.d_block_id = h->d_block_id;
+  b.d_evicted_id = h->d_evicted_id; b.d_p_after = h->d_p_after; b.h_stage = h->h_stage; b.h_result = h->h_result;
+  return b;
+}
+
+void install_step_buffers(arc_cache* h, const StepBuffers& b, uint32_t req_cap, uint64_t n_cap) {
+  h->d_offsets = b.d_offsets; h->d_keys = b.d_keys; h->d_node_acc = b.d_node_acc; h->d_dropped = b.d_dropped;
+  h->d_result_pack = b.d_result_pack; h->d_chain_state = b.d_chain_state; h->d_cls = b.d_cls; h->d_block_id = b.d_block_id;
+  h->d_evicted_id = b.d_evicted_id; h->d_p_after = b.d_p_after; h->h_stage = b.h_stage; h->h_result = b.h_result;
+  h->d_prefix_len = b.d_result_pack;
+  h->d_alloc_ids = b.d_result_pack ? b.d_result_pack + req_cap + 2 : nullptr;
+  h->d_evict_ids = b.d_result_pack ? h->d_alloc_ids + n_cap : nullptr;
+  h->req_cap = req_cap; h->n_cap = n_cap;
+}
+
+// Makes every buffer large enough for steps of (n_req, N).  Directory content is preserved.  Transactional towards the
+// caller: every part (node pool, table, rings, step buffers) is grown into new memory and committed only when it is
+// complete, and the sizes a step is checked against (req_cap, n_cap) are committed LAST, so a failure (out of memory,
+// the 30-bit node index) leaves a handle that works as before and simply tries again on the next larger step.  The one
+// failure that cannot be undone (a launch error while the rings move) poisons the handle: every later call fails.
 int ensure_capacity(arc_cache* h, uint32_t n_req, uint64_t N, cudaStream_t s) {
+  if (h->poisoned) return fail(h, ARC_ERR_CUDA, "the handle is unusable after an earlier CUDA failure during growth");
   if (n_req <= h->req_cap && N <= h->n_cap && h->d_state) return ARC_OK;
   const bool first = (h->d_state == nullptr);
-  if (!first) CUDA_TRY(h, cudaDeviceSynchronize());   // results of earlier steps die here (documented)
   const uint32_t req_cap = std::max<uint32_t>(first ? 64 : h->req_cap, pow2_at_least(n_req));
   uint64_t n_cap = std::max<uint64_t>(first ? 4096 : h->n_cap, N);
   if (!first && N > h->n_cap) n_cap = std::max<uint64_t>(n_cap, h->n_cap * 2);
-  int rc = alloc_step_buffers(h, req_cap, n_cap);
-  if (rc) return rc;
-
   const uint64_t node_cap64 = 2 * h->c + n_cap + 64;
   if (node_cap64 >= (1ull << 30)) return fail(h, ARC_ERR_UNSUPPORTED, "directory of %llu nodes exceeds the 30-bit node index", (unsigned long long)node_cap64);
   const uint32_t node_cap = (uint32_t)node_cap64;
   const uint32_t table_slots = pow2_at_least(2 * node_cap64);
   const uint32_t ring_cap = pow2_at_least(2 * (h->c + n_cap));
+  if (!first) CUDA_TRY(h, cudaDeviceSynchronize());   // results of earlier steps die here (documented)
 
   if (first) {
+    StepBuffers nb;
+    int rc = alloc_step_buffers(h, nb, req_cap, n_cap);
+    if (rc) { free_step_buffers(nb); return rc; }
+    install_step_buffers(h, nb, req_cap, n_cap);     // arc_create destroys the handle if anything below fails
     CUDA_TRY(h, dalloc(&h->d_state, 1));
     CUDA_TRY(h, dalloc(&h->d_nodes, node_cap));
     CUDA_TRY(h, dalloc(&h->d_node_key, node_cap));
@@ -241,6 +275,7 @@ int ensure_capacity(arc_cache* h, uint32_t n_req, uint64_t N, cudaStream_t s) {
     CUDA_TRY(h, dalloc(&h->d_node_stamp, node_cap));
     CUDA_TRY(h, cudaMemsetAsync(h->d_node_stamp, 0, (size_t)node_cap * sizeof(uint32_t), s));
     CUDA_TRY(h, dalloc(&h->d_table, table_slots));
+    CUDA_TRY(h, dalloc(&h->d_spare, K2_MAX_THREADS));
     for (int L = 1; L <= 4; ++L) {
       CUDA_TRY(h, dalloc(&h->d_ring[L], ring_cap));
       CUDA_TRY(h, dalloc(&h->d_ring_alt[L], ring_cap));
@@ -256,49 +291,93 @@ int ensure_capacity(arc_cache* h, uint32_t n_req, uint64_t N, cudaStream_t s) {
     return ARC_OK;
   }
 
-  if (node_cap > h->node_cap) {       // grow the node pool; ids are stable
-    Node* nodes; unsigned long long* keys; uint32_t* stack;
-    CUDA_TRY(h, dalloc(&nodes, node_cap));
-    CUDA_TRY(h, dalloc(&keys, node_cap));
-    CUDA_TRY(h, dalloc(&stack, node_cap));
-    CUDA_TRY(h, cudaMemcpyAsync(nodes, h->d_nodes, (size_t)h->node_cap * sizeof(Node), cudaMemcpyDeviceToDevice, s));
-    CUDA_TRY(h, cudaMemcpyAsync(keys, h->d_node_key, (size_t)h->node_cap * sizeof(unsigned long long), cudaMemcpyDeviceToDevice, s));
-    extend_free_stack_kernel<<<grid_for(node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, nodes, h->d_free_stack, stack, h->node_cap, node_cap);
-    bump_free_top_kernel<<<1, 1, 0, s>>>(h->d_state, node_cap - h->node_cap);
-    h->launches += 2;
-    CUDA_TRY(h, cudaStreamSynchronize(s));
-    dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_node_stamp);
-    CUDA_TRY(h, dalloc(&h->d_node_stamp, node_cap));       // stamps only matter inside a step: start again from zero
-    CUDA_TRY(h, cudaMemsetAsync(h->d_node_stamp, 0, (size_t)node_cap * sizeof(uint32_t), s));
-    h->d_nodes = nodes; h->d_node_key = keys; h->d_free_stack = stack; h->node_cap = node_cap;
-  }
-  if (table_slots > h->table_slots) {
-    dfree(h->d_table);
-    CUDA_TRY(h, dalloc(&h->d_table, table_slots));
-    h->table_slots = table_slots;
-    rc = launch_rebuild(h, s);
-    if (rc) return rc;
-  }
-  if (ring_cap > h->ring_cap) {
-    dfree(h->d_block_counts);
-    CUDA_TRY(h, dalloc(&h->d_block_counts, 4 * (size_t)std::max<uint32_t>(1, ring_cap / CMP_THREADS)));
-    for (int L = 1; L <= 4; ++L) {
-      dfree(h->d_ring_alt[L]);
-      CUDA_TRY(h, dalloc(&h->d_ring_alt[L], ring_cap));
-      rc = launch_compact(h, s, L, h->ring_cap, ring_cap);   // swaps: d_ring[L] is now the big one
-      if (rc) return rc;
-      CUDA_TRY(h, cudaStreamSynchronize(s));
-      dfree(h->d_ring_alt[L]);
-      CUDA_TRY(h, dalloc(&h->d_ring_alt[L], ring_cap));
+  // (1) the new step buffers, kept aside until everything else has grown
+  StepBuffers nb;
+  int rc = alloc_step_buffers(h, nb, req_cap, n_cap);
+  if (rc) { free_step_buffers(nb); return rc; }
+
+  if (node_cap > h->node_cap) {       // (2) the node pool; ids are stable
+    Node* nodes = nullptr; unsigned long long* keys = nullptr; uint32_t* stack = nullptr; uint32_t* stamp = nullptr;
+    cudaError_t e = dalloc(&nodes, node_cap);
+    if (e == cudaSuccess) e = dalloc(&keys, node_cap);
+    if (e == cudaSuccess) e = dalloc(&stack, node_cap);
+    if (e == cudaSuccess) e = dalloc(&stamp, node_cap);
+    if (e != cudaSuccess) {
+      dfree(nodes); dfree(keys); dfree(stack); dfree(stamp); free_step_buffers(nb);
+      cudaGetLastError();
+      return fail(h, ARC_ERR_OOM, "growing the node pool to %u nodes: %s", node_cap, cudaGetErrorString(e));
     }
+    e = cudaMemcpyAsync(nodes, h->d_nodes, (size_t)h->node_cap * sizeof(Node), cudaMemcpyDeviceToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(keys, h->d_node_key, (size_t)h->node_cap * sizeof(unsigned long long), cudaMemcpyDeviceToDevice, s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(stamp, 0, (size_t)node_cap * sizeof(uint32_t), s);   // stamps only matter inside a step
+    if (e == cudaSuccess) {
+      // the new stack is built from the old one without touching it; DevState::free_top moves only when all of it worked
+      extend_free_stack_kernel<<<grid_for(node_cap, 256, 148 * 8), 256, 0, s>>>(h->d_state, nodes, h->d_free_stack, stack, h->node_cap, node_cap);
+      h->launches += 1;
+      e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) {
+      dfree(nodes); dfree(keys); dfree(stack); dfree(stamp); free_step_buffers(nb);
+      return fail(h, ARC_ERR_CUDA, "growing the node pool: %s", cudaGetErrorString(e));
+    }
+    bump_free_top_kernel<<<1, 1, 0, s>>>(h->d_state, node_cap - h->node_cap);
+    h->launches += 1;
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) {           // the old pool is still whole and still the handle's
+      dfree(nodes); dfree(keys); dfree(stack); dfree(stamp); free_step_buffers(nb);
+      return fail(h, ARC_ERR_CUDA, "growing the node pool: %s", cudaGetErrorString(e));
+    }
+    dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_node_stamp);
+    h->d_nodes = nodes; h->d_node_key = keys; h->d_free_stack = stack; h->d_node_stamp = stamp; h->node_cap = node_cap;
+  }
+  if (table_slots > h->table_slots) {  // (3) the table: rebuilt from the node records into new memory
+    Slot* table = nullptr;
+    cudaError_t e = dalloc(&table, table_slots);
+    if (e != cudaSuccess) {
+      free_step_buffers(nb);
+      cudaGetLastError();
+      return fail(h, ARC_ERR_OOM, "growing the table to %u slots: %s", table_slots, cudaGetErrorString(e));
+    }
+    Slot* old = h->d_table; const uint32_t old_slots = h->table_slots;
+    h->d_table = table; h->table_slots = table_slots;
+    rc = launch_rebuild(h, s);          // writes the nodes' slot fields: from here on only the new table is valid
+    if (rc == ARC_OK && cudaStreamSynchronize(s) != cudaSuccess) rc = fail(h, ARC_ERR_CUDA, "rebuilding the table failed");
+    if (rc) { (void)old_slots; dfree(old); free_step_buffers(nb); h->poisoned = true; return rc; }
+    dfree(old);
+  }
+  if (ring_cap > h->ring_cap) {        // (4) the four rings: all eight new buffers first, then one compaction moves the lists
+    RingEnt* nr[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    RingEnt* na[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    uint32_t* counts = nullptr;
+    cudaError_t e = dalloc(&counts, 4 * (size_t)std::max<uint32_t>(1, ring_cap / CMP_THREADS));
+    for (int L = 1; L <= 4 && e == cudaSuccess; ++L) { e = dalloc(&nr[L], ring_cap); if (e == cudaSuccess) e = dalloc(&na[L], ring_cap); }
+    if (e != cudaSuccess) {
+      for (int L = 1; L <= 4; ++L) { dfree(nr[L]); dfree(na[L]); }
+      dfree(counts); free_step_buffers(nb);
+      cudaGetLastError();
+      return fail(h, ARC_ERR_OOM, "growing the rings to %u entries: %s", ring_cap, cudaGetErrorString(e));
+    }
+    dfree(h->d_block_counts); h->d_block_counts = counts;
+    for (int L = 1; L <= 4; ++L) { dfree(h->d_ring_alt[L]); h->d_ring_alt[L] = nr[L]; }
+    rc = launch_compact(h, s, 1, h->ring_cap, ring_cap, 4);   // swaps: d_ring[] are the big ones now, d_ring_alt[] the old small ones
+    if (rc == ARC_OK && cudaStreamSynchronize(s) != cudaSuccess) rc = fail(h, ARC_ERR_CUDA, "moving the rings failed");
+    if (rc) { for (int L = 1; L <= 4; ++L) dfree(na[L]); free_step_buffers(nb); h->poisoned = true; return rc; }
+    for (int L = 1; L <= 4; ++L) { dfree(h->d_ring_alt[L]); h->d_ring_alt[L] = na[L]; }
     h->ring_cap = ring_cap;
   }
+  // (5) commit: the step buffers and, last of all, the sizes steps are checked against
+  StepBuffers old = take_step_buffers(h);
+  free_step_buffers(old);
+  install_step_buffers(h, nb, req_cap, n_cap);
   return ARC_OK;
 }
 
 // Directory upkeep before a step of N accesses, decided from host-side upper bounds only.
 int maintain(arc_cache* h, uint64_t N, cudaStream_t s) {
-  if (h->slots_used_bound + N > (uint64_t)(0.70 * h->table_slots)) {
+  // buckets are one 32-byte sector = 2 slots: beyond a load of about 0.45 (live keys + tombstones) the probe chains grow
+  if (h->slots_used_bound + N > (uint64_t)(0.45 * h->table_slots)) {
     int rc = launch_rebuild(h, s);
     if (rc) return rc;
   }
@@ -455,9 +534,8 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
                   reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state);
     }
     if (h->profiling) cudaEventRecord(h->ev[2], s);
-    probe_reserve_kernel<<<grid_for(N, 32, 148 * 8), 256, 0, s>>>(P);                                     // K2
-    resolve_nodes_kernel<<<grid_for(N, 256, 148 * 8), 256, 0, s>>>(P);
-    h->launches += 3;
+    probe_reserve_kernel<<<grid_for(N, 256 * PROBE_ILP, 148 * 8), 256, 0, s>>>(P);                        // K2
+    h->launches += 2;
   } else {
     // no full block anywhere: every request keeps the state it came with
     if (n_req) {
@@ -582,8 +660,8 @@ int arc_reset(arc_cache* h) {
 void arc_destroy(arc_cache* h) {
   if (!h) return;
   cudaDeviceSynchronize();
-  free_step_buffers(h);
-  dfree(h->d_state); dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_table); dfree(h->d_node_stamp);
+  { StepBuffers b = take_step_buffers(h); free_step_buffers(b); }
+  dfree(h->d_state); dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_table); dfree(h->d_node_stamp); dfree(h->d_spare);
   for (int L = 1; L <= 4; ++L) { dfree(h->d_ring[L]); dfree(h->d_ring_alt[L]); }
   dfree(h->d_block_counts); dfree(h->d_tokens_stage); dfree(h->d_machine_scratch);
   dfree(h->d_node_of_block); dfree(h->d_rel_cnt); dfree(h->d_seg_end);
@@ -725,14 +803,27 @@ int arc_debug_probe(arc_cache* h, const uint64_t* d_keys, uint64_t n, uint32_t* 
   P.node_acc = d_nodes_out;
   P.n_access = (uint32_t)n; P.n_req = 0;
   if (n) {
-    probe_reserve_kernel<<<grid_for(n, 32, 148 * 8), 256, 0, s>>>(P);
-    resolve_nodes_kernel<<<grid_for(n, 256, 148 * 8), 256, 0, s>>>(P);
+    probe_reserve_kernel<<<grid_for(n, 256 * PROBE_ILP, 148 * 8), 256, 0, s>>>(P);
+    return_spares_kernel<<<1, 256, 0, s>>>(P);
     h->launches += 2;
   }
   CUDA_TRY(h, cudaGetLastError());
   // every used slot belongs to a node and this entry creates no tombstones
   h->slots_used_bound = std::min<uint64_t>(h->slots_used_bound + n, h->node_cap);
   h->last_stream = s;
+  return ARC_OK;
+}
+
+int arc_debug_gather_sectors(const uint64_t* d_keys, uint64_t n, const void* d_buf, uint64_t n_sectors, uint32_t* d_out, void* cuda_stream) {
+  if (n && (!d_keys || !d_buf || !d_out)) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
+  if (n >= (1ull << 31) || n_sectors == 0 || (n_sectors & (n_sectors - 1)) || n_sectors > (1ull << 32)) return fail(nullptr, ARC_ERR_INVALID_ARG, "n or n_sectors out of range");
+  if (reinterpret_cast<uintptr_t>(d_buf) & 31) return fail(nullptr, ARC_ERR_INVALID_ARG, "d_buf must be 32-byte aligned");
+  if (n) {
+    gather32_kernel<<<grid_for(n, 256 * PROBE_ILP, 148 * 8), 256, 0, (cudaStream_t)cuda_stream>>>(
+        reinterpret_cast<const unsigned long long*>(d_keys), (uint32_t)n, reinterpret_cast<const Slot*>(d_buf), (uint32_t)(n_sectors - 1), d_out);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "gather launch: %s", cudaGetErrorString(e));
+  }
   return ARC_OK;
 }
 

@@ -260,6 +260,7 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
   const bool hold = (P.pin_scope == 2);
   const int32_t c = P.capacity;
   const int64_t N = (int64_t)P.n_access;
+  if (P.state->error == DEV_ERR_NODE_POOL) return;       // K2 could not give every key a node: the step is void (sticky error)
   SerialCtx C;            // identical in every lane
   ctx_load(C, P);
   unsigned long long dbg[DBG_COUNT];

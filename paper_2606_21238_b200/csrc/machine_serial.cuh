@@ -139,8 +139,7 @@ __device__ __forceinline__ void ring_tomb(const StepParams& P, uint32_t list, ui
 // (natural order).  C.bound[T1/T2] must hold the tails recorded when the access's request began (R4).
 __device__ __noinline__ void serial_access(SerialCtx& C, const StepParams& P, int64_t a, int64_t out) {
   const int32_t c = P.capacity;
-  uint32_t n = P.node_acc[a];
-  if (n & SLOT_FLAG) n = __ldcg(&P.table[n & ~SLOT_FLAG].node) - 1;
+  const uint32_t n = P.node_acc[a];
   Node rec = ld_node(P.nodes + n);
   const bool held = (rec.list & NODE_HELD) != 0;             // pin scope 2 only: resident, in no ring, rec.pos = holds
   const uint32_t holds = held ? rec.pos : 0u;
@@ -212,6 +211,7 @@ __device__ __noinline__ void serial_access(SerialCtx& C, const StepParams& P, in
 
 __global__ void arc_machine_serial_kernel(const __grid_constant__ StepParams P) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  if (P.state->error == DEV_ERR_NODE_POOL) return;       // K2 could not give every key a node: the step is void (sticky error)
   SerialCtx C;
   ctx_load(C, P);
   for (uint32_t r = 0; r < P.n_req; ++r) {

@@ -7,9 +7,11 @@
 //   * warp w scans the LRU end of list w + 1 (T1, T2, B1, B2): 128 self-validating ring entries per round;
 //   * latencies (node fetch, ring fetch, barriers) are paid once per 128 accesses instead of once per 32.
 // The same node twice in a window is possible only through a 64-bit key collision inside one request (windows never
-// cross a request boundary).  K2 flags the steps in which some request reaches a node twice (DevState::step_twins); only
-// in those steps are twins looked for, exactly, with a 512-slot shared-memory hash set, and the window cut before the
-// second occurrence as in the 32-wide machine.  In all other steps the set is never touched.
+// cross a request boundary).  It is found exactly and for free: every owner stamps its node with the window's number by
+// an atomic EXCHANGE (node_stamp[]; normally one window ahead, together with the speculative record load, so the
+// latency is hidden); two threads of one window that own the same node exchange the same number, and whichever comes
+// second in the atomic's order reads it back.  Only then (next to never) does the window compare its node ids pairwise
+// and cut itself before the second occurrence, as the 32-wide machine does with __match_any_sync.
 #pragma once
 #include "machine_batched.cuh"
 
@@ -17,7 +19,6 @@ namespace arc {
 
 constexpr int WIDE_WARPS = 4;
 constexpr int WIDE_W = 32 * WIDE_WARPS;      // accesses per window
-constexpr int WIDE_SET = 512;                // slots of the twin-detection hash set
 constexpr int WIDE_IDS = 512;                // node-id staging ring: the current window, the next one and what is in flight
 
 __device__ __forceinline__ void cp_async_u32(uint32_t* smem_dst, const uint32_t* gmem_src) {
@@ -29,12 +30,11 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 struct WideShared {
   uint32_t m[4][WIDE_WARPS];                 // m0, m1, m2, me per chunk
   uint32_t bad[WIDE_WARPS];
-  uint32_t twin[WIDE_WARPS];
+  uint32_t twin[WIDE_WARPS], twinc[WIDE_WARPS];   // accesses that repeat an earlier node of the window; threads whose stamp exchange says "maybe"
+  uint32_t twin_k;                           // the window's size after a twin cut (written between the two twin barriers only)
   uint32_t found[5], more[5], need[5];       // scanners: live entries found so far, whether the list has more to scan; owners: victims needed
   uint32_t ctl_done, ctl_k, ctl_head[5], ctl_limit[5]; // published by thread 0 before a window's first barrier, read by the scanner warps
-  uint32_t ctl_twins;                        // the step carries K2's twin flag: no barrier of the sequence is ever skipped
   uint32_t red[WIDE_WARPS][5];               // per-warp class counts, summed by thread 0 at the end
-  uint32_t set_id[WIDE_SET], set_min[WIDE_SET];
   uint32_t ids[WIDE_IDS];                    // node ids of the upcoming accesses: access a sits in ids[a % WIDE_IDS] (filled by cp.async)
   uint4 vic[5][WIDE_W];                      // per list: entries found from the LRU end {node, block, -, position}
   SerialCtx ctx;                             // the machine state after a by-the-book access done by warp 0
@@ -61,6 +61,9 @@ __device__ __forceinline__ uint32_t wide_count(const uint32_t (&mask)[WIDE_WARPS
   for (int u = 0; u < WIDE_WARPS; ++u) r += (uint32_t)__popc(mask[u]);
   return r;
 }
+
+// window numbers: 31 bits, never 0 (0 = never stamped)
+__device__ __forceinline__ uint32_t wide_next_seq(uint32_t s) { s = (s + 1u) & 0x7FFFFFFFu; return s ? s : 1u; }
 
 struct WideDecisions {
   uint32_t s0[WIDE_WARPS], s1[WIDE_WARPS], d1[WIDE_WARPS], d2[WIDE_WARPS], fm[WIDE_WARPS];
@@ -180,7 +183,7 @@ __device__ __forceinline__ uint32_t wide_scan_round(const ScanRegs& regs, uint32
 // Scanner warp for list L (warps 4..7 of the CTA): follows the owners' barrier sequence window by window.  The first
 // 128 entries from the list head are scanned while the owners fetch node records and roll the counters forward; more
 // rounds follow only if the window turns out to need more victims than that.
-__device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S, volatile uint32_t* any_twin, uint32_t L, int lane) {
+__device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S, uint32_t L, int lane) {
   const uint32_t lt = (1u << lane) - 1u;
   const RingEnt* ring = P.ring[L];
   unsigned long long rounds = 0;
@@ -189,10 +192,10 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
     if (S.ctl_done) break;
     const uint32_t head = S.ctl_head[L], limit = S.ctl_limit[L];
     uint32_t q0 = head & ~3u, found = 0;
-    const int want = (int)S.ctl_k;
+    int want = (int)S.ctl_k;
     ScanRegs cur = wide_scan_load(ring, P.ring_mask, q0, lane);   // in flight while the owners fetch; used after B1
     __syncthreads();                                   // (B1) the scanners never hold this barrier up
-    if (*any_twin) { __syncthreads(); __syncthreads(); }
+    if (S.twinc[0] | S.twinc[1] | S.twinc[2] | S.twinc[3]) { __syncthreads(); __syncthreads(); want = (int)S.twin_k; }
     // while the owners roll (not in an all-hit window, which needs no victim): up to 3 rounds, until as many live entries
     // are known as the window has accesses, so that the owners rarely wait for a scan after the roll
     bool all_hit = true;
@@ -203,7 +206,7 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
       const uint32_t hit = (P.policy == POLICY_LRU) ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);
       all_hit = all_hit && ((hit & km) == km);
     }
-    if (all_hit && !S.ctl_twins) continue;             // the owners apply an all-hit window without any further barrier
+    if (all_hit) continue;                             // the owners apply an all-hit window without any further barrier
     for (int it = 0; !all_hit && it < 4 && (int)found < want && (int32_t)(limit - q0) > 0; ++it) {
       const ScanRegs nxt = wide_scan_load(ring, P.ring_mask, q0 + (uint32_t)WIDE_W, lane);
       found += wide_scan_round(cur, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
@@ -239,7 +242,6 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
 
 __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __grid_constant__ StepParams P) {
   __shared__ WideShared S;
-  __shared__ uint32_t s_any_twin;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
   uint32_t lm[WIDE_WARPS], me[WIDE_WARPS];   // see wide_rank / wide_has
@@ -247,20 +249,17 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
   for (int u = 0; u < WIDE_WARPS; ++u) { lm[u] = (u < warp) ? FULL : ((u == warp) ? lt : 0u); me[u] = (u == warp) ? (1u << lane) : 0u; }
   const bool lru = (P.policy == POLICY_LRU);
   const bool hold = (P.pin_scope == 2);      // held scope: see machine_batched.cuh
-  const bool twins = P.state->step_twins != 0;   // K2 saw a request reach some node twice: look for twins in every window
   const int32_t c = P.capacity;
   const int64_t N = (int64_t)P.n_access;
+  if (P.state->error == DEV_ERR_NODE_POOL) return;       // K2 could not give every key a node: the step is void (sticky error)
   SerialCtx C;            // identical in every thread
   ctx_load(C, P);
-  for (int i = tid; i < WIDE_SET; i += 2 * WIDE_W) { S.set_id[i] = 0xFFFFFFFFu; S.set_min[i] = 0xFFFFFFFFu; }
-  if (tid == 0) { s_any_twin = 0; S.ctl_twins = twins ? 1u : 0u; }
-  __syncthreads();
   unsigned long long dbg[DBG_COUNT];
 #pragma unroll
   for (int i = 0; i < DBG_COUNT; ++i) dbg[i] = 0;
   const long long t_begin = clock64();
   if (warp >= WIDE_WARPS) {                                 // warps 4..7 scan the LRU ends of T1, T2, B1, B2
-    wide_scanner(P, S, &s_any_twin, (uint32_t)(warp - WIDE_WARPS) + 1u, lane);
+    wide_scanner(P, S, (uint32_t)(warp - WIDE_WARPS) + 1u, lane);
     return;
   }
 
@@ -280,18 +279,19 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
   int64_t spec_base = -1;                                // the access index the speculative record below belongs to, minus tid
   // ... and so is the node RECORD, speculatively: it is loaded while the current window rolls (after B1, when everything
   // the previous window wrote is visible) and is exact unless the current window itself changes that node, which happens
-  // in two ways only: the window also accesses the node (found by probing the window's twin-detection set), or it takes
-  // the node as a victim / dropped ghost (the node's ring position lies in a range the window consumes).  Either way the
-  // record is then loaded again at the start of the next window, as it is after a cut window.  Without the step's twin
-  // flag no set exists; instead every owner writes its window's number into node_stamp[n] BEFORE the window's first
-  // barrier and the speculative load, issued AFTER it, reads the stamp along with the record: equal to the current
-  // window's number = this window accesses the node too (only a window of another request can).  With the flag (next to
-  // never) there is no speculation at all.
+  // in two ways only: the window also accesses the node, or it takes the node as a victim / dropped ghost (the node's
+  // ring position lies in a range the window consumes).  Either way the record is then loaded again at the start of the
+  // next window, as it is after a cut window.  Every node of a window carries the window's number in node_stamp[] BEFORE
+  // the window's first barrier; the speculative load, issued AFTER it, exchanges the stamp for the NEXT window's number
+  // and gets the old one back: equal to the current window's number = this window accesses the node too (only a window
+  // of another request can); equal to the next window's number = another thread of the next window owns the same node
+  // (a twin candidate, see the top of the file).  A window that does not start where the previous one was due to end
+  // (after a cut) stamps its nodes itself, synchronously, with a number no earlier exchange used.
   Node spec;
   spec.list = L_FREE; spec.pos = 0; spec.block = -1; spec.slot = 0;
   bool spec_ok = false;
   uint32_t win_seq = P.state->win_seq;                     // numbers the windows across steps; 31 bits, never 0
-  uint32_t spec_mark = 0;                                  // node_stamp of the speculated node, read with its record
+  uint32_t spec_mark = 0;                                  // what node_stamp of the speculated node held before this thread's exchange
   uint32_t my_cls[5] = {0, 0, 0, 0, 0};                  // accesses of general windows this thread applied, by class
 
   int64_t my_off = 0, my_off1 = 0;
@@ -308,6 +308,13 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       int k = kmax;
       const int64_t a0 = o + j;
       const bool act0 = tid < k;
+      // size of the window after this one if this one is not cut (an upper bound where it is not known cheaply)
+      int next_k = WIDE_W;
+      if (j + kmax < nb) next_k = (int)min((int64_t)WIDE_W, nb - j - kmax);
+      else if (((r + 1u) & 31u) != 0u && r + 1u < P.n_req) {
+        const int64_t nb1 = __shfl_sync(FULL, my_off1, (r + 1) & 31) - __shfl_sync(FULL, my_off, (r + 1) & 31);
+        if (nb1 > 0) next_k = (int)min((int64_t)WIDE_W, nb1);
+      }
       if (tid == 0) {
         S.ctl_done = 0; S.ctl_k = (uint32_t)kmax;
 #pragma unroll
@@ -319,30 +326,28 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       const uint32_t n = act0 ? S.ids[(uint32_t)(a0 + tid) & (WIDE_IDS - 1)] : NODE_NONE;
       Node rec;
       rec.list = L_FREE; rec.pos = 0; rec.block = -1; rec.slot = 0;
-      if (spec_mark == win_seq) spec_ok = false;                     // the previous window accessed the speculated node too
-      win_seq = (win_seq + 1u) & 0x7FFFFFFFu;
-      if (win_seq == 0) win_seq = 1;
+      const bool aligned = (spec_base == a0);                        // the window starts where the previous one was due to end:
+      const uint32_t prev_seq = win_seq;                             // its nodes were stamped with its number a window ago
+      win_seq = wide_next_seq(win_seq);
+      if (!aligned) win_seq = wide_next_seq(win_seq);                // a number no exchange has used yet
+      bool twin_c = false;                                           // the stamp says another thread of this window may own the same node
       if (act0) {
-        if (!twins) __stcg(P.node_stamp + n, win_seq);               // seen by the speculative loads after B1
-        if (spec_base == a0 && spec_ok) rec = spec; else rec = ld_node(P.nodes + n);
+        if (aligned) {
+          // The exchange returned the stamp's last value only.  This window's number there means another exchange for
+          // this window came first (a twin, or a thread that stamped a position beyond the window because next_k was an
+          // upper bound) and took away what the stamp said before: the record cannot be trusted either.
+          twin_c = (spec_mark == win_seq);
+          if (spec_mark == prev_seq || twin_c) spec_ok = false;      // the previous window accessed the speculated node too
+          if (spec_ok) rec = spec; else rec = ld_node(P.nodes + n);
+        } else {
+          const uint32_t old = atomicExch(P.node_stamp + n, win_seq);   // seen by the exchanges after B1
+          rec = ld_node(P.nodes + n);
+          twin_c = (old == win_seq);
+        }
       }
       // the id this thread will own if the next window starts where this one is due to end
       const uint32_t pre_n = (a0 + kmax + tid < N) ? S.ids[(uint32_t)(a0 + kmax + tid) & (WIDE_IDS - 1)] : NODE_NONE;
       ids_request(a0 + kmax + 2 * WIDE_W);
-
-      // (1) the same node twice in the window: exact detection with a shared-memory hash set
-      uint32_t slot = 0xFFFFFFFFu;
-      if (twins && act0) {
-        uint32_t h = (n * 2654435761u) >> 23;                        // 9 bits
-        for (;;) {
-          const uint32_t old = atomicCAS(&S.set_id[h], 0xFFFFFFFFu, n);
-          if (old == 0xFFFFFFFFu) break;
-          if (old == n) { s_any_twin = 1; break; }
-          h = (h + 1) & (WIDE_SET - 1);
-        }
-        slot = h;
-        atomicMin(&S.set_min[slot], (uint32_t)tid);
-      }
       const uint32_t lst = rec.list & NODE_LIST_MASK;
       const bool held = (rec.list & NODE_HELD) != 0;                 // held scope: in no ring, rec.pos = its holds
       {
@@ -350,11 +355,14 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         // hits on entries that were still evictable by this request (below bound): they stop being so
         const uint32_t be = __ballot_sync(FULL, !held && ((lst == L_T1 && (int32_t)(C.bound[L_T1] - rec.pos) > 0) ||
                                                               (lst == L_T2 && (int32_t)(C.bound[L_T2] - rec.pos) > 0)));
-        if (lane == 0) { S.m[0][warp] = b0; S.m[1][warp] = b1; S.m[2][warp] = b2; S.m[3][warp] = be; }
+        const uint32_t bt = __ballot_sync(FULL, twin_c);
+        if (lane == 0) { S.m[0][warp] = b0; S.m[1][warp] = b1; S.m[2][warp] = b2; S.m[3][warp] = be; S.twinc[warp] = bt; }
       }
-      __syncthreads();                                               // (B1) class masks and the hash set are complete
-      if (twins && s_any_twin) {                                     // CTA-uniform, next to never taken
-        const bool later = act0 && S.set_min[slot] < (uint32_t)tid;
+      __syncthreads();                                               // (B1) class masks and twin candidates are complete
+      // (1) the same node twice in the window: cut before the second occurrence
+      if (S.twinc[0] | S.twinc[1] | S.twinc[2] | S.twinc[3]) {       // CTA-uniform, next to never taken
+        bool later = false;                                          // an earlier access of the window has this thread's node
+        if (act0) for (int i = 0; i < tid; ++i) later = later || (S.ids[(uint32_t)(a0 + i) & (WIDE_IDS - 1)] == n);
         const uint32_t tb = __ballot_sync(FULL, later);
         if (lane == 0) S.twin[warp] = tb;
         __syncthreads();
@@ -362,15 +370,15 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
 #pragma unroll
         for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.twin[u]) first = 32 * u + __ffs(S.twin[u]) - 1;
         if (first < k) { k = first; dbg[DBG_CUT_TWIN]++; }
+        if (tid == 0) S.twin_k = (uint32_t)k;                        // the scanners judge "all hits" on the same accesses
         __syncthreads();
-        if (tid == 0) s_any_twin = 0;
       }
-      // the next window's record, speculatively (see above); a node this window accesses too is not trusted
+      // the next window's record, speculatively, and its stamp (see above); a node this window accesses too is not trusted
       spec_ok = false;
       spec_base = a0 + kmax;
-      if (!twins && pre_n != NODE_NONE) {
+      if (pre_n != NODE_NONE && tid < next_k) {                      // next_k >= the next window's size: every owner of it is covered
         spec = ld_node(P.nodes + pre_n);
-        spec_mark = __ldcg(P.node_stamp + pre_n);                    // looked at when the next window starts, not now
+        spec_mark = atomicExch(P.node_stamp + pre_n, wide_next_seq(win_seq));   // looked at when the next window starts, not now
         spec_ok = true;
       }
       uint32_t M0[WIDE_WARPS], M1[WIDE_WARPS], M2[WIDE_WARPS], ME[WIDE_WARPS], KM[WIDE_WARPS], HIT[WIDE_WARPS];
@@ -422,11 +430,6 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
         if (lane == 0) S.bad[warp] = 0;
         j += k;
         dbg[DBG_WIN_HIT]++; dbg[DBG_ACC_HIT_WIN] += (unsigned)k;
-        if (twins) {                                                 // the full barrier sequence (need = 0: no B2'), else none at all
-          if (act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
-          __syncthreads();                                           // (B2)
-          __syncthreads_or(0);                                       // (B3)
-        }
         dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw1);
         continue;
       }
@@ -496,7 +499,6 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
             __syncwarp();
             if (lane == 0) S.ctx = T;
           }
-          if (twins && act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
           __syncthreads();
           C = S.ctx;
           j += 1;
@@ -602,7 +604,6 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
       C.tail[L_B2] += need[L_T2];
       C.t1 = D.R.t1; C.t2 = D.R.t2; C.b1 = D.R.b1; C.b2 = D.R.b2; C.p = D.R.p; C.next_fresh = D.R.nf;
       C.elig1 = D.R.e1; C.elig2 = D.R.e2;
-      if (twins && act0) { S.set_id[slot] = 0xFFFFFFFFu; S.set_min[slot] = 0xFFFFFFFFu; }
       j += k;
       dbg[DBG_WIN_GENERAL]++; dbg[DBG_ACC_GENERAL_WIN] += (unsigned)k;
       dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw3);

@@ -276,6 +276,38 @@ def test_probe_alone_is_a_consistent_map(arc):
     gc.close()
 
 
+def test_probe_on_a_table_far_larger_than_l2(arc):
+    """K2 at c = 16 M blocks (a 2 GiB table, 16 x the 126 MB L2; the size bench.py's probe leg times): 16 M random keys
+    of which 1 M repeat inside the launch (they race for one slot and must share one node), every key found again at
+    its node in a second launch in another order, as many nodes as distinct keys, no device-side error; and the
+    random-sector ceiling kernel reads what the table holds."""
+    n = 1 << 24
+    g = torch.Generator(device="cuda")
+    g.manual_seed(16)
+    keys = torch.randint(2, 2 ** 62, (n,), dtype=torch.int64, device="cuda", generator=g)
+    keys[5:5 + 4096:2] = keys[4:4 + 4096:2]              # duplicates inside one launch: adjacent (same warp, same instant) ...
+    keys[n - (1 << 20):] = keys[:1 << 20]                # ... and far apart in the grid
+    gc = arc.ArcCache(n)
+    gc.reserve(1, n)
+    nodes = gc.debug_probe(keys).clone()
+    torch.cuda.synchronize()
+    assert torch.equal(nodes[n - (1 << 20):], nodes[:1 << 20])
+    assert torch.equal(nodes[5:5 + 4096:2], nodes[4:4 + 4096:2])
+    n_keys = torch.unique(keys).numel()
+    assert torch.unique(nodes).numel() == n_keys and int(nodes.min()) >= 0
+    perm = torch.randperm(n, device="cuda", generator=g)
+    again = gc.debug_probe(keys[perm].contiguous())
+    torch.cuda.synchronize()
+    assert torch.equal(again, nodes[perm])
+    gc.stats()                                           # raises on a device-side error (node pool, bad node)
+    gc.close()
+    buf = torch.arange(1 << 22, dtype=torch.int32, device="cuda")          # 16 MiB = 2^19 sectors
+    x = arc.debug_gather_sectors(keys[:4096], buf).cpu().numpy()
+    k = keys[:4096].cpu().numpy().view(np.uint64)
+    want = np.bitwise_xor.reduce(buf.cpu().numpy().reshape(-1, 8)[(k & np.uint64((1 << 19) - 1)).astype(np.int64)], axis=1)
+    assert np.array_equal(x, want)
+
+
 @pytest.mark.parametrize("machine", [0, 1, 2, 3])
 def test_step_wide_pin_scope(arc, machine):
     """NEXT-3 (part): ARC_PIN_STEP.  Hand trace G's situation (an earlier request's block is still pinned when a later

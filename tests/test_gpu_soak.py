@@ -17,7 +17,7 @@ from paper_2606_21238_b200 import workloads as W
 @pytest.fixture(scope="module")
 def A():
     if not torch.cuda.is_available():
-        pytest.skip("needs a CUDA device")
+        pytest.fail("-m gpu tests need a CUDA device")
     from paper_2606_21238_b200 import arc as A_
 
     A_.load_library()
