@@ -18,14 +18,13 @@ namespace arc {
 
 constexpr uint32_t L_ABSENT = 0, L_T1 = 1, L_T2 = 2, L_B1 = 3, L_B2 = 4, L_FREE = 5;
 constexpr unsigned long long KEY_EMPTY = 0ull, KEY_TOMB = 1ull;  // H5 keeps real keys >= 2
-constexpr uint32_t SLOT_NODE_PENDING = 0;        // Slot::node holds node id + 1; 0 = no node (EMPTY slot or tombstone).  Key and node
-                                                 // id are published together by one 128-bit CAS, so a live key always has its node
+constexpr uint32_t SLOT_NODE_PENDING = 0;        // Slot::node holds node id + 1; 0 = EMPTY slot, tombstone, or (inside K2 only) a key
+                                                 // whose winner has not published its node id yet
 constexpr uint32_t NODE_NONE = 0xFFFFFFFFu;
 constexpr uint32_t NODE_HELD = 0x100u;           // Node::list flag (pin scope 2): the node is resident, has holds and is in NO ring;
                                                  // Node::pos then carries the hold count instead of a ring position
 constexpr uint32_t NODE_LIST_MASK = 0xFFu;
 constexpr uint32_t BUCKET_SLOTS = 2;             // 2 x 16 B = one 32 B sector: what one probe reads
-constexpr uint32_t K2_MAX_THREADS = 148 * 8 * 256;   // largest K2 grid: at most one unused node id per thread comes back (StepParams::spare)
 
 enum : int { CLS_MISS = 0, CLS_HIT_T1 = 1, CLS_HIT_T2 = 2, CLS_GHOST_B1 = 3, CLS_GHOST_B2 = 4 };
 enum : int { POLICY_ARC = 0, POLICY_LRU = 1, POLICY_DBL = 2 };
@@ -68,7 +67,7 @@ struct DevState {
   uint32_t error;                 // DEV_ERR_*
   uint32_t tombs;                 // tombstones currently in the table
   uint32_t k1_ticket;             // K1 work ticket: 0 between steps (K4 resets it)
-  uint32_t n_spare;               // node ids K2 popped and did not use (lost slot races), listed in StepParams::spare; K4 pushes them back
+  uint32_t reserved0;
   unsigned long long stat[ST_COUNT];
   // scratch for ring compaction (old window of the list being compacted)
   uint32_t cmp_head[5], cmp_tail[5];
@@ -116,7 +115,6 @@ struct StepParams {
   int32_t pin_scope;              // 0: pins end with their request, 1: with the step, 2: held until arc_release
   uint32_t* node_of_block;        // pin scope 2: node id of the resident entry that owns each block id
   uint32_t* node_stamp;           // [node_cap] K3 wide machine: number of the last window that accessed the node (twin check, speculation)
-  uint32_t* spare;                // [K2_MAX_THREADS] see DevState::n_spare
   uint32_t* counts_out;           // [2] copy of DevState::counts next to prefix_len / alloc_ids / evict_ids (one D2H copy in arc_step_host)
   unsigned long long key_and;     // test hook (arc_debug_set_key_mask): keys are ANDed with this before the probe; all ones normally
 };

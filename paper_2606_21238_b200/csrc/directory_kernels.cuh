@@ -19,12 +19,18 @@ namespace cg = cooperative_groups;
 // has a never-used slot).  A probe therefore costs one sector = 32 B next to the 8 B of the key and the 4 B of the
 // node id: 44 B per key against 28 B algorithmic.  Each thread keeps PROBE_ILP keys in flight.
 //
-// Insert-if-absent: the lowest EMPTY slot of that bucket is claimed with ONE 128-bit compare-and-swap
-// (atom.cas.b128, sm_90+) that writes key and node id together, so a slot is never seen half-published: there is no
-// "claimed, node pending" state, no second pass and no spinning.  The node id is popped from the free stack before the
-// CAS; a thread that loses the race (another thread took the slot - possibly for the same key, which the re-read of
-// the bucket then finds) keeps the id for its next insert and hands a leftover to DevState::spare[], which K4 pushes
-// back (pushes never run concurrently with pops).  Tombstones are not reused; rebuild_table clears them.
+// Insert-if-absent, in warp-synchronous phases, so that (1) the free stack's top - one address for the whole GPU - sees
+// one atomic per warp and not one per insert, (2) exactly as many node ids are popped as keys are new, and (3) nobody
+// ever waits for a thread that could be waiting for him:
+//   A  every thread walks each of its keys' buckets until it finds the key or a bucket with a never-used slot;
+//   C1 claims: 64-bit CAS EMPTY -> key on the slot.  The winner of a key is the one thread whose CAS put it there; a
+//      thread that finds its key already there (CAS result, or a bucket read) is a waiter of that slot; a thread that
+//      finds another key there walks on;
+//   B  the warp pops one node id per winner with ONE atomicSub (shuffle scan of the counts);
+//   C2 winners write the node record and publish the id in the slot (Slot::node = id + 1);  __syncwarp;
+//   C3 waiters read the slot until the id is there.  The winner may sit in another warp; it never waits between its
+//      claim and its publish (C2 comes before C3 in every warp), so the wait is bounded and cannot be circular.
+// Tombstones are not reused; rebuild_table clears them.
 constexpr int PROBE_ILP = 4;
 
 struct Bucket { Slot s[BUCKET_SLOTS]; };
@@ -37,63 +43,143 @@ __device__ __forceinline__ Bucket ld_bucket(const Slot* p) {          // p is 32
   b.s[1].key = (unsigned long long)r[4] | ((unsigned long long)r[5] << 32); b.s[1].node = r[6]; b.s[1].pad = r[7];
   return b;
 }
-// {EMPTY, 0, 0} -> {key, node + 1, 0} in one atomic; true if this thread now owns the slot
-__device__ __forceinline__ bool slot_claim(Slot* p, unsigned long long key, uint32_t node_plus_1) {
-  unsigned long long ok, ov;
-  asm volatile("{\n\t.reg .b128 c, n, o;\n\tmov.b128 c, {%2, %3};\n\tmov.b128 n, {%4, %5};\n\t"
-               "atom.relaxed.gpu.global.cas.b128 o, [%6], c, n;\n\tmov.b128 {%0, %1}, o;\n\t}"
-               : "=l"(ok), "=l"(ov) : "l"(0ull), "l"(0ull), "l"(key), "l"((unsigned long long)node_plus_1), "l"(p) : "memory");
-  return ok == KEY_EMPTY && ov == 0ull;
+
+// the same load under a predicate (no branch, the destination keeps its content): keeps the buckets of a round in registers
+__device__ __forceinline__ void ld_bucket_if(Bucket& b, const Slot* p, bool take) {
+  uint32_t r0 = (uint32_t)b.s[0].key, r1 = (uint32_t)(b.s[0].key >> 32), r2 = b.s[0].node, r3 = b.s[0].pad;
+  uint32_t r4 = (uint32_t)b.s[1].key, r5 = (uint32_t)(b.s[1].key >> 32), r6 = b.s[1].node, r7 = b.s[1].pad;
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %9, 0;\n\t@q ld.global.cg.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"
+               : "+r"(r0), "+r"(r1), "+r"(r2), "+r"(r3), "+r"(r4), "+r"(r5), "+r"(r6), "+r"(r7) : "l"(p), "r"((uint32_t)take) : "memory");
+  b.s[0].key = (unsigned long long)r0 | ((unsigned long long)r1 << 32); b.s[0].node = r2; b.s[0].pad = r3;
+  b.s[1].key = (unsigned long long)r4 | ((unsigned long long)r5 << 32); b.s[1].node = r6; b.s[1].pad = r7;
 }
 
-// Finds or inserts `key`, starting with bucket content `b` already loaded for bucket index `bucket`.  `spare` is a node
-// id this thread popped earlier and did not use (NODE_NONE if none).  Returns the node id, or NODE_NONE when the node
-// pool is exhausted (sticky DEV_ERR_NODE_POOL: the step's results are void, K3 does not run).
-__device__ __forceinline__ uint32_t probe_one(const StepParams& P, unsigned long long key, uint32_t bucket, Bucket b, uint32_t& spare) {
+enum : uint32_t { PR_DONE = 0, PR_CLAIM = 1, PR_WAIT = 2, PR_WON = 3, PR_LOAD = 4 };
+
+// Looks at bucket content c (bucket index bk) for `key`: found with its node -> PR_DONE (node set); found, node not yet
+// published -> PR_WAIT (idx = the slot); a never-used slot -> PR_CLAIM (idx = that slot); else 0xFF: full of other keys.
+__device__ __forceinline__ uint32_t probe_bucket(const Bucket& c, uint32_t bk, unsigned long long key, uint32_t& node, uint32_t& idx) {
+#pragma unroll
+  for (int e = 0; e < (int)BUCKET_SLOTS; ++e)
+    if (c.s[e].key == key) {
+      idx = bk * BUCKET_SLOTS + (uint32_t)e;
+      if (c.s[e].node == SLOT_NODE_PENDING) return PR_WAIT;
+      node = c.s[e].node - 1;
+      return PR_DONE;
+    }
+#pragma unroll
+  for (int e = 0; e < (int)BUCKET_SLOTS; ++e)
+    if (c.s[e].key == KEY_EMPTY) { idx = bk * BUCKET_SLOTS + (uint32_t)e; return PR_CLAIM; }
+  return 0xFFu;
+}
+
+// One pass of a warp over 32 x PROBE_ILP keys (key u of lane l is access first + u * stride).  Phases A and C1 run as
+// ROUNDS over all of a thread's keys at once - every key that still needs a bucket gets its load issued, then every key
+// that found a never-used slot gets its CAS issued - so that the dependent memory round trips a warp pays are those of
+// its longest probe sequence, not the sum over its keys.
+__device__ __forceinline__ void probe_warp_pass(const StepParams& P, uint32_t first, uint32_t stride, int lane) {
+  const uint32_t FULL = 0xFFFFFFFFu;
+  unsigned long long key[PROBE_ILP];
+  uint32_t idx[PROBE_ILP], node[PROBE_ILP], st[PROBE_ILP];   // idx: bucket index while st = PR_LOAD, slot index otherwise
+#pragma unroll
+  for (int u = 0; u < PROBE_ILP; ++u) {
+    const uint32_t a = first + u * stride;
+    key[u] = (a < P.n_access) ? (__ldcg(P.keys_acc + a) & P.key_and) : 2ull;
+    if (key[u] < 2) key[u] += 2;                       // 0 and 1 stay reserved under the test mask too
+    idx[u] = (uint32_t)key[u] & P.bucket_mask;
+    node[u] = NODE_NONE;
+    st[u] = (a < P.n_access) ? PR_LOAD : PR_DONE;
+  }
+  uint32_t won = 0;
+  Bucket b[PROBE_ILP];
+#pragma unroll
+  for (int u = 0; u < PROBE_ILP; ++u) { b[u].s[0].key = b[u].s[1].key = 0; b[u].s[0].node = b[u].s[1].node = b[u].s[0].pad = b[u].s[1].pad = 0; }
   for (;;) {
-    if (b.s[0].key == key) return b.s[0].node - 1;
-    if (b.s[1].key == key) return b.s[1].node - 1;
-    const int e = (b.s[0].key == KEY_EMPTY) ? 0 : ((b.s[1].key == KEY_EMPTY) ? 1 : -1);
-    if (e < 0) { bucket = (bucket + 1) & P.bucket_mask; b = ld_bucket(P.table + (size_t)bucket * BUCKET_SLOTS); continue; }
-    if (spare == NODE_NONE) {
-      const uint32_t top = atomicSub(&P.state->free_top, 1u);
-      if (top == 0 || top > 0x7FFFFFFFu) {
-        atomicAdd(&P.state->free_top, 1u);
-        atomicExch(&P.state->error, DEV_ERR_NODE_POOL);
-        return NODE_NONE;
-      }
-      spare = P.free_stack[top - 1];
+    // A: one bucket for every key that needs one
+    bool busy = false;
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) {
+      const bool take = st[u] == PR_LOAD;
+      ld_bucket_if(b[u], P.table + (size_t)(take ? idx[u] : 0u) * BUCKET_SLOTS, take);
+      busy = busy || take;
     }
-    const uint32_t idx = bucket * BUCKET_SLOTS + (uint32_t)e;
-    st_node(P.nodes + spare, L_ABSENT, 0, -1, idx);        // read by K3 only, after the kernel boundary
-    P.node_key[spare] = key;
-    if (slot_claim(P.table + idx, key, spare + 1)) { const uint32_t got = spare; spare = NODE_NONE; return got; }
-    b = ld_bucket(P.table + (size_t)bucket * BUCKET_SLOTS);   // lost the race for that slot: the winner may hold our key
+    if (!busy) break;
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) {
+      if (st[u] != PR_LOAD) continue;
+      const uint32_t bk = idx[u];
+      st[u] = probe_bucket(b[u], bk, key[u], node[u], idx[u]);
+      if (st[u] == 0xFFu) { st[u] = PR_LOAD; idx[u] = (bk + 1) & P.bucket_mask; }   // full of other keys: the next bucket, next round
+    }
+    // C1: claims.  The winner of a key is the one thread whose CAS put it there.
+    unsigned long long old[PROBE_ILP];
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) if (st[u] == PR_CLAIM) old[u] = atomicCAS(&P.table[idx[u]].key, KEY_EMPTY, key[u]);
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) {
+      if (st[u] != PR_CLAIM) continue;
+      if (old[u] == KEY_EMPTY) { st[u] = PR_WON; ++won; }
+      else if (old[u] == key[u]) st[u] = PR_WAIT;
+      else { st[u] = PR_LOAD; idx[u] /= BUCKET_SLOTS; }   // another key took the slot: look at the same bucket again
+    }
   }
+  // B: one pop for the warp
+  uint32_t incl = won;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const uint32_t v = __shfl_up_sync(FULL, incl, d); if (lane >= d) incl += v; }
+  const uint32_t total = __shfl_sync(FULL, incl, 31);
+  if (total) {
+    uint32_t top = 0;
+    if (lane == 0) {
+      top = atomicSub(&P.state->free_top, total);
+      if (top < total || top > 0x7FFFFFFFu) {          // the pool cannot serve the warp: nothing is taken
+        atomicAdd(&P.state->free_top, total);
+        atomicExch(&P.state->error, DEV_ERR_NODE_POOL);
+        top = 0;
+      }
+    }
+    top = __shfl_sync(FULL, top, 0);
+    uint32_t next = top - (incl - won);                // this thread's ids: free_stack[next - 1], free_stack[next - 2], ...
+    // C2: winners publish.  On an exhausted pool (top == 0, sticky error, K3 will not run) the slot gets a value that
+    // makes every waiter leave with NODE_NONE.
+    uint32_t id[PROBE_ILP];
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) if (st[u] == PR_WON && top) id[u] = __ldcg(P.free_stack + (--next));
+#pragma unroll
+    for (int u = 0; u < PROBE_ILP; ++u) {
+      if (st[u] != PR_WON) continue;
+      uint32_t pub = NODE_NONE;
+      if (top) {
+        st_node(P.nodes + id[u], L_ABSENT, 0, -1, idx[u]);   // read by K3 only, after the kernel boundary
+        P.node_key[id[u]] = key[u];
+        node[u] = id[u];
+        pub = id[u] + 1u;
+      }
+      __stcg(&P.table[idx[u]].node, pub);
+    }
+  }
+  __syncwarp();
+  // C3: waiters
+#pragma unroll
+  for (int u = 0; u < PROBE_ILP; ++u) {
+    if (st[u] != PR_WAIT) continue;
+    const volatile uint32_t* p = &P.table[idx[u]].node;
+    uint32_t v;
+    while ((v = *p) == SLOT_NODE_PENDING) {}
+    node[u] = (v == NODE_NONE) ? NODE_NONE : v - 1u;   // NODE_NONE: the winner found the pool exhausted
+  }
+#pragma unroll
+  for (int u = 0; u < PROBE_ILP; ++u) if (first + u * stride < P.n_access) P.node_acc[first + u * stride] = node[u];
 }
 
-__device__ __forceinline__ void probe_range(const StepParams& P, uint32_t first, uint32_t stride) {
-  uint32_t spare = NODE_NONE;
-  for (uint32_t a0 = first; a0 < P.n_access; a0 += stride * PROBE_ILP) {
-    unsigned long long key[PROBE_ILP];
-    uint32_t bucket[PROBE_ILP];
-    Bucket b[PROBE_ILP];
-#pragma unroll
-    for (int u = 0; u < PROBE_ILP; ++u) {
-      const uint32_t a = a0 + u * stride;
-      key[u] = (a < P.n_access) ? (__ldcg(P.keys_acc + a) & P.key_and) : 2ull;
-      if (key[u] < 2) key[u] += 2;                   // 0 and 1 stay reserved under the test mask too
-      bucket[u] = (uint32_t)key[u] & P.bucket_mask;
-    }
-#pragma unroll
-    for (int u = 0; u < PROBE_ILP; ++u) b[u] = ld_bucket(P.table + (size_t)bucket[u] * BUCKET_SLOTS);
-#pragma unroll
-    for (int u = 0; u < PROBE_ILP; ++u) {
-      const uint32_t a = a0 + u * stride;
-      if (a < P.n_access) P.node_acc[a] = probe_one(P, key[u], bucket[u], b[u], spare);
-    }
-  }
-  if (spare != NODE_NONE) P.spare[atomicAdd(&P.state->n_spare, 1u)] = spare;     // at most one per thread: P.spare has K2_MAX_THREADS entries
+// Warp gw of n_warps takes chunks gw, gw + n_warps, ... of 32 x PROBE_ILP consecutive accesses: key u of lane l is access
+// chunk * 32 * PROBE_ILP + 32 u + l (every load of a warp is one coalesced 256-byte access).  The trip count is
+// warp-uniform (the passes use warp collectives).
+__device__ __forceinline__ void probe_range(const StepParams& P, uint32_t thread, uint32_t n_threads) {
+  const int lane = (int)(thread & 31u);
+  const uint32_t n_warps = n_threads >> 5;
+  for (uint64_t chunk = thread >> 5; chunk * (32u * PROBE_ILP) < P.n_access; chunk += n_warps)
+    probe_warp_pass(P, (uint32_t)(chunk * (32u * PROBE_ILP)) + (uint32_t)lane, 32u, lane);
 }
 
 __global__ void __launch_bounds__(256) probe_reserve_kernel(const __grid_constant__ StepParams P) {
@@ -121,22 +207,6 @@ __global__ void __launch_bounds__(256) gather32_kernel(const unsigned long long*
                           (uint32_t)b[u].s[1].key ^ (uint32_t)(b[u].s[1].key >> 32) ^ b[u].s[1].node ^ b[u].s[1].pad;
     }
   }
-}
-
-// Node ids that K2's threads popped and did not use go back on the free stack (no pop runs concurrently: K4, or the
-// tail of arc_debug_probe).
-__device__ __forceinline__ void return_spares(const StepParams& P, uint32_t tid, uint32_t nthr) {
-  const uint32_t n = P.state->n_spare;
-  for (uint32_t i = tid; i < n; i += nthr) {
-    const uint32_t d = P.spare[i];
-    st_node(P.nodes + d, L_FREE, 0, -1, 0);
-    P.free_stack[atomicAdd(&P.state->free_top, 1u)] = d;
-  }
-}
-__global__ void __launch_bounds__(256) return_spares_kernel(const __grid_constant__ StepParams P) {
-  return_spares(P, threadIdx.x, blockDim.x);
-  __syncthreads();
-  if (threadIdx.x == 0) P.state->n_spare = 0;
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -179,11 +249,6 @@ __device__ __forceinline__ void finalize_body(const StepParams& P) {
   if (tid == 0) {
     P.state->k1_ticket = 0;                                            // K1 of the next step starts from request 0
     P.counts_out[0] = P.state->counts[0]; P.counts_out[1] = P.state->counts[1];
-  }
-  if (blockIdx.x == 0 && P.state->n_spare) {                           // CTA-uniform (nobody writes n_spare during K4 but this CTA)
-    return_spares(P, threadIdx.x, blockDim.x);
-    __syncthreads();
-    if (threadIdx.x == 0) P.state->n_spare = 0;
   }
 }
 

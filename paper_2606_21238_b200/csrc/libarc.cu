@@ -70,7 +70,6 @@ struct arc_cache {
   unsigned long long* d_node_key = nullptr;
   uint32_t* d_free_stack = nullptr;
   uint32_t* d_node_stamp = nullptr;   // [node_cap] K3 wide machine: window numbers (twin check, speculation)
-  uint32_t* d_spare = nullptr;        // [K2_MAX_THREADS] node ids K2 popped and did not use
   unsigned long long* d_seg_end = nullptr;   // [kSegEndCap] end states of K1's segments (steps with few, long requests)
   Slot* d_table = nullptr;
   RingEnt* d_ring[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -150,7 +149,6 @@ StepParams make_params(arc_cache* h) {
   P.node_of_block = h->d_node_of_block;
   P.node_stamp = h->d_node_stamp;
   P.counts_out = reinterpret_cast<uint32_t*>(h->d_result_pack + h->req_cap);
-  P.spare = h->d_spare;
   return P;
 }
 
@@ -275,7 +273,6 @@ int ensure_capacity(arc_cache* h, uint32_t n_req, uint64_t N, cudaStream_t s) {
     CUDA_TRY(h, dalloc(&h->d_node_stamp, node_cap));
     CUDA_TRY(h, cudaMemsetAsync(h->d_node_stamp, 0, (size_t)node_cap * sizeof(uint32_t), s));
     CUDA_TRY(h, dalloc(&h->d_table, table_slots));
-    CUDA_TRY(h, dalloc(&h->d_spare, K2_MAX_THREADS));
     for (int L = 1; L <= 4; ++L) {
       CUDA_TRY(h, dalloc(&h->d_ring[L], ring_cap));
       CUDA_TRY(h, dalloc(&h->d_ring_alt[L], ring_cap));
@@ -661,7 +658,7 @@ void arc_destroy(arc_cache* h) {
   if (!h) return;
   cudaDeviceSynchronize();
   { StepBuffers b = take_step_buffers(h); free_step_buffers(b); }
-  dfree(h->d_state); dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_table); dfree(h->d_node_stamp); dfree(h->d_spare);
+  dfree(h->d_state); dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_table); dfree(h->d_node_stamp);
   for (int L = 1; L <= 4; ++L) { dfree(h->d_ring[L]); dfree(h->d_ring_alt[L]); }
   dfree(h->d_block_counts); dfree(h->d_tokens_stage); dfree(h->d_machine_scratch);
   dfree(h->d_node_of_block); dfree(h->d_rel_cnt); dfree(h->d_seg_end);
@@ -796,7 +793,9 @@ int arc_debug_probe(arc_cache* h, const uint64_t* d_keys, uint64_t n, uint32_t* 
   cudaStream_t s = (cudaStream_t)cuda_stream;
   int rc = ensure_capacity(h, 1, n, s);
   if (rc) return rc;
-  rc = maintain(h, n, s);
+  // this entry creates no tombstones and every used slot belongs to a node: the pool size bounds the load (0.375 of the table)
+  h->slots_used_bound = std::min<uint64_t>(h->slots_used_bound, h->node_cap);
+  rc = maintain(h, std::min<uint64_t>(n, h->node_cap - h->slots_used_bound), s);
   if (rc) return rc;
   StepParams P = make_params(h);
   P.keys_acc = const_cast<unsigned long long*>(reinterpret_cast<const unsigned long long*>(d_keys));
@@ -804,8 +803,7 @@ int arc_debug_probe(arc_cache* h, const uint64_t* d_keys, uint64_t n, uint32_t* 
   P.n_access = (uint32_t)n; P.n_req = 0;
   if (n) {
     probe_reserve_kernel<<<grid_for(n, 256 * PROBE_ILP, 148 * 8), 256, 0, s>>>(P);
-    return_spares_kernel<<<1, 256, 0, s>>>(P);
-    h->launches += 2;
+    h->launches += 1;
   }
   CUDA_TRY(h, cudaGetLastError());
   // every used slot belongs to a node and this entry creates no tombstones
