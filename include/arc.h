@@ -174,9 +174,19 @@ const char *arc_last_error(const arc_cache *h);
 
 /* Stateless K1: keys of every full block (H1-H6) in natural order, d_keys_out[blk_off[r] + i].
  *   d_tokens DEVICE, h_offsets HOST (as in arc_step), d_keys_out DEVICE uint64[N] with
- *   N = sum_r floor(len_r / block_size) (the caller computes it from the offsets). */
+ *   N = sum_r floor(len_r / block_size) (the caller computes it from the offsets).
+ * Asynchronous on cuda_stream; thread-safe; calls on different streams may overlap (every call has scratch of its own:
+ * the offsets go to the device through a library-owned copy stream, 16 (n_req + 1) + 16 bytes per call). */
 int arc_hash_blocks(const int32_t *d_tokens, const int64_t *h_offsets, uint32_t n_req, uint32_t block_size,
                     uint64_t *d_keys_out, void *cuda_stream);
+
+/* The same kernel with everything already on the device: the kernel-only figure of the K1 roofline run, and for callers
+ * that build their batch on the device.  d_offsets / d_blk_off: DEVICE int64[n_req+1] (token offsets; exclusive scan of
+ * the full blocks per request).  d_ticket: DEVICE, two uint32 words of caller-owned scratch that must be 0 at launch;
+ * the kernel leaves them 0 again, so one scratch zeroed once serves every later call ON THE SAME STREAM (calls that may
+ * run at the same time need scratch of their own).  Nothing is validated or copied; one kernel launch. */
+int arc_hash_blocks_device(const int32_t *d_tokens, const int64_t *d_offsets, const int64_t *d_blk_off, uint32_t n_req,
+                           uint32_t block_size, uint64_t *d_keys_out, uint32_t *d_ticket, void *cuda_stream);
 
 /* Diagnostics ------------------------------------------------------------------------------------ */
 

@@ -27,7 +27,7 @@ STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", 
 EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats", "arc_reset", "arc_destroy",
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
            "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe", "arc_set_pin_scope",
-           "arc_release", "arc_hold_units", "arc_step_resume", "arc_debug_gather_sectors"]
+           "arc_release", "arc_hold_units", "arc_step_resume", "arc_debug_gather_sectors", "arc_hash_blocks_device"]
 
 
 class ArcError(RuntimeError):
@@ -82,6 +82,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_last_error.argtypes = [vp]
     L.arc_last_error.restype = C.c_char_p
     L.arc_hash_blocks.argtypes = [vp, vp, u32, u32, vp, vp]
+    L.arc_hash_blocks_device.argtypes = [vp, vp, vp, u32, u32, vp, vp, vp]
     L.arc_set_profiling.argtypes = [vp, C.c_int]
     L.arc_last_kernel_times.argtypes = [vp, C.POINTER(_KernelTimes)]
     L.arc_launch_count.argtypes = [vp]
@@ -315,6 +316,16 @@ def hash_blocks(tokens, offsets, block_size: int = 16, out=None, stream=None):
     if out is None:
         out = torch.empty(n, dtype=torch.int64, device="cuda")
     rc = L.arc_hash_blocks(tokens.data_ptr(), o.ctypes.data, len(o) - 1, block_size, out.data_ptr(), _stream_ptr(stream))
+    if rc != OK:
+        raise ArcError(rc, L.arc_last_error(None).decode())
+    return out
+
+
+def hash_blocks_device(tokens, d_offsets, d_blk_off, n_req: int, out, ticket, block_size: int = 16, stream=None):
+    """arc_hash_blocks_device: offsets and block offsets are CUDA int64 tensors, ticket a zeroed CUDA int32[2] scratch."""
+    L = load_library()
+    rc = L.arc_hash_blocks_device(tokens.data_ptr(), d_offsets.data_ptr(), d_blk_off.data_ptr(), n_req, block_size, out.data_ptr(),
+                                  ticket.data_ptr(), _stream_ptr(stream))
     if rc != OK:
         raise ArcError(rc, L.arc_last_error(None).decode())
     return out

@@ -66,8 +66,8 @@ struct DevState {
   uint32_t counts[2];             // n_alloc, n_evict of the current step
   uint32_t error;                 // DEV_ERR_*
   uint32_t tombs;                 // tombstones currently in the table
-  uint32_t k1_ticket;             // K1 work ticket: 0 between steps (K4 resets it)
-  uint32_t reserved0;
+  uint32_t k1_ticket;             // K1 work ticket and, right behind it, the count of warps that have left the launch:
+  uint32_t k1_done;               // both 0 between launches (the last warp out resets them, hash_kernels.cuh k1_leave)
   unsigned long long stat[ST_COUNT];
   // scratch for ring compaction (old window of the list being compacted)
   uint32_t cmp_head[5], cmp_tail[5];

@@ -247,7 +247,6 @@ __device__ __forceinline__ void finalize_body(const StepParams& P) {
   }
   if (lane == 0 && tokens_hit) atomicAdd(&P.state->stat[ST_PREFIX_TOKENS], tokens_hit);
   if (tid == 0) {
-    P.state->k1_ticket = 0;                                            // K1 of the next step starts from request 0
     P.counts_out[0] = P.state->counts[0]; P.counts_out[1] = P.state->counts[1];
   }
 }

@@ -74,12 +74,33 @@ __device__ __forceinline__ unsigned long long kpow_small(int e) {
   return r;
 }
 
-// The tokens of one round as this lane sees them: vector 32*it + lane of the round's aligned cover (it = 0..3),
-// and vector 128 (x) in lane 0 only (needed when the request is misaligned and the round is full).
-struct RoundVecs {
-  uint4 v[4];
-  uint4 x;
-};
+// ---------------------------------------------------------------------------------------------------------------------
+// Token staging: every warp owns a ring of K1_STAGES shared-memory stages, each holding the 16-byte-aligned cover of one
+// round (32 blocks = 2 KB, plus one vector when the request is misaligned).  Lane 0 fills a stage with ONE bulk
+// asynchronous copy (cp.async.bulk global -> shared, the 1-D form of TMA; SASS UBLKCP) that signals the stage's mbarrier
+// with the byte count; the warp waits on the barrier's phase and hashes from shared memory.  K1_STAGES - 1 rounds are in
+// flight while one is hashed, with no load instruction, no address arithmetic and no register buffer in the hashing
+// loop.  The copies carry an L2 evict-first policy (the tokens are read once).
+constexpr int K1_STAGES = 4;
+constexpr int K1_STAGE_BYTES = 2080;                    // 129 vectors of 16 B, rounded up to a multiple of 32
+constexpr int K1_WARPS = 8;
+constexpr int K1_SMEM_BYTES = K1_WARPS * K1_STAGES * K1_STAGE_BYTES + K1_WARPS * K1_STAGES * 8;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile("{\n\t.reg .pred p;\n\tK1_WAIT:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@!p bra K1_WAIT;\n\t}"
+               ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, unsigned long long policy) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy) : "memory");
+}
 
 // 128-bit streaming load of tokens [g0, g0 + 4) (absolute token indices, tok + g0 is 16-byte aligned); words outside
 // the valid range [lo, hi) of the caller's buffer are not touched and read as 0.  Only rounds at the very edge of the
@@ -93,29 +114,57 @@ __device__ __noinline__ uint4 ld_tokens4_guarded(const uint32_t* __restrict__ to
   return r;
 }
 
-// va = absolute token index of the aligned cover's first word for this round; n_vec = vectors the round needs (0..129).
-__device__ __forceinline__ RoundVecs load_round(const uint32_t* __restrict__ tok, int64_t va, int n_vec, int lane, int64_t lo, int64_t hi) {
-  RoundVecs R;
-  if (va >= lo && va + 4 * (int64_t)n_vec <= hi) {            // the whole cover is inside the caller's buffer (warp-uniform)
-    const uint4* p = reinterpret_cast<const uint4*>(tok + va) + lane;
+// Per-warp pipeline state (registers; identical in every lane).
+struct WarpPipe {
+  uint32_t stage0;      // shared address of this warp's first stage
+  uint32_t bar0;        // shared address of this warp's first mbarrier
+  uint32_t parity;      // bit k: the phase stage k's barrier completes next
+  uint32_t manual;      // bit k: stage k was filled by the warp itself (an edge round), no barrier to wait on
+  unsigned long long policy;
+};
+
+__device__ __forceinline__ WarpPipe pipe_init(unsigned char* smem, int warp, int lane) {
+  WarpPipe W;
+  W.stage0 = smem_u32(smem) + (uint32_t)(warp * K1_STAGES * K1_STAGE_BYTES);
+  W.bar0 = smem_u32(smem) + (uint32_t)(K1_WARPS * K1_STAGES * K1_STAGE_BYTES + warp * K1_STAGES * 8);
+  W.parity = 0; W.manual = 0;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(W.policy));
+  if (lane == 0) {
 #pragma unroll
-    for (int it = 0; it < 4; ++it) R.v[it] = (it * 32 + lane < n_vec) ? __ldcs(p + it * 32) : make_uint4(0, 0, 0, 0);
-    R.x = (lane == 0 && n_vec > 128) ? __ldcs(p + 128) : make_uint4(0, 0, 0, 0);
-  } else {
-#pragma unroll
-    for (int it = 0; it < 4; ++it) {
-      const int e = it * 32 + lane;
-      R.v[it] = (e < n_vec) ? ld_tokens4_guarded(tok, va + 4 * (int64_t)e, lo, hi) : make_uint4(0, 0, 0, 0);
-    }
-    R.x = (lane == 0 && n_vec > 128) ? ld_tokens4_guarded(tok, va + 512, lo, hi) : make_uint4(0, 0, 0, 0);
+    for (int k = 0; k < K1_STAGES; ++k) mbar_init(W.bar0 + 8u * k, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  return R;
+  __syncwarp();
+  return W;
 }
 
-// word c (0..2) of the vector that FOLLOWS this lane's vector `cur` in the round: lane l+1's cur, and for lane 31
-// lane 0's `nxt` (the same lane-0 register of the next iteration / the 129th vector).
-__device__ __forceinline__ uint32_t next_word(uint32_t cur, uint32_t nxt, int lane) {
-  return __shfl_sync(0xFFFFFFFFu, lane == 0 ? nxt : cur, (lane + 1) & 31);
+// Starts the fill of stage k with the n_vec vectors from absolute token index va (tok + va is 16-byte aligned).
+__device__ __forceinline__ void pipe_issue(WarpPipe& W, int k, const uint32_t* __restrict__ tok, int64_t va, int n_vec, int lane,
+                                           int64_t lo, int64_t hi) {
+  const uint32_t dst = W.stage0 + (uint32_t)(k * K1_STAGE_BYTES);
+  if (va >= lo && va + 4 * (int64_t)n_vec <= hi) {          // the whole cover is inside the caller's buffer (warp-uniform)
+    if (lane == 0) {
+      mbar_expect_tx(W.bar0 + 8u * k, 16u * (uint32_t)n_vec);
+      bulk_g2s(dst, tok + va, 16u * (uint32_t)n_vec, W.bar0 + 8u * k, W.policy);
+    }
+  } else {                                                   // an edge of the buffer: words outside it are never touched
+    for (int e = lane; e < n_vec; e += 32) {
+      const uint4 v = ld_tokens4_guarded(tok, va + 4 * (int64_t)e, lo, hi);
+      asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 16u * e), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+    }
+    W.manual |= 1u << k;
+    __syncwarp();
+  }
+}
+__device__ __forceinline__ void pipe_wait(WarpPipe& W, int k) {
+  if (W.manual & (1u << k)) { W.manual &= ~(1u << k); return; }
+  mbar_wait(W.bar0 + 8u * k, (W.parity >> k) & 1u);
+  W.parity ^= 1u << k;
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+  return v;
 }
 
 struct LaneConsts {
@@ -123,20 +172,32 @@ struct LaneConsts {
   unsigned long long kp;             // K^(lane+1)
   int owner;                         // after the transpose-reduce, block i of the round sits in lane `owner` of lane i
 };
+__device__ __forceinline__ LaneConsts lane_consts(int lane) {
+  LaneConsts LC;
+  const int q = lane & 3;
+  LC.salt0 = (unsigned long long)(2 * q + 1) * H_M * H_C1;
+  LC.salt1 = (unsigned long long)(2 * q + 2) * H_M * H_C1;
+  LC.kp = kpow_small(lane + 1);
+  LC.owner = 4 * (lane & 7) + (lane >> 3);
+  return LC;
+}
 
-// Local chain states of one round: lane i returns sum_{j<=i} K^(i-j) g_j over the round's blocks (no carry-in);
-// lanes >= cnt contribute g = 0.  s = request misalignment in tokens.
-__device__ __forceinline__ unsigned long long round_local_scan(const RoundVecs& cur, int s, int cnt, int lane, const LaneConsts& LC) {
+// Local chain states of one round held in the stage at shared address `st`: lane i returns sum_{j<=i} K^(i-j) g_j over
+// the round's blocks (no carry-in); lanes >= cnt contribute g = 0.  s = request misalignment in tokens.  Lane l reads
+// vector 32 it + l (conflict-free) and, for a misaligned request, the vector after it: no shuffle realigns anything.
+__device__ __forceinline__ unsigned long long round_local_scan(uint32_t st, int s, int cnt, int lane, const LaneConsts& LC) {
   unsigned long long part[4];
 #pragma unroll
   for (int it = 0; it < 4; ++it) {
-    const uint4 v = cur.v[it];
-    const uint4 w = (it < 3) ? cur.v[it + 1] : cur.x;     // lane 0's copy is what lane 31 needs
-    uint32_t a, b, c2, d;
-    if (s == 0) { a = v.x; b = v.y; c2 = v.z; d = v.w; }
-    else if (s == 1) { a = v.y; b = v.z; c2 = v.w; d = next_word(v.x, w.x, lane); }
-    else if (s == 2) { a = v.z; b = v.w; c2 = next_word(v.x, w.x, lane); d = next_word(v.y, w.y, lane); }
-    else { a = v.w; b = next_word(v.x, w.x, lane); c2 = next_word(v.y, w.y, lane); d = next_word(v.z, w.z, lane); }
+    const uint32_t at = st + 16u * (uint32_t)(it * 32 + lane);
+    const uint4 v = lds128(at);
+    uint32_t a = v.x, b = v.y, c2 = v.z, d = v.w;
+    if (s) {
+      const uint4 w = lds128(at + 16u);
+      if (s == 1) { a = v.y; b = v.z; c2 = v.w; d = w.x; }
+      else if (s == 2) { a = v.z; b = v.w; c2 = w.x; d = w.y; }
+      else { a = v.w; b = w.x; c2 = w.y; d = w.z; }
+    }
     // fold((w + (k+1) M) C1) = fold(w C1 + (k+1) M C1)
     const unsigned long long e0 = ((unsigned long long)a | ((unsigned long long)b << 32)) * H_C1 + LC.salt0;
     const unsigned long long e1 = ((unsigned long long)c2 | ((unsigned long long)d << 32)) * H_C1 + LC.salt1;
@@ -152,44 +213,96 @@ __device__ __forceinline__ unsigned long long round_local_scan(const RoundVecs& 
   return warp_chain_scan(g, lane);
 }
 
+// One run of nbs consecutive blocks starting at absolute token index ts (a request, or a segment of one), hashed by one
+// warp through its stage ring.  emit(rb, cnt, st): lane l < cnt holds the chain state st of block rb + l of the run.
+// Returns the state after the run's last block.
+template <typename Emit>
+__device__ __forceinline__ unsigned long long hash_run(WarpPipe& W, const uint32_t* __restrict__ tok, int base_mis, int64_t lo, int64_t hi,
+                                                       int64_t ts, int64_t nbs, unsigned long long carry, int lane, const LaneConsts& LC,
+                                                       Emit emit) {
+  const int s = (int)((base_mis + ts) & 3);          // tokens of the run's start past a 16-byte boundary (same for every round)
+  const int64_t va = ts - s;                         // absolute token index of the aligned cover of round 0
+  const int64_t rounds = (nbs + 31) >> 5;
+  auto n_vec = [&](int64_t r) { return (int)((16 * min((int64_t)32, nbs - 32 * r) + s + 3) >> 2); };
+  int64_t issued = 0;
+  for (; issued < rounds && issued < K1_STAGES - 1; ++issued) pipe_issue(W, (int)issued, tok, va + 512 * issued, n_vec(issued), lane, lo, hi);
+  int k = 0, kn = K1_STAGES - 1;                     // stage of the round being hashed / of the next round to issue
+  for (int64_t r = 0; r < rounds; ++r) {
+    if (issued < rounds) {                           // the stage hashed last round is free: every lane has its words in registers
+      pipe_issue(W, kn, tok, va + 512 * issued, n_vec(issued), lane, lo, hi);
+      ++issued;
+      kn = (kn + 1 == K1_STAGES) ? 0 : kn + 1;
+    }
+    pipe_wait(W, k);
+    const int cnt = (int)min((int64_t)32, nbs - 32 * r);
+    const unsigned long long st = round_local_scan(W.stage0 + (uint32_t)(k * K1_STAGE_BYTES), s, cnt, lane, LC) + LC.kp * carry;
+    emit(32 * r, cnt, st);
+    carry = shfl64(st, cnt - 1);
+    __syncwarp();                                    // all lanes are done with stage k before it is filled again
+    k = (k + 1 == K1_STAGES) ? 0 : k + 1;
+  }
+  return carry;
+}
+
 // Length classes for the ticket passes: requests of at least K1_CLASS_MIN[c] blocks are started in pass c, so the
 // longest chains start first and the short requests fill the tail of the launch (longest-processing-time-first).
 constexpr int K1_PASSES = 4;
 __device__ __forceinline__ int k1_class(int64_t nb) { return nb >= 1024 ? 0 : nb >= 384 ? 1 : nb >= 128 ? 2 : 3; }
 
+// The last warp of a launch to leave puts the work ticket back to 0 (ticket[0] = ticket, ticket[1] = warps that left):
+// no reset kernel, and the ticket of a handle or of a caller's scratch is always 0 between launches.
+__device__ __forceinline__ void k1_leave(uint32_t* ticket, int lane) {
+  if (lane == 0) {
+    __threadfence();
+    const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
+    if (atomicAdd(ticket + 1, 1u) == n_warps - 1) { ticket[1] = 0; __threadfence(); ticket[0] = 0; }
+  }
+}
+
 // ACCESS_ORDER = true writes keys at blk_off[r] + (nb-1-i) (the order K3 consumes, R2); false writes natural
-// order (arc_hash_blocks).  ticket: device counter, 0 at launch, reset by the caller's stream work; it runs over
-// K1_PASSES * n_req values: ticket t is request t % n_req in pass t / n_req.
+// order (arc_hash_blocks).  ticket: two device words, 0 at launch (see k1_leave); it runs over K1_PASSES * n_req values:
+// ticket t is request t % n_req in pass t / n_req.
 // CHAIN = true reads each request's initial H4 state from chain_in (NULL = S0) and writes its final state to chain_out
 // (arc_step / arc_step_resume); false is the stateless arc_hash_blocks, which pays nothing for it.
-template <bool ACCESS_ORDER, bool CHAIN>
-__global__ void __launch_bounds__(256, 4) hash_blocks_kernel(const int32_t* __restrict__ tokens, const int64_t* __restrict__ offsets,
-                                                         const int64_t* __restrict__ blk_off, uint32_t n_req,
-                                                         unsigned long long* __restrict__ keys, uint32_t* __restrict__ ticket, uint32_t batch,
+// ACAP > 0: the offsets come as the kernel argument `arg` (steps of up to ACAP requests: a launch costs less than the copy
+// engine's round trip, and the step's first kernel waits for nothing) and CTA 0 also stores them to offsets_g / blk_off_g
+// for the kernels that follow; ACAP = 0: they are read from those arrays.  Two argument sizes are built: 253 requests
+// (4 KB, the classic parameter limit) and 1,999 requests (32 KB, the large-parameter limit of CUDA 12.1+ on sm_70+).
+constexpr uint32_t K1_INLINE_SMALL = 253, K1_INLINE_LARGE = 1999;
+template <int CAP> struct OffsetsArgT { long long v[2 * (CAP + 1)]; };   // offsets[n_req + 1] then blk_off[n_req + 1]
+constexpr uint32_t K1_TICKET_BATCH = 2;
+
+template <bool ACCESS_ORDER, bool CHAIN, int ACAP>
+__global__ void __launch_bounds__(256, 3) hash_blocks_kernel(const int32_t* __restrict__ tokens, int64_t* __restrict__ offsets_g,
+                                                         int64_t* __restrict__ blk_off_g, uint32_t n_req,
+                                                         unsigned long long* __restrict__ keys, uint32_t* __restrict__ ticket,
                                                          const unsigned long long* __restrict__ chain_in,
-                                                         unsigned long long* __restrict__ chain_out) {
+                                                         unsigned long long* __restrict__ chain_out,
+                                                         const __grid_constant__ OffsetsArgT<ACAP> arg) {
+  extern __shared__ __align__(128) unsigned char k1_smem[];
   const int lane = threadIdx.x & 31;
+  constexpr bool ARG = ACAP > 0;
+  const long long* offsets = ARG ? arg.v : reinterpret_cast<const long long*>(offsets_g);
+  const long long* blk_off = ARG ? arg.v + (n_req + 1) : reinterpret_cast<const long long*>(blk_off_g);
+  if (ARG && blockIdx.x == 0)
+    for (uint32_t i = threadIdx.x; i <= n_req; i += blockDim.x) { offsets_g[i] = arg.v[i]; blk_off_g[i] = arg.v[n_req + 1 + i]; }
   const uint32_t* tok = reinterpret_cast<const uint32_t*>(tokens);
   const int64_t lo = offsets[0], hi = offsets[n_req];
-  LaneConsts LC;
-  const int q = lane & 3;
-  LC.salt0 = (unsigned long long)(2 * q + 1) * H_M * H_C1;
-  LC.salt1 = (unsigned long long)(2 * q + 2) * H_M * H_C1;
-  LC.kp = kpow_small(lane + 1);
-  LC.owner = 4 * (lane & 7) + (lane >> 3);
+  const LaneConsts LC = lane_consts(lane);
+  WarpPipe W = pipe_init(k1_smem, threadIdx.x >> 5, lane);
   const int base_mis = (int)((reinterpret_cast<uintptr_t>(tok) >> 2) & 3);   // tokens of the buffer start past a 16-byte boundary
   const unsigned long long total = (unsigned long long)K1_PASSES * n_req;
 
   for (;;) {
-    // `batch` (<= 32) tickets per atomic: lane l < batch examines ticket t0 + l, the warp then hashes the ones that belong to the pass
+    // K1_TICKET_BATCH tickets per atomic: lane l < batch examines ticket t0 + l, the warp then hashes the ones that belong to the pass
     uint32_t t0 = 0;
-    if (lane == 0) t0 = atomicAdd(ticket, batch);
+    if (lane == 0) t0 = atomicAdd(ticket, K1_TICKET_BATCH);
     t0 = __shfl_sync(0xFFFFFFFFu, t0, 0);
     if (t0 >= total) break;
     const unsigned long long t = (unsigned long long)t0 + lane;
     bool mine = false;
     uint32_t my_r = 0;
-    if (t < total && (uint32_t)lane < batch) {
+    if (t < total && (uint32_t)lane < K1_TICKET_BATCH) {
       my_r = (uint32_t)(t % n_req);
       const int64_t nb = blk_off[my_r + 1] - blk_off[my_r];
       mine = nb > 0 && k1_class(nb) == (int)(t / n_req);
@@ -202,75 +315,43 @@ __global__ void __launch_bounds__(256, 4) hash_blocks_kernel(const int32_t* __re
       todo &= todo - 1;
       const uint32_t r = __shfl_sync(0xFFFFFFFFu, my_r, src);
       const int64_t o = blk_off[r], nb = blk_off[r + 1] - o;
-      const int64_t ts = offsets[r];
-      const int s = (int)((base_mis + ts) & 3);          // tokens of the request's start past a 16-byte boundary (same for every round)
-      unsigned long long carry = (CHAIN && chain_in) ? chain_in[r] : H_S0;     // the H4 state before block 0 (a prompt: S0)
-      const int64_t va = ts - s;                         // absolute token index of the aligned cover of round 0
-      // two register buffers ping-pong (no copies): the loads of round i+1 are in flight while round i is hashed
-      auto n_vec = [&](int64_t rb) { return (int)((16 * min((int64_t)32, nb - rb) + s + 3) >> 2); };
-      auto finish = [&](const RoundVecs& cur, int64_t rb) {
-        const int cnt = (int)min((int64_t)32, nb - rb);
-        const unsigned long long st = round_local_scan(cur, s, cnt, lane, LC) + LC.kp * carry;
-        if (lane < cnt) {
-          const int64_t i = rb + lane;
-          keys[ACCESS_ORDER ? (o + (nb - 1 - i)) : (o + i)] = finalize_key(st);
-          if (CHAIN && i == nb - 1) chain_out[r] = st;           // the state a continuation of this sequence starts from
-        }
-        carry = shfl64(st, 31);
-      };
-      RoundVecs A = load_round(tok, va, n_vec(0), lane, lo, hi), B;
-      for (int64_t rb = 0;;) {
-        if (rb + 32 < nb) B = load_round(tok, va + 16 * (rb + 32), n_vec(rb + 32), lane, lo, hi);
-        finish(A, rb);
-        rb += 32;
-        if (rb >= nb) break;
-        if (rb + 32 < nb) A = load_round(tok, va + 16 * (rb + 32), n_vec(rb + 32), lane, lo, hi);
-        finish(B, rb);
-        rb += 32;
-        if (rb >= nb) break;
-      }
+      const unsigned long long c0 = (CHAIN && chain_in) ? chain_in[r] : H_S0;     // the H4 state before block 0 (a prompt: S0)
+      const unsigned long long end = hash_run(W, tok, base_mis, lo, hi, offsets[r], nb, c0, lane, LC,
+        [&](int64_t rb, int cnt, unsigned long long st) {
+          if (lane < cnt) { const int64_t i = rb + lane; keys[ACCESS_ORDER ? (o + (nb - 1 - i)) : (o + i)] = finalize_key(st); }
+        });
+      if (CHAIN && lane == 0) chain_out[r] = end;                                 // the state a continuation of this sequence starts from
     }
   }
+  k1_leave(ticket, lane);
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
 // In-step hashing of steps with FEW requests: one warp per request leaves the step waiting for its longest request (a
 // 1,000-block document is 32 dependent rounds).  H4 is affine, so a request is cut into segments of K1_SEG blocks that are
-// scanned independently from a zero carry (hash_segments_kernel: one warp per segment, the same loads and scans as
+// scanned independently from a zero carry (hash_segments_kernel: one warp per segment, the same staging and scans as
 // above) and put together afterwards (hash_fixup_kernel): with c_s the true state before segment s and E_s the local end
 // state of the segment, c_{s+1} = E_s + K^len_s c_s, and block i of the segment has state local_i + K^(i+1) c_s.
-// Steps with up to K1_INLINE_REQ requests hand their offsets and block offsets to the device as a kernel argument: a launch
-// costs a few microseconds less than the copy engine's round trip, and the step's first kernel waits for them.
-constexpr uint32_t K1_INLINE_REQ = 253;
-struct OffsetsArg { long long v[2 * (K1_INLINE_REQ + 1)]; };       // offsets[n_req + 1] then blk_off[n_req + 1]: 4,064 bytes
-__global__ void __launch_bounds__(256) store_offsets_kernel(const __grid_constant__ OffsetsArg a, uint32_t n_req, int64_t* offsets, int64_t* blk_off) {
-  for (uint32_t i = threadIdx.x; i <= n_req; i += blockDim.x) { offsets[i] = a.v[i]; blk_off[i] = a.v[n_req + 1 + i]; }
-}
-
 constexpr int K1_SEG = 128;
 
 // states[] gets the LOCAL states, in access order (index blk_off[r] + nb - 1 - i); seg_end[r * max_seg + s] = E_s.
-// ARG = true: the offsets come as the kernel argument `arg` (steps of up to K1_INLINE_REQ requests) and CTA 0 also stores
-// them to offsets_g / blk_off_g for the kernels that follow; false: they are read from those arrays.
-template <bool ARG>
-__global__ void __launch_bounds__(256, 4) hash_segments_kernel(const int32_t* __restrict__ tokens, int64_t* __restrict__ offsets_g,
+template <int ACAP>
+__global__ void __launch_bounds__(256, 3) hash_segments_kernel(const int32_t* __restrict__ tokens, int64_t* __restrict__ offsets_g,
                                                                int64_t* __restrict__ blk_off_g, uint32_t n_req, uint32_t max_seg,
                                                                unsigned long long* __restrict__ states,
                                                                unsigned long long* __restrict__ seg_end, uint32_t* __restrict__ ticket,
-                                                               const __grid_constant__ OffsetsArg arg) {
+                                                               const __grid_constant__ OffsetsArgT<ACAP> arg) {
+  extern __shared__ __align__(128) unsigned char k1_smem[];
   const int lane = threadIdx.x & 31;
+  constexpr bool ARG = ACAP > 0;
   const long long* offsets = ARG ? arg.v : reinterpret_cast<const long long*>(offsets_g);
   const long long* blk_off = ARG ? arg.v + (n_req + 1) : reinterpret_cast<const long long*>(blk_off_g);
   if (ARG && blockIdx.x == 0)
     for (uint32_t i = threadIdx.x; i <= n_req; i += blockDim.x) { offsets_g[i] = arg.v[i]; blk_off_g[i] = arg.v[n_req + 1 + i]; }
   const uint32_t* tok = reinterpret_cast<const uint32_t*>(tokens);
   const int64_t lo = offsets[0], hi = offsets[n_req];
-  LaneConsts LC;
-  const int q = lane & 3;
-  LC.salt0 = (unsigned long long)(2 * q + 1) * H_M * H_C1;
-  LC.salt1 = (unsigned long long)(2 * q + 2) * H_M * H_C1;
-  LC.kp = kpow_small(lane + 1);
-  LC.owner = 4 * (lane & 7) + (lane >> 3);
+  const LaneConsts LC = lane_consts(lane);
+  WarpPipe W = pipe_init(k1_smem, threadIdx.x >> 5, lane);
   const int base_mis = (int)((reinterpret_cast<uintptr_t>(tok) >> 2) & 3);
   const unsigned long long total = (unsigned long long)max_seg * n_req;
   for (;;) {
@@ -279,38 +360,17 @@ __global__ void __launch_bounds__(256, 4) hash_segments_kernel(const int32_t* __
     t0 = __shfl_sync(0xFFFFFFFFu, t0, 0);
     if (t0 >= total) break;
     const uint32_t r = t0 % n_req, sg = t0 / n_req;                 // ticket t = segment t / n_req of request t % n_req
-    if ((int64_t)sg * K1_SEG >= blk_off[r + 1] - blk_off[r]) continue;
-    {
-      const int64_t o = blk_off[r], nb = blk_off[r + 1] - o;
-      const int64_t b0 = (int64_t)sg * K1_SEG, nbs = min((int64_t)K1_SEG, nb - b0);
-      const int64_t ts = offsets[r] + 16 * b0;
-      const int s = (int)((base_mis + ts) & 3);
-      const int64_t va = ts - s;
-      unsigned long long carry = 0;
-      auto n_vec = [&](int64_t rb) { return (int)((16 * min((int64_t)32, nbs - rb) + s + 3) >> 2); };
-      auto finish = [&](const RoundVecs& cur, int64_t rb) {
-        const int cnt = (int)min((int64_t)32, nbs - rb);
-        const unsigned long long st = round_local_scan(cur, s, cnt, lane, LC) + LC.kp * carry;
-        if (lane < cnt) {
-          const int64_t i = b0 + rb + lane;
-          states[o + (nb - 1 - i)] = st;
-          if (rb + lane == nbs - 1) seg_end[(size_t)r * max_seg + sg] = st;
-        }
-        carry = shfl64(st, 31);
-      };
-      RoundVecs A = load_round(tok, va, n_vec(0), lane, lo, hi), B;
-      for (int64_t rb = 0;;) {
-        if (rb + 32 < nbs) B = load_round(tok, va + 16 * (rb + 32), n_vec(rb + 32), lane, lo, hi);
-        finish(A, rb);
-        rb += 32;
-        if (rb >= nbs) break;
-        if (rb + 32 < nbs) A = load_round(tok, va + 16 * (rb + 32), n_vec(rb + 32), lane, lo, hi);
-        finish(B, rb);
-        rb += 32;
-        if (rb >= nbs) break;
-      }
-    }
+    const int64_t o = blk_off[r], nb = blk_off[r + 1] - o;
+    const int64_t b0 = (int64_t)sg * K1_SEG;
+    if (b0 >= nb) continue;
+    const int64_t nbs = min((int64_t)K1_SEG, nb - b0);
+    const unsigned long long end = hash_run(W, tok, base_mis, lo, hi, offsets[r] + 16 * b0, nbs, 0ull, lane, LC,
+      [&](int64_t rb, int cnt, unsigned long long st) {
+        if (lane < cnt) states[o + (nb - 1 - (b0 + rb + lane))] = st;
+      });
+    if (lane == 0) seg_end[(size_t)r * max_seg + sg] = end;
   }
+  k1_leave(ticket, lane);
 }
 
 // K^(128 m): square-and-multiply over the bits of m (m < 2^11)
@@ -376,9 +436,6 @@ __global__ void __launch_bounds__(256) hash_fixup_kernel(const int64_t* __restri
     }
   }
 }
-
-// the last thing on the stream after a hashing launch: the ticket returns to 0 for the next launch
-__global__ void reset_ticket_kernel(uint32_t* ticket) { *ticket = 0; }
 
 __global__ void fill_u64_kernel(unsigned long long* p, uint32_t n, unsigned long long v) {
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) p[i] = v;

@@ -2,6 +2,7 @@
 // Validates, sizes buffers from the host offsets, enqueues the kernels on the caller's stream and owns
 // all device buffers.  No torch types, no CPU fallback: every step of the path runs in the kernels.
 #include <algorithm>
+#include <atomic>
 #include <cstdarg>
 #include <cstddef>
 #include <cstdio>
@@ -25,7 +26,7 @@ using namespace arc;
 namespace {
 
 thread_local std::string g_create_error = "";
-uint64_t g_hash_launches = 0;
+std::atomic<uint64_t> g_hash_launches{0};
 
 constexpr int kStageSlots = 4;
 constexpr uint32_t kMaxReq = 1u << 20;
@@ -403,17 +404,67 @@ int validate_offsets(arc_cache* h, const int64_t* off, uint32_t n_req, uint32_t 
   return ARC_OK;
 }
 
-// K1 grid: persistent warps that take requests through the ticket; enough CTAs to fill the 148 SMs, never more
-// warps than requests.
-void launch_hash(const int32_t* d_tokens, const int64_t* d_offsets, const int64_t* d_blk_off, uint32_t n_req,
-                 unsigned long long* d_keys, uint32_t* d_ticket, bool access_order, cudaStream_t s,
-                 const unsigned long long* d_chain_in = nullptr, unsigned long long* d_chain_out = nullptr) {
-  const uint32_t blocks = grid_for(n_req, 8, 148 * 6);
-  static uint32_t batch = getenv("ARC_K1_BATCH") ? (uint32_t)atoi(getenv("ARC_K1_BATCH")) : 2u;
-  if (access_order)
-    hash_blocks_kernel<true, true><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, batch, d_chain_in, d_chain_out);
+// ---- K1 launches --------------------------------------------------------------------------------------------------
+// The hashing kernels stage tokens in dynamic shared memory (K1_SMEM_BYTES per CTA, above the 48 KB default): the
+// attribute is set once per process and device.
+enum { K1_ARG_NONE = 0, K1_ARG_SMALL = 1, K1_ARG_LARGE = 2 };
+struct K1HostArgs { OffsetsArgT<0> none; OffsetsArgT<K1_INLINE_SMALL> small; OffsetsArgT<K1_INLINE_LARGE> large; };
+
+cudaError_t k1_configure() {
+  static std::mutex mu;
+  static bool done[64] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
+  if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
+#define K1_ATTR(f) if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, K1_SMEM_BYTES)) != cudaSuccess) return e
+  K1_ATTR((hash_blocks_kernel<false, false, 0>));
+  K1_ATTR((hash_blocks_kernel<true, true, 0>));
+  K1_ATTR((hash_blocks_kernel<true, true, (int)K1_INLINE_SMALL>));
+  K1_ATTR((hash_blocks_kernel<true, true, (int)K1_INLINE_LARGE>));
+  K1_ATTR((hash_segments_kernel<0>));
+  K1_ATTR((hash_segments_kernel<(int)K1_INLINE_SMALL>));
+  K1_ATTR((hash_segments_kernel<(int)K1_INLINE_LARGE>));
+#undef K1_ATTR
+  if (dev >= 0 && dev < 64) done[dev] = true;
+  return cudaSuccess;
+}
+
+int k1_arg_mode(uint32_t n_req) { return n_req <= K1_INLINE_SMALL ? K1_ARG_SMALL : (n_req <= K1_INLINE_LARGE ? K1_ARG_LARGE : K1_ARG_NONE); }
+
+// offsets[n_req + 1] and blk_off[n_req + 1] side by side in the argument of the right size
+void k1_fill_args(K1HostArgs& A, int mode, const int64_t* off, const int64_t* blk_off, uint32_t n_req) {
+  long long* v = (mode == K1_ARG_SMALL) ? A.small.v : A.large.v;
+  memcpy(v, off, ((size_t)n_req + 1) * sizeof(int64_t));
+  memcpy(v + n_req + 1, blk_off, ((size_t)n_req + 1) * sizeof(int64_t));
+}
+
+// K1 grid: persistent warps that take requests through the ticket; enough CTAs to fill the 148 SMs three deep, never more
+// warps than requests.  step = true: keys in access order, chain states in and out (arc_step); false: arc_hash_blocks.
+void launch_hash_blocks(bool step, int mode, const K1HostArgs& A, const int32_t* d_tokens, int64_t* d_offsets, int64_t* d_blk_off,
+                        uint32_t n_req, unsigned long long* d_keys, uint32_t* d_ticket, cudaStream_t s,
+                        const unsigned long long* d_chain_in, unsigned long long* d_chain_out) {
+  const uint32_t blocks = grid_for(n_req, K1_WARPS, 148 * 3);
+  if (!step)
+    hash_blocks_kernel<false, false, 0><<<blocks, 256, K1_SMEM_BYTES, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, nullptr, nullptr, A.none);
+  else if (mode == K1_ARG_SMALL)
+    hash_blocks_kernel<true, true, (int)K1_INLINE_SMALL><<<blocks, 256, K1_SMEM_BYTES, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, d_chain_in, d_chain_out, A.small);
+  else if (mode == K1_ARG_LARGE)
+    hash_blocks_kernel<true, true, (int)K1_INLINE_LARGE><<<blocks, 256, K1_SMEM_BYTES, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, d_chain_in, d_chain_out, A.large);
   else
-    hash_blocks_kernel<false, false><<<blocks, 256, 0, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, batch, d_chain_in, d_chain_out);
+    hash_blocks_kernel<true, true, 0><<<blocks, 256, K1_SMEM_BYTES, s>>>(d_tokens, d_offsets, d_blk_off, n_req, d_keys, d_ticket, d_chain_in, d_chain_out, A.none);
+}
+
+void launch_hash_segments(int mode, const K1HostArgs& A, const int32_t* d_tokens, int64_t* d_offsets, int64_t* d_blk_off, uint32_t n_req,
+                          uint32_t max_seg, unsigned long long* d_states, unsigned long long* d_seg_end, uint32_t* d_ticket, cudaStream_t s) {
+  const uint32_t g = grid_for((uint64_t)n_req * max_seg, K1_WARPS, 148 * 3);
+  if (mode == K1_ARG_SMALL)
+    hash_segments_kernel<(int)K1_INLINE_SMALL><<<g, 256, K1_SMEM_BYTES, s>>>(d_tokens, d_offsets, d_blk_off, n_req, max_seg, d_states, d_seg_end, d_ticket, A.small);
+  else if (mode == K1_ARG_LARGE)
+    hash_segments_kernel<(int)K1_INLINE_LARGE><<<g, 256, K1_SMEM_BYTES, s>>>(d_tokens, d_offsets, d_blk_off, n_req, max_seg, d_states, d_seg_end, d_ticket, A.large);
+  else
+    hash_segments_kernel<0><<<g, 256, K1_SMEM_BYTES, s>>>(d_tokens, d_offsets, d_blk_off, n_req, max_seg, d_states, d_seg_end, d_ticket, A.none);
 }
 
 }  // namespace
@@ -433,6 +484,12 @@ int arc_create(uint64_t capacity_blocks, uint32_t block_size, int policy, arc_ca
   cudaError_t e = cudaGetDevice(&h->device);
   if (e != cudaSuccess) {
     int rc = fail(nullptr, ARC_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    delete h;
+    return rc;
+  }
+  e = k1_configure();
+  if (e != cudaSuccess) {
+    int rc = fail(nullptr, ARC_ERR_CUDA, "K1 configuration: %s", cudaGetErrorString(e));
     delete h;
     return rc;
   }
@@ -493,24 +550,20 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
   for (uint32_t r = 0; r < n_req; ++r) max_nb = std::max<uint64_t>(max_nb, (uint64_t)(blk_off[r + 1] - blk_off[r]));
   const uint32_t max_seg = (uint32_t)((max_nb + K1_SEG - 1) / K1_SEG);
   const bool segmented = N && n_req <= kSegMaxReq && max_seg >= 2 && max_seg <= 1024 && (uint64_t)n_req * max_seg <= kSegEndCap;
-  static thread_local OffsetsArg off_arg;
-  const bool inline_off = n_req <= K1_INLINE_REQ;      // small enough for a kernel argument: no copy-engine round trip, no staging
-  if (inline_off) {
-    memcpy(off_arg.v, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
-    memcpy(off_arg.v + n_req + 1, blk_off.data(), ((size_t)n_req + 1) * sizeof(int64_t));
-    if (!segmented) {                                  // the segmented K1 takes the argument itself and stores the arrays
-      store_offsets_kernel<<<1, 256, 0, s>>>(off_arg, n_req, h->d_offsets, h->d_offsets + (h->req_cap + 1));
-      h->launches += 1;
-    }
+  static thread_local K1HostArgs k1_args;
+  const int arg_mode = N ? k1_arg_mode(n_req) : K1_ARG_NONE;   // small enough for a kernel argument: no copy-engine round trip, no staging
+  if (arg_mode != K1_ARG_NONE) {
+    k1_fill_args(k1_args, arg_mode, h_offsets, blk_off.data(), n_req);   // K1 takes the argument and stores the arrays for K3 / K4
   } else {
-  const int slot = h->stage_next;
-  h->stage_next = (slot + 1) % kStageSlots;
-  CUDA_TRY(h, cudaEventSynchronize(h->stage_done[slot]));
-  int64_t* stage = h->h_stage + (size_t)slot * 2 * ((size_t)h->req_cap + 1);
-  memcpy(stage, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
-  memcpy(stage + (h->req_cap + 1), blk_off.data(), ((size_t)n_req + 1) * sizeof(int64_t));
-  CUDA_TRY(h, cudaMemcpyAsync(h->d_offsets, stage, 2 * ((size_t)h->req_cap + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, s));
-  CUDA_TRY(h, cudaEventRecord(h->stage_done[slot], s));
+    const int slot = h->stage_next;
+    h->stage_next = (slot + 1) % kStageSlots;
+    CUDA_TRY(h, cudaEventSynchronize(h->stage_done[slot]));
+    int64_t* stage = h->h_stage + (size_t)slot * 2 * ((size_t)h->req_cap + 1);
+    memcpy(stage, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
+    memcpy(stage + (h->req_cap + 1), blk_off.data(), ((size_t)n_req + 1) * sizeof(int64_t));
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_offsets, stage, ((size_t)n_req + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_offsets + (h->req_cap + 1), stage + (h->req_cap + 1), ((size_t)n_req + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaEventRecord(h->stage_done[slot], s));
   }
 
   StepParams P = make_params(h);
@@ -519,16 +572,14 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
     if (segmented) {
       // K1, few long requests: segments hashed independently, then put together (hash_kernels.cuh)
       if (!h->d_seg_end) CUDA_TRY(h, dalloc(&h->d_seg_end, kSegEndCap));
-      int64_t* d_off = h->d_offsets; int64_t* d_boff = h->d_offsets + (h->req_cap + 1);
-      const uint32_t g = grid_for((uint64_t)n_req * max_seg, 8, 148 * 4);
-      if (inline_off) hash_segments_kernel<true><<<g, 256, 0, s>>>(d_tokens, d_off, d_boff, n_req, max_seg, P.keys_acc, h->d_seg_end, &h->d_state->k1_ticket, off_arg);
-      else hash_segments_kernel<false><<<g, 256, 0, s>>>(d_tokens, d_off, d_boff, n_req, max_seg, P.keys_acc, h->d_seg_end, &h->d_state->k1_ticket, off_arg);
+      launch_hash_segments(arg_mode, k1_args, d_tokens, h->d_offsets, h->d_offsets + (h->req_cap + 1), n_req, max_seg, P.keys_acc, h->d_seg_end,
+                           &h->d_state->k1_ticket, s);
       hash_fixup_kernel<<<grid_for((uint64_t)n_req * max_seg, 8, 148 * 4), 256, 0, s>>>(P.blk_off, n_req, max_seg, P.keys_acc, h->d_seg_end,
                                                                     reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state);
       h->launches += 1;
     } else {
-      launch_hash(d_tokens, P.offsets, P.blk_off, n_req, P.keys_acc, &h->d_state->k1_ticket, true, s,               // K1
-                  reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state);
+      launch_hash_blocks(true, arg_mode, k1_args, d_tokens, h->d_offsets, h->d_offsets + (h->req_cap + 1), n_req, P.keys_acc,   // K1
+                         &h->d_state->k1_ticket, s, reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state);
     }
     if (h->profiling) cudaEventRecord(h->ev[2], s);
     probe_reserve_kernel<<<grid_for(N, 256 * PROBE_ILP, 148 * 8), 256, 0, s>>>(P);                        // K2
@@ -609,7 +660,7 @@ int arc_step_host(arc_cache* h, const int32_t* h_tokens, const int64_t* h_offset
   out->n_alloc = (uint32_t)h_counts[0]; out->n_evict = (uint32_t)h_counts[1];
   out->prefix_len = hp; out->alloc_ids = h_alloc; out->evict_ids = h_evict;
   out->h2d_bytes = (uint64_t)total * sizeof(int32_t) +
-                   2 * ((uint64_t)(n_req <= K1_INLINE_REQ ? n_req : h->req_cap) + 1) * sizeof(int64_t);   // offsets: kernel argument or staged copy
+                   2 * ((uint64_t)n_req + 1) * sizeof(int64_t);   // offsets and block offsets: kernel argument or staged copy
   out->d2h_bytes = ((uint64_t)h->req_cap + 2 + (N ? h->n_cap + N : 0)) * sizeof(int32_t);
   return ARC_OK;
 }
@@ -669,52 +720,104 @@ void arc_destroy(arc_cache* h) {
 
 const char* arc_last_error(const arc_cache* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
+// Scratch of the stateless hashing entry: a small ring of slots, each with a pinned host buffer, a device buffer
+// (ticket words, offsets, block offsets) and two events.  A call takes the next slot, fills it, copies it on the library's
+// own copy stream (so the copy overlaps whatever the caller's stream is still doing) and makes the caller's stream wait
+// for that copy; the slot is reused only after the kernel that read it has finished.  Calls on different streams or
+// threads therefore never share scratch, and a call moves 16 + 16 (n_req + 1) bytes, not a fixed capacity.
+namespace {
+struct HashSlot {
+  int64_t* h_buf = nullptr; int64_t* d_buf = nullptr; size_t cap = 0;     // cap in int64 entries
+  cudaEvent_t copied = nullptr, done = nullptr;
+};
+struct HashScratch {
+  std::mutex mu;
+  HashSlot slot[8];
+  int next = 0;
+  cudaStream_t copy_stream = nullptr;
+  int device = -1;
+};
+HashScratch g_hash;
+}  // namespace
+
 int arc_hash_blocks(const int32_t* d_tokens, const int64_t* h_offsets, uint32_t n_req, uint32_t block_size, uint64_t* d_keys_out, void* cuda_stream) {
   if (!h_offsets) return fail(nullptr, ARC_ERR_INVALID_ARG, "h_offsets is NULL");
   if (n_req > kMaxReq) return fail(nullptr, ARC_ERR_INVALID_ARG, "n_req > 2^20");
   if (block_size != 16) return fail(nullptr, ARC_ERR_UNSUPPORTED, "block_size %u: only 16 is built", block_size);
   cudaStream_t s = (cudaStream_t)cuda_stream;
-  // process-wide scratch for the offsets (grow-only); calls are serialised by the mutex and each call
-  // waits for the previous one's copy before reusing the pinned staging area
-  static std::mutex mu;
-  static int64_t* d_off = nullptr;
-  static int64_t* h_off = nullptr;
-  static uint32_t cap = 0;
-  static uint32_t* d_ticket = nullptr;
-  static cudaEvent_t copied = nullptr;
-  std::lock_guard<std::mutex> lock(mu);
-  if (n_req + 1 > cap) {
-    cudaDeviceSynchronize();
-    if (d_off) cudaFree(d_off);
-    if (h_off) cudaFreeHost(h_off);
-    cap = pow2_at_least((uint64_t)n_req + 1);
-    if (cudaMalloc((void**)&d_off, 2 * (size_t)cap * sizeof(int64_t)) != cudaSuccess ||
-        cudaMallocHost((void**)&h_off, 2 * (size_t)cap * sizeof(int64_t)) != cudaSuccess) {
-      cap = 0; d_off = nullptr; h_off = nullptr;
+  static thread_local std::vector<int64_t> blk_off;
+  blk_off.resize((size_t)n_req + 1);
+  uint64_t N = 0;
+  int rc = validate_offsets(nullptr, h_offsets, n_req, block_size, 0, blk_off.data(), &N);
+  if (rc) return rc;
+  if (N && (!d_tokens || !d_keys_out)) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
+  if (!N) return ARC_OK;
+  cudaError_t e = k1_configure();
+  if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "K1 configuration: %s", cudaGetErrorString(e));
+  int dev = 0;
+  cudaGetDevice(&dev);
+  std::lock_guard<std::mutex> lock(g_hash.mu);
+  if (g_hash.device != dev) {                      // first use, or the caller moved to another device: start again there
+    if (g_hash.device >= 0) cudaDeviceSynchronize();
+    for (HashSlot& k : g_hash.slot) {
+      if (k.h_buf) cudaFreeHost(k.h_buf);
+      if (k.d_buf) cudaFree(k.d_buf);
+      if (k.copied) cudaEventDestroy(k.copied);
+      if (k.done) cudaEventDestroy(k.done);
+      k = HashSlot();
+    }
+    if (g_hash.copy_stream) cudaStreamDestroy(g_hash.copy_stream);
+    g_hash.copy_stream = nullptr;
+    if (cudaStreamCreateWithFlags(&g_hash.copy_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "copy stream");
+    g_hash.device = dev;
+  }
+  HashSlot& k = g_hash.slot[g_hash.next];
+  g_hash.next = (g_hash.next + 1) % 8;
+  if (!k.copied) { cudaEventCreateWithFlags(&k.copied, cudaEventDisableTiming); cudaEventCreateWithFlags(&k.done, cudaEventDisableTiming); }
+  const size_t need = 2 + 2 * ((size_t)n_req + 1);                 // two ticket words (one int64), padding, offsets, block offsets
+  cudaEventSynchronize(k.done);                                     // the kernel that read this slot last has finished
+  if (need > k.cap) {
+    if (k.h_buf) cudaFreeHost(k.h_buf);
+    if (k.d_buf) cudaFree(k.d_buf);
+    k.cap = std::max<size_t>(need, 1024);
+    if (cudaMallocHost((void**)&k.h_buf, k.cap * sizeof(int64_t)) != cudaSuccess || cudaMalloc((void**)&k.d_buf, k.cap * sizeof(int64_t)) != cudaSuccess) {
+      if (k.h_buf) cudaFreeHost(k.h_buf);
+      k.h_buf = nullptr; k.d_buf = nullptr; k.cap = 0;
+      cudaGetLastError();
       return fail(nullptr, ARC_ERR_OOM, "scratch allocation failed");
     }
   }
-  if (!copied) cudaEventCreateWithFlags(&copied, cudaEventDisableTiming);
-  if (!d_ticket) {
-    if (cudaMalloc((void**)&d_ticket, sizeof(uint32_t)) != cudaSuccess) { d_ticket = nullptr; return fail(nullptr, ARC_ERR_OOM, "scratch allocation failed"); }
-    cudaMemset(d_ticket, 0, sizeof(uint32_t));
-  }
-  cudaEventSynchronize(copied);
-  uint64_t N = 0;
-  int rc = validate_offsets(nullptr, h_offsets, n_req, block_size, 0, h_off + cap, &N);
-  if (rc) return rc;
-  if (N && (!d_tokens || !d_keys_out)) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
-  memcpy(h_off, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
-  cudaError_t e = cudaMemcpyAsync(d_off, h_off, 2 * (size_t)cap * sizeof(int64_t), cudaMemcpyHostToDevice, s);
+  k.h_buf[0] = 0; k.h_buf[1] = 0;                                   // the ticket words travel with the offsets
+  memcpy(k.h_buf + 2, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
+  memcpy(k.h_buf + 2 + (n_req + 1), blk_off.data(), ((size_t)n_req + 1) * sizeof(int64_t));
+  e = cudaMemcpyAsync(k.d_buf, k.h_buf, need * sizeof(int64_t), cudaMemcpyHostToDevice, g_hash.copy_stream);
+  if (e == cudaSuccess) e = cudaEventRecord(k.copied, g_hash.copy_stream);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(s, k.copied, 0);
   if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "offset copy: %s", cudaGetErrorString(e));
-  cudaEventRecord(copied, s);
-  if (N) {
-    launch_hash(d_tokens, d_off, d_off + cap, n_req, (unsigned long long*)d_keys_out, d_ticket, false, s);
-    reset_ticket_kernel<<<1, 1, 0, s>>>(d_ticket);
-    g_hash_launches += 2;
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "hash launch: %s", cudaGetErrorString(e));
-  }
+  static const K1HostArgs no_args = {};
+  launch_hash_blocks(false, K1_ARG_NONE, no_args, d_tokens, k.d_buf + 2, k.d_buf + 2 + (n_req + 1), n_req, (unsigned long long*)d_keys_out,
+                     reinterpret_cast<uint32_t*>(k.d_buf), s, nullptr, nullptr);
+  g_hash_launches += 1;
+  e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaEventRecord(k.done, s);
+  if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "hash launch: %s", cudaGetErrorString(e));
+  return ARC_OK;
+}
+
+int arc_hash_blocks_device(const int32_t* d_tokens, const int64_t* d_offsets, const int64_t* d_blk_off, uint32_t n_req, uint32_t block_size,
+                           uint64_t* d_keys_out, uint32_t* d_ticket, void* cuda_stream) {
+  if (n_req > kMaxReq) return fail(nullptr, ARC_ERR_INVALID_ARG, "n_req > 2^20");
+  if (block_size != 16) return fail(nullptr, ARC_ERR_UNSUPPORTED, "block_size %u: only 16 is built", block_size);
+  if (!n_req) return ARC_OK;
+  if (!d_tokens || !d_offsets || !d_blk_off || !d_keys_out || !d_ticket) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
+  cudaError_t e = k1_configure();
+  if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "K1 configuration: %s", cudaGetErrorString(e));
+  static const K1HostArgs no_args = {};
+  launch_hash_blocks(false, K1_ARG_NONE, no_args, d_tokens, const_cast<int64_t*>(d_offsets), const_cast<int64_t*>(d_blk_off), n_req,
+                     (unsigned long long*)d_keys_out, d_ticket, (cudaStream_t)cuda_stream, nullptr, nullptr);
+  g_hash_launches += 1;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "hash launch: %s", cudaGetErrorString(e));
   return ARC_OK;
 }
 
@@ -738,7 +841,7 @@ int arc_last_kernel_times(arc_cache* h, arc_kernel_times* out) {
   return ARC_OK;
 }
 
-uint64_t arc_launch_count(const arc_cache* h) { return h ? h->launches : g_hash_launches; }
+uint64_t arc_launch_count(const arc_cache* h) { return h ? h->launches : g_hash_launches.load(); }
 
 int arc_set_machine(arc_cache* h, int which) {
   if (!h || which < 0 || which > 3) return ARC_ERR_INVALID_ARG;

@@ -90,6 +90,37 @@ def test_hash_parity_configs(arc, config):
         assert np.array_equal(got, want), (config, i)
 
 
+def test_hash_on_two_streams_and_from_device_offsets(arc):
+    """arc_hash_blocks keeps no shared scratch: calls on two streams that overlap (different request mixes, many calls in
+    flight, more than the scratch ring holds) all give the oracle's keys; arc_hash_blocks_device (offsets already on the
+    device, the caller's ticket scratch zeroed once) gives the same keys call after call."""
+    rng = np.random.default_rng(77)
+    jobs = []
+    for j in range(24):
+        n_req = int(rng.integers(1, 3000 if j % 3 == 0 else 40))
+        lens = rng.integers(0, 2000 if j % 2 else 300, size=n_req)
+        reqs = [rng.integers(0, 128000, size=int(n)).astype(np.int32) for n in lens]
+        tokens, offsets = W.pack_requests(reqs)
+        want, blk_off = O.hash_blocks(tokens, offsets)
+        jobs.append((dev(tokens), offsets, want, blk_off))
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    for j, (t, o, want, _) in enumerate(jobs):
+        outs.append(arc.hash_blocks(t, o, stream=(s1 if j % 2 else s2)))
+    torch.cuda.synchronize()
+    for (t, o, want, _), got in zip(jobs, outs):
+        assert np.array_equal(got.cpu().numpy().view(np.uint64), want)
+    ticket = torch.zeros(2, dtype=torch.int32, device="cuda")
+    for rep in range(2):
+        for t, o, want, blk_off in jobs[:8]:
+            if len(want) == 0:
+                continue
+            out = torch.empty(len(want), dtype=torch.int64, device="cuda")
+            arc.hash_blocks_device(t, torch.from_numpy(o).cuda(), torch.from_numpy(blk_off).cuda(), len(o) - 1, out, ticket)
+            assert np.array_equal(out.cpu().numpy().view(np.uint64), want)
+    assert int(ticket.abs().sum()) == 0
+
+
 # ------------------------------------------------------------------------------- whole arc_step
 
 @pytest.mark.parametrize("machine", [0, 1, 2, 3])
