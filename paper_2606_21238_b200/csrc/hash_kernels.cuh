@@ -51,14 +51,22 @@ __device__ __forceinline__ unsigned long long shfl64(unsigned long long v, int s
 __device__ __forceinline__ unsigned long long shfl_xor64(unsigned long long v, int m) { return __shfl_xor_sync(0xFFFFFFFFu, v, m); }
 __device__ __forceinline__ unsigned long long shfl_up64(unsigned long long v, int d) { return __shfl_up_sync(0xFFFFFFFFu, v, d); }
 
-// Inclusive warp scan of the affine chain: on return lane l holds sum_{j<=l} K^(l-j) g_j.
-__device__ __forceinline__ unsigned long long warp_chain_scan(unsigned long long g, int lane) {
-  unsigned long long s = g, up;
-  up = shfl_up64(s, 1);  if (lane >= 1)  s += kpow(1) * up;
-  up = shfl_up64(s, 2);  if (lane >= 2)  s += kpow(2) * up;
-  up = shfl_up64(s, 4);  if (lane >= 4)  s += kpow(4) * up;
-  up = shfl_up64(s, 8);  if (lane >= 8)  s += kpow(8) * up;
-  up = shfl_up64(s, 16); if (lane >= 16) s += kpow(16) * up;
+// Inclusive warp scan of the affine chain: on return lane l holds sum_{j<=l} K^(l-j) g_j.  sc[d] = K^(2^d) for the lanes
+// that take part in step d (lane >= 2^d) and 0 for the others: multiply-adds only, no branch, no select.
+struct ScanConsts { unsigned long long c[5]; };
+__device__ __forceinline__ ScanConsts scan_consts(int lane) {
+  ScanConsts S;
+  S.c[0] = lane >= 1 ? kpow(1) : 0ull; S.c[1] = lane >= 2 ? kpow(2) : 0ull; S.c[2] = lane >= 4 ? kpow(4) : 0ull;
+  S.c[3] = lane >= 8 ? kpow(8) : 0ull; S.c[4] = lane >= 16 ? kpow(16) : 0ull;
+  return S;
+}
+__device__ __forceinline__ unsigned long long warp_chain_scan(unsigned long long g, const ScanConsts& S) {
+  unsigned long long s = g;
+  s += S.c[0] * shfl_up64(s, 1);
+  s += S.c[1] * shfl_up64(s, 2);
+  s += S.c[2] * shfl_up64(s, 4);
+  s += S.c[3] * shfl_up64(s, 8);
+  s += S.c[4] * shfl_up64(s, 16);
   return s;
 }
 
@@ -119,7 +127,6 @@ struct WarpPipe {
   uint32_t stage0;      // shared address of this warp's first stage
   uint32_t bar0;        // shared address of this warp's first mbarrier
   uint32_t parity;      // bit k: the phase stage k's barrier completes next
-  uint32_t manual;      // bit k: stage k was filled by the warp itself (an edge round), no barrier to wait on
   unsigned long long policy;
 };
 
@@ -127,7 +134,7 @@ __device__ __forceinline__ WarpPipe pipe_init(unsigned char* smem, int warp, int
   WarpPipe W;
   W.stage0 = smem_u32(smem) + (uint32_t)(warp * K1_STAGES * K1_STAGE_BYTES);
   W.bar0 = smem_u32(smem) + (uint32_t)(K1_WARPS * K1_STAGES * K1_STAGE_BYTES + warp * K1_STAGES * 8);
-  W.parity = 0; W.manual = 0;
+  W.parity = 0;
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(W.policy));
   if (lane == 0) {
 #pragma unroll
@@ -152,12 +159,11 @@ __device__ __forceinline__ void pipe_issue(WarpPipe& W, int k, const uint32_t* _
       const uint4 v = ld_tokens4_guarded(tok, va + 4 * (int64_t)e, lo, hi);
       asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 16u * e), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
     }
-    W.manual |= 1u << k;
     __syncwarp();
+    if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(W.bar0 + 8u * k) : "memory");   // the phase completes as a copy's would
   }
 }
 __device__ __forceinline__ void pipe_wait(WarpPipe& W, int k) {
-  if (W.manual & (1u << k)) { W.manual &= ~(1u << k); return; }
   mbar_wait(W.bar0 + 8u * k, (W.parity >> k) & 1u);
   W.parity ^= 1u << k;
 }
@@ -171,6 +177,7 @@ struct LaneConsts {
   unsigned long long salt0, salt1;   // (k+1) M C1 for this lane's two words k = 2q, 2q+1 (the salt is folded into the multiply-add)
   unsigned long long kp;             // K^(lane+1)
   int owner;                         // after the transpose-reduce, block i of the round sits in lane `owner` of lane i
+  ScanConsts sc;
 };
 __device__ __forceinline__ LaneConsts lane_consts(int lane) {
   LaneConsts LC;
@@ -179,23 +186,25 @@ __device__ __forceinline__ LaneConsts lane_consts(int lane) {
   LC.salt1 = (unsigned long long)(2 * q + 2) * H_M * H_C1;
   LC.kp = kpow_small(lane + 1);
   LC.owner = 4 * (lane & 7) + (lane >> 3);
+  LC.sc = scan_consts(lane);
   return LC;
 }
 
 // Local chain states of one round held in the stage at shared address `st`: lane i returns sum_{j<=i} K^(i-j) g_j over
 // the round's blocks (no carry-in); lanes >= cnt contribute g = 0.  s = request misalignment in tokens.  Lane l reads
 // vector 32 it + l (conflict-free) and, for a misaligned request, the vector after it: no shuffle realigns anything.
-__device__ __forceinline__ unsigned long long round_local_scan(uint32_t st, int s, int cnt, int lane, const LaneConsts& LC) {
+template <int S>
+__device__ __forceinline__ unsigned long long round_local_scan(uint32_t st, int cnt, int lane, const LaneConsts& LC) {
   unsigned long long part[4];
 #pragma unroll
   for (int it = 0; it < 4; ++it) {
     const uint32_t at = st + 16u * (uint32_t)(it * 32 + lane);
     const uint4 v = lds128(at);
     uint32_t a = v.x, b = v.y, c2 = v.z, d = v.w;
-    if (s) {
+    if (S != 0) {
       const uint4 w = lds128(at + 16u);
-      if (s == 1) { a = v.y; b = v.z; c2 = v.w; d = w.x; }
-      else if (s == 2) { a = v.z; b = v.w; c2 = w.x; d = w.y; }
+      if (S == 1) { a = v.y; b = v.z; c2 = v.w; d = w.x; }
+      else if (S == 2) { a = v.z; b = v.w; c2 = w.x; d = w.y; }
       else { a = v.w; b = w.x; c2 = w.y; d = w.z; }
     }
     // fold((w + (k+1) M) C1) = fold(w C1 + (k+1) M C1)
@@ -210,38 +219,65 @@ __device__ __forceinline__ unsigned long long round_local_scan(uint32_t st, int 
   const unsigned long long g_own = (b1 ? pb : pa) + shfl_xor64(b1 ? pa : pb, 2);
   unsigned long long g = shfl64(g_own, LC.owner);      // lane i <- block i
   if (lane >= cnt) g = 0;
-  return warp_chain_scan(g, lane);
+  return warp_chain_scan(g, LC.sc);
 }
 
 // One run of nbs consecutive blocks starting at absolute token index ts (a request, or a segment of one), hashed by one
 // warp through its stage ring.  emit(rb, cnt, st): lane l < cnt holds the chain state st of block rb + l of the run.
-// Returns the state after the run's last block.
-template <typename Emit>
-__device__ __forceinline__ unsigned long long hash_run(WarpPipe& W, const uint32_t* __restrict__ tok, int base_mis, int64_t lo, int64_t hi,
-                                                       int64_t ts, int64_t nbs, unsigned long long carry, int lane, const LaneConsts& LC,
-                                                       Emit emit) {
-  const int s = (int)((base_mis + ts) & 3);          // tokens of the run's start past a 16-byte boundary (same for every round)
+// Returns the state after the run's last block.  Everything inside the round loop is 32-bit (nbs < 2^28).
+template <int S, typename Emit>
+__device__ __forceinline__ unsigned long long hash_run_s(WarpPipe& W, const uint32_t* __restrict__ tok, int64_t lo, int64_t hi,
+                                                         int64_t ts, uint32_t nbs, unsigned long long carry, int lane, const LaneConsts& LC,
+                                                         Emit emit) {
+  constexpr int s = S;                               // tokens of the run's start past a 16-byte boundary (same for every round)
   const int64_t va = ts - s;                         // absolute token index of the aligned cover of round 0
-  const int64_t rounds = (nbs + 31) >> 5;
-  auto n_vec = [&](int64_t r) { return (int)((16 * min((int64_t)32, nbs - 32 * r) + s + 3) >> 2); };
-  int64_t issued = 0;
-  for (; issued < rounds && issued < K1_STAGES - 1; ++issued) pipe_issue(W, (int)issued, tok, va + 512 * issued, n_vec(issued), lane, lo, hi);
+  const uint32_t rounds = (nbs + 31u) >> 5;
+  const uint32_t vec_full = (uint32_t)(512 + s + 3) >> 2, vec_last = (16u * (nbs - 32u * (rounds - 1)) + (uint32_t)s + 3u) >> 2;
+  // only the first and the last round of a run can reach outside the caller's buffer (the cover's few words before / after)
+  const bool head_in = va >= lo, tail_in = va + 512 * (int64_t)(rounds - 1) + 4 * (int64_t)vec_last <= hi;
+  const uint32_t* src = tok + va;                    // 16-byte aligned
+  auto issue = [&](uint32_t r, int k) {
+    const uint32_t nv = (r + 1 == rounds) ? vec_last : vec_full;
+    if ((r != 0 || head_in) && (r + 1 != rounds || tail_in)) {
+      if (lane == 0) {
+        mbar_expect_tx(W.bar0 + 8u * k, 16u * nv);
+        bulk_g2s(W.stage0 + (uint32_t)(k * K1_STAGE_BYTES), src + 512u * (size_t)r, 16u * nv, W.bar0 + 8u * k, W.policy);
+      }
+    } else {
+      pipe_issue(W, k, tok, va + 512 * (int64_t)r, (int)nv, lane, lo, hi);
+    }
+  };
+  uint32_t issued = 0;
+  for (; issued < rounds && issued < (uint32_t)(K1_STAGES - 1); ++issued) issue(issued, (int)issued);
   int k = 0, kn = K1_STAGES - 1;                     // stage of the round being hashed / of the next round to issue
-  for (int64_t r = 0; r < rounds; ++r) {
+  for (uint32_t r = 0; r < rounds; ++r) {
     if (issued < rounds) {                           // the stage hashed last round is free: every lane has its words in registers
-      pipe_issue(W, kn, tok, va + 512 * issued, n_vec(issued), lane, lo, hi);
+      issue(issued, kn);
       ++issued;
       kn = (kn + 1 == K1_STAGES) ? 0 : kn + 1;
     }
     pipe_wait(W, k);
-    const int cnt = (int)min((int64_t)32, nbs - 32 * r);
-    const unsigned long long st = round_local_scan(W.stage0 + (uint32_t)(k * K1_STAGE_BYTES), s, cnt, lane, LC) + LC.kp * carry;
-    emit(32 * r, cnt, st);
+    const int cnt = (int)min(32u, nbs - 32u * r);
+    const unsigned long long st = round_local_scan<S>(W.stage0 + (uint32_t)(k * K1_STAGE_BYTES), cnt, lane, LC) + LC.kp * carry;
+    emit(32u * r, cnt, st);
     carry = shfl64(st, cnt - 1);
     __syncwarp();                                    // all lanes are done with stage k before it is filled again
     k = (k + 1 == K1_STAGES) ? 0 : k + 1;
   }
   return carry;
+}
+
+// The misalignment is a property of the run: four copies of the round loop, none of them with a select or a branch on it.
+template <typename Emit>
+__device__ __forceinline__ unsigned long long hash_run(WarpPipe& W, const uint32_t* __restrict__ tok, int base_mis, int64_t lo, int64_t hi,
+                                                       int64_t ts, uint32_t nbs, unsigned long long carry, int lane, const LaneConsts& LC,
+                                                       Emit emit) {
+  switch ((int)((base_mis + ts) & 3)) {
+    case 0: return hash_run_s<0>(W, tok, lo, hi, ts, nbs, carry, lane, LC, emit);
+    case 1: return hash_run_s<1>(W, tok, lo, hi, ts, nbs, carry, lane, LC, emit);
+    case 2: return hash_run_s<2>(W, tok, lo, hi, ts, nbs, carry, lane, LC, emit);
+    default: return hash_run_s<3>(W, tok, lo, hi, ts, nbs, carry, lane, LC, emit);
+  }
 }
 
 // Length classes for the ticket passes: requests of at least K1_CLASS_MIN[c] blocks are started in pass c, so the
@@ -316,9 +352,10 @@ __global__ void __launch_bounds__(256, 3) hash_blocks_kernel(const int32_t* __re
       const uint32_t r = __shfl_sync(0xFFFFFFFFu, my_r, src);
       const int64_t o = blk_off[r], nb = blk_off[r + 1] - o;
       const unsigned long long c0 = (CHAIN && chain_in) ? chain_in[r] : H_S0;     // the H4 state before block 0 (a prompt: S0)
-      const unsigned long long end = hash_run(W, tok, base_mis, lo, hi, offsets[r], nb, c0, lane, LC,
-        [&](int64_t rb, int cnt, unsigned long long st) {
-          if (lane < cnt) { const int64_t i = rb + lane; keys[ACCESS_ORDER ? (o + (nb - 1 - i)) : (o + i)] = finalize_key(st); }
+      unsigned long long* out = keys + (ACCESS_ORDER ? (o + nb - 1 - lane) : (o + lane));    // this lane's key of round 0
+      const unsigned long long end = hash_run(W, tok, base_mis, lo, hi, offsets[r], (uint32_t)nb, c0, lane, LC,
+        [&](uint32_t rb, int cnt, unsigned long long st) {
+          if (lane < cnt) { if (ACCESS_ORDER) *(out - rb) = finalize_key(st); else out[rb] = finalize_key(st); }
         });
       if (CHAIN && lane == 0) chain_out[r] = end;                                 // the state a continuation of this sequence starts from
     }
@@ -364,9 +401,10 @@ __global__ void __launch_bounds__(256, 3) hash_segments_kernel(const int32_t* __
     const int64_t b0 = (int64_t)sg * K1_SEG;
     if (b0 >= nb) continue;
     const int64_t nbs = min((int64_t)K1_SEG, nb - b0);
-    const unsigned long long end = hash_run(W, tok, base_mis, lo, hi, offsets[r] + 16 * b0, nbs, 0ull, lane, LC,
-      [&](int64_t rb, int cnt, unsigned long long st) {
-        if (lane < cnt) states[o + (nb - 1 - (b0 + rb + lane))] = st;
+    unsigned long long* out = states + (o + nb - 1 - b0 - lane);
+    const unsigned long long end = hash_run(W, tok, base_mis, lo, hi, offsets[r] + 16 * b0, (uint32_t)nbs, 0ull, lane, LC,
+      [&](uint32_t rb, int cnt, unsigned long long st) {
+        if (lane < cnt) *(out - rb) = st;
       });
     if (lane == 0) seg_end[(size_t)r * max_seg + sg] = end;
   }
