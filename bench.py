@@ -1,28 +1,33 @@
 #!/usr/bin/env python
 """bench.py - the driver's benchmark contract for the arc_step hot path.
 
-One "step" = one arc_step (K1 chained block hashing, K2 directory probe + reserve, K3 ARC state
-machine, K4 finalize) over one scheduler batch of a seeded synthetic trace.  Default workload:
-BASELINE.json configs[1] (document-QA shaped: c = 8,192 blocks x 16 tokens, 64 requests per step).
+One "step" = one arc_step (K1 chained block hashing, K2 directory probe + reserve, K3 ARC state machine, K4 finalize)
+over one scheduler batch of a seeded synthetic trace.  Default workload: BASELINE.json configs[4], the largest
+single-GPU configuration (scale stress: c = 1,048,576 blocks x 16 tokens, 1,024 requests per step).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
 
 Prints ONE JSON line (rank 0).  Keys beyond the base contract:
   value            block accesses/s, steps enqueued back to back on one stream, tokens resident in HBM
   tokens_hashed_per_s, requests_per_s   the same timed region in the metric's other units
-  e2e              the same metric through arc_step_host (pinned HOST tokens in, results out, per step)
-  roofline         K1 (the HBM-bound kernel) through arc_hash_blocks on >= 1 GiB of D5-shaped requests
-  kernels          per-kernel device time of the timed steps (CUDA events between the kernels, separate pass)
-  hit_rate         ARC vs LRU on the same steps
+  e2e              the same metric through the host entry (pinned HOST tokens in, results out, per step)
+  roofline         K1 (the HBM-bound kernel) on >= 1 GiB of D5-shaped requests: through the API and kernel-only
+  dominant_kernel  K3 (latency-bound): share of the step, ns per access, warp instructions per access from the
+                   committed ncu export (profiles/), refused when the kernel sources changed since the capture
+  per_config       configs 1-5: value, e2e, K3 ns/access, synchronous step latency, hit rates, t1/c, oracle, parity digest
+  probe            K2 alone on a 2 GiB table against the measured random-sector ceiling
   cpu_baseline     the CPU oracle, as it stands, one thread, on the same steps
-Multi-GPU (--gpus N under torchrun): replicas only: every rank runs its own cache on its
-own seeded trace, no data-path collective; value = sum of accesses / max over ranks of the device time.
+Multi-GPU (--gpus N): replicas only: every rank runs its own cache on its own seeded trace, no data-path
+collective; value = sum of accesses / max over ranks of the device time.  Without torchrun, --gpus N > 1 starts the N
+ranks itself (torch.distributed.run on 127.0.0.1) and fails loudly when the box has fewer GPUs.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import re
 import subprocess
 import sys
 import threading
@@ -37,20 +42,27 @@ if str(ROOT) not in sys.path:
 
 METRIC = "arc_block_accesses_per_s"
 UNIT = "accesses/s"
-ALGO_BYTES_PER_BLOCK = 72          # K1: 64 B of tokens read + 8 B key written (DESIGN.md §7)
+ALGO_BYTES_PER_BLOCK = 72          # K1: 64 B of tokens read + 8 B key written (DESIGN.md 7)
+# steps of each config the per_config block runs (configs 1-3 fit whole or nearly; 4 and 5 are 160 M / 600 M accesses
+# in full: their whole traces are checked by tests/full_trace_parity.py, profiles/r02_full_trace_parity.md)
+PER_CONFIG_STEPS = {1: 250, 2: 120, 3: 120, 4: 30, 5: 25}
+PAPER_CONTEXT = ("+10.8% hit rate / -12.6% TTFT (doc QA), +2.1% / -2.0% (conversation): Qwen3-14B, vLLM, 1x H100 PCIe 80 GB "
+                 "(PAPER.md:7, :86, :111, :117)")
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=600)
-    ap.add_argument("--warmup", type=int, default=30)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index + 1 (default 2 = doc-QA)")
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json configs index + 1 (default 5 = the largest single-GPU config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--bulk-gib", type=float, default=1.0, help="size of the K1 roofline run in GiB of tokens")
-    ap.add_argument("--no-extras", action="store_true", help="skip the breakdown / roofline / hit-rate / cpu legs")
+    ap.add_argument("--no-extras", action="store_true", help="skip per_config / roofline / probe / cpu legs (for ncu captures)")
     ap.add_argument("--only-k1", action="store_true", help="run only the K1 bulk roofline leg (for ncu captures of the hashing kernel)")
+    ap.add_argument("--only-k2", action="store_true", help="run only the K2 probe leg (for ncu captures of the probe kernel)")
+    ap.add_argument("--print-source-hash", action="store_true", help="print the hash of the kernel sources (profiles/r02_ncu_evidence.json)")
     return ap.parse_args()
 
 
@@ -62,6 +74,45 @@ def peaks():
         except Exception:
             pass
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def source_hash() -> str:
+    """SHA-256 over the kernel sources: an ncu capture is quoted only while it still describes this code."""
+    h = hashlib.sha256()
+    for f in sorted((ROOT / "paper_2606_21238_b200" / "csrc").glob("*.cu*")):
+        h.update(f.name.encode())
+        h.update(f.read_bytes())
+    return h.hexdigest()
+
+
+def ncu_metric(csv_path: Path, kernel_pat: str, metric: str):
+    """Values of `metric` for the launches whose kernel name matches, from an `ncu --page raw --csv` export."""
+    import csv
+
+    rows = list(csv.reader(csv_path.open()))
+    hdr = rows[0]
+    if metric not in hdr or "Kernel Name" not in hdr:
+        return []
+    k, m = hdr.index("Kernel Name"), hdr.index(metric)
+    out = []
+    for r in rows[2:]:
+        if len(r) > m and re.search(kernel_pat, r[k]):
+            try:
+                out.append(float(r[m].replace(",", "")))
+            except ValueError:
+                pass
+    return out
+
+
+def ncu_evidence():
+    """profiles/r02_ncu_evidence.json names the committed raw exports and the source hash they were taken at."""
+    p = ROOT / "profiles" / "r02_ncu_evidence.json"
+    if not p.exists():
+        return None, "no committed ncu evidence file"
+    ev = json.loads(p.read_text())
+    if ev.get("csrc_sha256") != source_hash():
+        return None, "kernel sources changed since the committed ncu capture (profiles/r02_ncu_evidence.json): not quoted"
+    return ev, "profiles/r02_ncu_evidence.json"
 
 
 def build_steps(config: int, n_steps: int, seed: int):
@@ -138,16 +189,20 @@ def stage_on_device(torch, steps):
     return host, dev, bases
 
 
-def run_device_resident(torch, A, info, steps, dev, bases, warmup, policy, stream, profile=False):
-    """Replays steps on a fresh handle; returns (handle, elapsed_ms of the timed steps, per-kernel sums)."""
+def run_device_resident(torch, A, info, steps, dev, bases, warmup, policy, stream, profile=False, snapshot_at=None):
+    """Replays steps on a fresh handle; returns (handle, elapsed_ms of the timed steps, per-kernel sums, launches, snapshot).
+    snapshot_at: index of a step after which arc_stats is read (a synchronisation: only in untimed passes)."""
     cache = A.ArcCache(info.capacity_blocks, info.block_size, policy)
     acc, _, req = step_counts(steps)
     cache.reserve(max(req), max(acc))
     sp = int(stream.cuda_stream)
     base_ptr = dev.data_ptr()
+    snap = None
     for i in range(warmup):
         rc = cache.step_raw(base_ptr + 4 * bases[i], steps[i][1], sp)
         assert rc == 0, rc
+        if snapshot_at is not None and i == snapshot_at:
+            snap = cache.stats()
     sums = {}
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if profile:
@@ -161,14 +216,16 @@ def run_device_resident(torch, A, info, steps, dev, bases, warmup, policy, strea
         if profile:
             for k, v in cache.last_kernel_times().items():
                 sums[k] = sums.get(k, 0.0) + v
+        if snapshot_at is not None and i == snapshot_at:
+            snap = cache.stats()
     ev1.record(stream)
     stream.synchronize()
     cache.stats()      # raises on a device-side directory error
-    return cache, ev0.elapsed_time(ev1), sums, cache.launch_count() - launches0
+    return cache, ev0.elapsed_time(ev1), sums, cache.launch_count() - launches0, snap
 
 
 def run_e2e(torch, A, info, steps, host, bases, warmup, stream):
-    """arc_step_host: pinned HOST tokens -> device inside the call, results back to pinned host, per step."""
+    """The host entry: pinned HOST tokens -> device inside the call, results back to pinned host, per step."""
     cache = A.ArcCache(info.capacity_blocks, info.block_size, A.POLICY_ARC)
     acc, _, req = step_counts(steps)
     cache.reserve(max(req), max(acc))
@@ -190,6 +247,160 @@ def run_e2e(torch, A, info, steps, host, bases, warmup, stream):
     wall_ms = (time.perf_counter() - t0) * 1e3
     cache.close()
     return max(wall_ms, ev0.elapsed_time(ev1)), d2h, h2d
+
+
+def sync_latency(torch, A, info, steps, dev, bases, warmup, stream):
+    """Synchronous per-step latency: every step enqueued on an idle stream and waited for (first enqueue -> last kernel
+    done, CUDA events) - what a scheduler that needs the result before its next decision pays."""
+    cache = A.ArcCache(info.capacity_blocks, info.block_size, A.POLICY_ARC)
+    acc, _, req = step_counts(steps)
+    cache.reserve(max(req), max(acc))
+    sp, base_ptr = int(stream.cuda_stream), dev.data_ptr()
+    ms = []
+    for i in range(len(steps)):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        stream.synchronize()
+        a.record(stream)
+        rc = cache.step_raw(base_ptr + 4 * bases[i], steps[i][1], sp)
+        assert rc == 0, rc
+        b.record(stream)
+        stream.synchronize()
+        if i >= warmup:
+            ms.append(a.elapsed_time(b))
+    cache.close()
+    ms.sort()
+    return {"p50_ms": ms[len(ms) // 2], "p99_ms": ms[min(len(ms) - 1, int(0.99 * len(ms)))], "max_ms": ms[-1], "steps": len(ms)}
+
+
+def hit_rates(st, since=None):
+    """Block and prefix-token hit rates from arc_stats counters; since = an earlier snapshot to subtract (warm-up split)."""
+    d = (lambda k: st[k] - (since[k] if since else 0))
+    return {"block_hit_rate": (d("hit_t1") + d("hit_t2")) / max(1, d("accesses")),
+            "prefix_token_hit_rate": d("prefix_hit_tokens") / max(1, d("tokens_seen"))}
+
+
+def check_pass(torch, A, info, steps, oracle=True):
+    """GPU (through the C ABI, every output copied to the host) against the oracle, step by step: SHA-256 of
+    cls | block_id | evicted_id of every step on both sides, the counters at the end; the t1 / c series; the ARC hit rates
+    of the whole run and after the first 10 % of its requests; the oracle's own time (the cpu_baseline of this config)."""
+    from oracle import oracle as O
+
+    c = info.capacity_blocks
+    gc = A.ArcCache(c, info.block_size, A.POLICY_ARC)
+    oc = O.OracleCache(c, info.block_size, O.POLICY_ARC) if oracle else None
+    cut = max(1, int(np.ceil(0.1 * len(steps)))) - 1        # the step that ends the first 10 % of the requests
+    snap, t1 = None, []
+    same, n_acc, cpu_s = 0, 0, 0.0
+    dg, do = hashlib.sha256(), hashlib.sha256()
+    for i, (tokens, offsets) in enumerate(steps):
+        g = gc.step(torch.from_numpy(tokens).cuda(), offsets).to_host()
+        hg = hashlib.sha256(g["cls"].tobytes() + g["block_id"].tobytes() + g["evicted_id"].tobytes()).digest()
+        dg.update(hg)
+        if oc is not None:
+            t0 = time.perf_counter()
+            o = oc.step(tokens, offsets)
+            cpu_s += time.perf_counter() - t0
+            ho = hashlib.sha256(o["cls"].tobytes() + o["block_id"].tobytes() + o["evicted_id"].tobytes()).digest()
+            do.update(ho)
+            same += int(hg == ho)
+            n_acc += int(o["n_access"])
+        st = gc.stats()
+        t1.append(st["t1"] / c)
+        if i == cut:
+            snap = st
+    st = gc.stats()
+    out = {"steps": len(steps), "hit_rate_arc": {"whole_run": hit_rates(st), "after_first_10pct_of_requests": hit_rates(st, snap)},
+           "t1_over_c": {"mean": float(np.mean(t1)), "final": t1[-1]}, "p_over_c_final": st["p"] / c, "digest_gpu": dg.hexdigest()[:16]}
+    if oc is not None:
+        so = oc.stats()
+        keys = ("accesses", "hit_t1", "hit_t2", "ghost_b1", "ghost_b2", "miss", "evict_t1", "evict_t2", "p", "t1", "t2", "b1", "b2", "prefix_hit_tokens")
+        out["parity_spot_check"] = bool(same == len(steps) and all(st[k] == so[k] for k in keys))
+        out["parity_what"] = f"SHA-256 of cls | block_id | evicted_id of each of the {len(steps)} steps equal on {same}; 14 counters equal"
+        out["digest_oracle"] = do.hexdigest()[:16]
+        tm = oc.timing()
+        out["cpu_baseline"] = {"value": n_acc / max(cpu_s, 1e-9), "unit": UNIT, "cores": 1, "kind": "oracle", "cpu": cpu_model(),
+                               "sample": f"the same {len(steps)} steps from an empty cache, {n_acc} accesses, {cpu_s:.2f} s in oracle_step "
+                                         f"(hashing {tm['hash_seconds']:.2f} s + ARC {tm['arc_seconds']:.2f} s)"}
+        oc.close()
+    gc.close()
+    return out
+
+
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip() + f" ({os.cpu_count()} logical CPUs)"
+    except OSError:
+        pass
+    return f"unknown ({os.cpu_count()} logical CPUs)"
+
+
+def measure_config(torch, A, config, n_warm, n_timed, seed, stream, full=True, clock_index=None, dist=None, P=None):
+    """Everything per_config reports for one config; with clock_index the timed region is sampled with nvidia-smi and
+    (under torchrun) bracketed by barriers and reduced over the ranks (the headline)."""
+    info, steps = build_steps(config, n_warm + n_timed, seed)
+    acc, tok, req = step_counts(steps)
+    n_acc, n_tok, n_req = sum(acc[n_warm:]), sum(tok[n_warm:]), sum(req[n_warm:])
+    host, dev, bases = stage_on_device(torch, steps)
+    res = {"workload": f"BASELINE.json configs[{config - 1}] ({info.name}): c={info.capacity_blocks} blocks x {info.block_size} tokens, "
+                       f"{info.requests_per_step} requests/step, steps {n_warm}..{n_warm + n_timed - 1} of the seeded trace",
+           "steps": n_timed, "warmup": n_warm, "accesses_per_step": n_acc / n_timed, "tokens_per_step": n_tok / n_timed}
+    clk = None
+    if P is not None:
+        P.barrier(dist)
+    torch.cuda.synchronize()
+    if clock_index is not None:
+        with ClockSampler(clock_index) as clk:
+            cache, ms, _, launches, _ = run_device_resident(torch, A, info, steps, dev, bases, n_warm, A.POLICY_ARC, stream)
+    else:
+        cache, ms, _, launches, _ = run_device_resident(torch, A, info, steps, dev, bases, n_warm, A.POLICY_ARC, stream)
+    torch.cuda.synchronize()
+    if P is not None:
+        P.barrier(dist)
+    st_arc = cache.stats()
+    cache.close()
+    e2e_ms, d2h, h2d = run_e2e(torch, A, info, steps, host, bases, n_warm, stream)
+    if P is not None:
+        ms, tot_acc, tot_tok, tot_req = P.reduce_timing(dist, torch, ms, n_acc, n_tok, n_req)
+        e2e_ms, _, _, _ = P.reduce_timing(dist, torch, e2e_ms, n_acc, n_tok, n_req)
+    else:
+        tot_acc, tot_tok, tot_req = n_acc, n_tok, n_req
+    res.update(value=tot_acc / (ms * 1e-3), ms_per_step=ms / n_timed, tokens_hashed_per_s=16 * tot_acc / (ms * 1e-3),
+               tokens_seen_per_s=tot_tok / (ms * 1e-3), requests_per_s=tot_req / (ms * 1e-3), gpu_launches=launches,
+               launches_per_step=launches / n_timed,
+               e2e={"value": tot_acc / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / n_timed, "d2h_bytes_per_step": d2h / n_timed,
+                    "ms_per_step": e2e_ms / n_timed, "api": "arc_step_host (pinned host tokens in, prefix_len | counts | alloc_ids | evict_ids out)"},
+               state={k: st_arc[k] for k in ("t1", "t2", "b1", "b2", "p")})
+    if clk is not None:
+        res["clocks"] = clk.summary()
+    if not full:
+        return res, (info, steps, dev, bases, acc)
+    # per-kernel breakdown: a separate pass with CUDA events between the kernels (it syncs every step)
+    c2, _, sums, _, _ = run_device_resident(torch, A, info, steps, dev, bases, n_warm, A.POLICY_ARC, stream, profile=True)
+    res["k3_debug"] = c2.debug_counters()
+    c2.close()
+    tot = max(sums.get("total_ms", 0.0), 1e-9)
+    res["kernels"] = {k: {"us_per_step": 1e3 * v / n_timed, "share": v / tot} for k, v in sums.items() if k != "total_ms"}
+    res["k3_ns_per_access"] = 1e6 * sums.get("machine_ms", 0.0) / max(1, n_acc)
+    res["k3_share_of_step"] = sums.get("machine_ms", 0.0) / tot
+    res["k1_in_situ_GBps"] = ALGO_BYTES_PER_BLOCK * n_acc / max(sums.get("hash_ms", 0.0) * 1e-3, 1e-12) / 1e9
+    res["sync_step_latency"] = sync_latency(torch, A, info, steps, dev, bases, n_warm, stream)
+    # ARC vs LRU vs DBL on the same steps from an empty cache, whole run and after the first 10 % of the requests
+    cut = max(1, int(np.ceil(0.1 * len(steps)))) - 1
+    rates = {}
+    for name, pol in (("lru", A.POLICY_LRU), ("dbl", A.POLICY_DBL)):
+        c3, _, _, _, snap = run_device_resident(torch, A, info, steps, dev, bases, n_warm, pol, stream, snapshot_at=cut)
+        st = c3.stats()
+        c3.close()
+        rates[name] = {"whole_run": hit_rates(st), "after_first_10pct_of_requests": hit_rates(st, snap)}
+    chk = check_pass(torch, A, info, steps)
+    rates["arc"] = chk.pop("hit_rate_arc")
+    rates["arc_minus_lru_points"] = {w: {k: 100 * (rates["arc"][w][k] - rates["lru"][w][k]) for k in rates["arc"][w]} for w in rates["arc"]}
+    rates["scope"] = f"all {len(steps)} steps from an empty cache (warm-up steps of the timing included)"
+    res["hit_rate"] = rates
+    res.update(chk)
+    return res, (info, steps, dev, bases, acc)
 
 
 def k1_bulk_roofline(torch, A, gib, stream, seed):
@@ -236,33 +447,89 @@ def k1_bulk_roofline(torch, A, gib, stream, seed):
                 same_keys=same)
 
 
-def k2_probe_bench(torch, A, stream, seed, n_keys=1 << 24):
+def k2_probe_bench(torch, A, stream, seed, peak, n_keys=1 << 24):
     """K2 alone on a directory far larger than L2: capacity 16 M blocks (2 GiB table), 16 M distinct random keys inserted,
-    then looked up again in a different random order (every probe is one random 128-B bucket read from HBM)."""
+    then looked up again in a different random order (every probe is one random 32-byte sector read from HBM), and the
+    ceiling it is compared with: arc_debug_gather_sectors, the same grid and loads without the compare, on 2 GiB."""
     cache = A.ArcCache(n_keys, 16, A.POLICY_ARC)
     g = torch.Generator(device="cuda")
     g.manual_seed(seed + 91)
     keys = torch.randint(2, 2 ** 62, (n_keys,), dtype=torch.int64, device="cuda", generator=g)
     nodes = torch.empty(n_keys, dtype=torch.int32, device="cuda")
     cache.reserve(1, n_keys)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
     cache.debug_probe(keys, nodes, stream)                      # inserts
+    e1.record(stream)
     stream.synchronize()
+    insert_ms = e0.elapsed_time(e1)
     first = nodes.clone()
     perm = torch.randperm(n_keys, device="cuda", generator=g)
     keys2 = keys[perm].contiguous()
-    for _ in range(2):
-        cache.debug_probe(keys2, nodes, stream)
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
-    stream.synchronize()
-    for a, b in evs:
-        a.record(stream)
-        cache.debug_probe(keys2, nodes, stream)
-        b.record(stream)
-    stream.synchronize()
+
+    def timed(fn, reps=5):
+        for _ in range(3):
+            fn()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        stream.synchronize()
+        for a, b in evs:
+            a.record(stream)
+            fn()
+            b.record(stream)
+        stream.synchronize()
+        return float(np.mean([a.elapsed_time(b) for a, b in evs]))
+
+    ms = timed(lambda: cache.debug_probe(keys2, nodes, stream))
     ok = bool(torch.equal(nodes, first[perm]))                  # every key found again, at the node it was given
-    ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
     cache.close()
-    return n_keys, ms, ok
+    del first, nodes
+    buf = torch.zeros(1 << 29, dtype=torch.int32, device="cuda")            # 2 GiB, the size of the table
+    out = torch.empty(n_keys, dtype=torch.int32, device="cuda")
+    ceil_ms = timed(lambda: A.debug_gather_sectors(keys2, buf, out, stream))
+    kps, cps = n_keys / (ms * 1e-3), n_keys / (ceil_ms * 1e-3)
+    return {"kernel": "K2 probe_reserve (arc_debug_probe): one thread per key, one 32-byte bucket (two 16-byte slots) per probe",
+            "keys": n_keys, "ms_per_launch": ms, "keys_per_s": kps, "found_all": ok, "insert_ms_16M_new_keys": insert_ms,
+            "table": "capacity 16 M blocks: 2 GiB table, load 0.125",
+            "bytes_model": "algorithmic 28 B/key (8 B key + 16 B slot + 4 B node id); sector level 44 B/key (8 + one 32-B sector + 4): 1.57 x algorithmic",
+            "algorithmic_GBps": 28 * kps / 1e9, "sector_level_GBps": 44 * kps / 1e9,
+            "frac_of_measured_hbm_algorithmic": 28 * kps / 1e9 / peak, "frac_of_measured_hbm_sector_level": 44 * kps / 1e9 / peak,
+            "random_sector_ceiling": {"what": "arc_debug_gather_sectors: 16 M random 32-byte sector reads from a 2 GiB buffer, same grid and loads as K2",
+                                      "sectors_per_s": cps, "ms": ceil_ms, "GBps_of_sectors": 32 * cps / 1e9},
+            "frac_of_random_sector_ceiling": kps / cps}
+
+
+def windowed_zipf_leg(torch, A, stream, seed, cache_tokens=30000):
+    """The paper's own regime: batch size 1, one request per arc_step, the windowed-Zipf document-QA
+    workload (3,072 requests), cache of 30 K tokens.  Device-resident tokens, steps enqueued back to back."""
+    from paper_2606_21238_b200 import workloads as W
+
+    c = cache_tokens // 16
+    tr = W.make_windowed_zipf(c, seed=seed)
+    steps = [(t, o) for t, o in tr.steps() if int((np.diff(o) // 16).max(initial=0)) <= c]
+    acc, _, _ = step_counts(steps)
+    _, dev, bases = stage_on_device(torch, steps)
+    cache = A.ArcCache(c, 16, A.POLICY_ARC)
+    cache.reserve(1, max(acc))
+    sp, base_ptr = int(stream.cuda_stream), dev.data_ptr()
+    warm = 512                                                   # the first window warms the cache (cf. PAPER.md:115)
+    for i in range(warm):
+        cache.step_raw(base_ptr + 4 * bases[i], steps[i][1], sp)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream.synchronize()
+    l0 = cache.launch_count()
+    e0.record(stream)
+    for i in range(warm, len(steps)):
+        cache.step_raw(base_ptr + 4 * bases[i], steps[i][1], sp)
+    e1.record(stream)
+    stream.synchronize()
+    ms, n = e0.elapsed_time(e1), sum(acc[warm:])
+    st = cache.stats()
+    launches = cache.launch_count() - l0
+    cache.close()
+    return {"what": f"windowed Zipf, batch size 1: {len(steps)} one-request steps, c = {c} blocks ({cache_tokens} tokens), first 512 steps warm-up",
+            "steps": len(steps) - warm, "accesses_per_step": n / (len(steps) - warm), "us_per_step": 1e3 * ms / (len(steps) - warm),
+            "accesses_per_s": n / (ms * 1e-3), "requests_per_s": (len(steps) - warm) / (ms * 1e-3),
+            "launches_per_step": launches / (len(steps) - warm), "block_hit_rate": (st["hit_t1"] + st["hit_t2"]) / max(1, st["accesses"])}
 
 
 def serving_loop_leg(torch, A, info, steps, stream, seed, n_steps=240, new_per_step=8, decode_steps=2):
@@ -364,24 +631,21 @@ def serving_loop_leg(torch, A, info, steps, stream, seed, n_steps=240, new_per_s
             "cpu_oracle_accesses_per_s": n_acc / cpu_s, "parity_spot_check": same}
 
 
-def cpu_oracle_leg(info, steps, policy=0):
-    """The oracle as it stands (g++ -O2, std::list + unordered_map, one thread) over the same steps."""
-    from oracle import oracle as O
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` without torchrun: start the N ranks ourselves on 127.0.0.1 (one process per GPU)."""
+    import socket
 
-    oc = O.OracleCache(info.capacity_blocks, info.block_size, policy)
-    t0 = time.perf_counter()
-    n = 0
-    for tokens, offsets in steps:
-        n += oc.step(tokens, offsets, unpack=False)
-    dt = time.perf_counter() - t0
-    tm, st = oc.timing(), oc.stats()
-    oc.close()
-    return n, dt, tm, st
+    import torch
 
-
-def hit_rates(st):
-    a = max(1, st["accesses"])
-    return {"block_hit_rate": (st["hit_t1"] + st["hit_t2"]) / a, "prefix_token_hit_rate": st["prefix_hit_tokens"] / max(1, st["tokens_seen"])}
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    if have < args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus}: this box has {have} CUDA device(s); refusing to run fewer replicas than asked for")
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), str(Path(__file__).resolve())] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def run_ours(args):
@@ -390,9 +654,13 @@ def run_ours(args):
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback (use --impl reference for the oracle)")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        raise SystemExit(spawn_ranks(args))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus} was started with WORLD_SIZE={world}")
     torch.cuda.set_device(local)
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
@@ -401,115 +669,98 @@ def run_ours(args):
     from paper_2606_21238_b200 import parallel as P
 
     A.load_library()
+    peak, peak_src = peaks()
+    stream = torch.cuda.current_stream()
     if args.only_k1:
-        peak, peak_src = peaks()
-        k1 = k1_bulk_roofline(torch, A, args.bulk_gib, torch.cuda.current_stream(), args.seed)
+        k1 = k1_bulk_roofline(torch, A, args.bulk_gib, stream, args.seed)
         gb = ALGO_BYTES_PER_BLOCK * k1["blocks"] / 1e9
         k1.update(kernel="K1 chained block hashing", api_GBps=gb / (k1["api_ms"] * 1e-3), kernel_GBps=gb / (k1["kernel_ms"] * 1e-3), peak=peak,
                   frac=gb / (k1["api_ms"] * 1e-3) / peak, frac_kernel=gb / (k1["kernel_ms"] * 1e-3) / peak, peak_source=peak_src)
         print(json.dumps(k1))
         return
+    if args.only_k2:
+        print(json.dumps(k2_probe_bench(torch, A, stream, args.seed, peak)))
+        return
     W_, K = args.warmup, args.steps
-    info, steps = build_steps(args.config, W_ + K, P.replica_seed(args.seed, rank))
-    acc, tok, req = step_counts(steps)
-    n_acc, n_tok, n_req = sum(acc[W_:]), sum(tok[W_:]), sum(req[W_:])
-    host, dev, bases = stage_on_device(torch, steps)
-    stream = torch.cuda.current_stream()
-
-    # ---- timed region: K steps enqueued back to back, tokens resident in HBM --------------------------
-    P.barrier(dist if world > 1 else None)
-    torch.cuda.synchronize()
-    with ClockSampler(local) as clk:
-        cache, ms, _, launches = run_device_resident(torch, A, info, steps, dev, bases, W_, A.POLICY_ARC, stream)
-    torch.cuda.synchronize()
-    P.barrier(dist if world > 1 else None)
-    st_arc = cache.stats()
-    cache.close()
-    ms_max, tot_acc, tot_tok, tot_req = P.reduce_timing(dist if world > 1 else None, torch, ms, n_acc, n_tok, n_req)
-
-    # ---- e2e: the same steps through arc_step_host (H2D + D2H inside) ----------------------------------
-    e2e_ms, d2h, h2d_total = run_e2e(torch, A, info, steps, host, bases, W_, stream)
-    e2e_ms_max, _, _, _ = P.reduce_timing(dist if world > 1 else None, torch, e2e_ms, n_acc, n_tok, n_req)
-    h2d = h2d_total / K
-
+    D = dist if world > 1 else None
+    head, (info, steps, dev, bases, acc) = measure_config(torch, A, args.config, W_, K, P.replica_seed(args.seed, rank), stream,
+                                                          full=(rank == 0 and not args.no_extras), clock_index=local, dist=D, P=P)
     line = {
-        "metric": METRIC, "value": tot_acc / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
-        "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
+        "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u64 hash / i32 directory", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({info.name}): c={info.capacity_blocks} blocks x {info.block_size} tokens, "
-                               f"{info.requests_per_step} requests/step, steps {W_}..{W_ + K - 1} of the seeded trace",
-                   "accesses_per_step": n_acc / K, "tokens_per_step": n_tok / K, "policy": "ARC",
-                   "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": f"inputs larger than L2: every step reads its own slice of a {4 * sum(tok) / 1e6:.0f} MB token window staged in HBM; "
-                         "the directory is deliberately L2-resident"},
-        "tokens_hashed_per_s": 16 * tot_acc / (ms_max * 1e-3), "tokens_seen_per_s": tot_tok / (ms_max * 1e-3),
-        "requests_per_s": tot_req / (ms_max * 1e-3),
-        "e2e": {"value": tot_acc / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h / K,
-                "ms_per_step": e2e_ms_max / K, "api": "arc_step_host (synchronous, pinned host tokens)"},
-        "gpu_launches": launches,
-        "clocks": clk.summary(),
+        "config": {"workload": head["workload"], "accesses_per_step": head["accesses_per_step"], "tokens_per_step": head["tokens_per_step"],
+                   "policy": "ARC", "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": f"inputs larger than L2 or not re-read: every step reads its own slice of a {4 * sum(len(t) for t, _ in steps) / 1e6:.0f} MB token "
+                         "window staged in HBM (nothing is read twice); the directory stays where the hardware keeps it"},
+        "tokens_hashed_per_s": head["tokens_hashed_per_s"], "tokens_seen_per_s": head["tokens_seen_per_s"], "requests_per_s": head["requests_per_s"],
+        "e2e": head["e2e"], "gpu_launches": head["gpu_launches"], "clocks": head.get("clocks"),
     }
-
     if rank == 0 and not args.no_extras:
-        peak, peak_src = peaks()
-        # per-kernel breakdown: a separate pass with CUDA events between the kernels (it syncs every step)
-        c2, _, sums, _ = run_device_resident(torch, A, info, steps, dev, bases, W_, A.POLICY_ARC, stream, profile=True)
-        line["k3_debug"] = c2.debug_counters()
-        c2.close()
-        tot = max(sums.get("total_ms", 0.0), 1e-9)
-        line["kernels"] = {k: {"ms_per_step": v / K, "share": v / tot} for k, v in sums.items() if k != "total_ms"}
-        line["kernels"]["total_ms_per_step"] = tot / K
-        line["k3_ns_per_access"] = 1e6 * sums.get("machine_ms", 0.0) / max(1, n_acc)
-        line["dominant_kernel"] = {"kernel": "K3 ARC machine (arc_machine_wide_kernel, one CTA)", "share_of_step": sums.get("machine_ms", 0.0) / tot,
-                                   "bound": "latency: dependent instructions of one serial state machine (DESIGN.md 7.3); neither HBM nor tensor nor ALU throughput",
-                                   "ns_per_access": 1e6 * sums.get("machine_ms", 0.0) / max(1, n_acc),
-                                   "ncu": "profiles/r01e_held_resume_roll.md: about 43 warp instructions per access over 8 warps (38-52 on steps 15-17), 19 % issue-active per scheduler",
-                                   "issue_roofline": {"bound": "alu", "what": "warp-instruction issue of the ONE SM the machine runs on (4 schedulers x 1 instruction per clock)",
-                                                      "achieved": 43.0 * n_acc / max(sums.get("machine_ms", 0.0) * 1e-3, 1e-12), "unit": "warp instructions/s",
-                                                      "peak": 4 * 1.965e9, "frac": 43.0 * n_acc / max(sums.get("machine_ms", 0.0) * 1e-3, 1e-12) / (4 * 1.965e9),
-                                                      "instructions_per_access": "43, from the ncu capture named above (smsp__inst_executed.sum / accesses of that step)"}}
-        k1_insitu = ALGO_BYTES_PER_BLOCK * n_acc / max(sums.get("hash_ms", 0.0) * 1e-3, 1e-12) / 1e9
-        # K1 roofline: bulk run through arc_hash_blocks
-        nb, nreq_b, mean_ms, best_ms = k1_bulk_roofline(torch, A, args.bulk_gib, stream, args.seed)
-        achieved = ALGO_BYTES_PER_BLOCK * nb / (mean_ms * 1e-3) / 1e9
-        line["roofline"] = {"kernel": "K1 chained block hashing (arc_hash_blocks)", "bound": "hbm", "achieved": achieved, "peak": peak,
-                            "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8000": achieved / 8000.0, "peak_source": peak_src,
-                            "traffic": 1.168e9 if abs(args.bulk_gib - 1.0) < 1e-9 else None,
-                            "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this launch (profiles/r01e_held_resume_roll.md: 1.0855 GB + 82.3 MB)",
-                            "algorithmic_bytes_per_launch": ALGO_BYTES_PER_BLOCK * nb, "ms_per_launch": mean_ms,
-                            "best_ms": best_ms, "tokens_per_s": 16 * nb / (mean_ms * 1e-3),
-                            "workload": f"{nreq_b} D5-shaped requests, {nb} blocks, {64 * nb / 2**30:.2f} GiB of tokens (>> 126 MB L2)",
-                            "in_situ_GBps": k1_insitu}
-        # K2 alone, table >> L2
-        nk, k2_ms, k2_ok = k2_probe_bench(torch, A, stream, args.seed)
-        line["probe"] = {"kernel": "K2 probe_reserve + resolve (arc_debug_probe)", "keys": nk, "ms_per_launch": k2_ms, "keys_per_s": nk / (k2_ms * 1e-3),
-                         "found_all": k2_ok, "table": "capacity 16 M blocks: 2 GiB table of 16-B slots in 128-B buckets, load 0.125",
-                         "algorithmic_GBps": 28 * nk / (k2_ms * 1e-3) / 1e9, "sector_level_GBps": 140 * nk / (k2_ms * 1e-3) / 1e9,
-                         "frac_of_measured_hbm_sector_level": 140 * nk / (k2_ms * 1e-3) / 1e9 / peak,
-                         "bytes_model": "algorithmic 28 B/key (8 B key + 16 B slot + 4 B node id); sector level 140 B/key (8 + one 128-B bucket + 4)",
-                         "in_situ_us_per_step": 1e3 * sums.get("probe_ms", 0.0) / K}
-        # ARC vs LRU on the same steps
-        c3, _, _, _ = run_device_resident(torch, A, info, steps, dev, bases, W_, A.POLICY_LRU, stream)
-        st_lru = c3.stats()
-        c3.close()
-        c4, _, _, _ = run_device_resident(torch, A, info, steps, dev, bases, W_, A.POLICY_DBL, stream)
-        st_dbl = c4.stats()
-        c4.close()
-        ha, hl = hit_rates(st_arc), hit_rates(st_lru)
-        line["hit_rate"] = {"arc": ha, "lru": hl, "dbl": hit_rates(st_dbl),
-                            "arc_minus_lru_points": {k: 100 * (ha[k] - hl[k]) for k in ha},
-                            "scope": f"all {W_ + K} steps from an empty cache",
-                            "paper_context": "+10.8% hit rate / -12.6% TTFT (doc QA), +2.1% / -2.0% (conversation): Qwen3-14B, vLLM, 1x H100 PCIe 80 GB (PAPER.md:7, :86, :111, :117)"}
-        line["state"] = {k: st_arc[k] for k in ("t1", "t2", "b1", "b2", "p")}
-        # NEXT-3 measured: a continuous-batching loop under held pins (only where a batch fits the cache)
-        if args.config == 2:
-            line["serving_loop"] = serving_loop_leg(torch, A, info, steps, stream, args.seed)
-        # the CPU oracle on the same steps, on this box's host cores
-        n_o, dt, tm, st_o = cpu_oracle_leg(info, steps)
-        line["cpu_baseline"] = {"value": n_o / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                "sample": f"the same {W_ + K} steps (warm-up included), {n_o} accesses, {dt:.2f} s: hashing {tm['hash_seconds']:.2f} s + ARC {tm['arc_seconds']:.2f} s",
-                                "host_cpus": os.cpu_count()}
-        line["parity_spot_check"] = all(st_o[k] == st_arc[k] for k in ("accesses", "hit_t1", "hit_t2", "ghost_b1", "ghost_b2", "miss", "p", "t1", "t2", "b1", "b2"))
+        for k in ("kernels", "k3_ns_per_access", "k3_debug", "sync_step_latency", "hit_rate", "t1_over_c", "state", "parity_spot_check", "parity_what", "cpu_baseline"):
+            line[k] = head.get(k)
+        line["hit_rate"]["paper_context"] = PAPER_CONTEXT
+        # ---- the dominant kernel of the step: K3, latency-bound; instructions per access from the committed ncu export
+        ev, ev_note = ncu_evidence()
+        dom = {"kernel": "K3 ARC machine (arc_machine_wide_kernel, one CTA on one SM)", "share_of_step": head["k3_share_of_step"],
+               "ns_per_access": head["k3_ns_per_access"],
+               "bound": "latency: dependent instructions of one serial state machine (DESIGN.md 7.3); neither HBM nor tensor nor ALU throughput"}
+        if ev and ev.get("k3") and ev["k3"].get("config") == args.config and max(ev["k3"]["steps"]) < len(steps):
+            inst = ncu_metric(ROOT / "profiles" / ev["k3"]["csv"], "arc_machine_wide", "smsp__inst_executed.sum")
+            n = [acc[i] for i in ev["k3"]["steps"]]
+            if len(inst) == len(n) and sum(n):
+                ipa = sum(inst) / sum(n)
+                k3_s = head["kernels"]["machine_ms"]["us_per_step"] * 1e-6 * K
+                ach = ipa * head["accesses_per_step"] * K / max(k3_s, 1e-12)
+                dom["issue_roofline"] = {"bound": "alu", "what": "warp-instruction issue of the ONE SM the machine runs on (4 schedulers x 1 instruction per clock x 1.965 GHz)",
+                                         "instructions_per_access": ipa, "instructions_source": f"smsp__inst_executed.sum of steps {ev['k3']['steps']} in profiles/{ev['k3']['csv']} / their accesses",
+                                         "achieved": ach, "unit": "warp instructions/s", "peak": 4 * 1.965e9, "frac": ach / (4 * 1.965e9)}
+        else:
+            dom["issue_roofline"] = None
+            dom["issue_roofline_note"] = ev_note if not ev else "the committed K3 capture is of another config"
+        line["dominant_kernel"] = dom
+        # ---- K1 roofline: the HBM-bound kernel, bulk run, through the API and kernel-only
+        k1 = k1_bulk_roofline(torch, A, args.bulk_gib, stream, args.seed)
+        gb = ALGO_BYTES_PER_BLOCK * k1["blocks"] / 1e9
+        traffic, traffic_src = None, ev_note
+        if ev and ev.get("k1") and abs(args.bulk_gib - ev["k1"].get("bulk_gib", -1)) < 1e-9:
+            rd = ncu_metric(ROOT / "profiles" / ev["k1"]["csv"], "hash_blocks", "dram__bytes_read.sum")
+            wr = ncu_metric(ROOT / "profiles" / ev["k1"]["csv"], "hash_blocks", "dram__bytes_write.sum")
+            if rd and wr:
+                scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}
+                traffic = rd[0] * scale.get(ev["k1"].get("read_unit", "byte"), 1.0) + wr[0] * scale.get(ev["k1"].get("write_unit", "byte"), 1.0)
+                traffic_src = f"dram__bytes_read.sum + dram__bytes_write.sum of the launch in profiles/{ev['k1']['csv']} (ncu --set full)"
+        line["roofline"] = {"kernel": "K1 chained block hashing (hash_blocks_kernel: cp.async.bulk staging, mbarrier pipeline)", "bound": "hbm",
+                            "achieved": gb / (k1["api_ms"] * 1e-3), "peak": peak, "unit": "GB/s", "frac": gb / (k1["api_ms"] * 1e-3) / peak,
+                            "achieved_kernel": gb / (k1["kernel_ms"] * 1e-3), "frac_kernel": gb / (k1["kernel_ms"] * 1e-3) / peak,
+                            "frac_of_nominal_8000": gb / (k1["api_ms"] * 1e-3) / 8000.0, "frac_kernel_of_nominal_8000": gb / (k1["kernel_ms"] * 1e-3) / 8000.0,
+                            "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
+                            "algorithmic_bytes_per_launch": ALGO_BYTES_PER_BLOCK * k1["blocks"],
+                            "ms_per_launch_api": k1["api_ms"], "ms_per_launch_kernel": k1["kernel_ms"], "best_ms_api": k1["api_best_ms"], "best_ms_kernel": k1["kernel_best_ms"],
+                            "api": "arc_hash_blocks (host offsets in, copied by the call)", "kernel_only": "arc_hash_blocks_device (offsets already on the device)",
+                            "same_keys_both_ways": k1["same_keys"], "tokens_per_s": 16 * k1["blocks"] / (k1["api_ms"] * 1e-3),
+                            "workload": f"{k1['requests']} D5-shaped requests, {k1['blocks']} blocks, {64 * k1['blocks'] / 2**30:.2f} GiB of tokens (>> 126 MB L2)",
+                            "in_situ_GBps": head["k1_in_situ_GBps"]}
+        # ---- K2 alone, table >> L2, against the measured random-sector ceiling
+        line["probe"] = k2_probe_bench(torch, A, stream, args.seed, peak)
+        line["probe"]["in_situ_us_per_step"] = head["kernels"]["probe_ms"]["us_per_step"]
+        # ---- all five configs
+        per = {}
+        for cfg in (1, 2, 3, 4, 5):
+            if cfg == args.config:
+                r = head
+            else:
+                n = PER_CONFIG_STEPS[cfg]
+                w = max(3, n // 5)
+                r, _ = measure_config(torch, A, cfg, w, n - w, args.seed, stream, full=True)
+            per[str(cfg)] = {k: r.get(k) for k in ("workload", "steps", "warmup", "accesses_per_step", "value", "ms_per_step", "requests_per_s",
+                                                    "launches_per_step", "e2e", "k3_ns_per_access", "k3_share_of_step", "kernels", "sync_step_latency",
+                                                    "hit_rate", "t1_over_c", "p_over_c_final", "cpu_baseline", "parity_spot_check", "parity_what")}
+        line["per_config"] = per
+        # ---- the regimes of small steps: the paper's batch size 1, and a continuous-batching loop under held pins
+        line["windowed_zipf_batch1"] = windowed_zipf_leg(torch, A, stream, args.seed)
+        i2, s2 = build_steps(2, 320, args.seed)
+        line["serving_loop"] = serving_loop_leg(torch, A, i2, s2, stream, args.seed)
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
@@ -542,7 +793,7 @@ def run_reference(args):
                                f"{info.requests_per_step} requests/step, steps {args.warmup}..{args.warmup + args.steps - 1} of the seeded trace",
                    "policy": "ARC"},
         "tokens_hashed_per_s": 16 * v, "requests_per_s": sum(req) / dt,
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "cpu": cpu_model(),
                          "sample": f"every timed step is one whole step of the workload ({sum(acc)} accesses in {dt:.2f} s)"},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -551,4 +802,9 @@ def run_reference(args):
 
 if __name__ == "__main__":
     a = parse_args()
-    run_reference(a) if a.impl == "reference" else run_ours(a)
+    if a.print_source_hash:
+        print(source_hash())
+    elif a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

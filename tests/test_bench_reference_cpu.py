@@ -18,7 +18,7 @@ def test_reference_arm_prints_one_json_line():
     assert d["steps"] == 3 and d["warmup"] == 1 and d["value"] > 0 and d["higher_is_better"] is True
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] == 1
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0
-    assert "configs[1]" in d["config"]["workload"]
+    assert "configs[4]" in d["config"]["workload"]          # the largest single-GPU config is the default
 
 
 def test_our_arm_refuses_to_run_without_a_gpu():
