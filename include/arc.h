@@ -199,10 +199,13 @@ int arc_last_kernel_times(arc_cache *h, arc_kernel_times *out);
  * are counted in a process-wide counter returned when h == NULL). */
 uint64_t arc_launch_count(const arc_cache *h);
 
-/* Selects the K3 implementation (all give identical results): 0 = automatic (default): the wide machine, or the
- * one-warp machine for steps whose requests average fewer than 48 blocks; 1 = single-thread serial walk (the by-the-book
- * routine on the device, much slower); 2 = one-warp machine with 32-access windows; 3 = wide machine: one CTA of 8 warps,
- * 128-access windows. */
+/* Selects the implementation of a step (all give identical results): 0 = automatic (default): steps of up to 1,024
+ * accesses and 253 requests run as ONE kernel (K1-K4 as phases of a single CTA); larger steps run the
+ * four kernels with the wide K3 machine, or the one-warp machine when requests average fewer than 48 blocks;
+ * 1 = four kernels, K3 as a single-thread serial walk (the by-the-book routine on the device, much slower);
+ * 2 = four kernels, one-warp machine with 32-access windows; 3 = four kernels, wide machine: one CTA of 8 warps,
+ * 128-access windows; 4 = the one-launch kernel for every step it can take (up to 4,096 accesses and 253 requests),
+ * automatic otherwise. */
 int arc_set_machine(arc_cache *h, int which);
 
 /* K2 alone, for the probe microbenchmark and its tests: looks every key of d_keys (DEVICE uint64[n], values >= 2) up in

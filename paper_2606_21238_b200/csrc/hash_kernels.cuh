@@ -411,22 +411,18 @@ __global__ void __launch_bounds__(256, 3) hash_segments_kernel(const int32_t* __
   k1_leave(ticket, lane);
 }
 
-// K^(128 m): square-and-multiply over the bits of m (m < 2^11)
-__device__ __forceinline__ unsigned long long kpow_seg(uint32_t m) {
+// K^(2^LOG2 m): square-and-multiply over the bits of m (m < 2^11); the factors K^(2^(LOG2 + b)) are compile-time constants
+template <int LOG2>
+__device__ __forceinline__ unsigned long long kpow_segT(uint32_t m) {
   unsigned long long r = 1;
 #pragma unroll
   for (int b = 0; b < 11; ++b) {
-    unsigned long long f = 1;                       // K^(128 2^b) as a compile-time constant
-    switch (b) {
-      case 0: f = kpow(128u); break;       case 1: f = kpow(256u); break;      case 2: f = kpow(512u); break;
-      case 3: f = kpow(1024u); break;      case 4: f = kpow(2048u); break;     case 5: f = kpow(4096u); break;
-      case 6: f = kpow(8192u); break;      case 7: f = kpow(16384u); break;    case 8: f = kpow(32768u); break;
-      case 9: f = kpow(65536u); break;     default: f = kpow(131072u); break;
-    }
+    const unsigned long long f = kpow(1u << (LOG2 + b));
     if (m & (1u << b)) r *= f;
   }
   return r;
 }
+__device__ __forceinline__ unsigned long long kpow_seg(uint32_t m) { return kpow_segT<7>(m); }   // segments of K1_SEG = 128 blocks
 
 // One warp per segment (warp w: segment w / n_req of request w % n_req).  All segments before the warp's own are full,
 // so the true state before segment s is c_s = K^(128 s) c_0 + sum_{j<s} K^(128 (s-1-j)) E_j: one term per lane and a

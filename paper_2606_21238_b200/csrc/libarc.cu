@@ -20,6 +20,7 @@
 #include "machine_batched.cuh"
 #include "machine_serial.cuh"
 #include "machine_wide.cuh"
+#include "fused_small.cuh"
 
 using namespace arc;
 
@@ -32,6 +33,7 @@ constexpr int kStageSlots = 4;
 constexpr uint32_t kMaxReq = 1u << 20;
 constexpr uint64_t kMaxCapacity = 1ull << 28;   // node ids carry two flag bits
 constexpr uint32_t kSegEndCap = 1u << 16;       // n_req * segments-per-request the segmented K1 is used up to
+constexpr uint32_t kFusedAutoMax = 1024;        // steps of up to this many accesses take the one-launch kernel by default
 constexpr uint32_t kSegMaxReq = 512;            // with more requests than this one warp per request already fills the GPU
 
 uint32_t pow2_at_least(uint64_t x) {
@@ -426,6 +428,7 @@ cudaError_t k1_configure() {
   K1_ATTR((hash_segments_kernel<0>));
   K1_ATTR((hash_segments_kernel<(int)K1_INLINE_SMALL>));
   K1_ATTR((hash_segments_kernel<(int)K1_INLINE_LARGE>));
+  K1_ATTR(arc_fused_small_kernel);
 #undef K1_ATTR
   if (dev >= 0 && dev < 64) done[dev] = true;
   return cudaSuccess;
@@ -465,6 +468,25 @@ void launch_hash_segments(int mode, const K1HostArgs& A, const int32_t* d_tokens
     hash_segments_kernel<(int)K1_INLINE_LARGE><<<g, 256, K1_SMEM_BYTES, s>>>(d_tokens, d_offsets, d_blk_off, n_req, max_seg, d_states, d_seg_end, d_ticket, A.large);
   else
     hash_segments_kernel<0><<<g, 256, K1_SMEM_BYTES, s>>>(d_tokens, d_offsets, d_blk_off, n_req, max_seg, d_states, d_seg_end, d_ticket, A.none);
+}
+
+// host-side bookkeeping after a step's kernels are enqueued, and the result struct
+int finish_step(arc_cache* h, const int64_t* h_offsets, uint32_t n_req, uint64_t N, cudaStream_t s, const StepParams& P, arc_step_result* out) {
+  h->slots_used_bound += N;
+  for (int L = 1; L <= 4; ++L) h->window_bound[L] += N;
+  if (h->pin_scope == ARC_PIN_HELD) h->hold_units += N;
+  h->steps += 1; h->requests += n_req;
+  h->tokens_seen += (uint64_t)(h_offsets[n_req] - h_offsets[0]);
+  h->tokens_hashed += N * h->B;
+  h->last_stream = s;
+
+  out->n_access = N;
+  out->prefix_len = h->d_prefix_len; out->blk_off = P.blk_off; out->cls = h->d_cls; out->block_id = h->d_block_id;
+  out->evicted_id = h->d_evicted_id; out->p_after = h->d_p_after; out->alloc_ids = h->d_alloc_ids;
+  out->evict_ids = h->d_evict_ids;
+  out->chain_state = reinterpret_cast<const uint64_t*>(h->d_chain_state);
+  out->counts = reinterpret_cast<const uint32_t*>(reinterpret_cast<const char*>(h->d_state) + offsetof(DevState, counts));
+  return ARC_OK;
 }
 
 }  // namespace
@@ -551,6 +573,23 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
   const uint32_t max_seg = (uint32_t)((max_nb + K1_SEG - 1) / K1_SEG);
   const bool segmented = N && n_req <= kSegMaxReq && max_seg >= 2 && max_seg <= 1024 && (uint64_t)n_req * max_seg <= kSegEndCap;
   static thread_local K1HostArgs k1_args;
+  // small steps: K1-K4 as the phases of one kernel (fused_small.cuh); arc_set_machine(h, 4) asks for it whenever it fits
+  const bool fused = N && n_req <= K1_INLINE_SMALL && N <= FUSED_MAX_ACCESS &&
+                     (h->machine == 4 || (h->machine == 0 && N <= kFusedAutoMax));
+  if (fused) {
+    k1_fill_args(k1_args, K1_ARG_SMALL, h_offsets, blk_off.data(), n_req);
+    StepParams P = make_params(h);
+    P.tokens = d_tokens; P.n_req = n_req; P.n_access = (uint32_t)N;
+    arc_fused_small_kernel<<<1, 2 * WIDE_W, K1_SMEM_BYTES, s>>>(P, reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state, h->d_offsets,
+                                                             h->d_offsets + (h->req_cap + 1), (N < 48ull * n_req) ? 2 : 3, k1_args.small);
+    h->launches += 1;
+    if (h->profiling) {                  // one kernel: its whole time is booked under the machine
+      cudaEventRecord(h->ev[2], s); cudaEventRecord(h->ev[3], s); cudaEventRecord(h->ev[4], s); cudaEventRecord(h->ev[5], s);
+      h->ev_valid = true;
+    }
+    CUDA_TRY(h, cudaGetLastError());
+    return finish_step(h, h_offsets, n_req, N, s, P, out);
+  }
   const int arg_mode = N ? k1_arg_mode(n_req) : K1_ARG_NONE;   // small enough for a kernel argument: no copy-engine round trip, no staging
   if (arg_mode != K1_ARG_NONE) {
     k1_fill_args(k1_args, arg_mode, h_offsets, blk_off.data(), n_req);   // K1 takes the argument and stores the arrays for K3 / K4
@@ -608,21 +647,7 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
   if (h->profiling) { cudaEventRecord(h->ev[5], s); h->ev_valid = true; }
   CUDA_TRY(h, cudaGetLastError());
 
-  h->slots_used_bound += N;
-  for (int L = 1; L <= 4; ++L) h->window_bound[L] += N;
-  if (h->pin_scope == ARC_PIN_HELD) h->hold_units += N;
-  h->steps += 1; h->requests += n_req;
-  h->tokens_seen += (uint64_t)(h_offsets[n_req] - h_offsets[0]);
-  h->tokens_hashed += N * h->B;
-  h->last_stream = s;
-
-  out->n_access = N;
-  out->prefix_len = h->d_prefix_len; out->blk_off = P.blk_off; out->cls = h->d_cls; out->block_id = h->d_block_id;
-  out->evicted_id = h->d_evicted_id; out->p_after = h->d_p_after; out->alloc_ids = h->d_alloc_ids;
-  out->evict_ids = h->d_evict_ids;
-  out->chain_state = reinterpret_cast<const uint64_t*>(h->d_chain_state);
-  out->counts = reinterpret_cast<const uint32_t*>(reinterpret_cast<const char*>(h->d_state) + offsetof(DevState, counts));
-  return ARC_OK;
+  return finish_step(h, h_offsets, n_req, N, s, P, out);
 }
 
 int arc_step_host(arc_cache* h, const int32_t* h_tokens, const int64_t* h_offsets, uint32_t n_req, void* cuda_stream, arc_host_result* out) {
@@ -844,7 +869,7 @@ int arc_last_kernel_times(arc_cache* h, arc_kernel_times* out) {
 uint64_t arc_launch_count(const arc_cache* h) { return h ? h->launches : g_hash_launches.load(); }
 
 int arc_set_machine(arc_cache* h, int which) {
-  if (!h || which < 0 || which > 3) return ARC_ERR_INVALID_ARG;
+  if (!h || which < 0 || which > 4) return ARC_ERR_INVALID_ARG;
   h->machine = which;
   return ARC_OK;
 }

@@ -252,9 +252,10 @@ __device__ __forceinline__ Roll roll_forward(const SerialCtx& C, int32_t c, bool
   return R;
 }
 
-__global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_constant__ StepParams P) {
-  __shared__ uint4 s_vic[5][32];    // per list: the first entries found from the LRU end {node, block, slot, position}
-  const int lane = threadIdx.x;
+// The machine itself, run by ONE warp (s_vic: shared memory of that warp, per list the first entries found from the LRU
+// end {node, block, slot, position}).  Also the third phase of the one-launch small-step kernel when requests are short.
+__device__ __forceinline__ void batched_machine_run(const StepParams& P, uint4 (*s_vic)[32]) {
+  const int lane = threadIdx.x & 31;
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
   const bool lru = (P.policy == POLICY_LRU);
   const bool hold = (P.pin_scope == 2);
@@ -530,6 +531,11 @@ __global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_co
 #pragma unroll
     for (int i = 0; i < DBG_COUNT; ++i) P.state->dbg[i] += dbg[i];
   }
+}
+
+__global__ void __launch_bounds__(32) arc_machine_batched_kernel(const __grid_constant__ StepParams P) {
+  __shared__ uint4 s_vic[5][32];
+  batched_machine_run(P, s_vic);
 }
 
 inline void launch_machine_batched(const StepParams& P, cudaStream_t s) { arc_machine_batched_kernel<<<1, 32, 0, s>>>(P); }

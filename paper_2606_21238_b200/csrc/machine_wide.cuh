@@ -240,8 +240,9 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
   if (lane == 0 && rounds) atomicAdd(&P.state->dbg[DBG_SCAN_ROUNDS], rounds);
 }
 
-__global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __grid_constant__ StepParams P) {
-  __shared__ WideShared S;
+// The machine itself, run by the first 2 * WIDE_W threads of a CTA (all of them must call it; it ends with every thread
+// past the last barrier).  S: the CTA's WideShared.  Also the third phase of the one-launch small-step kernel.
+__device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared& S) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
   uint32_t lm[WIDE_WARPS], me[WIDE_WARPS];   // see wide_rank / wide_has
@@ -251,7 +252,7 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
   const bool hold = (P.pin_scope == 2);      // held scope: see machine_batched.cuh
   const int32_t c = P.capacity;
   const int64_t N = (int64_t)P.n_access;
-  if (P.state->error == DEV_ERR_NODE_POOL) return;       // K2 could not give every key a node: the step is void (sticky error)
+  if (P.state->error == DEV_ERR_NODE_POOL) return;       // K2 could not give every key a node: the step is void (sticky error; CTA-uniform)
   SerialCtx C;            // identical in every thread
   ctx_load(C, P);
   unsigned long long dbg[DBG_COUNT];
@@ -630,6 +631,11 @@ __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __gr
 #pragma unroll
     for (int i = 0; i < DBG_COUNT; ++i) P.state->dbg[i] += dbg[i];
   }
+}
+
+__global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __grid_constant__ StepParams P) {
+  __shared__ WideShared S;
+  wide_machine_run(P, S);
 }
 
 inline void launch_machine_wide(const StepParams& P, cudaStream_t s) { arc_machine_wide_kernel<<<1, 2 * WIDE_W, 0, s>>>(P); }
