@@ -67,15 +67,15 @@ typedef struct {
                                 *          to continue the sequence (the state the request came with if it had no full block) */
 } arc_step_result;
 
-/* Result of arc_step_host: every pointer is pinned HOST memory owned by the library, filled when the
- * call returns, valid until the next arc_step_host / arc_reset / arc_destroy on the handle. */
+/* Result of arc_step_host / arc_step_host_wait: every pointer is pinned HOST memory owned by the library, filled when the
+ * call returns, valid until the third arc_step_host(_async) after this step's, arc_reset or arc_destroy. */
 typedef struct {
   uint64_t n_access;
   uint32_t n_alloc, n_evict;
   const int32_t *prefix_len; /* [n_req] */
   const int32_t *alloc_ids;  /* [n_alloc] */
   const int32_t *evict_ids;  /* [n_evict] */
-  uint64_t h2d_bytes, d2h_bytes; /* what the call moved over the bus: tokens + offsets in; one packed copy out */
+  uint64_t h2d_bytes, d2h_bytes; /* what the step moved over the bus: tokens + offsets in; the packed results out */
 } arc_host_result;
 
 /* Cumulative counters since create/reset plus the current list sizes (R12). */
@@ -132,10 +132,21 @@ int arc_step(arc_cache *h, const int32_t *d_tokens, const int64_t *h_offsets, ui
 int arc_step_resume(arc_cache *h, const int32_t *d_tokens, const int64_t *h_offsets, const uint64_t *d_chain_in,
                     uint32_t n_req, void *cuda_stream, arc_step_result *out);
 
-/* Same step end to end from HOST memory: copies h_tokens (HOST int32, pinned or pageable) to a
- * library-owned device buffer, runs the step, copies prefix_len, counts, alloc_ids and evict_ids back
- * to pinned host memory (ONE device-to-host copy: the device keeps them in one buffer laid out like the
- * host's) and synchronises the stream before returning. */
+/* The same step end to end from HOST memory, pipelined: arc_step_host_async enqueues
+ *   - the copy of h_tokens (HOST int32; pinned memory makes the copy asynchronous) to a library-owned device buffer, on
+ *     the handle's own copy stream, so that it overlaps the steps still computing on cuda_stream,
+ *   - the step itself on cuda_stream (which waits for that copy),
+ *   - a kernel that writes the results straight into pinned, device-mapped host memory: n_alloc | n_evict |
+ *     prefix_len[n_req] | alloc_ids[n_alloc] | evict_ids[n_evict], exactly 4 (2 + n_req + n_alloc + n_evict) bytes,
+ * and returns a ticket (never 0).  arc_step_host_wait(ticket) blocks until that step is done and fills `out` with
+ * pointers into the pinned buffer, valid until the third arc_step_host_async after this step's.  Up to three steps may be
+ * in flight; a fourth arc_step_host_async before the oldest was waited for fails with ARC_ERR_INVALID_ARG and changes
+ * nothing.  h_tokens must stay valid and unchanged until its step has been waited for; h_offsets is copied before return.
+ * A step that needs larger buffers than the handle has (see arc_reserve) is accepted only with no step in flight.
+ * arc_step_host = arc_step_host_async + arc_step_host_wait. */
+int arc_step_host_async(arc_cache *h, const int32_t *h_tokens, const int64_t *h_offsets, uint32_t n_req, void *cuda_stream,
+                        uint32_t *ticket_out);
+int arc_step_host_wait(arc_cache *h, uint32_t ticket, arc_host_result *out);
 int arc_step_host(arc_cache *h, const int32_t *h_tokens, const int64_t *h_offsets, uint32_t n_req,
                   void *cuda_stream, arc_host_result *out);
 

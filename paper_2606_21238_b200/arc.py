@@ -27,7 +27,8 @@ STAT_FIELDS = ["steps", "requests", "tokens_seen", "tokens_hashed", "accesses", 
 EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats", "arc_reset", "arc_destroy",
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
            "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe", "arc_set_pin_scope",
-           "arc_release", "arc_hold_units", "arc_step_resume", "arc_debug_gather_sectors", "arc_hash_blocks_device"]
+           "arc_release", "arc_hold_units", "arc_step_resume", "arc_debug_gather_sectors", "arc_hash_blocks_device", "arc_step_host_async",
+           "arc_step_host_wait"]
 
 
 class ArcError(RuntimeError):
@@ -75,6 +76,8 @@ def load_library(path: Optional[Path] = None):
     L.arc_step.argtypes = [vp, vp, vp, u32, vp, C.POINTER(_StepResult)]
     L.arc_step_resume.argtypes = [vp, vp, vp, vp, u32, vp, C.POINTER(_StepResult)]
     L.arc_step_host.argtypes = [vp, vp, vp, u32, vp, C.POINTER(_HostResult)]
+    L.arc_step_host_async.argtypes = [vp, vp, vp, u32, vp, C.POINTER(u32)]
+    L.arc_step_host_wait.argtypes = [vp, u32, C.POINTER(_HostResult)]
     L.arc_stats.argtypes = [vp, C.POINTER(_Stats)]
     L.arc_reset.argtypes = [vp]
     L.arc_destroy.argtypes = [vp]
@@ -238,6 +241,31 @@ class ArcCache:
         take = lambda p, n: np.ctypeslib.as_array(p, shape=(n,)).copy() if n else np.zeros(0, np.int32)
         return dict(n_access=int(raw.n_access), prefix_len=take(raw.prefix_len, n_req), alloc_ids=take(raw.alloc_ids, raw.n_alloc),
                     evict_ids=take(raw.evict_ids, raw.n_evict), h2d_bytes=int(raw.h2d_bytes), d2h_bytes=int(raw.d2h_bytes))
+
+    def step_host_async(self, tokens: np.ndarray, offsets, stream=None) -> int:
+        """arc_step_host_async: enqueue the step from host memory (pinned memory keeps the copy asynchronous); returns the
+        ticket for step_host_wait.  Up to three steps may be in flight."""
+        t = np.ascontiguousarray(tokens, dtype=np.int32)
+        o = _offsets(offsets)
+        if o[-1] > t.size:
+            raise ValueError("offsets exceed the token array")
+        ticket = C.c_uint32()
+        self._check(self._L.arc_step_host_async(self._h, t.ctypes.data, o.ctypes.data, len(o) - 1, _stream_ptr(stream), C.byref(ticket)))
+        if not hasattr(self, "_inflight"):
+            self._inflight = {}
+        self._inflight[ticket.value] = (t, len(o) - 1)          # the tokens stay alive until the step has been waited for
+        return ticket.value
+
+    def step_host_wait(self, ticket: int, copy: bool = True) -> dict:
+        """arc_step_host_wait: blocks until the step is done; copy=False returns only the counts and byte counts."""
+        raw = _HostResult()
+        self._check(self._L.arc_step_host_wait(self._h, ticket, C.byref(raw)))
+        _, n_req = self._inflight.pop(ticket)
+        out = dict(n_access=int(raw.n_access), n_alloc=int(raw.n_alloc), n_evict=int(raw.n_evict), h2d_bytes=int(raw.h2d_bytes), d2h_bytes=int(raw.d2h_bytes))
+        if copy:
+            take = lambda p, n: np.ctypeslib.as_array(p, shape=(n,)).copy() if n else np.zeros(0, np.int32)
+            out.update(prefix_len=take(raw.prefix_len, n_req), alloc_ids=take(raw.alloc_ids, raw.n_alloc), evict_ids=take(raw.evict_ids, raw.n_evict))
+        return out
 
     def stats(self) -> dict:
         s = _Stats()

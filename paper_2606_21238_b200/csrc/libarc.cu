@@ -30,10 +30,11 @@ thread_local std::string g_create_error = "";
 std::atomic<uint64_t> g_hash_launches{0};
 
 constexpr int kStageSlots = 4;
+constexpr int kHostSlots = 3;                     // steps the host entry keeps in flight (arc_step_host_async)
 constexpr uint32_t kMaxReq = 1u << 20;
 constexpr uint64_t kMaxCapacity = 1ull << 28;   // node ids carry two flag bits
 constexpr uint32_t kSegEndCap = 1u << 16;       // n_req * segments-per-request the segmented K1 is used up to
-constexpr uint32_t kFusedAutoMax = 1024;        // steps of up to this many accesses take the one-launch kernel by default
+constexpr uint32_t kFusedAutoMax = 1536;        // steps of up to this many accesses take the one-launch kernel by default
 constexpr uint32_t kSegMaxReq = 512;            // with more requests than this one warp per request already fills the GPU
 
 uint32_t pow2_at_least(uint64_t x) {
@@ -98,9 +99,17 @@ struct arc_cache {
   cudaEvent_t stage_done[kStageSlots] = {};
   int stage_next = 0;
   // arc_step_host
-  int32_t* d_tokens_stage = nullptr;
-  uint64_t tokens_stage_cap = 0;
-  int32_t* h_result = nullptr;    // pinned: prefix_len[req_cap] | counts[2] | alloc[n_cap] | evict[n_cap]
+  // arc_step_host_async / _wait: kHostSlots steps in flight.  Per slot a device copy of the step's tokens (filled on the
+  // handle's own copy stream) and a pinned, device-mapped host buffer that K4's pack kernel writes the results into.
+  int32_t* d_tok[kHostSlots] = {};
+  uint64_t tok_cap[kHostSlots] = {};
+  int32_t* h_out[kHostSlots] = {};        // pinned + mapped: n_alloc | n_evict | prefix_len[n_req] | alloc_ids[n_alloc] | evict_ids[n_evict]
+  cudaEvent_t ev_h2d[kHostSlots] = {}, ev_comp[kHostSlots] = {};
+  uint32_t slot_ticket[kHostSlots] = {};  // 0 = free
+  uint32_t slot_n_req[kHostSlots] = {};
+  uint64_t slot_n_access[kHostSlots] = {}, slot_h2d[kHostSlots] = {};
+  uint32_t next_ticket = 1;
+  cudaStream_t copy_stream = nullptr;
   // host-side conservative bounds (no device read-back on the hot path)
   uint64_t slots_used_bound = 0;
   uint64_t window_bound[5] = {0, 0, 0, 0, 0};
@@ -199,7 +208,7 @@ struct StepBuffers {
   uint8_t* d_cls = nullptr;
   int32_t *d_block_id = nullptr, *d_evicted_id = nullptr, *d_p_after = nullptr;
   int64_t* h_stage = nullptr;
-  int32_t* h_result = nullptr;
+  int32_t* h_out[kHostSlots] = {};
 };
 
 void free_step_buffers(StepBuffers& b) {
@@ -207,8 +216,7 @@ void free_step_buffers(StepBuffers& b) {
   dfree(b.d_chain_state); dfree(b.d_cls); dfree(b.d_block_id); dfree(b.d_evicted_id); dfree(b.d_p_after);
   if (b.h_stage) cudaFreeHost(b.h_stage);
   b.h_stage = nullptr;
-  if (b.h_result) cudaFreeHost(b.h_result);
-  b.h_result = nullptr;
+  for (int k = 0; k < kHostSlots; ++k) { if (b.h_out[k]) cudaFreeHost(b.h_out[k]); b.h_out[k] = nullptr; }
 }
 
 int alloc_step_buffers(arc_cache* h, StepBuffers& b, uint32_t req_cap, uint64_t n_cap) {
@@ -223,7 +231,8 @@ int alloc_step_buffers(arc_cache* h, StepBuffers& b, uint32_t req_cap, uint64_t 
   CUDA_TRY(h, dalloc(&b.d_evicted_id, n_cap));
   CUDA_TRY(h, dalloc(&b.d_p_after, n_cap));
   CUDA_TRY(h, cudaMallocHost((void**)&b.h_stage, (size_t)kStageSlots * 2 * ((size_t)req_cap + 1) * sizeof(int64_t)));
-  CUDA_TRY(h, cudaMallocHost((void**)&b.h_result, ((size_t)req_cap + 2 + 2 * n_cap + 1) * sizeof(int32_t)));
+  for (int k = 0; k < kHostSlots; ++k)
+    CUDA_TRY(h, cudaHostAlloc((void**)&b.h_out[k], ((size_t)req_cap + 4 + 2 * n_cap) * sizeof(int32_t), cudaHostAllocMapped));
   return ARC_OK;
 }
 
@@ -231,14 +240,16 @@ StepBuffers take_step_buffers(arc_cache* h) {
   StepBuffers b;
   b.d_offsets = h->d_offsets; b.d_keys = h->d_keys; b.d_node_acc = h->d_node_acc; b.d_dropped = h->d_dropped;
   b.d_result_pack = h->d_result_pack; b.d_chain_state = h->d_chain_state; b.d_cls = h->d_cls; b.d_block_id = h->d_block_id;
-  b.d_evicted_id = h->d_evicted_id; b.d_p_after = h->d_p_after; b.h_stage = h->h_stage; b.h_result = h->h_result;
+  b.d_evicted_id = h->d_evicted_id; b.d_p_after = h->d_p_after; b.h_stage = h->h_stage;
+  for (int k = 0; k < kHostSlots; ++k) b.h_out[k] = h->h_out[k];
   return b;
 }
 
 void install_step_buffers(arc_cache* h, const StepBuffers& b, uint32_t req_cap, uint64_t n_cap) {
   h->d_offsets = b.d_offsets; h->d_keys = b.d_keys; h->d_node_acc = b.d_node_acc; h->d_dropped = b.d_dropped;
   h->d_result_pack = b.d_result_pack; h->d_chain_state = b.d_chain_state; h->d_cls = b.d_cls; h->d_block_id = b.d_block_id;
-  h->d_evicted_id = b.d_evicted_id; h->d_p_after = b.d_p_after; h->h_stage = b.h_stage; h->h_result = b.h_result;
+  h->d_evicted_id = b.d_evicted_id; h->d_p_after = b.d_p_after; h->h_stage = b.h_stage;
+  for (int k = 0; k < kHostSlots; ++k) h->h_out[k] = b.h_out[k];
   h->d_prefix_len = b.d_result_pack;
   h->d_alloc_ids = b.d_result_pack ? b.d_result_pack + req_cap + 2 : nullptr;
   h->d_evict_ids = b.d_result_pack ? h->d_alloc_ids + n_cap : nullptr;
@@ -580,13 +591,11 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
     k1_fill_args(k1_args, K1_ARG_SMALL, h_offsets, blk_off.data(), n_req);
     StepParams P = make_params(h);
     P.tokens = d_tokens; P.n_req = n_req; P.n_access = (uint32_t)N;
+    if (h->profiling) { cudaEventRecord(h->ev[2], s); cudaEventRecord(h->ev[3], s); }   // one kernel: its whole time is booked under the machine
     arc_fused_small_kernel<<<1, 2 * WIDE_W, K1_SMEM_BYTES, s>>>(P, reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state, h->d_offsets,
                                                              h->d_offsets + (h->req_cap + 1), (N < 48ull * n_req) ? 2 : 3, k1_args.small);
     h->launches += 1;
-    if (h->profiling) {                  // one kernel: its whole time is booked under the machine
-      cudaEventRecord(h->ev[2], s); cudaEventRecord(h->ev[3], s); cudaEventRecord(h->ev[4], s); cudaEventRecord(h->ev[5], s);
-      h->ev_valid = true;
-    }
+    if (h->profiling) { cudaEventRecord(h->ev[4], s); cudaEventRecord(h->ev[5], s); h->ev_valid = true; }
     CUDA_TRY(h, cudaGetLastError());
     return finish_step(h, h_offsets, n_req, N, s, P, out);
   }
@@ -650,9 +659,9 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
   return finish_step(h, h_offsets, n_req, N, s, P, out);
 }
 
-int arc_step_host(arc_cache* h, const int32_t* h_tokens, const int64_t* h_offsets, uint32_t n_req, void* cuda_stream, arc_host_result* out) {
+int arc_step_host_async(arc_cache* h, const int32_t* h_tokens, const int64_t* h_offsets, uint32_t n_req, void* cuda_stream, uint32_t* ticket_out) {
   if (!h) return ARC_ERR_INVALID_ARG;
-  if (!h_offsets || !out) return fail(h, ARC_ERR_INVALID_ARG, "NULL argument");
+  if (!h_offsets || !ticket_out) return fail(h, ARC_ERR_INVALID_ARG, "NULL argument");
   if (n_req > kMaxReq) return fail(h, ARC_ERR_INVALID_ARG, "n_req > 2^20");
   cudaStream_t s = (cudaStream_t)cuda_stream;
   uint64_t N = 0;
@@ -660,34 +669,77 @@ int arc_step_host(arc_cache* h, const int32_t* h_tokens, const int64_t* h_offset
   if (rc) return rc;
   const int64_t first = h_offsets[0], total = h_offsets[n_req] - first;
   if (!h_tokens && total > 0) return fail(h, ARC_ERR_INVALID_ARG, "h_tokens is NULL");
-  if ((uint64_t)total > h->tokens_stage_cap) {
-    CUDA_TRY(h, cudaStreamSynchronize(s));
-    dfree(h->d_tokens_stage);
-    h->tokens_stage_cap = std::max<uint64_t>((uint64_t)total, h->tokens_stage_cap * 2);
-    CUDA_TRY(h, dalloc(&h->d_tokens_stage, h->tokens_stage_cap));
+  const int k = (int)(h->next_ticket % kHostSlots);
+  if (h->slot_ticket[k]) return fail(h, ARC_ERR_INVALID_ARG, "%d steps are in flight: arc_step_host_wait(ticket %u) first", kHostSlots, h->slot_ticket[k]);
+  // growth (rare) drops the mapped result buffers of the steps in flight: only with none in flight
+  if (n_req > h->req_cap || N > h->n_cap) {
+    for (int q = 0; q < kHostSlots; ++q)
+      if (h->slot_ticket[q]) return fail(h, ARC_ERR_INVALID_ARG, "this step needs larger buffers: wait for the steps in flight first (or arc_reserve)");
+    rc = ensure_capacity(h, n_req, N, s);
+    if (rc) return rc;
   }
-  if (total) CUDA_TRY(h, cudaMemcpyAsync(h->d_tokens_stage, h_tokens + first, (size_t)total * sizeof(int32_t), cudaMemcpyHostToDevice, s));
-  // offsets relative to the staged copy
-  static thread_local std::vector<int64_t> rel;
+  if (!h->copy_stream) CUDA_TRY(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+  if (!h->ev_h2d[k]) {
+    CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_h2d[k], cudaEventDisableTiming));
+    CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_comp[k], cudaEventDisableTiming));
+  }
+  if ((uint64_t)total > h->tok_cap[k]) {
+    CUDA_TRY(h, cudaEventSynchronize(h->ev_comp[k]));           // the step that read this slot's tokens last has finished
+    dfree(h->d_tok[k]);
+    h->tok_cap[k] = std::max<uint64_t>((uint64_t)total, h->tok_cap[k] * 2);
+    CUDA_TRY(h, dalloc(&h->d_tok[k], h->tok_cap[k]));
+  }
+  // tokens: on the handle's copy stream, as soon as the slot's previous step is through with them - while the steps
+  // before this one are still computing on the caller's stream
+  CUDA_TRY(h, cudaStreamWaitEvent(h->copy_stream, h->ev_comp[k], 0));
+  if (total) CUDA_TRY(h, cudaMemcpyAsync(h->d_tok[k], h_tokens + first, (size_t)total * sizeof(int32_t), cudaMemcpyHostToDevice, h->copy_stream));
+  CUDA_TRY(h, cudaEventRecord(h->ev_h2d[k], h->copy_stream));
+  CUDA_TRY(h, cudaStreamWaitEvent(s, h->ev_h2d[k], 0));
+  static thread_local std::vector<int64_t> rel;             // offsets relative to the staged copy
   rel.resize((size_t)n_req + 1);
   for (uint32_t r = 0; r <= n_req; ++r) rel[r] = h_offsets[r] - first;
   arc_step_result res;
-  rc = arc_step(h, h->d_tokens_stage, rel.data(), n_req, cuda_stream, &res);
+  rc = arc_step(h, h->d_tok[k], rel.data(), n_req, cuda_stream, &res);
   if (rc) return rc;
-  int32_t* hp = h->h_result;
-  int32_t* h_counts = hp + h->req_cap;
-  int32_t* h_alloc = h_counts + 2;
-  int32_t* h_evict = h_alloc + h->n_cap;
-  // one copy: the device side keeps prefix_len | counts | alloc_ids | evict_ids in one buffer laid out like h_result
-  CUDA_TRY(h, cudaMemcpyAsync(hp, h->d_result_pack, ((size_t)h->req_cap + 2 + (N ? h->n_cap + N : 0)) * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-  CUDA_TRY(h, cudaStreamSynchronize(s));
-  out->n_access = N;
-  out->n_alloc = (uint32_t)h_counts[0]; out->n_evict = (uint32_t)h_counts[1];
-  out->prefix_len = hp; out->alloc_ids = h_alloc; out->evict_ids = h_evict;
-  out->h2d_bytes = (uint64_t)total * sizeof(int32_t) +
-                   2 * ((uint64_t)n_req + 1) * sizeof(int64_t);   // offsets and block offsets: kernel argument or staged copy
-  out->d2h_bytes = ((uint64_t)h->req_cap + 2 + (N ? h->n_cap + N : 0)) * sizeof(int32_t);
+  // results: packed by a kernel straight into pinned host memory (exactly the words that exist, no copy to size)
+  int32_t* d_view = nullptr;
+  CUDA_TRY(h, cudaHostGetDevicePointer((void**)&d_view, h->h_out[k], 0));
+  pack_results_kernel<<<grid_for(N + n_req, 1024, 32), 256, 0, s>>>(h->d_state, h->d_prefix_len, h->d_alloc_ids, h->d_evict_ids, n_req, d_view);
+  h->launches += 1;
+  CUDA_TRY(h, cudaGetLastError());
+  CUDA_TRY(h, cudaEventRecord(h->ev_comp[k], s));
+  h->slot_ticket[k] = h->next_ticket; h->slot_n_req[k] = n_req; h->slot_n_access[k] = N;
+  h->slot_h2d[k] = (uint64_t)total * sizeof(int32_t) + 2 * ((uint64_t)n_req + 1) * sizeof(int64_t);
+  *ticket_out = h->next_ticket;
+  h->next_ticket += 1;
+  if (h->next_ticket == 0) h->next_ticket = 1;
   return ARC_OK;
+}
+
+int arc_step_host_wait(arc_cache* h, uint32_t ticket, arc_host_result* out) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  if (!out || !ticket) return fail(h, ARC_ERR_INVALID_ARG, "NULL argument");
+  const int k = (int)(ticket % kHostSlots);
+  if (h->slot_ticket[k] != ticket) return fail(h, ARC_ERR_INVALID_ARG, "ticket %u is not in flight", ticket);
+  CUDA_TRY(h, cudaEventSynchronize(h->ev_comp[k]));
+  const int32_t* hp = h->h_out[k];
+  const uint32_t n_req = h->slot_n_req[k];
+  out->n_access = h->slot_n_access[k];
+  out->n_alloc = (uint32_t)hp[0]; out->n_evict = (uint32_t)hp[1];
+  out->prefix_len = hp + 2; out->alloc_ids = hp + 2 + n_req; out->evict_ids = hp + 2 + n_req + out->n_alloc;
+  out->h2d_bytes = h->slot_h2d[k];
+  out->d2h_bytes = (2ull + n_req + out->n_alloc + out->n_evict) * sizeof(int32_t);
+  h->slot_ticket[k] = 0;
+  return ARC_OK;
+}
+
+int arc_step_host(arc_cache* h, const int32_t* h_tokens, const int64_t* h_offsets, uint32_t n_req, void* cuda_stream, arc_host_result* out) {
+  if (!h) return ARC_ERR_INVALID_ARG;
+  if (!out) return fail(h, ARC_ERR_INVALID_ARG, "NULL argument");
+  uint32_t ticket = 0;
+  int rc = arc_step_host_async(h, h_tokens, h_offsets, n_req, cuda_stream, &ticket);
+  if (rc) return rc;
+  return arc_step_host_wait(h, ticket, out);
 }
 
 int arc_stats(arc_cache* h, arc_stats_t* out) {
@@ -724,6 +776,7 @@ int arc_reset(arc_cache* h) {
   if (h->d_node_of_block) CUDA_TRY(h, cudaMemset(h->d_node_of_block, 0xFF, (size_t)h->c * sizeof(uint32_t)));
   CUDA_TRY(h, cudaMemset(h->d_node_stamp, 0, (size_t)h->node_cap * sizeof(uint32_t)));
   h->hold_units = 0;
+  for (int k = 0; k < kHostSlots; ++k) h->slot_ticket[k] = 0;
   h->steps = h->requests = h->tokens_seen = h->tokens_hashed = 0;
   h->launches = 0;
   h->ev_valid = false;
@@ -736,7 +789,8 @@ void arc_destroy(arc_cache* h) {
   { StepBuffers b = take_step_buffers(h); free_step_buffers(b); }
   dfree(h->d_state); dfree(h->d_nodes); dfree(h->d_node_key); dfree(h->d_free_stack); dfree(h->d_table); dfree(h->d_node_stamp);
   for (int L = 1; L <= 4; ++L) { dfree(h->d_ring[L]); dfree(h->d_ring_alt[L]); }
-  dfree(h->d_block_counts); dfree(h->d_tokens_stage); dfree(h->d_machine_scratch);
+  dfree(h->d_block_counts); for (int k = 0; k < kHostSlots; ++k) { dfree(h->d_tok[k]); if (h->ev_h2d[k]) cudaEventDestroy(h->ev_h2d[k]); if (h->ev_comp[k]) cudaEventDestroy(h->ev_comp[k]); }
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream); dfree(h->d_machine_scratch);
   dfree(h->d_node_of_block); dfree(h->d_rel_cnt); dfree(h->d_seg_end);
   for (int i = 0; i < kStageSlots; ++i) if (h->stage_done[i]) cudaEventDestroy(h->stage_done[i]);
   for (int i = 0; i < 7; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);

@@ -239,6 +239,51 @@ def test_growth_reset_and_host_entry(arc):
     gc.close()
 
 
+def test_host_entry_pipelined(arc):
+    """arc_step_host_async / arc_step_host_wait: three steps in flight, the fourth refused, results (prefix lengths,
+    allocated and evicted IDs, in order) equal to the oracle's for every step; mixed with arc_step_host and arc_step."""
+    rng = np.random.default_rng(123)
+    c = 500
+    gc, oc = arc.ArcCache(c), O.OracleCache(c)
+    gc.reserve(64, 64 * 60)
+    docs = [rng.integers(0, 32000, size=16 * int(n) + int(rng.integers(0, 16)), dtype=np.int32) for n in rng.integers(1, 60, size=40)]
+    def batch():
+        reqs = [np.concatenate([docs[int(i)], rng.integers(0, 32000, size=int(rng.integers(0, 40)), dtype=np.int32)]) for i in rng.integers(0, 40, size=int(rng.integers(1, 30)))]
+        return W.pack_requests(reqs)
+    pinned = []
+    want = {}
+    inflight = []
+    for step in range(60):
+        tokens, offsets = batch()
+        buf = torch.from_numpy(tokens).pin_memory()
+        pinned.append(buf)
+        t = gc.step_host_async(buf.numpy(), offsets)
+        want[t] = oc.step(tokens, offsets)
+        inflight.append(t)
+        if len(inflight) == 3:
+            tk2, of2 = batch()
+            with pytest.raises(arc.ArcError):                      # a fourth step in flight is refused, nothing changes
+                gc.step_host_async(tk2, of2)
+            gc._inflight.pop(max(gc._inflight), None) if len(gc._inflight) > 3 else None
+        while len(inflight) > int(rng.integers(0, 3)):
+            tk = inflight.pop(0)
+            r, o = gc.step_host_wait(tk), want.pop(tk)
+            for k in ("prefix_len", "alloc_ids", "evict_ids"):
+                assert np.array_equal(r[k], o[k]), (step, k)
+            assert r["d2h_bytes"] == 4 * (2 + len(o["prefix_len"]) + len(o["alloc_ids"]) + len(o["evict_ids"]))
+    for tk in inflight:
+        r, o = gc.step_host_wait(tk), want.pop(tk)
+        assert np.array_equal(r["alloc_ids"], o["alloc_ids"])
+    tokens, offsets = batch()
+    h = gc.step_host(tokens, offsets)
+    o = oc.step(tokens, offsets)
+    assert np.array_equal(h["evict_ids"], o["evict_ids"]) and np.array_equal(h["prefix_len"], o["prefix_len"])
+    tokens, offsets = batch()
+    assert_same_step(gc.step(dev(tokens), offsets).to_host(), oc.step(tokens, offsets), "arc_step after host steps")
+    assert_same_state(gc, oc, "host entry")
+    gc.close()
+
+
 def test_maintenance_rebuild_and_compaction(arc):
     """Many small steps on one handle: the table rebuild and the ring compaction both trigger many times."""
     rng = np.random.default_rng(11)
