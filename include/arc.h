@@ -199,6 +199,13 @@ int arc_hash_blocks(const int32_t *d_tokens, const int64_t *h_offsets, uint32_t 
 int arc_hash_blocks_device(const int32_t *d_tokens, const int64_t *d_offsets, const int64_t *d_blk_off, uint32_t n_req,
                            uint32_t block_size, uint64_t *d_keys_out, uint32_t *d_ticket, void *cuda_stream);
 
+/* Prefix-affinity routing for N per-GPU caches behind a router: writes to
+ * d_dst_out[r] (DEVICE int32[n_req]) the shard of request r = (key of its first full block >> 33) mod world, 0 for a
+ * request shorter than one block - requests that share a document or conversation prefix meet in the same cache.
+ * d_tokens DEVICE, d_offsets DEVICE int64[n_req+1].  Stateless, one kernel, asynchronous on cuda_stream. */
+int arc_route_requests(const int32_t *d_tokens, const int64_t *d_offsets, uint32_t n_req, uint32_t block_size, uint32_t world,
+                       int32_t *d_dst_out, void *cuda_stream);
+
 /* Diagnostics ------------------------------------------------------------------------------------ */
 
 /* When enabled, arc_step records CUDA events between its kernels (on the step's stream); the times of

@@ -28,7 +28,7 @@ EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats"
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
            "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe", "arc_set_pin_scope",
            "arc_release", "arc_hold_units", "arc_step_resume", "arc_debug_gather_sectors", "arc_hash_blocks_device", "arc_step_host_async",
-           "arc_step_host_wait"]
+           "arc_step_host_wait", "arc_route_requests"]
 
 
 class ArcError(RuntimeError):
@@ -86,6 +86,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_last_error.restype = C.c_char_p
     L.arc_hash_blocks.argtypes = [vp, vp, u32, u32, vp, vp]
     L.arc_hash_blocks_device.argtypes = [vp, vp, vp, u32, u32, vp, vp, vp]
+    L.arc_route_requests.argtypes = [vp, vp, u32, u32, u32, vp, vp]
     L.arc_set_profiling.argtypes = [vp, C.c_int]
     L.arc_last_kernel_times.argtypes = [vp, C.POINTER(_KernelTimes)]
     L.arc_launch_count.argtypes = [vp]
@@ -357,6 +358,21 @@ def hash_blocks_device(tokens, d_offsets, d_blk_off, n_req: int, out, ticket, bl
     if rc != OK:
         raise ArcError(rc, L.arc_last_error(None).decode())
     return out
+
+
+def route_requests(tokens, offsets, world: int, block_size: int = 16, stream=None):
+    """arc_route_requests: destination shard of every request, computed on the device from its first block's key; returns a
+    CUDA int32 tensor [n_req].  offsets: host int64[n_req+1] (copied to the device here) or a CUDA int64 tensor."""
+    torch = _torch()
+    L = load_library()
+    if not (hasattr(offsets, "is_cuda") and offsets.is_cuda):
+        offsets = torch.from_numpy(_offsets(offsets)).to(tokens.device, non_blocking=True)
+    n_req = offsets.numel() - 1
+    dst = torch.empty(n_req, dtype=torch.int32, device=tokens.device)
+    rc = L.arc_route_requests(tokens.data_ptr(), offsets.data_ptr(), n_req, block_size, world, dst.data_ptr(), _stream_ptr(stream))
+    if rc != OK:
+        raise ArcError(rc, L.arc_last_error(None).decode())
+    return dst
 
 
 def debug_gather_sectors(keys, buf, out=None, stream=None):

@@ -471,6 +471,25 @@ __global__ void __launch_bounds__(256) hash_fixup_kernel(const int64_t* __restri
   }
 }
 
+// Prefix-affinity routing: destination shard of every request = (key of its FIRST block >> 33) mod
+// world, 0 for a request without a full block.  One thread per request: 16 tokens, H3, one step of H4 from S0, H5.
+__global__ void __launch_bounds__(256) route_first_block_kernel(const int32_t* __restrict__ tokens, const int64_t* __restrict__ offsets, uint32_t n_req,
+                                                                uint32_t world, int32_t* __restrict__ dst) {
+  const uint32_t* tok = reinterpret_cast<const uint32_t*>(tokens);
+  for (uint32_t r = blockIdx.x * blockDim.x + threadIdx.x; r < n_req; r += gridDim.x * blockDim.x) {
+    const int64_t a = offsets[r], len = offsets[r + 1] - a;
+    int32_t d = 0;
+    if (len >= 16) {
+      unsigned long long g = 0;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) g += hash_word(__ldg(tok + a + 2 * k), __ldg(tok + a + 2 * k + 1), (unsigned long long)(k + 1) * H_M);
+      const unsigned long long key = finalize_key(H_S0 * H_K + g);
+      d = (int32_t)((key >> 33) % world);
+    }
+    dst[r] = d;
+  }
+}
+
 __global__ void fill_u64_kernel(unsigned long long* p, uint32_t n, unsigned long long v) {
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) p[i] = v;
 }

@@ -883,6 +883,19 @@ int arc_hash_blocks(const int32_t* d_tokens, const int64_t* h_offsets, uint32_t 
   return ARC_OK;
 }
 
+int arc_route_requests(const int32_t* d_tokens, const int64_t* d_offsets, uint32_t n_req, uint32_t block_size, uint32_t world, int32_t* d_dst_out,
+                       void* cuda_stream) {
+  if (n_req > kMaxReq || world == 0) return fail(nullptr, ARC_ERR_INVALID_ARG, "n_req > 2^20 or world = 0");
+  if (block_size != 16) return fail(nullptr, ARC_ERR_UNSUPPORTED, "block_size %u: only 16 is built", block_size);
+  if (!n_req) return ARC_OK;
+  if (!d_offsets || !d_dst_out) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
+  route_first_block_kernel<<<grid_for(n_req, 256, 148 * 4), 256, 0, (cudaStream_t)cuda_stream>>>(d_tokens, d_offsets, n_req, world, d_dst_out);
+  g_hash_launches += 1;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "route launch: %s", cudaGetErrorString(e));
+  return ARC_OK;
+}
+
 int arc_hash_blocks_device(const int32_t* d_tokens, const int64_t* d_offsets, const int64_t* d_blk_off, uint32_t n_req, uint32_t block_size,
                            uint64_t* d_keys_out, uint32_t* d_ticket, void* cuda_stream) {
   if (n_req > kMaxReq) return fail(nullptr, ARC_ERR_INVALID_ARG, "n_req > 2^20");

@@ -83,23 +83,12 @@ class ShardedArc:
         self.caches = {s: A.ArcCache(capacity_blocks_per_shard, block_size, policy) for s in shards}
 
     def route(self, tokens, offsets):
-        """Destination shard of every request: by its first block's key (K1 on the first 16 tokens of each request);
-        requests without a full block go to shard 0 (they make no access anywhere)."""
+        """Destination shard of every request: by its first block's key, computed by ONE kernel on the device
+        (arc_route_requests); requests without a full block go to shard 0 (they make no access anywhere).  The result comes
+        back to the host (4 bytes per request) because arc_step takes its batch layout from host offsets."""
         import numpy as np
-        import torch
 
-        o = np.asarray(offsets, dtype=np.int64)
-        starts, has = first_block_offsets(o, self.B)
-        dst = np.zeros(len(starts), dtype=np.int64)
-        if has.any():
-            # one-block requests: [start, start + B) for every request that has a full block
-            sel = starts[has]
-            first = torch.stack([tokens[int(s):int(s) + self.B] for s in sel]).reshape(-1) if len(sel) < 64 else \
-                tokens[(torch.from_numpy(sel).to(tokens.device)[:, None] + torch.arange(self.B, device=tokens.device)[None, :]).reshape(-1)]
-            fo = np.arange(len(sel) + 1, dtype=np.int64) * self.B
-            keys = self._A.hash_blocks(first.contiguous(), fo, self.B).cpu().numpy().view(np.uint64)
-            dst[has] = route_requests(keys, self.world)
-        return dst
+        return self._A.route_requests(tokens, np.asarray(offsets, dtype=np.int64), self.world, self.B).cpu().numpy().astype(np.int64)
 
     def step(self, tokens, offsets):
         """-> {shard: (request indices, StepResult)} for the shards that live in this process."""

@@ -120,3 +120,58 @@ def test_prefix_affinity_shards_match_per_shard_oracles():
     assert tot["accesses"] == sum(o.stats()["accesses"] for o in oracles)
     assert tot["hit_t1"] + tot["hit_t2"] == sum(o.stats()["hit_t1"] + o.stats()["hit_t2"] for o in oracles)
     sh.close()
+
+
+def _sharded_rank_worker(rank, world, port, q):
+    import os
+
+    import torch.distributed as dist
+
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", rank))
+    from paper_2606_21238_b200 import parallel as P
+
+    c = 48
+    sh = P.ShardedArc(c, world, rank=rank)
+    oc = O.OracleCache(c, 16, 0)
+    tr = W.make_trace(1, seed=2)
+    ok = True
+    for tokens, offsets in tr.steps(max_steps=40):
+        dev_tokens = torch.from_numpy(tokens).cuda()
+        dst = sh.route(dev_tokens, offsets)
+        (idx, g), = sh.step(dev_tokens, offsets).values()
+        _, sub, slices = P.split_batch(offsets, dst, rank)
+        sub_tokens = np.concatenate([tokens[a:b] for a, b in slices]) if slices else np.zeros(0, np.int32)
+        o = oc.step(sub_tokens, sub)
+        g = g.to_host()
+        ok = ok and all(np.array_equal(g[k], o[k]) for k in OUT_KEYS)
+    tot = sh.stats(dist, torch)                               # one all-reduce over NCCL
+    q.put((rank, ok, tot["accesses"], oc.stats()["accesses"]))
+    sh.close()
+    dist.destroy_process_group()
+
+
+def test_prefix_affinity_shards_one_process_per_gpu_over_nccl():
+    """NEXT-4 as it would be deployed: one process per GPU, every rank owns one shard, routing on the device, counters
+    summed with one NCCL all-reduce.  Needs two GPUs; on a one-GPU box it is skipped (visibly)."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip(f"needs >= 2 CUDA devices, this box has {torch.cuda.device_count()}: the one-process-per-GPU mode has not run on hardware")
+    import socket
+
+    import torch.multiprocessing as mp
+
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_sharded_rank_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=300) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert all(ok for _, ok, _, _ in got)
+    assert got[0][2] == got[1][2] == got[0][3] + got[1][3]    # the all-reduced total is the sum of the shards' oracles
