@@ -38,7 +38,15 @@ class _Result(C.Structure):
 
 
 def build(force: bool = False) -> Path:
-    """g++ -O2, no SIMD intrinsics.  Building the checker is not using it."""
+    """g++ -O2, no SIMD intrinsics.  Building the checker is not using it.  With ARC_ORACLE_SANITIZE=1 in
+    the environment the library is built and loaded with -fsanitize=address,undefined instead (a separate file; the
+    process must then run with libasan preloaded: tests/test_oracle_sanitized.py)."""
+    if os.environ.get("ARC_ORACLE_SANITIZE") == "1":
+        lib = _HERE / "liboracle_san.so"
+        if force or not lib.exists() or lib.stat().st_mtime < _SRC.stat().st_mtime:
+            subprocess.check_call(["g++", "-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+                                   "-std=c++17", "-shared", "-fPIC", "-o", str(lib), str(_SRC)])
+        return lib
     if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
         subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-o", str(_LIB), str(_SRC)])
     return _LIB
