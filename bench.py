@@ -428,6 +428,8 @@ def k1_bulk_roofline(torch, A, gib, stream, seed):
     out = torch.empty(n_blocks, dtype=torch.int64, device="cuda")
 
     def timed(fn, reps=10, warm=10):
+        """-> (mean and minimum of `reps` launches timed one by one with their own CUDA event pairs, as in round 1; average
+        duration of the same launches enqueued back to back under ONE event pair: the chip under sustained load)."""
         for _ in range(warm):
             fn()
         evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
@@ -438,10 +440,16 @@ def k1_bulk_roofline(torch, A, gib, stream, seed):
             b.record(stream)
         stream.synchronize()
         ms = sorted(a.elapsed_time(b) for a, b in evs)
-        return float(np.mean(ms)), ms[0]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        stream.synchronize()
+        return float(np.mean(ms)), ms[0], e0.elapsed_time(e1) / reps
 
     # through the API: host offsets in, the call copies them (its own copy stream) and launches
-    api_mean, api_best = timed(lambda: A.hash_blocks(tokens, offs, 16, out=out, stream=stream))
+    api_mean, api_best, api_b2b = timed(lambda: A.hash_blocks(tokens, offs, 16, out=out, stream=stream))
     keys_api = out.clone()
     # the kernel alone: offsets and block offsets already on the device
     d_off = torch.from_numpy(offs).cuda()
@@ -450,10 +458,10 @@ def k1_bulk_roofline(torch, A, gib, stream, seed):
     d_blk = torch.from_numpy(blk).cuda()
     ticket = torch.zeros(2, dtype=torch.int32, device="cuda")
     out.zero_()
-    ker_mean, ker_best = timed(lambda: A.hash_blocks_device(tokens, d_off, d_blk, len(offs) - 1, out, ticket, stream=stream))
+    ker_mean, ker_best, ker_b2b = timed(lambda: A.hash_blocks_device(tokens, d_off, d_blk, len(offs) - 1, out, ticket, stream=stream))
     same = bool(torch.equal(out, keys_api))
     return dict(blocks=n_blocks, requests=len(offs) - 1, api_ms=api_mean, api_best_ms=api_best, kernel_ms=ker_mean, kernel_best_ms=ker_best,
-                same_keys=same)
+                api_back_to_back_ms=api_b2b, kernel_back_to_back_ms=ker_b2b, same_keys=same)
 
 
 def k2_probe_bench(torch, A, stream, seed, peak, n_keys=1 << 24):
@@ -746,6 +754,9 @@ def run_ours(args):
                             "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
                             "algorithmic_bytes_per_launch": ALGO_BYTES_PER_BLOCK * k1["blocks"],
                             "ms_per_launch_api": k1["api_ms"], "ms_per_launch_kernel": k1["kernel_ms"], "best_ms_api": k1["api_best_ms"], "best_ms_kernel": k1["kernel_best_ms"],
+                            "back_to_back": {"what": "the same 10 launches enqueued back to back under one event pair (sustained load)",
+                                             "ms_api": k1["api_back_to_back_ms"], "ms_kernel": k1["kernel_back_to_back_ms"],
+                                             "frac_api": gb / (k1["api_back_to_back_ms"] * 1e-3) / peak, "frac_kernel": gb / (k1["kernel_back_to_back_ms"] * 1e-3) / peak},
                             "api": "arc_hash_blocks (host offsets in, copied by the call)", "kernel_only": "arc_hash_blocks_device (offsets already on the device)",
                             "same_keys_both_ways": k1["same_keys"], "tokens_per_s": 16 * k1["blocks"] / (k1["api_ms"] * 1e-3),
                             "workload": f"{k1['requests']} D5-shaped requests, {k1['blocks']} blocks, {64 * k1['blocks'] / 2**30:.2f} GiB of tokens (>> 126 MB L2)",
