@@ -191,12 +191,18 @@ const char *arc_last_error(const arc_cache *h);
 int arc_hash_blocks(const int32_t *d_tokens, const int64_t *h_offsets, uint32_t n_req, uint32_t block_size,
                     uint64_t *d_keys_out, void *cuda_stream);
 
-/* The same kernel with everything already on the device: the kernel-only figure of the K1 roofline run, and for callers
- * that build their batch on the device.  d_offsets / d_blk_off: DEVICE int64[n_req+1] (token offsets; exclusive scan of
- * the full blocks per request).  d_ticket: DEVICE, two uint32 words of caller-owned scratch that must be 0 at launch;
- * the kernel leaves them 0 again, so one scratch zeroed once serves every later call ON THE SAME STREAM (calls that may
- * run at the same time need scratch of their own).  Nothing is validated or copied; one kernel launch. */
-int arc_hash_blocks_device(const int32_t *d_tokens, const int64_t *d_offsets, const int64_t *d_blk_off, uint32_t n_req,
+/* One entry of the work list of the bulk hashing kernel: a request (or any run of full blocks) of n_blocks blocks whose
+ * tokens start at d_tokens[tok_off] and whose keys go to d_keys_out[key_off ..].  32 bytes. */
+typedef struct { int64_t tok_off; int64_t key_off; uint32_t n_blocks; uint32_t reserved[3]; } arc_hash_item;
+
+/* The bulk hashing kernel with its work list already on the device: the kernel-only figure of the K1 roofline run, and
+ * for callers that build their batch on the device.  arc_hash_blocks builds exactly this list from the host offsets (one
+ * item per request with a full block, longest first) and copies it.  d_items: DEVICE arc_hash_item[n_items]; warps take
+ * the items in list order.  [tok_lo, tok_hi): the token indices of d_tokens the kernel may touch (the 16-byte-aligned
+ * bulk copies read nothing outside it).  d_ticket: DEVICE, two uint32 words of caller-owned scratch that must be 0 at
+ * launch; the kernel leaves them 0 again, so one scratch zeroed once serves every later call ON THE SAME STREAM (calls
+ * that may run at the same time need scratch of their own).  Nothing is validated or copied; one kernel launch. */
+int arc_hash_blocks_device(const int32_t *d_tokens, const arc_hash_item *d_items, uint32_t n_items, int64_t tok_lo, int64_t tok_hi,
                            uint32_t block_size, uint64_t *d_keys_out, uint32_t *d_ticket, void *cuda_stream);
 
 /* Prefix-affinity routing for N per-GPU caches behind a router: writes to

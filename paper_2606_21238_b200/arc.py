@@ -85,7 +85,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_last_error.argtypes = [vp]
     L.arc_last_error.restype = C.c_char_p
     L.arc_hash_blocks.argtypes = [vp, vp, u32, u32, vp, vp]
-    L.arc_hash_blocks_device.argtypes = [vp, vp, vp, u32, u32, vp, vp, vp]
+    L.arc_hash_blocks_device.argtypes = [vp, vp, u32, C.c_int64, C.c_int64, u32, vp, vp, vp]
     L.arc_route_requests.argtypes = [vp, vp, u32, u32, u32, vp, vp]
     L.arc_set_profiling.argtypes = [vp, C.c_int]
     L.arc_last_kernel_times.argtypes = [vp, C.POINTER(_KernelTimes)]
@@ -341,19 +341,35 @@ def hash_blocks(tokens, offsets, block_size: int = 16, out=None, stream=None):
     torch = _torch()
     L = load_library()
     o = _offsets(offsets)
-    n = int((np.diff(o) // block_size).sum())
     if out is None:
-        out = torch.empty(n, dtype=torch.int64, device="cuda")
+        out = torch.empty(int((np.diff(o) // block_size).sum()), dtype=torch.int64, device="cuda")
     rc = L.arc_hash_blocks(tokens.data_ptr(), o.ctypes.data, len(o) - 1, block_size, out.data_ptr(), _stream_ptr(stream))
     if rc != OK:
         raise ArcError(rc, L.arc_last_error(None).decode())
     return out
 
 
-def hash_blocks_device(tokens, d_offsets, d_blk_off, n_req: int, out, ticket, block_size: int = 16, stream=None):
-    """arc_hash_blocks_device: offsets and block offsets are CUDA int64 tensors, ticket a zeroed CUDA int32[2] scratch."""
+HASH_ITEM = np.dtype([("tok_off", "<i8"), ("key_off", "<i8"), ("n_blocks", "<u4"), ("reserved", "<u4", (3,))])   # arc_hash_item
+
+
+def hash_items(offsets, block_size: int = 16) -> np.ndarray:
+    """The work list arc_hash_blocks builds from host offsets: one HASH_ITEM per request with a full block, requests of
+    >= 1024 / 384 / 128 / fewer blocks in that order (input marshalling for arc_hash_blocks_device)."""
+    o = _offsets(offsets)
+    nb = np.diff(o) // block_size
+    key_off = np.concatenate([[0], np.cumsum(nb)])[:-1]
+    cls = np.where(nb >= 1024, 0, np.where(nb >= 384, 1, np.where(nb >= 128, 2, 3)))
+    idx = np.flatnonzero(nb > 0)
+    idx = idx[np.argsort(cls[idx], kind="stable")]
+    items = np.zeros(len(idx), HASH_ITEM)
+    items["tok_off"], items["key_off"], items["n_blocks"] = o[:-1][idx], key_off[idx], nb[idx]
+    return items
+
+
+def hash_blocks_device(tokens, d_items, n_items: int, tok_lo: int, tok_hi: int, out, ticket, block_size: int = 16, stream=None):
+    """arc_hash_blocks_device: d_items = CUDA uint8 tensor holding HASH_ITEM records, ticket a zeroed CUDA int32[2] scratch."""
     L = load_library()
-    rc = L.arc_hash_blocks_device(tokens.data_ptr(), d_offsets.data_ptr(), d_blk_off.data_ptr(), n_req, block_size, out.data_ptr(),
+    rc = L.arc_hash_blocks_device(tokens.data_ptr(), d_items.data_ptr(), n_items, tok_lo, tok_hi, block_size, out.data_ptr(),
                                   ticket.data_ptr(), _stream_ptr(stream))
     if rc != OK:
         raise ArcError(rc, L.arc_last_error(None).decode())

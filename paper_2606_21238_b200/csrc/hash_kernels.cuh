@@ -364,6 +364,53 @@ __global__ void __launch_bounds__(256, 3) hash_blocks_kernel(const int32_t* __re
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
+// The stateless bulk form (arc_hash_blocks): the host, which validates the offsets anyway, hands the kernel a WORK LIST -
+// one item per request with at least one full block, longest length class first (the same longest-processing-time-first
+// order the ticket passes above produce, without the tickets that find nothing) - and a warp always knows its NEXT
+// item: the ticket for the item after next is requested, and the next item is loaded, while the current one is hashed,
+// so neither the atomic nor the metadata load is ever waited for.  Keys in natural order, no chain states.
+struct __align__(16) HashItem { long long tok_off; long long key_off; uint32_t n_blocks; uint32_t reserved[3]; };   // 32 bytes = arc_hash_item (arc.h)
+
+__global__ void __launch_bounds__(256, 3) hash_items_kernel(const int32_t* __restrict__ tokens, const HashItem* __restrict__ items, uint32_t n_items,
+                                                            int64_t lo, int64_t hi, unsigned long long* __restrict__ keys, uint32_t* __restrict__ ticket) {
+  extern __shared__ __align__(128) unsigned char k1_smem[];
+  const int lane = threadIdx.x & 31;
+  const uint32_t* tok = reinterpret_cast<const uint32_t*>(tokens);
+  const LaneConsts LC = lane_consts(lane);
+  WarpPipe W = pipe_init(k1_smem, threadIdx.x >> 5, lane);
+  const int base_mis = (int)((reinterpret_cast<uintptr_t>(tok) >> 2) & 3);
+  uint32_t t_req = 0;                                   // lane 0: the ticket last requested
+  if (lane == 0) t_req = atomicAdd(ticket, 1u);
+  uint32_t t = __shfl_sync(0xFFFFFFFFu, t_req, 0);
+  if (t < n_items) {
+    const uint4* ip = reinterpret_cast<const uint4*>(items + t);     // 32-byte items: two aligned 16-byte loads
+    uint4 a = __ldg(ip);
+    uint4 b = __ldg(ip + 1);
+    if (lane == 0) t_req = atomicAdd(ticket, 1u);
+    for (;;) {
+      const long long tok_off = (long long)((unsigned long long)a.x | ((unsigned long long)a.y << 32));
+      const long long key_off = (long long)((unsigned long long)a.z | ((unsigned long long)a.w << 32));
+      const uint32_t nb = b.x;
+      // the item after this one: its ticket was requested an item ago; its words are on their way while this one is hashed
+      const uint32_t tn = __shfl_sync(0xFFFFFFFFu, t_req, 0);
+      uint4 na = make_uint4(0, 0, 0, 0), nbv = make_uint4(0, 0, 0, 0);
+      if (tn < n_items) {
+        const uint4* np = reinterpret_cast<const uint4*>(items + tn);
+        na = __ldg(np);
+        nbv = __ldg(np + 1);
+        if (lane == 0) t_req = atomicAdd(ticket, 1u);
+      }
+      unsigned long long* out = keys + (key_off + lane);
+      hash_run(W, tok, base_mis, lo, hi, tok_off, nb, H_S0, lane, LC,
+        [&](uint32_t rb, int cnt, unsigned long long st) { if (lane < cnt) out[rb] = finalize_key(st); });
+      if (tn >= n_items) break;
+      a = na; b = nbv;
+    }
+  }
+  k1_leave(ticket, lane);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
 // In-step hashing of steps with FEW requests: one warp per request leaves the step waiting for its longest request (a
 // 1,000-block document is 32 dependent rounds).  H4 is affine, so a request is cut into segments of K1_SEG blocks that are
 // scanned independently from a zero carry (hash_segments_kernel: one warp per segment, the same staging and scans as

@@ -406,7 +406,7 @@ int validate_offsets(arc_cache* h, const int64_t* off, uint32_t n_req, uint32_t 
   uint64_t N = 0;
   for (uint32_t r = 0; r < n_req; ++r) {
     if (off[r + 1] < off[r]) return fail(h, ARC_ERR_INVALID_ARG, "h_offsets not monotone at request %u", r);
-    const uint64_t nb = (uint64_t)(off[r + 1] - off[r]) / B;
+    const uint64_t nb = (B == 16) ? ((uint64_t)(off[r + 1] - off[r]) >> 4) : ((uint64_t)(off[r + 1] - off[r]) / B);
     if (c && nb > c) return fail(h, ARC_ERR_REQUEST_TOO_LARGE, "request %u has %llu blocks > capacity %llu", r, (unsigned long long)nb, (unsigned long long)c);
     if (blk_off_out) blk_off_out[r] = (int64_t)N;
     N += nb;
@@ -440,6 +440,7 @@ cudaError_t k1_configure() {
   K1_ATTR((hash_segments_kernel<(int)K1_INLINE_SMALL>));
   K1_ATTR((hash_segments_kernel<(int)K1_INLINE_LARGE>));
   K1_ATTR(arc_fused_small_kernel);
+  K1_ATTR(hash_items_kernel);
 #undef K1_ATTR
   if (dev >= 0 && dev < 64) done[dev] = true;
   return cudaSuccess;
@@ -824,13 +825,6 @@ int arc_hash_blocks(const int32_t* d_tokens, const int64_t* h_offsets, uint32_t 
   if (n_req > kMaxReq) return fail(nullptr, ARC_ERR_INVALID_ARG, "n_req > 2^20");
   if (block_size != 16) return fail(nullptr, ARC_ERR_UNSUPPORTED, "block_size %u: only 16 is built", block_size);
   cudaStream_t s = (cudaStream_t)cuda_stream;
-  static thread_local std::vector<int64_t> blk_off;
-  blk_off.resize((size_t)n_req + 1);
-  uint64_t N = 0;
-  int rc = validate_offsets(nullptr, h_offsets, n_req, block_size, 0, blk_off.data(), &N);
-  if (rc) return rc;
-  if (N && (!d_tokens || !d_keys_out)) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
-  if (!N) return ARC_OK;
   cudaError_t e = k1_configure();
   if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "K1 configuration: %s", cudaGetErrorString(e));
   int dev = 0;
@@ -853,12 +847,14 @@ int arc_hash_blocks(const int32_t* d_tokens, const int64_t* h_offsets, uint32_t 
   HashSlot& k = g_hash.slot[g_hash.next];
   g_hash.next = (g_hash.next + 1) % 8;
   if (!k.copied) { cudaEventCreateWithFlags(&k.copied, cudaEventDisableTiming); cudaEventCreateWithFlags(&k.done, cudaEventDisableTiming); }
-  const size_t need = 2 + 2 * ((size_t)n_req + 1);                 // two ticket words (one int64), padding, offsets, block offsets
+  // host staging: 16 bytes of ticket words, then one region of n_req items per length class (the classes' sizes are only
+  // known after the pass); device: the ticket words, then the items, classes back to back.  Sizes in int64 entries.
+  const size_t need = 2 + 4 * (size_t)K1_PASSES * n_req;
   cudaEventSynchronize(k.done);                                     // the kernel that read this slot last has finished
   if (need > k.cap) {
     if (k.h_buf) cudaFreeHost(k.h_buf);
     if (k.d_buf) cudaFree(k.d_buf);
-    k.cap = std::max<size_t>(need, 1024);
+    k.cap = std::max<size_t>(need, 4096);
     if (cudaMallocHost((void**)&k.h_buf, k.cap * sizeof(int64_t)) != cudaSuccess || cudaMalloc((void**)&k.d_buf, k.cap * sizeof(int64_t)) != cudaSuccess) {
       if (k.h_buf) cudaFreeHost(k.h_buf);
       k.h_buf = nullptr; k.d_buf = nullptr; k.cap = 0;
@@ -866,16 +862,41 @@ int arc_hash_blocks(const int32_t* d_tokens, const int64_t* h_offsets, uint32_t 
       return fail(nullptr, ARC_ERR_OOM, "scratch allocation failed");
     }
   }
-  k.h_buf[0] = 0; k.h_buf[1] = 0;                                   // the ticket words travel with the offsets
-  memcpy(k.h_buf + 2, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
-  memcpy(k.h_buf + 2 + (n_req + 1), blk_off.data(), ((size_t)n_req + 1) * sizeof(int64_t));
-  e = cudaMemcpyAsync(k.d_buf, k.h_buf, need * sizeof(int64_t), cudaMemcpyHostToDevice, g_hash.copy_stream);
+  // ONE pass over the offsets: validation, blocks per request (block_size is 16: a shift), and the work list - one
+  // 32-byte item per request with a full block, written to the region of its length class (longest class first on the
+  // device: the order the ticket passes of the in-step kernel produce, without the tickets that find nothing)
+  if (h_offsets[0] < 0) return fail(nullptr, ARC_ERR_INVALID_ARG, "h_offsets[0] < 0");
+  HashItem* region[K1_PASSES];
+  for (int c = 0; c < K1_PASSES; ++c) region[c] = reinterpret_cast<HashItem*>(k.h_buf + 2) + (size_t)c * n_req;
+  uint32_t cnt[K1_PASSES] = {};
+  uint64_t N = 0;
+  for (uint32_t r = 0; r < n_req; ++r) {
+    const int64_t len = h_offsets[r + 1] - h_offsets[r];
+    if (len < 0) return fail(nullptr, ARC_ERR_INVALID_ARG, "h_offsets not monotone at request %u", r);
+    const uint64_t nb = (uint64_t)len >> 4;
+    if (nb >= (1ull << 28)) return fail(nullptr, ARC_ERR_INVALID_ARG, "request %u is too large", r);
+    const uint32_t c = (uint32_t)(nb < 1024) + (uint32_t)(nb < 384) + (uint32_t)(nb < 128);      // = k1_class
+    HashItem& it = region[c][cnt[c]];
+    it.tok_off = h_offsets[r]; it.key_off = (long long)N; it.n_blocks = (uint32_t)nb; it.reserved[0] = it.reserved[1] = it.reserved[2] = 0;
+    cnt[c] += nb != 0;                                               // a request without a full block leaves no item
+    N += nb;
+  }
+  if (N >= (1ull << 31)) return fail(nullptr, ARC_ERR_INVALID_ARG, "%llu blocks in one call is too large", (unsigned long long)N);
+  if (!N) return ARC_OK;
+  if (!d_tokens || !d_keys_out) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
+  k.h_buf[0] = 0; k.h_buf[1] = 0;                                   // the ticket words travel with the items
+  e = cudaMemcpyAsync(k.d_buf, k.h_buf, 2 * sizeof(int64_t), cudaMemcpyHostToDevice, g_hash.copy_stream);
+  uint32_t n_items = 0;
+  for (int c = 0; c < K1_PASSES && e == cudaSuccess; ++c) {
+    if (cnt[c]) e = cudaMemcpyAsync(reinterpret_cast<HashItem*>(k.d_buf + 2) + n_items, region[c], (size_t)cnt[c] * sizeof(HashItem), cudaMemcpyHostToDevice, g_hash.copy_stream);
+    n_items += cnt[c];
+  }
   if (e == cudaSuccess) e = cudaEventRecord(k.copied, g_hash.copy_stream);
   if (e == cudaSuccess) e = cudaStreamWaitEvent(s, k.copied, 0);
-  if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "offset copy: %s", cudaGetErrorString(e));
-  static const K1HostArgs no_args = {};
-  launch_hash_blocks(false, K1_ARG_NONE, no_args, d_tokens, k.d_buf + 2, k.d_buf + 2 + (n_req + 1), n_req, (unsigned long long*)d_keys_out,
-                     reinterpret_cast<uint32_t*>(k.d_buf), s, nullptr, nullptr);
+  if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "work list copy: %s", cudaGetErrorString(e));
+  hash_items_kernel<<<grid_for(n_items, K1_WARPS, 148 * 3), 256, K1_SMEM_BYTES, s>>>(d_tokens, reinterpret_cast<const HashItem*>(k.d_buf + 2), n_items,
+                                                                                  h_offsets[0], h_offsets[n_req], (unsigned long long*)d_keys_out,
+                                                                                  reinterpret_cast<uint32_t*>(k.d_buf));
   g_hash_launches += 1;
   e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaEventRecord(k.done, s);
@@ -896,17 +917,17 @@ int arc_route_requests(const int32_t* d_tokens, const int64_t* d_offsets, uint32
   return ARC_OK;
 }
 
-int arc_hash_blocks_device(const int32_t* d_tokens, const int64_t* d_offsets, const int64_t* d_blk_off, uint32_t n_req, uint32_t block_size,
+int arc_hash_blocks_device(const int32_t* d_tokens, const arc_hash_item* d_items, uint32_t n_items, int64_t tok_lo, int64_t tok_hi, uint32_t block_size,
                            uint64_t* d_keys_out, uint32_t* d_ticket, void* cuda_stream) {
-  if (n_req > kMaxReq) return fail(nullptr, ARC_ERR_INVALID_ARG, "n_req > 2^20");
+  if (n_items > kMaxReq) return fail(nullptr, ARC_ERR_INVALID_ARG, "n_items > 2^20");
   if (block_size != 16) return fail(nullptr, ARC_ERR_UNSUPPORTED, "block_size %u: only 16 is built", block_size);
-  if (!n_req) return ARC_OK;
-  if (!d_tokens || !d_offsets || !d_blk_off || !d_keys_out || !d_ticket) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
+  if (!n_items) return ARC_OK;
+  if (!d_tokens || !d_items || !d_keys_out || !d_ticket) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
+  static_assert(sizeof(arc_hash_item) == sizeof(HashItem), "arc_hash_item is the kernel's HashItem");
   cudaError_t e = k1_configure();
   if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "K1 configuration: %s", cudaGetErrorString(e));
-  static const K1HostArgs no_args = {};
-  launch_hash_blocks(false, K1_ARG_NONE, no_args, d_tokens, const_cast<int64_t*>(d_offsets), const_cast<int64_t*>(d_blk_off), n_req,
-                     (unsigned long long*)d_keys_out, d_ticket, (cudaStream_t)cuda_stream, nullptr, nullptr);
+  hash_items_kernel<<<grid_for(n_items, K1_WARPS, 148 * 3), 256, K1_SMEM_BYTES, (cudaStream_t)cuda_stream>>>(
+      d_tokens, reinterpret_cast<const HashItem*>(d_items), n_items, tok_lo, tok_hi, (unsigned long long*)d_keys_out, d_ticket);
   g_hash_launches += 1;
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "hash launch: %s", cudaGetErrorString(e));

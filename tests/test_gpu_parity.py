@@ -115,8 +115,9 @@ def test_hash_on_two_streams_and_from_device_offsets(arc):
         for t, o, want, blk_off in jobs[:8]:
             if len(want) == 0:
                 continue
+            items = arc.hash_items(o)
             out = torch.empty(len(want), dtype=torch.int64, device="cuda")
-            arc.hash_blocks_device(t, torch.from_numpy(o).cuda(), torch.from_numpy(blk_off).cuda(), len(o) - 1, out, ticket)
+            arc.hash_blocks_device(t, torch.from_numpy(items.view(np.uint8)).cuda(), len(items), int(o[0]), int(o[-1]), out, ticket)
             assert np.array_equal(out.cpu().numpy().view(np.uint64), want)
     assert int(ticket.abs().sum()) == 0
 
