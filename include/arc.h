@@ -259,6 +259,12 @@ int arc_debug_set_key_mask(arc_cache *h, uint64_t mask);
  * calls of the roll-forward routine and of its phases.  Synchronises. */
 int arc_debug_counters(arc_cache *h, uint64_t *out, uint32_t n);
 
+/* Per-access latency of the by-the-book K3 machine (arc_set_machine(h, 1)) by class, cumulative since create/reset:
+ * out[cls * 16 + b] (HOST uint32[80], cls = ARC_MISS .. ARC_GHOST_B2) counts the accesses whose serial_access took
+ * fewer than 64 SM cycles (b = 0) or [64 * 2^(b-1), 64 * 2^b) cycles (b = 1..15; clock64 on the SM).  The window machines
+ * apply accesses in batches, so a per-access latency exists only here.  Synchronises. */
+int arc_debug_latency_hist(arc_cache *h, uint32_t *out);
+
 /* Copies one list (1 = T1, 2 = T2, 3 = B1, 4 = B2) in LRU -> MRU order to HOST arrays keys_out /
  * block_ids_out (either may be NULL), at most cap entries; *n_out receives the list length.
  * Synchronises.  For tests. */

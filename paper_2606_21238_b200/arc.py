@@ -28,7 +28,7 @@ EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats"
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
            "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe", "arc_set_pin_scope",
            "arc_release", "arc_hold_units", "arc_step_resume", "arc_debug_gather_sectors", "arc_hash_blocks_device", "arc_step_host_async",
-           "arc_step_host_wait", "arc_route_requests"]
+           "arc_step_host_wait", "arc_route_requests", "arc_debug_latency_hist"]
 
 
 class ArcError(RuntimeError):
@@ -100,6 +100,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_hold_units.argtypes = [vp]
     L.arc_hold_units.restype = u64
     L.arc_debug_list.argtypes = [vp, C.c_int, vp, vp, u64, C.POINTER(u64)]
+    L.arc_debug_latency_hist.argtypes = [vp, vp]
     L.arc_debug_gather_sectors.argtypes = [vp, u64, vp, u64, vp, vp]
     if path is None:
         _lib = L
@@ -314,6 +315,12 @@ class ArcCache:
         out = np.zeros(len(self.DEBUG_COUNTERS), np.uint64)
         self._check(self._L.arc_debug_counters(self._h, out.ctypes.data, len(out)))
         return {k: int(v) for k, v in zip(self.DEBUG_COUNTERS, out)}
+
+    def debug_latency_hist(self) -> np.ndarray:
+        """[5 classes, 16 bins] per-access latency histogram of the by-the-book machine (set_machine(1)); see arc.h."""
+        out = np.zeros((5, 16), np.uint32)
+        self._check(self._L.arc_debug_latency_hist(self._h, out.ctypes.data))
+        return out
 
     def debug_probe(self, keys, nodes_out=None, stream=None):
         """K2 alone: keys = CUDA int64 tensor holding uint64 bits (>= 2); returns the CUDA int32 tensor of node indices."""

@@ -77,6 +77,9 @@ struct DevState {
   int32_t u1, u2;
   uint32_t release_bad;           // scratch of release_kernel
   uint32_t win_seq;               // K3 wide machine: number of the last window (31 bits, never 0), see node_stamp
+  // by-the-book machine only (arc_set_machine(h, 1)): per-access latency in SM cycles (clock64 around serial_access) by
+  // class, 16 logarithmic bins: bin b holds the accesses that took [64 * 2^(b-1), 64 * 2^b) cycles, bin 0 fewer than 64
+  uint32_t lat_hist[5][16];
 };
 enum : int { DBG_WIN_HIT = 0, DBG_WIN_GENERAL, DBG_WIN_SERIAL, DBG_CUT_TWIN, DBG_CUT_CONFLICT, DBG_SCAN_ROUNDS, DBG_ACC_HIT_WIN,
              DBG_ACC_GENERAL_WIN, DBG_CYC_FETCH, DBG_CYC_ROLL, DBG_CYC_SCAN, DBG_CYC_APPLY, DBG_CYC_SERIAL, DBG_CYC_TOTAL, DBG_ROLL_CALLS, DBG_ROLL_PHASES, DBG_COUNT };

@@ -1056,6 +1056,13 @@ int arc_debug_counters(arc_cache* h, uint64_t* out, uint32_t n) {
   return ARC_OK;
 }
 
+int arc_debug_latency_hist(arc_cache* h, uint32_t* out) {
+  if (!h || !out) return ARC_ERR_INVALID_ARG;
+  CUDA_TRY(h, cudaStreamSynchronize(h->last_stream));
+  CUDA_TRY(h, cudaMemcpy(out, reinterpret_cast<const char*>(h->d_state) + offsetof(DevState, lat_hist), sizeof(uint32_t) * 5 * 16, cudaMemcpyDeviceToHost));
+  return ARC_OK;
+}
+
 int arc_debug_list(arc_cache* h, int which, uint64_t* keys_out, int32_t* block_ids_out, uint64_t cap, uint64_t* n_out) {
   if (!h || which < 1 || which > 4 || !n_out) return ARC_ERR_INVALID_ARG;
   cudaStream_t s = h->last_stream;

@@ -219,7 +219,13 @@ __global__ void arc_machine_serial_kernel(const __grid_constant__ StepParams P) 
     // step-wide scope: the pins of earlier requests of the step stay; held scope: nothing enters T1 / T2's rings during a
     // step, every ring entry is a possible victim (bound = tail, set by ctx_load) and elig1/2 carry over from DevState
     if (P.pin_scope != 2 && (r == 0 || P.pin_scope == 0)) begin_request(C);
-    for (int64_t j = 0; j < nb; ++j) serial_access(C, P, o + j, o + (nb - 1 - j));   // tail block first (R2)
+    for (int64_t j = 0; j < nb; ++j) {                                               // tail block first (R2)
+      const long long t0 = clock64();
+      serial_access(C, P, o + j, o + (nb - 1 - j));
+      const unsigned long long dt = (unsigned long long)(clock64() - t0);
+      const int bin = dt < 64 ? 0 : min(15, 64 - __clzll(dt) - 6);                  // the K3 per-access latency histogram
+      P.state->lat_hist[P.cls[o + (nb - 1 - j)]][bin] += 1;
+    }
   }
   ctx_store(C, P);
 }

@@ -333,6 +333,24 @@ def test_equal_keys_inside_a_request(arc, machine, bits):
         gc.close()
 
 
+def test_latency_histogram_of_the_by_the_book_machine(arc):
+    """arc_debug_latency_hist: with machine 1 every access lands in exactly one bin of its class (counts per class equal
+    the class counters), other machines leave it untouched."""
+    tr = W.make_trace(1, seed=4, scale=0.2)
+    gc = arc.ArcCache(64)
+    gc.set_machine(1)
+    for tokens, offsets in tr.steps():
+        gc.step(dev(tokens), offsets)
+    st, h = gc.stats(), gc.debug_latency_hist()
+    assert h.sum() == st["accesses"] > 0
+    assert [int(x) for x in h.sum(axis=1)] == [st["miss"], st["hit_t1"], st["hit_t2"], st["ghost_b1"], st["ghost_b2"]]
+    gc.set_machine(3)
+    for tokens, offsets in tr.steps(max_steps=5):
+        gc.step(dev(tokens), offsets)
+    assert gc.debug_latency_hist().sum() == h.sum()
+    gc.close()
+
+
 def test_probe_alone_is_a_consistent_map(arc):
     """K2 through arc_debug_probe: equal keys get equal nodes, different keys different nodes, lookups repeat."""
     g = torch.Generator(device="cuda")

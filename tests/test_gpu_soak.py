@@ -2,10 +2,15 @@
 releases under held pins), K3 machines and request mixes drawn from a persistent prefix tree (shared prefixes between
 consecutive requests, long and short requests, empty and duplicate requests).  Every output of every step, the
 counters and the four lists.  A time budget per configuration keeps the file at about half a minute."""
+import sys
 import time
+from pathlib import Path
 
 import numpy as np
 import pytest
+
+if str(Path(__file__).resolve().parent.parent) not in sys.path:      # also runnable as a script (the long soak, see main)
+    sys.path.insert(0, str(Path(__file__).resolve().parent.parent))
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -97,3 +102,47 @@ def run(A, seed, budget_s):
 def test_soak_random_configuration(A, seed):
     c, policy, scope, machine, steps, accesses, cuts, serial, twins = run(A, 2000 + seed, 2.5)
     assert steps > 5 and accesses > 0
+
+
+def main(argv=None):
+    """A long soak with a record: python tests/test_gpu_soak.py --minutes 8 --seed0 5000 --out gpurun_out/soak.log
+    One line per configuration (seed, cache size, policy, pin scope, K3 machine, steps, accesses, conflict cuts, by-the-book
+    accesses, twin cuts); any difference from the oracle raises.  The logs of the round's soaks are in profiles/."""
+    import argparse
+    import sys
+    from pathlib import Path
+
+    sys.path.insert(0, str(Path(__file__).resolve().parent.parent))
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--minutes", type=float, default=5.0)
+    ap.add_argument("--seed0", type=int, default=5000)
+    ap.add_argument("--per-config-s", type=float, default=8.0)
+    ap.add_argument("--out", default=None)
+    a = ap.parse_args(argv)
+    from paper_2606_21238_b200 import arc as A_
+
+    A_.load_library()
+    log = open(a.out, "w") if a.out else None
+    t0, seed, total = time.time(), a.seed0, 0
+    head = "# seed c policy pin_scope machine steps accesses conflict_cuts by_the_book twin_cuts"
+    print(head)
+    if log:
+        log.write(head + "\n")
+    while time.time() - t0 < 60 * a.minutes:
+        r = run(A_, seed, a.per_config_s)
+        total += r[5]
+        line = f"{seed} " + " ".join(str(x) for x in r)
+        print(line, flush=True)
+        if log:
+            log.write(line + "\n")
+            log.flush()
+        seed += 1
+    tail = f"# {seed - a.seed0} configurations, {total} accesses, {time.time() - t0:.0f} s, no difference from the oracle"
+    print(tail)
+    if log:
+        log.write(tail + "\n")
+        log.close()
+
+
+if __name__ == "__main__":
+    main()
