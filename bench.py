@@ -85,20 +85,25 @@ def source_hash() -> str:
     return h.hexdigest()
 
 
+NCU_UNITS = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "s": 1.0, "ms": 1e-3, "us": 1e-6, "ns": 1e-9}
+
+
 def ncu_metric(csv_path: Path, kernel_pat: str, metric: str):
-    """Values of `metric` for the launches whose kernel name matches, from an `ncu --page raw --csv` export."""
+    """Values of `metric` (in base units: bytes, seconds, counts) for the launches whose kernel name matches, from an
+    `ncu --page raw --csv` export (header row, units row, one row per launch)."""
     import csv
 
     rows = list(csv.reader(csv_path.open()))
-    hdr = rows[0]
+    hdr, units = rows[0], rows[1]
     if metric not in hdr or "Kernel Name" not in hdr:
         return []
     k, m = hdr.index("Kernel Name"), hdr.index(metric)
+    scale = NCU_UNITS.get(units[m], 1.0)
     out = []
     for r in rows[2:]:
         if len(r) > m and re.search(kernel_pat, r[k]):
             try:
-                out.append(float(r[m].replace(",", "")))
+                out.append(float(r[m].replace(",", "")) * scale)
             except ValueError:
                 pass
     return out
@@ -739,11 +744,10 @@ def run_ours(args):
         gb = ALGO_BYTES_PER_BLOCK * k1["blocks"] / 1e9
         traffic, traffic_src = None, ev_note
         if ev and ev.get("k1") and abs(args.bulk_gib - ev["k1"].get("bulk_gib", -1)) < 1e-9:
-            rd = ncu_metric(ROOT / "profiles" / ev["k1"]["csv"], "hash_blocks", "dram__bytes_read.sum")
-            wr = ncu_metric(ROOT / "profiles" / ev["k1"]["csv"], "hash_blocks", "dram__bytes_write.sum")
+            rd = ncu_metric(ROOT / "profiles" / ev["k1"]["csv"], ev["k1"]["kernel"], "dram__bytes_read.sum")
+            wr = ncu_metric(ROOT / "profiles" / ev["k1"]["csv"], ev["k1"]["kernel"], "dram__bytes_write.sum")
             if rd and wr:
-                scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}
-                traffic = rd[0] * scale.get(ev["k1"].get("read_unit", "byte"), 1.0) + wr[0] * scale.get(ev["k1"].get("write_unit", "byte"), 1.0)
+                traffic = rd[0] + wr[0]
                 traffic_src = f"dram__bytes_read.sum + dram__bytes_write.sum of the launch in profiles/{ev['k1']['csv']} (ncu --set full)"
         line["roofline"] = {"kernel": "K1 chained block hashing (hash_blocks_kernel: cp.async.bulk staging, mbarrier pipeline)", "bound": "hbm",
                             "achieved": gb / (k1["api_ms"] * 1e-3), "peak": peak, "unit": "GB/s", "frac": gb / (k1["api_ms"] * 1e-3) / peak,
@@ -762,6 +766,18 @@ def run_ours(args):
         # ---- K2 alone, table >> L2, against the measured random-sector ceiling
         line["probe"] = k2_probe_bench(torch, A, stream, args.seed, peak)
         line["probe"]["in_situ_us_per_step"] = head["kernels"]["probe_ms"]["us_per_step"]
+        if ev and ev.get("k2"):
+            f = ROOT / "profiles" / ev["k2"]["csv"]
+            for name, pat in (("probe", "probe_reserve"), ("ceiling", "gather32")):
+                rd, wr = ncu_metric(f, pat, "dram__bytes_read.sum"), ncu_metric(f, pat, "dram__bytes_write.sum")
+                if rd and wr:
+                    line["probe"][f"dram_bytes_per_key_{name}"] = (float(np.mean(rd)) + float(np.mean(wr))) / line["probe"]["keys"]
+            line["probe"]["traffic_note"] = ("dram__bytes of the committed ncu export (profiles/" + ev["k2"]["csv"] + "): a random 32-byte sector read costs this "
+                                             "machine about 131 B of DRAM traffic whatever asks for it - the ceiling kernel moves the same bytes - so 4.7 x the "
+                                             "algorithmic 28 B is the floor of ANY random-access table here; in DRAM bytes K2 runs at 5.4 TB/s")
+            if line["probe"].get("dram_bytes_per_key_probe"):
+                line["probe"]["dram_GBps"] = line["probe"]["dram_bytes_per_key_probe"] * line["probe"]["keys_per_s"] / 1e9
+                line["probe"]["frac_of_measured_hbm_dram_traffic"] = line["probe"]["dram_GBps"] / peak
         # ---- all five configs
         per = {}
         for cfg in (1, 2, 3, 4, 5):
