@@ -27,7 +27,8 @@ struct FusedShared {
   unsigned long long seg_end[FUSED_MAX_ITEMS];                    // local end state of every segment
 };
 
-// machine: 2 = one warp, 3 = wide
+// machine: 2 = one warp, 3 = wide.  LRU / HOLD as in the wide machine: every variant carries only its own code.
+template <bool LRU, bool HOLD>
 __global__ void __launch_bounds__(2 * WIDE_W, 1) arc_fused_small_kernel(const __grid_constant__ StepParams P, const unsigned long long* __restrict__ chain_in,
                                                                       unsigned long long* __restrict__ chain_out, int64_t* __restrict__ offsets_g,
                                                                       int64_t* __restrict__ blk_off_g, int machine,
@@ -120,7 +121,7 @@ __global__ void __launch_bounds__(2 * WIDE_W, 1) arc_fused_small_kernel(const __
   __syncthreads();
   // ---- phase 3: K3
   if (machine == 2) { if (warp == 0) batched_machine_run(P, F.vic); }
-  else wide_machine_run(P, F.wide);
+  else wide_machine_run<LRU, HOLD>(P, F.wide);
   __syncthreads();
   // ---- phase 4: K4
   finalize_body(P);

@@ -439,7 +439,10 @@ cudaError_t k1_configure() {
   K1_ATTR((hash_segments_kernel<0>));
   K1_ATTR((hash_segments_kernel<(int)K1_INLINE_SMALL>));
   K1_ATTR((hash_segments_kernel<(int)K1_INLINE_LARGE>));
-  K1_ATTR(arc_fused_small_kernel);
+  K1_ATTR((arc_fused_small_kernel<false, false>));
+  K1_ATTR((arc_fused_small_kernel<false, true>));
+  K1_ATTR((arc_fused_small_kernel<true, false>));
+  K1_ATTR((arc_fused_small_kernel<true, true>));
   K1_ATTR(hash_items_kernel);
 #undef K1_ATTR
   if (dev >= 0 && dev < 64) done[dev] = true;
@@ -593,8 +596,14 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
     StepParams P = make_params(h);
     P.tokens = d_tokens; P.n_req = n_req; P.n_access = (uint32_t)N;
     if (h->profiling) { cudaEventRecord(h->ev[2], s); cudaEventRecord(h->ev[3], s); }   // one kernel: its whole time is booked under the machine
-    arc_fused_small_kernel<<<1, 2 * WIDE_W, K1_SMEM_BYTES, s>>>(P, reinterpret_cast<const unsigned long long*>(d_chain_in), h->d_chain_state, h->d_offsets,
-                                                             h->d_offsets + (h->req_cap + 1), (N < 48ull * n_req) ? 2 : 3, k1_args.small);
+    const unsigned long long* ci = reinterpret_cast<const unsigned long long*>(d_chain_in);
+    int64_t* d_boff = h->d_offsets + (h->req_cap + 1);
+    const int mach = (N < 48ull * n_req) ? 2 : 3;
+    const bool lru = h->policy == ARC_POLICY_LRU, held = h->pin_scope == ARC_PIN_HELD;
+#define FUSED_LAUNCH(L, H) arc_fused_small_kernel<L, H><<<1, 2 * WIDE_W, K1_SMEM_BYTES, s>>>(P, ci, h->d_chain_state, h->d_offsets, d_boff, mach, k1_args.small)
+    if (lru) { if (held) FUSED_LAUNCH(true, true); else FUSED_LAUNCH(true, false); }
+    else { if (held) FUSED_LAUNCH(false, true); else FUSED_LAUNCH(false, false); }
+#undef FUSED_LAUNCH
     h->launches += 1;
     if (h->profiling) { cudaEventRecord(h->ev[4], s); cudaEventRecord(h->ev[5], s); h->ev_valid = true; }
     CUDA_TRY(h, cudaGetLastError());

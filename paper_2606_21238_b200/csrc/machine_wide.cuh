@@ -72,7 +72,8 @@ struct WideDecisions {
 };
 
 // The recurrence over the first k accesses of the window, chunk by chunk (every warp computes the same thing).
-__device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, int32_t c, bool lru, const WideShared& S, int k,
+template <bool lru>
+__device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, int32_t c, const WideShared& S, int k,
                                           int warp, int lane) {
   D.R = roll_init(C);
   D.my_p = C.p;
@@ -149,6 +150,14 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
   }
 }
 
+// The same recurrence out of line: after a conflict cut the window is rolled again over fewer accesses.  That happens once
+// in about eighty windows; a second inlined copy would double the largest routine of a kernel whose instruction fetch
+// nothing hides.
+template <bool lru>
+__device__ __noinline__ void wide_roll_again(WideDecisions& D, const SerialCtx& C, int32_t c, const WideShared& S, int k, int warp, int lane) {
+  wide_roll<lru>(D, C, c, S, k, warp, lane);
+}
+
 // One scan round of a scanner warp: 128 ring entries from q0 (a multiple of 4), 4 per lane; live entries are appended
 // to vic[] in LRU order.  Returns the number of live entries found in the round.
 struct ScanRegs { uint4 e0, e1; };
@@ -183,6 +192,7 @@ __device__ __forceinline__ uint32_t wide_scan_round(const ScanRegs& regs, uint32
 // Scanner warp for list L (warps 4..7 of the CTA): follows the owners' barrier sequence window by window.  The first
 // 128 entries from the list head are scanned while the owners fetch node records and roll the counters forward; more
 // rounds follow only if the window turns out to need more victims than that.
+template <bool LRU>
 __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S, uint32_t L, int lane) {
   const uint32_t lt = (1u << lane) - 1u;
   const RingEnt* ring = P.ring[L];
@@ -203,7 +213,7 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
     for (int u = 0; u < WIDE_WARPS; ++u) {
       const uint32_t km = bits_from(0, min(32, max(0, want - 32 * u)));
       const uint32_t m0 = S.m[0][u], m1 = S.m[1][u], m2 = S.m[2][u];
-      const uint32_t hit = (P.policy == POLICY_LRU) ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);
+      const uint32_t hit = LRU ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);
       all_hit = all_hit && ((hit & km) == km);
     }
     if (all_hit) continue;                             // the owners apply an all-hit window without any further barrier
@@ -242,14 +252,18 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
 
 // The machine itself, run by the first 2 * WIDE_W threads of a CTA (all of them must call it; it ends with every thread
 // past the last barrier).  S: the CTA's WideShared.  Also the third phase of the one-launch small-step kernel.
+// The policy (LRU or the two-list ARC / DBL) and the held pin scope are template parameters: the kernel is one CTA whose
+// instruction fetch nothing hides (ncu: one fetch stall per issued instruction, 20 % instruction-cache misses), so every
+// variant carries only its own code.
+template <bool LRU, bool HOLD>
 __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared& S) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
   uint32_t lm[WIDE_WARPS], me[WIDE_WARPS];   // see wide_rank / wide_has
 #pragma unroll
   for (int u = 0; u < WIDE_WARPS; ++u) { lm[u] = (u < warp) ? FULL : ((u == warp) ? lt : 0u); me[u] = (u == warp) ? (1u << lane) : 0u; }
-  const bool lru = (P.policy == POLICY_LRU);
-  const bool hold = (P.pin_scope == 2);      // held scope: see machine_batched.cuh
+  constexpr bool lru = LRU;
+  constexpr bool hold = HOLD;                // held scope: see machine_batched.cuh
   const int32_t c = P.capacity;
   const int64_t N = (int64_t)P.n_access;
   if (P.state->error == DEV_ERR_NODE_POOL) return;       // K2 could not give every key a node: the step is void (sticky error; CTA-uniform)
@@ -260,7 +274,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
   for (int i = 0; i < DBG_COUNT; ++i) dbg[i] = 0;
   const long long t_begin = clock64();
   if (warp >= WIDE_WARPS) {                                 // warps 4..7 scan the LRU ends of T1, T2, B1, B2
-    wide_scanner(P, S, (uint32_t)(warp - WIDE_WARPS) + 1u, lane);
+    wide_scanner<LRU>(P, S, (uint32_t)(warp - WIDE_WARPS) + 1u, lane);
     return;
   }
 
@@ -437,7 +451,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
 
       // ---- general window: roll the counters forward (every warp, identically), scan the lists (one warp each)
       WideDecisions D;
-      wide_roll(D, C, c, lru, S, k, warp, lane);
+      wide_roll<LRU>(D, C, c, S, k, warp, lane);
       const long long tw2 = clock64();
       dbg[DBG_CYC_ROLL] += (unsigned long long)(tw2 - tw1);
       uint32_t S2[WIDE_WARPS];                                     // evictions from T2
@@ -513,7 +527,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
           KM[u] = bits_from(0, min(32, max(0, k - 32 * u)));
           HIT[u] &= KM[u];
         }
-        wide_roll(D, C, c, lru, S, k, warp, lane);
+        wide_roll<LRU>(D, C, c, S, k, warp, lane);
 #pragma unroll
         for (int u = 0; u < WIDE_WARPS; ++u) S2[u] = D.s1[u] & ~D.s0[u];
         need[L_T1] = wide_count(D.s0); need[L_T2] = wide_count(S2); need[L_B1] = wide_count(D.d1); need[L_B2] = wide_count(D.d2);
@@ -633,11 +647,16 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
   }
 }
 
+template <bool LRU, bool HOLD>
 __global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __grid_constant__ StepParams P) {
   __shared__ WideShared S;
-  wide_machine_run(P, S);
+  wide_machine_run<LRU, HOLD>(P, S);
 }
 
-inline void launch_machine_wide(const StepParams& P, cudaStream_t s) { arc_machine_wide_kernel<<<1, 2 * WIDE_W, 0, s>>>(P); }
+inline void launch_machine_wide(const StepParams& P, cudaStream_t s) {
+  const bool lru = P.policy == POLICY_LRU, hold = P.pin_scope == 2;
+  if (lru) { if (hold) arc_machine_wide_kernel<true, true><<<1, 2 * WIDE_W, 0, s>>>(P); else arc_machine_wide_kernel<true, false><<<1, 2 * WIDE_W, 0, s>>>(P); }
+  else { if (hold) arc_machine_wide_kernel<false, true><<<1, 2 * WIDE_W, 0, s>>>(P); else arc_machine_wide_kernel<false, false><<<1, 2 * WIDE_W, 0, s>>>(P); }
+}
 
 }  // namespace arc
