@@ -96,10 +96,14 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
       return;
     }
   }
+  // ONE copy of the chunk body, looped over (not unrolled): the body with its inlined phases is the largest piece of code of
+  // the kernel, and four copies each run once per window are four times the instruction-cache footprint of one copy run
+  // four times.  The chunk's decision masks reach their (statically indexed, register) slots by predicated moves.
 #pragma unroll
+  for (int v = 0; v < WIDE_WARPS; ++v) D.s0[v] = D.s1[v] = D.d1[v] = D.d2[v] = D.fm[v] = 0;
+#pragma unroll 1
   for (int u = 0; u < WIDE_WARPS; ++u) {
     const int ku = min(32, max(0, k - 32 * u));
-    D.s0[u] = D.s1[u] = D.d1[u] = D.d2[u] = D.fm[u] = 0;
     if (ku > 0) {
       const uint32_t km = bits_from(0, ku);
       const uint32_t m0 = S.m[0][u] & km, m1 = S.m[1][u] & km, m2 = S.m[2][u] & km, me = S.m[3][u] & km;
@@ -144,18 +148,12 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
           i += n;
         }
       }
-      D.s0[u] = D.R.s0; D.s1[u] = D.R.s1; D.d1[u] = D.R.d1; D.d2[u] = D.R.d2; D.fm[u] = D.R.fm;
+#pragma unroll
+      for (int v = 0; v < WIDE_WARPS; ++v)
+        if (v == u) { D.s0[v] = D.R.s0; D.s1[v] = D.R.s1; D.d1[v] = D.R.d1; D.d2[v] = D.R.d2; D.fm[v] = D.R.fm; }
       if (u == warp) D.my_p = D.R.my_p;
     }
   }
-}
-
-// The same recurrence out of line: after a conflict cut the window is rolled again over fewer accesses.  That happens once
-// in about eighty windows; a second inlined copy would double the largest routine of a kernel whose instruction fetch
-// nothing hides.
-template <bool lru>
-__device__ __noinline__ void wide_roll_again(WideDecisions& D, const SerialCtx& C, int32_t c, const WideShared& S, int k, int warp, int lane) {
-  wide_roll<lru>(D, C, c, S, k, warp, lane);
 }
 
 // One scan round of a scanner warp: 128 ring entries from q0 (a multiple of 4), 4 per lane; live entries are appended
