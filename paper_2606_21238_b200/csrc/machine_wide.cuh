@@ -267,10 +267,10 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
   if (P.state->error == DEV_ERR_NODE_POOL) return;       // K2 could not give every key a node: the step is void (sticky error; CTA-uniform)
   SerialCtx C;            // identical in every thread
   ctx_load(C, P);
-  unsigned long long dbg[DBG_COUNT];
+  uint32_t dbg[DBG_COUNT];                    // per-step sums fit 32 bits (a step is a few 10^7 cycles); clock() is the low word of the SM clock
 #pragma unroll
   for (int i = 0; i < DBG_COUNT; ++i) dbg[i] = 0;
-  const long long t_begin = clock64();
+  const uint32_t t_begin = (uint32_t)clock();
   if (warp >= WIDE_WARPS) {                                 // warps 4..7 scan the LRU ends of T1, T2, B1, B2
     wide_scanner<LRU>(P, S, (uint32_t)(warp - WIDE_WARPS) + 1u, lane);
     return;
@@ -335,7 +335,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
       }
       cp_async_wait_all();                                           // ids requested in earlier windows have landed
       __syncthreads();                                               // (S0) the previous window's writes are visible; the scanners start
-      const long long tw0 = clock64();
+      const uint32_t tw0 = (uint32_t)clock();
       const uint32_t n = act0 ? S.ids[(uint32_t)(a0 + tid) & (WIDE_IDS - 1)] : NODE_NONE;
       Node rec;
       rec.list = L_FREE; rec.pos = 0; rec.block = -1; rec.slot = 0;
@@ -406,8 +406,8 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
         badnode |= M2[u] & M0[u] & KM[u];
       }
       if (badnode) C.err = DEV_ERR_BAD_NODE;                         // a FREE node reached K3
-      const long long tw1 = clock64();
-      dbg[DBG_CYC_FETCH] += (unsigned long long)(tw1 - tw0);
+      const uint32_t tw1 = (uint32_t)clock();
+      dbg[DBG_CYC_FETCH] += tw1 - tw0;
 
       if (all_hit) {
         // ---- every access of the window is a hit: no counter other than t1/t2 moves, nothing is evicted
@@ -443,15 +443,15 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
         if (lane == 0) S.bad[warp] = 0;
         j += k;
         dbg[DBG_WIN_HIT]++; dbg[DBG_ACC_HIT_WIN] += (unsigned)k;
-        dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw1);
+        dbg[DBG_CYC_APPLY] += (uint32_t)clock() - tw1;
         continue;
       }
 
       // ---- general window: roll the counters forward (every warp, identically), scan the lists (one warp each)
       WideDecisions D;
       wide_roll<LRU>(D, C, c, S, k, warp, lane);
-      const long long tw2 = clock64();
-      dbg[DBG_CYC_ROLL] += (unsigned long long)(tw2 - tw1);
+      const uint32_t tw2 = (uint32_t)clock();
+      dbg[DBG_CYC_ROLL] += tw2 - tw1;
       uint32_t S2[WIDE_WARPS];                                     // evictions from T2
 #pragma unroll
       for (int u = 0; u < WIDE_WARPS; ++u) S2[u] = D.s1[u] & ~D.s0[u];
@@ -499,8 +499,8 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
 #pragma unroll
         for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.bad[u]) first_bad = 32 * u + __ffs(S.bad[u]) - 1;
       }
-      const long long tw3 = clock64();
-      dbg[DBG_CYC_SCAN] += (unsigned long long)(tw3 - tw2);
+      const uint32_t tw3 = (uint32_t)clock();
+      dbg[DBG_CYC_SCAN] += tw3 - tw2;
       if (first_bad >= 0) {
         k = first_bad;
         dbg[DBG_CUT_CONFLICT]++;
@@ -517,7 +517,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
           j += 1;
           spec_ok = false;                             // the by-the-book access may have changed any node
           dbg[DBG_WIN_SERIAL]++;
-          dbg[DBG_CYC_SERIAL] += (unsigned long long)(clock64() - tw3);
+          dbg[DBG_CYC_SERIAL] += (uint32_t)clock() - tw3;
           continue;
         }
 #pragma unroll
@@ -619,7 +619,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
       C.elig1 = D.R.e1; C.elig2 = D.R.e2;
       j += k;
       dbg[DBG_WIN_GENERAL]++; dbg[DBG_ACC_GENERAL_WIN] += (unsigned)k;
-      dbg[DBG_CYC_APPLY] += (unsigned long long)(clock64() - tw3);
+      dbg[DBG_CYC_APPLY] += (uint32_t)clock() - tw3;
     }
   }
 #pragma unroll
@@ -636,7 +636,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
       C.stat[ST_GHOST_B1] += S.red[w][3]; C.stat[ST_GHOST_B2] += S.red[w][4];
     }
   }
-  dbg[DBG_CYC_TOTAL] = (unsigned long long)(clock64() - t_begin);
+  dbg[DBG_CYC_TOTAL] = (uint32_t)clock() - t_begin;
   if (tid == 0) {
     P.state->win_seq = win_seq;
     ctx_store(C, P);
