@@ -144,21 +144,28 @@ def _stream_ptr(stream) -> int:
 
 class StepResult:
     """Device-resident outputs of one arc_step (torch tensors viewing library-owned memory; valid until the
-    next step on the same cache)."""
+    next step on the same cache).  The views are made when they are first asked for: a caller that reads only
+    `block_id` pays for one view, not for nine."""
+
+    _FIELDS = {"prefix_len": ("prefix_len", "req", "<i4", "int32"), "blk_off": ("blk_off", "req1", "<i8", "int64"),
+               "cls": ("cls", "n", "|u1", "uint8"), "block_id": ("block_id", "n", "<i4", "int32"),
+               "evicted_id": ("evicted_id", "n", "<i4", "int32"), "p_after": ("p_after", "n", "<i4", "int32"),
+               "counts": ("counts", "two", "<i4", "int32"), "chain_state": ("chain_state", "req", "<i8", "int64")}   # chain_state: uint64 bit patterns
 
     def __init__(self, raw: _StepResult, n_req: int):
-        torch = _torch()
-        n = int(raw.n_access)
-        self.n_access = n
-        self.prefix_len = _view(raw.prefix_len, n_req, "<i4", torch.int32)
-        self.blk_off = _view(raw.blk_off, n_req + 1, "<i8", torch.int64)
-        self.cls = _view(raw.cls, n, "|u1", torch.uint8)
-        self.block_id = _view(raw.block_id, n, "<i4", torch.int32)
-        self.evicted_id = _view(raw.evicted_id, n, "<i4", torch.int32)
-        self.p_after = _view(raw.p_after, n, "<i4", torch.int32)
-        self.counts = _view(raw.counts, 2, "<i4", torch.int32)
-        self.chain_state = _view(raw.chain_state, n_req, "<i8", torch.int64)   # uint64 bit patterns
+        self.n_access = int(raw.n_access)
+        self._raw, self._n_req = raw, n_req
         self._alloc_ptr, self._evict_ptr = raw.alloc_ids, raw.evict_ids
+
+    def __getattr__(self, name):
+        f = StepResult._FIELDS.get(name)
+        if f is None:
+            raise AttributeError(name)
+        torch = _torch()
+        n = {"req": self._n_req, "req1": self._n_req + 1, "n": self.n_access, "two": 2}[f[1]]
+        v = _view(getattr(self._raw, f[0]), n, f[2], getattr(torch, f[3]))
+        setattr(self, name, v)
+        return v
 
     def to_host(self) -> dict:
         """Synchronising copy of everything to numpy (for tests)."""
