@@ -136,10 +136,12 @@ int arc_step_resume(arc_cache *h, const int32_t *d_tokens, const int64_t *h_offs
  *   - the copy of h_tokens (HOST int32; pinned memory makes the copy asynchronous) to a library-owned device buffer, on
  *     the handle's own copy stream, so that it overlaps the steps still computing on cuda_stream,
  *   - the step itself on cuda_stream (which waits for that copy),
- *   - a kernel that writes the results straight into pinned, device-mapped host memory: n_alloc | n_evict |
- *     prefix_len[n_req] | alloc_ids[n_alloc] | evict_ids[n_evict], exactly 4 (2 + n_req + n_alloc + n_evict) bytes,
+ *   - a kernel that writes the results straight into pinned, device-mapped host memory: n_alloc | n_evict | device error
+ *     | prefix_len[n_req] | alloc_ids[n_alloc] | evict_ids[n_evict], exactly 4 (3 + n_req + n_alloc + n_evict) bytes,
  * and returns a ticket (never 0).  arc_step_host_wait(ticket) blocks until that step is done and fills `out` with
- * pointers into the pinned buffer, valid until the third arc_step_host_async after this step's.  Up to three steps may be
+ * pointers into the pinned buffer, valid until the third arc_step_host_async after this step's; it returns ARC_ERR_CUDA
+ * (with `out` filled) when the handle carries a sticky device-side error (e.g. a bad arc_release), which therefore
+ * reaches a caller that never asks for arc_stats.  Up to three steps may be
  * in flight; a fourth arc_step_host_async before the oldest was waited for fails with ARC_ERR_INVALID_ARG and changes
  * nothing.  h_tokens must stay valid and unchanged until its step has been waited for; h_offsets is copied before return.
  * A step that needs larger buffers than the handle has (see arc_reserve) is accepted only with no step in flight.

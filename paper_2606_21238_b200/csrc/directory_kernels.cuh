@@ -254,19 +254,20 @@ __device__ __forceinline__ void finalize_body(const StepParams& P) {
 __global__ void __launch_bounds__(256) finalize_kernel(const __grid_constant__ StepParams P) { finalize_body(P); }
 
 // The host entry's results, written by the device straight into pinned, mapped HOST memory (arc_step_host_async): exactly
-// the words that exist - n_alloc | n_evict | prefix_len[n_req] | alloc_ids[n_alloc] | evict_ids[n_evict] - so no copy has
-// to be sized from an upper bound and nothing crosses the bus twice.
+// the words that exist - n_alloc | n_evict | device error | prefix_len[n_req] | alloc_ids[n_alloc] | evict_ids[n_evict] - so no
+// copy has to be sized from an upper bound and nothing crosses the bus twice.  The sticky device error (DEV_ERR_*: node
+// pool, bad release, ...) travels with every result, so a scheduler that never calls arc_stats still learns of it.
 __global__ void __launch_bounds__(256) pack_results_kernel(const DevState* __restrict__ st, const int32_t* __restrict__ prefix_len,
                                                            const int32_t* __restrict__ alloc_ids, const int32_t* __restrict__ evict_ids,
                                                            uint32_t n_req, int32_t* __restrict__ out) {
   const uint32_t n_alloc = st->counts[0], n_evict = st->counts[1];
-  const uint32_t total = 2u + n_req + n_alloc + n_evict;
+  const uint32_t total = 3u + n_req + n_alloc + n_evict;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
     int32_t v;
-    if (i < 2u) v = (int32_t)(i == 0 ? n_alloc : n_evict);
-    else if (i < 2u + n_req) v = prefix_len[i - 2u];
-    else if (i < 2u + n_req + n_alloc) v = alloc_ids[i - 2u - n_req];
-    else v = evict_ids[i - 2u - n_req - n_alloc];
+    if (i < 3u) v = (int32_t)(i == 0 ? n_alloc : (i == 1 ? n_evict : st->error));
+    else if (i < 3u + n_req) v = prefix_len[i - 3u];
+    else if (i < 3u + n_req + n_alloc) v = alloc_ids[i - 3u - n_req];
+    else v = evict_ids[i - 3u - n_req - n_alloc];
     out[i] = v;
   }
 }

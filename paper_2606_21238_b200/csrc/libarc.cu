@@ -103,7 +103,7 @@ struct arc_cache {
   // handle's own copy stream) and a pinned, device-mapped host buffer that K4's pack kernel writes the results into.
   int32_t* d_tok[kHostSlots] = {};
   uint64_t tok_cap[kHostSlots] = {};
-  int32_t* h_out[kHostSlots] = {};        // pinned + mapped: n_alloc | n_evict | prefix_len[n_req] | alloc_ids[n_alloc] | evict_ids[n_evict]
+  int32_t* h_out[kHostSlots] = {};        // pinned + mapped: n_alloc | n_evict | error | prefix_len[n_req] | alloc_ids[n_alloc] | evict_ids[n_evict]
   cudaEvent_t ev_h2d[kHostSlots] = {}, ev_comp[kHostSlots] = {};
   uint32_t slot_ticket[kHostSlots] = {};  // 0 = free
   uint32_t slot_n_req[kHostSlots] = {};
@@ -736,10 +736,11 @@ int arc_step_host_wait(arc_cache* h, uint32_t ticket, arc_host_result* out) {
   const uint32_t n_req = h->slot_n_req[k];
   out->n_access = h->slot_n_access[k];
   out->n_alloc = (uint32_t)hp[0]; out->n_evict = (uint32_t)hp[1];
-  out->prefix_len = hp + 2; out->alloc_ids = hp + 2 + n_req; out->evict_ids = hp + 2 + n_req + out->n_alloc;
+  out->prefix_len = hp + 3; out->alloc_ids = hp + 3 + n_req; out->evict_ids = hp + 3 + n_req + out->n_alloc;
   out->h2d_bytes = h->slot_h2d[k];
-  out->d2h_bytes = (2ull + n_req + out->n_alloc + out->n_evict) * sizeof(int32_t);
+  out->d2h_bytes = (3ull + n_req + out->n_alloc + out->n_evict) * sizeof(int32_t);
   h->slot_ticket[k] = 0;
+  if (hp[2]) return fail(h, ARC_ERR_CUDA, "device-side directory error %u (1 node pool, 2 no victim, 3 ring overflow, 4 bad node, 5 bad release)", (unsigned)hp[2]);
   return ARC_OK;
 }
 

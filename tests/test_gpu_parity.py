@@ -271,7 +271,7 @@ def test_host_entry_pipelined(arc):
             r, o = gc.step_host_wait(tk), want.pop(tk)
             for k in ("prefix_len", "alloc_ids", "evict_ids"):
                 assert np.array_equal(r[k], o[k]), (step, k)
-            assert r["d2h_bytes"] == 4 * (2 + len(o["prefix_len"]) + len(o["alloc_ids"]) + len(o["evict_ids"]))
+            assert r["d2h_bytes"] == 4 * (3 + len(o["prefix_len"]) + len(o["alloc_ids"]) + len(o["evict_ids"]))
     for tk in inflight:
         r, o = gc.step_host_wait(tk), want.pop(tk)
         assert np.array_equal(r["alloc_ids"], o["alloc_ids"])
@@ -597,6 +597,8 @@ def test_held_pins_protect_blocks_and_bad_release_is_flagged(arc):
     gc.release(bad)
     with pytest.raises(arc.ArcError):
         gc.stats()
+    with pytest.raises(arc.ArcError):                                 # the host entry reports the sticky error too (no arc_stats needed)
+        gc.step_host(np.zeros(0, np.int32), np.zeros(1, np.int64))
     gl, ol = gc.debug_lists(), oc.lists()
     for n in ("T1", "T2", "B1", "B2"):
         assert np.array_equal(gl[n][0], ol[n][0]), n                   # nothing changed
