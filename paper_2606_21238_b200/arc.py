@@ -316,7 +316,8 @@ class ArcCache:
         self._check(self._L.arc_set_machine(self._h, which))
 
     DEBUG_COUNTERS = ["win_hit", "win_general", "win_serial", "cut_twin", "cut_conflict", "scan_rounds", "acc_hit_win",
-                      "acc_general_win", "cyc_fetch", "cyc_roll", "cyc_scan", "cyc_apply", "cyc_serial", "cyc_total", "roll_calls", "roll_phases"]
+                      "acc_general_win", "cyc_fetch", "cyc_roll", "cyc_scan", "cyc_apply", "cyc_serial", "cyc_total", "roll_calls", "roll_phases",
+                      "prov_ok", "prov_miss"]
 
     def debug_counters(self) -> dict:
         out = np.zeros(len(self.DEBUG_COUNTERS), np.uint64)

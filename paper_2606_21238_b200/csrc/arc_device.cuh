@@ -82,7 +82,19 @@ struct DevState {
   uint32_t lat_hist[5][16];
 };
 enum : int { DBG_WIN_HIT = 0, DBG_WIN_GENERAL, DBG_WIN_SERIAL, DBG_CUT_TWIN, DBG_CUT_CONFLICT, DBG_SCAN_ROUNDS, DBG_ACC_HIT_WIN,
-             DBG_ACC_GENERAL_WIN, DBG_CYC_FETCH, DBG_CYC_ROLL, DBG_CYC_SCAN, DBG_CYC_APPLY, DBG_CYC_SERIAL, DBG_CYC_TOTAL, DBG_ROLL_CALLS, DBG_ROLL_PHASES, DBG_COUNT };
+             DBG_ACC_GENERAL_WIN, DBG_CYC_FETCH, DBG_CYC_ROLL, DBG_CYC_SCAN, DBG_CYC_APPLY, DBG_CYC_SERIAL, DBG_CYC_TOTAL, DBG_ROLL_CALLS, DBG_ROLL_PHASES,
+             DBG_PROV_OK, DBG_PROV_MISS,   // pipelined wide machine: windows whose roll-ahead stood / had to be rolled on request
+#ifdef ARC_PROBES
+             DBG_PROBE0, DBG_PROBE_END = DBG_PROBE0 + 13,   // ad-hoc cycle probes of a diagnostic build (-DARC_PROBES), see PROBE()
+#endif
+             DBG_COUNT };
+#ifdef ARC_PROBES
+#define PROBE(i) do { const uint32_t t_ = (uint32_t)clock(); dbg[DBG_PROBE0 + (i)] += t_ - tp_; tp_ = t_; } while (0)
+#define PROBE_RESET() do { tp_ = (uint32_t)clock(); } while (0)
+#else
+#define PROBE(i) do { } while (0)
+#define PROBE_RESET() do { } while (0)
+#endif
 
 // Everything a step's kernels need, passed by value.
 struct StepParams {

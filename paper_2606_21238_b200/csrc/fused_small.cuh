@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(2 * WIDE_W, 1) arc_fused_small_kernel(const __
   __syncthreads();
   // ---- phase 3: K3
   if (machine == 2) { if (warp == 0) batched_machine_run(P, F.vic); }
-  else wide_machine_run<LRU, HOLD>(P, F.wide);
+  else wide_machine_run<LRU, HOLD, false>(P, F.wide);
   __syncthreads();
   // ---- phase 4: K4
   finalize_body(P);

@@ -63,7 +63,7 @@ struct arc_cache {
   int policy = 0;
   unsigned long long key_and = ~0ull;   // test hook
   int pin_scope = ARC_PIN_REQUEST;
-  int machine = 0;            // 0 auto (wide, or one-warp when requests are short), 1 serial, 2 one-warp, 3 wide
+  int machine = 0;            // 0 auto (wide, or one-warp when requests are short), 1 serial, 2 one-warp, 3 wide with the roller warp, 4 one launch, 5 wide without it
   // capacities
   uint64_t n_cap = 0;         // max full blocks per step the buffers are sized for
   uint32_t req_cap = 0;
@@ -657,8 +657,10 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
     // one warp, 32-wide windows: a window of the wide machine costs about twice as much, which only pays when requests
     // are long enough to fill it (windows never cross a request boundary)
     launch_machine_batched(P, s);
+  } else if (h->machine == 5) {
+    launch_machine_wide<false>(P, s);                                                                    // K3 (8 warps, 128-wide windows; every owner warp rolls)
   } else {
-    launch_machine_wide(P, s);                                                                           // K3 (four warps, 128-wide windows)
+    launch_machine_wide<true>(P, s);                                                                     // K3 (the same with the roller warp a window ahead)
   }
   if (h->profiling) cudaEventRecord(h->ev[4], s);
   finalize_kernel<<<grid_for(std::max<uint64_t>(N, (uint64_t)n_req * 32), 256, 148 * 8), 256, 0, s>>>(P);  // K4
@@ -967,7 +969,7 @@ int arc_last_kernel_times(arc_cache* h, arc_kernel_times* out) {
 uint64_t arc_launch_count(const arc_cache* h) { return h ? h->launches : g_hash_launches.load(); }
 
 int arc_set_machine(arc_cache* h, int which) {
-  if (!h || which < 0 || which > 4) return ARC_ERR_INVALID_ARG;
+  if (!h || which < 0 || which > 5) return ARC_ERR_INVALID_ARG;
   h->machine = which;
   return ARC_OK;
 }

@@ -27,8 +27,49 @@ __device__ __forceinline__ void cp_async_u32(uint32_t* smem_dst, const uint32_t*
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
+// Named barriers of the pipelined form (PIPE): the owners and scanners meet on barrier 1 (256 threads) where the plain form
+// uses __syncthreads; the roller warps are handed their work on barrier 2 and hand it back on barrier 3 (128 owners +
+// 128 roller threads: one side arrives, the other waits).
+__device__ __forceinline__ void bar_sync_n(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_arrive_n(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+constexpr int BAR_CTA = 1, BAR_REQ = 2, BAR_DONE = 3;
+constexpr int ROLL_PARTIES = 2 * 32 * WIDE_WARPS;          // the owners and as many roller threads
+template <bool PIPE>
+__device__ __forceinline__ void cta_sync() {
+  if (PIPE) bar_sync_n(BAR_CTA, 2 * WIDE_W); else __syncthreads();
+}
+template <bool PIPE>
+__device__ __forceinline__ bool cta_or(bool pred) {
+  if (!PIPE) return __syncthreads_or(pred) != 0;
+  uint32_t r;
+  asm volatile("{\n\t.reg .pred p, q;\n\tsetp.ne.u32 q, %1, 0;\n\tbar.red.or.pred p, 1, 256, q;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(r) : "r"((uint32_t)pred) : "memory");
+  return r != 0;
+}
+static_assert(2 * WIDE_W == 256, "the reducing barrier above spells the thread count out");
+
+// What the owners hand the roller warp (one request outstanding at a time) and what comes back (two buffers, by the
+// request's parity: the scanners and owners of a window read one while the next request's result goes into the other).
+struct RollReq {
+  uint32_t m[4][WIDE_WARPS];                 // class masks m0, m1, m2, me per chunk
+  int32_t st[8];                             // t1, t2, b1, b2, p, next_fresh, elig1, elig2 before the window
+  int32_t k;
+  uint32_t quit;
+};
+struct RollRes {
+  uint4 plan[WIDE_W];                        // what each access does, as ranks inside the window (WidePlan, packed)
+  int32_t st[8];                             // the same eight after the window
+  uint32_t need[5];                          // victims / drops the window takes per list
+  uint32_t pt1, g1, nh, ev;                  // pushes to T1 and to B1, allocations, evictions of the window
+  uint32_t err, phases;
+};
+
 struct WideShared {
   uint32_t m[4][WIDE_WARPS];                 // m0, m1, m2, me per chunk
+  uint32_t reload[WIDE_WARPS];               // PIPE: owners that could not use their speculative record
+  uint32_t ctl_prov, ctl_par;                // PIPE: a result rolled ahead for this window exists, and its buffer
+  RollReq req;
+  RollRes res[2];
   uint32_t bad[WIDE_WARPS];
   uint32_t twin[WIDE_WARPS], twinc[WIDE_WARPS];   // accesses that repeat an earlier node of the window; threads whose stamp exchange says "maybe"
   uint32_t twin_k;                           // the window's size after a twin cut (written between the two twin barriers only)
@@ -72,18 +113,19 @@ struct WideDecisions {
 };
 
 // The recurrence over the first k accesses of the window, chunk by chunk (every warp computes the same thing).
+// Sm: the class masks m0, m1, m2, me per chunk (shared memory); warp = the chunk this thread's access is in.
 template <bool lru>
-__device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, int32_t c, const WideShared& S, int k,
+__device__ __forceinline__ void wide_roll(WideDecisions& D, const Roll& R0, int32_t c, const uint32_t (*Sm)[WIDE_WARPS], int k,
                                           int warp, int lane) {
-  D.R = roll_init(C);
-  D.my_p = C.p;
+  D.R = R0;
+  D.my_p = R0.p;
   {
     // The commonest whole window of a cache in steady state: every access a miss, case 4A (t1 + b1 = c) with T1 above its
     // target and enough evictable entries for all of them: each miss drops B1's LRU ghost and evicts T1's LRU entry, no
     // counter moves (phase_miss's first case, for the window instead of chunk by chunk).
     uint32_t any = 0;
 #pragma unroll
-    for (int u = 0; u < WIDE_WARPS; ++u) any |= (S.m[0][u] | S.m[1][u] | S.m[2][u]) & bits_from(0, min(32, max(0, k - 32 * u)));
+    for (int u = 0; u < WIDE_WARPS; ++u) any |= (Sm[0][u] | Sm[1][u] | Sm[2][u]) & bits_from(0, min(32, max(0, k - 32 * u)));
     Roll& R = D.R;
     if (!lru && any == 0 && R.t1 + R.t2 == c && R.t1 + R.b1 == c && R.t1 < c && R.t1 > R.p && R.e1 >= k) {
 #pragma unroll
@@ -106,7 +148,7 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
     const int ku = min(32, max(0, k - 32 * u));
     if (ku > 0) {
       const uint32_t km = bits_from(0, ku);
-      const uint32_t m0 = S.m[0][u] & km, m1 = S.m[1][u] & km, m2 = S.m[2][u] & km, me = S.m[3][u] & km;
+      const uint32_t m0 = Sm[0][u] & km, m1 = Sm[1][u] & km, m2 = Sm[2][u] & km, me = Sm[3][u] & km;
       Roll& R = D.R;
       const uint32_t hits = lru ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2);
       const uint32_t absent = ~(m0 | m1 | m2) & km, gb1 = m0 & m1 & ~m2, gb2 = m2 & ~m0 & ~m1;
@@ -156,6 +198,64 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const SerialCtx& C, 
   }
 }
 
+// What one access of a general window does, as ranks inside the window: everything the decision masks say about it.
+struct WidePlan {
+  uint32_t src;                              // eviction source: 0 none, 1 T1 -> B1, 2 T2 -> B2, 3 T1 without a ghost
+  bool d1, d2, fm;                           // drops the LRU ghost of B1 / B2; takes a fresh block id
+  uint32_t vic_rank;                         // its victim is the vic_rank-th live entry from the LRU end of T1 (src 1, 3) / T2 (src 2)
+  uint32_t gpush_rank;                       // ... and becomes the gpush_rank-th ghost the window appends to B1 (src 1) / B2 (src 2)
+  uint32_t drop_rank, fresh_rank;            // the ghost it drops; the fresh id it takes
+  uint32_t push_rank;                        // its own node is the push_rank-th the window appends to T1 (ABSENT; LRU: all) / T2
+  uint32_t alloc_rank, evict_rank;           // positions in the step's alloc_ids / evict_ids, counted from the window's first
+  int32_t p;                                 // p after the access
+};
+struct WideCounts { uint32_t need[5]; uint32_t pt1, g1, nh, ev; };
+
+__device__ __forceinline__ uint4 plan_pack(const WidePlan& A) {
+  return make_uint4(A.src | ((uint32_t)A.d1 << 2) | ((uint32_t)A.d2 << 3) | ((uint32_t)A.fm << 4) | (A.vic_rank << 8) | (A.gpush_rank << 16) | (A.drop_rank << 24),
+                    A.push_rank | (A.alloc_rank << 8) | (A.evict_rank << 16) | (A.fresh_rank << 24), (uint32_t)A.p, 0u);
+}
+__device__ __forceinline__ WidePlan plan_unpack(const uint4 v) {
+  WidePlan A;
+  A.src = v.x & 3u; A.d1 = (v.x >> 2) & 1u; A.d2 = (v.x >> 3) & 1u; A.fm = (v.x >> 4) & 1u;
+  A.vic_rank = (v.x >> 8) & 0xFFu; A.gpush_rank = (v.x >> 16) & 0xFFu; A.drop_rank = v.x >> 24;
+  A.push_rank = v.y & 0xFFu; A.alloc_rank = (v.y >> 8) & 0xFFu; A.evict_rank = (v.y >> 16) & 0xFFu; A.fresh_rank = v.y >> 24;
+  A.p = (int32_t)v.z;
+  return A;
+}
+
+// The plan of this thread's access and the window's counts from the decisions of a roll over k accesses.  Sm: the class
+// masks the roll used; lm / me: the thread's rank masks (wide_rank / wide_has).
+template <bool lru>
+__device__ __forceinline__ void wide_make_plan(WidePlan& A, WideCounts& N, const WideDecisions& D, const uint32_t (*Sm)[WIDE_WARPS], int k,
+                                               const uint32_t (&lm)[WIDE_WARPS], const uint32_t (&me)[WIDE_WARPS]) {
+  uint32_t S2[WIDE_WARPS], G1[WIDE_WARPS], PT1[WIDE_WARPS], PT2[WIDE_WARPS], NH[WIDE_WARPS], EV[WIDE_WARPS];
+#pragma unroll
+  for (int u = 0; u < WIDE_WARPS; ++u) {
+    const uint32_t km = bits_from(0, min(32, max(0, k - 32 * u)));
+    const uint32_t m0 = Sm[0][u], m1 = Sm[1][u], m2 = Sm[2][u];
+    const uint32_t hit = (lru ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2)) & km;
+    S2[u] = D.s1[u] & ~D.s0[u];                                        // evictions from T2 = pushes to B2
+    G1[u] = D.s0[u] & ~D.s1[u];                                        // pushes to B1, in access order
+    PT1[u] = lru ? km : (~(m0 | m1 | m2) & km);                        // ABSENT nodes enter T1 (LRU: everything)
+    PT2[u] = km & ~PT1[u];
+    NH[u] = km & ~hit;
+    EV[u] = D.s0[u] | D.s1[u];
+  }
+  A.src = (uint32_t)wide_has(D.s0, me) | ((uint32_t)wide_has(D.s1, me) << 1);
+  A.d1 = wide_has(D.d1, me); A.d2 = wide_has(D.d2, me); A.fm = wide_has(D.fm, me);
+  A.vic_rank = (A.src == 2) ? wide_rank(S2, lm) : wide_rank(D.s0, lm);
+  A.gpush_rank = (A.src == 1) ? wide_rank(G1, lm) : wide_rank(S2, lm);
+  A.drop_rank = A.d1 ? wide_rank(D.d1, lm) : wide_rank(D.d2, lm);
+  A.fresh_rank = wide_rank(D.fm, lm);
+  A.push_rank = wide_has(PT1, me) ? wide_rank(PT1, lm) : wide_rank(PT2, lm);
+  A.alloc_rank = wide_rank(NH, lm);
+  A.evict_rank = wide_rank(EV, lm);
+  A.p = D.my_p;
+  N.need[0] = 0; N.need[L_T1] = wide_count(D.s0); N.need[L_T2] = wide_count(S2); N.need[L_B1] = wide_count(D.d1); N.need[L_B2] = wide_count(D.d2);
+  N.pt1 = wide_count(PT1); N.g1 = wide_count(G1); N.nh = wide_count(NH); N.ev = wide_count(EV);
+}
+
 // One scan round of a scanner warp: 128 ring entries from q0 (a multiple of 4), 4 per lane; live entries are appended
 // to vic[] in LRU order.  Returns the number of live entries found in the round.
 struct ScanRegs { uint4 e0, e1; };
@@ -190,20 +290,20 @@ __device__ __forceinline__ uint32_t wide_scan_round(const ScanRegs& regs, uint32
 // Scanner warp for list L (warps 4..7 of the CTA): follows the owners' barrier sequence window by window.  The first
 // 128 entries from the list head are scanned while the owners fetch node records and roll the counters forward; more
 // rounds follow only if the window turns out to need more victims than that.
-template <bool LRU>
+template <bool LRU, bool PIPE>
 __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S, uint32_t L, int lane) {
   const uint32_t lt = (1u << lane) - 1u;
   const RingEnt* ring = P.ring[L];
   unsigned long long rounds = 0;
   for (;;) {
-    __syncthreads();                                   // (S0) the window's control block is published
+    cta_sync<PIPE>();                                  // (S0) the window's control block is published
     if (S.ctl_done) break;
     const uint32_t head = S.ctl_head[L], limit = S.ctl_limit[L];
     uint32_t q0 = head & ~3u, found = 0;
     int want = (int)S.ctl_k;
     ScanRegs cur = wide_scan_load(ring, P.ring_mask, q0, lane);   // in flight while the owners fetch; used after B1
-    __syncthreads();                                   // (B1) the scanners never hold this barrier up
-    if (S.twinc[0] | S.twinc[1] | S.twinc[2] | S.twinc[3]) { __syncthreads(); __syncthreads(); want = (int)S.twin_k; }
+    cta_sync<PIPE>();                                  // (B1) the scanners never hold this barrier up
+    if (S.twinc[0] | S.twinc[1] | S.twinc[2] | S.twinc[3]) { cta_sync<PIPE>(); cta_sync<PIPE>(); want = (int)S.twin_k; }
     // while the owners roll (not in an all-hit window, which needs no victim): up to 3 rounds, until as many live entries
     // are known as the window has accesses, so that the owners rarely wait for a scan after the roll
     bool all_hit = true;
@@ -215,14 +315,26 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
       all_hit = all_hit && ((hit & km) == km);
     }
     if (all_hit) continue;                             // the owners apply an all-hit window without any further barrier
-    for (int it = 0; !all_hit && it < 4 && (int)found < want && (int32_t)(limit - q0) > 0; ++it) {
-      const ScanRegs nxt = wide_scan_load(ring, P.ring_mask, q0 + (uint32_t)WIDE_W, lane);
-      found += wide_scan_round(cur, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
-      cur = nxt;
+    // PIPE: the window's decisions were rolled ahead and stand (the owners judge that the same way): what the window takes
+    // from this list is known now, and the owners are waiting for nothing else
+    const bool known = PIPE && S.ctl_prov && !(S.reload[0] | S.reload[1] | S.reload[2] | S.reload[3]) && want == (int)S.ctl_k;
+    if (known) {
+      const uint32_t need = S.res[S.ctl_par & 1u].need[L];
+      while (found < need && (int32_t)(limit - q0) > 0) {
+        const ScanRegs nxt = wide_scan_load(ring, P.ring_mask, q0 + (uint32_t)WIDE_W, lane);
+        found += wide_scan_round(cur, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
+        cur = nxt;
+      }
+    } else {
+      for (int it = 0; it < 4 && (int)found < want && (int32_t)(limit - q0) > 0; ++it) {
+        const ScanRegs nxt = wide_scan_load(ring, P.ring_mask, q0 + (uint32_t)WIDE_W, lane);
+        found += wide_scan_round(cur, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
+        cur = nxt;
+      }
     }
     __syncwarp();
     if (lane == 0) { S.found[L] = found; S.more[L] = (int32_t)(limit - q0) > 0; }
-    __syncthreads();                                   // (B2) the owners have published what the window needs, the scanners what they have
+    cta_sync<PIPE>();                                  // (B2) the owners have published what the window needs, the scanners what they have
     bool extra = false;                                // some list must be scanned further: CTA-uniform, computed by everybody
 #pragma unroll
     for (int X = 1; X <= 4; ++X) extra = extra || (S.found[X] < S.need[X] && S.more[X]);
@@ -232,20 +344,65 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
         cur = wide_scan_load(ring, P.ring_mask, q0, lane);
         found += wide_scan_round(cur, q0, head, limit, found, S.vic[L], lane, lt); q0 += (uint32_t)WIDE_W; ++rounds;
       }
-      __syncthreads();                                 // (B2x) everybody has read the first report
+      cta_sync<PIPE>();                                // (B2x) everybody has read the first report
       __syncwarp();
       if (lane == 0) S.found[L] = found;
-      __syncthreads();                                 // (B2') victims of all four lists are in shared memory
+      cta_sync<PIPE>();                                // (B2') victims of all four lists are in shared memory
     }
-    if (__syncthreads_or(0)) {                         // (B3) some access cannot be applied with the window
-      __syncthreads();                                 // (B3x) the owners' reports are in shared memory
+    if (cta_or<PIPE>(false)) {                         // (B3) some access cannot be applied with the window
+      cta_sync<PIPE>();                                // (B3x) the owners' reports are in shared memory
       bool serial = false;
 #pragma unroll
       for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.bad[u]) serial = (32 * u + __ffs(S.bad[u]) - 1) == 0;
-      if (serial) __syncthreads();                     // the by-the-book access of warp 0
+      if (serial) cta_sync<PIPE>();                    // the by-the-book access of warp 0
     }
   }
   if (lane == 0 && rounds) atomicAdd(&P.state->dbg[DBG_SCAN_ROUNDS], rounds);
+}
+
+// PIPE: the roller warps (warps 8..11).  The counter recurrence is the one strictly serial piece of a window and depends on
+// nothing but the class masks and eight counters, so it runs here, a window AHEAD of the owners: while they check and
+// apply window w, these warps roll window w + 1 from the masks of its speculative records and the counters after w, and
+// turn the decisions into one plan per access (WidePlan: what the access evicts, drops and pushes, as ranks) plus the
+// window's counts, so that the owners' part of a window is loads, checks and stores only.  The owners take the result if
+// every speculative record stood and w was applied whole; otherwise they ask again with what they then know.  The four
+// warps roll redundantly, like the owner warps of the plain form (no decision is ever broadcast); thread g plans access
+// g.  They keep no state of their own: every request carries the counters it starts from.
+template <bool LRU>
+__device__ __forceinline__ void wide_roller(const StepParams& P, WideShared& S, int g) {
+  const int lane = g & 31, w = g >> 5;
+  const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
+  uint32_t lm[WIDE_WARPS], me[WIDE_WARPS];
+#pragma unroll
+  for (int u = 0; u < WIDE_WARPS; ++u) { lm[u] = (u < w) ? FULL : ((u == w) ? lt : 0u); me[u] = (u == w) ? (1u << lane) : 0u; }
+  const int32_t c = P.capacity;
+  const bool dbl = (P.policy == POLICY_DBL);
+  for (uint32_t i = 0;; ++i) {
+    bar_sync_n(BAR_REQ, ROLL_PARTIES);                 // a request is in S.req
+    if (S.req.quit) break;
+    Roll R0;
+    R0.t1 = S.req.st[0]; R0.t2 = S.req.st[1]; R0.b1 = S.req.st[2]; R0.b2 = S.req.st[3]; R0.p = S.req.st[4]; R0.nf = S.req.st[5];
+    R0.e1 = S.req.st[6]; R0.e2 = S.req.st[7];
+    R0.s0 = R0.s1 = R0.d1 = R0.d2 = R0.fm = 0; R0.my_p = R0.p; R0.err = 0; R0.calls = 0; R0.phases = 0; R0.dbl = dbl;
+    const int k = S.req.k;
+    RollRes& Q = S.res[i & 1u];
+    WideDecisions D;
+    wide_roll<LRU>(D, R0, c, S.req.m, k, w, lane);
+    WidePlan A;
+    WideCounts N;
+    wide_make_plan<LRU>(A, N, D, S.req.m, k, lm, me);
+    Q.plan[g] = plan_pack(A);
+    if (g == 0) {
+      Q.st[0] = D.R.t1; Q.st[1] = D.R.t2; Q.st[2] = D.R.b1; Q.st[3] = D.R.b2; Q.st[4] = D.R.p; Q.st[5] = D.R.nf; Q.st[6] = D.R.e1; Q.st[7] = D.R.e2;
+#pragma unroll
+      for (int L = 0; L <= 4; ++L) Q.need[L] = N.need[L];
+      Q.pt1 = N.pt1; Q.g1 = N.g1; Q.nh = N.nh; Q.ev = N.ev;
+      Q.err = D.R.err; Q.phases = D.R.phases;
+    }
+    __threadfence_block();
+    __syncwarp();
+    bar_arrive_n(BAR_DONE, ROLL_PARTIES);              // the result is in S.res[i & 1]
+  }
 }
 
 // The machine itself, run by the first 2 * WIDE_W threads of a CTA (all of them must call it; it ends with every thread
@@ -253,7 +410,7 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
 // The policy (LRU or the two-list ARC / DBL) and the held pin scope are template parameters: the kernel is one CTA whose
 // instruction fetch nothing hides (ncu: one fetch stall per issued instruction, 20 % instruction-cache misses), so every
 // variant carries only its own code.
-template <bool LRU, bool HOLD>
+template <bool LRU, bool HOLD, bool PIPE>
 __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared& S) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
@@ -265,14 +422,18 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
   const int32_t c = P.capacity;
   const int64_t N = (int64_t)P.n_access;
   if (P.state->error == DEV_ERR_NODE_POOL) return;       // K2 could not give every key a node: the step is void (sticky error; CTA-uniform)
+  if (PIPE && warp >= 2 * WIDE_WARPS) { wide_roller<LRU>(P, S, tid - 2 * WIDE_W); return; }   // warps 8..11 roll the counters a window ahead
   SerialCtx C;            // identical in every thread
   ctx_load(C, P);
   uint32_t dbg[DBG_COUNT];                    // per-step sums fit 32 bits (a step is a few 10^7 cycles); clock() is the low word of the SM clock
 #pragma unroll
   for (int i = 0; i < DBG_COUNT; ++i) dbg[i] = 0;
   const uint32_t t_begin = (uint32_t)clock();
+#ifdef ARC_PROBES
+  uint32_t tp_ = t_begin;
+#endif
   if (warp >= WIDE_WARPS) {                                 // warps 4..7 scan the LRU ends of T1, T2, B1, B2
-    wide_scanner<LRU>(P, S, (uint32_t)(warp - WIDE_WARPS) + 1u, lane);
+    wide_scanner<LRU, PIPE>(P, S, (uint32_t)(warp - WIDE_WARPS) + 1u, lane);
     return;
   }
 
@@ -307,11 +468,29 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
   uint32_t spec_mark = 0;                                  // what node_stamp of the speculated node held before this thread's exchange
   uint32_t my_cls[5] = {0, 0, 0, 0, 0};                  // accesses of general windows this thread applied, by class
 
-  int64_t my_off = 0, my_off1 = 0;
+  // PIPE: the roller warp's mailbox.  At most one request is outstanding; request number i answers into S.res[i & 1].
+  uint32_t req_no = 0;
+  bool have_prov = false;                                  // a request for the NEXT window (rolled ahead) is outstanding
+  uint32_t prov_par = 0;                                   // ... and the buffer its result goes to
+  // every owner thread calls these (warp-uniform control flow); tid 0 has written the request's scalars
+  auto roll_send = [&]() -> uint32_t {
+    __threadfence_block();
+    bar_arrive_n(BAR_REQ, ROLL_PARTIES);
+    return (req_no++) & 1u;
+  };
+  auto roll_wait = [&]() { bar_sync_n(BAR_DONE, ROLL_PARTIES); };
+  auto roll_state = [&](int32_t t1, int32_t t2, int32_t b1, int32_t b2, int32_t p, int32_t nf, int32_t e1, int32_t e2, int kk) {
+    if (tid == 0) {
+      S.req.st[0] = t1; S.req.st[1] = t2; S.req.st[2] = b1; S.req.st[3] = b2; S.req.st[4] = p; S.req.st[5] = nf; S.req.st[6] = e1; S.req.st[7] = e2;
+      S.req.k = kk; S.req.quit = 0;
+    }
+  };
+
+  int64_t my_off = 0, my_off1 = 0, my_off2 = 0;
   for (uint32_t r = 0; r < P.n_req; ++r) {
     if ((r & 31u) == 0) {      // block offsets of the next 32 requests, one per lane (every warp keeps its own copy)
       const uint32_t rr = min(r + (uint32_t)lane, P.n_req - 1);
-      my_off = P.blk_off[rr]; my_off1 = P.blk_off[rr + 1];
+      my_off = P.blk_off[rr]; my_off1 = P.blk_off[rr + 1]; my_off2 = P.blk_off[min(rr + 2, P.n_req)];
     }
     const int64_t o = __shfl_sync(FULL, my_off, r & 31), nb = __shfl_sync(FULL, my_off1, r & 31) - o;
     if (!hold && (r == 0 || P.pin_scope == 0)) begin_request(C);   // step-wide scope: the pins of earlier requests of the step stay
@@ -321,20 +500,24 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
       int k = kmax;
       const int64_t a0 = o + j;
       const bool act0 = tid < k;
-      // size of the window after this one if this one is not cut (an upper bound where it is not known cheaply)
+      // size of the window after this one if this one is not cut (an upper bound where the next request is empty)
       int next_k = WIDE_W;
-      if (j + kmax < nb) next_k = (int)min((int64_t)WIDE_W, nb - j - kmax);
-      else if (((r + 1u) & 31u) != 0u && r + 1u < P.n_req) {
-        const int64_t nb1 = __shfl_sync(FULL, my_off1, (r + 1) & 31) - __shfl_sync(FULL, my_off, (r + 1) & 31);
-        if (nb1 > 0) next_k = (int)min((int64_t)WIDE_W, nb1);
+      bool next_exact = false, next_new_req = false;       // the size is exact; that window is the first of a request
+      if (j + kmax < nb) { next_k = (int)min((int64_t)WIDE_W, nb - j - kmax); next_exact = true; }
+      else if (r + 1u < P.n_req) {
+        const int64_t nb1 = __shfl_sync(FULL, my_off2, r & 31) - __shfl_sync(FULL, my_off1, r & 31);
+        if (nb1 > 0) { next_k = (int)min((int64_t)WIDE_W, nb1); next_exact = true; next_new_req = true; }
       }
       if (tid == 0) {
         S.ctl_done = 0; S.ctl_k = (uint32_t)kmax;
+        if (PIPE) { S.ctl_prov = have_prov ? 1u : 0u; S.ctl_par = prov_par; }
 #pragma unroll
         for (int L = 1; L <= 4; ++L) { S.ctl_head[L] = C.head[L]; S.ctl_limit[L] = (L <= 2) ? C.bound[L] : C.tail[L]; }
       }
       cp_async_wait_all();                                           // ids requested in earlier windows have landed
-      __syncthreads();                                               // (S0) the previous window's writes are visible; the scanners start
+      PROBE(0);                                                      // window top: loop, control block, ids landed
+      cta_sync<PIPE>();                                              // (S0) the previous window's writes are visible; the scanners start
+      PROBE(1);                                                      // S0 wait
       const uint32_t tw0 = (uint32_t)clock();
       const uint32_t n = act0 ? S.ids[(uint32_t)(a0 + tid) & (WIDE_IDS - 1)] : NODE_NONE;
       Node rec;
@@ -344,6 +527,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
       win_seq = wide_next_seq(win_seq);
       if (!aligned) win_seq = wide_next_seq(win_seq);                // a number no exchange has used yet
       bool twin_c = false;                                           // the stamp says another thread of this window may own the same node
+      bool reloaded = act0;                                          // this owner could not use a speculative record
       if (act0) {
         if (aligned) {
           // The exchange returned the stamp's last value only.  This window's number there means another exchange for
@@ -351,7 +535,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
           // upper bound) and took away what the stamp said before: the record cannot be trusted either.
           twin_c = (spec_mark == win_seq);
           if (spec_mark == prev_seq || twin_c) spec_ok = false;      // the previous window accessed the speculated node too
-          if (spec_ok) rec = spec; else rec = ld_node(P.nodes + n);
+          if (spec_ok) { rec = spec; reloaded = false; } else rec = ld_node(P.nodes + n);
         } else {
           const uint32_t old = atomicExch(P.node_stamp + n, win_seq);   // seen by the exchanges after B1
           rec = ld_node(P.nodes + n);
@@ -360,7 +544,24 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
       }
       // the id this thread will own if the next window starts where this one is due to end
       const uint32_t pre_n = (a0 + kmax + tid < N) ? S.ids[(uint32_t)(a0 + kmax + tid) & (WIDE_IDS - 1)] : NODE_NONE;
+      // The next window's record, speculatively, and its stamp (see above).  An aligned window's own stamps were written a
+      // window ago, so nothing of this window touches node_stamp before its first barrier and the exchange can go out right
+      // here, a whole fetch phase earlier: the round trip is then over when the next window starts even after an all-hit
+      // window.  (A window that stamps its nodes itself, above, sends it after the barrier instead.)
+      auto issue_spec = [&]() {
+        spec_ok = false;
+        spec_base = a0 + kmax;
+        if (pre_n != NODE_NONE && tid < next_k) {                      // next_k >= the next window's size: every owner of it is covered
+          spec = ld_node(P.nodes + pre_n);
+          spec_mark = atomicExch(P.node_stamp + pre_n, wide_next_seq(win_seq));   // looked at when the next window starts, not now
+          spec_ok = true;
+        }
+      };
+      PROBE(2);                                                      // ids, record (speculative or loaded)
+      if (aligned) issue_spec();
+      PROBE(12);
       ids_request(a0 + kmax + 2 * WIDE_W);
+      PROBE(13);
       const uint32_t lst = rec.list & NODE_LIST_MASK;
       const bool held = (rec.list & NODE_HELD) != 0;                 // held scope: in no ring, rec.pos = its holds
       {
@@ -369,31 +570,50 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
         const uint32_t be = __ballot_sync(FULL, !held && ((lst == L_T1 && (int32_t)(C.bound[L_T1] - rec.pos) > 0) ||
                                                               (lst == L_T2 && (int32_t)(C.bound[L_T2] - rec.pos) > 0)));
         const uint32_t bt = __ballot_sync(FULL, twin_c);
-        if (lane == 0) { S.m[0][warp] = b0; S.m[1][warp] = b1; S.m[2][warp] = b2; S.m[3][warp] = be; S.twinc[warp] = bt; }
+        const uint32_t br = PIPE ? __ballot_sync(FULL, reloaded) : 0u;
+        if (lane == 0) { S.m[0][warp] = b0; S.m[1][warp] = b1; S.m[2][warp] = b2; S.m[3][warp] = be; S.twinc[warp] = bt; if (PIPE) S.reload[warp] = br; }
       }
-      __syncthreads();                                               // (B1) class masks and twin candidates are complete
+      // PIPE: the result rolled ahead for this window is taken out of the mailbox before the barrier, so that the scanners
+      // may read it after the barrier; whether it stands is known after the barrier (to everybody, from shared memory)
+      const bool got_prov = PIPE && have_prov;
+      const uint32_t got_par = prov_par;
+      PROBE(3);                                                      // spec issue, ids request, ballots
+      if (got_prov) { roll_wait(); have_prov = false; }
+      PROBE(4);                                                      // wait for the roller
+      cta_sync<PIPE>();                                              // (B1) class masks and twin candidates are complete
+      PROBE(5);                                                      // B1 wait
       // (1) the same node twice in the window: cut before the second occurrence
       if (S.twinc[0] | S.twinc[1] | S.twinc[2] | S.twinc[3]) {       // CTA-uniform, next to never taken
         bool later = false;                                          // an earlier access of the window has this thread's node
         if (act0) for (int i = 0; i < tid; ++i) later = later || (S.ids[(uint32_t)(a0 + i) & (WIDE_IDS - 1)] == n);
         const uint32_t tb = __ballot_sync(FULL, later);
         if (lane == 0) S.twin[warp] = tb;
-        __syncthreads();
+        cta_sync<PIPE>();
         int first = k;
 #pragma unroll
         for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.twin[u]) first = 32 * u + __ffs(S.twin[u]) - 1;
         if (first < k) { k = first; dbg[DBG_CUT_TWIN]++; }
         if (tid == 0) S.twin_k = (uint32_t)k;                        // the scanners judge "all hits" on the same accesses
-        __syncthreads();
+        cta_sync<PIPE>();
       }
-      // the next window's record, speculatively, and its stamp (see above); a node this window accesses too is not trusted
-      spec_ok = false;
-      spec_base = a0 + kmax;
-      if (pre_n != NODE_NONE && tid < next_k) {                      // next_k >= the next window's size: every owner of it is covered
-        spec = ld_node(P.nodes + pre_n);
-        spec_mark = atomicExch(P.node_stamp + pre_n, wide_next_seq(win_seq));   // looked at when the next window starts, not now
-        spec_ok = true;
-      }
+      const bool prov_valid = got_prov && !(S.reload[0] | S.reload[1] | S.reload[2] | S.reload[3]) && k == kmax;
+      // PIPE: the request for the window after this one, from the masks of its speculative records and the counters this
+      // window leaves (t1 .. e2), on the assumption that this window is applied whole.  bn1 / bn2: where the victim scans of
+      // that window stop (its request's pin bound: the tails after this window if it starts a request).
+      auto roll_ahead = [&](int32_t t1, int32_t t2, int32_t b1, int32_t b2, int32_t p, int32_t nf, int32_t e1, int32_t e2,
+                            uint32_t tail1_after, uint32_t tail2_after) {
+        const bool fresh = next_new_req && !hold && P.pin_scope == 0;   // begin_request before that window
+        const uint32_t bn1 = fresh ? tail1_after : C.bound[L_T1], bn2 = fresh ? tail2_after : C.bound[L_T2];
+        const uint32_t ls = spec_ok ? (spec.list & NODE_LIST_MASK) : 0u;
+        const bool hd = spec_ok && (spec.list & NODE_HELD) != 0;
+        const uint32_t b0 = __ballot_sync(FULL, ls & 1u), b1m = __ballot_sync(FULL, ls & 2u), b2m = __ballot_sync(FULL, ls & 4u);
+        const uint32_t be = __ballot_sync(FULL, !hd && ((ls == L_T1 && (int32_t)(bn1 - spec.pos) > 0) || (ls == L_T2 && (int32_t)(bn2 - spec.pos) > 0)));
+        if (lane == 0) { S.req.m[0][warp] = b0; S.req.m[1][warp] = b1m; S.req.m[2][warp] = b2m; S.req.m[3][warp] = be; }
+        roll_state(t1, t2, b1, b2, p, nf, fresh ? t1 : e1, fresh ? t2 : e2, next_k);
+        prov_par = roll_send();
+        have_prov = true;
+      };
+      if (!aligned) issue_spec();                                    // a node this window accesses too is not trusted (its stamp says so)
       uint32_t M0[WIDE_WARPS], M1[WIDE_WARPS], M2[WIDE_WARPS], ME[WIDE_WARPS], KM[WIDE_WARPS], HIT[WIDE_WARPS];
       bool all_hit = true;
       uint32_t badnode = 0;
@@ -408,11 +628,28 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
       if (badnode) C.err = DEV_ERR_BAD_NODE;                         // a FREE node reached K3
       const uint32_t tw1 = (uint32_t)clock();
       dbg[DBG_CYC_FETCH] += tw1 - tw0;
+      PROBE(6);                                                      // twin check, masks
 
       if (all_hit) {
         // ---- every access of the window is a hit: no counter other than t1/t2 moves, nothing is evicted
+        const uint32_t q = (lru ? C.tail[L_T1] : C.tail[L_T2]) + (uint32_t)tid;
+        uint32_t t1hits = 0, e1d = 0, e2d = 0;
+#pragma unroll
+        for (int u = 0; u < WIDE_WARPS; ++u) {
+          t1hits += (uint32_t)__popc(M0[u] & KM[u]);
+          e1d += (uint32_t)__popc(ME[u] & M0[u] & KM[u]);
+          e2d += (uint32_t)__popc(ME[u] & M1[u] & KM[u]);
+        }
+        if (lru) { C.tail[L_T1] += hold ? 0u : (uint32_t)k; C.stat[ST_HIT_T1] += (uint32_t)k; }
+        else { C.tail[L_T2] += hold ? 0u : (uint32_t)k; C.t1 -= (int32_t)t1hits; C.t2 += (int32_t)t1hits; C.stat[ST_HIT_T1] += t1hits; C.stat[ST_HIT_T2] += (uint32_t)k - t1hits; }
+        C.elig1 -= (int32_t)e1d; C.elig2 -= (int32_t)e2d;
+        C.stat[ST_ACCESSES] += (uint32_t)k;
+        if (PIPE) {                                  // the counters after the window are known: the next one goes to the roller
+          dbg[prov_valid ? DBG_PROV_OK : DBG_PROV_MISS]++;   // first, so that it rolls while this one is stored
+          if (next_exact && k == kmax && a0 + kmax < N)
+            roll_ahead(C.t1, C.t2, C.b1, C.b2, C.p, C.next_fresh, C.elig1, C.elig2, C.tail[L_T1], C.tail[L_T2]);
+        }
         if (tid < k) {
-          const uint32_t q = (lru ? C.tail[L_T1] : C.tail[L_T2]) + (uint32_t)tid;
           if (!held) ring_tomb(P, lst, rec.pos);
           if (hold) {
             st_node(P.nodes + n, (lru ? L_T1 : L_T2) | NODE_HELD, held ? rec.pos + 1u : 1u, rec.block, rec.slot);
@@ -428,82 +665,106 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
           P.p_after[out] = C.p;
           P.dropped[a0 + tid] = NODE_NONE;
         }
-        uint32_t t1hits = 0, e1d = 0, e2d = 0;
-#pragma unroll
-        for (int u = 0; u < WIDE_WARPS; ++u) {
-          t1hits += (uint32_t)__popc(M0[u] & KM[u]);
-          e1d += (uint32_t)__popc(ME[u] & M0[u] & KM[u]);
-          e2d += (uint32_t)__popc(ME[u] & M1[u] & KM[u]);
-        }
-        if (lru) { C.tail[L_T1] += hold ? 0u : (uint32_t)k; C.stat[ST_HIT_T1] += (uint32_t)k; }
-        else { C.tail[L_T2] += hold ? 0u : (uint32_t)k; C.t1 -= (int32_t)t1hits; C.t2 += (int32_t)t1hits; C.stat[ST_HIT_T1] += t1hits; C.stat[ST_HIT_T2] += (uint32_t)k - t1hits; }
-        C.elig1 -= (int32_t)e1d; C.elig2 -= (int32_t)e2d;
-        C.stat[ST_ACCESSES] += (uint32_t)k;
         if (tid < 5) S.need[tid] = 0;
         if (lane == 0) S.bad[warp] = 0;
+        PROBE(7);                                                    // all-hit window: roll ahead + stores
         j += k;
         dbg[DBG_WIN_HIT]++; dbg[DBG_ACC_HIT_WIN] += (unsigned)k;
         dbg[DBG_CYC_APPLY] += (uint32_t)clock() - tw1;
         continue;
       }
 
-      // ---- general window: roll the counters forward (every warp, identically), scan the lists (one warp each)
-      WideDecisions D;
-      wide_roll<LRU>(D, C, c, S, k, warp, lane);
+      // ---- general window: the decisions (rolled ahead by the roller warps, or here by every owner warp), scans, checks, apply
+      WidePlan A;                                                    // what this thread's access does
+      WideCounts NC;                                                 // what the window takes and appends
+      int32_t RS[8];                                                 // t1, t2, b1, b2, p, next_fresh, elig1, elig2 after the window
+      uint32_t r_err = 0, r_phases = 0;
+      // PIPE: what the roller warps worked out (ahead of time, or now on request) comes out of their result buffer
+      auto roll_take = [&](uint32_t par) {
+        const RollRes& Q = S.res[par & 1u];
+        A = plan_unpack(Q.plan[tid]);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) RS[i] = Q.st[i];
+#pragma unroll
+        for (int L = 0; L <= 4; ++L) NC.need[L] = Q.need[L];
+        NC.pt1 = Q.pt1; NC.g1 = Q.g1; NC.nh = Q.nh; NC.ev = Q.ev;
+        r_err = Q.err; r_phases = Q.phases;
+      };
+      auto roll_now = [&](int kk) {                                  // this window's first kk accesses, from the state in C
+        if (PIPE) {
+          if (tid < 4 * WIDE_WARPS) (&S.req.m[0][0])[tid] = (&S.m[0][0])[tid];
+          roll_state(C.t1, C.t2, C.b1, C.b2, C.p, C.next_fresh, C.elig1, C.elig2, kk);
+          const uint32_t par = roll_send();
+          roll_wait();
+          roll_take(par);
+        } else {                                                     // the plain form: every owner warp rolls, every thread plans
+          WideDecisions D;
+          wide_roll<LRU>(D, roll_init(C), c, S.m, kk, warp, lane);
+          wide_make_plan<LRU>(A, NC, D, S.m, kk, lm, me);
+          RS[0] = D.R.t1; RS[1] = D.R.t2; RS[2] = D.R.b1; RS[3] = D.R.b2; RS[4] = D.R.p; RS[5] = D.R.nf; RS[6] = D.R.e1; RS[7] = D.R.e2;
+          r_err = D.R.err; r_phases = D.R.phases;
+        }
+      };
+      if (PIPE) {
+        dbg[prov_valid ? DBG_PROV_OK : DBG_PROV_MISS]++;
+        if (prov_valid) roll_take(got_par); else roll_now(k);
+        if (next_exact && k == kmax && a0 + kmax < N)
+          roll_ahead(RS[0], RS[1], RS[2], RS[3], RS[4], RS[5], RS[6], RS[7],
+                     C.tail[L_T1] + (hold ? 0u : NC.pt1), C.tail[L_T2] + (hold ? 0u : (uint32_t)k - NC.pt1));
+      } else {
+        roll_now(k);
+      }
       const uint32_t tw2 = (uint32_t)clock();
       dbg[DBG_CYC_ROLL] += tw2 - tw1;
-      uint32_t S2[WIDE_WARPS];                                     // evictions from T2
-#pragma unroll
-      for (int u = 0; u < WIDE_WARPS; ++u) S2[u] = D.s1[u] & ~D.s0[u];
-      uint32_t need[5];
-      need[0] = 0; need[L_T1] = wide_count(D.s0); need[L_T2] = wide_count(S2); need[L_B1] = wide_count(D.d1); need[L_B2] = wide_count(D.d2);
-      if (tid == 0) { S.need[L_T1] = need[L_T1]; S.need[L_T2] = need[L_T2]; S.need[L_B1] = need[L_B1]; S.need[L_B2] = need[L_B2]; }
-      __syncthreads();                                               // (B2) the scanners learn what the window needs, the owners what they have
+      PROBE(8);                                                      // decisions taken, next window sent ahead
+      if (tid == 0) { S.need[L_T1] = NC.need[L_T1]; S.need[L_T2] = NC.need[L_T2]; S.need[L_B1] = NC.need[L_B1]; S.need[L_B2] = NC.need[L_B2]; }
+      cta_sync<PIPE>();                                              // (B2) the scanners learn what the window needs, the owners what they have
+      PROBE(9);                                                      // need published, B2 wait
       uint32_t found[5], endpos[5];
       bool extra = false;                                            // CTA-uniform: some list must be scanned further
 #pragma unroll
-      for (int L = 1; L <= 4; ++L) { found[L] = S.found[L]; extra = extra || (found[L] < need[L] && S.more[L]); }
+      for (int L = 1; L <= 4; ++L) { found[L] = S.found[L]; extra = extra || (found[L] < NC.need[L] && S.more[L]); }
       if (extra) {
-        __syncthreads();                                             // (B2x) everybody has read the first report
-        __syncthreads();                                             // (B2') victims of all four lists are in shared memory
+        cta_sync<PIPE>();                                            // (B2x) everybody has read the first report
+        cta_sync<PIPE>();                                            // (B2') victims of all four lists are in shared memory
 #pragma unroll
         for (int L = 1; L <= 4; ++L) found[L] = S.found[L];
       }
 #pragma unroll
       for (int L = 1; L <= 4; ++L) {
         const uint32_t limit = (L <= 2) ? C.bound[L] : C.tail[L];
-        endpos[L] = need[L] ? ((found[L] >= need[L]) ? S.vic[L][need[L] - 1].w + 1u : limit) : C.head[L];
+        endpos[L] = NC.need[L] ? ((found[L] >= NC.need[L]) ? S.vic[L][NC.need[L] - 1].w + 1u : limit) : C.head[L];
       }
       // (2) an accessed node whose ring entry lies inside a consumed range, or a victim / drop that does not exist
       bool act = tid < k;
-      uint32_t my_src = (wide_has(D.s0, me)) | ((wide_has(D.s1, me)) << 1);
-      bool my_d1 = wide_has(D.d1, me), my_d2 = wide_has(D.d2, me);
       bool bad = false;
       if (act) {
 #pragma unroll
         for (int L = 1; L <= 4; ++L)
-          if (lst == (uint32_t)L && !held && need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
+          if (lst == (uint32_t)L && !held && NC.need[L] && (rec.pos - C.head[L]) < (endpos[L] - C.head[L])) bad = true;
         // a victim / drop can be missing only from a list that has fewer live entries than the window wants (uniform)
-        if (found[L_T1] < need[L_T1] || found[L_T2] < need[L_T2] || found[L_B1] < need[L_B1] || found[L_B2] < need[L_B2]) {
-          if ((my_src & 1u) && wide_rank(D.s0, lm) >= found[L_T1]) bad = true;
-          if (my_src == 2 && wide_rank(S2, lm) >= found[L_T2]) bad = true;
-          if (my_d1 && wide_rank(D.d1, lm) >= found[L_B1]) bad = true;
-          if (my_d2 && wide_rank(D.d2, lm) >= found[L_B2]) bad = true;
+        if (found[L_T1] < NC.need[L_T1] || found[L_T2] < NC.need[L_T2] || found[L_B1] < NC.need[L_B1] || found[L_B2] < NC.need[L_B2]) {
+          if ((A.src & 1u) && A.vic_rank >= found[L_T1]) bad = true;
+          if (A.src == 2 && A.vic_rank >= found[L_T2]) bad = true;
+          if (A.d1 && A.drop_rank >= found[L_B1]) bad = true;
+          if (A.d2 && A.drop_rank >= found[L_B2]) bad = true;
         }
       }
       int first_bad = -1;
-      if (__syncthreads_or(bad)) {                                   // (B3) next to always: nobody is bad, nothing to exchange
+      if (cta_or<PIPE>(bad)) {                                       // (B3) next to always: nobody is bad, nothing to exchange
         const uint32_t bb = __ballot_sync(FULL, bad);
         if (lane == 0) S.bad[warp] = bb;
-        __syncthreads();                                             // (B3x)
+        cta_sync<PIPE>();                                            // (B3x)
 #pragma unroll
         for (int u = WIDE_WARPS - 1; u >= 0; --u) if (S.bad[u]) first_bad = 32 * u + __ffs(S.bad[u]) - 1;
       }
       const uint32_t tw3 = (uint32_t)clock();
       dbg[DBG_CYC_SCAN] += tw3 - tw2;
+      PROBE(10);                                                     // checks, B3
       if (first_bad >= 0) {
         k = first_bad;
         dbg[DBG_CUT_CONFLICT]++;
+        if (PIPE && have_prov) { roll_wait(); have_prov = false; }   // the window after this one was rolled ahead for nothing
         if (k == 0) {
           // the by-the-book routine, by warp 0 alone; the new machine state reaches the other warps through shared memory
           if (warp == 0) {
@@ -512,7 +773,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
             __syncwarp();
             if (lane == 0) S.ctx = T;
           }
-          __syncthreads();
+          cta_sync<PIPE>();
           C = S.ctx;
           j += 1;
           spec_ok = false;                             // the by-the-book access may have changed any node
@@ -520,60 +781,40 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
           dbg[DBG_CYC_SERIAL] += (uint32_t)clock() - tw3;
           continue;
         }
+        roll_now(k);                                   // the decisions, plans and counts of the first k accesses alone
 #pragma unroll
-        for (int u = 0; u < WIDE_WARPS; ++u) {
-          KM[u] = bits_from(0, min(32, max(0, k - 32 * u)));
-          HIT[u] &= KM[u];
-        }
-        wide_roll<LRU>(D, C, c, S, k, warp, lane);
-#pragma unroll
-        for (int u = 0; u < WIDE_WARPS; ++u) S2[u] = D.s1[u] & ~D.s0[u];
-        need[L_T1] = wide_count(D.s0); need[L_T2] = wide_count(S2); need[L_B1] = wide_count(D.d1); need[L_B2] = wide_count(D.d2);
-#pragma unroll
-        for (int L = 1; L <= 4; ++L) endpos[L] = need[L] ? S.vic[L][need[L] - 1].w + 1u : C.head[L];
+        for (int L = 1; L <= 4; ++L) endpos[L] = NC.need[L] ? S.vic[L][NC.need[L] - 1].w + 1u : C.head[L];
         act = tid < k;
-        my_src = (wide_has(D.s0, me)) | ((wide_has(D.s1, me)) << 1);
-        my_d1 = wide_has(D.d1, me); my_d2 = wide_has(D.d2, me);
       }
-      if (D.R.err) C.err = D.R.err;
-      dbg[DBG_ROLL_CALLS] += D.R.calls; dbg[DBG_ROLL_PHASES] += D.R.phases;
+      if (r_err) C.err = r_err;
+      dbg[DBG_ROLL_PHASES] += r_phases;
 
-
-      // ---- apply (threads < k); ranks come from the decision masks of all chunks
-      uint32_t G1[WIDE_WARPS], PT1[WIDE_WARPS], PT2[WIDE_WARPS], NH[WIDE_WARPS], EV[WIDE_WARPS];
-#pragma unroll
-      for (int u = 0; u < WIDE_WARPS; ++u) {
-        G1[u] = D.s0[u] & ~D.s1[u];                                         // pushes to B1, in access order
-        PT1[u] = lru ? KM[u] : (~(M0[u] | M1[u] | M2[u]) & KM[u]);          // ABSENT nodes enter T1 (LRU: everything)
-        PT2[u] = KM[u] & ~PT1[u];
-        NH[u] = KM[u] & ~HIT[u];
-        EV[u] = D.s0[u] | D.s1[u];
-      }
+      // ---- apply (threads < k): the plan says what, the scans say which entries, C says where the lists end
       if (act) {
-        const bool is_hit = wide_has(HIT, me);
+        const bool is_hit = lru ? (lst == L_T1) : (lst == L_T1 || lst == L_T2);
+        const bool toT1 = lru || lst == L_ABSENT;                   // ABSENT nodes enter T1 (LRU: everything), the rest T2
         int32_t blk = rec.block, ev = -1;
         uint32_t dropped = NODE_NONE;
-        if (my_src) {
-          const uint4 v = (my_src == 2) ? S.vic[L_T2][wide_rank(S2, lm)] : S.vic[L_T1][wide_rank(D.s0, lm)];
+        if (A.src) {
+          const uint4 v = (A.src == 2) ? S.vic[L_T2][A.vic_rank] : S.vic[L_T1][A.vic_rank];
           blk = ev = (int32_t)v.y;
-          if (my_src == 3) {                        // leaves no ghost: the key leaves the directory in K4
+          if (A.src == 3) {                         // leaves no ghost: the key leaves the directory in K4
             st_node_keep_slot(P.nodes + v.x, L_ABSENT, 0, -1);
             dropped = v.x;
           } else {
-            const uint32_t q = (my_src == 1) ? C.tail[L_B1] + wide_rank(G1, lm) : C.tail[L_B2] + wide_rank(S2, lm);
-            __stcg(((my_src == 1) ? P.ring[L_B1] : P.ring[L_B2]) + (q & P.ring_mask), ring_ent(v.x, -1));
-            st_node_keep_slot(P.nodes + v.x, (my_src == 1) ? L_B1 : L_B2, q, -1);
+            const uint32_t q = ((A.src == 1) ? C.tail[L_B1] : C.tail[L_B2]) + A.gpush_rank;
+            __stcg(((A.src == 1) ? P.ring[L_B1] : P.ring[L_B2]) + (q & P.ring_mask), ring_ent(v.x, -1));
+            st_node_keep_slot(P.nodes + v.x, (A.src == 1) ? L_B1 : L_B2, q, -1);
           }
-        } else if (wide_has(D.fm, me)) {
-          blk = C.next_fresh + (int32_t)wide_rank(D.fm, lm);
+        } else if (A.fm) {
+          blk = C.next_fresh + (int32_t)A.fresh_rank;
         }
-        if (my_d1 || my_d2) {
-          const uint4 d = my_d1 ? S.vic[L_B1][wide_rank(D.d1, lm)] : S.vic[L_B2][wide_rank(D.d2, lm)];
+        if (A.d1 || A.d2) {
+          const uint4 d = A.d1 ? S.vic[L_B1][A.drop_rank] : S.vic[L_B2][A.drop_rank];
           st_node_keep_slot(P.nodes + d.x, L_ABSENT, 0, -1);
           dropped = d.x;
         }
-        const bool toT1 = wide_has(PT1, me);
-        const uint32_t q = toT1 ? C.tail[L_T1] + wide_rank(PT1, lm) : C.tail[L_T2] + wide_rank(PT2, lm);
+        const uint32_t q = (toT1 ? C.tail[L_T1] : C.tail[L_T2]) + A.push_rank;
         if (lst >= L_T1 && lst <= L_B2 && !held) ring_tomb(P, lst, rec.pos);     // the node leaves its old position
         if (hold) {
           st_node(P.nodes + n, (toT1 ? L_T1 : L_T2) | NODE_HELD, held ? rec.pos + 1u : 1u, blk, rec.slot);
@@ -586,10 +827,10 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
         P.cls[out] = (uint8_t)lst;                    // ABSENT -> MISS(0), T1 -> 1, T2 -> 2, B1 -> 3, B2 -> 4
         P.block_id[out] = blk;
         P.evicted_id[out] = ev;
-        P.p_after[out] = D.my_p;
+        P.p_after[out] = A.p;
         P.dropped[a0 + tid] = dropped;
-        if (!is_hit) P.alloc_ids[C.n_alloc + wide_rank(NH, lm)] = blk;
-        if (ev >= 0) P.evict_ids[C.n_evict + wide_rank(EV, lm)] = ev;
+        if (!is_hit) P.alloc_ids[C.n_alloc + A.alloc_rank] = blk;
+        if (ev >= 0) P.evict_ids[C.n_evict + A.evict_rank] = ev;
       }
       // class counts: every thread counts its own access, the warps add them up at the end of the kernel
       if (act) {
@@ -598,28 +839,29 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
       }
       // uniform state (every thread computes the same)
       C.stat[ST_ACCESSES] += (uint32_t)k;
-      C.stat[ST_EVICT_T1] += need[L_T1];
-      C.stat[ST_EVICT_T2] += need[L_T2];
-      C.stat[ST_DROP_B1] += need[L_B1];
-      C.stat[ST_DROP_B2] += need[L_B2];
-      C.stat[ST_FRESH] += (uint32_t)(D.R.nf - C.next_fresh);
-      C.n_alloc += wide_count(NH);
-      C.n_evict += wide_count(EV);
+      C.stat[ST_EVICT_T1] += NC.need[L_T1];
+      C.stat[ST_EVICT_T2] += NC.need[L_T2];
+      C.stat[ST_DROP_B1] += NC.need[L_B1];
+      C.stat[ST_DROP_B2] += NC.need[L_B2];
+      C.stat[ST_FRESH] += (uint32_t)(RS[5] - C.next_fresh);
+      C.n_alloc += NC.nh;
+      C.n_evict += NC.ev;
       if (spec_ok) {                                 // did this window take the speculated node as a victim or drop it?
 #pragma unroll
         for (int L = 1; L <= 4; ++L)
-          if (spec.list == (uint32_t)L && need[L] && (spec.pos - C.head[L]) < (endpos[L] - C.head[L])) spec_ok = false;
+          if (spec.list == (uint32_t)L && NC.need[L] && (spec.pos - C.head[L]) < (endpos[L] - C.head[L])) spec_ok = false;
       }
 #pragma unroll
       for (int L = 1; L <= 4; ++L) C.head[L] = endpos[L];
-      if (!hold) { C.tail[L_T1] += wide_count(PT1); C.tail[L_T2] += wide_count(PT2); }
-      C.tail[L_B1] += wide_count(G1);
-      C.tail[L_B2] += need[L_T2];
-      C.t1 = D.R.t1; C.t2 = D.R.t2; C.b1 = D.R.b1; C.b2 = D.R.b2; C.p = D.R.p; C.next_fresh = D.R.nf;
-      C.elig1 = D.R.e1; C.elig2 = D.R.e2;
+      if (!hold) { C.tail[L_T1] += NC.pt1; C.tail[L_T2] += (uint32_t)k - NC.pt1; }
+      C.tail[L_B1] += NC.g1;
+      C.tail[L_B2] += NC.need[L_T2];
+      C.t1 = RS[0]; C.t2 = RS[1]; C.b1 = RS[2]; C.b2 = RS[3]; C.p = RS[4]; C.next_fresh = RS[5];
+      C.elig1 = RS[6]; C.elig2 = RS[7];
       j += k;
       dbg[DBG_WIN_GENERAL]++; dbg[DBG_ACC_GENERAL_WIN] += (unsigned)k;
       dbg[DBG_CYC_APPLY] += (uint32_t)clock() - tw3;
+      PROBE(11);                                                     // apply of a general window
     }
   }
 #pragma unroll
@@ -628,7 +870,12 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
     if (lane == 0) S.red[warp][i] = t;
   }
   if (tid == 0) S.ctl_done = 1;
-  __syncthreads();                                                   // the scanners leave; the last window's writes are done
+  cta_sync<PIPE>();                                                  // the scanners leave; the last window's writes are done
+  if (PIPE) {                                                        // so does the roller warp
+    if (have_prov) roll_wait();
+    if (tid == 0) S.req.quit = 1;
+    roll_send();
+  }
   if (tid == 0) {
 #pragma unroll
     for (int w = 0; w < WIDE_WARPS; ++w) {
@@ -645,16 +892,19 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
   }
 }
 
-template <bool LRU, bool HOLD>
-__global__ void __launch_bounds__(2 * WIDE_W) arc_machine_wide_kernel(const __grid_constant__ StepParams P) {
+// PIPE: 8 warps as above plus the four roller warps (384 threads); plain: 8 warps, every owner warp rolls for itself.
+template <bool LRU, bool HOLD, bool PIPE>
+__global__ void __launch_bounds__(2 * WIDE_W + (PIPE ? WIDE_W : 0)) arc_machine_wide_kernel(const __grid_constant__ StepParams P) {
   __shared__ WideShared S;
-  wide_machine_run<LRU, HOLD>(P, S);
+  wide_machine_run<LRU, HOLD, PIPE>(P, S);
 }
 
+template <bool PIPE>
 inline void launch_machine_wide(const StepParams& P, cudaStream_t s) {
   const bool lru = P.policy == POLICY_LRU, hold = P.pin_scope == 2;
-  if (lru) { if (hold) arc_machine_wide_kernel<true, true><<<1, 2 * WIDE_W, 0, s>>>(P); else arc_machine_wide_kernel<true, false><<<1, 2 * WIDE_W, 0, s>>>(P); }
-  else { if (hold) arc_machine_wide_kernel<false, true><<<1, 2 * WIDE_W, 0, s>>>(P); else arc_machine_wide_kernel<false, false><<<1, 2 * WIDE_W, 0, s>>>(P); }
+  constexpr int T = 2 * WIDE_W + (PIPE ? WIDE_W : 0);
+  if (lru) { if (hold) arc_machine_wide_kernel<true, true, PIPE><<<1, T, 0, s>>>(P); else arc_machine_wide_kernel<true, false, PIPE><<<1, T, 0, s>>>(P); }
+  else { if (hold) arc_machine_wide_kernel<false, true, PIPE><<<1, T, 0, s>>>(P); else arc_machine_wide_kernel<false, false, PIPE><<<1, T, 0, s>>>(P); }
 }
 
 }  // namespace arc

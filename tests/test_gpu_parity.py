@@ -124,7 +124,7 @@ def test_hash_on_two_streams_and_from_device_offsets(arc):
 
 # ------------------------------------------------------------------------------- whole arc_step
 
-@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("policy", [0, 1, 2])
 def test_config1_full_trace(arc, policy, machine):
     """BASELINE.json configs[0]: c = 64, 2,000 requests, 8 per step, ARC and LRU, every output of every step."""
@@ -133,7 +133,7 @@ def test_config1_full_trace(arc, policy, machine):
     assert st["requests"] == 2000
 
 
-@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("config,scale,max_steps", [(2, 0.06, 40), (3, 0.03, 40), (4, 0.004, 8)])
 def test_larger_configs_scaled(arc, config, scale, max_steps, machine):
     tr = W.make_trace(config, seed=0, scale=scale)
@@ -151,7 +151,7 @@ def test_config2_lru_and_small_cache_pressure(arc, policy):
     run_trace(arc, steps, 600, policy, 0, ctx=f"pressure policy {policy}")
 
 
-@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("c", [1, 2, 3, 5, 8])
 def test_tiny_caches_prefix_trees(arc, c, machine):
     """Adversarial micro-traces: duplicate requests inside one step, keys dropped from a ghost list and
@@ -304,7 +304,7 @@ def test_maintenance_rebuild_and_compaction(arc):
         gc.close()
 
 
-@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("bits", [3, 6])
 def test_equal_keys_inside_a_request(arc, machine, bits):
     """The same key several times inside one request (forced with the key-mask test hook; the 64-bit hash never does
@@ -403,7 +403,7 @@ def test_probe_on_a_table_far_larger_than_l2(arc):
     assert np.array_equal(x, want)
 
 
-@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4, 5])
 def test_step_wide_pin_scope(arc, machine):
     """NEXT-3 (part): ARC_PIN_STEP.  Hand trace G's situation (an earlier request's block is still pinned when a later
     request of the same step needs a victim), the admission rule, and random steps on small caches, against the oracle."""
@@ -521,7 +521,7 @@ def _serving_loop(arc, gc, oc, rng, c, steps, ctx, table, max_req_blocks=6):
     return live, refused
 
 
-@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("machine", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("policy", [0, 1, 2])
 def test_held_pins_and_release(arc, policy, machine):
     """NEXT-3: ARC_PIN_HELD and arc_release.  A serving loop - steps add holds, finished requests give

@@ -44,7 +44,7 @@ def tree_request(rng, table, nb):
 def run(A, seed, budget_s):
     rng = np.random.default_rng(seed)
     c = int(rng.choice([40, 300, 2000, 9000]))
-    policy = int(rng.integers(0, 3)); scope = int(rng.choice([0, 0, 1, 2])); machine = int(rng.choice([0, 3, 3, 2, 4, 4]))
+    policy = int(rng.integers(0, 3)); scope = int(rng.choice([0, 0, 1, 2])); machine = int(rng.choice([0, 3, 3, 3, 2, 4, 4, 5]))
     depth = int(rng.integers(3, 40)); br = int(rng.choice([2, 3]))
     table = rng.integers(0, 1000, size=(depth, br, 16), dtype=np.int32)
     gc, oc = A.ArcCache(c, 16, policy), O.OracleCache(c, 16, policy)
