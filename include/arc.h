@@ -207,6 +207,20 @@ typedef struct { int64_t tok_off; int64_t key_off; uint32_t n_blocks; uint32_t r
 int arc_hash_blocks_device(const int32_t *d_tokens, const arc_hash_item *d_items, uint32_t n_items, int64_t tok_lo, int64_t tok_hi,
                            uint32_t block_size, uint64_t *d_keys_out, uint32_t *d_ticket, void *cuda_stream);
 
+/* arc_hash_blocks for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same keys (natural order, every chain from S0), but the call and everything it
+ * launches allocate NOTHING - no cudaMalloc / cudaFree / cudaMallocHost, no copy through a staging buffer.  The offsets
+ * travel as a 4 KB kernel argument and the kernels' scratch is a fixed 34 KB (34,816-byte) __device__ array inside the library image
+ * (every GPU that loads the library holds it until the process exits).  Limits, checked before anything is enqueued
+ * (ARC_ERR_REQUEST_TOO_LARGE with the numbers in arc_last_error(NULL)): n_req <= 253, and n_req x ceil(longest request in
+ * blocks / 128) <= 4,096 segments, no request longer than 1,024 segments (e.g. 64 requests of up to 8,192 blocks = 131,072
+ * tokens each, or 4 of 131,072 blocks).  Two launches (requests cut into 128-block segments hashed from a zero carry, then put
+ * together: H4 is affine), asynchronous on cuda_stream.  Every call on a device SHARES the one scratch array: calls whose
+ * kernels may overlap on the GPU (different streams, several host threads) race and give wrong keys - keep them on one
+ * stream or order them with events.  Nothing in the array has to be cleared: a call reads only words it has written. */
+int arc_hash_blocks_static(const int32_t *d_tokens, const int64_t *h_offsets, uint32_t n_req, uint32_t block_size,
+                           uint64_t *d_keys_out, void *cuda_stream);
+
 /* Prefix-affinity routing for N per-GPU caches behind a router: writes to
  * d_dst_out[r] (DEVICE int32[n_req]) the shard of request r = (key of its first full block >> 33) mod world, 0 for a
  * request shorter than one block - requests that share a document or conversation prefix meet in the same cache.

@@ -28,7 +28,7 @@ EXPORTS = ["arc_create", "arc_reserve", "arc_step", "arc_step_host", "arc_stats"
            "arc_last_error", "arc_hash_blocks", "arc_set_profiling", "arc_last_kernel_times", "arc_launch_count",
            "arc_set_machine", "arc_debug_list", "arc_debug_counters", "arc_debug_set_key_mask", "arc_debug_probe", "arc_set_pin_scope",
            "arc_release", "arc_hold_units", "arc_step_resume", "arc_debug_gather_sectors", "arc_hash_blocks_device", "arc_step_host_async",
-           "arc_step_host_wait", "arc_route_requests", "arc_debug_latency_hist"]
+           "arc_step_host_wait", "arc_route_requests", "arc_debug_latency_hist", "arc_hash_blocks_static"]
 
 
 class ArcError(RuntimeError):
@@ -85,6 +85,7 @@ def load_library(path: Optional[Path] = None):
     L.arc_last_error.argtypes = [vp]
     L.arc_last_error.restype = C.c_char_p
     L.arc_hash_blocks.argtypes = [vp, vp, u32, u32, vp, vp]
+    L.arc_hash_blocks_static.argtypes = [vp, vp, u32, u32, vp, vp]
     L.arc_hash_blocks_device.argtypes = [vp, vp, u32, C.c_int64, C.c_int64, u32, vp, vp, vp]
     L.arc_route_requests.argtypes = [vp, vp, u32, u32, u32, vp, vp]
     L.arc_set_profiling.argtypes = [vp, C.c_int]
@@ -349,6 +350,17 @@ class ArcCache:
             self._check(self._L.arc_debug_list(self._h, which, keys.ctypes.data, blocks.ctypes.data, cap, C.byref(n)))
             out[name] = (keys[:n.value].copy(), blocks[:n.value].copy())
         return out
+
+
+def hash_blocks_static(tokens, offsets, out, block_size: int = 16, stream=None):
+    """arc_hash_blocks_static: the same keys as hash_blocks into the caller's `out` (CUDA int64[N]); neither this wrapper
+    nor the library allocates (at most 253 requests and 4,096 128-block segments per call, see arc.h)."""
+    L = load_library()
+    o = _offsets(offsets)
+    rc = L.arc_hash_blocks_static(tokens.data_ptr(), o.ctypes.data, len(o) - 1, block_size, out.data_ptr(), _stream_ptr(stream))
+    if rc != OK:
+        raise ArcError(rc, L.arc_last_error(None).decode())
+    return out
 
 
 def hash_blocks(tokens, offsets, block_size: int = 16, out=None, stream=None):

@@ -20,6 +20,7 @@
 #include "machine_batched.cuh"
 #include "machine_serial.cuh"
 #include "machine_wide.cuh"
+#include "hash_static.cuh"
 #include "fused_small.cuh"
 
 using namespace arc;
@@ -941,6 +942,76 @@ int arc_hash_blocks_device(const int32_t* d_tokens, const arc_hash_item* d_items
   hash_items_kernel<<<grid_for(n_items, K1_WARPS, 148 * 3), 256, K1_SMEM_BYTES, (cudaStream_t)cuda_stream>>>(
       d_tokens, reinterpret_cast<const HashItem*>(d_items), n_items, tok_lo, tok_hi, (unsigned long long*)d_keys_out, d_ticket);
   g_hash_launches += 1;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "hash launch: %s", cudaGetErrorString(e));
+  return ARC_OK;
+}
+
+// ---- K1 without any allocation (arc_hash_blocks_static) -----------------------------------------------------------
+// The scratch of the segmented hashing lives in the library image: one file-scope __device__ array per GPU that loads the
+// library, held until the process exits.  In host code the array's NAME is only a stand-in for the symbol: the device
+// address comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_k1_static_scratch[sizeof(K1StaticScratch)];
+
+namespace {
+struct K1StaticSetup { std::mutex mu; K1StaticScratch* ptr[64] = {}; };
+K1StaticSetup g_k1_static;
+
+// the scratch's device address on the CURRENT device (set-up on first use: no allocation, two attribute / symbol queries)
+cudaError_t k1_static_scratch(K1StaticScratch** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_k1_static.mu);
+  if (!g_k1_static.ptr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_k1_static_scratch);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(hash_segments_static_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, K1_SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    g_k1_static.ptr[dev] = static_cast<K1StaticScratch*>(p);
+  }
+  *out = g_k1_static.ptr[dev];
+  return cudaSuccess;
+}
+}  // namespace
+
+int arc_hash_blocks_static(const int32_t* d_tokens, const int64_t* h_offsets, uint32_t n_req, uint32_t block_size, uint64_t* d_keys_out,
+                           void* cuda_stream) {
+  if (!h_offsets) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL argument");
+  if (block_size != 16) return fail(nullptr, ARC_ERR_UNSUPPORTED, "block_size %u: only 16 is built", block_size);
+  if (n_req > K1_STATIC_MAX_REQ)
+    return fail(nullptr, ARC_ERR_REQUEST_TOO_LARGE, "arc_hash_blocks_static takes at most %u requests per call (got %u)", K1_STATIC_MAX_REQ, n_req);
+  if (h_offsets[0] < 0) return fail(nullptr, ARC_ERR_INVALID_ARG, "h_offsets[0] < 0");
+  static thread_local OffsetsArgT<K1_STATIC_MAX_REQ> arg;           // offsets[n_req + 1] then blk_off[n_req + 1]
+  uint64_t N = 0, max_nb = 0;
+  arg.v[n_req + 1] = 0;
+  for (uint32_t r = 0; r < n_req; ++r) {
+    const int64_t len = h_offsets[r + 1] - h_offsets[r];
+    if (len < 0) return fail(nullptr, ARC_ERR_INVALID_ARG, "h_offsets not monotone at request %u", r);
+    const uint64_t nb = (uint64_t)len >> 4;
+    max_nb = std::max(max_nb, nb);
+    N += nb;
+    arg.v[n_req + 1 + r + 1] = (long long)N;
+  }
+  const uint64_t max_seg = (max_nb + K1_SEG - 1) / K1_SEG;
+  if (max_seg > K1_STATIC_MAX_SEG_PER_REQ || (uint64_t)n_req * max_seg > K1_STATIC_MAX_SEGS)
+    return fail(nullptr, ARC_ERR_REQUEST_TOO_LARGE,
+                "arc_hash_blocks_static: %u requests x %llu segments of %d blocks (the longest request has %llu blocks) exceed the fixed scratch of %u segments",
+                n_req, (unsigned long long)max_seg, K1_SEG, (unsigned long long)max_nb, K1_STATIC_MAX_SEGS);
+  if (!N) return ARC_OK;
+  if (!d_tokens || !d_keys_out) return fail(nullptr, ARC_ERR_INVALID_ARG, "NULL device pointer");
+  memcpy(arg.v, h_offsets, ((size_t)n_req + 1) * sizeof(int64_t));
+  K1StaticScratch* sc = nullptr;
+  cudaError_t e = k1_static_scratch(&sc);
+  if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "static scratch set-up: %s", cudaGetErrorString(e));
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const uint32_t total = n_req * (uint32_t)max_seg;
+  hash_segments_static_kernel<<<grid_for(total, K1_WARPS, 148 * 3), 256, K1_SMEM_BYTES, s>>>(d_tokens, n_req, (uint32_t)max_seg,
+                                                                                            (unsigned long long*)d_keys_out, sc, arg);
+  hash_fixup_static_kernel<<<grid_for(total, 8, 148 * 4), 256, 0, s>>>(n_req, (uint32_t)max_seg, (unsigned long long*)d_keys_out, sc);
+  g_hash_launches += 2;
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(nullptr, ARC_ERR_CUDA, "hash launch: %s", cudaGetErrorString(e));
   return ARC_OK;
