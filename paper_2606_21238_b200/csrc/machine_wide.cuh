@@ -386,6 +386,38 @@ __device__ __forceinline__ void wide_roller(const StepParams& P, WideShared& S, 
     R0.s0 = R0.s1 = R0.d1 = R0.d2 = R0.fm = 0; R0.my_p = R0.p; R0.err = 0; R0.calls = 0; R0.phases = 0; R0.dbl = dbl;
     const int k = S.req.k;
     RollRes& Q = S.res[i & 1u];
+    {
+      // A window of hits only (half of all windows of a warm cache) on a short path of its own: T1 entries move to T2,
+      // evictable entries stop being so, nothing else.
+      bool all_hit = true;
+      int32_t h1 = 0, e1d = 0, e2d = 0;
+#pragma unroll
+      for (int u = 0; u < WIDE_WARPS; ++u) {
+        const uint32_t km = bits_from(0, min(32, max(0, k - 32 * u)));
+        const uint32_t m0 = S.req.m[0][u] & km, m1 = S.req.m[1][u] & km, m2 = S.req.m[2][u] & km, mev = S.req.m[3][u] & km;
+        all_hit = all_hit && ((LRU ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2)) == km);
+        h1 += __popc(m0); e1d += __popc(mev & m0); e2d += __popc(mev & m1);
+      }
+      if (all_hit) {
+        // (the plan is still written: a window cut back to its leading hits after a conflict is applied by the general path)
+        WidePlan A;
+        A.src = 0; A.d1 = A.d2 = A.fm = false; A.vic_rank = A.gpush_rank = A.drop_rank = A.fresh_rank = A.alloc_rank = A.evict_rank = 0;
+        A.push_rank = (uint32_t)g;                       // every access pushes its node to T2 (LRU: T1), in access order
+        A.p = R0.p;
+        Q.plan[g] = plan_pack(A);
+        if (g == 0) {
+          Q.st[0] = R0.t1 - (LRU ? 0 : h1); Q.st[1] = R0.t2 + (LRU ? 0 : h1); Q.st[2] = R0.b1; Q.st[3] = R0.b2; Q.st[4] = R0.p; Q.st[5] = R0.nf;
+          Q.st[6] = R0.e1 - e1d; Q.st[7] = R0.e2 - (LRU ? 0 : e2d);
+#pragma unroll
+          for (int L = 0; L <= 4; ++L) Q.need[L] = 0;
+          Q.pt1 = LRU ? (uint32_t)k : 0u; Q.g1 = 0; Q.nh = 0; Q.ev = 0; Q.err = 0; Q.phases = 0;
+        }
+        __threadfence_block();
+        __syncwarp();
+        bar_arrive_n(BAR_DONE, ROLL_PARTIES);
+        continue;
+      }
+    }
     WideDecisions D;
     wide_roll<LRU>(D, R0, c, S.req.m, k, w, lane);
     WidePlan A;
