@@ -42,7 +42,7 @@ struct __align__(16) Node {
   uint32_t list;   // L_*
   uint32_t pos;    // absolute ring position of the live entry (mod 2^32)
   int32_t block;   // physical block id if resident, -1 otherwise
-  uint32_t slot;   // index of this key's table slot
+  uint32_t slot;   // index of this key's table slot when K2 or a rebuild wrote the record; not maintained by K3 (see st_node_keep_slot)
 };
 
 struct __align__(16) Slot {
@@ -145,10 +145,12 @@ __device__ __forceinline__ Node ld_node(const Node* p) {
 __device__ __forceinline__ void st_node(Node* p, uint32_t list, uint32_t pos, int32_t block, uint32_t slot) {
   __stcg(reinterpret_cast<uint4*>(p), make_uint4(list, pos, (uint32_t)block, slot));
 }
-// same, leaving the slot field as it is (for nodes whose record was never read: victims taken from a ring entry)
+// A record written for a node whose record was never read (a victim or a dropped ghost, known from its ring entry): ONE
+// 16-byte store.  The slot word is not kept up by K3 any more - K4 finds the table slot of a key that leaves the directory
+// by probing for it (finalize_body) - because the two narrower stores that left it alone cost K3 one more random sector
+// per victim and per dropped ghost, and K3's apply is bound by the store sectors its one SM can issue.
 __device__ __forceinline__ void st_node_keep_slot(Node* p, uint32_t list, uint32_t pos, int32_t block) {
-  __stcg(reinterpret_cast<uint2*>(p), make_uint2(list, pos));
-  __stcg(reinterpret_cast<int*>(p) + 2, block);
+  __stcg(reinterpret_cast<uint4*>(p), make_uint4(list, pos, (uint32_t)block, 0u));
 }
 
 }  // namespace arc

@@ -218,7 +218,18 @@ __device__ __forceinline__ void finalize_body(const StepParams& P) {
     const uint32_t d = P.dropped[a];
     if (d == NODE_NONE) continue;
     if (atomicCAS(&P.nodes[d].list, L_ABSENT, L_FREE) == L_ABSENT) {   // still absent, and only once
-      const uint32_t slot = P.nodes[d].slot;
+      // the key's slot: found by probing (the key is in the table: this thread is the one that takes it out; a probe
+      // sequence never crosses a never-used slot)
+      const unsigned long long key = P.node_key[d];
+      const uint32_t slot_mask = (P.bucket_mask + 1u) * BUCKET_SLOTS - 1u;
+      uint32_t slot = ((uint32_t)key & P.bucket_mask) * BUCKET_SLOTS;
+      for (;;) {
+        const unsigned long long k2 = __ldcg(&P.table[slot].key);
+        if (k2 == key) break;
+        if (k2 == KEY_EMPTY) { P.state->error = DEV_ERR_BAD_NODE; break; }
+        slot = (slot + 1u) & slot_mask;
+      }
+      if (P.table[slot].key != key) continue;
       P.table[slot].node = SLOT_NODE_PENDING;
       P.table[slot].key = KEY_TOMB;
       const uint32_t top = atomicAdd(&P.state->free_top, 1u);
