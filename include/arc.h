@@ -243,10 +243,12 @@ uint64_t arc_launch_count(const arc_cache *h);
  * accesses and 253 requests run as ONE kernel (K1-K4 as phases of a single CTA); larger steps run the
  * four kernels with the wide K3 machine, or the one-warp machine when requests average fewer than 48 blocks;
  * 1 = four kernels, K3 as a single-thread serial walk (the by-the-book routine on the device, much slower);
- * 2 = four kernels, one-warp machine with 32-access windows; 3 = four kernels, wide machine: one CTA of 9 warps,
- * 128-access windows, the counter recurrence rolled a window ahead by a warp of its own; 4 = the one-launch kernel for
- * every step it can take (up to 4,096 accesses and 253 requests), automatic otherwise; 5 = the wide machine without
- * the roller warp (8 warps, every owner warp rolls its window itself: round 1's form, and the one-launch kernel's). */
+ * 2 = four kernels, one-warp machine with 32-access windows; 3 = four kernels, wide machine, pipelined form: one CTA of
+ * 12 warps, 128-access windows - four owner warps (fetch, checks, apply), four scanner warps (victims from the LRU ends of
+ * the four lists) and four roller warps that work out the counter recurrence and every access's plan one window AHEAD of
+ * the owners; 4 = the one-launch kernel for every step it can take (up to 4,096 accesses and 253 requests), automatic
+ * otherwise; 5 = the wide machine without the roller warps (8 warps, every owner warp rolls its window itself: round
+ * 1's form, and the one-launch kernel's). */
 int arc_set_machine(arc_cache *h, int which);
 
 /* K2 alone, for the probe microbenchmark and its tests: looks every key of d_keys (DEVICE uint64[n], values >= 2) up in

@@ -1,5 +1,9 @@
-// K3, wide form: one CTA of 4 warps consumes the step's accesses in the fixed order R2, a window of up to 128
-// accesses at a time.  Same equivalence argument as machine_batched.cuh; what changes is who does what:
+// K3, wide form: one CTA consumes the step's accesses in the fixed order R2, a window of up to 128 accesses at a time.
+// Two forms of one source (template parameter PIPE): the plain form (8 warps: owners 0..3, scanners 4..7; every owner warp
+// rolls the counters of its window itself; also the third phase of the one-launch kernel) and the pipelined form (12
+// warps: four ROLLER warps work out the recurrence and every access's plan one window ahead of the owners, see
+// wide_roller; named barriers instead of __syncthreads).
+// Same equivalence argument as machine_batched.cuh; what changes is who does what:
 //   * thread g = 32 w + lane owns access g of the window: it fetches the node record, checks the window's cut
 //     conditions for its access, and applies its access;
 //   * the counter recurrence (wide_roll: 32 accesses at a time, phases inlined) is run redundantly and identically by all four
@@ -106,11 +110,32 @@ __device__ __forceinline__ uint32_t wide_count(const uint32_t (&mask)[WIDE_WARPS
 // window numbers: 31 bits, never 0 (0 = never stamped)
 __device__ __forceinline__ uint32_t wide_next_seq(uint32_t s) { s = (s + 1u) & 0x7FFFFFFFu; return s ? s : 1u; }
 
+// What a thread keeps of the decisions of a roll: not the masks of all four chunks (the chunk loop is not unrolled, so
+// they would be reached by chains of predicated moves: 250 of the 720 instructions a roller warp spent per window) but,
+// for each of the six decision masks, exactly what its plan and the window's counts need - the mask of ITS chunk, the
+// bits set in the chunks below it, the bits set in the whole window - accumulated chunk by chunk while the roll goes on.
+enum : int { F_S0 = 0,                       // evicts T1's LRU entry (with or without a ghost)
+             F_S2,                           // evicts T2's LRU entry (it becomes a ghost of B2)
+             F_G1,                           // its T1 victim becomes a ghost of B1
+             F_D1, F_D2,                     // drops the LRU ghost of B1 / B2
+             F_FM,                           // takes a fresh block id
+             F_COUNT };
 struct WideDecisions {
-  uint32_t s0[WIDE_WARPS], s1[WIDE_WARPS], d1[WIDE_WARPS], d2[WIDE_WARPS], fm[WIDE_WARPS];
+  uint32_t mine[F_COUNT], below[F_COUNT], total[F_COUNT];
   int32_t my_p;
   Roll R;                                    // state after the window
 };
+// chunk u's decision masks join the accumulators of a thread whose access is in chunk `warp`
+__device__ __forceinline__ void wide_acc(WideDecisions& D, int u, int warp, uint32_t s0, uint32_t s1, uint32_t d1, uint32_t d2, uint32_t fm) {
+  const uint32_t f[F_COUNT] = {s0, s1 & ~s0, s0 & ~s1, d1, d2, fm};
+#pragma unroll
+  for (int i = 0; i < F_COUNT; ++i) {
+    const uint32_t pc = (uint32_t)__popc(f[i]);
+    D.total[i] += pc;
+    if (u < warp) D.below[i] += pc;
+    if (u == warp) D.mine[i] = f[i];
+  }
+}
 
 // The recurrence over the first k accesses of the window, chunk by chunk (every warp computes the same thing).
 // Sm: the class masks m0, m1, m2, me per chunk (shared memory); warp = the chunk this thread's access is in.
@@ -128,10 +153,12 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const Roll& R0, int3
     for (int u = 0; u < WIDE_WARPS; ++u) any |= (Sm[0][u] | Sm[1][u] | Sm[2][u]) & bits_from(0, min(32, max(0, k - 32 * u)));
     Roll& R = D.R;
     if (!lru && any == 0 && R.t1 + R.t2 == c && R.t1 + R.b1 == c && R.t1 < c && R.t1 > R.p && R.e1 >= k) {
+      // every access evicts from T1 into B1 and drops B1's LRU ghost
+      const uint32_t mine = bits_from(0, min(32, max(0, k - 32 * warp))), below = (uint32_t)min(k, 32 * warp);
 #pragma unroll
-      for (int u = 0; u < WIDE_WARPS; ++u) {
-        const uint32_t km = bits_from(0, min(32, max(0, k - 32 * u)));
-        D.s0[u] = km; D.d1[u] = km; D.s1[u] = D.d2[u] = D.fm[u] = 0;
+      for (int i = 0; i < F_COUNT; ++i) {
+        const bool on = (i == F_S0 || i == F_G1 || i == F_D1);
+        D.mine[i] = on ? mine : 0u; D.below[i] = on ? below : 0u; D.total[i] = on ? (uint32_t)k : 0u;
       }
       R.e1 -= k;
       R.phases++;
@@ -140,9 +167,9 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const Roll& R0, int3
   }
   // ONE copy of the chunk body, looped over (not unrolled): the body with its inlined phases is the largest piece of code of
   // the kernel, and four copies each run once per window are four times the instruction-cache footprint of one copy run
-  // four times.  The chunk's decision masks reach their (statically indexed, register) slots by predicated moves.
+  // four times.
 #pragma unroll
-  for (int v = 0; v < WIDE_WARPS; ++v) D.s0[v] = D.s1[v] = D.d1[v] = D.d2[v] = D.fm[v] = 0;
+  for (int i = 0; i < F_COUNT; ++i) D.mine[i] = D.below[i] = D.total[i] = 0;
 #pragma unroll 1
   for (int u = 0; u < WIDE_WARPS; ++u) {
     const int ku = min(32, max(0, k - 32 * u));
@@ -190,9 +217,7 @@ __device__ __forceinline__ void wide_roll(WideDecisions& D, const Roll& R0, int3
           i += n;
         }
       }
-#pragma unroll
-      for (int v = 0; v < WIDE_WARPS; ++v)
-        if (v == u) { D.s0[v] = D.R.s0; D.s1[v] = D.R.s1; D.d1[v] = D.R.d1; D.d2[v] = D.R.d2; D.fm[v] = D.R.fm; }
+      if (hits != km) wide_acc(D, u, warp, D.R.s0, D.R.s1, D.R.d1, D.R.d2, D.R.fm);   // (a chunk of hits decides nothing)
       if (u == warp) D.my_p = D.R.my_p;
     }
   }
@@ -224,36 +249,39 @@ __device__ __forceinline__ WidePlan plan_unpack(const uint4 v) {
   return A;
 }
 
-// The plan of this thread's access and the window's counts from the decisions of a roll over k accesses.  Sm: the class
-// masks the roll used; lm / me: the thread's rank masks (wide_rank / wide_has).
+// The plan of this thread's access and the window's counts from what the roll over k accesses accumulated (D).  Sm: the
+// class masks the roll used; lm / me: the thread's rank masks (wide_rank / wide_has); g: its index in the window.  Ranks in
+// the decision masks come from the accumulators; the pushes to T1 and to T2 partition the window, so do hits and
+// allocations, and an eviction comes either from T1 or from T2: two ranks are counted in the class masks, the rest follows.
 template <bool lru>
 __device__ __forceinline__ void wide_make_plan(WidePlan& A, WideCounts& N, const WideDecisions& D, const uint32_t (*Sm)[WIDE_WARPS], int k,
-                                               const uint32_t (&lm)[WIDE_WARPS], const uint32_t (&me)[WIDE_WARPS]) {
-  uint32_t S2[WIDE_WARPS], G1[WIDE_WARPS], PT1[WIDE_WARPS], PT2[WIDE_WARPS], NH[WIDE_WARPS], EV[WIDE_WARPS];
+                                               uint32_t g, const uint32_t (&lm)[WIDE_WARPS], const uint32_t (&me)[WIDE_WARPS]) {
+  uint32_t PT1[WIDE_WARPS], HIT[WIDE_WARPS];
 #pragma unroll
   for (int u = 0; u < WIDE_WARPS; ++u) {
     const uint32_t km = bits_from(0, min(32, max(0, k - 32 * u)));
     const uint32_t m0 = Sm[0][u], m1 = Sm[1][u], m2 = Sm[2][u];
-    const uint32_t hit = (lru ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2)) & km;
-    S2[u] = D.s1[u] & ~D.s0[u];                                        // evictions from T2 = pushes to B2
-    G1[u] = D.s0[u] & ~D.s1[u];                                        // pushes to B1, in access order
     PT1[u] = lru ? km : (~(m0 | m1 | m2) & km);                        // ABSENT nodes enter T1 (LRU: everything)
-    PT2[u] = km & ~PT1[u];
-    NH[u] = km & ~hit;
-    EV[u] = D.s0[u] | D.s1[u];
+    HIT[u] = (lru ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2)) & km;
   }
-  A.src = (uint32_t)wide_has(D.s0, me) | ((uint32_t)wide_has(D.s1, me) << 1);
-  A.d1 = wide_has(D.d1, me); A.d2 = wide_has(D.d2, me); A.fm = wide_has(D.fm, me);
-  A.vic_rank = (A.src == 2) ? wide_rank(S2, lm) : wide_rank(D.s0, lm);
-  A.gpush_rank = (A.src == 1) ? wide_rank(G1, lm) : wide_rank(S2, lm);
-  A.drop_rank = A.d1 ? wide_rank(D.d1, lm) : wide_rank(D.d2, lm);
-  A.fresh_rank = wide_rank(D.fm, lm);
-  A.push_rank = wide_has(PT1, me) ? wide_rank(PT1, lm) : wide_rank(PT2, lm);
-  A.alloc_rank = wide_rank(NH, lm);
-  A.evict_rank = wide_rank(EV, lm);
+  const uint32_t bit = 1u << (g & 31u), lt = bit - 1u;
+  uint32_t rk[F_COUNT];
+  bool on[F_COUNT];
+#pragma unroll
+  for (int i = 0; i < F_COUNT; ++i) { on[i] = (D.mine[i] & bit) != 0; rk[i] = D.below[i] + (uint32_t)__popc(D.mine[i] & lt); }
+  A.src = on[F_S2] ? 2u : (on[F_S0] ? (on[F_G1] ? 1u : 3u) : 0u);
+  A.d1 = on[F_D1]; A.d2 = on[F_D2]; A.fm = on[F_FM];
+  A.vic_rank = on[F_S2] ? rk[F_S2] : rk[F_S0];
+  A.gpush_rank = on[F_G1] ? rk[F_G1] : rk[F_S2];
+  A.drop_rank = on[F_D1] ? rk[F_D1] : rk[F_D2];
+  A.fresh_rank = rk[F_FM];
+  const uint32_t r_pt1 = wide_rank(PT1, lm);
+  A.push_rank = wide_has(PT1, me) ? r_pt1 : g - r_pt1;
+  A.alloc_rank = g - wide_rank(HIT, lm);
+  A.evict_rank = rk[F_S0] + rk[F_S2];
   A.p = D.my_p;
-  N.need[0] = 0; N.need[L_T1] = wide_count(D.s0); N.need[L_T2] = wide_count(S2); N.need[L_B1] = wide_count(D.d1); N.need[L_B2] = wide_count(D.d2);
-  N.pt1 = wide_count(PT1); N.g1 = wide_count(G1); N.nh = wide_count(NH); N.ev = wide_count(EV);
+  N.need[0] = 0; N.need[L_T1] = D.total[F_S0]; N.need[L_T2] = D.total[F_S2]; N.need[L_B1] = D.total[F_D1]; N.need[L_B2] = D.total[F_D2];
+  N.pt1 = wide_count(PT1); N.g1 = D.total[F_G1]; N.nh = (uint32_t)k - wide_count(HIT); N.ev = D.total[F_S0] + D.total[F_S2];
 }
 
 // One scan round of a scanner warp: 128 ring entries from q0 (a multiple of 4), 4 per lane; live entries are appended
@@ -422,7 +450,7 @@ __device__ __forceinline__ void wide_roller(const StepParams& P, WideShared& S, 
     wide_roll<LRU>(D, R0, c, S.req.m, k, w, lane);
     WidePlan A;
     WideCounts N;
-    wide_make_plan<LRU>(A, N, D, S.req.m, k, lm, me);
+    wide_make_plan<LRU>(A, N, D, S.req.m, k, (uint32_t)g, lm, me);
     Q.plan[g] = plan_pack(A);
     if (g == 0) {
       Q.st[0] = D.R.t1; Q.st[1] = D.R.t2; Q.st[2] = D.R.b1; Q.st[3] = D.R.b2; Q.st[4] = D.R.p; Q.st[5] = D.R.nf; Q.st[6] = D.R.e1; Q.st[7] = D.R.e2;
@@ -732,7 +760,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
         } else {                                                     // the plain form: every owner warp rolls, every thread plans
           WideDecisions D;
           wide_roll<LRU>(D, roll_init(C), c, S.m, kk, warp, lane);
-          wide_make_plan<LRU>(A, NC, D, S.m, kk, lm, me);
+          wide_make_plan<LRU>(A, NC, D, S.m, kk, (uint32_t)tid, lm, me);
           RS[0] = D.R.t1; RS[1] = D.R.t2; RS[2] = D.R.b1; RS[3] = D.R.b2; RS[4] = D.R.p; RS[5] = D.R.nf; RS[6] = D.R.e1; RS[7] = D.R.e2;
           r_err = D.R.err; r_phases = D.R.phases;
         }
