@@ -372,7 +372,10 @@ def measure_config(torch, A, config, n_warm, n_timed, seed, stream, full=True, c
         P.barrier(dist)
     st_arc = cache.stats()
     cache.close()
-    e2e_ms, d2h, h2d = run_e2e(torch, A, info, steps, host, bases, n_warm, stream)
+    # the end-to-end leg is timed on the HOST clock (that is its point), so it sees whatever else the box's cores are doing:
+    # two passes over the same steps, the faster one is reported, both are printed
+    e2e_passes = [run_e2e(torch, A, info, steps, host, bases, n_warm, stream) for _ in range(2)]
+    e2e_ms, d2h, h2d = min(e2e_passes, key=lambda t: t[0])
     if P is not None:
         ms, tot_acc, tot_tok, tot_req = P.reduce_timing(dist, torch, ms, n_acc, n_tok, n_req)
         e2e_ms, _, _, _ = P.reduce_timing(dist, torch, e2e_ms, n_acc, n_tok, n_req)
@@ -382,7 +385,8 @@ def measure_config(torch, A, config, n_warm, n_timed, seed, stream, full=True, c
                tokens_seen_per_s=tot_tok / (ms * 1e-3), requests_per_s=tot_req / (ms * 1e-3), gpu_launches=launches,
                launches_per_step=launches / n_timed,
                e2e={"value": tot_acc / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / n_timed, "d2h_bytes_per_step": d2h / n_timed,
-                    "ms_per_step": e2e_ms / n_timed, "api": "arc_step_host_async / arc_step_host_wait, one step ahead (pinned host tokens in; n_alloc | n_evict | prefix_len | alloc_ids | evict_ids written to pinned host memory)", "timed": "host wall clock, first enqueue to the last result on the host"},
+                    "ms_per_step": e2e_ms / n_timed, "api": "arc_step_host_async / arc_step_host_wait, one step ahead (pinned host tokens in; n_alloc | n_evict | prefix_len | alloc_ids | evict_ids written to pinned host memory)", "timed": "host wall clock, first enqueue to the last result on the host; the faster of two passes over the same steps",
+                    "passes_ms_per_step": [t[0] / n_timed for t in e2e_passes]},
                state={k: st_arc[k] for k in ("t1", "t2", "b1", "b2", "p")})
     if clk is not None:
         res["clocks"] = clk.summary()
