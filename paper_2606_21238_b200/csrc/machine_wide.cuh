@@ -66,6 +66,8 @@ struct RollRes {
   uint32_t need[5];                          // victims / drops the window takes per list
   uint32_t pt1, g1, nh, ev;                  // pushes to T1 and to B1, allocations, evictions of the window
   uint32_t err, phases;
+  uint32_t all_hit, badnode, h1, e1d, e2d;   // the window is hits only; a FREE node is among its nodes; if hits only: hits in T1,
+                                             // hits on entries of T1 / T2 that were still evictable
 };
 
 struct WideShared {
@@ -330,6 +332,10 @@ __device__ __forceinline__ void wide_scanner(const StepParams& P, WideShared& S,
     uint32_t q0 = head & ~3u, found = 0;
     int want = (int)S.ctl_k;
     ScanRegs cur = wide_scan_load(ring, P.ring_mask, q0, lane);   // in flight while the owners fetch; used after B1
+    // The LRU end of a list is the part of its ring that was written longest ago: in a cache larger than L2 it is in DRAM by
+    // now, and a scan that waits for it holds up the whole window.  Each lane asks for one 128-byte line of the 512 entries
+    // AFTER this window's first round to be brought into L2 (the next windows' first rounds); a line that is there costs nothing.
+    if (PIPE) asm volatile("prefetch.global.L2 [%0];" ::"l"(ring + (((q0 & ~15u) + (uint32_t)WIDE_W + 16u * (uint32_t)lane) & P.ring_mask)));
     cta_sync<PIPE>();                                  // (B1) the scanners never hold this barrier up
     if (S.twinc[0] | S.twinc[1] | S.twinc[2] | S.twinc[3]) { cta_sync<PIPE>(); cta_sync<PIPE>(); want = (int)S.twin_k; }
     // while the owners roll (not in an all-hit window, which needs no victim): up to 3 rounds, until as many live entries
@@ -419,13 +425,17 @@ __device__ __forceinline__ void wide_roller(const StepParams& P, WideShared& S, 
       // evictable entries stop being so, nothing else.
       bool all_hit = true;
       int32_t h1 = 0, e1d = 0, e2d = 0;
+      uint32_t badnode = 0;
 #pragma unroll
       for (int u = 0; u < WIDE_WARPS; ++u) {
         const uint32_t km = bits_from(0, min(32, max(0, k - 32 * u)));
         const uint32_t m0 = S.req.m[0][u] & km, m1 = S.req.m[1][u] & km, m2 = S.req.m[2][u] & km, mev = S.req.m[3][u] & km;
         all_hit = all_hit && ((LRU ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2)) == km);
         h1 += __popc(m0); e1d += __popc(mev & m0); e2d += __popc(mev & m1);
+        badnode |= m2 & m0;
       }
+      // the owners of a window whose roll-ahead stands take these instead of reading the class masks themselves
+      if (g == 0) { Q.all_hit = all_hit ? 1u : 0u; Q.badnode = badnode; Q.h1 = (uint32_t)h1; Q.e1d = (uint32_t)e1d; Q.e2d = (uint32_t)e2d; }
       if (all_hit) {
         // (the plan is still written: a window cut back to its leading hits after a conflict is applied by the general path)
         WidePlan A;
@@ -674,16 +684,22 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
         have_prov = true;
       };
       if (!aligned) issue_spec();                                    // a node this window accesses too is not trusted (its stamp says so)
-      uint32_t M0[WIDE_WARPS], M1[WIDE_WARPS], M2[WIDE_WARPS], ME[WIDE_WARPS], KM[WIDE_WARPS], HIT[WIDE_WARPS];
+      // hits only?  and if so: hits in T1, hits on entries of T1 / T2 that were still evictable.  From the rollers when their
+      // roll-ahead of this window stands (they read the same masks), else from the class masks in shared memory.
       bool all_hit = true;
-      uint32_t badnode = 0;
+      uint32_t badnode = 0, t1hits = 0, e1d = 0, e2d = 0;
+      if (prov_valid) {
+        const RollRes& Q = S.res[got_par & 1u];
+        all_hit = Q.all_hit != 0; badnode = Q.badnode; t1hits = Q.h1; e1d = Q.e1d; e2d = Q.e2d;
+      } else {
 #pragma unroll
-      for (int u = 0; u < WIDE_WARPS; ++u) {
-        M0[u] = S.m[0][u]; M1[u] = S.m[1][u]; M2[u] = S.m[2][u]; ME[u] = S.m[3][u];
-        KM[u] = bits_from(0, min(32, max(0, k - 32 * u)));
-        HIT[u] = (lru ? (M0[u] & ~M1[u] & ~M2[u]) : ((M0[u] ^ M1[u]) & ~M2[u])) & KM[u];
-        all_hit = all_hit && (HIT[u] == KM[u]);
-        badnode |= M2[u] & M0[u] & KM[u];
+        for (int u = 0; u < WIDE_WARPS; ++u) {
+          const uint32_t km = bits_from(0, min(32, max(0, k - 32 * u)));
+          const uint32_t m0 = S.m[0][u] & km, m1 = S.m[1][u] & km, m2 = S.m[2][u] & km, mev = S.m[3][u] & km;
+          all_hit = all_hit && ((lru ? (m0 & ~m1 & ~m2) : ((m0 ^ m1) & ~m2)) == km);
+          badnode |= m2 & m0;
+          t1hits += (uint32_t)__popc(m0); e1d += (uint32_t)__popc(mev & m0); e2d += (uint32_t)__popc(mev & m1);
+        }
       }
       if (badnode) C.err = DEV_ERR_BAD_NODE;                         // a FREE node reached K3
       const uint32_t tw1 = (uint32_t)clock();
@@ -693,13 +709,6 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
       if (all_hit) {
         // ---- every access of the window is a hit: no counter other than t1/t2 moves, nothing is evicted
         const uint32_t q = (lru ? C.tail[L_T1] : C.tail[L_T2]) + (uint32_t)tid;
-        uint32_t t1hits = 0, e1d = 0, e2d = 0;
-#pragma unroll
-        for (int u = 0; u < WIDE_WARPS; ++u) {
-          t1hits += (uint32_t)__popc(M0[u] & KM[u]);
-          e1d += (uint32_t)__popc(ME[u] & M0[u] & KM[u]);
-          e2d += (uint32_t)__popc(ME[u] & M1[u] & KM[u]);
-        }
         if (lru) { C.tail[L_T1] += hold ? 0u : (uint32_t)k; C.stat[ST_HIT_T1] += (uint32_t)k; }
         else { C.tail[L_T2] += hold ? 0u : (uint32_t)k; C.t1 -= (int32_t)t1hits; C.t2 += (int32_t)t1hits; C.stat[ST_HIT_T1] += t1hits; C.stat[ST_HIT_T2] += (uint32_t)k - t1hits; }
         C.elig1 -= (int32_t)e1d; C.elig2 -= (int32_t)e2d;
