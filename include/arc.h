@@ -275,7 +275,10 @@ int arc_debug_set_key_mask(arc_cache *h, uint64_t mask);
  * all-hit windows, general windows, by-the-book single accesses, windows cut at a repeated node, windows cut at a
  * conflict, ring scan rounds, accesses applied in all-hit windows, accesses applied in general windows, then
  * SM cycles spent in: fetch, roll-forward, victim scan, apply, single accesses, the whole kernel; then the number of
- * calls of the roll-forward routine and of its phases.  Synchronises. */
+ * calls of the roll-forward routine and of its phases; then (pipelined wide machine) the windows whose decisions had been
+ * rolled ahead by the roller warps and stood, and the windows that had to be rolled on request.  Synchronises.  (In the
+ * pipelined form "roll-forward" cycles are what the owners spend taking the rollers' result; the wait for it is booked
+ * under fetch.) */
 int arc_debug_counters(arc_cache *h, uint64_t *out, uint32_t n);
 
 /* Per-access latency of the by-the-book K3 machine (arc_set_machine(h, 1)) by class, cumulative since create/reset:
