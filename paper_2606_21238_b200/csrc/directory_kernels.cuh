@@ -209,6 +209,20 @@ __global__ void __launch_bounds__(256) gather32_kernel(const unsigned long long*
   }
 }
 
+// Step-wide / held pins: the wide K3 machine lets a window span requests there and takes each access's natural-order index
+// (blk_off[r] + i for the access at blk_off[r] + nb_r - 1 - i) from nat[]: one warp per request.  Launched after K2 into the
+// buffer of the keys, which nothing reads after the probe.
+__device__ __forceinline__ void nat_index_body(const StepParams& P, uint32_t warp, uint32_t n_warps, uint32_t lane) {
+  uint32_t* nat = reinterpret_cast<uint32_t*>(P.keys_acc);
+  for (uint32_t r = warp; r < P.n_req; r += n_warps) {
+    const int64_t o = P.blk_off[r], nb = P.blk_off[r + 1] - o;
+    for (int64_t i = lane; i < nb; i += 32) nat[o + (nb - 1 - i)] = (uint32_t)(o + i);
+  }
+}
+__global__ void __launch_bounds__(256) nat_index_kernel(const __grid_constant__ StepParams P) {
+  nat_index_body(P, (blockIdx.x * blockDim.x + threadIdx.x) >> 5, (gridDim.x * blockDim.x) >> 5, threadIdx.x & 31);
+}
+
 // ---------------------------------------------------------------------------------------------------
 // K4: (1) keys whose node ended the step ABSENT (dropped ghosts, evictions that leave no ghost) leave
 // the table and their nodes return to the free stack; (2) prefix_len[r] = B x leading hit blocks (R9).

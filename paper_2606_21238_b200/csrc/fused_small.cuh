@@ -119,6 +119,10 @@ __global__ void __launch_bounds__(2 * WIDE_W, 1) arc_fused_small_kernel(const __
   // ---- phase 2: K2
   probe_range(P, (uint32_t)tid, blockDim.x);
   __syncthreads();
+  if (P.pin_scope != 0) {                                            // the window machines' windows span requests there (nat_index_body)
+    nat_index_body(P, (uint32_t)warp, blockDim.x >> 5, (uint32_t)lane);
+    __syncthreads();
+  }
   // ---- phase 3: K3
   if (machine == 2) { if (warp == 0) batched_machine_run(P, F.vic); }
   else wide_machine_run<LRU, HOLD, false>(P, F.wide);

@@ -643,6 +643,10 @@ int arc_step_resume(arc_cache* h, const int32_t* d_tokens, const int64_t* h_offs
     if (h->profiling) cudaEventRecord(h->ev[2], s);
     probe_reserve_kernel<<<grid_for(N, 256 * PROBE_ILP, 148 * 8), 256, 0, s>>>(P);                        // K2
     h->launches += 2;
+    if (h->machine != 1 && h->pin_scope != ARC_PIN_REQUEST) {     // windows of the window machines span requests there: natural-order indices
+      nat_index_kernel<<<grid_for((uint64_t)n_req * 32, 256, 148 * 4), 256, 0, s>>>(P);
+      h->launches += 1;
+    }
   } else {
     // no full block anywhere: every request keeps the state it came with
     if (n_req) {

@@ -273,13 +273,19 @@ __device__ __forceinline__ void batched_machine_run(const StepParams& P, uint4 (
   int64_t pre_base = 0;
   uint32_t pre_n = (lane < N) ? P.node_acc[lane] : NODE_NONE;
 
+  // step-wide and held pins: nothing restarts at a request boundary, so the step is one run of accesses and a window may
+  // span requests (16 one-block decode appends are one window); the natural-order index of an access then comes from
+  // nat_acc[] (see machine_wide.cuh)
+  const bool merged = P.pin_scope != 0;
+  const uint32_t* nat_acc = reinterpret_cast<const uint32_t*>(P.keys_acc);
+  const uint32_t n_groups = merged ? 1u : P.n_req;
   int64_t my_off = 0, my_off1 = 0;
-  for (uint32_t r = 0; r < P.n_req; ++r) {
-    if ((r & 31u) == 0) {      // block offsets of the next 32 requests, one per lane
+  for (uint32_t r = 0; r < n_groups; ++r) {
+    if (!merged && (r & 31u) == 0) {      // block offsets of the next 32 requests, one per lane
       const uint32_t rr = min(r + (uint32_t)lane, P.n_req - 1);
       my_off = P.blk_off[rr]; my_off1 = P.blk_off[rr + 1];
     }
-    const int64_t o = __shfl_sync(FULL, my_off, r & 31), nb = __shfl_sync(FULL, my_off1, r & 31) - o;
+    const int64_t o = merged ? 0 : __shfl_sync(FULL, my_off, r & 31), nb = merged ? N : __shfl_sync(FULL, my_off1, r & 31) - o;
     // step-wide scope: the pins of earlier requests of the step stay.  Held scope (2): accessed nodes leave the rings and
     // come back through arc_release, so every ring entry is a possible victim (bound = tail), no tail of T1 / T2 moves
     // during a step, and elig1 / elig2 (the unheld entries) carry over from step to step in DevState.
@@ -338,7 +344,7 @@ __device__ __forceinline__ void batched_machine_run(const StepParams& P, uint4 (
             __stcg((lru ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, rec.block));
             st_node(P.nodes + n, Lp, q, rec.block, rec.slot);
           }
-          const int64_t out = o + (nb - 1 - (j + lane));
+          const int64_t out = merged ? (int64_t)__ldcg(nat_acc + a0 + lane) : o + (nb - 1 - (j + lane));
           P.cls[out] = (uint8_t)lst;                               // L_T1 == CLS_HIT_T1, L_T2 == CLS_HIT_T2
           P.block_id[out] = rec.block;
           P.evicted_id[out] = -1;
@@ -425,7 +431,7 @@ __device__ __forceinline__ void batched_machine_run(const StepParams& P, uint4 (
         dbg[DBG_CUT_CONFLICT]++;
         if (k == 0) {                       // the by-the-book routine, run identically by every lane
           SerialCtx T = C;                           // the callee is not inlined: keep C itself in registers
-          serial_access(T, P, a0, o + (nb - 1 - j));
+          serial_access(T, P, a0, merged ? (int64_t)__ldcg(nat_acc + a0) : o + (nb - 1 - j));
           C = T;
           j += 1;
           __syncwarp();
@@ -488,7 +494,7 @@ __device__ __forceinline__ void batched_machine_run(const StepParams& P, uint4 (
           __stcg((toT1 ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, blk));
           st_node(P.nodes + n, Lp, q, blk, rec.slot);
         }
-        const int64_t out = o + (nb - 1 - (j + lane));
+        const int64_t out = merged ? (int64_t)__ldcg(nat_acc + a0 + lane) : o + (nb - 1 - (j + lane));
         P.cls[out] = (uint8_t)lst;                    // ABSENT -> MISS(0), T1 -> 1, T2 -> 2, B1 -> 3, B2 -> 4
         P.block_id[out] = blk;
         P.evicted_id[out] = ev;

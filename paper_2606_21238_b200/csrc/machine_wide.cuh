@@ -556,13 +556,21 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
     }
   };
 
+  // Step-wide and held pins: nothing restarts at a request boundary (the pin bound and the evictable counts are those of
+  // the step, or carry over), so the whole step is ONE run of accesses and a window may span requests: 24 one-block decode
+  // appends are one window, not 24.  Only the natural-order index of an access then depends on its request: it comes
+  // from nat_acc[] (nat_index_kernel / the one-launch kernel).  A node that two requests of a window share is a repeated node
+  // like any other: the window is cut before its second occurrence.
+  const bool merged = hold || P.pin_scope == 1;
+  const uint32_t* nat_acc = reinterpret_cast<const uint32_t*>(P.keys_acc);   // the keys are K2's input only: their buffer is free now
+  const uint32_t n_groups = merged ? 1u : P.n_req;
   int64_t my_off = 0, my_off1 = 0, my_off2 = 0;
-  for (uint32_t r = 0; r < P.n_req; ++r) {
-    if ((r & 31u) == 0) {      // block offsets of the next 32 requests, one per lane (every warp keeps its own copy)
+  for (uint32_t r = 0; r < n_groups; ++r) {
+    if (!merged && (r & 31u) == 0) {      // block offsets of the next 32 requests, one per lane (every warp keeps its own copy)
       const uint32_t rr = min(r + (uint32_t)lane, P.n_req - 1);
       my_off = P.blk_off[rr]; my_off1 = P.blk_off[rr + 1]; my_off2 = P.blk_off[min(rr + 2, P.n_req)];
     }
-    const int64_t o = __shfl_sync(FULL, my_off, r & 31), nb = __shfl_sync(FULL, my_off1, r & 31) - o;
+    const int64_t o = merged ? 0 : __shfl_sync(FULL, my_off, r & 31), nb = merged ? N : __shfl_sync(FULL, my_off1, r & 31) - o;
     if (!hold && (r == 0 || P.pin_scope == 0)) begin_request(C);   // step-wide scope: the pins of earlier requests of the step stay
     int64_t j = 0;
     while (j < nb) {
@@ -574,7 +582,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
       int next_k = WIDE_W;
       bool next_exact = false, next_new_req = false;       // the size is exact; that window is the first of a request
       if (j + kmax < nb) { next_k = (int)min((int64_t)WIDE_W, nb - j - kmax); next_exact = true; }
-      else if (r + 1u < P.n_req) {
+      else if (!merged && r + 1u < P.n_req) {
         const int64_t nb1 = __shfl_sync(FULL, my_off2, r & 31) - __shfl_sync(FULL, my_off1, r & 31);
         if (nb1 > 0) { next_k = (int)min((int64_t)WIDE_W, nb1); next_exact = true; next_new_req = true; }
       }
@@ -727,7 +735,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
             __stcg((lru ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, rec.block));
             st_node(P.nodes + n, lru ? L_T1 : L_T2, q, rec.block, rec.slot);
           }
-          const int64_t out = o + (nb - 1 - (j + tid));
+          const int64_t out = merged ? (int64_t)__ldcg(nat_acc + a0 + tid) : o + (nb - 1 - (j + tid));
           P.cls[out] = (uint8_t)lst;                               // L_T1 == CLS_HIT_T1, L_T2 == CLS_HIT_T2
           P.block_id[out] = rec.block;
           P.evicted_id[out] = -1;
@@ -838,7 +846,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
           // the by-the-book routine, by warp 0 alone; the new machine state reaches the other warps through shared memory
           if (warp == 0) {
             SerialCtx T = C;                           // the callee is not inlined: keep C itself in registers
-            serial_access(T, P, a0, o + (nb - 1 - j));
+            serial_access(T, P, a0, merged ? (int64_t)__ldcg(nat_acc + a0) : o + (nb - 1 - j));
             __syncwarp();
             if (lane == 0) S.ctx = T;
           }
@@ -892,7 +900,7 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
           __stcg((toT1 ? P.ring[L_T1] : P.ring[L_T2]) + (q & P.ring_mask), ring_ent(n, blk));
           st_node(P.nodes + n, toT1 ? L_T1 : L_T2, q, blk, rec.slot);
         }
-        const int64_t out = o + (nb - 1 - (j + tid));
+        const int64_t out = merged ? (int64_t)__ldcg(nat_acc + a0 + tid) : o + (nb - 1 - (j + tid));
         P.cls[out] = (uint8_t)lst;                    // ABSENT -> MISS(0), T1 -> 1, T2 -> 2, B1 -> 3, B2 -> 4
         P.block_id[out] = blk;
         P.evicted_id[out] = ev;
