@@ -556,12 +556,13 @@ __device__ __forceinline__ void wide_machine_run(const StepParams& P, WideShared
     }
   };
 
-  // Step-wide and held pins: nothing restarts at a request boundary (the pin bound and the evictable counts are those of
-  // the step, or carry over), so the whole step is ONE run of accesses and a window may span requests: 24 one-block decode
+  // Held pins: nothing restarts at a request boundary (the evictable counts carry over, every ring entry is a possible
+  // victim), so the whole step is ONE run of accesses and a window may span requests: 24 one-block decode
   // appends are one window, not 24.  Only the natural-order index of an access then depends on its request: it comes
   // from nat_acc[] (nat_index_kernel / the one-launch kernel).  A node that two requests of a window share is a repeated node
   // like any other: the window is cut before its second occurrence.
-  const bool merged = hold || P.pin_scope == 1;
+  constexpr bool merged = HOLD;            // (a compile-time fact on purpose: as a run-time flag for the step-wide scope too it cost
+                                           // the default scope 12 - 19 % - seven more registers and a different schedule of the whole loop)
   const uint32_t* nat_acc = reinterpret_cast<const uint32_t*>(P.keys_acc);   // the keys are K2's input only: their buffer is free now
   const uint32_t n_groups = merged ? 1u : P.n_req;
   int64_t my_off = 0, my_off1 = 0, my_off2 = 0;
