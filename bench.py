@@ -593,8 +593,8 @@ def serving_loop_leg(torch, A, info, steps, stream, seed, n_steps=240, new_per_s
     dev_tok = [torch.from_numpy(t).cuda() for t, _, _, _ in plan]
     s0_new = torch.full((new_per_step,), S0, dtype=torch.int64, device="cuda")                 # S0 < 2^63: same bit pattern
 
-    def run(cache, on_gpu):
-        """One pass of the loop; returns (accesses, ids released)."""
+    def run(cache, on_gpu, prof=None):
+        """One pass of the loop; returns (accesses, ids released).  prof: a dict that collects the library's own kernel times."""
         hist = []                # per step: (block ids of each of its sequences so far, their chain states)
         n_acc = n_rel = 0
         for i, (tok, off, n_new, n_dec) in enumerate(plan):
@@ -603,6 +603,9 @@ def serving_loop_leg(torch, A, info, steps, stream, seed, n_steps=240, new_per_s
             if on_gpu:
                 chain = torch.cat([s0_new] + [c["state"] for c in cohorts])
                 r = cache.step(dev_tok[i], off, stream, chain_in=chain)
+                if prof is not None:
+                    for k, v in cache.last_kernel_times().items():
+                        prof[k] = prof.get(k, 0.0) + v
                 ids, st, bo = r.block_id.clone(), r.chain_state.clone(), off // 16
             else:
                 chain = np.concatenate([np.full(n_new, S0, np.uint64)] + [c["state"] for c in cohorts])
@@ -637,6 +640,9 @@ def serving_loop_leg(torch, A, info, steps, stream, seed, n_steps=240, new_per_s
     stream.synchronize()
     ms = ev0.elapsed_time(ev1)
     st = cache.stats()
+    prof = {}                                                             # a third pass with the library's events between its kernels
+    cache.set_profiling(True)
+    run(cache, True, prof)
     cache.close()
     oc = O.OracleCache(info.capacity_blocks, info.block_size, 0)
     oc.set_pin_scope(2)
@@ -650,6 +656,9 @@ def serving_loop_leg(torch, A, info, steps, stream, seed, n_steps=240, new_per_s
                     f"(one per step) and then releases everything it holds; c={info.capacity_blocks}",
             "steps": n_steps, "accesses_per_step": n_acc / n_steps, "released_ids_per_step": n_rel / n_steps,
             "ms_per_step": ms / n_steps, "accesses_per_s": n_acc / (ms * 1e-3),
+            "step_kernels_us_per_step": {k: 1e3 * v / n_steps for k, v in prof.items()},
+            "step_kernels_note": "CUDA-event time of arc_step_resume's own kernels per step (a separate pass with arc_set_profiling); the rest of "
+                                 "ms_per_step is the release launch, the binding's torch work and the host's enqueue time",
             "includes": "binding work per step (chain-state gather, clone of block_id for the later release) and one release launch",
             "hit_rate_blocks": (st["hit_t1"] + st["hit_t2"]) / max(1, st["accesses"]),
             "cpu_oracle_accesses_per_s": n_acc / cpu_s, "parity_spot_check": same}

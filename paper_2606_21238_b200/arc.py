@@ -123,11 +123,22 @@ class _DevView:
         self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr or 0, False), "version": 3, "strides": None}
 
 
+_views = {}     # (device pointer, typestr) -> the longest view made of it so far
+
+
 def _view(ptr, n, typestr, dtype):
+    """A tensor over n elements of library-owned device memory.  Wrapping a raw pointer costs tens of microseconds on the
+    host, and a handle hands out the same buffers step after step, so the wrapper is kept per pointer and sliced: the
+    view owns nothing, and only the n elements the library has just declared valid are ever reachable through it."""
     torch = _torch()
     if n == 0 or not ptr:
         return torch.zeros(0, dtype=dtype, device="cuda")
-    return torch.as_tensor(_DevView(ptr, n, typestr), device="cuda")
+    v = _views.get((ptr, typestr))
+    if v is None or v.numel() < n:
+        if len(_views) >= 512:
+            _views.clear()
+        v = _views[(ptr, typestr)] = torch.as_tensor(_DevView(ptr, n, typestr), device="cuda")
+    return v if v.numel() == n else v[:n]
 
 
 def _offsets(offsets) -> np.ndarray:
