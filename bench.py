@@ -580,6 +580,8 @@ def serving_loop_leg(torch, A, info, steps, stream, seed, n_steps=240, new_per_s
         n_dec = new_per_step * min(i, decode_steps)
         # admission (the scheduler's job): holds outstanding + this step's blocks <= c; the longest prompts are cut until it fits
         budget = info.capacity_blocks - sum(held) - n_dec
+        if budget < 0:
+            raise SystemExit(f"serving_loop_leg: {new_per_step} prompts x {decode_steps} decode steps hold more than c = {info.capacity_blocks} blocks")
         while sum(len(p) for p in new) // 16 > budget:
             k = max(range(len(new)), key=lambda j: len(new[j]))
             new[k] = new[k][:len(new[k]) // 32 * 16]
