@@ -62,6 +62,7 @@ def parse_args():
     ap.add_argument("--no-extras", action="store_true", help="skip per_config / roofline / probe / cpu legs (for ncu captures)")
     ap.add_argument("--only-k1", action="store_true", help="run only the K1 bulk roofline leg (for ncu captures of the hashing kernel)")
     ap.add_argument("--only-k2", action="store_true", help="run only the K2 probe leg (for ncu captures of the probe kernel)")
+    ap.add_argument("--only-zipf", action="store_true", help="run only the batch-size-1 windowed-Zipf leg (for ncu captures of the one-launch kernel)")
     ap.add_argument("--print-source-hash", action="store_true", help="print the hash of the kernel sources (profiles/r02_ncu_evidence.json)")
     return ap.parse_args()
 
@@ -715,6 +716,9 @@ def run_ours(args):
         return
     if args.only_k2:
         print(json.dumps(k2_probe_bench(torch, A, stream, args.seed, peak)))
+        return
+    if args.only_zipf:
+        print(json.dumps(windowed_zipf_leg(torch, A, stream, args.seed)))
         return
     W_, K = args.warmup, args.steps
     D = dist if world > 1 else None
